@@ -1,0 +1,260 @@
+"""ctypes wrapper of the CPU oracle (oracle/pf_oracle.cpp).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this module.  It never imports the CUDA
+package and the CUDA package never imports it.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "pf_oracle.cpp")
+_LIB = os.path.join(_HERE, "libpf_oracle.so")
+_lib = None
+
+c_dp = ctypes.POINTER(ctypes.c_double)
+c_ip = ctypes.POINTER(ctypes.c_int)
+c_u8p = ctypes.POINTER(ctypes.c_uint8)
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle: g++ -O2 -ffp-contract=off (every operation rounded as written)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", _SRC, "-o", _LIB]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+        _lib.pfo_kappa.restype = ctypes.c_double
+        _lib.pfo_kT_over_e_volt.restype = ctypes.c_double
+        _lib.pfo_molar_to_per_A3.restype = ctypes.c_double
+        _lib.pfo_dot.restype = ctypes.c_double
+    return _lib
+
+
+def _d(a):
+    return None if a is None else a.ctypes.data_as(c_dp)
+
+
+def _i(a):
+    return None if a is None else a.ctypes.data_as(c_ip)
+
+
+def _u8(a):
+    return None if a is None else a.ctypes.data_as(c_u8p)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _bc(bc_type, bc_value):
+    return np.ascontiguousarray(bc_type, dtype=np.int32), np.ascontiguousarray(bc_value, dtype=np.float64)
+
+
+def kappa() -> float:
+    return lib().pfo_kappa()
+
+
+def kT_over_e_volt() -> float:
+    return lib().pfo_kT_over_e_volt()
+
+
+def molar_to_per_A3() -> float:
+    return lib().pfo_molar_to_per_A3()
+
+
+def dot(a, b) -> float:
+    a = _f64(a)
+    b = _f64(b)
+    return lib().pfo_dot(ctypes.c_int64(a.size), _d(a), _d(b))
+
+
+def assemble_poisson(nx, ny, nz, h, bc_type, bc_value, eps, sigma=None) -> np.ndarray:
+    """Rows of -div(eps grad u) + sigma u in the paper's A0..A6 format; returns (7, N)."""
+    n = nx * ny * nz
+    t, v = _bc(bc_type, bc_value)
+    eps = _f64(eps)
+    sigma = None if sigma is None else _f64(sigma)
+    A = np.empty((7, n), dtype=np.float64)
+    lib().pfo_assemble_poisson(nx, ny, nz, ctypes.c_double(h), _i(t), _d(v), _d(eps), _d(sigma), _d(A))
+    return A
+
+
+def solvent_mask(eps) -> np.ndarray:
+    eps = _f64(eps)
+    m = np.empty(eps.size, dtype=np.uint8)
+    lib().pfo_solvent_mask(ctypes.c_int64(eps.size), _d(eps), _u8(m))
+    return m
+
+
+def assemble_pf1(nx, ny, nz, h, bc_type, bc_value, eps, solvent, lc) -> np.ndarray:
+    n = nx * ny * nz
+    t, v = _bc(bc_type, bc_value)
+    eps = _f64(eps)
+    solvent = np.ascontiguousarray(solvent, dtype=np.uint8)
+    A = np.empty((7, n), dtype=np.float64)
+    lib().pfo_assemble_pf1(nx, ny, nz, ctypes.c_double(h), _i(t), _d(v), _d(eps), _u8(solvent),
+                           ctypes.c_double(lc), _d(A))
+    return A
+
+
+def dia_spmv(nx, ny, nz, A, x) -> np.ndarray:
+    A = _f64(A)
+    x = _f64(x)
+    y = np.empty(nx * ny * nz, dtype=np.float64)
+    lib().pfo_dia_spmv(nx, ny, nz, _d(A), _d(x), _d(y))
+    return y
+
+
+def set_dirichlet(nx, ny, nz, bc_type, bc_value, x) -> np.ndarray:
+    t, v = _bc(bc_type, bc_value)
+    x = _f64(x).copy()
+    lib().pfo_set_dirichlet(nx, ny, nz, _i(t), _d(v), _d(x))
+    return x
+
+
+def deposit_charges(nx, ny, nz, h, charges) -> np.ndarray:
+    ch = _f64(charges).reshape(-1, 4)
+    b = np.zeros(nx * ny * nz, dtype=np.float64)
+    lib().pfo_deposit_charges(nx, ny, nz, ctypes.c_double(h), _d(ch), int(ch.shape[0]), _d(b))
+    return b
+
+
+def bicgstab(nx, ny, nz, A, b, x0=None, tol=1e-10, maxit=10000, precond=True, history=False):
+    """Table 3 (+Jacobi).  Returns dict(x, status, iters, relres, true_relres[, hist])."""
+    A = _f64(A)
+    b = _f64(b)
+    n = nx * ny * nz
+    x = np.zeros(n) if x0 is None else _f64(x0).copy()
+    it = ctypes.c_int(0)
+    rr = ctypes.c_double(0)
+    tr = ctypes.c_double(0)
+    hist = np.full(maxit + 1, np.nan) if history else None
+    st = lib().pfo_bicgstab(nx, ny, nz, _d(A), _d(b), _d(x), ctypes.c_double(tol), int(maxit),
+                            int(bool(precond)), ctypes.byref(it), ctypes.byref(rr), ctypes.byref(tr), _d(hist))
+    out = dict(x=x, status=st, iters=it.value, relres=rr.value, true_relres=tr.value)
+    if history:
+        out["hist"] = hist[: it.value + 1]
+    return out
+
+
+def solve_linear(nx, ny, nz, h, bc_type, bc_value, eps, rhs, x0=None, sigma=None, tol=1e-10,
+                 maxit=10000, precond=True, history=False):
+    """What pf_solve_linear computes: the grid's Poisson operator, Dirichlet data forced."""
+    n = nx * ny * nz
+    t, v = _bc(bc_type, bc_value)
+    eps = _f64(eps)
+    rhs = _f64(rhs)
+    sigma = None if sigma is None else _f64(sigma)
+    x = np.zeros(n) if x0 is None else _f64(x0).copy()
+    it = ctypes.c_int(0)
+    rr = ctypes.c_double(0)
+    tr = ctypes.c_double(0)
+    hist = np.full(maxit + 1, np.nan) if history else None
+    st = lib().pfo_solve_linear(nx, ny, nz, ctypes.c_double(h), _i(t), _d(v), _d(eps), _d(sigma), _d(rhs),
+                                _d(x), ctypes.c_double(tol), int(maxit), int(bool(precond)),
+                                ctypes.byref(it), ctypes.byref(rr), ctypes.byref(tr), _d(hist))
+    out = dict(x=x, status=st, iters=it.value, relres=rr.value, true_relres=tr.value)
+    if history:
+        out["hist"] = hist[: it.value + 1]
+    return out
+
+
+def fermi_pointwise(valence, bath_molar, radii, phi, solvent=None, water_molar=55.5):
+    """Eq (1) solved per node.  Returns dict(rho, sigma, S, conc[(K+1),N], gammaB, status)."""
+    valence = _f64(valence)
+    bath = _f64(bath_molar)
+    radii = _f64(radii)
+    K = valence.size
+    phi = _f64(phi).reshape(-1)
+    n = phi.size
+    solvent = np.ones(n, dtype=np.uint8) if solvent is None else np.ascontiguousarray(solvent, dtype=np.uint8)
+    rho = np.empty(n)
+    sigma = np.empty(n)
+    S = np.empty(n)
+    conc = np.empty((K + 1, n))
+    gB = ctypes.c_double(0)
+    st = lib().pfo_fermi_pointwise(int(K), _d(valence), _d(bath), _d(radii), ctypes.c_double(water_molar),
+                                   ctypes.c_int64(n), _d(phi), _u8(solvent), _d(rho), _d(sigma), _d(S),
+                                   _d(conc), ctypes.byref(gB))
+    return dict(rho=rho, sigma=sigma, S=S, conc=conc, gammaB=gB.value, status=st)
+
+
+def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar, radii, l_c, tol,
+             omega_pf=0.3, lin_tol=1e-10, lin_maxit=10000, max_outer=200, water_molar=55.5):
+    """The outer loop of Table 2 / Table 4 (R5)."""
+    n = nx * ny * nz
+    t, v = _bc(bc_type, bc_value)
+    eps = _f64(eps)
+    ch = _f64(charges).reshape(-1, 4)
+    valence = _f64(valence)
+    bath = _f64(bath_molar)
+    radii = _f64(radii)
+    K = valence.size
+    phi = np.zeros(n)
+    psi = np.zeros(n)
+    conc = np.zeros((K + 1, n))
+    steric = np.zeros(n)
+    outer = ctypes.c_int(0)
+    lin = ctypes.c_int(0)
+    cap = 2 * max_outer + 1
+    lhist = np.zeros(cap, dtype=np.int32)
+    ihist = np.zeros(max_outer, dtype=np.float64)
+    st = lib().pfo_solve_pf(nx, ny, nz, ctypes.c_double(h), _i(t), _d(v), _d(eps), _d(ch), int(ch.shape[0]),
+                            int(K), _d(valence), _d(bath), _d(radii), ctypes.c_double(water_molar),
+                            ctypes.c_double(l_c), ctypes.c_double(tol), ctypes.c_double(omega_pf),
+                            ctypes.c_double(lin_tol), int(lin_maxit), int(max_outer),
+                            _d(phi), _d(psi), _d(conc), _d(steric), ctypes.byref(outer), ctypes.byref(lin),
+                            _i(lhist), int(cap), _d(ihist))
+    return dict(phi=phi, psi=psi, conc=conc, steric=steric, status=st, outer_iters=outer.value,
+                linear_iters=lin.value, lin_iters_hist=lhist[: 2 * outer.value + 1].copy(),
+                incr_hist=ihist[: outer.value].copy())
+
+
+def pf_residuals(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar, radii, l_c,
+                 phi, psi, water_molar=55.5):
+    t, v = _bc(bc_type, bc_value)
+    eps = _f64(eps)
+    ch = _f64(charges).reshape(-1, 4)
+    valence = _f64(valence)
+    bath = _f64(bath_molar)
+    radii = _f64(radii)
+    phi = _f64(phi)
+    psi = _f64(psi)
+    r1 = ctypes.c_double(0)
+    r2 = ctypes.c_double(0)
+    st = lib().pfo_pf_residuals(nx, ny, nz, ctypes.c_double(h), _i(t), _d(v), _d(eps), _d(ch), int(ch.shape[0]),
+                                int(valence.size), _d(valence), _d(bath), _d(radii), ctypes.c_double(water_molar),
+                                ctypes.c_double(l_c), _d(phi), _d(psi), ctypes.byref(r1), ctypes.byref(r2))
+    return dict(status=st, res_pf1=r1.value, res_pf2=r2.value)
+
+
+def dia_to_dense(nx, ny, nz, A) -> np.ndarray:
+    A = _f64(A)
+    n = nx * ny * nz
+    D = np.empty((n, n))
+    lib().pfo_dia_to_dense(nx, ny, nz, _d(A), _d(D))
+    return D
+
+
+def dense_lu_solve(dense, b) -> np.ndarray:
+    a = _f64(dense).copy()
+    b = _f64(b)
+    n = b.size
+    x = np.empty(n)
+    rc = lib().pfo_dense_lu_solve(ctypes.c_int64(n), _d(a), _d(b), _d(x))
+    if rc:
+        raise RuntimeError("singular matrix in oracle dense LU")
+    return x

@@ -1,0 +1,233 @@
+"""Pins for the oracle's linear solver (rows L3-L8 of 8(a)).
+
+Closed forms, a dense LU, a library sparse LU, an independent numpy transcription of the
+paper's Table 3, and exact rational arithmetic for the inner product.
+"""
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from paper_1711_04060_b200 import workloads as W
+
+D, NEU = 0, 1
+ALL_D = ([D] * 6, [0.0] * 6)
+
+
+def test_dot_is_correctly_rounded(oracle):
+    """Dot2 equals the exactly computed, once-rounded inner product (rational arithmetic)."""
+    rng = np.random.default_rng(0)
+    for trial in range(20):
+        n = 200
+        a = rng.standard_normal(n) * 10.0 ** rng.integers(-8, 8, n)
+        b = rng.standard_normal(n) * 10.0 ** rng.integers(-8, 8, n)
+        if trial % 2:                      # heavy cancellation: append the negated terms, jittered
+            a = np.concatenate([a, -a * (1 + 1e-9)])
+            b = np.concatenate([b, b])
+        exact = sum(Fraction(float(x)) * Fraction(float(y)) for x, y in zip(a, b))
+        assert oracle.dot(a, b) == float(exact)
+    # order independence on a long vector
+    a = rng.standard_normal(100000)
+    b = rng.standard_normal(100000)
+    p = rng.permutation(100000)
+    assert oracle.dot(a, b) == oracle.dot(a[p], b[p])
+
+
+def test_discrete_sine_mode_closed_form(oracle):
+    """eps constant: sin*sin*sin is an eigenvector, lambda_h = (12 eps/h^2) sin^2(pi h / 2L)."""
+    n, h, e = 17, 0.5, 3.0
+    L = (n - 1) * h
+    s = np.sin(np.pi * np.arange(n) * h / L)
+    f = (s[:, None, None] * s[None, :, None] * s[None, None, :]).ravel()
+    lam = 12 * e / h ** 2 * np.sin(np.pi * h / (2 * L)) ** 2
+    A = oracle.assemble_poisson(n, n, n, h, *ALL_D, np.full(n ** 3, e))
+    Af = oracle.dia_spmv(n, n, n, A, f)
+    interior = np.zeros((n, n, n), bool)
+    interior[1:-1, 1:-1, 1:-1] = True
+    assert np.abs(Af - lam * f)[interior.ravel()].max() < 1e-12 * lam
+    r = oracle.solve_linear(n, n, n, h, *ALL_D, np.full(n ** 3, e), f, tol=1e-13)
+    assert r["status"] == 0
+    assert np.abs(r["x"] - f / lam).max() < 1e-11 * (1 / lam)
+
+
+def test_second_order_convergence_smooth_variable_eps(oracle):
+    """Manufactured solution with smooth eps(x,y,z): error ratio -> 4 under h -> h/2."""
+    L = 8.0
+    errs = []
+    for n in (9, 17, 33):
+        h = L / (n - 1)
+        c = np.arange(n) * h
+        z, y, x = np.meshgrid(c, c, c, indexing="ij")
+        k = np.pi / L
+        u = np.sin(k * x) * np.sin(2 * k * y) * np.sin(k * z)
+        eps = 2.0 + np.sin(k * x) * np.cos(k * y)
+        # f = -div(eps grad u), analytic
+        ux = k * np.cos(k * x) * np.sin(2 * k * y) * np.sin(k * z)
+        uy = 2 * k * np.sin(k * x) * np.cos(2 * k * y) * np.sin(k * z)
+        lap = -(k * k + 4 * k * k + k * k) * u
+        ex = k * np.cos(k * x) * np.cos(k * y)
+        ey = -k * np.sin(k * x) * np.sin(k * y)
+        f = -(eps * lap + ex * ux + ey * uy)
+        r = oracle.solve_linear(n, n, n, h, *ALL_D, eps.ravel(), f.ravel(), tol=1e-12)
+        assert r["status"] == 0
+        errs.append(np.abs(r["x"] - u.ravel()).max())
+    assert 3.5 < errs[0] / errs[1] < 4.6
+    assert 3.7 < errs[1] / errs[2] < 4.3
+
+
+def _random_problem(n, seed, bt, bv):
+    rng = np.random.default_rng(seed)
+    N = n ** 3
+    eps = rng.choice([2.0, 80.0], size=N)
+    sigma = rng.uniform(0.0, 5.0, size=N)
+    rhs = rng.standard_normal(N)
+    return eps, sigma, rhs
+
+
+@pytest.mark.parametrize("bt,bv", [([D] * 6, [0.3, -0.2, 0.0, 1.0, 0.5, -1.0]),
+                                   ([NEU, NEU, NEU, NEU, D, D], [0, 0, 0, 0, 0.0, 2.0])])
+def test_dense_lu_8cubed(oracle, bt, bv):
+    """BiCGSTAB solution equals dense LU with partial pivoting on a random two-region 8^3 problem."""
+    n, h = 8, 0.5
+    eps, sigma, rhs = _random_problem(n, 11, bt, bv)
+    A = oracle.assemble_poisson(n, n, n, h, bt, bv, eps, sigma)
+    b = oracle.set_dirichlet(n, n, n, bt, bv, rhs)
+    dense = oracle.dia_to_dense(n, n, n, A)
+    x_lu = oracle.dense_lu_solve(dense, b)
+    # the oracle's LU itself against numpy's LAPACK
+    x_np = np.linalg.solve(dense, b)
+    assert np.linalg.norm(x_lu - x_np) <= 1e-11 * np.linalg.norm(x_np)
+    r = oracle.solve_linear(n, n, n, h, bt, bv, eps, rhs, sigma=sigma, tol=1e-13)
+    assert r["status"] == 0
+    assert np.linalg.norm(r["x"] - x_lu) <= 1e-10 * np.linalg.norm(x_lu)
+    # recurrence residual and true residual agree while well above the rounding floor
+    r9 = oracle.solve_linear(n, n, n, h, bt, bv, eps, rhs, sigma=sigma, tol=1e-9)
+    assert r9["status"] == 0 and r9["relres"] <= 1e-9
+    assert abs(r9["relres"] - r9["true_relres"]) <= 1e-3 * r9["relres"]
+
+
+def test_sparse_lu_config1_small(oracle):
+    """Library pin: scipy's sparse LU on the matrix read out of A0..A6 (config-1 generator, 20^3)."""
+    import scipy.sparse as sp
+    import scipy.sparse.linalg as spla
+    w = W.config1(20, ncharges=30)
+    n = w.nx
+    N = w.n
+    A = oracle.assemble_poisson(n, n, n, w.h, w.bc_type, w.bc_value, w.eps)
+    offs = [0, 1, -1, -n, n, -n * n, n * n]
+    rows, cols, vals = [], [], []
+    idx = np.arange(N)
+    for d, o in enumerate(offs):
+        j = idx + o
+        ok = (j >= 0) & (j < N) & (A[d] != 0)
+        rows.append(idx[ok]); cols.append(j[ok]); vals.append(A[d][ok])
+    M = sp.csc_matrix((np.concatenate(vals), (np.concatenate(rows), np.concatenate(cols))), shape=(N, N))
+    b = oracle.set_dirichlet(n, n, n, w.bc_type, w.bc_value, w.rhs)
+    x_ref = spla.splu(M).solve(b)
+    r = oracle.solve_linear(n, n, n, w.h, w.bc_type, w.bc_value, w.eps, w.rhs, tol=1e-13)
+    assert r["status"] == 0 and r["true_relres"] < 2e-13
+    assert np.linalg.norm(r["x"] - x_ref) <= 1e-10 * np.linalg.norm(x_ref)
+
+
+def _table3_numpy(matvec, b, x0, tol, maxit):
+    """Independent transcription of Table 3, no preconditioner, in numpy."""
+    x = x0.copy()
+    r = b - matvec(x)                                     # step 2
+    rt = r.copy()
+    bn = np.linalg.norm(b)
+    hist = [np.linalg.norm(r) / bn]
+    p = v = None
+    rho_old = alpha = omega = 1.0
+    for i in range(1, maxit + 1):                          # step 3
+        rho = rt @ r                                       # step 4
+        if i == 1:
+            p = r.copy()                                   # step 6
+        else:
+            beta = (rho * alpha) / (rho_old * omega)       # step 8
+            p = r + beta * (p - omega * v)                 # step 9
+        v = matvec(p)                                      # step 11
+        alpha = rho / (rt @ v)                             # step 12
+        s = r - alpha * v                                  # step 13
+        t = matvec(s)                                      # step 14
+        omega = (t @ s) / (t @ t)                          # step 15
+        x = x + alpha * p + omega * s                      # step 16
+        r = s - omega * t                                  # step 17
+        hist.append(np.linalg.norm(r) / bn)                # step 18
+        rho_old = rho
+        if hist[-1] <= tol:                                # step 19
+            break
+    return x, np.array(hist)
+
+
+def test_identity_preconditioner_reproduces_table3(oracle):
+    n, h = 10, 0.5
+    bt, bv = [D] * 6, [0.0] * 6
+    eps, sigma, rhs = _random_problem(n, 3, bt, bv)
+    A = oracle.assemble_poisson(n, n, n, h, bt, bv, eps, sigma)
+    b = oracle.set_dirichlet(n, n, n, bt, bv, rhs)
+    mv = lambda u: oracle.dia_spmv(n, n, n, A, u)
+    x_np, hist_np = _table3_numpy(mv, b, np.zeros(n ** 3), 1e-10, 500)
+    r = oracle.bicgstab(n, n, n, A, b, tol=1e-10, maxit=500, precond=False, history=True)
+    assert r["status"] == 0
+    m = min(25, len(hist_np), len(r["hist"]))
+    # early history agrees to rounding (later iterations drift: BiCGSTAB amplifies last-bit noise)
+    assert np.allclose(r["hist"][:m], hist_np[:m], rtol=1e-6)
+    assert abs(r["iters"] - (len(hist_np) - 1)) <= max(3, 0.1 * r["iters"])
+    assert np.linalg.norm(r["x"] - x_np) <= 1e-8 * np.linalg.norm(x_np)
+
+
+def test_jacobi_is_right_preconditioning(oracle):
+    """With M = diag(A): same solution, r stays the true residual, and (for this badly scaled
+    system) fewer iterations than M = I.  Also equals Table 3 applied to A D^-1 in y = D x."""
+    n, h = 10, 0.5
+    bt, bv = [D] * 6, [0.0] * 6
+    eps, sigma, rhs = _random_problem(n, 4, bt, bv)
+    sigma = sigma * 200
+    A = oracle.assemble_poisson(n, n, n, h, bt, bv, eps, sigma)
+    b = oracle.set_dirichlet(n, n, n, bt, bv, rhs)
+    rj = oracle.bicgstab(n, n, n, A, b, tol=1e-11, precond=True, history=True)
+    ri = oracle.bicgstab(n, n, n, A, b, tol=1e-11, precond=False)
+    assert rj["status"] == 0 and ri["status"] == 0
+    assert rj["iters"] < ri["iters"]
+    assert np.linalg.norm(rj["x"] - ri["x"]) <= 1e-8 * np.linalg.norm(ri["x"])
+    assert abs(rj["relres"] - rj["true_relres"]) <= 1e-3 * rj["relres"]
+    mv = lambda y: oracle.dia_spmv(n, n, n, A, y / A[0])
+    y_np, hist_np = _table3_numpy(mv, b, np.zeros(n ** 3), 1e-11, 500)
+    m = min(20, len(hist_np), len(rj["hist"]))
+    assert np.allclose(rj["hist"][:m], hist_np[:m], rtol=1e-6)
+    assert np.linalg.norm(y_np / A[0] - rj["x"]) <= 1e-8 * np.linalg.norm(rj["x"])
+
+
+def test_debye_hueckel_sinh_profile(oracle):
+    """Constant sigma in 1-D: phi_j = V sinh(mu j)/sinh(mu (n-1)), cosh mu = 1 + sigma h^2/(2 eps).
+    Pins the diagonal addend."""
+    nx = ny = 3
+    nz, h, V, e, sg = 41, 0.5, 1.0, 78.5, 0.9
+    bt, bv = [NEU, NEU, NEU, NEU, D, D], [0, 0, 0, 0, 0.0, V]
+    N = nx * ny * nz
+    r = oracle.solve_linear(nx, ny, nz, h, bt, bv, np.full(N, e), np.zeros(N), sigma=np.full(N, sg), tol=1e-14)
+    mu = np.arccosh(1 + sg * h * h / (2 * e))
+    exact = V * np.sinh(mu * np.arange(nz)) / np.sinh(mu * (nz - 1))
+    phi = r["x"].reshape(nz, ny, nx)
+    assert np.abs(phi - exact[:, None, None]).max() < 1e-11
+
+
+def test_degenerate_cases(oracle):
+    n, h = 6, 0.5
+    N = n ** 3
+    eps = np.full(N, 2.0)
+    # b = 0 => x = 0 in zero iterations (Q3)
+    r = oracle.solve_linear(n, n, n, h, *ALL_D, eps, np.zeros(N), x0=np.ones(N))
+    assert r["status"] == 0 and r["iters"] == 0 and np.all(r["x"] == 0)
+    # warm start at the solution => zero iterations
+    rhs = np.random.default_rng(1).standard_normal(N)
+    r1 = oracle.solve_linear(n, n, n, h, *ALL_D, eps, rhs, tol=1e-13)
+    r2 = oracle.solve_linear(n, n, n, h, *ALL_D, eps, rhs, x0=r1["x"], tol=1e-10)
+    assert r2["iters"] == 0 and r2["status"] == 0
+    # maxit reached => status 1, x holds the last iterate
+    r3 = oracle.solve_linear(n, n, n, h, *ALL_D, eps, rhs, tol=0.0, maxit=5)
+    assert r3["status"] == 1 and r3["iters"] == 5
+    # Dirichlet values are forced into x0 and kept
+    bv = [0.5, 0.5, 0.5, 0.5, 0.5, 0.5]
+    r4 = oracle.solve_linear(n, n, n, h, [D] * 6, bv, eps, np.zeros(N), tol=1e-13)
+    assert np.allclose(r4["x"], 0.5, atol=1e-12)      # harmonic, constant data => constant

@@ -1,0 +1,147 @@
+"""Pins for the oracle's nonlinear outer loop (rows N2-N5 of 8(a)).
+
+Table 2 steps 2-5 / Table 4 steps 4-7.  Pins: the PF -> PB reduction
+ against the Gouy-Chapman closed form with O(h^2) convergence, Psi = Laplacian(phi)
+ evaluated with numpy, independence of the converged field from omega_PF, the
+discrete PF1/PF2 equations re-evaluated in numpy at the fixed point, and the relaxation formula.
+Full 3-D PF with l_c > 0 and unequal radii has no closed form: PARITY UNPINNED beyond these.
+"""
+import numpy as np
+import pytest
+
+from paper_1711_04060_b200 import workloads as W
+
+D, NEU = 0, 1
+MOLAR = 6.02214076e-4
+
+
+def _gouy_chapman_error(oracle, nz, h, phi_w):
+    """1-D electrolyte column: a 3x3 solvent core inside a ring of (almost) non-polarisable wall
+    nodes (eps = 1e-6), so that the lateral box-boundary nodes are NOT solvent.  Needed because the
+    reading Q15 puts Psi = 0 on every box-boundary node, which would otherwise strip the ionic
+    charge from lateral solvent nodes; the wall couples to the core only at relative order 1e-8."""
+    nx = ny = 5
+    eps3 = np.full((nz, ny, nx), 1e-6)
+    eps3[:, 1:-1, 1:-1] = 78.5
+    bt, bv = [NEU, NEU, NEU, NEU, D, D], [0, 0, 0, 0, phi_w, 0.0]
+    r = oracle.solve_pf(nx, ny, nz, h, bt, bv, eps3.ravel(), np.zeros((0, 4)), [1.0, -1.0], [0.1, 0.1],
+                        [0.0, 0.0, 0.0], 0.0, 1e-10, lin_tol=1e-12, max_outer=400)
+    assert r["status"] == 0
+    kap = oracle.kappa()
+    lam_d = np.sqrt(78.5 / (2 * kap * 0.1 * MOLAR))
+    assert abs(lam_d - 9.62) < 0.01                                   # survey: 9.62 A at 100 mM
+    z = np.arange(nz) * h
+    exact = 4 * np.arctanh(np.tanh(phi_w / 4) * np.exp(-z / lam_d))
+    core = r["phi"].reshape(nz, ny, nx)[:, 1:-1, 1:-1]
+    assert np.abs(core - core[:, :1, :1]).max() < 1e-6               # 1-D: no lateral variation
+    return np.abs(core[:, 1, 1] - exact).max(), r
+
+
+def test_pb_reduction_gouy_chapman(oracle):
+    """l_c = 0 and steric off => nonlinear PB; 1:1 electrolyte at a wall of potential phi_w:
+    phi(z) = 4 atanh(tanh(phi_w/4) e^{-z/lambda_D}), second-order in h."""
+    phi_w = 2.0
+    e1, _ = _gouy_chapman_error(oracle, 257, 0.5, phi_w)       # L = 128 A = 13.3 lambda_D
+    e2, r = _gouy_chapman_error(oracle, 513, 0.25, phi_w)
+    assert e2 < 2e-4 * phi_w
+    assert 3.5 < e1 / e2 < 4.5
+    # with l_c = 0 PF1 is algebraic: Psi = -kappa rho / eps on interior solvent nodes
+    phi = r["phi"]
+    rho = -2 * 0.1 * MOLAR * np.sinh(phi)
+    psi = r["psi"].reshape(513, 5, 5)[1:-1, 1:-1, 1:-1]
+    expect = (-oracle.kappa() * rho / 78.5).reshape(513, 5, 5)[1:-1, 1:-1, 1:-1]
+    assert np.allclose(psi, expect, rtol=1e-6, atol=1e-9)
+
+
+def _small_channel(n=16):
+    h = 0.5
+    eps = W.channel_eps(n, n, n, h, slab_thick=3.0, pore_radius=1.6)
+    ch = np.array([[2.7, 4.9, 3.6, 0.5], [5.2, 2.3, 3.9, -0.5], [4.9, 5.6, 3.4, 0.5]])
+    bt, bv = [NEU, NEU, NEU, NEU, D, D], [0, 0, 0, 0, 0.0, 1.0]
+    return n, h, eps, ch, bt, bv
+
+
+def _lap7(u3, h):
+    return (u3[2:, 1:-1, 1:-1] + u3[:-2, 1:-1, 1:-1] + u3[1:-1, 2:, 1:-1] + u3[1:-1, :-2, 1:-1]
+            + u3[1:-1, 1:-1, 2:] + u3[1:-1, 1:-1, :-2] - 6 * u3[1:-1, 1:-1, 1:-1]) / h ** 2
+
+
+def test_fixed_point_equations_in_numpy(oracle):
+    """At convergence the discrete split system holds, re-evaluated here with numpy stencils:
+    PF1  eps (l_c^2 Lap - 1) Psi = kappa rho(phi)                    (Eq 12)
+    PF2  -div(eps grad phi) = -eps Psi + fixed, i.e. Psi = Lap phi where eps is locally uniform (Eq 13)
+    """
+    n, h, eps, ch, bt, bv = _small_channel()
+    sp = W.NACACL
+    lc = 1.2
+    r = oracle.solve_pf(n, n, n, h, bt, bv, eps, ch, sp.valence, sp.bath_molar, sp.radii, lc, 1e-10,
+                        lin_tol=1e-12, max_outer=600)
+    assert r["status"] == 0
+    res = oracle.pf_residuals(n, n, n, h, bt, bv, eps, ch, sp.valence, sp.bath_molar, sp.radii, lc, r["phi"], r["psi"])
+    assert res["res_pf1"] < 1e-8 and res["res_pf2"] < 1e-8
+    phi3, psi3, eps3 = (a.reshape(n, n, n) for a in (r["phi"], r["psi"], eps))
+    solv = eps3 > 40
+    # nodes whose whole stencil is solvent and that carry no fixed charge
+    core = solv[1:-1, 1:-1, 1:-1].copy()
+    for sl in ((slice(2, None), slice(1, -1), slice(1, -1)), (slice(None, -2), slice(1, -1), slice(1, -1)),
+               (slice(1, -1), slice(2, None), slice(1, -1)), (slice(1, -1), slice(None, -2), slice(1, -1)),
+               (slice(1, -1), slice(1, -1), slice(2, None)), (slice(1, -1), slice(1, -1), slice(None, -2))):
+        core &= solv[sl]
+    fixed = oracle.deposit_charges(n, n, n, h, ch).reshape(n, n, n)[1:-1, 1:-1, 1:-1]
+    core &= fixed == 0
+    assert core.sum() > 500
+    # the fixed point is reached only to ~tol/(1-contraction): compare at 1e-6 of the field scale
+    lap_phi = _lap7(phi3, h)
+    scale = np.abs(lap_phi[core]).max()
+    assert np.abs(psi3[1:-1, 1:-1, 1:-1] - lap_phi)[core].max() < 1e-6 * scale
+    # PF1 with rho from the returned concentrations (K = 3 ions)
+    rho = (sp.valence[:, None] * r["conc"][:3]).sum(0).reshape(n, n, n)[1:-1, 1:-1, 1:-1]
+    lhs = 78.5 * (lc ** 2 * _lap7(psi3, h) - psi3[1:-1, 1:-1, 1:-1])
+    rhs = oracle.kappa() * rho
+    # only where the PF1 stencil stays inside interior solvent nodes (Psi = 0 outside, Q15, is part of it anyway)
+    inner = solv[1:-1, 1:-1, 1:-1]
+    assert np.abs(lhs - rhs)[inner].max() < 1e-6 * np.abs(rhs[inner]).max()
+    # Psi = 0 on non-solvent nodes and on every box-boundary node (Eq 14, Q15)
+    assert np.all(psi3[~solv] == 0)
+    assert np.all(psi3[0] == 0) and np.all(psi3[-1] == 0) and np.all(psi3[:, 0] == 0) and np.all(psi3[:, :, -1] == 0)
+    # Dirichlet data kept, concentrations vanish outside the solvent
+    assert np.all(phi3[0] == 0.0) and np.all(phi3[-1] == 1.0)
+    assert np.all(r["conc"].reshape(4, n, n, n)[:, ~solv] == 0)
+
+
+def test_converged_field_independent_of_omega(oracle):
+    """Relaxation (Table 2 step 5) changes the path, not the fixed point; and the increment
+    history follows Phi := omega Phi0 + (1-omega) Phi (Q8): a smaller omega moves further per step."""
+    n, h, eps, ch, bt, bv = _small_channel(12)
+    ch = ch * np.array([0.7, 0.7, 0.7, 1.0])
+    sp = W.NACL
+    out = {}
+    for om in (0.3, 0.5):
+        out[om] = oracle.solve_pf(n, n, n, h, bt, bv, eps, ch, sp.valence, sp.bath_molar, sp.radii, 1.2, 1e-10,
+                                  omega_pf=om, lin_tol=1e-12, max_outer=800)
+        assert out[om]["status"] == 0
+    a, b = out[0.3], out[0.5]
+    assert np.abs(a["phi"] - b["phi"]).max() < 2e-8 * max(1.0, np.abs(a["phi"]).max())
+    assert np.linalg.norm(a["conc"] - b["conc"]) < 1e-7 * np.linalg.norm(a["conc"])
+    # first increments: both runs start from the same phi0 and see the same first Newton update U,
+    # so d1 = (1-omega) ||U - phi0||: ratio (1-0.3)/(1-0.5)
+    assert np.isclose(a["incr_hist"][0] / b["incr_hist"][0], 0.7 / 0.5, rtol=1e-6)
+    assert a["outer_iters"] < b["outer_iters"]
+    assert a["incr_hist"][-1] <= 1e-10 < a["incr_hist"][-2]
+    # bookkeeping: one initial solve + two per outer iteration
+    assert len(a["lin_iters_hist"]) == 2 * a["outer_iters"] + 1
+    assert a["lin_iters_hist"].sum() == a["linear_iters"]
+
+
+def test_initial_guess_is_linear_poisson(oracle):
+    """Table 2 step 2: phi0 solves PF2 with rho' = Psi = 0, i.e. the plain Poisson problem with the
+    deposited charges.  With max_outer = 0 the loop is skipped and solve_pf returns that phi0."""
+    n, h, eps, ch, bt, bv = _small_channel(12)
+    ch = ch * np.array([0.7, 0.7, 0.7, 1.0])
+    sp = W.NACL
+    r = oracle.solve_pf(n, n, n, h, bt, bv, eps, ch, sp.valence, sp.bath_molar, sp.radii, 1.2, 1e-8,
+                        lin_tol=1e-12, max_outer=0)
+    fixed = oracle.deposit_charges(n, n, n, h, ch)
+    lin = oracle.solve_linear(n, n, n, h, bt, bv, eps, fixed, tol=1e-12)
+    assert r["status"] == 1 and r["outer_iters"] == 0
+    assert np.array_equal(r["phi"], lin["x"])
