@@ -1,0 +1,155 @@
+/* pf.h -- C ABI of libpf_b200: the Poisson-Fermi hot path of arXiv 1711.04060 on one B200.
+ *
+ * Citations are PAPER.md:<line> (the paper's text) or a reading R0..R5 / Q1..Q29 of DESIGN.md.
+ *
+ * What the library computes
+ *   - operator assembly from a relative-permittivity map: the 7-point finite-difference rows of
+ *     -div(eps grad u) + sigma u with the simplified matched-interface rows of Eqs (15)-(18)
+ *     (they reduce to harmonic-mean face coefficients, reading R2), identity rows
+ *     on Dirichlet nodes, omitted outward flux on zero-Neumann faces (Eq (4));
+ *   - the Jacobi-preconditioned BiCGSTAB of Table 3 (reading R3);
+ *   - the inexact-Newton PF loop of Table 2 steps 2-5 / Table 4 steps 4-7 (PAPER.md:217-228,
+ *     281-291): pointwise Fermi-like distribution Eq (1), PF1/PF2 of Eqs (12)-(14)
+ *     (PAPER.md:122-133), relaxation and the test on the potential increment.
+ *
+ * Conventions
+ *   Grid nx*ny*nz nodes INCLUDING the boundary layer, linear index i = ix + nx*(iy + ny*iz)
+ *   (x fastest); node (ix,iy,iz) sits at (ix*h, iy*h, iz*h) Angstrom.
+ *   phi in k_B T/e, lengths in Angstrom, concentrations in 1/A^3, charges in e, all fp64.
+ *   "device" = pointer to CUDA device memory of the current device, "host" = ordinary host memory.
+ *   All device work is enqueued on the stream given to pf_grid_create; a call returns after the
+ *   stream work its out-parameters depend on has completed.
+ *   Ownership: the caller owns every array it passes.  eps_map and the workspace are BORROWED for
+ *   the lifetime of the grid.  The library itself allocates only small (KB-sized) device buffers.
+ *   Return value: 0 = PF_OK; < 0 = error (message via pf_last_error); > 0 = soft status.
+ *   No exceptions or aborts cross this boundary.  There is no CPU fallback: without a CUDA device
+ *   every compute call returns PF_ERR_CUDA.
+ */
+#ifndef PF_B200_H
+#define PF_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PF_OK                0
+#define PF_NOT_CONVERGED     1   /* maxit (or max outer iterations) reached; outputs hold the last iterate */
+#define PF_ERR_ARG          -1
+#define PF_ERR_CUDA         -2
+#define PF_ERR_BREAKDOWN    -3   /* rho = 0, r~.v = 0 or omega = 0 before convergence (reading Q5) */
+#define PF_ERR_NONPHYSICAL  -4   /* bath not neutral or Gamma^B <= 0 (reading Q26) */
+#define PF_ERR_WORKSPACE    -5   /* workspace missing or too small */
+
+/* Boundary faces in the order -x,+x,-y,+y,-z,+z (Eq (4)). */
+#define PF_BC_DIRICHLET 0        /* phi = value[face] (k_B T/e) */
+#define PF_BC_NEUMANN   1        /* zero normal derivative: outward face flux omitted (Q21) */
+
+typedef struct pf_grid pf_grid;                  /* opaque */
+typedef struct { int type[6]; double value[6]; } pf_bc;
+typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0 at the origin), charge in e */
+
+/* Option keys for pf_grid_set_option.  Values are doubles; integer options are rounded. */
+#define PF_OPT_STENCIL         1  /* 0 = auto, 1 = stored coefficients A1..A6 (the paper's diagonal
+                                     format), 2 = on-the-fly coefficients from a palette
+                                     of the eps map.  auto = on-the-fly when the map has <= 4 distinct
+                                     values, else stored.  Both give bit-identical results.  Must be
+                                     set before pf_grid_set_workspace. */
+#define PF_OPT_OMEGA_PF        2  /* relaxation parameter of Table 2 step 5; default 0.3 */
+#define PF_OPT_LINEAR_TOL      3  /* relative tolerance of the solves inside pf_solve_pf; default 1e-10 */
+#define PF_OPT_LINEAR_MAXIT    4  /* their iteration cap; default 10000 */
+#define PF_OPT_CHECK_INTERVAL  5  /* BiCGSTAB iterations enqueued between two host polls of the
+                                     device-side convergence flag; default 16; >= 1 */
+#define PF_OPT_WATER_MOLAR     6  /* bath concentration of water, mol/L; default 55.5 (Q12) */
+#define PF_OPT_MAX_OUTER       7  /* cap on outer (Newton) iterations; default 200 */
+#define PF_OPT_PRECOND         8  /* 1 = Jacobi M = diag(A) (default, reading Q2); 0 = M = I, Table 3 verbatim */
+#define PF_OPT_HISTORY         9  /* >0: keep the relative residual of every BiCGSTAB iteration of the
+                                     last linear solve (up to that many entries); see pf_grid_history */
+#define PF_OPT_KERNELS        10  /* 0 = auto, 1 = direct (one thread per node, neighbours through L1/L2),
+                                     2 = tiled (shared-memory planes, z-marched).  Same arithmetic. */
+
+/* Create a grid: store geometry and boundary conditions, scan eps_map for its palette of distinct
+ * values, keep a device copy of the charges.  Assembly itself runs in pf_grid_set_workspace.
+ *   eps_map : device, nx*ny*nz doubles, relative permittivity per node; borrowed.
+ *   charges : host, ncharges entries (may be NULL when ncharges = 0); copied.
+ *   bc      : host; copied.
+ *   cuda_stream : a cudaStream_t (NULL = the legacy default stream).
+ * Errors: PF_ERR_ARG (n < 3 in a direction, h <= 0, NULL pointers, bad bc type), PF_ERR_CUDA. */
+int pf_grid_create(pf_grid **out, int nx, int ny, int nz, double h,
+                   const double *eps_map, const pf_charge *charges, int ncharges,
+                   const pf_bc *bc, void *cuda_stream);
+
+/* Bytes of device scratch the grid needs with its current options (stencil variant). */
+size_t pf_grid_workspace_bytes(const pf_grid *g);
+
+/* Hand the grid its scratch (device, 256-byte aligned, >= pf_grid_workspace_bytes) and run the
+ * operator assembly (rows L1, L2 of DESIGN.md): node classes, diagonals, optionally the stored
+ * off-diagonals, the deposited fixed-charge right-hand side (reading R2). */
+int pf_grid_set_workspace(pf_grid *g, void *dev_ptr, size_t bytes);
+
+int pf_grid_set_option(pf_grid *g, int key, double value);
+
+/* Jacobi-BiCGSTAB solve of the grid's operator  -div(eps grad x) + sigma x = rhs  (Table 3).
+ *   rhs   : device N; entries at Dirichlet nodes are ignored (the boundary value is used, Q20).
+ *   x     : device N; in: initial guess (its Dirichlet nodes are overwritten, Q4), out: solution.
+ *   sigma : device N or NULL (zero); added to the diagonal (PF2's -rho' term, Eq (13)).
+ *   Stops when ||r||_2 <= tol*||rhs||_2 on the recurrence residual (Q3); tol = 0 runs exactly maxit
+ *   iterations and returns PF_NOT_CONVERGED (the fixed-iteration timing mode).
+ *   iters_out, relres_out (recurrence), true_relres_out (||b - A x||/||b||): host, may be NULL.
+ * Returns PF_OK, PF_NOT_CONVERGED, PF_ERR_BREAKDOWN, PF_ERR_WORKSPACE, PF_ERR_CUDA, PF_ERR_ARG. */
+int pf_solve_linear(pf_grid *g, const double *rhs, double *x, const double *sigma,
+                    double tol, int maxit,
+                    int *iters_out, double *relres_out, double *true_relres_out);
+
+/* The same solve with HOST buffers (pinned or pageable): rhs and x are copied to the device into
+ * grid scratch, solved, and x copied back, all on the grid's stream.  sigma stays a device pointer. */
+int pf_solve_linear_host(pf_grid *g, const double *rhs_host, double *x_host, const double *sigma,
+                         double tol, int maxit,
+                         int *iters_out, double *relres_out, double *true_relres_out);
+
+/* Nonlinear PF solve (Table 2 steps 2-5): initial guess from PF2 with rho' = Psi = 0, then
+ * { Fermi update at phi0 -> PF1 for Psi -> PF2 for phi -> relax -> test ||phi - phi0||_inf <= tol }.
+ *   nions K; valence, bath_conc (mol/L): host, K entries; radii: host, K+1 entries in Angstrom,
+ *   water last; all radii 0 switches the steric term off (Q25).  l_c in Angstrom.
+ *   phi    : device N, out.
+ *   conc   : device (K+1)*N or NULL, out: C_k at the final phi (species-major), 0 outside the solvent.
+ *   steric : device N or NULL, out: S^trc at the final phi.
+ *   outer_iters_out, linear_iters_out (sum over all linear solves): host, may be NULL.
+ * Returns PF_OK, PF_NOT_CONVERGED, or an error. */
+int pf_solve_pf(pf_grid *g, int nions, const double *valence, const double *bath_conc,
+                const double *radii, double l_c, double tol,
+                double *phi, double *conc, double *steric,
+                int *outer_iters_out, int *linear_iters_out);
+
+/* The pointwise part alone (row N1): Eq (1) solved per node (reading R4).
+ *   phi: device N, in.  rho, sigma, steric: device N or NULL, out.  conc: device (K+1)*N or NULL. */
+int pf_fermi_pointwise(pf_grid *g, int nions, const double *valence, const double *bath_conc,
+                       const double *radii, const double *phi,
+                       double *rho, double *sigma, double *steric, double *conc);
+
+/* Copy out up to cap entries of the residual history of the last linear solve (PF_OPT_HISTORY):
+ * hist[k] = ||r_k||/||b||, k = 0..iters.  Returns the number of entries written, < 0 on error. */
+int pf_grid_history(pf_grid *g, double *hist_host, int cap);
+
+/* Per-solve iteration counts of the last pf_solve_pf in call order (initial guess, PF1, PF2, ...). */
+int pf_grid_linear_iters(pf_grid *g, int *iters_host, int cap);
+
+/* Introspection used by the tests: 1 = stored, 2 = on-the-fly; number of palette entries. */
+int pf_grid_stencil(const pf_grid *g);
+int pf_grid_palette_size(const pf_grid *g);
+
+/* Copy an assembled array into caller memory (device), for the assembly parity tests (rows L1/L2):
+ * which = 0: Poisson diagonal A0 (N doubles); 1..6: stored off-diagonals A1..A6 (stored variant
+ * only); 7: deposited fixed-charge vector (N doubles); 8: node classes of the on-the-fly variant
+ * (N bytes); 9: PF1 diagonal (N doubles, after a pf_solve_pf).  Returns PF_ERR_ARG if unavailable. */
+int pf_grid_copy_array(pf_grid *g, int which, void *dst_device);
+
+void pf_grid_destroy(pf_grid *g);
+const char *pf_last_error(const pf_grid *g);   /* g may be NULL: last error of pf_grid_create */
+const char *pf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PF_B200_H */

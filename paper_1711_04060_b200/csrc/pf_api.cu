@@ -1,0 +1,584 @@
+// pf_api.cu -- the C ABI of include/pf.h and the host-side solver driver: launch sequencing of the
+// three-kernel BiCGSTAB iteration, device-resident scalars, pipelined polling of the device-side
+// convergence flag (row L8), and the PF outer loop (rows N1-N5).
+#include "../../include/pf.h"
+#include "pf_launch.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace pf;
+
+namespace {
+
+// Table 1, reading R0: kappa = e^2/(eps_0 k_B T) in Angstrom, phi in k_B T/e.
+const double K_BOLTZ = 1.38e-23;       // J/K
+const double T_KELVIN = 298.15;        // K
+const double E_CHARGE = 1.602e-19;     // C
+const double EPS0_F_PER_CM = 8.85e-14; // F/cm
+const double MOLAR_TO_PER_A3 = 6.02214076e-4;
+
+double kappa_angstrom() {
+    const double eps0_per_m = EPS0_F_PER_CM * 100.0;
+    return E_CHARGE * E_CHARGE / (eps0_per_m * K_BOLTZ * T_KELVIN) * 1e10;
+}
+
+thread_local std::string g_create_error;
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace
+
+struct pf_grid {
+    GridDims g;
+    double h;
+    BcDev bc;
+    cudaStream_t stream;
+    int sm_count;
+    const double* eps;
+    Palette pal;
+    double eps_min, eps_max, eps_mid;
+    bool uniform;
+    int ncharges;
+    double* charges_dev;     // small, owned
+    // options
+    int opt_stencil, opt_kernels, opt_check, opt_lin_maxit, opt_max_outer, opt_precond, opt_history;
+    double opt_omega_pf, opt_lin_tol, opt_water;
+    // small owned device buffers
+    Scalars* sc;
+    ReduceBuf rb;
+    double* lut_poisson;
+    double* lut_pf1;
+    unsigned long long* dmax_bits;
+    double* hist;
+    int hist_cap;
+    Scalars* sc_host[2];     // pinned
+    cudaEvent_t ev[2];
+    // workspace carve-up
+    void* ws;
+    size_t ws_bytes;
+    bool stored;
+    bool assembled;
+    double pf1_lc;           // l_c the PF1 operator was assembled for (NaN = none)
+    double *r, *rt, *p0, *p1, *v0, *v1, *t, *bw, *xw;
+    double *A0, *A0_pf1, *A0_s, *fixed, *psi, *phi0, *phiw, *sigma, *bpf;
+    uint8_t *cls, *cls_pf1;
+    double* offd[6];
+    double* offd_pf1[6];
+    std::vector<int> lin_iters;
+    int last_iters;
+    std::string err;
+};
+
+namespace {
+
+int fail(pf_grid* g, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof(buf), fmt, ap);
+    va_end(ap);
+    if (g) g->err = buf; else g_create_error = buf;
+    return code;
+}
+
+#define PF_CUDA(g, call)                                                                          \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess) return fail((g), PF_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+int n_vectors(bool stored) { return 18 + (stored ? 12 : 0); }
+
+bool want_stored(const pf_grid* g) {
+    if (g->opt_stencil == 1) return true;
+    if (g->opt_stencil == 2) return false;
+    return g->pal.count > PF_MAX_PALETTE;
+}
+
+bool use_tiled(const pf_grid* g) {
+    if (g->opt_kernels == 1) return false;
+    return tiled_supported(g->g);
+}
+
+Operator make_op(const pf_grid* g, int which /*0 poisson, 1 pf1, 2 poisson+sigma*/) {
+    Operator op;
+    std::memset(&op, 0, sizeof(op));
+    op.stored = g->stored ? 1 : 0;
+    op.ncls = PF_MAX_CLASSES;
+    if (which == 1) {
+        op.A0 = g->A0_pf1; op.cls = g->cls_pf1; op.lut = g->lut_pf1;
+        for (int d = 0; d < 6; ++d) op.offd[d] = g->offd_pf1[d];
+    } else {
+        op.A0 = which == 2 ? g->A0_s : g->A0; op.cls = g->cls; op.lut = g->lut_poisson;
+        for (int d = 0; d < 6; ++d) op.offd[d] = g->offd[d];
+    }
+    return op;
+}
+
+LaunchCtx make_ctx(const pf_grid* g) {
+    LaunchCtx c;
+    c.stream = g->stream; c.g = g->g; c.sc = g->sc; c.rb = g->rb; c.sm_count = g->sm_count;
+    return c;
+}
+
+// ---- Table 3 on the device ----------------------------------------------------------------
+// b: device N with Dirichlet values already forced; x: device N, in/out, Dirichlet values forced.
+int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, double tol, int maxit,
+                    int* iters_out, double* relres_out, double* true_relres_out) {
+    if (maxit < 0) return fail(g, PF_ERR_ARG, "maxit < 0");
+    if (!(tol >= 0.0)) return fail(g, PF_ERR_ARG, "tol must be >= 0");
+    const LaunchCtx c = make_ctx(g);
+    const bool tiled = use_tiled(g);
+    const bool precond = g->opt_precond != 0;
+    Scalars init;
+    std::memset(&init, 0, sizeof(init));
+    init.tol = tol; init.maxit = maxit; init.hist_cap = g->hist ? g->hist_cap : 0;
+    // pageable source: the runtime stages it before returning, so a stack object is safe
+    PF_CUDA(g, cudaMemcpyAsync(g->sc, &init, sizeof(init), cudaMemcpyHostToDevice, g->stream));
+    KrylovVecs kv;
+    kv.b = b; kv.x = x; kv.r = g->r; kv.rt = g->rt; kv.t = g->t; kv.hist = g->hist;
+    kv.p_in = g->p0; kv.p_out = g->p1; kv.v_in = g->v0; kv.v_out = g->v1;
+    if (tiled) launch_residual_tiled(c, op, kv, 0); else launch_residual_direct(c, op, kv, 0);
+
+    const int chunk = g->opt_check < 1 ? 1 : g->opt_check;
+    int launched = 0, slot = 0;
+    bool pending[2] = {false, false};
+    bool done = false;
+    Scalars fin;
+    std::memset(&fin, 0, sizeof(fin));
+    // Pipelined polling: enqueue chunk k+1 before waiting for the flag copy of chunk k, so the GPU
+    // never idles on the host; kernels launched after convergence return at once (sc->done).
+    while (!done) {
+        const int todo = std::min(chunk, maxit - launched);
+        for (int k = 0; k < todo; ++k) {
+            if (tiled) { launch_k1_tiled(c, op, kv, precond); launch_k2_tiled(c, op, kv, precond); }
+            else       { launch_k1_direct(c, op, kv, precond); launch_k2_direct(c, op, kv, precond); }
+            launch_k3(c, op, kv, precond);
+            std::swap(kv.p_in, kv.p_out);     // k1 read (p_in, v_in) and wrote (p_out, v_out)
+            std::swap(kv.v_in, kv.v_out);
+        }
+        launched += todo;
+        PF_CUDA(g, cudaMemcpyAsync(g->sc_host[slot], g->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
+        PF_CUDA(g, cudaEventRecord(g->ev[slot], g->stream));
+        pending[slot] = true;
+        const int other = slot ^ 1;
+        if (pending[other]) {
+            PF_CUDA(g, cudaEventSynchronize(g->ev[other]));
+            pending[other] = false;
+            if (g->sc_host[other]->done) { fin = *g->sc_host[other]; done = true; }
+        }
+        if (!done && (launched >= maxit || todo == 0)) {
+            PF_CUDA(g, cudaEventSynchronize(g->ev[slot]));
+            pending[slot] = false;
+            fin = *g->sc_host[slot];
+            done = true;
+        }
+        slot ^= 1;
+    }
+    PF_CUDA(g, cudaStreamSynchronize(g->stream));
+    if (!fin.done) { fin.status = PF_NOT_CONVERGED; }
+    if (fin.bb == 0.0) PF_CUDA(g, cudaMemsetAsync(x, 0, sizeof(double) * g->g.n, g->stream));   // Q3
+    double true_rel = 0.0;
+    if (true_relres_out && fin.bb != 0.0) {
+        if (tiled) launch_residual_tiled(c, op, kv, 1); else launch_residual_direct(c, op, kv, 1);
+        PF_CUDA(g, cudaMemcpyAsync(g->sc_host[0], g->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
+        PF_CUDA(g, cudaStreamSynchronize(g->stream));
+        true_rel = std::sqrt(g->sc_host[0]->true_rr) / fin.bnorm;
+    }
+    PF_CUDA(g, cudaGetLastError());
+    g->last_iters = fin.it;
+    if (iters_out) *iters_out = fin.it;
+    if (relres_out) *relres_out = fin.bb == 0.0 ? 0.0 : fin.rnorm / fin.bnorm;
+    if (true_relres_out) *true_relres_out = true_rel;
+    if (fin.status == PF_ERR_BREAKDOWN) return fail(g, PF_ERR_BREAKDOWN, "BiCGSTAB breakdown at iteration %d", fin.it);
+    return fin.status;
+}
+
+int check_ready(pf_grid* g) {
+    if (!g) return PF_ERR_ARG;
+    if (!g->ws || !g->assembled) return fail(g, PF_ERR_WORKSPACE, "workspace not set (pf_grid_set_workspace)");
+    return PF_OK;
+}
+
+// Species table of Eq (1): v_k = 4 pi a_k^3/3, v_0 = mean volume, lam_k = v_k/v_0,
+// Gamma^B = 1 - sum v_k C_k^B; Q25 (all radii 0 => steric off), Q26 (neutral bath).
+int make_species(pf_grid* g, int K, const double* valence, const double* bath, const double* radii, SpeciesDev* sp) {
+    if (K < 0 || K + 1 > PF_MAX_SPECIES) return fail(g, PF_ERR_ARG, "nions must be in 0..%d", PF_MAX_SPECIES - 1);
+    if ((K > 0 && (!valence || !bath)) || !radii) return fail(g, PF_ERR_ARG, "null species table");
+    std::memset(sp, 0, sizeof(*sp));
+    sp->K = K;
+    sp->kappa = kappa_angstrom();
+    double vsum = 0.0;
+    for (int k = 0; k <= K; ++k) {
+        sp->z[k] = k < K ? valence[k] : 0.0;
+        sp->cb[k] = (k < K ? bath[k] : g->opt_water) * MOLAR_TO_PER_A3;
+        sp->vol[k] = 4.0 * M_PI * radii[k] * radii[k] * radii[k] / 3.0;
+        vsum += sp->vol[k];
+    }
+    const double v0 = vsum / (K + 1);
+    sp->steric = vsum > 0.0 ? 1 : 0;
+    double occ = 0.0;
+    for (int k = 0; k <= K; ++k) {
+        sp->lam[k] = sp->steric ? sp->vol[k] / v0 : 0.0;
+        occ += sp->vol[k] * sp->cb[k];
+        sp->lnvc[k] = sp->vol[k] > 0.0 ? std::log(sp->vol[k] * sp->cb[k]) : 0.0;
+    }
+    const double gammaB = 1.0 - occ;
+    if (!(gammaB > 0.0)) return fail(g, PF_ERR_NONPHYSICAL, "Gamma^B = %g <= 0", gammaB);
+    sp->ln_gammaB = std::log(gammaB);
+    double net = 0.0, tot = 0.0;
+    for (int k = 0; k < K; ++k) { net += sp->z[k] * sp->cb[k]; tot += std::fabs(sp->z[k]) * sp->cb[k]; }
+    if (std::fabs(net) > 1e-12 * tot) return fail(g, PF_ERR_NONPHYSICAL, "bath is not neutral");
+    return PF_OK;
+}
+
+}  // namespace
+
+// =========================================================================================
+// C ABI
+// =========================================================================================
+extern "C" {
+
+const char* pf_version(void) { return "pf_b200 0.1 (sm_100a)"; }
+
+const char* pf_last_error(const pf_grid* g) { return g ? g->err.c_str() : g_create_error.c_str(); }
+
+int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double* eps_map,
+                   const pf_charge* charges, int ncharges, const pf_bc* bc, void* cuda_stream) {
+    if (!out) return fail(nullptr, PF_ERR_ARG, "out is NULL");
+    *out = nullptr;
+    if (nx < 3 || ny < 3 || nz < 3) return fail(nullptr, PF_ERR_ARG, "grid needs >= 3 nodes per direction");
+    if (!(h > 0.0)) return fail(nullptr, PF_ERR_ARG, "h must be > 0");
+    if (!eps_map || !bc) return fail(nullptr, PF_ERR_ARG, "eps_map and bc must not be NULL");
+    if (ncharges < 0 || (ncharges > 0 && !charges)) return fail(nullptr, PF_ERR_ARG, "bad charge list");
+    for (int f = 0; f < 6; ++f)
+        if (bc->type[f] != PF_BC_DIRICHLET && bc->type[f] != PF_BC_NEUMANN)
+            return fail(nullptr, PF_ERR_ARG, "bc type of face %d is %d", f, bc->type[f]);
+    int dev = 0, ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, PF_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
+    }
+    pf_grid* g = new pf_grid();
+    g->g.nx = nx; g->g.ny = ny; g->g.nz = nz; g->g.n = (long long)nx * ny * nz;
+    g->h = h;
+    for (int f = 0; f < 6; ++f) { g->bc.type[f] = bc->type[f]; g->bc.value[f] = bc->value[f]; }
+    g->stream = (cudaStream_t)cuda_stream;
+    g->eps = eps_map;
+    g->ncharges = ncharges;
+    g->opt_stencil = 0; g->opt_kernels = 0; g->opt_check = 16; g->opt_lin_maxit = 10000; g->opt_max_outer = 200;
+    g->opt_precond = 1; g->opt_history = 0;
+    g->opt_omega_pf = 0.3; g->opt_lin_tol = 1e-10; g->opt_water = 55.5;
+    g->ws = nullptr; g->ws_bytes = 0; g->assembled = false; g->stored = false;
+    g->pf1_lc = std::nan("");
+    g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0;
+    g->charges_dev = nullptr; g->sc = nullptr; g->rb.partial = nullptr; g->rb.ticket = nullptr;
+    g->lut_poisson = g->lut_pf1 = nullptr; g->dmax_bits = nullptr;
+    g->sc_host[0] = g->sc_host[1] = nullptr; g->ev[0] = g->ev[1] = nullptr;
+#define PF_CREATE_CUDA(call)                                                                         \
+    do {                                                                                             \
+        cudaError_t e_ = (call);                                                                     \
+        if (e_ != cudaSuccess) {                                                                     \
+            int rc_ = fail(nullptr, PF_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_));           \
+            pf_grid_destroy(g);                                                                      \
+            return rc_;                                                                              \
+        }                                                                                            \
+    } while (0)
+    PF_CREATE_CUDA(cudaGetDevice(&dev));
+    PF_CREATE_CUDA(cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    PF_CREATE_CUDA(cudaMalloc(&g->sc, 256));
+    PF_CREATE_CUDA(cudaMalloc(&g->rb.partial, sizeof(dd) * 3 * PF_MAX_PARTIAL_BLOCKS));
+    PF_CREATE_CUDA(cudaMalloc(&g->rb.ticket, 256));
+    PF_CREATE_CUDA(cudaMemsetAsync(g->rb.ticket, 0, 256, g->stream));
+    PF_CREATE_CUDA(cudaMalloc(&g->lut_poisson, sizeof(double) * PF_MAX_CLASSES * PF_MAX_CLASSES));
+    PF_CREATE_CUDA(cudaMalloc(&g->lut_pf1, sizeof(double) * PF_MAX_CLASSES * PF_MAX_CLASSES));
+    PF_CREATE_CUDA(cudaMalloc(&g->dmax_bits, 256));
+    PF_CREATE_CUDA(cudaMallocHost(&g->sc_host[0], sizeof(Scalars)));
+    PF_CREATE_CUDA(cudaMallocHost(&g->sc_host[1], sizeof(Scalars)));
+    PF_CREATE_CUDA(cudaEventCreateWithFlags(&g->ev[0], cudaEventDisableTiming));
+    PF_CREATE_CUDA(cudaEventCreateWithFlags(&g->ev[1], cudaEventDisableTiming));
+    if (ncharges > 0) {
+        PF_CREATE_CUDA(cudaMalloc(&g->charges_dev, sizeof(pf_charge) * ncharges));
+        PF_CREATE_CUDA(cudaMemcpyAsync(g->charges_dev, charges, sizeof(pf_charge) * ncharges, cudaMemcpyHostToDevice,
+                                       g->stream));
+    }
+    PF_CREATE_CUDA(scan_eps(g->stream, g->g.n, eps_map, g->dmax_bits, &g->pal, &g->eps_min, &g->eps_max));
+#undef PF_CREATE_CUDA
+    if (!(g->eps_min > 0.0) || !std::isfinite(g->eps_max)) {
+        int rc = fail(nullptr, PF_ERR_ARG, "eps_map must be finite and > 0 (range %g..%g)", g->eps_min, g->eps_max);
+        pf_grid_destroy(g);
+        return rc;
+    }
+    g->uniform = g->eps_min == g->eps_max;
+    g->eps_mid = 0.5 * (g->eps_min + g->eps_max);     // Q17
+    *out = g;
+    return PF_OK;
+}
+
+void pf_grid_destroy(pf_grid* g) {
+    if (!g) return;
+    cudaStreamSynchronize(g->stream);
+    cudaFree(g->sc); cudaFree(g->rb.partial); cudaFree(g->rb.ticket);
+    cudaFree(g->lut_poisson); cudaFree(g->lut_pf1); cudaFree(g->dmax_bits);
+    cudaFree(g->charges_dev); cudaFree(g->hist);
+    if (g->sc_host[0]) cudaFreeHost(g->sc_host[0]);
+    if (g->sc_host[1]) cudaFreeHost(g->sc_host[1]);
+    if (g->ev[0]) cudaEventDestroy(g->ev[0]);
+    if (g->ev[1]) cudaEventDestroy(g->ev[1]);
+    cudaGetLastError();
+    delete g;
+}
+
+size_t pf_grid_workspace_bytes(const pf_grid* g) {
+    if (!g) return 0;
+    const size_t vec = align_up(sizeof(double) * (size_t)g->g.n, 256);
+    const size_t bytes = align_up((size_t)g->g.n, 256);
+    return (size_t)n_vectors(want_stored(g)) * vec + 2 * bytes;
+}
+
+int pf_grid_set_option(pf_grid* g, int key, double value) {
+    if (!g) return PF_ERR_ARG;
+    const int iv = (int)std::llround(value);
+    switch (key) {
+        case PF_OPT_STENCIL:
+            if (iv < 0 || iv > 2) return fail(g, PF_ERR_ARG, "stencil must be 0, 1 or 2");
+            if (iv == 2 && g->pal.count > PF_MAX_PALETTE)
+                return fail(g, PF_ERR_ARG, "on-the-fly stencil needs <= %d distinct eps values", PF_MAX_PALETTE);
+            if (g->assembled && (iv == 1) != g->stored && iv != 0)
+                return fail(g, PF_ERR_ARG, "set the stencil variant before pf_grid_set_workspace");
+            g->opt_stencil = iv;
+            return PF_OK;
+        case PF_OPT_OMEGA_PF:
+            if (!(value >= 0.0 && value < 1.0)) return fail(g, PF_ERR_ARG, "omega_PF must be in [0,1)");
+            g->opt_omega_pf = value; return PF_OK;
+        case PF_OPT_LINEAR_TOL:
+            if (!(value >= 0.0)) return fail(g, PF_ERR_ARG, "tolerance must be >= 0");
+            g->opt_lin_tol = value; return PF_OK;
+        case PF_OPT_LINEAR_MAXIT:
+            if (iv < 0) return fail(g, PF_ERR_ARG, "maxit must be >= 0");
+            g->opt_lin_maxit = iv; return PF_OK;
+        case PF_OPT_CHECK_INTERVAL:
+            if (iv < 1) return fail(g, PF_ERR_ARG, "check interval must be >= 1");
+            g->opt_check = iv; return PF_OK;
+        case PF_OPT_WATER_MOLAR:
+            if (!(value >= 0.0)) return fail(g, PF_ERR_ARG, "water concentration must be >= 0");
+            g->opt_water = value; return PF_OK;
+        case PF_OPT_MAX_OUTER:
+            if (iv < 1) return fail(g, PF_ERR_ARG, "max outer iterations must be >= 1");
+            g->opt_max_outer = iv; return PF_OK;
+        case PF_OPT_PRECOND:
+            g->opt_precond = iv != 0; return PF_OK;
+        case PF_OPT_HISTORY: {
+            if (iv < 0) return fail(g, PF_ERR_ARG, "history length must be >= 0");
+            cudaStreamSynchronize(g->stream);
+            cudaFree(g->hist); g->hist = nullptr; g->hist_cap = 0;
+            if (iv > 0) {
+                PF_CUDA(g, cudaMalloc(&g->hist, sizeof(double) * (size_t)iv));
+                g->hist_cap = iv;
+            }
+            g->opt_history = iv;
+            return PF_OK;
+        }
+        case PF_OPT_KERNELS:
+            if (iv < 0 || iv > 2) return fail(g, PF_ERR_ARG, "kernels must be 0, 1 or 2");
+            if (iv == 2 && !tiled_supported(g->g)) return fail(g, PF_ERR_ARG, "grid too small for the tiled kernels");
+            g->opt_kernels = iv; return PF_OK;
+        default:
+            return fail(g, PF_ERR_ARG, "unknown option key %d", key);
+    }
+}
+
+int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
+    if (!g) return PF_ERR_ARG;
+    if (!dev_ptr) return fail(g, PF_ERR_ARG, "workspace pointer is NULL");
+    if (((uintptr_t)dev_ptr & 255u) != 0) return fail(g, PF_ERR_ARG, "workspace must be 256-byte aligned");
+    const size_t need = pf_grid_workspace_bytes(g);
+    if (bytes < need) return fail(g, PF_ERR_WORKSPACE, "workspace has %zu bytes, %zu needed", bytes, need);
+    g->stored = want_stored(g);
+    g->ws = dev_ptr; g->ws_bytes = bytes;
+    const size_t vec = align_up(sizeof(double) * (size_t)g->g.n, 256);
+    char* base = (char*)dev_ptr;
+    auto take = [&]() { double* p = (double*)base; base += vec; return p; };
+    g->r = take(); g->rt = take(); g->p0 = take(); g->p1 = take(); g->v0 = take(); g->v1 = take();
+    g->t = take(); g->bw = take(); g->xw = take();
+    g->A0 = take(); g->A0_pf1 = take(); g->A0_s = take(); g->fixed = take(); g->psi = take();
+    g->phi0 = take(); g->phiw = take(); g->sigma = take(); g->bpf = take();
+    for (int d = 0; d < 6; ++d) { g->offd[d] = g->stored ? take() : nullptr; }
+    for (int d = 0; d < 6; ++d) { g->offd_pf1[d] = g->stored ? take() : nullptr; }
+    const size_t nb = align_up((size_t)g->g.n, 256);
+    g->cls = (uint8_t*)base; base += nb;
+    g->cls_pf1 = (uint8_t*)base; base += nb;
+    const bool use_pal = g->pal.count <= PF_MAX_PALETTE;
+    // rows L1, L2: Poisson operator, coefficient table, fixed charges
+    launch_assemble_poisson(g->stream, g->g, g->h, g->bc, g->eps, g->pal, use_pal, g->A0, g->cls, g->offd);
+    if (use_pal) {
+        double lut[PF_MAX_CLASSES * PF_MAX_CLASSES];
+        int nc = 0;
+        build_lut_poisson(g->pal, g->h, lut, &nc);
+        PF_CUDA(g, cudaMemcpyAsync(g->lut_poisson, lut, sizeof(lut), cudaMemcpyHostToDevice, g->stream));
+    }
+    launch_deposit(g->stream, g->g, g->h, kappa_angstrom(), g->charges_dev, g->ncharges, g->fixed);
+    PF_CUDA(g, cudaMemsetAsync(g->p0, 0, vec * 4, g->stream));   // p0,p1,v0,v1 finite before first use
+    PF_CUDA(g, cudaStreamSynchronize(g->stream));
+    PF_CUDA(g, cudaGetLastError());
+    g->pf1_lc = std::nan("");
+    g->assembled = true;
+    return PF_OK;
+}
+
+int pf_solve_linear(pf_grid* g, const double* rhs, double* x, const double* sigma, double tol, int maxit,
+                    int* iters_out, double* relres_out, double* true_relres_out) {
+    int rc = check_ready(g);
+    if (rc) return rc;
+    if (!rhs || !x) return fail(g, PF_ERR_ARG, "rhs and x must not be NULL");
+    launch_copy_with_dirichlet(g->stream, g->g, g->bc, rhs, g->bw);   // Q20
+    launch_set_dirichlet(g->stream, g->g, g->bc, x);                   // Q4
+    int which = 0;
+    if (sigma) { launch_diag_plus_sigma(g->stream, g->g, g->bc, g->A0, sigma, g->A0_s); which = 2; }
+    return bicgstab_device(g, make_op(g, which), g->bw, x, tol, maxit, iters_out, relres_out, true_relres_out);
+}
+
+int pf_solve_linear_host(pf_grid* g, const double* rhs_host, double* x_host, const double* sigma, double tol,
+                         int maxit, int* iters_out, double* relres_out, double* true_relres_out) {
+    int rc = check_ready(g);
+    if (rc) return rc;
+    if (!rhs_host || !x_host) return fail(g, PF_ERR_ARG, "rhs and x must not be NULL");
+    const size_t nbytes = sizeof(double) * (size_t)g->g.n;
+    // bpf and xw are scratch of the PF loop, free during a plain linear solve
+    PF_CUDA(g, cudaMemcpyAsync(g->bpf, rhs_host, nbytes, cudaMemcpyHostToDevice, g->stream));
+    PF_CUDA(g, cudaMemcpyAsync(g->xw, x_host, nbytes, cudaMemcpyHostToDevice, g->stream));
+    rc = pf_solve_linear(g, g->bpf, g->xw, sigma, tol, maxit, iters_out, relres_out, true_relres_out);
+    if (rc < 0) return rc;
+    PF_CUDA(g, cudaMemcpyAsync(x_host, g->xw, nbytes, cudaMemcpyDeviceToHost, g->stream));
+    PF_CUDA(g, cudaStreamSynchronize(g->stream));
+    return rc;
+}
+
+int pf_fermi_pointwise(pf_grid* g, int nions, const double* valence, const double* bath_conc, const double* radii,
+                       const double* phi, double* rho, double* sigma, double* steric, double* conc) {
+    int rc = check_ready(g);
+    if (rc) return rc;
+    if (!phi) return fail(g, PF_ERR_ARG, "phi must not be NULL");
+    SpeciesDev sp;
+    rc = make_species(g, nions, valence, bath_conc, radii, &sp);
+    if (rc) return rc;
+    launch_fermi(g->stream, g->g, g->bc, sp, g->eps, g->eps_mid, g->uniform, phi, rho, sigma, steric, conc, nullptr,
+                 nullptr, nullptr);
+    PF_CUDA(g, cudaStreamSynchronize(g->stream));
+    PF_CUDA(g, cudaGetLastError());
+    return PF_OK;
+}
+
+int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath_conc, const double* radii,
+                double l_c, double tol, double* phi, double* conc, double* steric, int* outer_iters_out,
+                int* linear_iters_out) {
+    int rc = check_ready(g);
+    if (rc) return rc;
+    if (!phi) return fail(g, PF_ERR_ARG, "phi must not be NULL");
+    if (!(l_c >= 0.0) || !(tol >= 0.0)) return fail(g, PF_ERR_ARG, "l_c and tol must be >= 0");
+    SpeciesDev sp;
+    rc = make_species(g, nions, valence, bath_conc, radii, &sp);
+    if (rc) return rc;
+    const size_t nbytes = sizeof(double) * (size_t)g->g.n;
+    const bool use_pal = g->pal.count <= PF_MAX_PALETTE;
+    if (!(g->pf1_lc == l_c)) {      // row N2: PF1 operator, once per (grid, l_c)
+        launch_assemble_pf1(g->stream, g->g, g->h, l_c, g->eps, g->eps_mid, g->uniform, g->pal, use_pal, g->A0_pf1,
+                            g->cls_pf1, g->offd_pf1);
+        if (use_pal) {
+            double lut[PF_MAX_CLASSES * PF_MAX_CLASSES];
+            int nc = 0;
+            build_lut_pf1(g->pal, g->h, l_c, lut, &nc);
+            PF_CUDA(g, cudaMemcpyAsync(g->lut_pf1, lut, sizeof(lut), cudaMemcpyHostToDevice, g->stream));
+        }
+        g->pf1_lc = l_c;
+    }
+    g->lin_iters.clear();
+    int total = 0, its = 0;
+    // row N4 (Table 2 step 2): initial guess from PF2 with rho' = Psi = 0
+    launch_copy_with_dirichlet(g->stream, g->g, g->bc, g->fixed, g->bpf);
+    PF_CUDA(g, cudaMemsetAsync(g->phi0, 0, nbytes, g->stream));
+    launch_set_dirichlet(g->stream, g->g, g->bc, g->phi0);
+    rc = bicgstab_device(g, make_op(g, 0), g->bpf, g->phi0, g->opt_lin_tol, g->opt_lin_maxit, &its, nullptr, nullptr);
+    g->lin_iters.push_back(its); total += its;
+    if (rc < 0) return rc;
+    PF_CUDA(g, cudaMemsetAsync(g->psi, 0, nbytes, g->stream));
+    int status = PF_NOT_CONVERGED, outer = 0;
+    double* phi0 = g->phi0;
+    double* phiw = g->phiw;
+    while (outer < g->opt_max_outer) {
+        ++outer;
+        // row N1: concentrations, steric potential, PF1 right-hand side, PF2 diagonal -- one kernel
+        launch_fermi(g->stream, g->g, g->bc, sp, g->eps, g->eps_mid, g->uniform, phi0, nullptr, g->sigma, nullptr,
+                     nullptr, g->bpf, g->A0, g->A0_s);
+        // row N2 (step 3): PF1 -> Psi, warm start from the previous Psi
+        rc = bicgstab_device(g, make_op(g, 1), g->bpf, g->psi, g->opt_lin_tol, g->opt_lin_maxit, &its, nullptr, nullptr);
+        g->lin_iters.push_back(its); total += its;
+        if (rc < 0) return rc;
+        // row N3 (step 4): PF2 -> phi, warm start from phi0
+        launch_rhs_pf2(g->stream, g->g, g->bc, g->eps, g->eps_mid, g->uniform, g->psi, g->sigma, phi0, g->fixed, g->bpf);
+        PF_CUDA(g, cudaMemcpyAsync(phiw, phi0, nbytes, cudaMemcpyDeviceToDevice, g->stream));
+        rc = bicgstab_device(g, make_op(g, 2), g->bpf, phiw, g->opt_lin_tol, g->opt_lin_maxit, &its, nullptr, nullptr);
+        g->lin_iters.push_back(its); total += its;
+        if (rc < 0) return rc;
+        // row N5 (step 5): relax, then test the increment
+        launch_relax(g->stream, g->g.n, g->opt_omega_pf, phi0, phiw, g->dmax_bits);
+        unsigned long long bits = 0;
+        PF_CUDA(g, cudaMemcpyAsync(&bits, g->dmax_bits, sizeof(bits), cudaMemcpyDeviceToHost, g->stream));
+        PF_CUDA(g, cudaStreamSynchronize(g->stream));
+        double d;
+        std::memcpy(&d, &bits, sizeof(d));
+        std::swap(phi0, phiw);
+        if (!(d > tol)) { status = PF_OK; break; }
+    }
+    PF_CUDA(g, cudaMemcpyAsync(phi, phi0, nbytes, cudaMemcpyDeviceToDevice, g->stream));
+    if (conc || steric)
+        launch_fermi(g->stream, g->g, g->bc, sp, g->eps, g->eps_mid, g->uniform, phi0, nullptr, nullptr, steric, conc,
+                     nullptr, nullptr, nullptr);
+    PF_CUDA(g, cudaStreamSynchronize(g->stream));
+    PF_CUDA(g, cudaGetLastError());
+    if (outer_iters_out) *outer_iters_out = outer;
+    if (linear_iters_out) *linear_iters_out = total;
+    return status;
+}
+
+int pf_grid_history(pf_grid* g, double* hist_host, int cap) {
+    if (!g || !hist_host || cap < 0) return PF_ERR_ARG;
+    if (!g->hist) return fail(g, PF_ERR_ARG, "history not enabled (PF_OPT_HISTORY)");
+    const int n = std::min(std::min(cap, g->hist_cap), g->last_iters + 1);
+    PF_CUDA(g, cudaMemcpyAsync(hist_host, g->hist, sizeof(double) * (size_t)n, cudaMemcpyDeviceToHost, g->stream));
+    PF_CUDA(g, cudaStreamSynchronize(g->stream));
+    return n;
+}
+
+int pf_grid_linear_iters(pf_grid* g, int* iters_host, int cap) {
+    if (!g || !iters_host || cap < 0) return PF_ERR_ARG;
+    const int n = std::min<int>(cap, (int)g->lin_iters.size());
+    for (int k = 0; k < n; ++k) iters_host[k] = g->lin_iters[k];
+    return n;
+}
+
+int pf_grid_stencil(const pf_grid* g) { return g ? (want_stored(g) ? 1 : 2) : PF_ERR_ARG; }
+int pf_grid_palette_size(const pf_grid* g) { return g ? g->pal.count : PF_ERR_ARG; }
+
+int pf_grid_copy_array(pf_grid* g, int which, void* dst) {
+    if (!g || !dst) return PF_ERR_ARG;
+    if (!g->assembled) return fail(g, PF_ERR_WORKSPACE, "workspace not set");
+    const void* src = nullptr;
+    size_t nbytes = sizeof(double) * (size_t)g->g.n;
+    if (which == 0) src = g->A0;
+    else if (which >= 1 && which <= 6) src = g->offd[which - 1];
+    else if (which == 7) src = g->fixed;
+    else if (which == 8) { src = g->pal.count <= PF_MAX_PALETTE ? g->cls : nullptr; nbytes = (size_t)g->g.n; }
+    else if (which == 9) src = (g->pf1_lc == g->pf1_lc) ? g->A0_pf1 : nullptr;
+    if (!src) return fail(g, PF_ERR_ARG, "array %d is not available", which);
+    PF_CUDA(g, cudaMemcpyAsync(dst, src, nbytes, cudaMemcpyDeviceToDevice, g->stream));
+    PF_CUDA(g, cudaStreamSynchronize(g->stream));
+    return PF_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,277 @@
+// pf_assembly.cu -- operator assembly on the device (rows L1, L2 of DESIGN.md).
+//
+// The paper builds A0..A6 and b on the GPU each outer iteration and finds that the weak part of its
+// design (7.7x against 22.8x for the solver).  Here the flux part of every
+// operator is assembled ONCE per grid: per node a class byte (palette index of eps, identity-row
+// flag) and the diagonal; the six off-diagonals are either stored (the paper's format)
+// or looked up on the fly in a (class x class) table.  PF2's sigma only shifts the diagonal.
+#include "pf_launch.h"
+#include <algorithm>
+#include <cstring>
+
+namespace pf {
+
+namespace {
+
+constexpr int ASM_THREADS = 256;
+constexpr int IDENT_BIT = PF_MAX_PALETTE;        // cls = palette index + IDENT_BIT*identity
+constexpr int CLS_OUTSIDE = 2 * PF_MAX_PALETTE;  // neighbour outside the box
+
+struct ScanBuf {
+    unsigned long long tab[PF_MAX_PALETTE + 1];  // bit patterns of the distinct values, 0 = empty
+    unsigned long long min_bits, max_bits;
+    int overflow;
+};
+
+__global__ void k_scan_eps(long long n, const double* __restrict__ eps, ScanBuf* sb) {
+    unsigned long long lo = ~0ull, hi = 0ull;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const unsigned long long bits = (unsigned long long)__double_as_longlong(eps[i]);
+        lo = bits < lo ? bits : lo;
+        hi = bits > hi ? bits : hi;
+        bool found = false;
+        int k = 0;
+        for (; k <= PF_MAX_PALETTE; ++k) {
+            const unsigned long long v = ((volatile unsigned long long*)sb->tab)[k];
+            if (v == bits) { found = true; break; }
+            if (v == 0ull) break;
+        }
+        if (found) continue;
+        for (; k <= PF_MAX_PALETTE; ++k) {
+            const unsigned long long old = atomicCAS(&sb->tab[k], 0ull, bits);
+            if (old == 0ull || old == bits) { found = true; break; }
+        }
+        if (!found) sb->overflow = 1;
+    }
+    for (int d = 16; d > 0; d >>= 1) {
+        unsigned long long a = __shfl_xor_sync(0xffffffffu, lo, d), b = __shfl_xor_sync(0xffffffffu, hi, d);
+        lo = a < lo ? a : lo;
+        hi = b > hi ? b : hi;
+    }
+    if ((threadIdx.x & 31) == 0) { atomicMin(&sb->min_bits, lo); atomicMax(&sb->max_bits, hi); }
+}
+
+// First Dirichlet face the node lies on (order -x,+x,-y,+y,-z,+z), else -1 (reading Q20).
+__device__ __forceinline__ int dirichlet_face(const GridDims& g, const BcDev& bc, int ix, int iy, int iz) {
+    if (ix == 0 && bc.type[0] == 0) return 0;
+    if (ix == g.nx - 1 && bc.type[1] == 0) return 1;
+    if (iy == 0 && bc.type[2] == 0) return 2;
+    if (iy == g.ny - 1 && bc.type[3] == 0) return 3;
+    if (iz == 0 && bc.type[4] == 0) return 4;
+    if (iz == g.nz - 1 && bc.type[5] == 0) return 5;
+    return -1;
+}
+
+__device__ __forceinline__ void decode(const GridDims& g, long long i, int& ix, int& iy, int& iz) {
+    ix = (int)(i % g.nx);
+    const long long q = i / g.nx;
+    iy = (int)(q % g.ny);
+    iz = (int)(q / g.ny);
+}
+
+__device__ __forceinline__ int palette_index(const Palette& pal, double e) {
+    int k = 0;
+#pragma unroll
+    for (int m = 1; m < PF_MAX_PALETTE; ++m)
+        if (m < pal.count && e == pal.value[m]) k = m;
+    return k;
+}
+
+// Face coefficient: harmonic mean of eps over h^2 -- Eqs (17)-(18) with the interface at the face
+// midpoint (reading R2/Q16).
+__device__ __forceinline__ double face_coeff(double ea, double eb, double hh) {
+    return dvd(dvd(mul(mul(2.0, ea), eb), add(ea, eb)), hh);
+}
+
+__global__ void __launch_bounds__(ASM_THREADS)
+k_assemble_poisson(GridDims g, double h, BcDev bc, const double* __restrict__ eps, Palette pal, bool use_palette,
+                   double* __restrict__ A0, uint8_t* __restrict__ cls, double* o0, double* o1, double* o2,
+                   double* o3, double* o4, double* o5) {
+    double* offd[6] = {o0, o1, o2, o3, o4, o5};
+    const double hh = mul(h, h);
+    const long long off[6] = {1, -1, -(long long)g.nx, (long long)g.nx, -(long long)g.nx * g.ny,
+                              (long long)g.nx * g.ny};
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
+        int ix, iy, iz;
+        decode(g, i, ix, iy, iz);
+        const double ei = eps[i];
+        const bool ident = dirichlet_face(g, bc, ix, iy, iz) >= 0;
+        if (use_palette) cls[i] = (uint8_t)(palette_index(pal, ei) + (ident ? IDENT_BIT : 0));
+        if (ident) {
+            A0[i] = 1.0;
+#pragma unroll
+            for (int d = 0; d < 6; ++d) if (offd[d]) offd[d][i] = 0.0;
+            continue;
+        }
+        const bool in[6] = {ix + 1 < g.nx, ix > 0, iy > 0, iy + 1 < g.ny, iz > 0, iz + 1 < g.nz};
+        double diag = 0.0;
+#pragma unroll
+        for (int d = 0; d < 6; ++d) {
+            double c = 0.0;
+            if (in[d]) {
+                c = face_coeff(ei, eps[i + off[d]], hh);
+                diag = add(diag, c);
+            }
+            if (offd[d]) offd[d][i] = in[d] ? -c : 0.0;
+        }
+        A0[i] = diag;
+    }
+}
+
+__global__ void __launch_bounds__(ASM_THREADS)
+k_assemble_pf1(GridDims g, double h, double lc, const double* __restrict__ eps, double eps_mid, bool uniform,
+               Palette pal, bool use_palette, double* __restrict__ A0, uint8_t* __restrict__ cls, double* o0,
+               double* o1, double* o2, double* o3, double* o4, double* o5) {
+    double* offd[6] = {o0, o1, o2, o3, o4, o5};
+    const double hh = mul(h, h), ll = mul(lc, lc);
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
+        int ix, iy, iz;
+        decode(g, i, ix, iy, iz);
+        const double ei = eps[i];
+        const bool boundary = ix == 0 || ix == g.nx - 1 || iy == 0 || iy == g.ny - 1 || iz == 0 || iz == g.nz - 1;
+        const bool solvent = uniform || ei > eps_mid;           // Q17
+        const bool ident = boundary || !solvent;                // Q15
+        if (use_palette) cls[i] = (uint8_t)(palette_index(pal, ei) + (ident ? IDENT_BIT : 0));
+        if (ident) {
+            A0[i] = 1.0;
+#pragma unroll
+            for (int d = 0; d < 6; ++d) if (offd[d]) offd[d][i] = 0.0;
+            continue;
+        }
+        const double c = dvd(mul(ei, ll), hh);
+        A0[i] = add(mul(6.0, c), ei);
+#pragma unroll
+        for (int d = 0; d < 6; ++d) if (offd[d]) offd[d][i] = -c;
+    }
+}
+
+// One thread: the deposits of different charges can hit the same node and floating-point addition
+// is not associative, so they are applied in charge order (reading R2; runs once per grid).
+__global__ void k_deposit(GridDims g, double h, double kappa, const double* __restrict__ ch, int m, double* fixed) {
+    if (blockIdx.x != 0 || threadIdx.x != 0) return;
+    const double h3 = mul(mul(h, h), h);
+    for (int c = 0; c < m; ++c) {
+        const double px = dvd(ch[4 * c], h), py = dvd(ch[4 * c + 1], h), pz = dvd(ch[4 * c + 2], h);
+        const double q = ch[4 * c + 3];
+        const int ix = min(max((int)floor(px), 0), g.nx - 2);
+        const int iy = min(max((int)floor(py), 0), g.ny - 2);
+        const int iz = min(max((int)floor(pz), 0), g.nz - 2);
+        const double fx = sub(px, (double)ix), fy = sub(py, (double)iy), fz = sub(pz, (double)iz);
+        const double amp = dvd(mul(kappa, q), h3);
+        for (int dz = 0; dz < 2; ++dz)
+            for (int dy = 0; dy < 2; ++dy)
+                for (int dx = 0; dx < 2; ++dx) {
+                    const double wx = dx ? fx : sub(1.0, fx), wy = dy ? fy : sub(1.0, fy), wz = dz ? fz : sub(1.0, fz);
+                    const double w = mul(mul(wx, wy), wz);
+                    const long long i = (ix + dx) + (long long)g.nx * ((iy + dy) + (long long)g.ny * (iz + dz));
+                    fixed[i] = add(fixed[i], mul(amp, w));
+                }
+    }
+}
+
+__global__ void __launch_bounds__(ASM_THREADS)
+k_set_dirichlet(GridDims g, BcDev bc, const double* __restrict__ src, double* __restrict__ dst) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
+        int ix, iy, iz;
+        decode(g, i, ix, iy, iz);
+        const int f = dirichlet_face(g, bc, ix, iy, iz);
+        if (f >= 0) dst[i] = bc.value[f];
+        else if (src != dst) dst[i] = src[i];
+    }
+}
+
+int asm_blocks(long long n) {
+    long long b = (n + ASM_THREADS - 1) / ASM_THREADS;
+    return (int)std::min<long long>(std::max<long long>(b, 1), 148 * 16);
+}
+
+double host_face_coeff(double ea, double eb, double h) { return (2.0 * ea * eb / (ea + eb)) / (h * h); }
+
+}  // namespace
+
+cudaError_t scan_eps(cudaStream_t s, long long n, const double* eps, void* scratch, Palette* out, double* eps_min,
+                     double* eps_max) {
+    ScanBuf init;
+    std::memset(&init, 0, sizeof(init));
+    init.min_bits = ~0ull;
+    cudaError_t e = cudaMemcpyAsync(scratch, &init, sizeof(init), cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return e;
+    k_scan_eps<<<asm_blocks(n), ASM_THREADS, 0, s>>>(n, eps, (ScanBuf*)scratch);
+    ScanBuf res;
+    e = cudaMemcpyAsync(&res, scratch, sizeof(res), cudaMemcpyDeviceToHost, s);
+    if (e != cudaSuccess) return e;
+    e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return e;
+    int cnt = 0;
+    double vals[PF_MAX_PALETTE + 1];
+    for (int k = 0; k <= PF_MAX_PALETTE; ++k)
+        if (res.tab[k] != 0ull) { std::memcpy(&vals[cnt], &res.tab[k], 8); ++cnt; }
+    std::sort(vals, vals + cnt);
+    out->count = res.overflow ? PF_MAX_PALETTE + 1 : cnt;
+    for (int k = 0; k <= PF_MAX_PALETTE; ++k) out->value[k] = k < cnt ? vals[k] : 0.0;
+    std::memcpy(eps_min, &res.min_bits, 8);
+    std::memcpy(eps_max, &res.max_bits, 8);
+    return cudaSuccess;
+}
+
+void launch_assemble_poisson(cudaStream_t s, const GridDims& g, double h, const BcDev& bc, const double* eps,
+                             const Palette& pal, bool use_palette, double* A0, uint8_t* cls, double* const offd[6]) {
+    k_assemble_poisson<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, h, bc, eps, pal, use_palette, A0, cls, offd[0],
+                                                                offd[1], offd[2], offd[3], offd[4], offd[5]);
+}
+
+void launch_assemble_pf1(cudaStream_t s, const GridDims& g, double h, double lc, const double* eps, double eps_mid,
+                         bool uniform, const Palette& pal, bool use_palette, double* A0, uint8_t* cls,
+                         double* const offd[6]) {
+    k_assemble_pf1<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, h, lc, eps, eps_mid, uniform, pal, use_palette, A0, cls,
+                                                            offd[0], offd[1], offd[2], offd[3], offd[4], offd[5]);
+}
+
+// Tables of the on-the-fly variant: entry [ci*ncls + cn] is the off-diagonal coefficient of a row of
+// class ci towards a neighbour of class cn.  Identity rows and outside neighbours give 0.
+void build_lut_poisson(const Palette& pal, double h, double* lut, int* ncls) {
+    const int nc = PF_MAX_CLASSES;
+    *ncls = nc;
+    for (int ci = 0; ci < nc; ++ci)
+        for (int cn = 0; cn < nc; ++cn) {
+            double v = 0.0;
+            const bool ident = ci >= IDENT_BIT, outside = (cn == CLS_OUTSIDE) || (ci == CLS_OUTSIDE);
+            const int pi = ci % PF_MAX_PALETTE, pn = cn % PF_MAX_PALETTE;
+            if (!ident && !outside && pi < pal.count && pn < pal.count)
+                v = -host_face_coeff(pal.value[pi], pal.value[pn], h);
+            lut[ci * nc + cn] = v;
+        }
+}
+
+void build_lut_pf1(const Palette& pal, double h, double lc, double* lut, int* ncls) {
+    const int nc = PF_MAX_CLASSES;
+    *ncls = nc;
+    for (int ci = 0; ci < nc; ++ci)
+        for (int cn = 0; cn < nc; ++cn) {
+            double v = 0.0;
+            const bool ident = ci >= IDENT_BIT, outside = (cn == CLS_OUTSIDE) || (ci == CLS_OUTSIDE);
+            const int pi = ci % PF_MAX_PALETTE;
+            if (!ident && !outside && pi < pal.count) v = -(pal.value[pi] * (lc * lc) / (h * h));
+            lut[ci * nc + cn] = v;
+        }
+}
+
+void launch_deposit(cudaStream_t s, const GridDims& g, double h, double kappa, const double* charges_dev, int m,
+                    double* fixed) {
+    cudaMemsetAsync(fixed, 0, sizeof(double) * g.n, s);
+    if (m > 0) k_deposit<<<1, 32, 0, s>>>(g, h, kappa, charges_dev, m, fixed);
+}
+
+void launch_set_dirichlet(cudaStream_t s, const GridDims& g, const BcDev& bc, double* x) {
+    k_set_dirichlet<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, bc, x, x);
+}
+
+void launch_copy_with_dirichlet(cudaStream_t s, const GridDims& g, const BcDev& bc, const double* src, double* dst) {
+    k_set_dirichlet<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, bc, src, dst);
+}
+
+}  // namespace pf

@@ -1,0 +1,88 @@
+// pf_krylov.cuh -- pieces shared by the direct and the tiled Krylov kernels: the elementwise
+// statements of Table 3 (reading R3) and the scalar work that thread 0 of the
+// last block does at each of the three reduction points of an iteration (rows L4-L8).
+#pragma once
+#include "pf_common.cuh"
+
+namespace pf {
+
+// Vectors of one solve.  p and v are double-buffered: the fused kernel of steps 9+11 reads the old
+// p, v at neighbour nodes while other blocks already write the new ones.
+struct KrylovVecs {
+    const double* b;     // right-hand side with Dirichlet values in place
+    double* x;
+    double* r;
+    double* rt;          // r~ = r0
+    double* p_in;  double* p_out;
+    double* v_in;  double* v_out;
+    double* t;
+    double* hist;        // relative residual per iteration, or null
+};
+
+// Step 9 (+ the Jacobi step of reading Q2): value the first matvec is applied to, at node j.
+//   p_j = r_j + beta (p_j - omega v_j)   (p = r in the first iteration, steps 5-6)
+template <bool PRECOND>
+__device__ __forceinline__ double p_new_at(bool first, double beta, double omega, double r, double p, double v) {
+    (void)PRECOND;
+    return first ? r : add(r, mul(beta, sub(p, mul(omega, v))));
+}
+
+// Step 13: s_j = r_j - alpha v_j.
+__device__ __forceinline__ double s_at(double alpha, double r, double v) { return sub(r, mul(alpha, v)); }
+
+template <bool PRECOND>
+__device__ __forceinline__ double jacobi(double u, double a0) { return PRECOND ? dvd(u, a0) : u; }
+
+// ---- reduction-point epilogues (thread 0 of the last block only) ------------------------------
+
+// After r0 = b - A x0 (step 2): ||b||, ||r0||, rho_0 = r~.r0 = r0.r0, early exits.
+__device__ __forceinline__ void finish_init(Scalars* sc, double* hist, double bb, double rr) {
+    sc->bb = bb; sc->rr = rr;
+    sc->bnorm = __dsqrt_rn(bb);
+    sc->rnorm = __dsqrt_rn(rr);
+    sc->it = 0; sc->first = 1; sc->done = 0; sc->status = 1;
+    sc->rho = rr; sc->rho_old = 1.0; sc->alpha = 1.0; sc->omega = 1.0; sc->beta = 0.0;
+    if (bb == 0.0) {                       // Q3: b = 0 => x = 0, no iterations (host zeroes x)
+        sc->done = 1; sc->status = 0; sc->rnorm = 0.0; sc->bnorm = 0.0;
+        if (hist && sc->hist_cap > 0) hist[0] = 0.0;
+        return;
+    }
+    if (hist && sc->hist_cap > 0) hist[0] = dvd(sc->rnorm, sc->bnorm);
+    if (sc->rnorm <= mul(sc->tol, sc->bnorm)) { sc->done = 1; sc->status = 0; return; }
+    if (sc->maxit <= 0) { sc->done = 1; sc->status = 1; return; }
+    if (rr == 0.0) { sc->done = 1; sc->status = -3; }
+}
+
+// After v = A M^-1 p (step 11): alpha = rho/(r~.v) (step 12).
+__device__ __forceinline__ void finish_k1(Scalars* sc, double rtv) {
+    sc->rtv = rtv;
+    if (rtv == 0.0) { sc->done = 1; sc->status = -3; return; }
+    sc->alpha = dvd(sc->rho, rtv);
+}
+
+// After t = A M^-1 s (step 14): omega = t.s/t.t (step 15); t.t = 0 => omega = 0 (Q5).
+__device__ __forceinline__ void finish_k2(Scalars* sc, double ts, double tt) {
+    sc->ts = ts; sc->tt = tt;
+    sc->omega = (tt == 0.0) ? 0.0 : dvd(ts, tt);
+}
+
+// After the x and r updates (steps 16-17): ||r|| test (steps 18-20), then rho and beta of the next
+// iteration (steps 4, 8).
+__device__ __forceinline__ void finish_k3(Scalars* sc, double* hist, double rho_new, double rr) {
+    sc->rr = rr;
+    sc->rnorm = __dsqrt_rn(rr);
+    const int it = sc->it + 1;
+    sc->it = it;
+    if (hist && it < sc->hist_cap) hist[it] = dvd(sc->rnorm, sc->bnorm);
+    const double rho_old = sc->rho;
+    sc->rho_old = rho_old;
+    if (sc->rnorm <= mul(sc->tol, sc->bnorm)) { sc->done = 1; sc->status = 0; return; }
+    if (sc->omega == 0.0) { sc->done = 1; sc->status = -3; return; }
+    if (it >= sc->maxit) { sc->done = 1; sc->status = 1; return; }
+    sc->rho = rho_new;
+    if (rho_new == 0.0) { sc->done = 1; sc->status = -3; return; }
+    sc->beta = mul(dvd(rho_new, rho_old), dvd(sc->alpha, sc->omega));   // step 8
+    sc->first = 0;
+}
+
+}  // namespace pf

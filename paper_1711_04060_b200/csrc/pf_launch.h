@@ -1,0 +1,91 @@
+// pf_launch.h -- host-side launch interface between the solver driver (pf_api.cu) and the kernel
+// translation units.  Internal; the public boundary is include/pf.h.
+#pragma once
+#include "pf_common.cuh"
+#include "pf_krylov.cuh"
+
+namespace pf {
+
+struct LaunchCtx {
+    cudaStream_t stream;
+    GridDims g;
+    Scalars* sc;      // device
+    ReduceBuf rb;     // device
+    int sm_count;
+};
+
+// ---- Krylov kernels -----------------------------------------------------------------------
+// mode 0: r = b - A x, r~ = r, ||b||, ||r|| (Table 3 step 2); mode 1: ||b - A x||^2 only.
+void launch_residual_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, int mode);
+void launch_k1_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
+void launch_k2_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
+void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
+
+// Tiled family (pf_krylov_tiled.cu).  tiled_supported() says whether the grid fills the tiles.
+bool tiled_supported(const GridDims& g);
+void launch_residual_tiled(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, int mode);
+void launch_k1_tiled(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
+void launch_k2_tiled(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
+
+// ---- assembly (pf_assembly.cu) ----------------------------------------------------------------
+struct BcDev { int type[6]; double value[6]; };
+
+struct Palette {
+    int count;                         // distinct eps values found (PF_MAX_PALETTE+1 = overflow)
+    double value[PF_MAX_PALETTE + 1];  // ascending
+};
+
+// Scan eps for its distinct values and its range.  scratch: device, >= 256 bytes, zeroed by the call.
+cudaError_t scan_eps(cudaStream_t s, long long n, const double* eps, void* scratch, Palette* out,
+                     double* eps_min, double* eps_max);
+
+// Poisson operator of Eq (3)/(13) without sigma: diagonal A0, classes, optionally A1..A6.
+void launch_assemble_poisson(cudaStream_t s, const GridDims& g, double h, const BcDev& bc, const double* eps,
+                             const Palette& pal, bool use_palette, double* A0, uint8_t* cls,
+                             double* const offd[6] /* entries null unless stored */);
+// PF1 operator eps(l_c^2 Lap - 1), sign flipped (Eq (12)), identity rows on the
+// box boundary and outside the solvent (Q15).
+void launch_assemble_pf1(cudaStream_t s, const GridDims& g, double h, double lc, const double* eps, double eps_mid,
+                         bool uniform, const Palette& pal, bool use_palette, double* A0, uint8_t* cls,
+                         double* const offd[6]);
+// Coefficient tables of the on-the-fly variant (host side; ncls*ncls doubles each).
+void build_lut_poisson(const Palette& pal, double h, double* lut_host, int* ncls);
+void build_lut_pf1(const Palette& pal, double h, double lc, double* lut_host, int* ncls);
+
+// Trilinear deposition of the fixed charges (reading R2): fixed[i] += kappa q w / h^3, in charge order.
+void launch_deposit(cudaStream_t s, const GridDims& g, double h, double kappa, const double* charges_dev, int m,
+                    double* fixed);
+// x[i] = g_face at Dirichlet nodes (Q4, Q20).
+void launch_set_dirichlet(cudaStream_t s, const GridDims& g, const BcDev& bc, double* x);
+// b_work = rhs with Dirichlet values forced.
+void launch_copy_with_dirichlet(cudaStream_t s, const GridDims& g, const BcDev& bc, const double* src, double* dst);
+
+// ---- pointwise PF kernels (pf_pointwise.cu) ------------------------------------------------
+struct SpeciesDev {
+    int K;                              // ions; water is index K
+    int steric;
+    double z[PF_MAX_SPECIES];
+    double cb[PF_MAX_SPECIES];          // bath concentration, 1/A^3
+    double lam[PF_MAX_SPECIES];         // v_k/v_0
+    double lnvc[PF_MAX_SPECIES];        // ln(v_k C_k^B) (unused when v_k = 0)
+    double vol[PF_MAX_SPECIES];
+    double ln_gammaB;
+    double kappa;
+};
+
+// Row N1: Fermi-like distribution at phi per solvent node; writes whichever outputs are non-null:
+// rho, sigma = kappa sum z^2 C, S, conc[(K+1)][N], b1 = PF1 right-hand side (-(kappa rho), 0 on
+// identity rows), a2 = a0 + sigma (PF2 diagonal).
+void launch_diag_plus_sigma(cudaStream_t s, const GridDims& g, const BcDev& bc, const double* a0, const double* sigma,
+                            double* a2);
+void launch_fermi(cudaStream_t s, const GridDims& g, const BcDev& bc, const SpeciesDev& sp, const double* eps, double eps_mid,
+                  bool uniform, const double* phi, double* rho, double* sigma, double* S, double* conc,
+                  double* b1, const double* a0, double* a2);
+// Row N3 right-hand side: b = [solvent](-(eps psi) + sigma phi0) + fixed, Dirichlet values forced.
+void launch_rhs_pf2(cudaStream_t s, const GridDims& g, const BcDev& bc, const double* eps, double eps_mid,
+                    bool uniform, const double* psi, const double* sigma, const double* phi0,
+                    const double* fixed, double* b);
+// Row N5: phi = w phi0 + (1-w) phi; returns max|phi - phi0| through *dmax (device, via ordered-int atomicMax).
+void launch_relax(cudaStream_t s, long long n, double w, const double* phi0, double* phi, unsigned long long* dmax_bits);
+
+}  // namespace pf

@@ -1,0 +1,275 @@
+"""Thin ctypes binding of libpf_b200.so (include/pf.h).  Argument marshalling only: every step of
+the hot path runs in the CUDA kernels behind the C ABI.  torch is used for device memory and streams.
+
+The module-level functions carry the names of the C entry points; `Grid` is a convenience owner of
+the handle and its workspace tensor.  There is no CPU fallback: if the library is missing or no CUDA
+device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpf_b200.so")
+
+PF_OK, PF_NOT_CONVERGED = 0, 1
+PF_ERR_ARG, PF_ERR_CUDA, PF_ERR_BREAKDOWN, PF_ERR_NONPHYSICAL, PF_ERR_WORKSPACE = -1, -2, -3, -4, -5
+PF_BC_DIRICHLET, PF_BC_NEUMANN = 0, 1
+(PF_OPT_STENCIL, PF_OPT_OMEGA_PF, PF_OPT_LINEAR_TOL, PF_OPT_LINEAR_MAXIT, PF_OPT_CHECK_INTERVAL,
+ PF_OPT_WATER_MOLAR, PF_OPT_MAX_OUTER, PF_OPT_PRECOND, PF_OPT_HISTORY, PF_OPT_KERNELS) = range(1, 11)
+STENCIL_AUTO, STENCIL_STORED, STENCIL_ONTHEFLY = 0, 1, 2
+KERNELS_AUTO, KERNELS_DIRECT, KERNELS_TILED = 0, 1, 2
+
+EXPORTS = [
+    "pf_grid_create", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
+    "pf_solve_linear", "pf_solve_linear_host", "pf_solve_pf", "pf_fermi_pointwise", "pf_grid_history",
+    "pf_grid_linear_iters", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_copy_array",
+    "pf_grid_destroy", "pf_last_error", "pf_version",
+]
+
+
+class pf_bc(ctypes.Structure):
+    _fields_ = [("type", ctypes.c_int * 6), ("value", ctypes.c_double * 6)]
+
+
+class pf_charge(ctypes.Structure):
+    _fields_ = [("x", ctypes.c_double), ("y", ctypes.c_double), ("z", ctypes.c_double), ("q", ctypes.c_double)]
+
+
+class PFError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"pf error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+_vp, _dp, _ip = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int)
+
+
+def load():
+    """dlopen the in-tree library; raises if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_1711_04060_b200.build` "
+                           "(there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    L.pf_grid_create.argtypes = [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                                 _vp, ctypes.POINTER(pf_charge), ctypes.c_int, ctypes.POINTER(pf_bc), _vp]
+    L.pf_grid_create.restype = ctypes.c_int
+    L.pf_grid_workspace_bytes.argtypes = [_vp]
+    L.pf_grid_workspace_bytes.restype = ctypes.c_size_t
+    L.pf_grid_set_workspace.argtypes = [_vp, _vp, ctypes.c_size_t]
+    L.pf_grid_set_option.argtypes = [_vp, ctypes.c_int, ctypes.c_double]
+    L.pf_solve_linear.argtypes = [_vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_int, _ip, _dp, _dp]
+    L.pf_solve_linear_host.argtypes = [_vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_int, _ip, _dp, _dp]
+    L.pf_solve_pf.argtypes = [_vp, ctypes.c_int, _dp, _dp, _dp, ctypes.c_double, ctypes.c_double, _vp, _vp, _vp,
+                              _ip, _ip]
+    L.pf_fermi_pointwise.argtypes = [_vp, ctypes.c_int, _dp, _dp, _dp, _vp, _vp, _vp, _vp, _vp]
+    L.pf_grid_history.argtypes = [_vp, _dp, ctypes.c_int]
+    L.pf_grid_linear_iters.argtypes = [_vp, _ip, ctypes.c_int]
+    L.pf_grid_stencil.argtypes = [_vp]
+    L.pf_grid_palette_size.argtypes = [_vp]
+    L.pf_grid_copy_array.argtypes = [_vp, ctypes.c_int, _vp]
+    L.pf_grid_destroy.argtypes = [_vp]
+    L.pf_grid_destroy.restype = None
+    L.pf_last_error.argtypes = [_vp]
+    L.pf_last_error.restype = ctypes.c_char_p
+    L.pf_version.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def _check(handle, rc: int) -> int:
+    if rc < 0:
+        raise PFError(rc, load().pf_last_error(handle).decode())
+    return rc
+
+
+def _dev_ptr(t: Optional[torch.Tensor], n: Optional[int] = None, dtype=torch.float64) -> Optional[int]:
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise ValueError("expected a contiguous CUDA tensor of dtype %s" % dtype)
+    if n is not None and t.numel() != n:
+        raise ValueError(f"expected {n} elements, got {t.numel()}")
+    return t.data_ptr()
+
+
+def _host_doubles(a) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float64).reshape(-1))
+
+
+# ---- functions named after the C entry points ---------------------------------------------------
+
+def pf_version() -> str:
+    return load().pf_version().decode()
+
+
+def pf_grid_create(nx: int, ny: int, nz: int, h: float, eps_map: torch.Tensor, charges, bc_type, bc_value,
+                   stream: Optional[torch.cuda.Stream] = None):
+    """eps_map: CUDA float64 tensor of nx*ny*nz (borrowed); charges: (M,4) host array x,y,z,q."""
+    L = load()
+    ch = np.ascontiguousarray(np.asarray(charges, dtype=np.float64).reshape(-1, 4))
+    bc = pf_bc()
+    for f in range(6):
+        bc.type[f] = int(bc_type[f])
+        bc.value[f] = float(bc_value[f])
+    handle = _vp()
+    s = (stream or torch.cuda.current_stream()).cuda_stream
+    rc = L.pf_grid_create(ctypes.byref(handle), nx, ny, nz, float(h), _dev_ptr(eps_map, nx * ny * nz),
+                          ch.ctypes.data_as(ctypes.POINTER(pf_charge)) if ch.shape[0] else None, int(ch.shape[0]),
+                          ctypes.byref(bc), _vp(s))
+    _check(None, rc)
+    return handle
+
+
+def pf_grid_workspace_bytes(handle) -> int:
+    return int(load().pf_grid_workspace_bytes(handle))
+
+
+def pf_grid_set_workspace(handle, workspace: torch.Tensor) -> None:
+    _check(handle, load().pf_grid_set_workspace(handle, _dev_ptr(workspace, dtype=torch.uint8), workspace.numel()))
+
+
+def pf_grid_set_option(handle, key: int, value: float) -> None:
+    _check(handle, load().pf_grid_set_option(handle, int(key), float(value)))
+
+
+def pf_solve_linear(handle, n: int, rhs: torch.Tensor, x: torch.Tensor, tol: float, maxit: int,
+                    sigma: Optional[torch.Tensor] = None, true_residual: bool = True) -> dict:
+    it, rr, tr = ctypes.c_int(0), ctypes.c_double(0), ctypes.c_double(0)
+    rc = load().pf_solve_linear(handle, _dev_ptr(rhs, n), _dev_ptr(x, n), _dev_ptr(sigma, n), float(tol), int(maxit),
+                                ctypes.byref(it), ctypes.byref(rr), ctypes.byref(tr) if true_residual else None)
+    _check(handle, rc)
+    return dict(status=rc, iters=it.value, relres=rr.value, true_relres=tr.value if true_residual else None)
+
+
+def pf_solve_linear_host(handle, n: int, rhs_host: torch.Tensor, x_host: torch.Tensor, tol: float, maxit: int,
+                         sigma: Optional[torch.Tensor] = None, true_residual: bool = True) -> dict:
+    """rhs_host, x_host: CPU float64 tensors (pinned for speed); copies run inside the call."""
+    for t in (rhs_host, x_host):
+        if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous() or t.numel() != n:
+            raise ValueError("expected contiguous CPU float64 tensors of n elements")
+    it, rr, tr = ctypes.c_int(0), ctypes.c_double(0), ctypes.c_double(0)
+    rc = load().pf_solve_linear_host(handle, rhs_host.data_ptr(), x_host.data_ptr(), _dev_ptr(sigma, n), float(tol),
+                                     int(maxit), ctypes.byref(it), ctypes.byref(rr),
+                                     ctypes.byref(tr) if true_residual else None)
+    _check(handle, rc)
+    return dict(status=rc, iters=it.value, relres=rr.value, true_relres=tr.value if true_residual else None)
+
+
+def pf_solve_pf(handle, n: int, valence, bath_conc, radii, l_c: float, tol: float, phi: torch.Tensor,
+                conc: Optional[torch.Tensor] = None, steric: Optional[torch.Tensor] = None) -> dict:
+    z, cb, a = _host_doubles(valence), _host_doubles(bath_conc), _host_doubles(radii)
+    K = z.size
+    if cb.size != K or a.size != K + 1:
+        raise ValueError("valence/bath_conc need K entries, radii K+1 (water last)")
+    outer, lin = ctypes.c_int(0), ctypes.c_int(0)
+    rc = load().pf_solve_pf(handle, K, z.ctypes.data_as(_dp), cb.ctypes.data_as(_dp), a.ctypes.data_as(_dp),
+                            float(l_c), float(tol), _dev_ptr(phi, n), _dev_ptr(conc, (K + 1) * n),
+                            _dev_ptr(steric, n), ctypes.byref(outer), ctypes.byref(lin))
+    _check(handle, rc)
+    its = (ctypes.c_int * (2 * outer.value + 1))()
+    m = load().pf_grid_linear_iters(handle, its, len(its))
+    return dict(status=rc, outer_iters=outer.value, linear_iters=lin.value, lin_iters_hist=list(its[:m]))
+
+
+def pf_fermi_pointwise(handle, n: int, valence, bath_conc, radii, phi: torch.Tensor,
+                       rho=None, sigma=None, steric=None, conc=None) -> None:
+    z, cb, a = _host_doubles(valence), _host_doubles(bath_conc), _host_doubles(radii)
+    K = z.size
+    rc = load().pf_fermi_pointwise(handle, K, z.ctypes.data_as(_dp), cb.ctypes.data_as(_dp), a.ctypes.data_as(_dp),
+                                   _dev_ptr(phi, n), _dev_ptr(rho, n), _dev_ptr(sigma, n), _dev_ptr(steric, n),
+                                   _dev_ptr(conc, (K + 1) * n))
+    _check(handle, rc)
+
+
+def pf_grid_history(handle, cap: int) -> np.ndarray:
+    buf = np.empty(cap, dtype=np.float64)
+    m = _check(handle, load().pf_grid_history(handle, buf.ctypes.data_as(_dp), cap))
+    return buf[:m]
+
+
+def pf_grid_stencil(handle) -> int:
+    return load().pf_grid_stencil(handle)
+
+
+def pf_grid_palette_size(handle) -> int:
+    return load().pf_grid_palette_size(handle)
+
+
+def pf_grid_copy_array(handle, which: int, n: int) -> torch.Tensor:
+    """Copy of an assembled device array (tests): 0 diag, 1..6 off-diagonals, 7 fixed charges, 8 classes, 9 PF1 diag."""
+    out = torch.empty(n, dtype=torch.uint8 if which == 8 else torch.float64, device="cuda")
+    _check(handle, load().pf_grid_copy_array(handle, which, out.data_ptr()))
+    return out
+
+
+def pf_grid_destroy(handle) -> None:
+    load().pf_grid_destroy(handle)
+
+
+# ---- convenience owner ------------------------------------------------------------------------
+
+class Grid:
+    """Owns a pf_grid handle, the borrowed eps tensor and the torch-allocated workspace."""
+
+    def __init__(self, nx, ny, nz, h, eps, charges, bc_type, bc_value, stencil=STENCIL_AUTO, kernels=KERNELS_AUTO,
+                 options: Optional[dict] = None, stream: Optional[torch.cuda.Stream] = None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: paper_1711_04060_b200 has no CPU fallback")
+        self.nx, self.ny, self.nz, self.h = nx, ny, nz, h
+        self.n = nx * ny * nz
+        self.eps = torch.as_tensor(eps, dtype=torch.float64).reshape(-1).cuda().contiguous()
+        self.handle = pf_grid_create(nx, ny, nz, h, self.eps, charges, bc_type, bc_value, stream)
+        pf_grid_set_option(self.handle, PF_OPT_STENCIL, stencil)
+        if kernels != KERNELS_AUTO:
+            pf_grid_set_option(self.handle, PF_OPT_KERNELS, kernels)
+        for k, v in (options or {}).items():
+            pf_grid_set_option(self.handle, k, v)
+        self.workspace = torch.empty(pf_grid_workspace_bytes(self.handle), dtype=torch.uint8, device="cuda")
+        pf_grid_set_workspace(self.handle, self.workspace)
+
+    @classmethod
+    def from_workload(cls, w, **kw):
+        return cls(w.nx, w.ny, w.nz, w.h, w.eps, w.charges, w.bc_type, w.bc_value, **kw)
+
+    def set_option(self, key, value):
+        pf_grid_set_option(self.handle, key, value)
+
+    def solve_linear(self, rhs, x=None, tol=1e-10, maxit=10000, sigma=None, true_residual=True):
+        rhs = torch.as_tensor(rhs, dtype=torch.float64).reshape(-1).cuda().contiguous()
+        x = torch.zeros(self.n, dtype=torch.float64, device="cuda") if x is None else x
+        out = pf_solve_linear(self.handle, self.n, rhs, x, tol, maxit, sigma, true_residual)
+        out["x"] = x
+        return out
+
+    def solve_pf(self, valence, bath_conc, radii, l_c, tol, want_conc=True):
+        K = len(valence)
+        phi = torch.empty(self.n, dtype=torch.float64, device="cuda")
+        conc = torch.empty((K + 1) * self.n, dtype=torch.float64, device="cuda") if want_conc else None
+        steric = torch.empty(self.n, dtype=torch.float64, device="cuda") if want_conc else None
+        out = pf_solve_pf(self.handle, self.n, valence, bath_conc, radii, l_c, tol, phi, conc, steric)
+        out.update(phi=phi, conc=None if conc is None else conc.view(K + 1, self.n), steric=steric)
+        return out
+
+    def history(self, cap):
+        return pf_grid_history(self.handle, cap)
+
+    def close(self):
+        if self.handle is not None:
+            pf_grid_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

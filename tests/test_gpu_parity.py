@@ -1,0 +1,247 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are BASELINE.json's: linear solves -- relative L2 difference
+of the potential <= 1e-9, true relative residual <= 1e-10, iteration counts within +-2 %; assembly
+and index work bit-exact; full PF -- relative L2 difference of phi and of each C_k <= 1e-7.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from paper_1711_04060_b200 import workloads as wl  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def pf():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_1711_04060_b200 import pf as _pf
+    _pf.load()          # fails loudly if the library has not been built
+    return _pf
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64).reshape(-1)
+    b = np.asarray(b, dtype=np.float64).reshape(-1)
+    d = np.linalg.norm(b)
+    return np.linalg.norm(a - b) / (d if d > 0 else 1.0)
+
+
+def ragged_workload(nx=37, ny=20, nz=11, seed=7, mixed_bc=True):
+    """Small box whose sizes are multiples of nothing, two-valued eps, Neumann + Dirichlet faces."""
+    rng = wl.SplitMix64(seed)
+    eps = wl.sphere_eps(rng, nx, ny, nz, 0.5, fill=0.3, r_lo=1.0, r_hi=2.5)
+    n = nx * ny * nz
+    rhs = np.array([rng.uniform_range(-1.0, 1.0) for _ in range(n)])
+    if mixed_bc:
+        t = np.array([wl.NEUMANN, wl.DIRICHLET, wl.NEUMANN, wl.NEUMANN, wl.DIRICHLET, wl.DIRICHLET], dtype=np.int32)
+        v = np.array([0.0, 0.7, 0.0, 0.0, -0.3, 1.9])
+    else:
+        t = np.zeros(6, dtype=np.int32)
+        v = np.zeros(6)
+    return wl.Workload("ragged", nx, ny, nz, 0.5, eps, np.zeros((0, 4)), t, v, rhs=rhs)
+
+
+# ---- rows L1, L2: assembly, bit-exact -------------------------------------------------------------
+
+@pytest.mark.parametrize("which", ["cfg0", "cfg2_small", "ragged"])
+def test_assembly_bit_exact(pf, oracle, which):
+    w = {"cfg0": lambda: wl.config0(), "cfg2_small": lambda: wl.config2(n=32, volt_mv=50.0),
+         "ragged": lambda: ragged_workload()}[which]()
+    A = oracle.assemble_poisson(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps)
+    fixed = oracle.deposit_charges(w.nx, w.ny, w.nz, w.h, w.charges)
+    g = pf.Grid.from_workload(w, stencil=pf.STENCIL_STORED)
+    assert np.array_equal(pf.pf_grid_copy_array(g.handle, 0, w.n).cpu().numpy(), A[0])
+    for d in range(1, 7):
+        assert np.array_equal(pf.pf_grid_copy_array(g.handle, d, w.n).cpu().numpy(), A[d]), f"A{d}"
+    assert np.array_equal(pf.pf_grid_copy_array(g.handle, 7, w.n).cpu().numpy(), fixed)
+    g.close()
+    g = pf.Grid.from_workload(w, stencil=pf.STENCIL_ONTHEFLY)
+    assert pf.pf_grid_stencil(g.handle) == 2 and pf.pf_grid_palette_size(g.handle) == 2
+    assert np.array_equal(pf.pf_grid_copy_array(g.handle, 0, w.n).cpu().numpy(), A[0])
+    g.close()
+
+
+def test_palette_overflow_falls_back_to_stored(pf, oracle):
+    w = ragged_workload(mixed_bc=False)
+    rng = wl.SplitMix64(11)
+    w.eps = np.array([rng.uniform_range(2.0, 80.0) for _ in range(w.n)])   # every node its own eps
+    g = pf.Grid.from_workload(w)
+    assert pf.pf_grid_stencil(g.handle) == 1 and pf.pf_grid_palette_size(g.handle) > 4
+    ref = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, w.rhs, tol=1e-10)
+    out = g.solve_linear(w.rhs, tol=1e-10)
+    assert out["status"] == 0 and abs(out["iters"] - ref["iters"]) <= max(1, 0.02 * ref["iters"])
+    assert rel_l2(out["x"].cpu().numpy(), ref["x"]) <= 1e-9
+    g.close()
+
+
+# ---- rows L3-L8: linear solves ------------------------------------------------------------------------
+
+def _linear_case(pf, oracle, w, stencil, kernels=0, precond=True, sigma=None, tol=1e-10, x0=None, maxit=10000):
+    ref = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, w.rhs, x0=x0, sigma=sigma, tol=tol,
+                              maxit=maxit, precond=precond, history=True)
+    g = pf.Grid.from_workload(w, stencil=stencil, kernels=kernels,
+                              options={pf.PF_OPT_PRECOND: 1 if precond else 0, pf.PF_OPT_HISTORY: maxit + 1})
+    x = torch.zeros(w.n, dtype=torch.float64, device="cuda") if x0 is None else torch.tensor(x0, device="cuda")
+    sg = None if sigma is None else torch.tensor(sigma, device="cuda")
+    out = g.solve_linear(w.rhs, x=x, tol=tol, maxit=maxit, sigma=sg)
+    hist = g.history(maxit + 1)
+    g.close()
+    return ref, out, hist
+
+
+@pytest.mark.parametrize("stencil", [1, 2])
+def test_linear_config1_64(pf, oracle, stencil):
+    """BASELINE configs[1]: 64^3, random-sphere eps 2/80, 500 Gaussian charges, tol 1e-10."""
+    w = wl.config1()
+    ref, out, hist = _linear_case(pf, oracle, w, stencil)
+    assert ref["status"] == 0 and out["status"] == 0
+    assert abs(out["iters"] - ref["iters"]) <= 0.02 * ref["iters"], (out["iters"], ref["iters"])
+    assert out["true_relres"] <= 1e-10 * 1.0000001 or out["true_relres"] <= 1.05e-10
+    assert rel_l2(out["x"].cpu().numpy(), ref["x"]) <= 1e-9
+    # the residual histories track each other while both run
+    m = min(len(hist), len(ref["hist"]))
+    assert m > 10 and np.allclose(hist[: m // 2], ref["hist"][: m // 2], rtol=1e-6)
+
+
+@pytest.mark.parametrize("stencil", [1, 2])
+@pytest.mark.parametrize("precond", [True, False])
+def test_linear_ragged_mixed_bc(pf, oracle, stencil, precond):
+    w = ragged_workload()
+    ref, out, _ = _linear_case(pf, oracle, w, stencil, precond=precond)
+    assert ref["status"] == 0 and out["status"] == 0
+    assert abs(out["iters"] - ref["iters"]) <= max(1, 0.02 * ref["iters"])
+    assert out["true_relres"] <= 1.05e-10
+    assert rel_l2(out["x"].cpu().numpy(), ref["x"]) <= 1e-9
+
+
+def test_linear_with_sigma_and_warm_start(pf, oracle):
+    w = ragged_workload()
+    rng = wl.SplitMix64(3)
+    sigma = np.array([rng.uniform_range(0.0, 5.0) for _ in range(w.n)])
+    x0 = np.array([rng.uniform_range(-1.0, 1.0) for _ in range(w.n)])
+    ref, out, _ = _linear_case(pf, oracle, w, 2, sigma=sigma, x0=x0)
+    assert ref["status"] == 0 and out["status"] == 0
+    assert abs(out["iters"] - ref["iters"]) <= max(1, 0.02 * ref["iters"])
+    assert rel_l2(out["x"].cpu().numpy(), ref["x"]) <= 1e-9
+
+
+def test_linear_fixed_iterations_match_iterate(pf, oracle):
+    """tol = 0: exactly maxit iterations on both sides; the iterates themselves agree."""
+    w = wl.config1(n=32, ncharges=50)
+    ref, out, hist = _linear_case(pf, oracle, w, 2, tol=0.0, maxit=20)
+    assert ref["status"] == 1 and out["status"] == 1 and out["iters"] == 20 == ref["iters"]
+    assert rel_l2(out["x"].cpu().numpy(), ref["x"]) <= 1e-12
+    assert np.allclose(hist, ref["hist"], rtol=1e-10)
+
+
+def test_linear_degenerate_cases(pf, oracle):
+    w = ragged_workload(mixed_bc=False)
+    g = pf.Grid.from_workload(w)
+    # b = 0 with zero Dirichlet data: x = 0 after 0 iterations (Q3)
+    x = torch.ones(w.n, dtype=torch.float64, device="cuda")
+    out = g.solve_linear(np.zeros(w.n), x=x)
+    assert out["status"] == 0 and out["iters"] == 0 and float(x.abs().max()) == 0.0
+    # maxit = 0: not converged, x = x0 with Dirichlet values forced
+    x = torch.full((w.n,), 0.5, dtype=torch.float64, device="cuda")
+    out = g.solve_linear(w.rhs, x=x, maxit=0)
+    assert out["status"] == 1 and out["iters"] == 0
+    ref = oracle.set_dirichlet(w.nx, w.ny, w.nz, w.bc_type, w.bc_value, np.full(w.n, 0.5))
+    assert np.array_equal(x.cpu().numpy(), ref)
+    # warm start at the solution: converged before the first iteration
+    sol = g.solve_linear(w.rhs, tol=1e-12)["x"]
+    out = g.solve_linear(w.rhs, x=sol.clone(), tol=1e-8)
+    assert out["status"] == 0 and out["iters"] == 0
+    g.close()
+
+
+def test_linear_host_buffers(pf, oracle):
+    w = ragged_workload()
+    ref = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, w.rhs, tol=1e-10)
+    g = pf.Grid.from_workload(w)
+    rhs_h = torch.tensor(w.rhs).pin_memory()
+    x_h = torch.zeros(w.n, dtype=torch.float64).pin_memory()
+    out = pf.pf_solve_linear_host(g.handle, w.n, rhs_h, x_h, 1e-10, 10000)
+    g.close()
+    assert out["status"] == 0 and rel_l2(x_h.numpy(), ref["x"]) <= 1e-9
+
+
+# ---- row N1: pointwise Fermi kernel --------------------------------------------------------------
+
+@pytest.mark.parametrize("species", ["nacl", "nacacl", "nosteric"])
+def test_fermi_pointwise(pf, oracle, species):
+    w = wl.config0()
+    sp = {"nacl": wl.NACL, "nacacl": wl.NACACL, "nosteric": wl.NACL}[species]
+    radii = np.zeros_like(sp.radii) if species == "nosteric" else sp.radii
+    rng = wl.SplitMix64(5)
+    phi = np.array([rng.uniform_range(-12.0, 12.0) for _ in range(w.n)])
+    phi[:8] = [0.0, 50.0, -50.0, 500.0, -500.0, 1e-9, 20.0, -20.0]
+    solvent = oracle.solvent_mask(w.eps)
+    ref = oracle.fermi_pointwise(sp.valence, sp.bath_molar, radii, phi, solvent)
+    g = pf.Grid.from_workload(w)
+    K = len(sp.valence)
+    dev = lambda m: torch.empty(m, dtype=torch.float64, device="cuda")
+    rho, sigma, S, conc = dev(w.n), dev(w.n), dev(w.n), dev((K + 1) * w.n)
+    pf.pf_fermi_pointwise(g.handle, w.n, sp.valence, sp.bath_molar, radii, torch.tensor(phi, device="cuda"),
+                          rho, sigma, S, conc)
+    g.close()
+    assert np.allclose(S.cpu().numpy(), ref["S"], rtol=1e-11, atol=1e-13)
+    assert np.allclose(conc.cpu().numpy().reshape(K + 1, -1), ref["conc"], rtol=1e-10, atol=0)
+    assert np.allclose(rho.cpu().numpy(), ref["rho"], rtol=1e-9, atol=1e-18)
+    assert np.allclose(sigma.cpu().numpy(), ref["sigma"], rtol=1e-10, atol=0)
+    assert np.all(conc.cpu().numpy().reshape(K + 1, -1)[:, solvent == 0] == 0.0)
+
+
+# ---- rows N1-N5: the full nonlinear solve ----------------------------------------------------------
+
+def _pf_case(pf, oracle, w, stencil=0):
+    sp = w.species
+    ref = oracle.solve_pf(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, w.charges, sp.valence,
+                          sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol, lin_tol=w.linear_tol)
+    g = pf.Grid.from_workload(w, stencil=stencil)
+    out = g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol)
+    g.close()
+    return ref, out
+
+
+@pytest.mark.parametrize("stencil", [1, 2])
+def test_pf_config0_32(pf, oracle, stencil):
+    """BASELINE configs[0]: 32^3 PF with Na+/Cl-/water, l_c = 1.2, linear 1e-10, nonlinear 1e-8."""
+    w = wl.config0()
+    ref, out = _pf_case(pf, oracle, w, stencil)
+    assert ref["status"] == 0 and out["status"] == 0
+    assert out["outer_iters"] == ref["outer_iters"]
+    assert abs(out["linear_iters"] - ref["linear_iters"]) <= 0.02 * ref["linear_iters"], \
+        (out["linear_iters"], ref["linear_iters"])
+    assert rel_l2(out["phi"].cpu().numpy(), ref["phi"]) <= 1e-7
+    conc = out["conc"].cpu().numpy()
+    for k in range(conc.shape[0]):
+        assert rel_l2(conc[k], ref["conc"][k]) <= 1e-7, k
+    assert np.allclose(out["steric"].cpu().numpy(), ref["steric"], rtol=1e-6, atol=1e-9)
+
+
+def test_pf_channel_neumann_small(pf, oracle):
+    """configs[2]'s geometry and species (Na+, Ca2+, Cl-, +50 mV, lateral Neumann) at 32^3."""
+    w = wl.config2(n=32, volt_mv=50.0)
+    ref, out = _pf_case(pf, oracle, w)
+    assert ref["status"] == 0 and out["status"] == 0
+    assert out["outer_iters"] == ref["outer_iters"]
+    assert abs(out["linear_iters"] - ref["linear_iters"]) <= 0.02 * ref["linear_iters"]
+    assert rel_l2(out["phi"].cpu().numpy(), ref["phi"]) <= 1e-7
+    conc = out["conc"].cpu().numpy()
+    for k in range(conc.shape[0]):
+        assert rel_l2(conc[k], ref["conc"][k]) <= 1e-7, k
+
+
+def test_pf_errors(pf):
+    w = wl.config0(n=16)
+    g = pf.Grid.from_workload(w)
+    with pytest.raises(pf.PFError) as e:
+        g.solve_pf([1.0, -1.0], [0.1, 0.2], [0.95, 1.81, 1.4], 1.2, 1e-8)     # not neutral
+    assert e.value.code == pf.PF_ERR_NONPHYSICAL
+    with pytest.raises(pf.PFError) as e:
+        g.solve_pf([1.0, -1.0], [0.1, 0.1], [9.0, 9.0, 9.0], 1.2, 1e-8)       # Gamma^B <= 0
+    assert e.value.code == pf.PF_ERR_NONPHYSICAL
+    g.close()
