@@ -1,0 +1,348 @@
+#!/usr/bin/env python
+"""bench.py -- BiCGSTAB iterations/s of the Poisson-Fermi hot path on BASELINE.json configs[3]
+(256^3 fp64 channel grid), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--n 256] [--stencil onthefly|stored]
+    python bench.py --impl reference ...      # the CPU oracle on the host cores (bounded sample)
+
+One STEP = one pass of the whole hot path:
+  rows L1-L2  pf_grid_create + pf_grid_set_workspace: eps scan, node classes, diagonal, (stored
+              off-diagonals), fixed-charge deposition
+  rows L3-L8  pf_solve_linear, tol = 0, 200 fixed Jacobi-BiCGSTAB iterations (configs[3] (ii))
+  rows N1-N5  pf_solve_pf capped at one outer iteration with 25 fixed iterations per linear solve:
+              initial guess, fused Fermi kernel, PF1, PF2, relaxation + max-norm (3 x 25 iterations)
+value = BiCGSTAB iterations of the step (275) / step time, whole job.  Inputs are resident in HBM
+for `value`; `e2e` repeats the step through the C ABI with HOST buffers (copies inside the timing).
+Multi-GPU: the path does not shard (replicas only) -- every rank runs the same step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+LINEAR_ITERS = 200
+PF_INNER_ITERS = 25
+STEP_ITERS = LINEAR_ITERS + 3 * PF_INNER_ITERS
+METRIC = "bicgstab_iterations_per_s"
+UNIT = "iterations/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--n", type=int, default=256, help="grid nodes per direction (configs[3] = 256)")
+    ap.add_argument("--stencil", choices=["onthefly", "stored"], default="onthefly")
+    ap.add_argument("--kernels", choices=["auto", "direct", "tiled"], default="auto")
+    ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--ref-iters", type=int, default=4, help="oracle iterations per reference step")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.lines:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peak_gbs():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def kernel_bytes_per_unknown(stored: bool) -> dict:
+    """Algorithmic HBM bytes per unknown per launch: every input vector
+    read once, every output written once, halos served on chip."""
+    if stored:
+        return {"k1": (5 + 6 + 2) * 8, "k2": (3 + 6 + 1) * 8, "k3": (7 + 2) * 8}
+    return {"k1": (5 + 2) * 8 + 1, "k2": (3 + 1) * 8 + 1, "k3": (7 + 2) * 8}
+
+
+# ---------------------------------------------------------------------------------------------------
+# reference arm: the oracle on the host cores
+# ---------------------------------------------------------------------------------------------------
+
+def oracle_sample(w, iters: int):
+    """Assembly + `iters` fixed Jacobi-BiCGSTAB iterations of the workload in the CPU oracle; seconds."""
+    from oracle import pf_oracle as oracle
+    import numpy as np
+    rhs = oracle.deposit_charges(w.nx, w.ny, w.nz, w.h, w.charges) if w.rhs is None else w.rhs
+    t0 = time.perf_counter()
+    out = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, rhs, tol=0.0, maxit=iters)
+    dt = time.perf_counter() - t0
+    assert out["iters"] == iters and np.isfinite(out["relres"])
+    return dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1711_04060_b200 import workloads as wl
+    from oracle import pf_oracle as oracle
+    oracle.build()
+    w = wl.config3(n=args.n)
+    for _ in range(args.warmup):
+        oracle_sample(w, 1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_sample(w, args.ref_iters)
+    dt = time.perf_counter() - t0
+    value = args.steps * args.ref_iters / dt
+    sample = (f"per step: DIA assembly + {args.ref_iters} fixed Jacobi-BiCGSTAB iterations of the {args.n}^3 "
+              f"configs[3] workload, single thread, g++ -O2")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"configs[3] channel {args.n}^3 fp64, h=0.5 A, seed 3", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------------
+# B200 arm
+# ---------------------------------------------------------------------------------------------------
+
+def run_b200(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1711_04060_b200 import pf, workloads as wl
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the library has no CPU fallback")
+    pf.load()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    w = wl.config3(n=args.n)
+    sp = w.species
+    n = w.n
+    stencil = pf.STENCIL_STORED if args.stencil == "stored" else pf.STENCIL_ONTHEFLY
+    kernels = {"auto": 0, "direct": 1, "tiled": 2}[args.kernels]
+    rng = np.random.default_rng(3)
+    rhs_np = rng.standard_normal(n)                      # configs[3]: timing RHS, dense random
+    eps_host = torch.tensor(w.eps).pin_memory()
+    rhs_host = torch.tensor(rhs_np).pin_memory()
+    x_host = torch.zeros(n, dtype=torch.float64).pin_memory()
+    phi_host = torch.zeros(n, dtype=torch.float64).pin_memory()
+    eps_dev = eps_host.cuda()
+    rhs_dev = rhs_host.cuda()
+    x_dev = torch.zeros(n, dtype=torch.float64, device="cuda")
+    phi_dev = torch.zeros(n, dtype=torch.float64, device="cuda")
+
+    # workspace is allocated once, outside the timing: it is caller-owned scratch by the ABI
+    probe = pf.pf_grid_create(w.nx, w.ny, w.nz, w.h, eps_dev, w.charges, w.bc_type, w.bc_value)
+    pf.pf_grid_set_option(probe, pf.PF_OPT_STENCIL, stencil)
+    ws = torch.empty(pf.pf_grid_workspace_bytes(probe), dtype=torch.uint8, device="cuda")
+    pf.pf_grid_destroy(probe)
+    prof_tot = {k: dict(ms=0.0, launches=0) for k in ("k1", "k2", "k3")}
+
+    def step(host_buffers: bool, profile: bool):
+        if host_buffers:
+            eps_dev.copy_(eps_host, non_blocking=True)
+        h = pf.pf_grid_create(w.nx, w.ny, w.nz, w.h, eps_dev, w.charges, w.bc_type, w.bc_value)
+        pf.pf_grid_set_option(h, pf.PF_OPT_STENCIL, stencil)
+        if kernels:
+            pf.pf_grid_set_option(h, pf.PF_OPT_KERNELS, kernels)
+        pf.pf_grid_set_option(h, pf.PF_OPT_LINEAR_TOL, 0.0)
+        pf.pf_grid_set_option(h, pf.PF_OPT_LINEAR_MAXIT, PF_INNER_ITERS)
+        pf.pf_grid_set_option(h, pf.PF_OPT_MAX_OUTER, 1)
+        if profile:
+            pf.pf_grid_set_option(h, pf.PF_OPT_PROFILE, LINEAR_ITERS)
+        pf.pf_grid_set_workspace(h, ws)                                            # rows L1, L2
+        if host_buffers:
+            x_host.zero_()
+            out = pf.pf_solve_linear_host(h, n, rhs_host, x_host, 0.0, LINEAR_ITERS, true_residual=False)
+        else:
+            x_dev.zero_()
+            out = pf.pf_solve_linear(h, n, rhs_dev, x_dev, 0.0, LINEAR_ITERS, true_residual=False)   # rows L3-L8
+        assert out["iters"] == LINEAR_ITERS, out
+        res = pf.pf_solve_pf(h, n, sp.valence, sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol, phi_dev)  # N1-N5
+        assert res["linear_iters"] == 3 * PF_INNER_ITERS, res
+        if host_buffers:
+            phi_host.copy_(phi_dev, non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+        if profile:
+            p = pf.pf_grid_profile(h)
+            for k in prof_tot:
+                prof_tot[k]["ms"] += p[k]["ms"]
+                prof_tot[k]["launches"] += p[k]["launches"]
+        pf.pf_grid_destroy(h)
+        return out
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(nsteps, host_buffers, profile):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for _ in range(nsteps):
+            step(host_buffers, profile)
+        e1.record()
+        barrier()
+        ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        return float(ms.item())
+
+    for _ in range(max(args.warmup, 3)):
+        step(False, False)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = pf.pf_launch_count()
+    ms_total = timed(args.steps, False, True)
+    launches = pf.pf_launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+
+    e2e = None
+    if not args.no_e2e:
+        step(True, False)
+        e2e_steps = max(1, min(args.steps, 3))
+        ms_e2e = timed(e2e_steps, True, False)
+        e2e = {"value": world * STEP_ITERS * e2e_steps / (ms_e2e * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": 8 * n * 3, "d2h_bytes_per_step": 8 * n * 2,
+               "ms_per_step": ms_e2e / e2e_steps,
+               "what": "eps, rhs, x0 host->device; x, phi device->host; C-ABI pf_solve_linear_host"}
+
+    if rank == 0:
+        peak, peak_src = measured_peak_gbs()
+        stored = args.stencil == "stored"
+        bpu = kernel_bytes_per_unknown(stored)
+        kernels_rep = {}
+        for k in ("k1", "k2", "k3"):
+            if prof_tot[k]["launches"]:
+                avg_ms = prof_tot[k]["ms"] / prof_tot[k]["launches"]
+                gbs = bpu[k] * n / (avg_ms * 1e-3) / 1e9
+                kernels_rep[k] = {"avg_ms": avg_ms, "launches": prof_tot[k]["launches"],
+                                  "bytes_per_unknown": bpu[k], "gbs": gbs, "frac": gbs / peak}
+        dom = max(kernels_rep, key=lambda k: kernels_rep[k]["avg_ms"] * kernels_rep[k]["launches"])
+        iter_ms = sum(kernels_rep[k]["avg_ms"] for k in kernels_rep)
+        iter_bytes = sum(bpu.values()) * n
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tpath):
+            try:
+                with open(tpath) as f:
+                    traffic = json.load(f).get(f"{args.stencil}_{args.n}", {}).get(dom)
+            except Exception:
+                traffic = None
+        roofline = {"bound": "hbm", "kernel": {"k1": "k1 (p-update + matvec + r~.v)", "k2": "k2 (s-update + matvec + t.s,t.t)",
+                                                "k3": "k3 (x,r update + r~.r, r.r)"}[dom],
+                    "achieved": kernels_rep[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                    "frac": kernels_rep[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
+                    "per_kernel": kernels_rep,
+                    "iteration": {"ms": iter_ms, "bytes_per_unknown": sum(bpu.values()),
+                                  "gbs": iter_bytes / (iter_ms * 1e-3) / 1e9,
+                                  "frac": iter_bytes / (iter_ms * 1e-3) / 1e9 / peak,
+                                  "iterations_per_s_linear_solve": 1e3 / iter_ms,
+                                  "mupdates_per_s": n / iter_ms / 1e3}}
+        cpu = None
+        if not args.no_cpu_baseline and world == 1:
+            from oracle import pf_oracle as oracle
+            oracle.build()
+            cpu_iters = 12 if args.n >= 256 else 100
+            dt = oracle_sample(w, cpu_iters)
+            cpu = {"value": cpu_iters / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                   "host_cores_available": os.cpu_count(),
+                   "sample": f"DIA assembly + {cpu_iters} fixed Jacobi-BiCGSTAB iterations of the same {args.n}^3 "
+                             f"workload ({dt:.1f} s), single thread, g++ -O2"}
+        value = world * STEP_ITERS * args.steps / (ms_total * 1e-3)
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"configs[3] channel {args.n}^3 fp64 (slab 60 A, pore 8 A, 1536 charges, seed 3), "
+                                       f"h=0.5 A; step = assembly + {LINEAR_ITERS} fixed Jacobi-BiCGSTAB iterations + "
+                                       f"one PF outer pass with 3x{PF_INNER_ITERS} inner iterations",
+                           "stencil": args.stencil, "kernels": args.kernels, "unknowns": n,
+                           "iterations_per_step": STEP_ITERS, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                           "l2": "inputs larger than L2 (working set %.1f GB)" % (ws.numel() / 1e9)},
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+                "paper_context": "paper: 22.8x linear-solver, 16.9x total speedup, GTX TITAN X vs Xeon E5-1650 "
+                                 "(PAPER.md:305-311); other hardware, context only"}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -69,6 +69,10 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
 #define PF_OPT_KERNELS        10  /* 0 = auto, 1 = direct (one thread per node, neighbours through L1/L2),
                                      2 = tiled (shared-memory planes, z-marched).  Same arithmetic. */
 
+#define PF_OPT_PROFILE        11  /* n > 0: bracket the three kernels of the first n iterations of every
+                                     linear solve with CUDA events and accumulate their durations
+                                     (pf_grid_profile); setting it resets the sums; 0 = off */
+
 /* Create a grid: store geometry and boundary conditions, scan eps_map for its palette of distinct
  * values, keep a device copy of the charges.  Assembly itself runs in pf_grid_set_workspace.
  *   eps_map : device, nx*ny*nz doubles, relative permittivity per node; borrowed.
@@ -134,6 +138,14 @@ int pf_grid_history(pf_grid *g, double *hist_host, int cap);
 
 /* Per-solve iteration counts of the last pf_solve_pf in call order (initial guess, PF1, PF2, ...). */
 int pf_grid_linear_iters(pf_grid *g, int *iters_host, int cap);
+
+/* Accumulated device time (ms) and launch count of the three per-iteration kernels since
+ * PF_OPT_PROFILE was set: index 0 = p-update + matvec + r~.v (row L4), 1 = s-update + matvec + t.s,
+ * t.t (row L5), 2 = x, r update + r~.r, r.r (row L6).  ms_out, launches_out: host, 3 entries. */
+int pf_grid_profile(pf_grid *g, double *ms_out, long long *launches_out);
+
+/* Kernel launches issued by the library in this process so far. */
+long long pf_launch_count(void);
 
 /* Introspection used by the tests: 1 = stored, 2 = on-the-fly; number of palette entries. */
 int pf_grid_stencil(const pf_grid *g);

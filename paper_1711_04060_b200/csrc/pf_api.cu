@@ -13,6 +13,8 @@
 
 using namespace pf;
 
+long long pf::g_launch_count = 0;
+
 namespace {
 
 // Table 1, reading R0: kappa = e^2/(eps_0 k_B T) in Angstrom, phi in k_B T/e.
@@ -70,6 +72,11 @@ struct pf_grid {
     double* offd[6];
     double* offd_pf1[6];
     std::vector<int> lin_iters;
+    // per-kernel timing (PF_OPT_PROFILE): events around k1, k2, k3 of every iteration
+    std::vector<cudaEvent_t> prof_ev;
+    double prof_ms[3];
+    long long prof_launches[3];
+    int opt_profile;
     int last_iters;
     std::string err;
 };
@@ -156,9 +163,15 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     while (!done) {
         const int todo = std::min(chunk, maxit - launched);
         for (int k = 0; k < todo; ++k) {
-            if (tiled) { launch_k1_tiled(c, op, kv, precond); launch_k2_tiled(c, op, kv, precond); }
-            else       { launch_k1_direct(c, op, kv, precond); launch_k2_direct(c, op, kv, precond); }
+            const bool prof = g->opt_profile && (size_t)(4 * (launched + k) + 3) < g->prof_ev.size();
+            cudaEvent_t* pe = prof ? &g->prof_ev[4 * (launched + k)] : nullptr;
+            if (prof) cudaEventRecord(pe[0], g->stream);
+            if (tiled) launch_k1_tiled(c, op, kv, precond); else launch_k1_direct(c, op, kv, precond);
+            if (prof) cudaEventRecord(pe[1], g->stream);
+            if (tiled) launch_k2_tiled(c, op, kv, precond); else launch_k2_direct(c, op, kv, precond);
+            if (prof) cudaEventRecord(pe[2], g->stream);
             launch_k3(c, op, kv, precond);
+            if (prof) cudaEventRecord(pe[3], g->stream);
             std::swap(kv.p_in, kv.p_out);     // k1 read (p_in, v_in) and wrote (p_out, v_out)
             std::swap(kv.v_in, kv.v_out);
         }
@@ -181,6 +194,16 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
         slot ^= 1;
     }
     PF_CUDA(g, cudaStreamSynchronize(g->stream));
+    if (g->opt_profile) {       // only iterations that ran (kernels after convergence return at once)
+        const int nprof = std::min<int>(fin.it, (int)g->prof_ev.size() / 4);
+        for (int k = 0; k < nprof; ++k)
+            for (int j = 0; j < 3; ++j) {
+                float ms = 0.f;
+                if (cudaEventElapsedTime(&ms, g->prof_ev[4 * k + j], g->prof_ev[4 * k + j + 1]) == cudaSuccess) {
+                    g->prof_ms[j] += ms; g->prof_launches[j] += 1;
+                }
+            }
+    }
     if (!fin.done) { fin.status = PF_NOT_CONVERGED; }
     if (fin.bb == 0.0) PF_CUDA(g, cudaMemsetAsync(x, 0, sizeof(double) * g->g.n, g->stream));   // Q3
     double true_rel = 0.0;
@@ -276,6 +299,8 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->opt_omega_pf = 0.3; g->opt_lin_tol = 1e-10; g->opt_water = 55.5;
     g->ws = nullptr; g->ws_bytes = 0; g->assembled = false; g->stored = false;
     g->pf1_lc = std::nan("");
+    g->opt_profile = 0; g->prof_ms[0] = g->prof_ms[1] = g->prof_ms[2] = 0.0;
+    g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0;
     g->charges_dev = nullptr; g->sc = nullptr; g->rb.partial = nullptr; g->rb.ticket = nullptr;
     g->lut_poisson = g->lut_pf1 = nullptr; g->dmax_bits = nullptr;
@@ -330,6 +355,7 @@ void pf_grid_destroy(pf_grid* g) {
     if (g->sc_host[1]) cudaFreeHost(g->sc_host[1]);
     if (g->ev[0]) cudaEventDestroy(g->ev[0]);
     if (g->ev[1]) cudaEventDestroy(g->ev[1]);
+    for (cudaEvent_t e : g->prof_ev) cudaEventDestroy(e);
     cudaGetLastError();
     delete g;
 }
@@ -382,6 +408,20 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
                 g->hist_cap = iv;
             }
             g->opt_history = iv;
+            return PF_OK;
+        }
+        case PF_OPT_PROFILE: {
+            if (iv < 0 || iv > 100000) return fail(g, PF_ERR_ARG, "profile: iterations to time must be in 0..100000");
+            cudaStreamSynchronize(g->stream);
+            for (cudaEvent_t e : g->prof_ev) cudaEventDestroy(e);
+            g->prof_ev.clear();
+            for (int k = 0; k < 4 * iv; ++k) {
+                cudaEvent_t e;
+                PF_CUDA(g, cudaEventCreate(&e));
+                g->prof_ev.push_back(e);
+            }
+            g->opt_profile = iv;
+            for (int j = 0; j < 3; ++j) { g->prof_ms[j] = 0.0; g->prof_launches[j] = 0; }
             return PF_OK;
         }
         case PF_OPT_KERNELS:
@@ -560,6 +600,14 @@ int pf_grid_linear_iters(pf_grid* g, int* iters_host, int cap) {
     const int n = std::min<int>(cap, (int)g->lin_iters.size());
     for (int k = 0; k < n; ++k) iters_host[k] = g->lin_iters[k];
     return n;
+}
+
+long long pf_launch_count(void) { return pf::g_launch_count; }
+
+int pf_grid_profile(pf_grid* g, double* ms_out, long long* launches_out) {
+    if (!g || !ms_out || !launches_out) return PF_ERR_ARG;
+    for (int j = 0; j < 3; ++j) { ms_out[j] = g->prof_ms[j]; launches_out[j] = g->prof_launches[j]; }
+    return PF_OK;
 }
 
 int pf_grid_stencil(const pf_grid* g) { return g ? (want_stored(g) ? 1 : 2) : PF_ERR_ARG; }

@@ -200,6 +200,7 @@ cudaError_t scan_eps(cudaStream_t s, long long n, const double* eps, void* scrat
     init.min_bits = ~0ull;
     cudaError_t e = cudaMemcpyAsync(scratch, &init, sizeof(init), cudaMemcpyHostToDevice, s);
     if (e != cudaSuccess) return e;
+    ++g_launch_count;
     k_scan_eps<<<asm_blocks(n), ASM_THREADS, 0, s>>>(n, eps, (ScanBuf*)scratch);
     ScanBuf res;
     e = cudaMemcpyAsync(&res, scratch, sizeof(res), cudaMemcpyDeviceToHost, s);
@@ -220,6 +221,7 @@ cudaError_t scan_eps(cudaStream_t s, long long n, const double* eps, void* scrat
 
 void launch_assemble_poisson(cudaStream_t s, const GridDims& g, double h, const BcDev& bc, const double* eps,
                              const Palette& pal, bool use_palette, double* A0, uint8_t* cls, double* const offd[6]) {
+    ++g_launch_count;
     k_assemble_poisson<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, h, bc, eps, pal, use_palette, A0, cls, offd[0],
                                                                 offd[1], offd[2], offd[3], offd[4], offd[5]);
 }
@@ -227,6 +229,7 @@ void launch_assemble_poisson(cudaStream_t s, const GridDims& g, double h, const 
 void launch_assemble_pf1(cudaStream_t s, const GridDims& g, double h, double lc, const double* eps, double eps_mid,
                          bool uniform, const Palette& pal, bool use_palette, double* A0, uint8_t* cls,
                          double* const offd[6]) {
+    ++g_launch_count;
     k_assemble_pf1<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, h, lc, eps, eps_mid, uniform, pal, use_palette, A0, cls,
                                                             offd[0], offd[1], offd[2], offd[3], offd[4], offd[5]);
 }
@@ -263,14 +266,16 @@ void build_lut_pf1(const Palette& pal, double h, double lc, double* lut, int* nc
 void launch_deposit(cudaStream_t s, const GridDims& g, double h, double kappa, const double* charges_dev, int m,
                     double* fixed) {
     cudaMemsetAsync(fixed, 0, sizeof(double) * g.n, s);
-    if (m > 0) k_deposit<<<1, 32, 0, s>>>(g, h, kappa, charges_dev, m, fixed);
+    if (m > 0) { ++g_launch_count; k_deposit<<<1, 32, 0, s>>>(g, h, kappa, charges_dev, m, fixed); }
 }
 
 void launch_set_dirichlet(cudaStream_t s, const GridDims& g, const BcDev& bc, double* x) {
+    ++g_launch_count;
     k_set_dirichlet<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, bc, x, x);
 }
 
 void launch_copy_with_dirichlet(cudaStream_t s, const GridDims& g, const BcDev& bc, const double* src, double* dst) {
+    ++g_launch_count;
     k_set_dirichlet<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, bc, src, dst);
 }
 

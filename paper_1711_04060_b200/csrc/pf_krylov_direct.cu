@@ -187,26 +187,26 @@ static int direct_blocks(long long n, int sm_count) {
 
 void launch_residual_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, int mode) {
     const int nb = direct_blocks(c.g.n, c.sm_count);
-    if (mode == 0) k_residual<0><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb);
-    else           k_residual<1><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb);
+    if (mode == 0) { ++g_launch_count; k_residual<0><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb); }
+    else           { ++g_launch_count; k_residual<1><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb); }
 }
 
 void launch_k1_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond) {
     const int nb = direct_blocks(c.g.n, c.sm_count);
-    if (precond) k1_direct<true><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb);
-    else         k1_direct<false><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb);
+    if (precond) { ++g_launch_count; k1_direct<true><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb); }
+    else         { ++g_launch_count; k1_direct<false><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb); }
 }
 
 void launch_k2_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond) {
     const int nb = direct_blocks(c.g.n, c.sm_count);
-    if (precond) k2_direct<true><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb);
-    else         k2_direct<false><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb);
+    if (precond) { ++g_launch_count; k2_direct<true><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb); }
+    else         { ++g_launch_count; k2_direct<false><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb); }
 }
 
 void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond) {
     const int nb = direct_blocks(c.g.n, c.sm_count);
-    if (precond) k3_update<true><<<nb, 256, 0, c.stream>>>(c.g.n, op.A0, kv, c.sc, c.rb);
-    else         k3_update<false><<<nb, 256, 0, c.stream>>>(c.g.n, op.A0, kv, c.sc, c.rb);
+    if (precond) { ++g_launch_count; k3_update<true><<<nb, 256, 0, c.stream>>>(c.g.n, op.A0, kv, c.sc, c.rb); }
+    else         { ++g_launch_count; k3_update<false><<<nb, 256, 0, c.stream>>>(c.g.n, op.A0, kv, c.sc, c.rb); }
 }
 
 }  // namespace pf

@@ -6,6 +6,9 @@
 
 namespace pf {
 
+// Kernel launches issued by this library since load (bench.py reports the difference over the timed region).
+extern long long g_launch_count;
+
 struct LaunchCtx {
     cudaStream_t stream;
     GridDims g;

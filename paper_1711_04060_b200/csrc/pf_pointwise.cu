@@ -153,24 +153,28 @@ k_diag_plus_sigma(GridDims g, BcDev bc, const double* __restrict__ a0, const dou
 
 void launch_diag_plus_sigma(cudaStream_t s, const GridDims& g, const BcDev& bc, const double* a0, const double* sigma,
                             double* a2) {
+    ++g_launch_count;
     k_diag_plus_sigma<<<pw_blocks(g.n), PW_THREADS, 0, s>>>(g, bc, a0, sigma, a2);
 }
 
 void launch_fermi(cudaStream_t s, const GridDims& g, const BcDev& bc, const SpeciesDev& sp, const double* eps, double eps_mid,
                   bool uniform, const double* phi, double* rho, double* sigma, double* S, double* conc, double* b1,
                   const double* a0, double* a2) {
+    ++g_launch_count;
     k_fermi<<<pw_blocks(g.n), PW_THREADS, 0, s>>>(g, bc, sp, eps, eps_mid, uniform, phi, rho, sigma, S, conc, b1, a0, a2);
 }
 
 void launch_rhs_pf2(cudaStream_t s, const GridDims& g, const BcDev& bc, const double* eps, double eps_mid,
                     bool uniform, const double* psi, const double* sigma, const double* phi0, const double* fixed,
                     double* b) {
+    ++g_launch_count;
     k_rhs_pf2<<<pw_blocks(g.n), PW_THREADS, 0, s>>>(g, bc, eps, eps_mid, uniform, psi, sigma, phi0, fixed, b);
 }
 
 void launch_relax(cudaStream_t s, long long n, double w, const double* phi0, double* phi,
                   unsigned long long* dmax_bits) {
     cudaMemsetAsync(dmax_bits, 0, sizeof(unsigned long long), s);
+    ++g_launch_count;
     k_relax<<<pw_blocks(n), PW_THREADS, 0, s>>>(n, w, 1.0 - w, phi0, phi, dmax_bits);
 }
 

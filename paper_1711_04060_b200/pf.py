@@ -21,7 +21,7 @@ PF_OK, PF_NOT_CONVERGED = 0, 1
 PF_ERR_ARG, PF_ERR_CUDA, PF_ERR_BREAKDOWN, PF_ERR_NONPHYSICAL, PF_ERR_WORKSPACE = -1, -2, -3, -4, -5
 PF_BC_DIRICHLET, PF_BC_NEUMANN = 0, 1
 (PF_OPT_STENCIL, PF_OPT_OMEGA_PF, PF_OPT_LINEAR_TOL, PF_OPT_LINEAR_MAXIT, PF_OPT_CHECK_INTERVAL,
- PF_OPT_WATER_MOLAR, PF_OPT_MAX_OUTER, PF_OPT_PRECOND, PF_OPT_HISTORY, PF_OPT_KERNELS) = range(1, 11)
+ PF_OPT_WATER_MOLAR, PF_OPT_MAX_OUTER, PF_OPT_PRECOND, PF_OPT_HISTORY, PF_OPT_KERNELS, PF_OPT_PROFILE) = range(1, 12)
 STENCIL_AUTO, STENCIL_STORED, STENCIL_ONTHEFLY = 0, 1, 2
 KERNELS_AUTO, KERNELS_DIRECT, KERNELS_TILED = 0, 1, 2
 
@@ -29,7 +29,7 @@ EXPORTS = [
     "pf_grid_create", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
     "pf_solve_linear", "pf_solve_linear_host", "pf_solve_pf", "pf_fermi_pointwise", "pf_grid_history",
     "pf_grid_linear_iters", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_copy_array",
-    "pf_grid_destroy", "pf_last_error", "pf_version",
+    "pf_grid_profile", "pf_launch_count", "pf_grid_destroy", "pf_last_error", "pf_version",
 ]
 
 
@@ -77,6 +77,8 @@ def load():
     L.pf_grid_stencil.argtypes = [_vp]
     L.pf_grid_palette_size.argtypes = [_vp]
     L.pf_grid_copy_array.argtypes = [_vp, ctypes.c_int, _vp]
+    L.pf_grid_profile.argtypes = [_vp, _dp, ctypes.POINTER(ctypes.c_longlong)]
+    L.pf_launch_count.restype = ctypes.c_longlong
     L.pf_grid_destroy.argtypes = [_vp]
     L.pf_grid_destroy.restype = None
     L.pf_last_error.argtypes = [_vp]
@@ -195,6 +197,17 @@ def pf_grid_history(handle, cap: int) -> np.ndarray:
     buf = np.empty(cap, dtype=np.float64)
     m = _check(handle, load().pf_grid_history(handle, buf.ctypes.data_as(_dp), cap))
     return buf[:m]
+
+
+def pf_grid_profile(handle) -> dict:
+    ms = (ctypes.c_double * 3)()
+    cnt = (ctypes.c_longlong * 3)()
+    _check(handle, load().pf_grid_profile(handle, ms, cnt))
+    return {name: dict(ms=ms[j], launches=cnt[j]) for j, name in enumerate(("k1", "k2", "k3"))}
+
+
+def pf_launch_count() -> int:
+    return int(load().pf_launch_count())
 
 
 def pf_grid_stencil(handle) -> int:
