@@ -140,7 +140,6 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     if (maxit < 0) return fail(g, PF_ERR_ARG, "maxit < 0");
     if (!(tol >= 0.0)) return fail(g, PF_ERR_ARG, "tol must be >= 0");
     const LaunchCtx c = make_ctx(g);
-    const bool tiled = use_tiled(g);
     const bool precond = g->opt_precond != 0;
     Scalars init;
     std::memset(&init, 0, sizeof(init));
@@ -150,6 +149,7 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     KrylovVecs kv;
     kv.b = b; kv.x = x; kv.r = g->r; kv.rt = g->rt; kv.t = g->t; kv.hist = g->hist;
     kv.p_in = g->p0; kv.p_out = g->p1; kv.v_in = g->v0; kv.v_out = g->v1;
+    const bool tiled = use_tiled(g) && tiled_pointers_ok(kv);
     if (tiled) launch_residual_tiled(c, op, kv, 0); else launch_residual_direct(c, op, kv, 0);
 
     const int chunk = g->opt_check < 1 ? 1 : g->opt_check;

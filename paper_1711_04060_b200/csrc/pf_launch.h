@@ -26,6 +26,7 @@ void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, boo
 
 // Tiled family (pf_krylov_tiled.cu).  tiled_supported() says whether the grid fills the tiles.
 bool tiled_supported(const GridDims& g);
+bool tiled_pointers_ok(const KrylovVecs& kv);   // 128-bit accesses need 16-byte aligned x and b
 void launch_residual_tiled(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, int mode);
 void launch_k1_tiled(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
 void launch_k2_tiled(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);

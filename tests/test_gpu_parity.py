@@ -117,6 +117,33 @@ def test_linear_ragged_mixed_bc(pf, oracle, stencil, precond):
     assert rel_l2(out["x"].cpu().numpy(), ref["x"]) <= 1e-9
 
 
+@pytest.mark.parametrize("stencil", [1, 2])
+@pytest.mark.parametrize("precond", [True, False])
+def test_tiled_kernels_ragged_even(pf, oracle, stencil, precond):
+    """Partial tiles in x and y, several z chunks, mixed bc: tiled == direct bit for bit, both == oracle."""
+    w = ragged_workload(nx=70, ny=37, nz=19, seed=9)
+    ref, out_t, hist_t = _linear_case(pf, oracle, w, stencil, kernels=2, precond=precond)
+    _, out_d, hist_d = _linear_case(pf, oracle, w, stencil, kernels=1, precond=precond)
+    assert out_t["status"] == 0 and out_t["iters"] == out_d["iters"]
+    assert torch.equal(out_t["x"], out_d["x"])
+    assert np.array_equal(hist_t, hist_d)
+    assert abs(out_t["iters"] - ref["iters"]) <= max(1, 0.02 * ref["iters"])
+    assert out_t["true_relres"] <= 1.05e-10
+    assert rel_l2(out_t["x"].cpu().numpy(), ref["x"]) <= 1e-9
+
+
+def test_tiled_kernels_neumann_channel(pf, oracle):
+    """configs[3] geometry at 64^3 (lateral Neumann, Dirichlet 0/V in z, charges as RHS), tiled kernels."""
+    w = wl.config3(n=64)
+    w.rhs = oracle.deposit_charges(w.nx, w.ny, w.nz, w.h, w.charges)
+    w.bc_value = w.bc_value.copy(); w.bc_value[5] = 1.9
+    ref, out, _ = _linear_case(pf, oracle, w, 2, kernels=2)
+    assert ref["status"] == 0 and out["status"] == 0
+    assert abs(out["iters"] - ref["iters"]) <= 0.02 * ref["iters"], (out["iters"], ref["iters"])
+    assert out["true_relres"] <= 1.05e-10
+    assert rel_l2(out["x"].cpu().numpy(), ref["x"]) <= 1e-9
+
+
 def test_linear_with_sigma_and_warm_start(pf, oracle):
     w = ragged_workload()
     rng = wl.SplitMix64(3)
