@@ -114,9 +114,12 @@ def measured_peak_gbs():
 def kernel_bytes_per_unknown(stored: bool) -> dict:
     """Algorithmic HBM bytes per unknown per launch: every input vector
     read once, every output written once, halos served on chip."""
+    # k1 reads r, p, v, A0, r~ and writes p', v'; k2 reads r, v', A0 and writes t; k3 reads r, v', p', y, t, r~
+    # and writes y, r; the on-the-fly variant adds a 2-byte stencil code per node to k1 and k2, the stored
+    # variant six 8-byte off-diagonals.
     if stored:
-        return {"k1": (5 + 6 + 2) * 8, "k2": (3 + 6 + 1) * 8, "k3": (7 + 2) * 8}
-    return {"k1": (5 + 2) * 8 + 1, "k2": (3 + 1) * 8 + 1, "k3": (7 + 2) * 8}
+        return {"k1": (5 + 6 + 2) * 8, "k2": (3 + 6 + 1) * 8, "k3": (6 + 2) * 8}
+    return {"k1": (5 + 2) * 8 + 2, "k2": (3 + 1) * 8 + 2, "k3": (6 + 2) * 8}
 
 
 # ---------------------------------------------------------------------------------------------------

@@ -52,8 +52,9 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
 
 /* Option keys for pf_grid_set_option.  Values are doubles; integer options are rounded. */
 #define PF_OPT_STENCIL         1  /* 0 = auto, 1 = stored coefficients A1..A6 (the paper's diagonal
-                                     format), 2 = on-the-fly coefficients from a palette
-                                     of the eps map.  auto = on-the-fly when the map has <= 4 distinct
+                                     format), 2 = on-the-fly coefficients: per node a packed
+                                     code of six indices into the table of distinct face coefficients of
+                                     the eps map.  auto = on-the-fly when the map has <= 4 distinct
                                      values, else stored.  Both give bit-identical results.  Must be
                                      set before pf_grid_set_workspace. */
 #define PF_OPT_OMEGA_PF        2  /* relaxation parameter of Table 2 step 5; default 0.3 */
@@ -67,7 +68,9 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
 #define PF_OPT_HISTORY         9  /* >0: keep the relative residual of every BiCGSTAB iteration of the
                                      last linear solve (up to that many entries); see pf_grid_history */
 #define PF_OPT_KERNELS        10  /* 0 = auto, 1 = direct (one thread per node, neighbours through L1/L2),
-                                     2 = tiled (shared-memory planes, z-marched).  Same arithmetic. */
+                                     2 = tiled (planes staged in shared memory by TMA, z-marched; needs an
+                                     even nx >= 32, ny >= 16, nz >= 8 and 16-byte aligned vectors).  Same
+                                     arithmetic, bit-identical vectors. */
 
 #define PF_OPT_PROFILE        11  /* n > 0: bracket the three kernels of the first n iterations of every
                                      linear solve with CUDA events and accumulate their durations
@@ -97,6 +100,8 @@ int pf_grid_set_option(pf_grid *g, int key, double value);
 /* Jacobi-BiCGSTAB solve of the grid's operator  -div(eps grad x) + sigma x = rhs  (Table 3).
  *   rhs   : device N; entries at Dirichlet nodes are ignored (the boundary value is used, Q20).
  *   x     : device N; in: initial guess (its Dirichlet nodes are overwritten, Q4), out: solution.
+ *           With the Jacobi preconditioner x is written once, at the end of the solve (x = x0 + M^-1 y,
+ *           reading D3 of DESIGN.md).
  *   sigma : device N or NULL (zero); added to the diagonal (PF2's -rho' term, Eq (13)).
  *   Stops when ||r||_2 <= tol*||rhs||_2 on the recurrence residual (Q3); tol = 0 runs exactly maxit
  *   iterations and returns PF_NOT_CONVERGED (the fixed-iteration timing mode).
@@ -151,10 +156,18 @@ long long pf_launch_count(void);
 int pf_grid_stencil(const pf_grid *g);
 int pf_grid_palette_size(const pf_grid *g);
 
+/* Layout of the stencil codes of the on-the-fly variant: bits per code (16: six 2-bit fields, 32: six
+ * 4-bit fields, 0: none -- more than 4 distinct eps values), row pitch in codes (nx rounded up to 8;
+ * code of node (ix,iy,iz) at ix + pitch*(iy + ny*iz)), bytes of one code array.  Field d-1 (d = 1..6 in
+ * the order east, west, south, north, down, up of PAPER.md:219) indexes the coefficient table; index 0
+ * is the coefficient 0.  Out-pointers: host, may be NULL. */
+int pf_grid_code_layout(const pf_grid *g, int *bits_out, int *pitch_out, size_t *bytes_out);
+
 /* Copy an assembled array into caller memory (device), for the assembly parity tests (rows L1/L2):
  * which = 0: Poisson diagonal A0 (N doubles); 1..6: stored off-diagonals A1..A6 (stored variant
- * only); 7: deposited fixed-charge vector (N doubles); 8: node classes of the on-the-fly variant
- * (N bytes); 9: PF1 diagonal (N doubles, after a pf_solve_pf).  Returns PF_ERR_ARG if unavailable. */
+ * only); 7: deposited fixed-charge vector (N doubles); 8: Poisson stencil codes (pf_grid_code_layout
+ * bytes); 9: PF1 diagonal (N doubles, after a pf_solve_pf); 10: Poisson coefficient table (16 doubles);
+ * 11: PF1 stencil codes; 12: PF1 coefficient table.  Returns PF_ERR_ARG if unavailable. */
 int pf_grid_copy_array(pf_grid *g, int which, void *dst_device);
 
 void pf_grid_destroy(pf_grid *g);

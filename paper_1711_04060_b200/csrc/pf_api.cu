@@ -53,8 +53,9 @@ struct pf_grid {
     // small owned device buffers
     Scalars* sc;
     ReduceBuf rb;
-    double* lut_poisson;
-    double* lut_pf1;
+    double* ctab_poisson;    // PF_CTAB doubles each
+    double* ctab_pf1;
+    TmaSet* tma;
     unsigned long long* dmax_bits;
     double* hist;
     int hist_cap;
@@ -66,9 +67,11 @@ struct pf_grid {
     bool stored;
     bool assembled;
     double pf1_lc;           // l_c the PF1 operator was assembled for (NaN = none)
-    double *r, *rt, *p0, *p1, *v0, *v1, *t, *bw, *xw;
+    double *r, *rt, *p0, *p1, *v0, *v1, *t, *y, *bw, *xw;
     double *A0, *A0_pf1, *A0_s, *fixed, *psi, *phi0, *phiw, *sigma, *bpf;
-    uint8_t *cls, *cls_pf1;
+    void *code, *code_pf1;   // stencil codes of the on-the-fly variant (pf_common.cuh Operator)
+    int code_mode;           // 0 none (palette overflow), 1 uint16, 2 uint32
+    int cpitch;
     double* offd[6];
     double* offd_pf1[6];
     std::vector<int> lin_iters;
@@ -99,7 +102,14 @@ int fail(pf_grid* g, int code, const char* fmt, ...) {
         if (e_ != cudaSuccess) return fail((g), PF_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
     } while (0)
 
-int n_vectors(bool stored) { return 18 + (stored ? 12 : 0); }
+int n_vectors(bool stored) { return 19 + (stored ? 12 : 0); }
+
+int code_mode_of(const pf_grid* g) { return g->pal.count > PF_MAX_PALETTE ? 0 : (g->pal.count <= 2 ? 1 : 2); }
+int cpitch_of(const pf_grid* g) { return (g->g.nx + 7) & ~7; }
+size_t code_bytes_of(const pf_grid* g) {
+    const int m = code_mode_of(g);
+    return m == 0 ? 0 : align_up((size_t)cpitch_of(g) * g->g.ny * g->g.nz * (m == 1 ? 2 : 4), 256);
+}
 
 bool want_stored(const pf_grid* g) {
     if (g->opt_stencil == 1) return true;
@@ -109,19 +119,20 @@ bool want_stored(const pf_grid* g) {
 
 bool use_tiled(const pf_grid* g) {
     if (g->opt_kernels == 1) return false;
-    return tiled_supported(g->g);
+    return tma_supported(g->g) && tma_available();
 }
 
 Operator make_op(const pf_grid* g, int which /*0 poisson, 1 pf1, 2 poisson+sigma*/) {
     Operator op;
     std::memset(&op, 0, sizeof(op));
     op.stored = g->stored ? 1 : 0;
-    op.ncls = PF_MAX_CLASSES;
+    op.code32 = g->code_mode == 2 ? 1 : 0;
+    op.cpitch = g->cpitch;
     if (which == 1) {
-        op.A0 = g->A0_pf1; op.cls = g->cls_pf1; op.lut = g->lut_pf1;
+        op.A0 = g->A0_pf1; op.code = g->code_pf1; op.ctab = g->ctab_pf1;
         for (int d = 0; d < 6; ++d) op.offd[d] = g->offd_pf1[d];
     } else {
-        op.A0 = which == 2 ? g->A0_s : g->A0; op.cls = g->cls; op.lut = g->lut_poisson;
+        op.A0 = which == 2 ? g->A0_s : g->A0; op.code = g->code; op.ctab = g->ctab_poisson;
         for (int d = 0; d < 6; ++d) op.offd[d] = g->offd[d];
     }
     return op;
@@ -149,8 +160,16 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     KrylovVecs kv;
     kv.b = b; kv.x = x; kv.r = g->r; kv.rt = g->rt; kv.t = g->t; kv.hist = g->hist;
     kv.p_in = g->p0; kv.p_out = g->p1; kv.v_in = g->v0; kv.v_out = g->v1;
-    const bool tiled = use_tiled(g) && tiled_pointers_ok(kv);
-    if (tiled) launch_residual_tiled(c, op, kv, 0); else launch_residual_direct(c, op, kv, 0);
+    // D3: with the Jacobi preconditioner step 16 accumulates y = sum(alpha p + omega s); x = x0 + M^-1 y at the end
+    kv.y = precond ? g->y : x;
+    if (precond) PF_CUDA(g, cudaMemsetAsync(g->y, 0, sizeof(double) * g->g.n, g->stream));
+    bool tiled = use_tiled(g) && tma_pointers_ok(kv, op);
+    if (tiled && !tma_set_build(g->tma, g->g, op, kv)) {
+        if (g->opt_kernels == 2) return fail(g, PF_ERR_CUDA, "tensor-map encoding failed");
+        tiled = false;
+    }
+    if (g->opt_kernels == 2 && !tiled) return fail(g, PF_ERR_ARG, "tiled kernels need 16-byte aligned vectors");
+    if (tiled) launch_residual_tma(c, op, kv, g->tma, 0); else launch_residual_direct(c, op, kv, 0);
 
     const int chunk = g->opt_check < 1 ? 1 : g->opt_check;
     int launched = 0, slot = 0;
@@ -166,9 +185,10 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
             const bool prof = g->opt_profile && (size_t)(4 * (launched + k) + 3) < g->prof_ev.size();
             cudaEvent_t* pe = prof ? &g->prof_ev[4 * (launched + k)] : nullptr;
             if (prof) cudaEventRecord(pe[0], g->stream);
-            if (tiled) launch_k1_tiled(c, op, kv, precond); else launch_k1_direct(c, op, kv, precond);
+            const int parity = (launched + k) & 1;
+            if (tiled) launch_k1_tma(c, op, kv, g->tma, precond, parity); else launch_k1_direct(c, op, kv, precond);
             if (prof) cudaEventRecord(pe[1], g->stream);
-            if (tiled) launch_k2_tiled(c, op, kv, precond); else launch_k2_direct(c, op, kv, precond);
+            if (tiled) launch_k2_tma(c, op, kv, g->tma, precond, parity); else launch_k2_direct(c, op, kv, precond);
             if (prof) cudaEventRecord(pe[2], g->stream);
             launch_k3(c, op, kv, precond);
             if (prof) cudaEventRecord(pe[3], g->stream);
@@ -193,6 +213,7 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
         }
         slot ^= 1;
     }
+    if (precond) launch_finish_x(c, op, kv);
     PF_CUDA(g, cudaStreamSynchronize(g->stream));
     if (g->opt_profile) {       // only iterations that ran (kernels after convergence return at once)
         const int nprof = std::min<int>(fin.it, (int)g->prof_ev.size() / 4);
@@ -208,7 +229,7 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     if (fin.bb == 0.0) PF_CUDA(g, cudaMemsetAsync(x, 0, sizeof(double) * g->g.n, g->stream));   // Q3
     double true_rel = 0.0;
     if (true_relres_out && fin.bb != 0.0) {
-        if (tiled) launch_residual_tiled(c, op, kv, 1); else launch_residual_direct(c, op, kv, 1);
+        if (tiled) launch_residual_tma(c, op, kv, g->tma, 1); else launch_residual_direct(c, op, kv, 1);
         PF_CUDA(g, cudaMemcpyAsync(g->sc_host[0], g->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
         PF_CUDA(g, cudaStreamSynchronize(g->stream));
         true_rel = std::sqrt(g->sc_host[0]->true_rr) / fin.bnorm;
@@ -303,7 +324,8 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0;
     g->charges_dev = nullptr; g->sc = nullptr; g->rb.partial = nullptr; g->rb.ticket = nullptr;
-    g->lut_poisson = g->lut_pf1 = nullptr; g->dmax_bits = nullptr;
+    g->ctab_poisson = g->ctab_pf1 = nullptr; g->dmax_bits = nullptr; g->tma = nullptr;
+    g->code = g->code_pf1 = nullptr; g->code_mode = 0; g->cpitch = 0;
     g->sc_host[0] = g->sc_host[1] = nullptr; g->ev[0] = g->ev[1] = nullptr;
 #define PF_CREATE_CUDA(call)                                                                         \
     do {                                                                                             \
@@ -320,8 +342,9 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     PF_CREATE_CUDA(cudaMalloc(&g->rb.partial, sizeof(dd) * 3 * PF_MAX_PARTIAL_BLOCKS));
     PF_CREATE_CUDA(cudaMalloc(&g->rb.ticket, 256));
     PF_CREATE_CUDA(cudaMemsetAsync(g->rb.ticket, 0, 256, g->stream));
-    PF_CREATE_CUDA(cudaMalloc(&g->lut_poisson, sizeof(double) * PF_MAX_CLASSES * PF_MAX_CLASSES));
-    PF_CREATE_CUDA(cudaMalloc(&g->lut_pf1, sizeof(double) * PF_MAX_CLASSES * PF_MAX_CLASSES));
+    PF_CREATE_CUDA(cudaMalloc(&g->ctab_poisson, sizeof(double) * PF_CTAB));
+    PF_CREATE_CUDA(cudaMalloc(&g->ctab_pf1, sizeof(double) * PF_CTAB));
+    g->tma = tma_set_create();
     PF_CREATE_CUDA(cudaMalloc(&g->dmax_bits, 256));
     PF_CREATE_CUDA(cudaMallocHost(&g->sc_host[0], sizeof(Scalars)));
     PF_CREATE_CUDA(cudaMallocHost(&g->sc_host[1], sizeof(Scalars)));
@@ -349,7 +372,8 @@ void pf_grid_destroy(pf_grid* g) {
     if (!g) return;
     cudaStreamSynchronize(g->stream);
     cudaFree(g->sc); cudaFree(g->rb.partial); cudaFree(g->rb.ticket);
-    cudaFree(g->lut_poisson); cudaFree(g->lut_pf1); cudaFree(g->dmax_bits);
+    cudaFree(g->ctab_poisson); cudaFree(g->ctab_pf1); cudaFree(g->dmax_bits);
+    if (g->tma) tma_set_destroy(g->tma);
     cudaFree(g->charges_dev); cudaFree(g->hist);
     if (g->sc_host[0]) cudaFreeHost(g->sc_host[0]);
     if (g->sc_host[1]) cudaFreeHost(g->sc_host[1]);
@@ -363,8 +387,7 @@ void pf_grid_destroy(pf_grid* g) {
 size_t pf_grid_workspace_bytes(const pf_grid* g) {
     if (!g) return 0;
     const size_t vec = align_up(sizeof(double) * (size_t)g->g.n, 256);
-    const size_t bytes = align_up((size_t)g->g.n, 256);
-    return (size_t)n_vectors(want_stored(g)) * vec + 2 * bytes;
+    return (size_t)n_vectors(want_stored(g)) * vec + 2 * code_bytes_of(g);
 }
 
 int pf_grid_set_option(pf_grid* g, int key, double value) {
@@ -426,7 +449,8 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
         }
         case PF_OPT_KERNELS:
             if (iv < 0 || iv > 2) return fail(g, PF_ERR_ARG, "kernels must be 0, 1 or 2");
-            if (iv == 2 && !tiled_supported(g->g)) return fail(g, PF_ERR_ARG, "grid too small for the tiled kernels");
+            if (iv == 2 && !(tma_supported(g->g) && tma_available()))
+                return fail(g, PF_ERR_ARG, "the tiled kernels need an even nx >= 32, ny >= 16, nz >= 8");
             g->opt_kernels = iv; return PF_OK;
         default:
             return fail(g, PF_ERR_ARG, "unknown option key %d", key);
@@ -445,22 +469,24 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     char* base = (char*)dev_ptr;
     auto take = [&]() { double* p = (double*)base; base += vec; return p; };
     g->r = take(); g->rt = take(); g->p0 = take(); g->p1 = take(); g->v0 = take(); g->v1 = take();
-    g->t = take(); g->bw = take(); g->xw = take();
+    g->t = take(); g->y = take(); g->bw = take(); g->xw = take();
     g->A0 = take(); g->A0_pf1 = take(); g->A0_s = take(); g->fixed = take(); g->psi = take();
     g->phi0 = take(); g->phiw = take(); g->sigma = take(); g->bpf = take();
     for (int d = 0; d < 6; ++d) { g->offd[d] = g->stored ? take() : nullptr; }
     for (int d = 0; d < 6; ++d) { g->offd_pf1[d] = g->stored ? take() : nullptr; }
-    const size_t nb = align_up((size_t)g->g.n, 256);
-    g->cls = (uint8_t*)base; base += nb;
-    g->cls_pf1 = (uint8_t*)base; base += nb;
-    const bool use_pal = g->pal.count <= PF_MAX_PALETTE;
+    g->code_mode = code_mode_of(g);
+    g->cpitch = cpitch_of(g);
+    const size_t cb = code_bytes_of(g);
+    g->code = cb ? (void*)base : nullptr; base += cb;
+    g->code_pf1 = cb ? (void*)base : nullptr; base += cb;
     // rows L1, L2: Poisson operator, coefficient table, fixed charges
-    launch_assemble_poisson(g->stream, g->g, g->h, g->bc, g->eps, g->pal, use_pal, g->A0, g->cls, g->offd);
-    if (use_pal) {
-        double lut[PF_MAX_CLASSES * PF_MAX_CLASSES];
-        int nc = 0;
-        build_lut_poisson(g->pal, g->h, lut, &nc);
-        PF_CUDA(g, cudaMemcpyAsync(g->lut_poisson, lut, sizeof(lut), cudaMemcpyHostToDevice, g->stream));
+    if (cb) PF_CUDA(g, cudaMemsetAsync(g->code, 0, 2 * cb, g->stream));    // padding columns of the code rows
+    launch_assemble_poisson(g->stream, g->g, g->h, g->bc, g->eps, g->pal, g->code_mode, g->A0, g->code, g->cpitch,
+                            g->offd);
+    if (g->code_mode) {
+        double ctab[PF_CTAB];
+        build_ctab_poisson(g->pal, g->h, ctab);
+        PF_CUDA(g, cudaMemcpyAsync(g->ctab_poisson, ctab, sizeof(ctab), cudaMemcpyHostToDevice, g->stream));
     }
     launch_deposit(g->stream, g->g, g->h, kappa_angstrom(), g->charges_dev, g->ncharges, g->fixed);
     PF_CUDA(g, cudaMemsetAsync(g->p0, 0, vec * 4, g->stream));   // p0,p1,v0,v1 finite before first use
@@ -525,15 +551,13 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
     rc = make_species(g, nions, valence, bath_conc, radii, &sp);
     if (rc) return rc;
     const size_t nbytes = sizeof(double) * (size_t)g->g.n;
-    const bool use_pal = g->pal.count <= PF_MAX_PALETTE;
     if (!(g->pf1_lc == l_c)) {      // row N2: PF1 operator, once per (grid, l_c)
-        launch_assemble_pf1(g->stream, g->g, g->h, l_c, g->eps, g->eps_mid, g->uniform, g->pal, use_pal, g->A0_pf1,
-                            g->cls_pf1, g->offd_pf1);
-        if (use_pal) {
-            double lut[PF_MAX_CLASSES * PF_MAX_CLASSES];
-            int nc = 0;
-            build_lut_pf1(g->pal, g->h, l_c, lut, &nc);
-            PF_CUDA(g, cudaMemcpyAsync(g->lut_pf1, lut, sizeof(lut), cudaMemcpyHostToDevice, g->stream));
+        launch_assemble_pf1(g->stream, g->g, g->h, l_c, g->eps, g->eps_mid, g->uniform, g->pal, g->code_mode, g->A0_pf1,
+                            g->code_pf1, g->cpitch, g->offd_pf1);
+        if (g->code_mode) {
+            double ctab[PF_CTAB];
+            build_ctab_pf1(g->pal, g->h, l_c, ctab);
+            PF_CUDA(g, cudaMemcpyAsync(g->ctab_pf1, ctab, sizeof(ctab), cudaMemcpyHostToDevice, g->stream));
         }
         g->pf1_lc = l_c;
     }
@@ -613,6 +637,15 @@ int pf_grid_profile(pf_grid* g, double* ms_out, long long* launches_out) {
 int pf_grid_stencil(const pf_grid* g) { return g ? (want_stored(g) ? 1 : 2) : PF_ERR_ARG; }
 int pf_grid_palette_size(const pf_grid* g) { return g ? g->pal.count : PF_ERR_ARG; }
 
+int pf_grid_code_layout(const pf_grid* g, int* bits_out, int* pitch_out, size_t* bytes_out) {
+    if (!g) return PF_ERR_ARG;
+    const int m = code_mode_of(g);
+    if (bits_out) *bits_out = m == 0 ? 0 : (m == 1 ? 16 : 32);
+    if (pitch_out) *pitch_out = cpitch_of(g);
+    if (bytes_out) *bytes_out = code_bytes_of(g);
+    return PF_OK;
+}
+
 int pf_grid_copy_array(pf_grid* g, int which, void* dst) {
     if (!g || !dst) return PF_ERR_ARG;
     if (!g->assembled) return fail(g, PF_ERR_WORKSPACE, "workspace not set");
@@ -621,8 +654,11 @@ int pf_grid_copy_array(pf_grid* g, int which, void* dst) {
     if (which == 0) src = g->A0;
     else if (which >= 1 && which <= 6) src = g->offd[which - 1];
     else if (which == 7) src = g->fixed;
-    else if (which == 8) { src = g->pal.count <= PF_MAX_PALETTE ? g->cls : nullptr; nbytes = (size_t)g->g.n; }
+    else if (which == 8) { src = g->code; nbytes = code_bytes_of(g); }
     else if (which == 9) src = (g->pf1_lc == g->pf1_lc) ? g->A0_pf1 : nullptr;
+    else if (which == 10) { src = g->code_mode ? g->ctab_poisson : nullptr; nbytes = sizeof(double) * PF_CTAB; }
+    else if (which == 11) { src = (g->pf1_lc == g->pf1_lc) ? g->code_pf1 : nullptr; nbytes = code_bytes_of(g); }
+    else if (which == 12) { src = (g->pf1_lc == g->pf1_lc && g->code_mode) ? g->ctab_pf1 : nullptr; nbytes = sizeof(double) * PF_CTAB; }
     if (!src) return fail(g, PF_ERR_ARG, "array %d is not available", which);
     PF_CUDA(g, cudaMemcpyAsync(dst, src, nbytes, cudaMemcpyDeviceToDevice, g->stream));
     PF_CUDA(g, cudaStreamSynchronize(g->stream));

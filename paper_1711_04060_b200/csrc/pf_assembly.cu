@@ -2,9 +2,10 @@
 //
 // The paper builds A0..A6 and b on the GPU each outer iteration and finds that the weak part of its
 // design (7.7x against 22.8x for the solver).  Here the flux part of every
-// operator is assembled ONCE per grid: per node a class byte (palette index of eps, identity-row
-// flag) and the diagonal; the six off-diagonals are either stored (the paper's format)
-// or looked up on the fly in a (class x class) table.  PF2's sigma only shifts the diagonal.
+// operator is assembled ONCE per grid: per node the diagonal and either the six stored off-diagonals
+// (the paper's format) or a packed code of six table indices, one per face, into the
+// short table of distinct face coefficients of the map (on-the-fly variant; pf_common.cuh Operator).
+// PF2's sigma only shifts the diagonal.
 #include "pf_launch.h"
 #include <algorithm>
 #include <cstring>
@@ -14,8 +15,16 @@ namespace pf {
 namespace {
 
 constexpr int ASM_THREADS = 256;
-constexpr int IDENT_BIT = PF_MAX_PALETTE;        // cls = palette index + IDENT_BIT*identity
-constexpr int CLS_OUTSIDE = 2 * PF_MAX_PALETTE;  // neighbour outside the box
+// Table index of the face between palette entries a and b (unordered pair), 1-based; 0 = no coupling.
+__host__ __device__ inline int pair_index(int a, int b, int count) {
+    const int lo = a < b ? a : b, hi = a < b ? b : a;
+    return 1 + lo * count - lo * (lo - 1) / 2 + (hi - lo);
+}
+
+__device__ __forceinline__ void store_code(void* code, int code_mode, long long k, unsigned int c) {
+    if (code_mode == 1) static_cast<unsigned short*>(code)[k] = (unsigned short)c;
+    else if (code_mode == 2) static_cast<unsigned int*>(code)[k] = c;
+}
 
 struct ScanBuf {
     unsigned long long tab[PF_MAX_PALETTE + 1];  // bit patterns of the distinct values, 0 = empty
@@ -84,65 +93,82 @@ __device__ __forceinline__ double face_coeff(double ea, double eb, double hh) {
     return dvd(dvd(mul(mul(2.0, ea), eb), add(ea, eb)), hh);
 }
 
+// code_mode: 0 = no codes (palette overflow), 1 = uint16 / 2-bit fields, 2 = uint32 / 4-bit fields.
 __global__ void __launch_bounds__(ASM_THREADS)
-k_assemble_poisson(GridDims g, double h, BcDev bc, const double* __restrict__ eps, Palette pal, bool use_palette,
-                   double* __restrict__ A0, uint8_t* __restrict__ cls, double* o0, double* o1, double* o2,
+k_assemble_poisson(GridDims g, double h, BcDev bc, const double* __restrict__ eps, Palette pal, int code_mode,
+                   double* __restrict__ A0, void* __restrict__ code, int cpitch, double* o0, double* o1, double* o2,
                    double* o3, double* o4, double* o5) {
     double* offd[6] = {o0, o1, o2, o3, o4, o5};
     const double hh = mul(h, h);
     const long long off[6] = {1, -1, -(long long)g.nx, (long long)g.nx, -(long long)g.nx * g.ny,
                               (long long)g.nx * g.ny};
+    const int fbits = code_mode == 2 ? 4 : 2;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
         int ix, iy, iz;
         decode(g, i, ix, iy, iz);
+        const long long k = ix + (long long)cpitch * (iy + (long long)g.ny * iz);
         const double ei = eps[i];
         const bool ident = dirichlet_face(g, bc, ix, iy, iz) >= 0;
-        if (use_palette) cls[i] = (uint8_t)(palette_index(pal, ei) + (ident ? IDENT_BIT : 0));
         if (ident) {
             A0[i] = 1.0;
+            store_code(code, code_mode, k, 0u);
 #pragma unroll
             for (int d = 0; d < 6; ++d) if (offd[d]) offd[d][i] = 0.0;
             continue;
         }
         const bool in[6] = {ix + 1 < g.nx, ix > 0, iy > 0, iy + 1 < g.ny, iz > 0, iz + 1 < g.nz};
+        const int pi = code_mode ? palette_index(pal, ei) : 0;
         double diag = 0.0;
+        unsigned int cw = 0u;
 #pragma unroll
         for (int d = 0; d < 6; ++d) {
             double c = 0.0;
             if (in[d]) {
-                c = face_coeff(ei, eps[i + off[d]], hh);
+                const double en = eps[i + off[d]];
+                c = face_coeff(ei, en, hh);
                 diag = add(diag, c);
+                if (code_mode) cw |= (unsigned int)pair_index(pi, palette_index(pal, en), pal.count) << (fbits * d);
             }
             if (offd[d]) offd[d][i] = in[d] ? -c : 0.0;
         }
         A0[i] = diag;
+        store_code(code, code_mode, k, cw);
     }
 }
 
 __global__ void __launch_bounds__(ASM_THREADS)
 k_assemble_pf1(GridDims g, double h, double lc, const double* __restrict__ eps, double eps_mid, bool uniform,
-               Palette pal, bool use_palette, double* __restrict__ A0, uint8_t* __restrict__ cls, double* o0,
+               Palette pal, int code_mode, double* __restrict__ A0, void* __restrict__ code, int cpitch, double* o0,
                double* o1, double* o2, double* o3, double* o4, double* o5) {
     double* offd[6] = {o0, o1, o2, o3, o4, o5};
     const double hh = mul(h, h), ll = mul(lc, lc);
+    const int fbits = code_mode == 2 ? 4 : 2;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
         int ix, iy, iz;
         decode(g, i, ix, iy, iz);
+        const long long k = ix + (long long)cpitch * (iy + (long long)g.ny * iz);
         const double ei = eps[i];
         const bool boundary = ix == 0 || ix == g.nx - 1 || iy == 0 || iy == g.ny - 1 || iz == 0 || iz == g.nz - 1;
         const bool solvent = uniform || ei > eps_mid;           // Q17
         const bool ident = boundary || !solvent;                // Q15
-        if (use_palette) cls[i] = (uint8_t)(palette_index(pal, ei) + (ident ? IDENT_BIT : 0));
         if (ident) {
             A0[i] = 1.0;
+            store_code(code, code_mode, k, 0u);
 #pragma unroll
             for (int d = 0; d < 6; ++d) if (offd[d]) offd[d][i] = 0.0;
             continue;
         }
         const double c = dvd(mul(ei, ll), hh);
         A0[i] = add(mul(6.0, c), ei);
+        if (code_mode) {           // all six faces carry the node's own coefficient: table index 1 + palette index
+            const unsigned int f = 1u + (unsigned int)palette_index(pal, ei);
+            unsigned int cw = 0u;
+#pragma unroll
+            for (int d = 0; d < 6; ++d) cw |= f << (fbits * d);
+            store_code(code, code_mode, k, cw);
+        }
 #pragma unroll
         for (int d = 0; d < 6; ++d) if (offd[d]) offd[d][i] = -c;
     }
@@ -220,47 +246,34 @@ cudaError_t scan_eps(cudaStream_t s, long long n, const double* eps, void* scrat
 }
 
 void launch_assemble_poisson(cudaStream_t s, const GridDims& g, double h, const BcDev& bc, const double* eps,
-                             const Palette& pal, bool use_palette, double* A0, uint8_t* cls, double* const offd[6]) {
+                             const Palette& pal, int code_mode, double* A0, void* code, int cpitch,
+                             double* const offd[6]) {
     ++g_launch_count;
-    k_assemble_poisson<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, h, bc, eps, pal, use_palette, A0, cls, offd[0],
+    k_assemble_poisson<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, h, bc, eps, pal, code_mode, A0, code, cpitch, offd[0],
                                                                 offd[1], offd[2], offd[3], offd[4], offd[5]);
 }
 
 void launch_assemble_pf1(cudaStream_t s, const GridDims& g, double h, double lc, const double* eps, double eps_mid,
-                         bool uniform, const Palette& pal, bool use_palette, double* A0, uint8_t* cls,
+                         bool uniform, const Palette& pal, int code_mode, double* A0, void* code, int cpitch,
                          double* const offd[6]) {
     ++g_launch_count;
-    k_assemble_pf1<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, h, lc, eps, eps_mid, uniform, pal, use_palette, A0, cls,
-                                                            offd[0], offd[1], offd[2], offd[3], offd[4], offd[5]);
+    k_assemble_pf1<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, h, lc, eps, eps_mid, uniform, pal, code_mode, A0, code,
+                                                            cpitch, offd[0], offd[1], offd[2], offd[3], offd[4], offd[5]);
 }
 
-// Tables of the on-the-fly variant: entry [ci*ncls + cn] is the off-diagonal coefficient of a row of
-// class ci towards a neighbour of class cn.  Identity rows and outside neighbours give 0.
-void build_lut_poisson(const Palette& pal, double h, double* lut, int* ncls) {
-    const int nc = PF_MAX_CLASSES;
-    *ncls = nc;
-    for (int ci = 0; ci < nc; ++ci)
-        for (int cn = 0; cn < nc; ++cn) {
-            double v = 0.0;
-            const bool ident = ci >= IDENT_BIT, outside = (cn == CLS_OUTSIDE) || (ci == CLS_OUTSIDE);
-            const int pi = ci % PF_MAX_PALETTE, pn = cn % PF_MAX_PALETTE;
-            if (!ident && !outside && pi < pal.count && pn < pal.count)
-                v = -host_face_coeff(pal.value[pi], pal.value[pn], h);
-            lut[ci * nc + cn] = v;
-        }
+// Coefficient tables of the on-the-fly variant (host side, PF_CTAB doubles): entry 0 is 0.0, entry
+// pair_index(a, b) the off-diagonal -H(eps_a, eps_b)/h^2 (Poisson) resp. entry 1 + a the off-diagonal
+// -eps_a l_c^2/h^2 (PF1), computed with the same operations in the same order as the kernels above.
+void build_ctab_poisson(const Palette& pal, double h, double* ctab) {
+    for (int k = 0; k < PF_CTAB; ++k) ctab[k] = 0.0;
+    for (int a = 0; a < pal.count && a < PF_MAX_PALETTE; ++a)
+        for (int b = a; b < pal.count && b < PF_MAX_PALETTE; ++b)
+            ctab[pair_index(a, b, pal.count)] = -host_face_coeff(pal.value[a], pal.value[b], h);
 }
 
-void build_lut_pf1(const Palette& pal, double h, double lc, double* lut, int* ncls) {
-    const int nc = PF_MAX_CLASSES;
-    *ncls = nc;
-    for (int ci = 0; ci < nc; ++ci)
-        for (int cn = 0; cn < nc; ++cn) {
-            double v = 0.0;
-            const bool ident = ci >= IDENT_BIT, outside = (cn == CLS_OUTSIDE) || (ci == CLS_OUTSIDE);
-            const int pi = ci % PF_MAX_PALETTE;
-            if (!ident && !outside && pi < pal.count) v = -(pal.value[pi] * (lc * lc) / (h * h));
-            lut[ci * nc + cn] = v;
-        }
+void build_ctab_pf1(const Palette& pal, double h, double lc, double* ctab) {
+    for (int k = 0; k < PF_CTAB; ++k) ctab[k] = 0.0;
+    for (int a = 0; a < pal.count && a < PF_MAX_PALETTE; ++a) ctab[1 + a] = -(pal.value[a] * (lc * lc) / (h * h));
 }
 
 void launch_deposit(cudaStream_t s, const GridDims& g, double h, double kappa, const double* charges_dev, int m,

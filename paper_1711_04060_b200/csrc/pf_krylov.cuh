@@ -11,6 +11,7 @@ namespace pf {
 struct KrylovVecs {
     const double* b;     // right-hand side with Dirichlet values in place
     double* x;
+    double* y;           // preconditioned solves accumulate step 16 here (reading D3); == x when M = I
     double* r;
     double* rt;          // r~ = r0
     double* p_in;  double* p_out;

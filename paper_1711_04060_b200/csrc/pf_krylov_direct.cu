@@ -6,8 +6,8 @@
 // One BiCGSTAB iteration (Table 3) is three launches, one per reduction point:
 //   k1: steps 5-11   p = r + beta(p - omega v);  v = A M^-1 p;           reduces r~.v        (row L4)
 //   k2: steps 12-14  alpha; s = r - alpha v;  t = A M^-1 s;              reduces t.s, t.t    (row L5)
-//   k3: steps 15-18  omega; x += alpha M^-1 p + omega M^-1 s; r = s - omega t;
-//                    reduces r~.r (step 4 of the next iteration) and r.r (step 18)            (row L6)
+//   k3: steps 15-18  omega; y += alpha p + omega s (x = x0 + M^-1 y at the end, reading D3);
+//                    r = s - omega t; reduces r~.r (step 4 of the next iteration) and r.r     (row L6)
 #include "pf_krylov.cuh"
 #include "pf_launch.h"
 
@@ -20,6 +20,7 @@ constexpr int DIRECT_THREADS = 256;
 struct Nbr {
     long long j[6];
     bool in[6];
+    int ix, iy, iz;
 };
 
 __device__ __forceinline__ Nbr neighbours(const GridDims& g, long long i) {
@@ -29,6 +30,7 @@ __device__ __forceinline__ Nbr neighbours(const GridDims& g, long long i) {
     const int iz = (int)(q / g.ny);
     const long long sx = 1, sy = g.nx, sz = (long long)g.nx * g.ny;
     Nbr n;
+    n.ix = ix; n.iy = iy; n.iz = iz;
     n.j[0] = i + sx; n.in[0] = ix + 1 < g.nx;
     n.j[1] = i - sx; n.in[1] = ix > 0;
     n.j[2] = i - sy; n.in[2] = iy > 0;
@@ -40,21 +42,21 @@ __device__ __forceinline__ Nbr neighbours(const GridDims& g, long long i) {
 
 // Off-diagonal coefficients of row i (0 where the neighbour is outside the box or the row is an
 // identity row).
-__device__ __forceinline__ void row_coeffs(const Operator& op, const double* lut_s, long long i, const Nbr& n,
-                                           double (&c)[6]) {
+__device__ __forceinline__ void row_coeffs(const Operator& op, const GridDims& g, const double* ctab_s, long long i,
+                                           const Nbr& n, double (&c)[6]) {
     if (op.stored) {
 #pragma unroll
         for (int d = 0; d < 6; ++d) c[d] = n.in[d] ? __ldg(op.offd[d] + i) : 0.0;
     } else {
-        const int ci = op.cls[i] * op.ncls;
+        const unsigned int code = load_code(op, g, n.ix, n.iy, n.iz);
 #pragma unroll
-        for (int d = 0; d < 6; ++d) c[d] = n.in[d] ? lut_s[ci + op.cls[n.j[d]]] : 0.0;
+        for (int d = 0; d < 6; ++d) c[d] = ctab_s[code_field(code, op.code32, d)];
     }
 }
 
-__device__ __forceinline__ void load_lut(const Operator& op, double* lut_s) {
+__device__ __forceinline__ void load_ctab(const Operator& op, double* ctab_s) {
     if (!op.stored)
-        for (int k = threadIdx.x; k < op.ncls * op.ncls; k += blockDim.x) lut_s[k] = op.lut[k];
+        for (int k = threadIdx.x; k < PF_CTAB; k += blockDim.x) ctab_s[k] = op.ctab[k];
     __syncthreads();
 }
 
@@ -62,15 +64,15 @@ __device__ __forceinline__ void load_lut(const Operator& op, double* lut_s) {
 template <int MODE>
 __global__ void __launch_bounds__(DIRECT_THREADS)
 k_residual(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
-    __shared__ double lut_s[PF_MAX_CLASSES * PF_MAX_CLASSES];
+    __shared__ double ctab_s[PF_CTAB];
     __shared__ dd scratch[2 * 32];
-    load_lut(op, lut_s);
+    load_ctab(op, ctab_s);
     dd q[2] = {dd_zero(), dd_zero()};
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
         Nbr n = neighbours(g, i);
         double c[6];
-        row_coeffs(op, lut_s, i, n, c);
+        row_coeffs(op, g, ctab_s, i, n, c);
         double acc = mul(op.A0[i], kv.x[i]);
 #pragma unroll
         for (int d = 0; d < 6; ++d)
@@ -94,9 +96,9 @@ template <bool PRECOND>
 __global__ void __launch_bounds__(DIRECT_THREADS)
 k1_direct(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
     if (sc->done) return;
-    __shared__ double lut_s[PF_MAX_CLASSES * PF_MAX_CLASSES];
+    __shared__ double ctab_s[PF_CTAB];
     __shared__ dd scratch[32];
-    load_lut(op, lut_s);
+    load_ctab(op, ctab_s);
     const bool first = sc->first != 0;
     const double beta = sc->beta, omega = sc->omega;
     dd q[1] = {dd_zero()};
@@ -104,7 +106,7 @@ k1_direct(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
         Nbr n = neighbours(g, i);
         double c[6];
-        row_coeffs(op, lut_s, i, n, c);
+        row_coeffs(op, g, ctab_s, i, n, c);
         const double a0 = op.A0[i];
         const double pi = p_new_at<PRECOND>(first, beta, omega, kv.r[i], kv.p_in[i], kv.v_in[i]);
         double acc = mul(a0, jacobi<PRECOND>(pi, a0));
@@ -126,16 +128,16 @@ template <bool PRECOND>
 __global__ void __launch_bounds__(DIRECT_THREADS)
 k2_direct(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
     if (sc->done) return;
-    __shared__ double lut_s[PF_MAX_CLASSES * PF_MAX_CLASSES];
+    __shared__ double ctab_s[PF_CTAB];
     __shared__ dd scratch[2 * 32];
-    load_lut(op, lut_s);
+    load_ctab(op, ctab_s);
     const double alpha = sc->alpha;
     dd q[2] = {dd_zero(), dd_zero()};
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
         Nbr n = neighbours(g, i);
         double c[6];
-        row_coeffs(op, lut_s, i, n, c);
+        row_coeffs(op, g, ctab_s, i, n, c);
         const double a0 = op.A0[i];
         const double si = s_at(alpha, kv.r[i], kv.v_out[i]);
         double acc = mul(a0, jacobi<PRECOND>(si, a0));
@@ -155,27 +157,84 @@ k2_direct(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
 
 }  // namespace
 
-// Steps 16-17 are pointwise; this kernel serves both kernel families.
-template <bool PRECOND>
-__global__ void __launch_bounds__(256)
-k3_update(long long n, const double* __restrict__ A0, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
+// Steps 16-17 are pointwise; this kernel serves both kernel families.  Reads r, v, p, y, t, r~ and
+// writes y, r: a pure streaming kernel, 128-bit accesses, two independent groups in flight per thread.
+// With M = I the accumulator y IS x and the statement is Table 3 step 16 verbatim; with the Jacobi
+// preconditioner y collects alpha p + omega s and x = x0 + M^-1 y is formed once (k_finish_x, D3).
+struct K3Elem { double r, v, p, y, t, rt; };
+
+__device__ __forceinline__ void k3_point(const K3Elem& e, double alpha, double omega, double& y_new, double& r_new,
+                                         dd& q0, dd& q1) {
+    const double s = s_at(alpha, e.r, e.v);
+    y_new = add(add(e.y, mul(alpha, e.p)), mul(omega, s));       // step 16
+    r_new = sub(s, mul(omega, e.t));                              // step 17
+    dd_fma(q0, e.rt, r_new);
+    dd_fma(q1, r_new, r_new);
+}
+
+template <bool VEC>
+__global__ void __launch_bounds__(256, 3)
+k3_update(long long n, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
     if (sc->done) return;
     __shared__ dd scratch[2 * 32];
     const double alpha = sc->alpha, omega = sc->omega;
-    dd q[2] = {dd_zero(), dd_zero()};
+    dd qa[2] = {dd_zero(), dd_zero()}, qb[2] = {dd_zero(), dd_zero()};
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const double a0 = PRECOND ? A0[i] : 1.0;
-        const double s = s_at(alpha, kv.r[i], kv.v_out[i]);
-        const double ph = jacobi<PRECOND>(kv.p_out[i], a0);
-        const double sh = jacobi<PRECOND>(s, a0);
-        kv.x[i] = add(add(kv.x[i], mul(alpha, ph)), mul(omega, sh));   // step 16
-        const double rn = sub(s, mul(omega, kv.t[i]));                  // step 17
-        kv.r[i] = rn;
-        dd_fma(q[0], kv.rt[i], rn);
-        dd_fma(q[1], rn, rn);
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (VEC) {
+        const long long n2 = n >> 1;
+        const double2* r2 = reinterpret_cast<const double2*>(kv.r);
+        const double2* v2 = reinterpret_cast<const double2*>(kv.v_out);
+        const double2* p2 = reinterpret_cast<const double2*>(kv.p_out);
+        const double2* y2 = reinterpret_cast<const double2*>(kv.y);
+        const double2* t2 = reinterpret_cast<const double2*>(kv.t);
+        const double2* rt2 = reinterpret_cast<const double2*>(kv.rt);
+        double2* yo = reinterpret_cast<double2*>(kv.y);
+        double2* ro = reinterpret_cast<double2*>(kv.r);
+        long long i = tid;
+        for (; i + stride < n2; i += 2 * stride) {
+            const long long j = i + stride;
+            const double2 ra = r2[i], va = v2[i], pa = p2[i], ya = y2[i], ta = t2[i], wa = rt2[i];
+            const double2 rb2 = r2[j], vb = v2[j], pb = p2[j], yb = y2[j], tb = t2[j], wb = rt2[j];
+            double2 yn, rn;
+            k3_point({ra.x, va.x, pa.x, ya.x, ta.x, wa.x}, alpha, omega, yn.x, rn.x, qa[0], qa[1]);
+            k3_point({ra.y, va.y, pa.y, ya.y, ta.y, wa.y}, alpha, omega, yn.y, rn.y, qb[0], qb[1]);
+            yo[i] = yn; ro[i] = rn;
+            k3_point({rb2.x, vb.x, pb.x, yb.x, tb.x, wb.x}, alpha, omega, yn.x, rn.x, qa[0], qa[1]);
+            k3_point({rb2.y, vb.y, pb.y, yb.y, tb.y, wb.y}, alpha, omega, yn.y, rn.y, qb[0], qb[1]);
+            yo[j] = yn; ro[j] = rn;
+        }
+        for (; i < n2; i += stride) {
+            const double2 ra = r2[i], va = v2[i], pa = p2[i], ya = y2[i], ta = t2[i], wa = rt2[i];
+            double2 yn, rn;
+            k3_point({ra.x, va.x, pa.x, ya.x, ta.x, wa.x}, alpha, omega, yn.x, rn.x, qa[0], qa[1]);
+            k3_point({ra.y, va.y, pa.y, ya.y, ta.y, wa.y}, alpha, omega, yn.y, rn.y, qb[0], qb[1]);
+            yo[i] = yn; ro[i] = rn;
+        }
+        if ((n & 1) && tid == 0) {                    // odd tail
+            const long long k = n - 1;
+            double yn, rn;
+            k3_point({kv.r[k], kv.v_out[k], kv.p_out[k], kv.y[k], kv.t[k], kv.rt[k]}, alpha, omega, yn, rn, qa[0], qa[1]);
+            kv.y[k] = yn; kv.r[k] = rn;
+        }
+    } else {
+        for (long long i = tid; i < n; i += stride) {
+            double yn, rn;
+            k3_point({kv.r[i], kv.v_out[i], kv.p_out[i], kv.y[i], kv.t[i], kv.rt[i]}, alpha, omega, yn, rn, qa[0], qa[1]);
+            kv.y[i] = yn; kv.r[i] = rn;
+        }
     }
-    if (grid_reduce_dd<2>(q, scratch, rb)) finish_k3(sc, kv.hist, dd_round(q[0]), dd_round(q[1]));
+    dd_add(qa[0], qb[0]);
+    dd_add(qa[1], qb[1]);
+    if (grid_reduce_dd<2>(qa, scratch, rb)) finish_k3(sc, kv.hist, dd_round(qa[0]), dd_round(qa[1]));
+}
+
+// x = x + M^-1 y (reading D3).  y is exactly 0 on identity rows, so Dirichlet values of x are kept.
+__global__ void __launch_bounds__(256)
+k_finish_x(long long n, const double* __restrict__ A0, const double* __restrict__ y, double* __restrict__ x) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        x[i] = add(x[i], dvd(y[i], A0[i]));
 }
 
 static int direct_blocks(long long n, int sm_count) {
@@ -204,9 +263,23 @@ void launch_k2_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& 
 }
 
 void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond) {
+    (void)op; (void)precond;
+    // 3 blocks of 256 threads per SM, each thread two 16-byte groups in flight per vector
+    long long want = (c.g.n / 2 + 255) / 256;
+    long long cap = (long long)c.sm_count * 3;
+    if (cap > PF_MAX_PARTIAL_BLOCKS) cap = PF_MAX_PARTIAL_BLOCKS;
+    const int nb = (int)(want < cap ? (want < 1 ? 1 : want) : cap);
+    const bool vec = (((uintptr_t)kv.y | (uintptr_t)kv.r | (uintptr_t)kv.v_out | (uintptr_t)kv.p_out | (uintptr_t)kv.t |
+                       (uintptr_t)kv.rt) & 15u) == 0;
+    ++g_launch_count;
+    if (vec) k3_update<true><<<nb, 256, 0, c.stream>>>(c.g.n, kv, c.sc, c.rb);
+    else     k3_update<false><<<nb, 256, 0, c.stream>>>(c.g.n, kv, c.sc, c.rb);
+}
+
+void launch_finish_x(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv) {
     const int nb = direct_blocks(c.g.n, c.sm_count);
-    if (precond) { ++g_launch_count; k3_update<true><<<nb, 256, 0, c.stream>>>(c.g.n, op.A0, kv, c.sc, c.rb); }
-    else         { ++g_launch_count; k3_update<false><<<nb, 256, 0, c.stream>>>(c.g.n, op.A0, kv, c.sc, c.rb); }
+    ++g_launch_count;
+    k_finish_x<<<nb, 256, 0, c.stream>>>(c.g.n, op.A0, kv.y, kv.x);
 }
 
 }  // namespace pf

@@ -23,13 +23,24 @@ void launch_residual_direct(const LaunchCtx& c, const Operator& op, const Krylov
 void launch_k1_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
 void launch_k2_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
 void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
+// x += M^-1 y at the end of a preconditioned solve (reading D3).
+void launch_finish_x(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv);
 
-// Tiled family (pf_krylov_tiled.cu).  tiled_supported() says whether the grid fills the tiles.
-bool tiled_supported(const GridDims& g);
-bool tiled_pointers_ok(const KrylovVecs& kv);   // 128-bit accesses need 16-byte aligned x and b
-void launch_residual_tiled(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, int mode);
-void launch_k1_tiled(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
-void launch_k2_tiled(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
+// Tiled family (pf_krylov_tma.cu): TMA-staged planes, z-marched.  Needs an even nx (16-byte row
+// strides) and 16-byte aligned vectors; tma_supported() says whether the grid qualifies.
+struct TmaSet;                                   // tensor maps of one solve (opaque here)
+bool tma_available();                            // driver entry point for tensor-map encoding found
+bool tma_supported(const GridDims& g);
+bool tma_pointers_ok(const KrylovVecs& kv, const Operator& op);
+TmaSet* tma_set_create();
+void tma_set_destroy(TmaSet* t);
+// (Re)build the tensor maps for the vectors and operator of a solve; false on failure.
+bool tma_set_build(TmaSet* t, const GridDims& g, const Operator& op, const KrylovVecs& kv);
+void launch_residual_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, int mode);
+void launch_k1_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond,
+                   int parity /* which of the two (p, v) buffer pairs is the input */);
+void launch_k2_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond,
+                   int parity);
 
 // ---- assembly (pf_assembly.cu) ----------------------------------------------------------------
 struct BcDev { int type[6]; double value[6]; };
@@ -43,18 +54,19 @@ struct Palette {
 cudaError_t scan_eps(cudaStream_t s, long long n, const double* eps, void* scratch, Palette* out,
                      double* eps_min, double* eps_max);
 
-// Poisson operator of Eq (3)/(13) without sigma: diagonal A0, classes, optionally A1..A6.
+// Poisson operator of Eq (3)/(13) without sigma: diagonal A0, stencil codes (code_mode 0 none, 1 uint16,
+// 2 uint32; rows padded to cpitch), optionally A1..A6.
 void launch_assemble_poisson(cudaStream_t s, const GridDims& g, double h, const BcDev& bc, const double* eps,
-                             const Palette& pal, bool use_palette, double* A0, uint8_t* cls,
+                             const Palette& pal, int code_mode, double* A0, void* code, int cpitch,
                              double* const offd[6] /* entries null unless stored */);
 // PF1 operator eps(l_c^2 Lap - 1), sign flipped (Eq (12)), identity rows on the
 // box boundary and outside the solvent (Q15).
 void launch_assemble_pf1(cudaStream_t s, const GridDims& g, double h, double lc, const double* eps, double eps_mid,
-                         bool uniform, const Palette& pal, bool use_palette, double* A0, uint8_t* cls,
+                         bool uniform, const Palette& pal, int code_mode, double* A0, void* code, int cpitch,
                          double* const offd[6]);
-// Coefficient tables of the on-the-fly variant (host side; ncls*ncls doubles each).
-void build_lut_poisson(const Palette& pal, double h, double* lut_host, int* ncls);
-void build_lut_pf1(const Palette& pal, double h, double lc, double* lut_host, int* ncls);
+// Coefficient tables of the on-the-fly variant (host side; PF_CTAB doubles each).
+void build_ctab_poisson(const Palette& pal, double h, double* ctab_host);
+void build_ctab_pf1(const Palette& pal, double h, double lc, double* ctab_host);
 
 // Trilinear deposition of the fixed charges (reading R2): fixed[i] += kappa q w / h^3, in charge order.
 void launch_deposit(cudaStream_t s, const GridDims& g, double h, double kappa, const double* charges_dev, int m,

@@ -28,7 +28,7 @@ KERNELS_AUTO, KERNELS_DIRECT, KERNELS_TILED = 0, 1, 2
 EXPORTS = [
     "pf_grid_create", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
     "pf_solve_linear", "pf_solve_linear_host", "pf_solve_pf", "pf_fermi_pointwise", "pf_grid_history",
-    "pf_grid_linear_iters", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_copy_array",
+    "pf_grid_linear_iters", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_code_layout", "pf_grid_copy_array",
     "pf_grid_profile", "pf_launch_count", "pf_grid_destroy", "pf_last_error", "pf_version",
 ]
 
@@ -77,6 +77,7 @@ def load():
     L.pf_grid_stencil.argtypes = [_vp]
     L.pf_grid_palette_size.argtypes = [_vp]
     L.pf_grid_copy_array.argtypes = [_vp, ctypes.c_int, _vp]
+    L.pf_grid_code_layout.argtypes = [_vp, _ip, _ip, ctypes.POINTER(ctypes.c_size_t)]
     L.pf_grid_profile.argtypes = [_vp, _dp, ctypes.POINTER(ctypes.c_longlong)]
     L.pf_launch_count.restype = ctypes.c_longlong
     L.pf_grid_destroy.argtypes = [_vp]
@@ -218,11 +219,35 @@ def pf_grid_palette_size(handle) -> int:
     return load().pf_grid_palette_size(handle)
 
 
+def pf_grid_code_layout(handle) -> dict:
+    bits, pitch, nbytes = ctypes.c_int(0), ctypes.c_int(0), ctypes.c_size_t(0)
+    _check(handle, load().pf_grid_code_layout(handle, ctypes.byref(bits), ctypes.byref(pitch), ctypes.byref(nbytes)))
+    return dict(bits=bits.value, pitch=pitch.value, bytes=nbytes.value)
+
+
 def pf_grid_copy_array(handle, which: int, n: int) -> torch.Tensor:
-    """Copy of an assembled device array (tests): 0 diag, 1..6 off-diagonals, 7 fixed charges, 8 classes, 9 PF1 diag."""
-    out = torch.empty(n, dtype=torch.uint8 if which == 8 else torch.float64, device="cuda")
+    """Copy of an assembled device array (tests): 0 diag, 1..6 off-diagonals, 7 fixed charges, 8 / 11 stencil
+    codes (raw bytes), 9 PF1 diag, 10 / 12 coefficient tables (16 doubles)."""
+    if which in (8, 11):
+        out = torch.empty(pf_grid_code_layout(handle)["bytes"], dtype=torch.uint8, device="cuda")
+    elif which in (10, 12):
+        out = torch.empty(16, dtype=torch.float64, device="cuda")
+    else:
+        out = torch.empty(n, dtype=torch.float64, device="cuda")
     _check(handle, load().pf_grid_copy_array(handle, which, out.data_ptr()))
     return out
+
+
+def decode_offdiagonals(handle, nx: int, ny: int, nz: int, pf1: bool = False):
+    """Off-diagonals A1..A6 (numpy, 6 x N) that the on-the-fly stencil codes and table stand for."""
+    lay = pf_grid_code_layout(handle)
+    raw = pf_grid_copy_array(handle, 11 if pf1 else 8, 0).cpu().numpy()
+    tab = pf_grid_copy_array(handle, 12 if pf1 else 10, 0).cpu().numpy()
+    dt = np.uint16 if lay["bits"] == 16 else np.uint32
+    fb = 2 if lay["bits"] == 16 else 4
+    codes = raw[: lay["pitch"] * ny * nz * (lay["bits"] // 8)].view(dt).reshape(nz, ny, lay["pitch"])[:, :, :nx]
+    codes = codes.reshape(-1).astype(np.uint32)
+    return np.stack([tab[(codes >> (fb * d)) & ((1 << fb) - 1)] for d in range(6)])
 
 
 def pf_grid_destroy(handle) -> None:

@@ -60,7 +60,49 @@ def test_assembly_bit_exact(pf, oracle, which):
     g.close()
     g = pf.Grid.from_workload(w, stencil=pf.STENCIL_ONTHEFLY)
     assert pf.pf_grid_stencil(g.handle) == 2 and pf.pf_grid_palette_size(g.handle) == 2
+    assert pf.pf_grid_code_layout(g.handle)["bits"] == 16
     assert np.array_equal(pf.pf_grid_copy_array(g.handle, 0, w.n).cpu().numpy(), A[0])
+    # the packed stencil codes + coefficient table stand for exactly the oracle's A1..A6
+    offd = pf.decode_offdiagonals(g.handle, w.nx, w.ny, w.nz)
+    for d in range(1, 7):
+        assert np.array_equal(offd[d - 1], A[d]), f"decoded A{d}"
+    g.close()
+
+
+@pytest.mark.parametrize("levels", [3, 4])
+def test_assembly_codes_four_level_map(pf, oracle, levels):
+    """Maps with 3 or 4 distinct eps values use 32-bit codes (4-bit fields); decoded rows and the PF1
+    operator are bit-exact, and a solve through the tiled kernels matches the oracle."""
+    w = ragged_workload(nx=40, ny=18, nz=12, seed=21)
+    rng = wl.SplitMix64(22)
+    vals = [2.0, 4.0, 20.0, 78.5][:levels]
+    w.eps = np.array([vals[int(rng.uniform() * levels) % levels] for _ in range(w.n)])
+    A = oracle.assemble_poisson(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps)
+    g = pf.Grid.from_workload(w, stencil=pf.STENCIL_ONTHEFLY, kernels=2)
+    assert pf.pf_grid_code_layout(g.handle)["bits"] == 32 and pf.pf_grid_palette_size(g.handle) == levels
+    offd = pf.decode_offdiagonals(g.handle, w.nx, w.ny, w.nz)
+    for d in range(1, 7):
+        assert np.array_equal(offd[d - 1], A[d]), f"decoded A{d}"
+    ref = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, w.rhs, tol=1e-10)
+    out = g.solve_linear(w.rhs, tol=1e-10)
+    assert out["status"] == 0 and abs(out["iters"] - ref["iters"]) <= max(1, 0.02 * ref["iters"])
+    assert rel_l2(out["x"].cpu().numpy(), ref["x"]) <= 1e-9
+    g.close()
+
+
+def test_assembly_pf1_codes(pf, oracle):
+    """PF1 operator (row N2): diagonal and decoded off-diagonals bit-exact after a (capped) PF solve."""
+    w = wl.config0()
+    sp = w.species
+    solvent = oracle.solvent_mask(w.eps)
+    A1 = oracle.assemble_pf1(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, solvent, w.l_c)
+    g = pf.Grid.from_workload(w, stencil=pf.STENCIL_ONTHEFLY,
+                              options={pf.PF_OPT_MAX_OUTER: 1, pf.PF_OPT_LINEAR_MAXIT: 2})
+    g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol, want_conc=False)
+    assert np.array_equal(pf.pf_grid_copy_array(g.handle, 9, w.n).cpu().numpy(), A1[0])
+    offd = pf.decode_offdiagonals(g.handle, w.nx, w.ny, w.nz, pf1=True)
+    for d in range(1, 7):
+        assert np.array_equal(offd[d - 1], A1[d]), f"decoded PF1 A{d}"
     g.close()
 
 
