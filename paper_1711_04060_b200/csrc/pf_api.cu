@@ -147,7 +147,7 @@ LaunchCtx make_ctx(const pf_grid* g) {
 // ---- Table 3 on the device ----------------------------------------------------------------
 // b: device N with Dirichlet values already forced; x: device N, in/out, Dirichlet values forced.
 int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, double tol, int maxit,
-                    int* iters_out, double* relres_out, double* true_relres_out) {
+                    int* iters_out, double* relres_out, double* true_relres_out, bool allow_tiled = true) {
     if (maxit < 0) return fail(g, PF_ERR_ARG, "maxit < 0");
     if (!(tol >= 0.0)) return fail(g, PF_ERR_ARG, "tol must be >= 0");
     const LaunchCtx c = make_ctx(g);
@@ -163,12 +163,13 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     // D3: with the Jacobi preconditioner step 16 accumulates y = sum(alpha p + omega s); x = x0 + M^-1 y at the end
     kv.y = precond ? g->y : x;
     if (precond) PF_CUDA(g, cudaMemsetAsync(g->y, 0, sizeof(double) * g->g.n, g->stream));
-    bool tiled = use_tiled(g) && tma_pointers_ok(kv, op);
+    bool tiled = allow_tiled && use_tiled(g) && tma_pointers_ok(kv, op);
     if (tiled && !tma_set_build(g->tma, g->g, op, kv)) {
         if (g->opt_kernels == 2) return fail(g, PF_ERR_CUDA, "tensor-map encoding failed");
         tiled = false;
     }
-    if (g->opt_kernels == 2 && !tiled) return fail(g, PF_ERR_ARG, "tiled kernels need 16-byte aligned vectors");
+    if (g->opt_kernels == 2 && allow_tiled && !tiled)
+        return fail(g, PF_ERR_ARG, "tiled kernels need 16-byte aligned vectors");
     if (tiled) launch_residual_tma(c, op, kv, g->tma, 0); else launch_residual_direct(c, op, kv, 0);
 
     const int chunk = g->opt_check < 1 ? 1 : g->opt_check;
@@ -212,6 +213,12 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
             done = true;
         }
         slot ^= 1;
+    }
+    if (tiled && fin.fault) {
+        // operands outside the range of the tiled kernels' branch-free division (pf_common.cuh dvd_nb): x has
+        // not been touched yet (D3), so the solve is simply repeated with the kernels that use __ddiv_rn
+        PF_CUDA(g, cudaStreamSynchronize(g->stream));
+        return bicgstab_device(g, op, b, x, tol, maxit, iters_out, relres_out, true_relres_out, false);
     }
     if (precond) launch_finish_x(c, op, kv);
     PF_CUDA(g, cudaStreamSynchronize(g->stream));

@@ -1,12 +1,17 @@
 // pf_krylov_tma.cu -- the fused stencil kernels of the BiCGSTAB iteration for B200: planes staged in
-// shared memory by TMA, z marched in registers.
+// shared memory by TMA, z marched in registers, warp-specialised.
 //
-// Work decomposition.  The xy plane is cut into tiles of TX x TY = 64 x 16 nodes; a block of 512 threads
-// (warp = one 512-byte row, lane = two x-adjacent nodes) marches its tile along z over a chunk of planes.
-// One elected thread keeps a ring of S stages filled: per plane one 3-D tensor-map copy
-// (cp.async.bulk.tensor, completion on an mbarrier) per operand, of the tile PLUS its halo ring -- box
-// (TX+4) x (TY+2) so that every thread's pair of nodes is 16-byte aligned in shared memory.  Nodes outside
-// the grid are zero-filled by the TMA unit, so no thread computes an address or a bounds test for a load.
+// Work decomposition.  The xy plane is cut into tiles of TX x TY = 64 x 16 nodes; a block marches its tile
+// along z over a chunk of planes.  Roles of its 19 warps:
+//   producer (1 warp, one lane)  keeps a ring of S stages filled: per plane one 3-D tensor-map copy
+//       (cp.async.bulk.tensor, completion on a "full" mbarrier) per operand, of the tile PLUS its halo ring --
+//       box (TX+4) x (TY+2) so that every thread's pair of nodes is 16-byte aligned in shared memory.  Nodes
+//       outside the grid are zero-filled by the TMA unit: no thread computes an address or a bounds test for
+//       a load.  A stage is refilled as soon as the 18 consumer warps have released it ("empty" mbarrier).
+//   main (16 warps)  warp = one 512-byte tile row, lane = two x-adjacent nodes: form u at the own nodes,
+//       difference the plane, store, accumulate the inner products.
+//   halo (2 warps)   form u on the halo ring (rows y0-1 and y0+TY, columns x0-1 and x0+TX), off the main
+//       warps' critical path.
 //
 // What is fused (rows L3-L5 of DESIGN.md).  The vector update that precedes a matvec in Table 3
 // is recomputed on the fly at the tile AND at its halo ring, so the updated vector is
@@ -15,8 +20,9 @@
 //   MODE_K2  u = M^-1 (r - alpha v)             (step 13),            t  = A u (step 14), t.s, t.t
 //   MODE_R0  u = x,  r = b - A u, r~ = r, b.b, r.r (step 2);  MODE_R1: ||b - A x||^2 only
 // u of the plane being differenced sits in shared memory (xy neighbours, double-buffered); the z
-// neighbours stay in registers of the marching thread.  Per plane: wait for the stage, form u(z+1),
-// difference plane z, one __syncthreads, refill the stage just consumed (S-1 planes of loads in flight).
+// neighbours stay in registers of the marching thread (three register slots renamed, not moved, by a
+// three-way unrolled loop).  Per plane: wait for the stage, form u(z+1), release the stage, difference
+// plane z, one named barrier among the consumer warps.
 //
 // Arithmetic is the same statement for statement as the direct kernels (pf_krylov_direct.cu): both
 // families give bit-identical vectors.
@@ -32,14 +38,15 @@ namespace pf {
 namespace {
 
 constexpr int TX = 64;                   // tile width in nodes (32 lanes x 2)
-constexpr int TY = 16;                   // tile height = warps per block
-constexpr int NT = 32 * TY;
+constexpr int TY = 16;                   // tile height = main warps per block
+constexpr int NW_CONSUMER = TY + 2;      // 16 main warps (one tile row each) + 2 halo warps
+constexpr int NT_CONSUMER = 32 * NW_CONSUMER;
+constexpr int NT = NT_CONSUMER + 32;     // + the producer warp
 constexpr int BX = TX + 4;               // box: two halo columns each side (one used; two keep 16-byte alignment)
 constexpr int BY = TY + 2;
 constexpr int FIELD_BYTES = ((BX * BY * 8 + 127) / 128) * 128;   // 9856
 constexpr int OWN_BYTES = TX * TY * 8;                            // 8192
-constexpr int NHALO = 2 * TX + 2 * TY;                            // 160 halo nodes per plane
-static_assert(NHALO <= NT, "one halo node per thread");
+static_assert(TY <= 32, "one halo column node per lane of a halo warp");
 
 enum { MODE_R0 = 0, MODE_R1 = 1, MODE_K1 = 2, MODE_K2 = 3 };
 
@@ -69,7 +76,7 @@ struct Layout {
     static constexpr int CTAB_OFF = U_OFF + 2 * FIELD_BYTES;
     static constexpr int SCRATCH_OFF = CTAB_OFF + PF_CTAB * 8;
     static constexpr int BAR_OFF = SCRATCH_OFF + 2 * 32 * (int)sizeof(dd);
-    static constexpr int TOTAL = BAR_OFF + 8 * T::STAGES;
+    static constexpr int TOTAL = BAR_OFF + 16 * T::STAGES;           // full[S], empty[S]
     static constexpr unsigned TX_BYTES = (unsigned)(T::NF * BX * BY * 8 + (T::OWN ? OWN_BYTES : 0) + CODE_BYTES);
 };
 
@@ -105,11 +112,11 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
 
 template <int MODE, bool PRECOND>
 __device__ __forceinline__ double u_of(double r, double p, double v, double a, bool first, double c1, double c2,
-                                       double& numer) {
-    if (MODE == MODE_K1) { numer = p_new_at<PRECOND>(first, c1, c2, r, p, v); return jacobi<PRECOND>(numer, a); }
-    if (MODE == MODE_K2) { numer = s_at(c1, r, v); return jacobi<PRECOND>(numer, a); }
-    numer = r;           // residual modes: the field is x itself (passed in r)
-    return r;
+                                       double& numer, unsigned& fault) {
+    if (MODE == MODE_K1) numer = p_new_at<PRECOND>(first, c1, c2, r, p, v);
+    else if (MODE == MODE_K2) numer = s_at(c1, r, v);
+    else { numer = r; return r; }    // residual modes: the field is x itself (passed in r)
+    return PRECOND ? dvd_nb(numer, a, fault) : numer;   // == jacobi<PRECOND>(numer, a) of the direct kernels
 }
 
 // Byte offset into the coefficient table of field d of node e (0 or 1) of the thread's code word(s).
@@ -125,6 +132,20 @@ __device__ __forceinline__ unsigned ctab_off(unsigned w0, unsigned w1, int e, in
     }
 }
 
+// Registers of one plane of a main thread: u at its two nodes, the numerators (p' or s), the diagonal,
+// the own-only operand (r~ or b) and the stencil code word(s).
+struct Slot {
+    double u[2], n[2], a[2];
+    double2 w;
+    unsigned k0, k1;
+};
+
+__device__ __forceinline__ void consumer_barrier() { asm volatile("bar.sync 1, %0;" ::"n"(NT_CONSUMER) : "memory"); }
+
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
 template <int MODE, bool PRECOND, bool STORED, bool CODE32>
 __global__ void __launch_bounds__(NT, 1)
 k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb, int zchunk) {
@@ -136,195 +157,198 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     extern __shared__ __align__(128) unsigned char smem[];
     double* ctab_s = reinterpret_cast<double*>(smem + L::CTAB_OFF);
     dd* scratch = reinterpret_cast<dd*>(smem + L::SCRATCH_OFF);
-    unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem + L::BAR_OFF);
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + L::BAR_OFF);
+    unsigned long long* empty = full + S;
 
-    const int tid = threadIdx.x, lane = tid & 31, ty = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
     const int z0 = blockIdx.z * zchunk, z1 = min(z0 + zchunk, g.nz);
+    const int nq = z1 - z0 + 2;            // plane q of this block's load sequence is z0 - 1 + q
 
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < S; ++s) mbar_init(&bars[s], 1);
+        for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW_CONSUMER); }
         fence_proxy_async();
     }
     if (!STORED && tid < PF_CTAB) ctab_s[tid] = op.ctab[tid];
     __syncthreads();
 
-    // plane q of this block's load sequence is z0 - 1 + q; q = 0 .. nq-1
-    const int nq = z1 - z0 + 2;
-    auto issue = [&](int q) {                       // tid 0 only
-        const int s = q % S;
-        unsigned char* st = smem + s * L::STAGE_BYTES;
-        const int z = z0 - 1 + q;
-        mbar_expect_tx(&bars[s], L::TX_BYTES);
-#pragma unroll
-        for (int f = 0; f < NF; ++f) tma_load_3d(st + f * FIELD_BYTES, &tm.f[f], &bars[s], x0 - 2, y0 - 1, z);
-        if (T::OWN) tma_load_3d(st + L::OWN_OFF, &tm.own, &bars[s], x0, y0, z);
-        if (!STORED) tma_load_3d(st + L::CODE_OFF, &tm.code, &bars[s], x0, y0, z);
-    };
-    if (tid == 0)
-        for (int q = 0; q < S && q < nq; ++q) issue(q);
-
-    bool first = false; double c1 = 0.0, c2 = 0.0;
-    if (MODE == MODE_K1) { first = sc->first != 0; c1 = sc->beta; c2 = sc->omega; }
-    else if (MODE == MODE_K2) { c1 = sc->alpha; }
-
-    // own slot: nodes (x, y) and (x+1, y); nx is even so both are inside or both outside
-    const int x = x0 + 2 * lane, y = y0 + ty;
-    const bool own_ok = x < g.nx && y < g.ny;
-    const long long plane = (long long)g.nx * g.ny;
-    const long long own_off = x + (long long)g.nx * y;
-    const int own_box = (ty + 1) * BX + 2 + 2 * lane;              // element offset in a halo box
-    const int own_tile = ty * TX + 2 * lane;                        // element offset in an own-only box
-    // halo slot: one node per thread, threads 0..NHALO-1
-    int hbox = 0; bool h_ok = false;
-    const bool h_any = tid < NHALO;
-    if (h_any) {
-        int hx, hy;
-        if (tid < TX)            { hx = 2 + tid;        hy = 0; }
-        else if (tid < 2 * TX)   { hx = 2 + tid - TX;   hy = BY - 1; }
-        else if (tid < 2 * TX + TY) { hx = 1;           hy = 1 + tid - 2 * TX; }
-        else                     { hx = BX - 2;         hy = 1 + tid - 2 * TX - TY; }
-        hbox = hy * BX + hx;
-        const int gx = x0 - 2 + hx, gy = y0 - 1 + hy;
-        h_ok = gx >= 0 && gx < g.nx && gy >= 0 && gy < g.ny;
-    }
-
-    double u_dn[2] = {0, 0}, u_c[2] = {0, 0}, u_up[2] = {0, 0};
-    double n_c[2] = {0, 0}, n_up[2] = {0, 0};              // numerators: p' (K1) or s (K2)
-    double a_c[2] = {1, 1}, a_up[2] = {1, 1};
-    double2 w_c = make_double2(0, 0), w_up = make_double2(0, 0);    // own-only operand: r~ (K1) or b (R0/R1)
-    unsigned k0_c = 0, k1_c = 0, k0_up = 0, k1_up = 0;              // code word(s) of the thread's two nodes
-
-    // form u of plane z0-1+q from its stage: own nodes -> registers (+ shared), halo nodes -> shared
-    auto prepare = [&](int q, bool to_shared) {
-        const int s = q % S;
-        const unsigned par = (unsigned)(q / S) & 1u;
-        while (!mbar_try_wait(&bars[s], par)) {}
-        const unsigned char* st = smem + s * L::STAGE_BYTES;
-        const int z = z0 - 1 + q;
-        const bool zin = z >= 0 && z < g.nz;
-        double* u_s = reinterpret_cast<double*>(smem + L::U_OFF + (q & 1) * FIELD_BYTES);
-        const double* F0 = reinterpret_cast<const double*>(st);
-        const double* F1 = reinterpret_cast<const double*>(st + FIELD_BYTES);
-        const double* F2 = reinterpret_cast<const double*>(st + 2 * FIELD_BYTES);
-        const double* F3 = reinterpret_cast<const double*>(st + 3 * FIELD_BYTES);
-        double2 fr = *reinterpret_cast<const double2*>(F0 + own_box), fp = make_double2(0, 0), fv = make_double2(0, 0), fa;
-        if (MODE == MODE_K1) {
-            fp = *reinterpret_cast<const double2*>(F1 + own_box);
-            fv = *reinterpret_cast<const double2*>(F2 + own_box);
-            fa = *reinterpret_cast<const double2*>(F3 + own_box);
-        } else if (MODE == MODE_K2) {
-            fv = *reinterpret_cast<const double2*>(F1 + own_box);
-            fa = *reinterpret_cast<const double2*>(F2 + own_box);
-        } else {
-            fa = *reinterpret_cast<const double2*>(F1 + own_box);
-        }
-        const bool ok = own_ok && zin;
-        if (!ok) fa = make_double2(1.0, 1.0);                       // zero-filled nodes: keep u finite (0/1)
-        u_up[0] = u_of<MODE, PRECOND>(fr.x, fp.x, fv.x, fa.x, first, c1, c2, n_up[0]);
-        u_up[1] = u_of<MODE, PRECOND>(fr.y, fp.y, fv.y, fa.y, first, c1, c2, n_up[1]);
-        a_up[0] = fa.x; a_up[1] = fa.y;
-        if (T::OWN) w_up = *reinterpret_cast<const double2*>(reinterpret_cast<const double*>(st + L::OWN_OFF) + own_tile);
-        if (!STORED) {
-            if (CODE32) {
-                const uint2 cw = *reinterpret_cast<const uint2*>(st + L::CODE_OFF + 4 * own_tile);
-                k0_up = cw.x; k1_up = cw.y;
-            } else {
-                k0_up = *reinterpret_cast<const unsigned*>(st + L::CODE_OFF + 2 * own_tile);
-            }
-        }
-        if (MODE == MODE_K1 && ok && z >= z0 && z < z1)             // p' is an output of steps 5-9
-            *reinterpret_cast<double2*>(kv.p_out + own_off + plane * z) = make_double2(n_up[0], n_up[1]);
-        if (to_shared) {
-            *reinterpret_cast<double2*>(u_s + own_box) = make_double2(u_up[0], u_up[1]);
-            if (h_any) {
-                double hr = F0[hbox], hp = 0.0, hv = 0.0, ha;
-                if (MODE == MODE_K1) { hp = F1[hbox]; hv = F2[hbox]; ha = F3[hbox]; }
-                else if (MODE == MODE_K2) { hv = F1[hbox]; ha = F2[hbox]; }
-                else ha = 1.0;
-                if (!(h_ok && zin)) ha = 1.0;
-                double dummy;
-                u_s[hbox] = u_of<MODE, PRECOND>(hr, hp, hv, ha, first, c1, c2, dummy);
-            }
-        }
-    };
-    auto rotate = [&]() {
-#pragma unroll
-        for (int e = 0; e < 2; ++e) {
-            u_dn[e] = u_c[e]; u_c[e] = u_up[e]; n_c[e] = n_up[e]; a_c[e] = a_up[e];
-        }
-        w_c = w_up; k0_c = k0_up; k1_c = k1_up;
-    };
-
     dd q[2] = {dd_zero(), dd_zero()};
+    unsigned fault = 0u;
 
-    prepare(0, false); rotate();           // plane z0-1: registers only
-    prepare(1, true);  rotate();           // plane z0
-    __syncthreads();
-    if (tid == 0) {                        // stages of q = 0, 1 are consumed
-        if (S + 0 < nq) issue(S + 0);
-        if (S + 1 < nq) issue(S + 1);
-    }
-
-    for (int z = z0; z < z1; ++z) {
-        const int qn = z - z0 + 2;         // load-sequence index of plane z+1
-        const long long i = own_off + plane * z;
-        double2 cf[6];
-        if (STORED && own_ok) {
+    if (wid == NW_CONSUMER) {
+        // ---- producer warp: one lane keeps the ring of stages filled ----------------------------
+        if (lane == 0) {
+            for (int k = 0; k < nq; ++k) {
+                const int s = k % S;
+                if (k >= S) { const unsigned par = (unsigned)(k / S - 1) & 1u; while (!mbar_try_wait(&empty[s], par)) {} }
+                unsigned char* st = smem + s * L::STAGE_BYTES;
+                const int z = z0 - 1 + k;
+                mbar_expect_tx(&full[s], L::TX_BYTES);
 #pragma unroll
-            for (int d = 0; d < 6; ++d) cf[d] = *reinterpret_cast<const double2*>(op.offd[d] + i);
+                for (int f = 0; f < NF; ++f) tma_load_3d(st + f * FIELD_BYTES, &tm.f[f], &full[s], x0 - 2, y0 - 1, z);
+                if (T::OWN) tma_load_3d(st + L::OWN_OFF, &tm.own, &full[s], x0, y0, z);
+                if (!STORED) tma_load_3d(st + L::CODE_OFF, &tm.code, &full[s], x0, y0, z);
+            }
         }
-        prepare(qn, true);                 // u(z+1): registers + the other shared buffer
-        if (own_ok) {
-            const double* u_s = reinterpret_cast<const double*>(smem + L::U_OFF + ((qn - 1) & 1) * FIELD_BYTES);
-            const double2 us = *reinterpret_cast<const double2*>(u_s + own_box - BX);
-            const double2 un = *reinterpret_cast<const double2*>(u_s + own_box + BX);
-            const double uw = u_s[own_box - 1], ue = u_s[own_box + 2];
+        __syncwarp();
+    } else {
+        bool first = false; double c1 = 0.0, c2 = 0.0;
+        if (MODE == MODE_K1) { first = sc->first != 0; c1 = sc->beta; c2 = sc->omega; }
+        else if (MODE == MODE_K2) { c1 = sc->alpha; }
+        const bool is_main = wid < TY;
+        // main thread: nodes (x, y) and (x+1, y) of box row wid+1; nx is even so both are inside or both outside.
+        // halo warp TY: box row 0 (pairs) and box column 1 (lanes 0..15); halo warp TY+1: row BY-1 and column BX-2.
+        const int brow = is_main ? wid + 1 : (wid == TY ? 0 : BY - 1);
+        const int x = x0 + 2 * lane, y = y0 - 1 + brow;
+        const bool pair_ok = x < g.nx && y >= 0 && y < g.ny;
+        const long long plane = (long long)g.nx * g.ny;
+        const long long own_off = x + (long long)g.nx * y;
+        const int pair_box = brow * BX + 2 + 2 * lane;                 // element offset in a halo box
+        const int own_tile = (brow - 1) * TX + 2 * lane;               // element offset in an own-only box (main)
+        int col_box = 0; bool col_ok = false;
+        const bool col_any = !is_main && lane < TY;
+        if (col_any) {
+            const int hx = wid == TY ? 1 : BX - 2, hy = 1 + lane;
+            col_box = hy * BX + hx;
+            const int gx = x0 - 2 + hx, gy = y0 - 1 + hy;
+            col_ok = gx >= 0 && gx < g.nx && gy < g.ny;
+        }
+
+        // form u of plane z0-1+k from its stage: main nodes -> slot (+ shared), halo nodes -> shared
+        auto prepare = [&](int k, Slot& up, bool to_shared) {
+            const int s = k % S;
+            const unsigned par = (unsigned)(k / S) & 1u;
+            while (!mbar_try_wait(&full[s], par)) {}
+            const unsigned char* st = smem + s * L::STAGE_BYTES;
+            const int z = z0 - 1 + k;
+            const bool zin = z >= 0 && z < g.nz;
+            double* u_s = reinterpret_cast<double*>(smem + L::U_OFF + (k & 1) * FIELD_BYTES);
+            const double* F0 = reinterpret_cast<const double*>(st);
+            const double* F1 = reinterpret_cast<const double*>(st + FIELD_BYTES);
+            const double* F2 = reinterpret_cast<const double*>(st + 2 * FIELD_BYTES);
+            const double* F3 = reinterpret_cast<const double*>(st + 3 * FIELD_BYTES);
+            if (is_main || to_shared) {
+                double2 fr = *reinterpret_cast<const double2*>(F0 + pair_box), fp = make_double2(0, 0),
+                        fv = make_double2(0, 0), fa;
+                if (MODE == MODE_K1) {
+                    fp = *reinterpret_cast<const double2*>(F1 + pair_box);
+                    fv = *reinterpret_cast<const double2*>(F2 + pair_box);
+                    fa = *reinterpret_cast<const double2*>(F3 + pair_box);
+                } else if (MODE == MODE_K2) {
+                    fv = *reinterpret_cast<const double2*>(F1 + pair_box);
+                    fa = *reinterpret_cast<const double2*>(F2 + pair_box);
+                } else {
+                    fa = *reinterpret_cast<const double2*>(F1 + pair_box);
+                }
+                const bool ok = pair_ok && zin;
+                if (!ok) fa = make_double2(1.0, 1.0);                   // zero-filled nodes: keep u finite (0/1)
+                up.u[0] = u_of<MODE, PRECOND>(fr.x, fp.x, fv.x, fa.x, first, c1, c2, up.n[0], fault);
+                up.u[1] = u_of<MODE, PRECOND>(fr.y, fp.y, fv.y, fa.y, first, c1, c2, up.n[1], fault);
+                up.a[0] = fa.x; up.a[1] = fa.y;
+                if (is_main) {
+                    if (T::OWN)
+                        up.w = *reinterpret_cast<const double2*>(reinterpret_cast<const double*>(st + L::OWN_OFF) + own_tile);
+                    if (!STORED) {
+                        if (CODE32) {
+                            const uint2 cw = *reinterpret_cast<const uint2*>(st + L::CODE_OFF + 4 * own_tile);
+                            up.k0 = cw.x; up.k1 = cw.y;
+                        } else {
+                            up.k0 = *reinterpret_cast<const unsigned*>(st + L::CODE_OFF + 2 * own_tile);
+                        }
+                    }
+                    if (MODE == MODE_K1 && ok && z >= z0 && z < z1)     // p' is an output of steps 5-9
+                        *reinterpret_cast<double2*>(kv.p_out + own_off + plane * z) = make_double2(up.n[0], up.n[1]);
+                }
+                if (to_shared) *reinterpret_cast<double2*>(u_s + pair_box) = make_double2(up.u[0], up.u[1]);
+            }
+            if (col_any && to_shared) {
+                double hr = F0[col_box], hp = 0.0, hv = 0.0, ha;
+                if (MODE == MODE_K1) { hp = F1[col_box]; hv = F2[col_box]; ha = F3[col_box]; }
+                else if (MODE == MODE_K2) { hv = F1[col_box]; ha = F2[col_box]; }
+                else ha = 1.0;
+                if (!(col_ok && zin)) ha = 1.0;
+                double dummy;
+                u_s[col_box] = u_of<MODE, PRECOND>(hr, hp, hv, ha, first, c1, c2, dummy, fault);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);                      // this warp is done with the stage
+        };
+        // difference plane z (slot c) with its z neighbours in slots dn and up; xy neighbours from shared
+        auto compute = [&](int z, const Slot& dn, const Slot& c, const Slot& up) {
+            const int k = z - z0 + 1;
+            const long long i = own_off + plane * z;
+            const double* u_s = reinterpret_cast<const double*>(smem + L::U_OFF + (k & 1) * FIELD_BYTES);
+            const double2 us = *reinterpret_cast<const double2*>(u_s + pair_box - BX);
+            const double2 un = *reinterpret_cast<const double2*>(u_s + pair_box + BX);
+            const double uw = u_s[pair_box - 1], ue = u_s[pair_box + 2];
+            double2 cf[6];
+            if (STORED) {
+#pragma unroll
+                for (int d = 0; d < 6; ++d) cf[d] = *reinterpret_cast<const double2*>(op.offd[d] + i);
+            }
             double out[2];
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                double c[6];
+                double cc[6];
                 if (STORED) {
 #pragma unroll
-                    for (int d = 0; d < 6; ++d) c[d] = e == 0 ? cf[d].x : cf[d].y;
+                    for (int d = 0; d < 6; ++d) cc[d] = e == 0 ? cf[d].x : cf[d].y;
                 } else {
 #pragma unroll
                     for (int d = 0; d < 6; ++d)
-                        c[d] = *reinterpret_cast<const double*>(reinterpret_cast<const unsigned char*>(ctab_s) +
-                                                                ctab_off<CODE32>(k0_c, k1_c, e, d));
+                        cc[d] = *reinterpret_cast<const double*>(reinterpret_cast<const unsigned char*>(ctab_s) +
+                                                                 ctab_off<CODE32>(c.k0, c.k1, e, d));
                 }
-                double acc = mul(a_c[e], u_c[e]);
-                acc = add(acc, mul(c[0], e == 0 ? u_c[1] : ue));
-                acc = add(acc, mul(c[1], e == 1 ? u_c[0] : uw));
-                acc = add(acc, mul(c[2], e == 0 ? us.x : us.y));
-                acc = add(acc, mul(c[3], e == 0 ? un.x : un.y));
-                acc = add(acc, mul(c[4], u_dn[e]));
-                acc = add(acc, mul(c[5], u_up[e]));
+                double acc = mul(c.a[e], c.u[e]);
+                acc = add(acc, mul(cc[0], e == 0 ? c.u[1] : ue));
+                acc = add(acc, mul(cc[1], e == 1 ? c.u[0] : uw));
+                acc = add(acc, mul(cc[2], e == 0 ? us.x : us.y));
+                acc = add(acc, mul(cc[3], e == 0 ? un.x : un.y));
+                acc = add(acc, mul(cc[4], dn.u[e]));
+                acc = add(acc, mul(cc[5], up.u[e]));
                 out[e] = acc;
             }
             if (MODE == MODE_K1) {
                 *reinterpret_cast<double2*>(kv.v_out + i) = make_double2(out[0], out[1]);
-                dd_fma(q[0], w_c.x, out[0]); dd_fma(q[1], w_c.y, out[1]);
+                dd_fma(q[0], c.w.x, out[0]); dd_fma(q[1], c.w.y, out[1]);
             } else if (MODE == MODE_K2) {
                 *reinterpret_cast<double2*>(kv.t + i) = make_double2(out[0], out[1]);
-                dd_fma(q[0], out[0], n_c[0]); dd_fma(q[0], out[1], n_c[1]);
+                dd_fma(q[0], out[0], c.n[0]); dd_fma(q[0], out[1], c.n[1]);
                 dd_fma(q[1], out[0], out[0]); dd_fma(q[1], out[1], out[1]);
             } else {
-                const double r0 = sub(w_c.x, out[0]), r1 = sub(w_c.y, out[1]);
+                const double r0 = sub(c.w.x, out[0]), r1 = sub(c.w.y, out[1]);
                 if (MODE == MODE_R0) {
                     *reinterpret_cast<double2*>(kv.r + i) = make_double2(r0, r1);
                     *reinterpret_cast<double2*>(kv.rt + i) = make_double2(r0, r1);
-                    dd_fma(q[0], w_c.x, w_c.x); dd_fma(q[0], w_c.y, w_c.y);
+                    dd_fma(q[0], c.w.x, c.w.x); dd_fma(q[0], c.w.y, c.w.y);
                 }
                 dd_fma(q[1], r0, r0); dd_fma(q[1], r1, r1);
             }
+        };
+        // one plane: u(z+1) into slot up and the other shared buffer, difference plane z, barrier
+        auto step = [&](int z, const Slot& dn, const Slot& c, Slot& up) {
+            prepare(z - z0 + 2, up, true);
+            if (is_main && pair_ok) compute(z, dn, c, up);
+            consumer_barrier();
+        };
+
+        Slot s0, s1, s2;
+        s0.w = s1.w = s2.w = make_double2(0, 0);
+        s0.k0 = s0.k1 = s1.k0 = s1.k1 = s2.k0 = s2.k1 = 0u;
+        prepare(0, s0, false);                 // plane z0-1: registers only
+        prepare(1, s1, true);                  // plane z0
+        consumer_barrier();
+        for (int z = z0; z < z1; z += 3) {     // slots rotate by renaming, not by moving registers
+            step(z, s0, s1, s2);
+            if (z + 1 >= z1) break;
+            step(z + 1, s1, s2, s0);
+            if (z + 2 >= z1) break;
+            step(z + 2, s2, s0, s1);
         }
-        rotate();
-        __syncthreads();
-        if (tid == 0 && qn + S < nq) issue(qn + S);     // the stage of plane z+1 is consumed: refill it
     }
 
+    if (fault) sc->fault = 1;              // the host repeats the solve with the __ddiv_rn kernels
     if (MODE == MODE_K1) {
         dd_add(q[0], q[1]);                // two chains for instruction-level parallelism, one quantity
         dd q1[1] = {q[0]};
