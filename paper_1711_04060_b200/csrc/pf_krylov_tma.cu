@@ -206,145 +206,176 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
         const long long own_off = x + (long long)g.nx * y;
         const int pair_box = brow * BX + 2 + 2 * lane;                 // element offset in a halo box
         const int own_tile = (brow - 1) * TX + 2 * lane;               // element offset in an own-only box (main)
-        int col_box = 0; bool col_ok = false;
-        const bool col_any = !is_main && lane < TY;
-        if (col_any) {
-            const int hx = wid == TY ? 1 : BX - 2, hy = 1 + lane;
-            col_box = hy * BX + hx;
-            const int gx = x0 - 2 + hx, gy = y0 - 1 + hy;
-            col_ok = gx >= 0 && gx < g.nx && gy < g.ny;
-        }
 
-        // form u of plane z0-1+k from its stage: main nodes -> slot (+ shared), halo nodes -> shared
-        auto prepare = [&](int k, Slot& up, bool to_shared) {
-            const int s = k % S;
-            const unsigned par = (unsigned)(k / S) & 1u;
-            while (!mbar_try_wait(&full[s], par)) {}
-            const unsigned char* st = smem + s * L::STAGE_BYTES;
-            const int z = z0 - 1 + k;
-            const bool zin = z >= 0 && z < g.nz;
-            double* u_s = reinterpret_cast<double*>(smem + L::U_OFF + (k & 1) * FIELD_BYTES);
+        // operands of the thread's pair of nodes in plane z0-1+k -> u, numerator, diagonal
+        auto form_pair = [&](const unsigned char* st, bool ok, double (&u)[2], double (&n)[2], double (&a)[2]) {
             const double* F0 = reinterpret_cast<const double*>(st);
             const double* F1 = reinterpret_cast<const double*>(st + FIELD_BYTES);
             const double* F2 = reinterpret_cast<const double*>(st + 2 * FIELD_BYTES);
             const double* F3 = reinterpret_cast<const double*>(st + 3 * FIELD_BYTES);
-            if (is_main || to_shared) {
-                double2 fr = *reinterpret_cast<const double2*>(F0 + pair_box), fp = make_double2(0, 0),
-                        fv = make_double2(0, 0), fa;
-                if (MODE == MODE_K1) {
-                    fp = *reinterpret_cast<const double2*>(F1 + pair_box);
-                    fv = *reinterpret_cast<const double2*>(F2 + pair_box);
-                    fa = *reinterpret_cast<const double2*>(F3 + pair_box);
-                } else if (MODE == MODE_K2) {
-                    fv = *reinterpret_cast<const double2*>(F1 + pair_box);
-                    fa = *reinterpret_cast<const double2*>(F2 + pair_box);
-                } else {
-                    fa = *reinterpret_cast<const double2*>(F1 + pair_box);
-                }
-                const bool ok = pair_ok && zin;
-                if (!ok) fa = make_double2(1.0, 1.0);                   // zero-filled nodes: keep u finite (0/1)
-                up.u[0] = u_of<MODE, PRECOND>(fr.x, fp.x, fv.x, fa.x, first, c1, c2, up.n[0], fault);
-                up.u[1] = u_of<MODE, PRECOND>(fr.y, fp.y, fv.y, fa.y, first, c1, c2, up.n[1], fault);
-                up.a[0] = fa.x; up.a[1] = fa.y;
-                if (is_main) {
-                    if (T::OWN)
-                        up.w = *reinterpret_cast<const double2*>(reinterpret_cast<const double*>(st + L::OWN_OFF) + own_tile);
-                    if (!STORED) {
-                        if (CODE32) {
-                            const uint2 cw = *reinterpret_cast<const uint2*>(st + L::CODE_OFF + 4 * own_tile);
-                            up.k0 = cw.x; up.k1 = cw.y;
-                        } else {
-                            up.k0 = *reinterpret_cast<const unsigned*>(st + L::CODE_OFF + 2 * own_tile);
-                        }
-                    }
-                    if (MODE == MODE_K1 && ok && z >= z0 && z < z1)     // p' is an output of steps 5-9
-                        *reinterpret_cast<double2*>(kv.p_out + own_off + plane * z) = make_double2(up.n[0], up.n[1]);
-                }
-                if (to_shared) *reinterpret_cast<double2*>(u_s + pair_box) = make_double2(up.u[0], up.u[1]);
-            }
-            if (col_any && to_shared) {
-                double hr = F0[col_box], hp = 0.0, hv = 0.0, ha;
-                if (MODE == MODE_K1) { hp = F1[col_box]; hv = F2[col_box]; ha = F3[col_box]; }
-                else if (MODE == MODE_K2) { hv = F1[col_box]; ha = F2[col_box]; }
-                else ha = 1.0;
-                if (!(col_ok && zin)) ha = 1.0;
-                double dummy;
-                u_s[col_box] = u_of<MODE, PRECOND>(hr, hp, hv, ha, first, c1, c2, dummy, fault);
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[s]);                      // this warp is done with the stage
-        };
-        // difference plane z (slot c) with its z neighbours in slots dn and up; xy neighbours from shared
-        auto compute = [&](int z, const Slot& dn, const Slot& c, const Slot& up) {
-            const int k = z - z0 + 1;
-            const long long i = own_off + plane * z;
-            const double* u_s = reinterpret_cast<const double*>(smem + L::U_OFF + (k & 1) * FIELD_BYTES);
-            const double2 us = *reinterpret_cast<const double2*>(u_s + pair_box - BX);
-            const double2 un = *reinterpret_cast<const double2*>(u_s + pair_box + BX);
-            const double uw = u_s[pair_box - 1], ue = u_s[pair_box + 2];
-            double2 cf[6];
-            if (STORED) {
-#pragma unroll
-                for (int d = 0; d < 6; ++d) cf[d] = *reinterpret_cast<const double2*>(op.offd[d] + i);
-            }
-            double out[2];
-#pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                double cc[6];
-                if (STORED) {
-#pragma unroll
-                    for (int d = 0; d < 6; ++d) cc[d] = e == 0 ? cf[d].x : cf[d].y;
-                } else {
-#pragma unroll
-                    for (int d = 0; d < 6; ++d)
-                        cc[d] = *reinterpret_cast<const double*>(reinterpret_cast<const unsigned char*>(ctab_s) +
-                                                                 ctab_off<CODE32>(c.k0, c.k1, e, d));
-                }
-                double acc = mul(c.a[e], c.u[e]);
-                acc = add(acc, mul(cc[0], e == 0 ? c.u[1] : ue));
-                acc = add(acc, mul(cc[1], e == 1 ? c.u[0] : uw));
-                acc = add(acc, mul(cc[2], e == 0 ? us.x : us.y));
-                acc = add(acc, mul(cc[3], e == 0 ? un.x : un.y));
-                acc = add(acc, mul(cc[4], dn.u[e]));
-                acc = add(acc, mul(cc[5], up.u[e]));
-                out[e] = acc;
-            }
+            double2 fr = *reinterpret_cast<const double2*>(F0 + pair_box), fp = make_double2(0, 0),
+                    fv = make_double2(0, 0), fa;
             if (MODE == MODE_K1) {
-                *reinterpret_cast<double2*>(kv.v_out + i) = make_double2(out[0], out[1]);
-                dd_fma(q[0], c.w.x, out[0]); dd_fma(q[1], c.w.y, out[1]);
+                fp = *reinterpret_cast<const double2*>(F1 + pair_box);
+                fv = *reinterpret_cast<const double2*>(F2 + pair_box);
+                fa = *reinterpret_cast<const double2*>(F3 + pair_box);
             } else if (MODE == MODE_K2) {
-                *reinterpret_cast<double2*>(kv.t + i) = make_double2(out[0], out[1]);
-                dd_fma(q[0], out[0], c.n[0]); dd_fma(q[0], out[1], c.n[1]);
-                dd_fma(q[1], out[0], out[0]); dd_fma(q[1], out[1], out[1]);
+                fv = *reinterpret_cast<const double2*>(F1 + pair_box);
+                fa = *reinterpret_cast<const double2*>(F2 + pair_box);
             } else {
-                const double r0 = sub(c.w.x, out[0]), r1 = sub(c.w.y, out[1]);
-                if (MODE == MODE_R0) {
-                    *reinterpret_cast<double2*>(kv.r + i) = make_double2(r0, r1);
-                    *reinterpret_cast<double2*>(kv.rt + i) = make_double2(r0, r1);
-                    dd_fma(q[0], c.w.x, c.w.x); dd_fma(q[0], c.w.y, c.w.y);
-                }
-                dd_fma(q[1], r0, r0); dd_fma(q[1], r1, r1);
+                fa = *reinterpret_cast<const double2*>(F1 + pair_box);
             }
+            if (!ok) fa = make_double2(1.0, 1.0);                       // zero-filled nodes: keep u finite (0/1)
+            u[0] = u_of<MODE, PRECOND>(fr.x, fp.x, fv.x, fa.x, first, c1, c2, n[0], fault);
+            u[1] = u_of<MODE, PRECOND>(fr.y, fp.y, fv.y, fa.y, first, c1, c2, n[1], fault);
+            a[0] = fa.x; a[1] = fa.y;
         };
-        // one plane: u(z+1) into slot up and the other shared buffer, difference plane z, barrier
-        auto step = [&](int z, const Slot& dn, const Slot& c, Slot& up) {
-            prepare(z - z0 + 2, up, true);
-            if (is_main && pair_ok) compute(z, dn, c, up);
-            consumer_barrier();
+        auto wait_full = [&](int k) -> const unsigned char* {
+            const int s = k % S;
+            const unsigned par = (unsigned)(k / S) & 1u;
+            while (!mbar_try_wait(&full[s], par)) {}
+            return smem + s * L::STAGE_BYTES;
+        };
+        auto release = [&](int k) {                                     // this warp is done with the stage of plane k
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[k % S]);
         };
 
-        Slot s0, s1, s2;
-        s0.w = s1.w = s2.w = make_double2(0, 0);
-        s0.k0 = s0.k1 = s1.k0 = s1.k1 = s2.k0 = s2.k1 = 0u;
-        prepare(0, s0, false);                 // plane z0-1: registers only
-        prepare(1, s1, true);                  // plane z0
-        consumer_barrier();
-        for (int z = z0; z < z1; z += 3) {     // slots rotate by renaming, not by moving registers
-            step(z, s0, s1, s2);
-            if (z + 1 >= z1) break;
-            step(z + 1, s1, s2, s0);
-            if (z + 2 >= z1) break;
-            step(z + 2, s2, s0, s1);
+        if (!is_main) {
+            // ---- halo warps: u on the halo ring of every plane that gets differenced ---------------
+            int col_box = 0; bool col_ok = false;
+            const bool col_any = lane < TY;
+            if (col_any) {
+                const int hx = wid == TY ? 1 : BX - 2, hy = 1 + lane;
+                col_box = hy * BX + hx;
+                const int gx = x0 - 2 + hx, gy = y0 - 1 + hy;
+                col_ok = gx >= 0 && gx < g.nx && gy < g.ny;
+            }
+            wait_full(0); release(0);                                   // plane z0-1 has no xy neighbours to serve
+            for (int k = 1; k < nq; ++k) {
+                const unsigned char* st = wait_full(k);
+                const int z = z0 - 1 + k;
+                const bool zin = z >= 0 && z < g.nz;
+                double* u_s = reinterpret_cast<double*>(smem + L::U_OFF + (k & 1) * FIELD_BYTES);
+                double u[2], n[2], a[2];
+                form_pair(st, pair_ok && zin, u, n, a);
+                *reinterpret_cast<double2*>(u_s + pair_box) = make_double2(u[0], u[1]);
+                if (col_any) {
+                    const double* F0 = reinterpret_cast<const double*>(st);
+                    const double* F1 = reinterpret_cast<const double*>(st + FIELD_BYTES);
+                    const double* F2 = reinterpret_cast<const double*>(st + 2 * FIELD_BYTES);
+                    const double* F3 = reinterpret_cast<const double*>(st + 3 * FIELD_BYTES);
+                    double hr = F0[col_box], hp = 0.0, hv = 0.0, ha;
+                    if (MODE == MODE_K1) { hp = F1[col_box]; hv = F2[col_box]; ha = F3[col_box]; }
+                    else if (MODE == MODE_K2) { hv = F1[col_box]; ha = F2[col_box]; }
+                    else ha = 1.0;
+                    if (!(col_ok && zin)) ha = 1.0;
+                    double dummy;
+                    u_s[col_box] = u_of<MODE, PRECOND>(hr, hp, hv, ha, first, c1, c2, dummy, fault);
+                }
+                release(k);
+                consumer_barrier();
+            }
+        } else {
+            // ---- main warps -------------------------------------------------------------------------
+            // form u(z+1) into slot `up` (+ the other shared buffer) and difference plane z (slot c, z neighbours
+            // in dn and up, xy neighbours from shared).  Everything between the wait and the stage release is
+            // one basic block: the divisions of plane z+1 and the stencil chain of plane z are independent and
+            // get interleaved by the scheduler.  Nodes outside the grid see zero operands and zero codes, give
+            // exact zeros and add nothing to the inner products; only their stores are predicated.
+            auto load_slot = [&](int k, Slot& up, bool to_shared) {
+                const unsigned char* st = wait_full(k);
+                const int z = z0 - 1 + k;
+                const bool ok = pair_ok && z >= 0 && z < g.nz;
+                form_pair(st, ok, up.u, up.n, up.a);
+                if (T::OWN)
+                    up.w = *reinterpret_cast<const double2*>(reinterpret_cast<const double*>(st + L::OWN_OFF) + own_tile);
+                if (!STORED) {
+                    if (CODE32) {
+                        const uint2 cw = *reinterpret_cast<const uint2*>(st + L::CODE_OFF + 4 * own_tile);
+                        up.k0 = cw.x; up.k1 = cw.y;
+                    } else {
+                        up.k0 = *reinterpret_cast<const unsigned*>(st + L::CODE_OFF + 2 * own_tile);
+                    }
+                }
+                if (MODE == MODE_K1 && ok && z >= z0 && z < z1)         // p' is an output of steps 5-9
+                    *reinterpret_cast<double2*>(kv.p_out + own_off + plane * z) = make_double2(up.n[0], up.n[1]);
+                if (to_shared) {
+                    double* u_s = reinterpret_cast<double*>(smem + L::U_OFF + (k & 1) * FIELD_BYTES);
+                    *reinterpret_cast<double2*>(u_s + pair_box) = make_double2(up.u[0], up.u[1]);
+                }
+            };
+            auto step = [&](int z, const Slot& dn, const Slot& c, Slot& up) {
+                const int k = z - z0 + 1;                               // load-sequence index of plane z
+                const long long i = own_off + plane * z;
+                const double* u_s = reinterpret_cast<const double*>(smem + L::U_OFF + (k & 1) * FIELD_BYTES);
+                load_slot(k + 1, up, true);
+                const double2 us = *reinterpret_cast<const double2*>(u_s + pair_box - BX);
+                const double2 un = *reinterpret_cast<const double2*>(u_s + pair_box + BX);
+                const double uw = u_s[pair_box - 1], ue = u_s[pair_box + 2];
+                double2 cf[6];
+                if (STORED) {
+#pragma unroll
+                    for (int d = 0; d < 6; ++d)
+                        cf[d] = pair_ok ? *reinterpret_cast<const double2*>(op.offd[d] + i) : make_double2(0, 0);
+                }
+                double out[2];
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    double cc[6];
+                    if (STORED) {
+#pragma unroll
+                        for (int d = 0; d < 6; ++d) cc[d] = e == 0 ? cf[d].x : cf[d].y;
+                    } else {
+#pragma unroll
+                        for (int d = 0; d < 6; ++d)
+                            cc[d] = *reinterpret_cast<const double*>(reinterpret_cast<const unsigned char*>(ctab_s) +
+                                                                     ctab_off<CODE32>(c.k0, c.k1, e, d));
+                    }
+                    double acc = mul(c.a[e], c.u[e]);
+                    acc = add(acc, mul(cc[0], e == 0 ? c.u[1] : ue));
+                    acc = add(acc, mul(cc[1], e == 1 ? c.u[0] : uw));
+                    acc = add(acc, mul(cc[2], e == 0 ? us.x : us.y));
+                    acc = add(acc, mul(cc[3], e == 0 ? un.x : un.y));
+                    acc = add(acc, mul(cc[4], dn.u[e]));
+                    acc = add(acc, mul(cc[5], up.u[e]));
+                    out[e] = acc;
+                }
+                if (MODE == MODE_K1) {
+                    if (pair_ok) *reinterpret_cast<double2*>(kv.v_out + i) = make_double2(out[0], out[1]);
+                    dd_fma(q[0], c.w.x, out[0]); dd_fma(q[1], c.w.y, out[1]);
+                } else if (MODE == MODE_K2) {
+                    if (pair_ok) *reinterpret_cast<double2*>(kv.t + i) = make_double2(out[0], out[1]);
+                    dd_fma(q[0], out[0], c.n[0]); dd_fma(q[0], out[1], c.n[1]);
+                    dd_fma(q[1], out[0], out[0]); dd_fma(q[1], out[1], out[1]);
+                } else {
+                    const double r0 = sub(c.w.x, out[0]), r1 = sub(c.w.y, out[1]);
+                    if (MODE == MODE_R0) {
+                        if (pair_ok) {
+                            *reinterpret_cast<double2*>(kv.r + i) = make_double2(r0, r1);
+                            *reinterpret_cast<double2*>(kv.rt + i) = make_double2(r0, r1);
+                        }
+                        dd_fma(q[0], c.w.x, c.w.x); dd_fma(q[0], c.w.y, c.w.y);
+                    }
+                    dd_fma(q[1], r0, r0); dd_fma(q[1], r1, r1);
+                }
+                release(k + 1);
+                consumer_barrier();
+            };
+
+            Slot s0, s1, s2;
+            s0.w = s1.w = s2.w = make_double2(0, 0);
+            s0.k0 = s0.k1 = s1.k0 = s1.k1 = s2.k0 = s2.k1 = 0u;
+            load_slot(0, s0, false); release(0);   // plane z0-1: registers only
+            load_slot(1, s1, true);  release(1);   // plane z0
+            consumer_barrier();
+            for (int z = z0; z < z1; z += 3) {     // slots rotate by renaming, not by moving registers
+                step(z, s0, s1, s2);
+                if (z + 1 >= z1) break;
+                step(z + 1, s1, s2, s0);
+                if (z + 2 >= z1) break;
+                step(z + 2, s2, s0, s1);
+            }
         }
     }
 
