@@ -33,6 +33,7 @@ if ROOT not in sys.path:
 LINEAR_ITERS = 200
 PF_INNER_ITERS = 25
 STEP_ITERS = LINEAR_ITERS + 3 * PF_INNER_ITERS
+PROFILE_ITERS = 40      # iterations per linear solve whose three kernels are bracketed by CUDA events
 METRIC = "bicgstab_iterations_per_s"
 UNIT = "iterations/s"
 
@@ -219,7 +220,7 @@ def run_b200(args):
         pf.pf_grid_set_option(h, pf.PF_OPT_LINEAR_MAXIT, PF_INNER_ITERS)
         pf.pf_grid_set_option(h, pf.PF_OPT_MAX_OUTER, 1)
         if profile:
-            pf.pf_grid_set_option(h, pf.PF_OPT_PROFILE, LINEAR_ITERS)
+            pf.pf_grid_set_option(h, pf.PF_OPT_PROFILE, PROFILE_ITERS)
         pf.pf_grid_set_workspace(h, ws)                                            # rows L1, L2
         if host_buffers:
             x_host.zero_()

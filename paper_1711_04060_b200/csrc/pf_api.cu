@@ -8,6 +8,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -33,6 +34,60 @@ thread_local std::string g_create_error;
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// The small per-grid buffers (device scalars, reduction partials, coefficient tables, charge list, pinned
+// mirrors of the scalars, two events) are recycled through a process-wide free list: cudaMalloc,
+// cudaMallocHost and their frees cost milliseconds and synchronise the device, which would dominate the
+// creation of a grid (rows L1/L2).  A set is owned by one grid at a time.
+struct SmallSet {
+    int device = -1;
+    char* dev = nullptr;            // one device allocation, carved up below
+    size_t charge_cap = 0;          // pf_charge entries the tail of `dev` holds
+    char* host = nullptr;           // pinned, 2 x 256 bytes
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+};
+constexpr size_t SS_SC = 0, SS_TICKET = 256, SS_DMAX = 512, SS_CTAB0 = 768, SS_CTAB1 = 1024,
+                 SS_PARTIAL = 1280, SS_CHARGES = SS_PARTIAL + sizeof(dd) * 3 * PF_MAX_PARTIAL_BLOCKS;
+static_assert(sizeof(Scalars) <= 256, "Scalars slots of the small set");
+std::mutex g_pool_mutex;
+std::vector<SmallSet*> g_pool;
+
+void small_set_free(SmallSet* s) {
+    if (!s) return;
+    cudaFree(s->dev);
+    if (s->host) cudaFreeHost(s->host);
+    if (s->ev[0]) cudaEventDestroy(s->ev[0]);
+    if (s->ev[1]) cudaEventDestroy(s->ev[1]);
+    delete s;
+}
+
+cudaError_t small_set_acquire(int device, size_t ncharges, SmallSet** out) {
+    {
+        std::lock_guard<std::mutex> lock(g_pool_mutex);
+        for (size_t k = 0; k < g_pool.size(); ++k)
+            if (g_pool[k]->device == device && g_pool[k]->charge_cap >= ncharges) {
+                *out = g_pool[k];
+                g_pool.erase(g_pool.begin() + k);
+                return cudaSuccess;
+            }
+    }
+    SmallSet* s = new SmallSet();
+    s->device = device;
+    s->charge_cap = std::max<size_t>(4096, ncharges);
+    cudaError_t e = cudaMalloc(&s->dev, SS_CHARGES + sizeof(pf_charge) * s->charge_cap);
+    if (e == cudaSuccess) e = cudaMallocHost(&s->host, 512);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->ev[0], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->ev[1], cudaEventDisableTiming);
+    if (e != cudaSuccess) { small_set_free(s); return e; }
+    *out = s;
+    return cudaSuccess;
+}
+
+void small_set_release(SmallSet* s) {
+    if (!s) return;
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    if (g_pool.size() < 8) g_pool.push_back(s); else small_set_free(s);
+}
+
 }  // namespace
 
 struct pf_grid {
@@ -46,7 +101,8 @@ struct pf_grid {
     double eps_min, eps_max, eps_mid;
     bool uniform;
     int ncharges;
-    double* charges_dev;     // small, owned
+    SmallSet* small;         // recycled small buffers; the pointers below point into it
+    double* charges_dev;
     // options
     int opt_stencil, opt_kernels, opt_check, opt_lin_maxit, opt_max_outer, opt_precond, opt_history;
     double opt_omega_pf, opt_lin_tol, opt_water;
@@ -330,6 +386,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->opt_profile = 0; g->prof_ms[0] = g->prof_ms[1] = g->prof_ms[2] = 0.0;
     g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0;
+    g->small = nullptr;
     g->charges_dev = nullptr; g->sc = nullptr; g->rb.partial = nullptr; g->rb.ticket = nullptr;
     g->ctab_poisson = g->ctab_pf1 = nullptr; g->dmax_bits = nullptr; g->tma = nullptr;
     g->code = g->code_pf1 = nullptr; g->code_mode = 0; g->cpitch = 0;
@@ -345,20 +402,20 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     } while (0)
     PF_CREATE_CUDA(cudaGetDevice(&dev));
     PF_CREATE_CUDA(cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev));
-    PF_CREATE_CUDA(cudaMalloc(&g->sc, 256));
-    PF_CREATE_CUDA(cudaMalloc(&g->rb.partial, sizeof(dd) * 3 * PF_MAX_PARTIAL_BLOCKS));
-    PF_CREATE_CUDA(cudaMalloc(&g->rb.ticket, 256));
+    PF_CREATE_CUDA(small_set_acquire(dev, (size_t)ncharges, &g->small));
+    g->sc = reinterpret_cast<Scalars*>(g->small->dev + SS_SC);
+    g->rb.ticket = reinterpret_cast<unsigned int*>(g->small->dev + SS_TICKET);
+    g->dmax_bits = reinterpret_cast<unsigned long long*>(g->small->dev + SS_DMAX);
+    g->ctab_poisson = reinterpret_cast<double*>(g->small->dev + SS_CTAB0);
+    g->ctab_pf1 = reinterpret_cast<double*>(g->small->dev + SS_CTAB1);
+    g->rb.partial = reinterpret_cast<dd*>(g->small->dev + SS_PARTIAL);
+    g->sc_host[0] = reinterpret_cast<Scalars*>(g->small->host);
+    g->sc_host[1] = reinterpret_cast<Scalars*>(g->small->host + 256);
+    g->ev[0] = g->small->ev[0]; g->ev[1] = g->small->ev[1];
     PF_CREATE_CUDA(cudaMemsetAsync(g->rb.ticket, 0, 256, g->stream));
-    PF_CREATE_CUDA(cudaMalloc(&g->ctab_poisson, sizeof(double) * PF_CTAB));
-    PF_CREATE_CUDA(cudaMalloc(&g->ctab_pf1, sizeof(double) * PF_CTAB));
     g->tma = tma_set_create();
-    PF_CREATE_CUDA(cudaMalloc(&g->dmax_bits, 256));
-    PF_CREATE_CUDA(cudaMallocHost(&g->sc_host[0], sizeof(Scalars)));
-    PF_CREATE_CUDA(cudaMallocHost(&g->sc_host[1], sizeof(Scalars)));
-    PF_CREATE_CUDA(cudaEventCreateWithFlags(&g->ev[0], cudaEventDisableTiming));
-    PF_CREATE_CUDA(cudaEventCreateWithFlags(&g->ev[1], cudaEventDisableTiming));
     if (ncharges > 0) {
-        PF_CREATE_CUDA(cudaMalloc(&g->charges_dev, sizeof(pf_charge) * ncharges));
+        g->charges_dev = reinterpret_cast<double*>(g->small->dev + SS_CHARGES);
         PF_CREATE_CUDA(cudaMemcpyAsync(g->charges_dev, charges, sizeof(pf_charge) * ncharges, cudaMemcpyHostToDevice,
                                        g->stream));
     }
@@ -378,14 +435,9 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
 void pf_grid_destroy(pf_grid* g) {
     if (!g) return;
     cudaStreamSynchronize(g->stream);
-    cudaFree(g->sc); cudaFree(g->rb.partial); cudaFree(g->rb.ticket);
-    cudaFree(g->ctab_poisson); cudaFree(g->ctab_pf1); cudaFree(g->dmax_bits);
+    small_set_release(g->small);
+    cudaFree(g->hist);
     if (g->tma) tma_set_destroy(g->tma);
-    cudaFree(g->charges_dev); cudaFree(g->hist);
-    if (g->sc_host[0]) cudaFreeHost(g->sc_host[0]);
-    if (g->sc_host[1]) cudaFreeHost(g->sc_host[1]);
-    if (g->ev[0]) cudaEventDestroy(g->ev[0]);
-    if (g->ev[1]) cudaEventDestroy(g->ev[1]);
     for (cudaEvent_t e : g->prof_ev) cudaEventDestroy(e);
     cudaGetLastError();
     delete g;

@@ -174,27 +174,63 @@ k_assemble_pf1(GridDims g, double h, double lc, const double* __restrict__ eps, 
     }
 }
 
-// One thread: the deposits of different charges can hit the same node and floating-point addition
-// is not associative, so they are applied in charge order (reading R2; runs once per grid).
-__global__ void k_deposit(GridDims g, double h, double kappa, const double* __restrict__ ch, int m, double* fixed) {
-    if (blockIdx.x != 0 || threadIdx.x != 0) return;
+// Deposits of different charges can hit the same node and floating-point addition is not associative,
+// so they must be applied in charge order (reading R2).  One block walks the list in chunks of DEP_CHUNK
+// charges, one charge per thread: a chunk in which no two charges touch a common node (cells at least two
+// apart in some direction -- the usual case) is applied in parallel, otherwise serially by one thread;
+// chunks follow one another in order.  The result is identical to the serial loop.
+constexpr int DEP_CHUNK = 256;
+
+__device__ __forceinline__ void deposit_one(const GridDims& g, double h, double h3, double kappa,
+                                            const double* __restrict__ ch, int c, double* fixed) {
+    const double px = dvd(ch[4 * c], h), py = dvd(ch[4 * c + 1], h), pz = dvd(ch[4 * c + 2], h);
+    const double q = ch[4 * c + 3];
+    const int ix = min(max((int)floor(px), 0), g.nx - 2);
+    const int iy = min(max((int)floor(py), 0), g.ny - 2);
+    const int iz = min(max((int)floor(pz), 0), g.nz - 2);
+    const double fx = sub(px, (double)ix), fy = sub(py, (double)iy), fz = sub(pz, (double)iz);
+    const double amp = dvd(mul(kappa, q), h3);
+    for (int dz = 0; dz < 2; ++dz)
+        for (int dy = 0; dy < 2; ++dy)
+            for (int dx = 0; dx < 2; ++dx) {
+                const double wx = dx ? fx : sub(1.0, fx), wy = dy ? fy : sub(1.0, fy), wz = dz ? fz : sub(1.0, fz);
+                const double w = mul(mul(wx, wy), wz);
+                const long long i = (ix + dx) + (long long)g.nx * ((iy + dy) + (long long)g.ny * (iz + dz));
+                fixed[i] = add(fixed[i], mul(amp, w));
+            }
+}
+
+__global__ void __launch_bounds__(DEP_CHUNK)
+k_deposit(GridDims g, double h, double kappa, const double* __restrict__ ch, int m, double* fixed) {
+    __shared__ int cell[DEP_CHUNK][3];
+    __shared__ int conflict;
     const double h3 = mul(mul(h, h), h);
-    for (int c = 0; c < m; ++c) {
-        const double px = dvd(ch[4 * c], h), py = dvd(ch[4 * c + 1], h), pz = dvd(ch[4 * c + 2], h);
-        const double q = ch[4 * c + 3];
-        const int ix = min(max((int)floor(px), 0), g.nx - 2);
-        const int iy = min(max((int)floor(py), 0), g.ny - 2);
-        const int iz = min(max((int)floor(pz), 0), g.nz - 2);
-        const double fx = sub(px, (double)ix), fy = sub(py, (double)iy), fz = sub(pz, (double)iz);
-        const double amp = dvd(mul(kappa, q), h3);
-        for (int dz = 0; dz < 2; ++dz)
-            for (int dy = 0; dy < 2; ++dy)
-                for (int dx = 0; dx < 2; ++dx) {
-                    const double wx = dx ? fx : sub(1.0, fx), wy = dy ? fy : sub(1.0, fy), wz = dz ? fz : sub(1.0, fz);
-                    const double w = mul(mul(wx, wy), wz);
-                    const long long i = (ix + dx) + (long long)g.nx * ((iy + dy) + (long long)g.ny * (iz + dz));
-                    fixed[i] = add(fixed[i], mul(amp, w));
-                }
+    const int t = threadIdx.x;
+    for (int base = 0; base < m; base += DEP_CHUNK) {
+        const int c = base + t;
+        const int cnt = min(DEP_CHUNK, m - base);
+        if (t == 0) conflict = 0;
+        if (c < m) {
+            cell[t][0] = min(max((int)floor(dvd(ch[4 * c], h)), 0), g.nx - 2);
+            cell[t][1] = min(max((int)floor(dvd(ch[4 * c + 1], h)), 0), g.ny - 2);
+            cell[t][2] = min(max((int)floor(dvd(ch[4 * c + 2], h)), 0), g.nz - 2);
+        }
+        __syncthreads();
+        if (c < m) {
+            bool hit = false;
+            for (int k = 0; k < t; ++k)
+                hit = hit || (abs(cell[k][0] - cell[t][0]) <= 1 && abs(cell[k][1] - cell[t][1]) <= 1 &&
+                              abs(cell[k][2] - cell[t][2]) <= 1);
+            if (hit) conflict = 1;
+        }
+        __syncthreads();
+        if (!conflict) {
+            if (c < m) deposit_one(g, h, h3, kappa, ch, c, fixed);
+        } else if (t == 0) {
+            for (int k = 0; k < cnt; ++k) deposit_one(g, h, h3, kappa, ch, base + k, fixed);
+        }
+        __threadfence_block();
+        __syncthreads();
     }
 }
 
@@ -279,7 +315,7 @@ void build_ctab_pf1(const Palette& pal, double h, double lc, double* ctab) {
 void launch_deposit(cudaStream_t s, const GridDims& g, double h, double kappa, const double* charges_dev, int m,
                     double* fixed) {
     cudaMemsetAsync(fixed, 0, sizeof(double) * g.n, s);
-    if (m > 0) { ++g_launch_count; k_deposit<<<1, 32, 0, s>>>(g, h, kappa, charges_dev, m, fixed); }
+    if (m > 0) { ++g_launch_count; k_deposit<<<1, DEP_CHUNK, 0, s>>>(g, h, kappa, charges_dev, m, fixed); }
 }
 
 void launch_set_dirichlet(cudaStream_t s, const GridDims& g, const BcDev& bc, double* x) {

@@ -77,6 +77,7 @@ struct Layout {
     static constexpr int SCRATCH_OFF = CTAB_OFF + PF_CTAB * 8;
     static constexpr int BAR_OFF = SCRATCH_OFF + 2 * 32 * (int)sizeof(dd);
     static constexpr int TOTAL = BAR_OFF + 16 * T::STAGES;           // full[S], empty[S]
+    static_assert(CTAB_OFF % 128 == 0, "ctab_at ORs table offsets into the table address");
     static constexpr unsigned TX_BYTES = (unsigned)(T::NF * BX * BY * 8 + (T::OWN ? OWN_BYTES : 0) + CODE_BYTES);
 };
 
@@ -119,17 +120,22 @@ __device__ __forceinline__ double u_of(double r, double p, double v, double a, b
     return PRECOND ? dvd_nb(numer, a, fault) : numer;   // == jacobi<PRECOND>(numer, a) of the direct kernels
 }
 
-// Byte offset into the coefficient table of field d of node e (0 or 1) of the thread's code word(s).
+// Coefficient of field d of node e (0 or 1) of the thread's code word(s): one shift, one three-input logic
+// operation that masks the field and ORs in the (128-byte aligned) shared address of the table, one load.
 template <bool CODE32>
-__device__ __forceinline__ unsigned ctab_off(unsigned w0, unsigned w1, int e, int d) {
+__device__ __forceinline__ double ctab_at(unsigned ctab_addr, unsigned w0, unsigned w1, int e, int d) {
+    unsigned off;
     if (CODE32) {
         const unsigned w = e ? w1 : w0;
         const int sh = 4 * d - 3;
-        return (sh >= 0 ? (w >> sh) : (w << -sh)) & 0x78u;
+        off = ((sh >= 0 ? (w >> sh) : (w << -sh)) & 0x78u) | ctab_addr;
     } else {
         const int sh = 16 * e + 2 * d - 3;
-        return (sh >= 0 ? (w0 >> sh) : (w0 << -sh)) & 0x18u;
+        off = ((sh >= 0 ? (w0 >> sh) : (w0 << -sh)) & 0x18u) | ctab_addr;
     }
+    double c;
+    asm("ld.shared.f64 %0, [%1];" : "=d"(c) : "r"(off));
+    return c;
 }
 
 // Registers of one plane of a main thread: u at its two nodes, the numerators (p' or s), the diagonal,
@@ -171,6 +177,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
         fence_proxy_async();
     }
     if (!STORED && tid < PF_CTAB) ctab_s[tid] = op.ctab[tid];
+    const unsigned ctab_addr = smem_u32(ctab_s);           // 128-byte aligned: CTAB_OFF and the smem base are
     __syncthreads();
 
     dd q[2] = {dd_zero(), dd_zero()};
@@ -329,8 +336,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     } else {
 #pragma unroll
                         for (int d = 0; d < 6; ++d)
-                            cc[d] = *reinterpret_cast<const double*>(reinterpret_cast<const unsigned char*>(ctab_s) +
-                                                                     ctab_off<CODE32>(c.k0, c.k1, e, d));
+                            cc[d] = ctab_at<CODE32>(ctab_addr, c.k0, c.k1, e, d);
                     }
                     double acc = mul(c.a[e], c.u[e]);
                     acc = add(acc, mul(cc[0], e == 0 ? c.u[1] : ue));

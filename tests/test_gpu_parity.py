@@ -46,10 +46,11 @@ def ragged_workload(nx=37, ny=20, nz=11, seed=7, mixed_bc=True):
 
 # ---- rows L1, L2: assembly, bit-exact -------------------------------------------------------------
 
-@pytest.mark.parametrize("which", ["cfg0", "cfg2_small", "ragged"])
+@pytest.mark.parametrize("which", ["cfg0", "cfg2_small", "cfg3_64", "ragged"])
 def test_assembly_bit_exact(pf, oracle, which):
+    # cfg3_64: 1536 charges, chunks with and without node conflicts in the parallel in-order deposition
     w = {"cfg0": lambda: wl.config0(), "cfg2_small": lambda: wl.config2(n=32, volt_mv=50.0),
-         "ragged": lambda: ragged_workload()}[which]()
+         "cfg3_64": lambda: wl.config3(n=64), "ragged": lambda: ragged_workload()}[which]()
     A = oracle.assemble_poisson(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps)
     fixed = oracle.deposit_charges(w.nx, w.ny, w.nz, w.h, w.charges)
     g = pf.Grid.from_workload(w, stencil=pf.STENCIL_STORED)
