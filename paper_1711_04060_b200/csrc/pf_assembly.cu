@@ -176,9 +176,9 @@ k_assemble_pf1(GridDims g, double h, double lc, const double* __restrict__ eps, 
 
 // Deposits of different charges can hit the same node and floating-point addition is not associative,
 // so they must be applied in charge order (reading R2).  One block walks the list in chunks of DEP_CHUNK
-// charges, one charge per thread: a chunk in which no two charges touch a common node (cells at least two
-// apart in some direction -- the usual case) is applied in parallel, otherwise serially by one thread;
-// chunks follow one another in order.  The result is identical to the serial loop.
+// charges, one charge per thread, in rounds: a charge is applied once every earlier charge of the chunk
+// whose cell is adjacent to its own (the only ones that can share a node with it) has been applied.
+// Charges applied in the same round touch disjoint nodes.  The result is identical to the serial loop.
 constexpr int DEP_CHUNK = 256;
 
 __device__ __forceinline__ void deposit_one(const GridDims& g, double h, double h3, double kappa,
@@ -203,33 +203,33 @@ __device__ __forceinline__ void deposit_one(const GridDims& g, double h, double 
 __global__ void __launch_bounds__(DEP_CHUNK)
 k_deposit(GridDims g, double h, double kappa, const double* __restrict__ ch, int m, double* fixed) {
     __shared__ int cell[DEP_CHUNK][3];
-    __shared__ int conflict;
+    __shared__ unsigned char done[DEP_CHUNK];
     const double h3 = mul(mul(h, h), h);
     const int t = threadIdx.x;
     for (int base = 0; base < m; base += DEP_CHUNK) {
         const int c = base + t;
-        const int cnt = min(DEP_CHUNK, m - base);
-        if (t == 0) conflict = 0;
-        if (c < m) {
+        bool pending = c < m;
+        done[t] = 0;
+        if (pending) {
             cell[t][0] = min(max((int)floor(dvd(ch[4 * c], h)), 0), g.nx - 2);
             cell[t][1] = min(max((int)floor(dvd(ch[4 * c + 1], h)), 0), g.ny - 2);
             cell[t][2] = min(max((int)floor(dvd(ch[4 * c + 2], h)), 0), g.nz - 2);
         }
-        __syncthreads();
-        if (c < m) {
-            bool hit = false;
-            for (int k = 0; k < t; ++k)
-                hit = hit || (abs(cell[k][0] - cell[t][0]) <= 1 && abs(cell[k][1] - cell[t][1]) <= 1 &&
-                              abs(cell[k][2] - cell[t][2]) <= 1);
-            if (hit) conflict = 1;
+        while (__syncthreads_or(pending)) {
+            bool ready = pending;
+            if (pending)
+                for (int k = 0; k < t && ready; ++k)
+                    if (!done[k] && abs(cell[k][0] - cell[t][0]) <= 1 && abs(cell[k][1] - cell[t][1]) <= 1 &&
+                        abs(cell[k][2] - cell[t][2]) <= 1)
+                        ready = false;
+            __syncthreads();                  // every thread has read done[] of this round
+            if (ready) {
+                deposit_one(g, h, h3, kappa, ch, c, fixed);
+                __threadfence_block();
+                done[t] = 1;
+                pending = false;
+            }
         }
-        __syncthreads();
-        if (!conflict) {
-            if (c < m) deposit_one(g, h, h3, kappa, ch, c, fixed);
-        } else if (t == 0) {
-            for (int k = 0; k < cnt; ++k) deposit_one(g, h, h3, kappa, ch, base + k, fixed);
-        }
-        __threadfence_block();
         __syncthreads();
     }
 }
