@@ -46,6 +46,7 @@ constexpr int BX = TX + 4;               // box: two halo columns each side (one
 constexpr int BY = TY + 2;
 constexpr int FIELD_BYTES = ((BX * BY * 8 + 127) / 128) * 128;   // 9856
 constexpr int OWN_BYTES = TX * TY * 8;                            // 8192
+constexpr int NU = 3;                    // shared buffers of u (planes k, k+1 live, k+2 being written)
 static_assert(TY <= 32, "one halo column node per lane of a halo warp");
 
 enum { MODE_R0 = 0, MODE_R1 = 1, MODE_K1 = 2, MODE_K2 = 3 };
@@ -73,10 +74,10 @@ struct Layout {
     static constexpr int CODE_OFF = OWN_OFF + (T::OWN ? OWN_BYTES : 0);
     static constexpr int U_BYTES = BX * BY * 8;                     // one buffer of u
     static constexpr int U_OFF = T::STAGES * STAGE_BYTES;
-    static constexpr int CTAB_OFF = U_OFF + 2 * FIELD_BYTES;
+    static constexpr int CTAB_OFF = U_OFF + NU * FIELD_BYTES;
     static constexpr int SCRATCH_OFF = CTAB_OFF + PF_CTAB * 8;
     static constexpr int BAR_OFF = SCRATCH_OFF + 2 * 32 * (int)sizeof(dd);
-    static constexpr int TOTAL = BAR_OFF + 16 * T::STAGES;           // full[S], empty[S]
+    static constexpr int TOTAL = BAR_OFF + 16 * T::STAGES + 8 * NU;  // full[S], empty[S], ready[NU]
     static_assert(CTAB_OFF % 128 == 0, "ctab_at ORs table offsets into the table address");
     static constexpr unsigned TX_BYTES = (unsigned)(T::NF * BX * BY * 8 + (T::OWN ? OWN_BYTES : 0) + CODE_BYTES);
 };
@@ -146,8 +147,6 @@ struct Slot {
     unsigned k0, k1;
 };
 
-__device__ __forceinline__ void consumer_barrier() { asm volatile("bar.sync 1, %0;" ::"n"(NT_CONSUMER) : "memory"); }
-
 __device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
@@ -165,6 +164,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     dd* scratch = reinterpret_cast<dd*>(smem + L::SCRATCH_OFF);
     unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + L::BAR_OFF);
     unsigned long long* empty = full + S;
+    unsigned long long* ready = empty + S;     // ready[b]: all 18 consumer warps have written their part of u buffer b
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
@@ -174,6 +174,8 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW_CONSUMER); }
+#pragma unroll
+        for (int b = 0; b < NU; ++b) mbar_init(&ready[b], NW_CONSUMER);
         fence_proxy_async();
     }
     if (!STORED && tid < PF_CTAB) ctab_s[tid] = op.ctab[tid];
@@ -247,6 +249,21 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[k % S]);
         };
+        // u of plane k (k >= 1) lives in shared buffer (k-1) % NU.  publish: this warp's part is written (and its
+        // stage released); wait_ready: every consumer warp has published plane k.  No block-wide barrier: a warp
+        // that waits for plane k before it overwrites plane k-2's buffer with plane k+1 cannot race a reader
+        // (every warp that published plane k has finished differencing plane k-2).
+        auto u_buf = [&](int k) -> double* {
+            return reinterpret_cast<double*>(smem + L::U_OFF + ((k - 1) % NU) * FIELD_BYTES);
+        };
+        auto publish = [&](int k) {
+            __syncwarp();
+            if (lane == 0) { mbar_arrive(&ready[(k - 1) % NU]); mbar_arrive(&empty[k % S]); }
+        };
+        auto wait_ready = [&](int k) {
+            const unsigned par = (unsigned)((k - 1) / NU) & 1u;
+            while (!mbar_try_wait(&ready[(k - 1) % NU], par)) {}
+        };
 
         if (!is_main) {
             // ---- halo warps: u on the halo ring of every plane that gets differenced ---------------
@@ -260,10 +277,11 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             }
             wait_full(0); release(0);                                   // plane z0-1 has no xy neighbours to serve
             for (int k = 1; k < nq; ++k) {
+                if (k >= 2) wait_ready(k - 1);                           // plane k-3 (same buffer) is no longer read
                 const unsigned char* st = wait_full(k);
                 const int z = z0 - 1 + k;
                 const bool zin = z >= 0 && z < g.nz;
-                double* u_s = reinterpret_cast<double*>(smem + L::U_OFF + (k & 1) * FIELD_BYTES);
+                double* u_s = u_buf(k);
                 double u[2], n[2], a[2];
                 form_pair(st, pair_ok && zin, u, n, a);
                 *reinterpret_cast<double2*>(u_s + pair_box) = make_double2(u[0], u[1]);
@@ -280,8 +298,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     double dummy;
                     u_s[col_box] = u_of<MODE, PRECOND>(hr, hp, hv, ha, first, c1, c2, dummy, fault);
                 }
-                release(k);
-                consumer_barrier();
+                publish(k);
             }
         } else {
             // ---- main warps -------------------------------------------------------------------------
@@ -307,15 +324,13 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 }
                 if (MODE == MODE_K1 && ok && z >= z0 && z < z1)         // p' is an output of steps 5-9
                     *reinterpret_cast<double2*>(kv.p_out + own_off + plane * z) = make_double2(up.n[0], up.n[1]);
-                if (to_shared) {
-                    double* u_s = reinterpret_cast<double*>(smem + L::U_OFF + (k & 1) * FIELD_BYTES);
-                    *reinterpret_cast<double2*>(u_s + pair_box) = make_double2(up.u[0], up.u[1]);
-                }
+                if (to_shared) *reinterpret_cast<double2*>(u_buf(k) + pair_box) = make_double2(up.u[0], up.u[1]);
             };
             auto step = [&](int z, const Slot& dn, const Slot& c, Slot& up) {
                 const int k = z - z0 + 1;                               // load-sequence index of plane z
                 const long long i = own_off + plane * z;
-                const double* u_s = reinterpret_cast<const double*>(smem + L::U_OFF + (k & 1) * FIELD_BYTES);
+                const double* u_s = u_buf(k);
+                wait_ready(k);
                 load_slot(k + 1, up, true);
                 const double2 us = *reinterpret_cast<const double2*>(u_s + pair_box - BX);
                 const double2 un = *reinterpret_cast<const double2*>(u_s + pair_box + BX);
@@ -326,7 +341,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     for (int d = 0; d < 6; ++d)
                         cf[d] = pair_ok ? *reinterpret_cast<const double2*>(op.offd[d] + i) : make_double2(0, 0);
                 }
-                double out[2];
+                double out[2], c5[2];
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     double cc[6];
@@ -344,9 +359,12 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     acc = add(acc, mul(cc[2], e == 0 ? us.x : us.y));
                     acc = add(acc, mul(cc[3], e == 0 ? un.x : un.y));
                     acc = add(acc, mul(cc[4], dn.u[e]));
-                    acc = add(acc, mul(cc[5], up.u[e]));
                     out[e] = acc;
+                    c5[e] = cc[5];
                 }
+                publish(k + 1);                                         // u(z+1) is in shared memory
+                out[0] = add(out[0], mul(c5[0], up.u[0]));
+                out[1] = add(out[1], mul(c5[1], up.u[1]));
                 if (MODE == MODE_K1) {
                     if (pair_ok) *reinterpret_cast<double2*>(kv.v_out + i) = make_double2(out[0], out[1]);
                     dd_fma(q[0], c.w.x, out[0]); dd_fma(q[1], c.w.y, out[1]);
@@ -365,16 +383,13 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     }
                     dd_fma(q[1], r0, r0); dd_fma(q[1], r1, r1);
                 }
-                release(k + 1);
-                consumer_barrier();
             };
 
             Slot s0, s1, s2;
             s0.w = s1.w = s2.w = make_double2(0, 0);
             s0.k0 = s0.k1 = s1.k0 = s1.k1 = s2.k0 = s2.k1 = 0u;
             load_slot(0, s0, false); release(0);   // plane z0-1: registers only
-            load_slot(1, s1, true);  release(1);   // plane z0
-            consumer_barrier();
+            load_slot(1, s1, true);  publish(1);   // plane z0
             for (int z = z0; z < z1; z += 3) {     // slots rotate by renaming, not by moving registers
                 step(z, s0, s1, s2);
                 if (z + 1 >= z1) break;
