@@ -63,7 +63,7 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
 #define PF_OPT_CHECK_INTERVAL  5  /* BiCGSTAB iterations enqueued between two host polls of the
                                      device-side convergence flag; default 16; >= 1 */
 #define PF_OPT_WATER_MOLAR     6  /* bath concentration of water, mol/L; default 55.5 (Q12) */
-#define PF_OPT_MAX_OUTER       7  /* cap on outer (Newton) iterations; default 200 */
+#define PF_OPT_MAX_OUTER       7  /* cap on outer (Newton) iterations; default 1000 */
 #define PF_OPT_PRECOND         8  /* 1 = Jacobi M = diag(A) (default, reading Q2); 0 = M = I, Table 3 verbatim */
 #define PF_OPT_HISTORY         9  /* >0: keep the relative residual of every BiCGSTAB iteration of the
                                      last linear solve (up to that many entries); see pf_grid_history */
@@ -144,6 +144,10 @@ int pf_grid_history(pf_grid *g, double *hist_host, int cap);
 /* Per-solve iteration counts of the last pf_solve_pf in call order (initial guess, PF1, PF2, ...). */
 int pf_grid_linear_iters(pf_grid *g, int *iters_host, int cap);
 
+/* ||Phi - Phi0||_inf (after relaxation, Table 2 step 5) of every outer iteration of the last pf_solve_pf.
+ * Returns the number of entries written (<= cap). */
+int pf_grid_increments(pf_grid *g, double *incr_host, int cap);
+
 /* Accumulated device time (ms) and launch count of the three per-iteration kernels since
  * PF_OPT_PROFILE was set: index 0 = p-update + matvec + r~.v (row L4), 1 = s-update + matvec + t.s,
  * t.t (row L5), 2 = x, r update + r~.r, r.r (row L6).  ms_out, launches_out: host, 3 entries. */
@@ -167,7 +171,8 @@ int pf_grid_code_layout(const pf_grid *g, int *bits_out, int *pitch_out, size_t 
  * which = 0: Poisson diagonal A0 (N doubles); 1..6: stored off-diagonals A1..A6 (stored variant
  * only); 7: deposited fixed-charge vector (N doubles); 8: Poisson stencil codes (pf_grid_code_layout
  * bytes); 9: PF1 diagonal (N doubles, after a pf_solve_pf); 10: Poisson coefficient table (16 doubles);
- * 11: PF1 stencil codes; 12: PF1 coefficient table.  Returns PF_ERR_ARG if unavailable. */
+ * 11: PF1 stencil codes; 12: PF1 coefficient table; 13: Psi of the last pf_solve_pf (N doubles).
+ * Returns PF_ERR_ARG if unavailable. */
 int pf_grid_copy_array(pf_grid *g, int which, void *dst_device);
 
 void pf_grid_destroy(pf_grid *g);

@@ -131,6 +131,7 @@ struct pf_grid {
     double* offd[6];
     double* offd_pf1[6];
     std::vector<int> lin_iters;
+    std::vector<double> increments;      // ||Phi - Phi0||_inf of every outer iteration of the last pf_solve_pf
     // per-kernel timing (PF_OPT_PROFILE): events around k1, k2, k3 of every iteration
     std::vector<cudaEvent_t> prof_ev;
     double prof_ms[3];
@@ -378,7 +379,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->stream = (cudaStream_t)cuda_stream;
     g->eps = eps_map;
     g->ncharges = ncharges;
-    g->opt_stencil = 0; g->opt_kernels = 0; g->opt_check = 16; g->opt_lin_maxit = 10000; g->opt_max_outer = 200;
+    g->opt_stencil = 0; g->opt_kernels = 0; g->opt_check = 16; g->opt_lin_maxit = 10000; g->opt_max_outer = 1000;
     g->opt_precond = 1; g->opt_history = 0;
     g->opt_omega_pf = 0.3; g->opt_lin_tol = 1e-10; g->opt_water = 55.5;
     g->ws = nullptr; g->ws_bytes = 0; g->assembled = false; g->stored = false;
@@ -621,6 +622,7 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
         g->pf1_lc = l_c;
     }
     g->lin_iters.clear();
+    g->increments.clear();
     int total = 0, its = 0;
     // row N4 (Table 2 step 2): initial guess from PF2 with rho' = Psi = 0
     launch_copy_with_dirichlet(g->stream, g->g, g->bc, g->fixed, g->bpf);
@@ -655,6 +657,7 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
         PF_CUDA(g, cudaStreamSynchronize(g->stream));
         double d;
         std::memcpy(&d, &bits, sizeof(d));
+        g->increments.push_back(d);
         std::swap(phi0, phiw);
         if (!(d > tol)) { status = PF_OK; break; }
     }
@@ -682,6 +685,13 @@ int pf_grid_linear_iters(pf_grid* g, int* iters_host, int cap) {
     if (!g || !iters_host || cap < 0) return PF_ERR_ARG;
     const int n = std::min<int>(cap, (int)g->lin_iters.size());
     for (int k = 0; k < n; ++k) iters_host[k] = g->lin_iters[k];
+    return n;
+}
+
+int pf_grid_increments(pf_grid* g, double* incr_host, int cap) {
+    if (!g || !incr_host || cap < 0) return PF_ERR_ARG;
+    const int n = std::min<int>(cap, (int)g->increments.size());
+    for (int k = 0; k < n; ++k) incr_host[k] = g->increments[k];
     return n;
 }
 
@@ -717,6 +727,7 @@ int pf_grid_copy_array(pf_grid* g, int which, void* dst) {
     else if (which == 9) src = (g->pf1_lc == g->pf1_lc) ? g->A0_pf1 : nullptr;
     else if (which == 10) { src = g->code_mode ? g->ctab_poisson : nullptr; nbytes = sizeof(double) * PF_CTAB; }
     else if (which == 11) { src = (g->pf1_lc == g->pf1_lc) ? g->code_pf1 : nullptr; nbytes = code_bytes_of(g); }
+    else if (which == 13) src = (g->pf1_lc == g->pf1_lc) ? g->psi : nullptr;
     else if (which == 12) { src = (g->pf1_lc == g->pf1_lc && g->code_mode) ? g->ctab_pf1 : nullptr; nbytes = sizeof(double) * PF_CTAB; }
     if (!src) return fail(g, PF_ERR_ARG, "array %d is not available", which);
     PF_CUDA(g, cudaMemcpyAsync(dst, src, nbytes, cudaMemcpyDeviceToDevice, g->stream));

@@ -28,7 +28,7 @@ KERNELS_AUTO, KERNELS_DIRECT, KERNELS_TILED = 0, 1, 2
 EXPORTS = [
     "pf_grid_create", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
     "pf_solve_linear", "pf_solve_linear_host", "pf_solve_pf", "pf_fermi_pointwise", "pf_grid_history",
-    "pf_grid_linear_iters", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_code_layout", "pf_grid_copy_array",
+    "pf_grid_linear_iters", "pf_grid_increments", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_code_layout", "pf_grid_copy_array",
     "pf_grid_profile", "pf_launch_count", "pf_grid_destroy", "pf_last_error", "pf_version",
 ]
 
@@ -74,6 +74,7 @@ def load():
     L.pf_fermi_pointwise.argtypes = [_vp, ctypes.c_int, _dp, _dp, _dp, _vp, _vp, _vp, _vp, _vp]
     L.pf_grid_history.argtypes = [_vp, _dp, ctypes.c_int]
     L.pf_grid_linear_iters.argtypes = [_vp, _ip, ctypes.c_int]
+    L.pf_grid_increments.argtypes = [_vp, _dp, ctypes.c_int]
     L.pf_grid_stencil.argtypes = [_vp]
     L.pf_grid_palette_size.argtypes = [_vp]
     L.pf_grid_copy_array.argtypes = [_vp, ctypes.c_int, _vp]
@@ -181,7 +182,8 @@ def pf_solve_pf(handle, n: int, valence, bath_conc, radii, l_c: float, tol: floa
     _check(handle, rc)
     its = (ctypes.c_int * (2 * outer.value + 1))()
     m = load().pf_grid_linear_iters(handle, its, len(its))
-    return dict(status=rc, outer_iters=outer.value, linear_iters=lin.value, lin_iters_hist=list(its[:m]))
+    return dict(status=rc, outer_iters=outer.value, linear_iters=lin.value, lin_iters_hist=list(its[:m]),
+                incr_hist=pf_grid_increments(handle, outer.value))
 
 
 def pf_fermi_pointwise(handle, n: int, valence, bath_conc, radii, phi: torch.Tensor,
@@ -198,6 +200,13 @@ def pf_grid_history(handle, cap: int) -> np.ndarray:
     buf = np.empty(cap, dtype=np.float64)
     m = _check(handle, load().pf_grid_history(handle, buf.ctypes.data_as(_dp), cap))
     return buf[:m]
+
+
+def pf_grid_increments(handle, cap: int) -> np.ndarray:
+    """||Phi - Phi0||_inf of every outer iteration of the last pf_solve_pf."""
+    buf = np.empty(max(cap, 1), dtype=np.float64)
+    k = _check(handle, load().pf_grid_increments(handle, buf.ctypes.data_as(_dp), int(buf.size)))
+    return buf[:k].copy()
 
 
 def pf_grid_profile(handle) -> dict:
