@@ -43,7 +43,10 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--n", type=int, default=256, help="grid nodes per direction (configs[3] = 256)")
+    ap.add_argument("--n", type=int, default=0, help="grid nodes per direction (default: 256 for configs[3], 512 for configs[4])")
+    ap.add_argument("--workload", choices=["config3", "config4"], default="config3",
+                    help="config3: the metric's 256^3 channel grid (default); config4: the 512^3 bandwidth stress "
+                         "(100 fixed iterations + one PF pass, BASELINE.json configs[4])")
     ap.add_argument("--stencil", choices=["onthefly", "stored"], default="onthefly")
     ap.add_argument("--kernels", choices=["auto", "direct", "tiled"], default="auto")
     ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
@@ -146,7 +149,8 @@ def run_reference(args):
     from paper_1711_04060_b200 import workloads as wl
     from oracle import pf_oracle as oracle
     oracle.build()
-    w = wl.config3(n=args.n)
+    w, _, wdesc = make_workload(args)
+    args.n = w.nx
     for _ in range(args.warmup):
         oracle_sample(w, 1)
     t0 = time.perf_counter()
@@ -155,11 +159,11 @@ def run_reference(args):
     dt = time.perf_counter() - t0
     value = args.steps * args.ref_iters / dt
     sample = (f"per step: DIA assembly + {args.ref_iters} fixed Jacobi-BiCGSTAB iterations of the {args.n}^3 "
-              f"configs[3] workload, single thread, g++ -O2")
+              f"{args.workload} workload, single thread, g++ -O2")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"configs[3] channel {args.n}^3 fp64, h=0.5 A, seed 3", "sample": sample},
+            "config": {"workload": wdesc, "sample": sample},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -186,13 +190,15 @@ def run_b200(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    w = wl.config3(n=args.n)
+    w, lin_iters, wdesc = make_workload(args)
+    args.n = w.nx
+    step_iters = lin_iters + 3 * PF_INNER_ITERS
     sp = w.species
     n = w.n
     stencil = pf.STENCIL_STORED if args.stencil == "stored" else pf.STENCIL_ONTHEFLY
     kernels = {"auto": 0, "direct": 1, "tiled": 2}[args.kernels]
     rng = np.random.default_rng(3)
-    rhs_np = rng.standard_normal(n)                      # configs[3]: timing RHS, dense random
+    rhs_np = rng.standard_normal(n) if w.rhs is None else w.rhs    # configs[3]: timing RHS, dense random
     eps_host = torch.tensor(w.eps).pin_memory()
     rhs_host = torch.tensor(rhs_np).pin_memory()
     x_host = torch.zeros(n, dtype=torch.float64).pin_memory()
@@ -224,11 +230,11 @@ def run_b200(args):
         pf.pf_grid_set_workspace(h, ws)                                            # rows L1, L2
         if host_buffers:
             x_host.zero_()
-            out = pf.pf_solve_linear_host(h, n, rhs_host, x_host, 0.0, LINEAR_ITERS, true_residual=False)
+            out = pf.pf_solve_linear_host(h, n, rhs_host, x_host, 0.0, lin_iters, true_residual=False)
         else:
             x_dev.zero_()
-            out = pf.pf_solve_linear(h, n, rhs_dev, x_dev, 0.0, LINEAR_ITERS, true_residual=False)   # rows L3-L8
-        assert out["iters"] == LINEAR_ITERS, out
+            out = pf.pf_solve_linear(h, n, rhs_dev, x_dev, 0.0, lin_iters, true_residual=False)   # rows L3-L8
+        assert out["iters"] == lin_iters, out
         res = pf.pf_solve_pf(h, n, sp.valence, sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol, phi_dev)  # N1-N5
         assert res["linear_iters"] == 3 * PF_INNER_ITERS, res
         if host_buffers:
@@ -275,7 +281,7 @@ def run_b200(args):
         step(True, False)
         e2e_steps = max(1, min(args.steps, 3))
         ms_e2e = timed(e2e_steps, True, False)
-        e2e = {"value": world * STEP_ITERS * e2e_steps / (ms_e2e * 1e-3), "unit": UNIT,
+        e2e = {"value": world * step_iters * e2e_steps / (ms_e2e * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": 8 * n * 3, "d2h_bytes_per_step": 8 * n * 2,
                "ms_per_step": ms_e2e / e2e_steps,
                "what": "eps, rhs, x0 host->device; x, phi device->host; C-ABI pf_solve_linear_host"}
@@ -316,21 +322,20 @@ def run_b200(args):
         if not args.no_cpu_baseline and world == 1:
             from oracle import pf_oracle as oracle
             oracle.build()
-            cpu_iters = 12 if args.n >= 256 else 100
+            cpu_iters = 3 if args.n >= 512 else (12 if args.n >= 256 else 100)
             dt = oracle_sample(w, cpu_iters)
             cpu = {"value": cpu_iters / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                    "host_cores_available": os.cpu_count(),
                    "sample": f"DIA assembly + {cpu_iters} fixed Jacobi-BiCGSTAB iterations of the same {args.n}^3 "
                              f"workload ({dt:.1f} s), single thread, g++ -O2"}
-        value = world * STEP_ITERS * args.steps / (ms_total * 1e-3)
+        value = world * step_iters * args.steps / (ms_total * 1e-3)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": f"configs[3] channel {args.n}^3 fp64 (slab 60 A, pore 8 A, 1536 charges, seed 3), "
-                                       f"h=0.5 A; step = assembly + {LINEAR_ITERS} fixed Jacobi-BiCGSTAB iterations + "
+                "config": {"workload": f"{wdesc}; step = assembly + {lin_iters} fixed Jacobi-BiCGSTAB iterations + "
                                        f"one PF outer pass with 3x{PF_INNER_ITERS} inner iterations",
                            "stencil": args.stencil, "kernels": args.kernels, "unknowns": n,
-                           "iterations_per_step": STEP_ITERS, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                           "iterations_per_step": step_iters, "parallelism": "replicas only" if world > 1 else "1 GPU",
                            "l2": "inputs larger than L2 (working set %.1f GB)" % (ws.numel() / 1e9)},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
                 "paper_context": "paper: 22.8x linear-solver, 16.9x total speedup, GTX TITAN X vs Xeon E5-1650 "
@@ -338,6 +343,18 @@ def run_b200(args):
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def make_workload(args):
+    """(workload, linear iterations per step, description)."""
+    from paper_1711_04060_b200 import workloads as wl
+    if args.workload == "config4":
+        n = args.n or 512
+        return wl.config4(n=n), 100, (f"configs[4] bandwidth stress {n}^3 fp64 (random spheres eps 2/80, 30 % fill, seed 4, "
+                                      f"Gaussian-smeared right-hand side), h=0.5 A")
+    n = args.n or 256
+    return wl.config3(n=n), LINEAR_ITERS, (f"configs[3] channel {n}^3 fp64 (slab 60 A, pore 8 A, 1536 charges, seed 3), "
+                                           f"h=0.5 A")
 
 
 def main():

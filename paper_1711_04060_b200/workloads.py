@@ -272,9 +272,23 @@ def config3(n: int = 256) -> Workload:
 
 
 def config4(n: int = 512) -> Workload:
-    """512^3 bandwidth stress: cfg-1 generator, seed 4, plus NaCl species for one PF step."""
-    w = config1(n=n, seed=4, ncharges=500 if n >= 256 else 100)
+    """512^3 bandwidth stress: cfg-1 generator, seed 4, plus NaCl species for one PF step.
+
+    The linear solve uses the Gaussian-smeared right-hand side; the PF step needs fixed charges in the
+    library's own form (point charges, deposited by the method), so the workload also carries the same number
+    of point charges q ~ U[-1,1] e at uniform positions at least five cells inside the box (own seed)."""
+    ncharges = 500 if n >= 256 else 100
+    w = config1(n=n, seed=4, ncharges=ncharges)
     w.name = f"cfg4_stress_{n}"
     w.species = NACL
     w.l_c = 1.2
+    rng = SplitMix64(1004)
+    L = (n - 1) * w.h
+    ch = np.zeros((ncharges, 4))
+    for k in range(ncharges):
+        ch[k, 0] = rng.uniform_range(5 * w.h, L - 5 * w.h)
+        ch[k, 1] = rng.uniform_range(5 * w.h, L - 5 * w.h)
+        ch[k, 2] = rng.uniform_range(5 * w.h, L - 5 * w.h)
+        ch[k, 3] = rng.uniform_range(-1.0, 1.0)
+    w.charges = ch
     return w
