@@ -19,10 +19,11 @@
 //   MODE_K1  u = M^-1 (r + beta (p - omega v))  (steps 5-9, Jacobi Q2), v' = A u (step 11), r~.v'
 //   MODE_K2  u = M^-1 (r - alpha v)             (step 13),            t  = A u (step 14), t.s, t.t
 //   MODE_R0  u = x,  r = b - A u, r~ = r, b.b, r.r (step 2);  MODE_R1: ||b - A x||^2 only
-// u of the plane being differenced sits in shared memory (xy neighbours, double-buffered); the z
+// u of the plane being differenced sits in shared memory (xy neighbours, three buffers); the z
 // neighbours stay in registers of the marching thread (three register slots renamed, not moved, by a
-// three-way unrolled loop).  Per plane: wait for the stage, form u(z+1), release the stage, difference
-// plane z, one named barrier among the consumer warps.
+// three-way unrolled loop).  Per plane: wait for the stage, form u(z+1), publish it and release the stage,
+// difference plane z.  There is no block-wide barrier in the loop: a "ready" mbarrier per u buffer (one
+// arrival per consumer warp) orders the writers and readers of the buffers, so warps drift by up to a plane.
 //
 // Arithmetic is the same statement for statement as the direct kernels (pf_krylov_direct.cu): both
 // families give bit-identical vectors.
