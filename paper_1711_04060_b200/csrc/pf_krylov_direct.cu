@@ -175,6 +175,8 @@ __device__ __forceinline__ void k3_point(const K3Elem& e, double alpha, double o
 template <bool VEC>
 __global__ void __launch_bounds__(256, 3)
 k3_update(long long n, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
+    pdl_launch_dependents();
+    pdl_wait();
     if (sc->done) return;
     __shared__ dd scratch[2 * 32];
     const double alpha = sc->alpha, omega = sc->omega;
@@ -272,8 +274,8 @@ void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, boo
     const bool vec = (((uintptr_t)kv.y | (uintptr_t)kv.r | (uintptr_t)kv.v_out | (uintptr_t)kv.p_out | (uintptr_t)kv.t |
                        (uintptr_t)kv.rt) & 15u) == 0;
     ++g_launch_count;
-    if (vec) k3_update<true><<<nb, 256, 0, c.stream>>>(c.g.n, kv, c.sc, c.rb);
-    else     k3_update<false><<<nb, 256, 0, c.stream>>>(c.g.n, kv, c.sc, c.rb);
+    if (vec) launch_pdl(k3_update<true>, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, c.sc, c.rb);
+    else     launch_pdl(k3_update<false>, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, c.sc, c.rb);
 }
 
 void launch_finish_x(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv) {

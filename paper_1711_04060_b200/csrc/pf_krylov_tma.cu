@@ -159,7 +159,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     using T = ModeTraits<MODE>;
     constexpr int S = T::STAGES;
     constexpr int NF = T::NF;
-    if (MODE >= MODE_K1 && sc->done) return;
+    pdl_launch_dependents();
     extern __shared__ __align__(128) unsigned char smem[];
     double* ctab_s = reinterpret_cast<double*>(smem + L::CTAB_OFF);
     dd* scratch = reinterpret_cast<dd*>(smem + L::SCRATCH_OFF);
@@ -182,6 +182,8 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     if (!STORED && tid < PF_CTAB) ctab_s[tid] = op.ctab[tid];
     const unsigned ctab_addr = smem_u32(ctab_s);           // 128-byte aligned: CTAB_OFF and the smem base are
     __syncthreads();
+    pdl_wait();                                            // everything above is independent of the previous kernel
+    if (MODE >= MODE_K1 && sc->done) return;
 
     dd q[2] = {dd_zero(), dd_zero()};
     unsigned fault = 0u;
@@ -484,7 +486,7 @@ void launch_inst(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, c
         configured = true;
     }
     ++g_launch_count;
-    kern<<<grid, NT, L::TOTAL, c.stream>>>(tm, c.g, op, kv, c.sc, c.rb, depth);
+    launch_pdl(kern, grid, dim3(NT), (size_t)L::TOTAL, c.stream, tm, c.g, op, kv, c.sc, c.rb, depth);
 }
 
 template <int MODE>

@@ -9,6 +9,21 @@ namespace pf {
 // Kernel launches issued by this library since load (bench.py reports the difference over the timed region).
 extern long long g_launch_count;
 
+// Launch with programmatic dependent launch allowed: the grid may be scheduled while the preceding kernel of
+// the stream drains (its blocks run their prologue on SMs that are already free); the kernel itself calls
+// pdl_wait() before it touches anything the preceding kernel wrote.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+                              Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 struct LaunchCtx {
     cudaStream_t stream;
     GridDims g;
