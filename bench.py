@@ -43,7 +43,7 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--n", type=int, default=0, help="grid nodes per direction (default: 256 for configs[3], 512 for configs[4])")
+    ap.add_argument("--n", "--grid", dest="n", type=int, default=0, help="grid nodes per direction (default: 256 for configs[3], 512 for configs[4])")
     ap.add_argument("--workload", choices=["config3", "config4"], default="config3",
                     help="config3: the metric's 256^3 channel grid (default); config4: the 512^3 bandwidth stress "
                          "(100 fixed iterations + one PF pass, BASELINE.json configs[4])")
