@@ -156,6 +156,10 @@ int pf_grid_profile(pf_grid *g, double *ms_out, long long *launches_out);
 /* Kernel launches issued by the library in this process so far. */
 long long pf_launch_count(void);
 
+/* Number of linear solves of this grid that were repeated by the direct kernels because the tiled kernels met
+ * operands outside the range of their branch-free division (reading D4 of DESIGN.md). */
+int pf_grid_fault_repeats(const pf_grid *g);
+
 /* Introspection used by the tests: 1 = stored, 2 = on-the-fly; number of palette entries. */
 int pf_grid_stencil(const pf_grid *g);
 int pf_grid_palette_size(const pf_grid *g);

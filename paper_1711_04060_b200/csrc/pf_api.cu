@@ -138,6 +138,7 @@ struct pf_grid {
     long long prof_launches[3];
     int opt_profile;
     int last_iters;
+    int fault_repeats;       // solves repeated by the direct kernels after a division range fault (D4)
     std::string err;
 };
 
@@ -275,6 +276,7 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
         // operands outside the range of the tiled kernels' branch-free division (pf_common.cuh dvd_nb): x has
         // not been touched yet (D3), so the solve is simply repeated with the kernels that use __ddiv_rn
         PF_CUDA(g, cudaStreamSynchronize(g->stream));
+        ++g->fault_repeats;
         return bicgstab_device(g, op, b, x, tol, maxit, iters_out, relres_out, true_relres_out, false);
     }
     if (precond) launch_finish_x(c, op, kv);
@@ -386,7 +388,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->pf1_lc = std::nan("");
     g->opt_profile = 0; g->prof_ms[0] = g->prof_ms[1] = g->prof_ms[2] = 0.0;
     g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
-    g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0;
+    g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
     g->small = nullptr;
     g->charges_dev = nullptr; g->sc = nullptr; g->rb.partial = nullptr; g->rb.ticket = nullptr;
     g->ctab_poisson = g->ctab_pf1 = nullptr; g->dmax_bits = nullptr; g->tma = nullptr;
@@ -702,6 +704,8 @@ int pf_grid_profile(pf_grid* g, double* ms_out, long long* launches_out) {
     for (int j = 0; j < 3; ++j) { ms_out[j] = g->prof_ms[j]; launches_out[j] = g->prof_launches[j]; }
     return PF_OK;
 }
+
+int pf_grid_fault_repeats(const pf_grid* g) { return g ? g->fault_repeats : PF_ERR_ARG; }
 
 int pf_grid_stencil(const pf_grid* g) { return g ? (want_stored(g) ? 1 : 2) : PF_ERR_ARG; }
 int pf_grid_palette_size(const pf_grid* g) { return g ? g->pal.count : PF_ERR_ARG; }

@@ -28,7 +28,7 @@ KERNELS_AUTO, KERNELS_DIRECT, KERNELS_TILED = 0, 1, 2
 EXPORTS = [
     "pf_grid_create", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
     "pf_solve_linear", "pf_solve_linear_host", "pf_solve_pf", "pf_fermi_pointwise", "pf_grid_history",
-    "pf_grid_linear_iters", "pf_grid_increments", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_code_layout", "pf_grid_copy_array",
+    "pf_grid_linear_iters", "pf_grid_increments", "pf_grid_fault_repeats", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_code_layout", "pf_grid_copy_array",
     "pf_grid_profile", "pf_launch_count", "pf_grid_destroy", "pf_last_error", "pf_version",
 ]
 
@@ -75,6 +75,7 @@ def load():
     L.pf_grid_history.argtypes = [_vp, _dp, ctypes.c_int]
     L.pf_grid_linear_iters.argtypes = [_vp, _ip, ctypes.c_int]
     L.pf_grid_increments.argtypes = [_vp, _dp, ctypes.c_int]
+    L.pf_grid_fault_repeats.argtypes = [_vp]
     L.pf_grid_stencil.argtypes = [_vp]
     L.pf_grid_palette_size.argtypes = [_vp]
     L.pf_grid_copy_array.argtypes = [_vp, ctypes.c_int, _vp]
@@ -218,6 +219,10 @@ def pf_grid_profile(handle) -> dict:
 
 def pf_launch_count() -> int:
     return int(load().pf_launch_count())
+
+
+def pf_grid_fault_repeats(handle) -> int:
+    return load().pf_grid_fault_repeats(handle)
 
 
 def pf_grid_stencil(handle) -> int:
