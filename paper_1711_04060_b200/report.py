@@ -1,0 +1,161 @@
+"""Report table of BASELINE.md section 4: one row per config x stencil variant, GPU next to the CPU oracle.
+
+    python -m paper_1711_04060_b200.report [--out gpurun_out/report.md] [--skip-512]
+
+Needs a CUDA device (the GPU columns) and builds the oracle for the CPU columns; the oracle is only ever
+run where it finishes in about a minute (full solves up to 64^3, a few iterations beyond).
+"""
+from __future__ import annotations
+
+import argparse
+import os
+import sys
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1711_04060_b200 import pf, workloads as wl  # noqa: E402
+
+PEAK_NOMINAL = 8000.0
+
+
+def measured_peak():
+    import json
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"])
+    except Exception:
+        return 6650.0
+
+
+def bytes_per_iter(stored: bool) -> int:
+    return 248 if stored else 156
+
+
+def rel_l2(a, b):
+    d = np.linalg.norm(b)
+    return float(np.linalg.norm(a - b) / (d if d > 0 else 1.0))
+
+
+def gpu_fixed_iterations(w, rhs, stencil, iters):
+    """ms per iteration of `iters` fixed iterations (second of two runs), whole-solve CUDA-event time."""
+    g = pf.Grid.from_workload(w, stencil=stencil)
+    x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+    rhs_d = torch.as_tensor(rhs, dtype=torch.float64).cuda()
+    ms = None
+    for _ in range(2):
+        x.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        pf.pf_solve_linear(g.handle, w.n, rhs_d, x, 0.0, iters, true_residual=False)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / iters
+    g.close()
+    return ms
+
+
+def linear_rows(name, w, rhs, oracle, oracle_full: bool, oracle_iters: int, peak):
+    rows = []
+    ref = None
+    o_s_per_it = None
+    if oracle_full:
+        t0 = time.perf_counter()
+        ref = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, rhs, tol=1e-10)
+        o_s_per_it = (time.perf_counter() - t0) / max(ref["iters"], 1)
+    elif oracle_iters:
+        t0 = time.perf_counter()
+        oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, rhs, tol=0.0, maxit=oracle_iters)
+        o_s_per_it = (time.perf_counter() - t0) / oracle_iters
+    for stencil, sname in ((pf.STENCIL_STORED, "stored"), (pf.STENCIL_ONTHEFLY, "on-the-fly")):
+        g = pf.Grid.from_workload(w, stencil=stencil)
+        out = g.solve_linear(rhs, tol=1e-10)
+        x = out["x"].cpu().numpy()
+        g.close()
+        ms = gpu_fixed_iterations(w, rhs, stencil, 200 if w.n >= 128 ** 3 else 400)
+        bpi = bytes_per_iter(stencil == pf.STENCIL_STORED)
+        gbs = bpi * w.n / (ms * 1e-3) / 1e9
+        rows.append(dict(config=name, N=w.n, variant=sname,
+                         iters=f"{out['iters']} / {ref['iters'] if ref else 'n/a'}",
+                         relres=f"{out['true_relres']:.2e}",
+                         diff=f"{rel_l2(x, ref['x']):.1e}" if ref else "n/a",
+                         ms=f"{ms:.4f}", its=f"{1e3 / ms:.0f}", mup=f"{w.n / ms / 1e3:.0f}", bpi=bpi,
+                         gbs=f"{gbs:.0f}", p8=f"{100 * gbs / PEAK_NOMINAL:.0f} %", pm=f"{100 * gbs / peak:.0f} %",
+                         osit=f"{o_s_per_it:.3f}" if o_s_per_it else "n/a", outer="-", pft="-"))
+    return rows
+
+
+def pf_row(name, w, oracle, oracle_full: bool):
+    sp = w.species
+    g = pf.Grid.from_workload(w)
+    g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol, want_conc=False)   # warm-up
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    out = g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol)
+    torch.cuda.synchronize()
+    tg = time.perf_counter() - t0
+    g.close()
+    to, diff, oiters = None, "n/a", "n/a"
+    if oracle_full:
+        t0 = time.perf_counter()
+        ref = oracle.solve_pf(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, w.charges, sp.valence,
+                              sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol, lin_tol=w.linear_tol, max_outer=1000)
+        to = time.perf_counter() - t0
+        diff = f"{rel_l2(out['phi'].cpu().numpy(), ref['phi']):.1e}"
+        oiters = f"{ref['outer_iters']} ({ref['linear_iters']} lin.)"
+    return dict(config=name, N=w.n, variant="PF (auto)", iters=f"{out['linear_iters']} lin. / {oiters}",
+                relres="-", diff=diff, ms=f"{1e3 * tg / max(out['linear_iters'], 1):.4f}", its="-", mup="-", bpi="-",
+                gbs="-", p8="-", pm="-", osit="-", outer=str(out["outer_iters"]),
+                pft=f"{tg:.2f} s / {to:.0f} s" if to else f"{tg:.2f} s / n/a")
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "report.md"))
+    ap.add_argument("--skip-512", action="store_true")
+    args = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise RuntimeError("report needs a CUDA device")
+    pf.load()
+    from oracle import pf_oracle as oracle
+    oracle.build()
+    peak = measured_peak()
+    rows = []
+    w = wl.config0()
+    rows += linear_rows("0 (32^3 channel)", w, oracle.deposit_charges(w.nx, w.ny, w.nz, w.h, w.charges), oracle, True, 0, peak)
+    rows.append(pf_row("0 (32^3 channel)", w, oracle, True))
+    w = wl.config1()
+    rows += linear_rows("1 (64^3 spheres)", w, w.rhs, oracle, True, 0, peak)
+    w = wl.config2(volt_mv=50.0)
+    rows += linear_rows("2 (128^3 channel, +50 mV)", w, oracle.deposit_charges(w.nx, w.ny, w.nz, w.h, w.charges), oracle,
+                        False, 20, peak)
+    rows.append(pf_row("2 (128^3 channel, +50 mV)", w, oracle, False))
+    w = wl.config3()
+    rows += linear_rows("3 (256^3 channel)", w, oracle.deposit_charges(w.nx, w.ny, w.nz, w.h, w.charges), oracle, False, 6,
+                        peak)
+    if not args.skip_512:
+        w = wl.config4()
+        rows += linear_rows("4 (512^3 spheres)", w, w.rhs, oracle, False, 0, peak)
+    hdr = ["config", "N", "variant", "iters to 1e-10 (GPU / oracle)", "true rel. residual", "rel. L2 diff vs oracle",
+           "ms/iter", "iterations/s", "Mupdates/s", "model B/unknown/iter", "effective GB/s (model)", "% of 8.0 TB/s",
+           f"% of {peak / 1e3:.2f} TB/s", "oracle s/iter (1 core)", "PF outer iters", "PF total time GPU / oracle"]
+    keys = ["config", "N", "variant", "iters", "relres", "diff", "ms", "its", "mup", "bpi", "gbs", "p8", "pm", "osit",
+            "outer", "pft"]
+    lines = ["| " + " | ".join(hdr) + " |", "|" + "---|" * len(hdr)]
+    for r in rows:
+        lines.append("| " + " | ".join(str(r[k]) for k in keys) + " |")
+    text = "\n".join(lines) + "\n"
+    os.makedirs(os.path.dirname(args.out), exist_ok=True)
+    with open(args.out, "w") as f:
+        f.write(text)
+    print(text)
+
+
+if __name__ == "__main__":
+    main()
