@@ -76,6 +76,9 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
                                      linear solve with CUDA events and accumulate their durations
                                      (pf_grid_profile); setting it resets the sums; 0 = off */
 
+#define PF_OPT_GRAPH          12  /* 1 (default): on grids of up to 2^22 unknowns, which are bound by launch latency,
+                                     replay each polling chunk of iterations as one CUDA graph; 0 = plain launches */
+
 /* Create a grid: store geometry and boundary conditions, scan eps_map for its palette of distinct
  * values, keep a device copy of the charges.  Assembly itself runs in pf_grid_set_workspace.
  *   eps_map : device, nx*ny*nz doubles, relative permittivity per node; borrowed.

@@ -138,6 +138,11 @@ struct pf_grid {
     long long prof_launches[3];
     int opt_profile;
     int last_iters;
+    // CUDA graphs of one polling chunk of iterations, for grids small enough to be launch-bound
+    struct ChunkGraph { const void *a0, *code, *b, *x, *y, *hist; int precond, tiled, chunk; cudaGraphExec_t exec; };
+    std::vector<ChunkGraph> graphs;
+    cudaStream_t capture_stream;
+    int opt_graph;
     int fault_repeats;       // solves repeated by the direct kernels after a division range fault (D4)
     std::string err;
 };
@@ -198,8 +203,55 @@ Operator make_op(const pf_grid* g, int which /*0 poisson, 1 pf1, 2 poisson+sigma
 
 LaunchCtx make_ctx(const pf_grid* g) {
     LaunchCtx c;
-    c.stream = g->stream; c.g = g->g; c.sc = g->sc; c.rb = g->rb; c.sm_count = g->sm_count;
+    c.stream = g->stream; c.g = g->g; c.sc = g->sc; c.rb = g->rb; c.sm_count = g->sm_count; c.pdl = true;
     return c;
+}
+
+// One BiCGSTAB iteration = three launches (rows L4, L5, L6).  kv's (p, v) buffers are swapped on return.
+void enqueue_iteration(const LaunchCtx& c, const Operator& op, KrylovVecs& kv, const TmaSet* tma, bool tiled,
+                       bool precond, int parity, cudaEvent_t* pe) {
+    if (pe) cudaEventRecord(pe[0], c.stream);
+    if (tiled) launch_k1_tma(c, op, kv, tma, precond, parity); else launch_k1_direct(c, op, kv, precond);
+    if (pe) cudaEventRecord(pe[1], c.stream);
+    if (tiled) launch_k2_tma(c, op, kv, tma, precond, parity); else launch_k2_direct(c, op, kv, precond);
+    if (pe) cudaEventRecord(pe[2], c.stream);
+    launch_k3(c, op, kv, precond);
+    if (pe) cudaEventRecord(pe[3], c.stream);
+    std::swap(kv.p_in, kv.p_out);     // k1 read (p_in, v_in) and wrote (p_out, v_out)
+    std::swap(kv.v_in, kv.v_out);
+}
+
+// Grids of up to ~4 M unknowns are bound by launch latency, not by HBM: one polling chunk of iterations
+// (an even number, so the (p, v) double buffers are back in place) is captured once into a CUDA graph per
+// (operator, vectors, kernel family) and replayed.  Returns null when graphs do not apply.
+cudaGraphExec_t chunk_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool tiled,
+                            bool precond, int chunk) {
+    if (!g->opt_graph || g->opt_profile || (chunk & 1) || g->g.n > (1ll << 22)) return nullptr;
+    for (const auto& cg : g->graphs)
+        if (cg.a0 == op.A0 && cg.code == op.code && cg.b == kv.b && cg.x == kv.x && cg.y == kv.y && cg.hist == kv.hist &&
+            cg.precond == (int)precond && cg.tiled == (int)tiled && cg.chunk == chunk)
+            return cg.exec;
+    if (!g->capture_stream &&
+        cudaStreamCreateWithFlags(&g->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError(); g->opt_graph = 0; return nullptr;
+    }
+    LaunchCtx cc = c;
+    cc.stream = g->capture_stream; cc.pdl = false;
+    KrylovVecs kc = kv;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    const long long launches0 = pf::g_launch_count;
+    bool ok = cudaStreamBeginCapture(cc.stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+    if (ok) {
+        for (int k = 0; k < chunk; ++k) enqueue_iteration(cc, op, kc, g->tma, tiled, precond, k & 1, nullptr);
+        ok = cudaStreamEndCapture(cc.stream, &graph) == cudaSuccess && graph;
+    }
+    pf::g_launch_count = launches0;            // nothing ran; replays are counted where they are launched
+    if (ok) ok = cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess;
+    if (graph) cudaGraphDestroy(graph);
+    if (!ok) { cudaGetLastError(); g->opt_graph = 0; return nullptr; }
+    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled, chunk, exec});
+    return exec;
 }
 
 // ---- Table 3 on the device ----------------------------------------------------------------
@@ -240,19 +292,16 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     // never idles on the host; kernels launched after convergence return at once (sc->done).
     while (!done) {
         const int todo = std::min(chunk, maxit - launched);
-        for (int k = 0; k < todo; ++k) {
-            const bool prof = g->opt_profile && (size_t)(4 * (launched + k) + 3) < g->prof_ev.size();
-            cudaEvent_t* pe = prof ? &g->prof_ev[4 * (launched + k)] : nullptr;
-            if (prof) cudaEventRecord(pe[0], g->stream);
-            const int parity = (launched + k) & 1;
-            if (tiled) launch_k1_tma(c, op, kv, g->tma, precond, parity); else launch_k1_direct(c, op, kv, precond);
-            if (prof) cudaEventRecord(pe[1], g->stream);
-            if (tiled) launch_k2_tma(c, op, kv, g->tma, precond, parity); else launch_k2_direct(c, op, kv, precond);
-            if (prof) cudaEventRecord(pe[2], g->stream);
-            launch_k3(c, op, kv, precond);
-            if (prof) cudaEventRecord(pe[3], g->stream);
-            std::swap(kv.p_in, kv.p_out);     // k1 read (p_in, v_in) and wrote (p_out, v_out)
-            std::swap(kv.v_in, kv.v_out);
+        cudaGraphExec_t exec = todo == chunk ? chunk_graph(g, c, op, kv, tiled, precond, chunk) : nullptr;
+        if (exec) {
+            PF_CUDA(g, cudaGraphLaunch(exec, g->stream));
+            pf::g_launch_count += 3ll * chunk;
+        } else {
+            for (int k = 0; k < todo; ++k) {
+                const bool prof = g->opt_profile && (size_t)(4 * (launched + k) + 3) < g->prof_ev.size();
+                enqueue_iteration(c, op, kv, g->tma, tiled, precond, (launched + k) & 1,
+                                  prof ? &g->prof_ev[4 * (launched + k)] : nullptr);
+            }
         }
         launched += todo;
         PF_CUDA(g, cudaMemcpyAsync(g->sc_host[slot], g->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
@@ -389,6 +438,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->opt_profile = 0; g->prof_ms[0] = g->prof_ms[1] = g->prof_ms[2] = 0.0;
     g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
+    g->capture_stream = nullptr; g->opt_graph = 1;
     g->small = nullptr;
     g->charges_dev = nullptr; g->sc = nullptr; g->rb.partial = nullptr; g->rb.ticket = nullptr;
     g->ctab_poisson = g->ctab_pf1 = nullptr; g->dmax_bits = nullptr; g->tma = nullptr;
@@ -439,6 +489,8 @@ void pf_grid_destroy(pf_grid* g) {
     if (!g) return;
     cudaStreamSynchronize(g->stream);
     small_set_release(g->small);
+    for (auto& cg : g->graphs) cudaGraphExecDestroy(cg.exec);
+    if (g->capture_stream) cudaStreamDestroy(g->capture_stream);
     cudaFree(g->hist);
     if (g->tma) tma_set_destroy(g->tma);
     for (cudaEvent_t e : g->prof_ev) cudaEventDestroy(e);
@@ -509,6 +561,8 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
             for (int j = 0; j < 3; ++j) { g->prof_ms[j] = 0.0; g->prof_launches[j] = 0; }
             return PF_OK;
         }
+        case PF_OPT_GRAPH:
+            g->opt_graph = iv != 0; return PF_OK;
         case PF_OPT_KERNELS:
             if (iv < 0 || iv > 2) return fail(g, PF_ERR_ARG, "kernels must be 0, 1 or 2");
             if (iv == 2 && !(tma_supported(g->g) && tma_available()))

@@ -274,8 +274,8 @@ void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, boo
     const bool vec = (((uintptr_t)kv.y | (uintptr_t)kv.r | (uintptr_t)kv.v_out | (uintptr_t)kv.p_out | (uintptr_t)kv.t |
                        (uintptr_t)kv.rt) & 15u) == 0;
     ++g_launch_count;
-    if (vec) launch_pdl(k3_update<true>, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, c.sc, c.rb);
-    else     launch_pdl(k3_update<false>, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, c.sc, c.rb);
+    if (vec) launch_pdl(c.pdl, k3_update<true>, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, c.sc, c.rb);
+    else     launch_pdl(c.pdl, k3_update<false>, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, c.sc, c.rb);
 }
 
 void launch_finish_x(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv) {

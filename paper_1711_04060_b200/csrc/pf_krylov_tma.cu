@@ -486,7 +486,7 @@ void launch_inst(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, c
         configured = true;
     }
     ++g_launch_count;
-    launch_pdl(kern, grid, dim3(NT), (size_t)L::TOTAL, c.stream, tm, c.g, op, kv, c.sc, c.rb, depth);
+    launch_pdl(c.pdl, kern, grid, dim3(NT), (size_t)L::TOTAL, c.stream, tm, c.g, op, kv, c.sc, c.rb, depth);
 }
 
 template <int MODE>

@@ -13,14 +13,14 @@ extern long long g_launch_count;
 // the stream drains (its blocks run their prologue on SMs that are already free); the kernel itself calls
 // pdl_wait() before it touches anything the preceding kernel wrote.
 template <typename... KArgs, typename... Args>
-inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+inline cudaError_t launch_pdl(bool pdl, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
                               Args&&... args) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;      // off while a CUDA graph is being captured
     return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
@@ -30,6 +30,7 @@ struct LaunchCtx {
     Scalars* sc;      // device
     ReduceBuf rb;     // device
     int sm_count;
+    bool pdl;         // programmatic dependent launch allowed
 };
 
 // ---- Krylov kernels -----------------------------------------------------------------------
