@@ -132,7 +132,10 @@ def deposit_charges(nx, ny, nz, h, charges) -> np.ndarray:
     return b
 
 
-def bicgstab(nx, ny, nz, A, b, x0=None, tol=1e-10, maxit=10000, precond=True, history=False):
+NORM_REL_L2, NORM_ABS_INF = 0, 1     # stopping test: BASELINE's relative 2-norm / the paper's absolute maximum norm
+
+
+def bicgstab(nx, ny, nz, A, b, x0=None, tol=1e-10, maxit=10000, precond=True, history=False, norm=NORM_REL_L2):
     """Table 3 (+Jacobi).  Returns dict(x, status, iters, relres, true_relres[, hist])."""
     A = _f64(A)
     b = _f64(b)
@@ -143,7 +146,8 @@ def bicgstab(nx, ny, nz, A, b, x0=None, tol=1e-10, maxit=10000, precond=True, hi
     tr = ctypes.c_double(0)
     hist = np.full(maxit + 1, np.nan) if history else None
     st = lib().pfo_bicgstab(nx, ny, nz, _d(A), _d(b), _d(x), ctypes.c_double(tol), int(maxit),
-                            int(bool(precond)), ctypes.byref(it), ctypes.byref(rr), ctypes.byref(tr), _d(hist))
+                            int(bool(precond)), ctypes.byref(it), ctypes.byref(rr), ctypes.byref(tr), _d(hist),
+                            int(norm))
     out = dict(x=x, status=st, iters=it.value, relres=rr.value, true_relres=tr.value)
     if history:
         out["hist"] = hist[: it.value + 1]
@@ -151,7 +155,7 @@ def bicgstab(nx, ny, nz, A, b, x0=None, tol=1e-10, maxit=10000, precond=True, hi
 
 
 def solve_linear(nx, ny, nz, h, bc_type, bc_value, eps, rhs, x0=None, sigma=None, tol=1e-10,
-                 maxit=10000, precond=True, history=False):
+                 maxit=10000, precond=True, history=False, norm=NORM_REL_L2):
     """What pf_solve_linear computes: the grid's Poisson operator, Dirichlet data forced."""
     n = nx * ny * nz
     t, v = _bc(bc_type, bc_value)
@@ -165,7 +169,7 @@ def solve_linear(nx, ny, nz, h, bc_type, bc_value, eps, rhs, x0=None, sigma=None
     hist = np.full(maxit + 1, np.nan) if history else None
     st = lib().pfo_solve_linear(nx, ny, nz, ctypes.c_double(h), _i(t), _d(v), _d(eps), _d(sigma), _d(rhs),
                                 _d(x), ctypes.c_double(tol), int(maxit), int(bool(precond)),
-                                ctypes.byref(it), ctypes.byref(rr), ctypes.byref(tr), _d(hist))
+                                ctypes.byref(it), ctypes.byref(rr), ctypes.byref(tr), _d(hist), int(norm))
     out = dict(x=x, status=st, iters=it.value, relres=rr.value, true_relres=tr.value)
     if history:
         out["hist"] = hist[: it.value + 1]
@@ -193,7 +197,7 @@ def fermi_pointwise(valence, bath_molar, radii, phi, solvent=None, water_molar=5
 
 
 def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar, radii, l_c, tol,
-             omega_pf=0.3, lin_tol=1e-10, lin_maxit=10000, max_outer=200, water_molar=55.5):
+             omega_pf=0.3, lin_tol=1e-10, lin_maxit=10000, max_outer=200, water_molar=55.5, norm=NORM_REL_L2):
     """The outer loop of Table 2 / Table 4 (R5)."""
     n = nx * ny * nz
     t, v = _bc(bc_type, bc_value)
@@ -215,7 +219,7 @@ def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar
     st = lib().pfo_solve_pf(nx, ny, nz, ctypes.c_double(h), _i(t), _d(v), _d(eps), _d(ch), int(ch.shape[0]),
                             int(K), _d(valence), _d(bath), _d(radii), ctypes.c_double(water_molar),
                             ctypes.c_double(l_c), ctypes.c_double(tol), ctypes.c_double(omega_pf),
-                            ctypes.c_double(lin_tol), int(lin_maxit), int(max_outer),
+                            ctypes.c_double(lin_tol), int(lin_maxit), int(max_outer), int(norm),
                             _d(phi), _d(psi), _d(conc), _d(steric), ctypes.byref(outer), ctypes.byref(lin),
                             _i(lhist), int(cap), _d(ihist))
     return dict(phi=phi, psi=psi, conc=conc, steric=steric, status=st, outer_iters=outer.value,

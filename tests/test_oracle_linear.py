@@ -231,3 +231,37 @@ def test_degenerate_cases(oracle):
     bv = [0.5, 0.5, 0.5, 0.5, 0.5, 0.5]
     r4 = oracle.solve_linear(n, n, n, h, [D] * 6, bv, eps, np.zeros(N), tol=1e-13)
     assert np.allclose(r4["x"], 0.5, atol=1e-12)      # harmonic, constant data => constant
+
+
+def test_paper_stopping_test_max_norm(oracle):
+    """Table 3 steps 18-19 as the paper writes them: stop when ||r||_inf < ErrTol, absolute.
+    The oracle's max-norm mode follows an independent numpy run of Table 3 and stops at the first iterate whose
+    maximum norm is below the tolerance."""
+    n, h = 10, 0.5
+    bt, bv = [D] * 6, [0.0] * 6
+    eps, sigma, rhs = _random_problem(n, 5, bt, bv)
+    A = oracle.assemble_poisson(n, n, n, h, bt, bv, eps, sigma)
+    b = oracle.set_dirichlet(n, n, n, bt, bv, rhs)
+    mv = lambda u: oracle.dia_spmv(n, n, n, A, u)
+    tol = 1e-6
+    # numpy Table 3 run long enough, recording max norms
+    x = np.zeros(n ** 3); r = b - mv(x); rt = r.copy(); p = v = None; rho_old = alpha = omega = 1.0
+    maxn = [np.abs(r).max()]
+    for i in range(1, 400):
+        rho = rt @ r
+        p = r.copy() if i == 1 else r + (rho * alpha) / (rho_old * omega) * (p - omega * v)
+        v = mv(p); alpha = rho / (rt @ v); s = r - alpha * v; t = mv(s); omega = (t @ s) / (t @ t)
+        x = x + alpha * p + omega * s; r = s - omega * t; rho_old = rho
+        maxn.append(np.abs(r).max())
+        if maxn[-1] < tol:
+            break
+    out = oracle.bicgstab(n, n, n, A, b, tol=tol, maxit=400, precond=False, history=True, norm=oracle.NORM_ABS_INF)
+    assert out["status"] == 0
+    assert out["hist"][-1] < tol and np.all(out["hist"][:-1] >= tol)          # first iterate below ErrTol
+    assert out["relres"] == out["hist"][-1] and abs(out["true_relres"] - out["relres"]) < 1e-3 * tol
+    m = min(20, len(maxn), len(out["hist"]))
+    assert np.allclose(out["hist"][:m], maxn[:m], rtol=1e-6)                  # absolute max norms, same run
+    assert abs(out["iters"] - (len(maxn) - 1)) <= max(3, 0.1 * out["iters"])
+    # the L2-relative mode on the same system stops elsewhere: the modes are really different tests
+    out2 = oracle.bicgstab(n, n, n, A, b, tol=tol, maxit=400, precond=False)
+    assert out2["status"] == 0 and out2["relres"] <= tol
