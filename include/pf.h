@@ -79,6 +79,11 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
 #define PF_OPT_GRAPH          12  /* 1 (default): on grids of up to 2^22 unknowns, which are bound by launch latency,
                                      replay each polling chunk of iterations as one CUDA graph; 0 = plain launches */
 
+#define PF_OPT_NORM           13  /* stopping test of every linear solve.  0 (default, reading Q3): ||r||_2 <= tol ||b||_2;
+                                     1: the paper's own test, Table 3 steps 18-19: ||r||_inf < tol,
+                                     absolute.  With 1, relres_out, true_relres_out and the history are absolute
+                                     maximum norms. */
+
 /* Create a grid: store geometry and boundary conditions, scan eps_map for its palette of distinct
  * values, keep a device copy of the charges.  Assembly itself runs in pf_grid_set_workspace.
  *   eps_map : device, nx*ny*nz doubles, relative permittivity per node; borrowed.

@@ -143,6 +143,7 @@ struct pf_grid {
     std::vector<ChunkGraph> graphs;
     cudaStream_t capture_stream;
     int opt_graph;
+    int opt_norm;            // 0: relative 2-norm (Q3), 1: the paper's absolute maximum norm
     int fault_repeats;       // solves repeated by the direct kernels after a division range fault (D4)
     std::string err;
 };
@@ -264,7 +265,7 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     const bool precond = g->opt_precond != 0;
     Scalars init;
     std::memset(&init, 0, sizeof(init));
-    init.tol = tol; init.maxit = maxit; init.hist_cap = g->hist ? g->hist_cap : 0;
+    init.tol = tol; init.maxit = maxit; init.hist_cap = g->hist ? g->hist_cap : 0; init.norm_mode = g->opt_norm;
     // pageable source: the runtime stages it before returning, so a stack object is safe
     PF_CUDA(g, cudaMemcpyAsync(g->sc, &init, sizeof(init), cudaMemcpyHostToDevice, g->stream));
     KrylovVecs kv;
@@ -347,7 +348,7 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
         if (tiled) launch_residual_tma(c, op, kv, g->tma, 1); else launch_residual_direct(c, op, kv, 1);
         PF_CUDA(g, cudaMemcpyAsync(g->sc_host[0], g->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
         PF_CUDA(g, cudaStreamSynchronize(g->stream));
-        true_rel = std::sqrt(g->sc_host[0]->true_rr) / fin.bnorm;
+        true_rel = g->opt_norm == 1 ? g->sc_host[0]->true_rmax : std::sqrt(g->sc_host[0]->true_rr) / fin.bnorm;
     }
     PF_CUDA(g, cudaGetLastError());
     g->last_iters = fin.it;
@@ -438,7 +439,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->opt_profile = 0; g->prof_ms[0] = g->prof_ms[1] = g->prof_ms[2] = 0.0;
     g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
-    g->capture_stream = nullptr; g->opt_graph = 1;
+    g->capture_stream = nullptr; g->opt_graph = 1; g->opt_norm = 0;
     g->small = nullptr;
     g->charges_dev = nullptr; g->sc = nullptr; g->rb.partial = nullptr; g->rb.ticket = nullptr;
     g->ctab_poisson = g->ctab_pf1 = nullptr; g->dmax_bits = nullptr; g->tma = nullptr;
@@ -561,6 +562,9 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
             for (int j = 0; j < 3; ++j) { g->prof_ms[j] = 0.0; g->prof_launches[j] = 0; }
             return PF_OK;
         }
+        case PF_OPT_NORM:
+            if (iv != 0 && iv != 1) return fail(g, PF_ERR_ARG, "norm must be 0 or 1");
+            g->opt_norm = iv; return PF_OK;
         case PF_OPT_GRAPH:
             g->opt_graph = iv != 0; return PF_OK;
         case PF_OPT_KERNELS:

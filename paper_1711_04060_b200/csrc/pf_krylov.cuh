@@ -37,10 +37,16 @@ __device__ __forceinline__ double jacobi(double u, double a0) { return PRECOND ?
 // ---- reduction-point epilogues (thread 0 of the last block only) ------------------------------
 
 // After r0 = b - A x0 (step 2): ||b||, ||r0||, rho_0 = r~.r0 = r0.r0, early exits.
-__device__ __forceinline__ void finish_init(Scalars* sc, double* hist, double bb, double rr) {
-    sc->bb = bb; sc->rr = rr;
-    sc->bnorm = __dsqrt_rn(bb);
-    sc->rnorm = __dsqrt_rn(rr);
+// norm_mode 1 (Table 3 steps 18-19 as written): the measure is ||r||_inf, absolute, the test
+// strict; rnorm then holds the maximum norm and bnorm the scale 1.
+__device__ __forceinline__ bool converged(const Scalars* sc) {
+    return sc->norm_mode == 1 ? sc->rnorm < sc->tol : sc->rnorm <= mul(sc->tol, sc->bnorm);
+}
+
+__device__ __forceinline__ void finish_init(Scalars* sc, double* hist, double bb, double rr, double rmax) {
+    sc->bb = bb; sc->rr = rr; sc->rmax = rmax;
+    sc->bnorm = sc->norm_mode == 1 ? 1.0 : __dsqrt_rn(bb);
+    sc->rnorm = sc->norm_mode == 1 ? rmax : __dsqrt_rn(rr);
     sc->it = 0; sc->first = 1; sc->done = 0; sc->status = 1;
     sc->rho = rr; sc->rho_old = 1.0; sc->alpha = 1.0; sc->omega = 1.0; sc->beta = 0.0;
     if (bb == 0.0) {                       // Q3: b = 0 => x = 0, no iterations (host zeroes x)
@@ -49,7 +55,7 @@ __device__ __forceinline__ void finish_init(Scalars* sc, double* hist, double bb
         return;
     }
     if (hist && sc->hist_cap > 0) hist[0] = dvd(sc->rnorm, sc->bnorm);
-    if (sc->rnorm <= mul(sc->tol, sc->bnorm)) { sc->done = 1; sc->status = 0; return; }
+    if (converged(sc)) { sc->done = 1; sc->status = 0; return; }
     if (sc->maxit <= 0) { sc->done = 1; sc->status = 1; return; }
     if (rr == 0.0) { sc->done = 1; sc->status = -3; }
 }
@@ -69,15 +75,15 @@ __device__ __forceinline__ void finish_k2(Scalars* sc, double ts, double tt) {
 
 // After the x and r updates (steps 16-17): ||r|| test (steps 18-20), then rho and beta of the next
 // iteration (steps 4, 8).
-__device__ __forceinline__ void finish_k3(Scalars* sc, double* hist, double rho_new, double rr) {
-    sc->rr = rr;
-    sc->rnorm = __dsqrt_rn(rr);
+__device__ __forceinline__ void finish_k3(Scalars* sc, double* hist, double rho_new, double rr, double rmax) {
+    sc->rr = rr; sc->rmax = rmax;
+    sc->rnorm = sc->norm_mode == 1 ? rmax : __dsqrt_rn(rr);
     const int it = sc->it + 1;
     sc->it = it;
     if (hist && it < sc->hist_cap) hist[it] = dvd(sc->rnorm, sc->bnorm);
     const double rho_old = sc->rho;
     sc->rho_old = rho_old;
-    if (sc->rnorm <= mul(sc->tol, sc->bnorm)) { sc->done = 1; sc->status = 0; return; }
+    if (converged(sc)) { sc->done = 1; sc->status = 0; return; }
     if (sc->omega == 0.0) { sc->done = 1; sc->status = -3; return; }
     if (it >= sc->maxit) { sc->done = 1; sc->status = 1; return; }
     sc->rho = rho_new;

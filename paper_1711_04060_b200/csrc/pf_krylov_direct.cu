@@ -65,9 +65,10 @@ template <int MODE>
 __global__ void __launch_bounds__(DIRECT_THREADS)
 k_residual(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
     __shared__ double ctab_s[PF_CTAB];
-    __shared__ dd scratch[2 * 32];
+    __shared__ dd scratch[3 * 32];
     load_ctab(op, ctab_s);
     dd q[2] = {dd_zero(), dd_zero()};
+    double rmax = 0.0;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
         Nbr n = neighbours(g, i);
@@ -85,10 +86,11 @@ k_residual(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
             dd_fma(q[0], bi, bi);
         }
         dd_fma(q[1], ri, ri);
+        rmax = fmax(rmax, fabs(ri));
     }
-    if (grid_reduce_dd<2>(q, scratch, rb)) {
-        if (MODE == 0) finish_init(sc, kv.hist, dd_round(q[0]), dd_round(q[1]));
-        else sc->true_rr = dd_round(q[1]);
+    if (grid_reduce_dd_max<2>(q, rmax, scratch, rb)) {
+        if (MODE == 0) finish_init(sc, kv.hist, dd_round(q[0]), dd_round(q[1]), rmax);
+        else { sc->true_rr = dd_round(q[1]); sc->true_rmax = rmax; }
     }
 }
 
@@ -164,12 +166,13 @@ k2_direct(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
 struct K3Elem { double r, v, p, y, t, rt; };
 
 __device__ __forceinline__ void k3_point(const K3Elem& e, double alpha, double omega, double& y_new, double& r_new,
-                                         dd& q0, dd& q1) {
+                                         dd& q0, dd& q1, double& rmax) {
     const double s = s_at(alpha, e.r, e.v);
     y_new = add(add(e.y, mul(alpha, e.p)), mul(omega, s));       // step 16
     r_new = sub(s, mul(omega, e.t));                              // step 17
     dd_fma(q0, e.rt, r_new);
     dd_fma(q1, r_new, r_new);
+    rmax = fmax(rmax, fabs(r_new));          // ||r||_inf of Table 3 step 18
 }
 
 template <bool VEC>
@@ -178,9 +181,10 @@ k3_update(long long n, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
     pdl_launch_dependents();
     pdl_wait();
     if (sc->done) return;
-    __shared__ dd scratch[2 * 32];
+    __shared__ dd scratch[3 * 32];
     const double alpha = sc->alpha, omega = sc->omega;
     dd qa[2] = {dd_zero(), dd_zero()}, qb[2] = {dd_zero(), dd_zero()};
+    double rmax = 0.0;
     const long long stride = (long long)gridDim.x * blockDim.x;
     const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (VEC) {
@@ -199,36 +203,36 @@ k3_update(long long n, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
             const double2 ra = r2[i], va = v2[i], pa = p2[i], ya = y2[i], ta = t2[i], wa = rt2[i];
             const double2 rb2 = r2[j], vb = v2[j], pb = p2[j], yb = y2[j], tb = t2[j], wb = rt2[j];
             double2 yn, rn;
-            k3_point({ra.x, va.x, pa.x, ya.x, ta.x, wa.x}, alpha, omega, yn.x, rn.x, qa[0], qa[1]);
-            k3_point({ra.y, va.y, pa.y, ya.y, ta.y, wa.y}, alpha, omega, yn.y, rn.y, qb[0], qb[1]);
+            k3_point({ra.x, va.x, pa.x, ya.x, ta.x, wa.x}, alpha, omega, yn.x, rn.x, qa[0], qa[1], rmax);
+            k3_point({ra.y, va.y, pa.y, ya.y, ta.y, wa.y}, alpha, omega, yn.y, rn.y, qb[0], qb[1], rmax);
             yo[i] = yn; ro[i] = rn;
-            k3_point({rb2.x, vb.x, pb.x, yb.x, tb.x, wb.x}, alpha, omega, yn.x, rn.x, qa[0], qa[1]);
-            k3_point({rb2.y, vb.y, pb.y, yb.y, tb.y, wb.y}, alpha, omega, yn.y, rn.y, qb[0], qb[1]);
+            k3_point({rb2.x, vb.x, pb.x, yb.x, tb.x, wb.x}, alpha, omega, yn.x, rn.x, qa[0], qa[1], rmax);
+            k3_point({rb2.y, vb.y, pb.y, yb.y, tb.y, wb.y}, alpha, omega, yn.y, rn.y, qb[0], qb[1], rmax);
             yo[j] = yn; ro[j] = rn;
         }
         for (; i < n2; i += stride) {
             const double2 ra = r2[i], va = v2[i], pa = p2[i], ya = y2[i], ta = t2[i], wa = rt2[i];
             double2 yn, rn;
-            k3_point({ra.x, va.x, pa.x, ya.x, ta.x, wa.x}, alpha, omega, yn.x, rn.x, qa[0], qa[1]);
-            k3_point({ra.y, va.y, pa.y, ya.y, ta.y, wa.y}, alpha, omega, yn.y, rn.y, qb[0], qb[1]);
+            k3_point({ra.x, va.x, pa.x, ya.x, ta.x, wa.x}, alpha, omega, yn.x, rn.x, qa[0], qa[1], rmax);
+            k3_point({ra.y, va.y, pa.y, ya.y, ta.y, wa.y}, alpha, omega, yn.y, rn.y, qb[0], qb[1], rmax);
             yo[i] = yn; ro[i] = rn;
         }
         if ((n & 1) && tid == 0) {                    // odd tail
             const long long k = n - 1;
             double yn, rn;
-            k3_point({kv.r[k], kv.v_out[k], kv.p_out[k], kv.y[k], kv.t[k], kv.rt[k]}, alpha, omega, yn, rn, qa[0], qa[1]);
+            k3_point({kv.r[k], kv.v_out[k], kv.p_out[k], kv.y[k], kv.t[k], kv.rt[k]}, alpha, omega, yn, rn, qa[0], qa[1], rmax);
             kv.y[k] = yn; kv.r[k] = rn;
         }
     } else {
         for (long long i = tid; i < n; i += stride) {
             double yn, rn;
-            k3_point({kv.r[i], kv.v_out[i], kv.p_out[i], kv.y[i], kv.t[i], kv.rt[i]}, alpha, omega, yn, rn, qa[0], qa[1]);
+            k3_point({kv.r[i], kv.v_out[i], kv.p_out[i], kv.y[i], kv.t[i], kv.rt[i]}, alpha, omega, yn, rn, qa[0], qa[1], rmax);
             kv.y[i] = yn; kv.r[i] = rn;
         }
     }
     dd_add(qa[0], qb[0]);
     dd_add(qa[1], qb[1]);
-    if (grid_reduce_dd<2>(qa, scratch, rb)) finish_k3(sc, kv.hist, dd_round(qa[0]), dd_round(qa[1]));
+    if (grid_reduce_dd_max<2>(qa, rmax, scratch, rb)) finish_k3(sc, kv.hist, dd_round(qa[0]), dd_round(qa[1]), rmax);
 }
 
 // x = x + M^-1 y (reading D3).  y is exactly 0 on identity rows, so Dirichlet values of x are kept.

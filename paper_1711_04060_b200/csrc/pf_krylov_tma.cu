@@ -77,7 +77,7 @@ struct Layout {
     static constexpr int U_OFF = T::STAGES * STAGE_BYTES;
     static constexpr int CTAB_OFF = U_OFF + NU * FIELD_BYTES;
     static constexpr int SCRATCH_OFF = CTAB_OFF + PF_CTAB * 8;
-    static constexpr int BAR_OFF = SCRATCH_OFF + 2 * 32 * (int)sizeof(dd);
+    static constexpr int BAR_OFF = SCRATCH_OFF + 3 * 32 * (int)sizeof(dd);
     static constexpr int TOTAL = BAR_OFF + 16 * T::STAGES + 8 * NU;  // full[S], empty[S], ready[NU]
     static_assert(CTAB_OFF % 128 == 0, "ctab_at ORs table offsets into the table address");
     static constexpr unsigned TX_BYTES = (unsigned)(T::NF * BX * BY * 8 + (T::OWN ? OWN_BYTES : 0) + CODE_BYTES);
@@ -186,6 +186,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     if (MODE >= MODE_K1 && sc->done) return;
 
     dd q[2] = {dd_zero(), dd_zero()};
+    double rmax = 0.0;                     // residual modes: ||b - A x||_inf
     unsigned fault = 0u;
 
     if (wid == NW_CONSUMER) {
@@ -385,6 +386,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                         dd_fma(q[0], c.w.x, c.w.x); dd_fma(q[0], c.w.y, c.w.y);
                     }
                     dd_fma(q[1], r0, r0); dd_fma(q[1], r1, r1);
+                    rmax = fmax(rmax, fmax(fabs(r0), fabs(r1)));
                 }
             };
 
@@ -408,10 +410,11 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
         dd_add(q[0], q[1]);                // two chains for instruction-level parallelism, one quantity
         dd q1[1] = {q[0]};
         if (grid_reduce_dd<1>(q1, scratch, rb)) finish_k1(sc, dd_round(q1[0]));
-    } else if (grid_reduce_dd<2>(q, scratch, rb)) {
-        if (MODE == MODE_K2) finish_k2(sc, dd_round(q[0]), dd_round(q[1]));
-        else if (MODE == MODE_R0) finish_init(sc, kv.hist, dd_round(q[0]), dd_round(q[1]));
-        else sc->true_rr = dd_round(q[1]);
+    } else if (MODE == MODE_K2) {
+        if (grid_reduce_dd<2>(q, scratch, rb)) finish_k2(sc, dd_round(q[0]), dd_round(q[1]));
+    } else if (grid_reduce_dd_max<2>(q, rmax, scratch, rb)) {
+        if (MODE == MODE_R0) finish_init(sc, kv.hist, dd_round(q[0]), dd_round(q[1]), rmax);
+        else { sc->true_rr = dd_round(q[1]); sc->true_rmax = rmax; }
     }
 }
 
