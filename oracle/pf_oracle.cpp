@@ -31,6 +31,9 @@
 //   outer loop    : l_c=0 + steric off => nonlinear PB (Gouy-Chapman closed form in 1-D);
 //                   independence of omega_PF; fixed-point residuals of PF1/PF2 at convergence
 //   full PF, l_c>0, unequal radii, 3-D: PARITY UNPINNED beyond the reductions above.
+//   singular charges (Eqs 5-10): Coulomb sums vs numpy; 1-D closed form with a prescribed flux jump (c0, d0 of
+//                   Eqs 17-18); discrete Gauss law sum b^IF h^3 = kappa sum q; harmonic phi^L; Born ion;
+//                   agreement with the independent deposition model in the solvent (tests/test_oracle_singular.py)
 
 #include <cmath>
 #include <cstdint>
@@ -420,6 +423,143 @@ void rhs_pf2(const Grid& g, const double* eps, const uint8_t* solvent, const dou
 }  // namespace
 
 // =========================================================================================
+// Singular-charge decomposition, Eqs (5)-(10) and the flux-jump terms of Eqs (17)-(18)
+// (readings S1-S5 of DESIGN.md).
+//   phi = phi~ + phi* + phi^L in Omega_m (the non-solvent nodes),  phi = phi~ in Omega_s.
+//   phi*(r) = kappa/(4 pi eps_m) sum_j q_j/|r - r_j|                              (Eq 5, units R0)
+//   Laplace phi^L = 0 in Omega_m,  phi^L = -phi* on the boundary of Omega_m        (Eqs 9-10, S1)
+//   [eps grad phi~ . n] = eps_m grad(phi* + phi^L) . n on the interface            (Eq 8)
+// Discretisation (S2): the interface cuts every face between an Omega_m node i and an Omega_s
+// node j at its midpoint x_f (Q16).  Laplace rows at interior Omega_m nodes: (u_i - u_nb)/h^2 per
+// face towards an Omega_m neighbour, 2 (u_i - g_f)/h^2 per interface face (ghost value 2 g_f - u_i,
+// g_f = -phi*(x_f)); Omega_m nodes on the box boundary carry u = -phi* (S3: Eq (10) on ALL of the
+// boundary of Omega_m); Omega_s nodes are identity rows with u = 0.
+// Flux jump on an interface face, n from i (Omega_m) to j (Omega_s):
+//   J_f = eps_i [ dphi*/dn (x_f) + 2 (g_f - u_i)/h ]                                (Eq 8)
+// enters the two rows next to the face exactly as c0, d0 of Eqs (17)-(18):
+//   b_i += -eps_i J_f/((eps_i + eps_j) h),   b_j += -eps_j J_f/((eps_i + eps_j) h).
+// =========================================================================================
+namespace {
+
+const double FOUR_PI = 4.0 * M_PI;
+
+// phi* at the point (x, y, z) [Angstrom]; charges summed in list order.
+double coulomb_potential(const double* ch, int M, double eps_m, double x, double y, double z) {
+    double s = 0.0;
+    for (int j = 0; j < M; ++j) {
+        double dx = x - ch[4 * j], dy = y - ch[4 * j + 1], dz = z - ch[4 * j + 2];
+        double r = std::sqrt(dx * dx + dy * dy + dz * dz);
+        s = s + ch[4 * j + 3] / r;
+    }
+    return (kappa_angstrom() / (FOUR_PI * eps_m)) * s;
+}
+
+// d phi*/d x_axis at the point: -kappa/(4 pi eps_m) sum q (x_axis - r_j,axis)/r^3.
+double coulomb_gradient(const double* ch, int M, double eps_m, double x, double y, double z, int axis) {
+    double s = 0.0;
+    for (int j = 0; j < M; ++j) {
+        double dx = x - ch[4 * j], dy = y - ch[4 * j + 1], dz = z - ch[4 * j + 2];
+        double r2 = dx * dx + dy * dy + dz * dz;
+        double r = std::sqrt(r2);
+        double comp = axis == 0 ? dx : (axis == 1 ? dy : dz);
+        s = s + ch[4 * j + 3] * comp / (r2 * r);
+    }
+    return -((kappa_angstrom() / (FOUR_PI * eps_m)) * s);
+}
+
+// Face d (1..6, PAPER.md:219 order) of node (ix,iy,iz): neighbour offset, axis and outward sign.
+const int FACE_DX[7] = {0, 1, -1, 0, 0, 0, 0};
+const int FACE_DY[7] = {0, 0, 0, -1, 1, 0, 0};
+const int FACE_DZ[7] = {0, 0, 0, 0, 0, -1, 1};
+const int FACE_AXIS[7] = {0, 0, 0, 1, 1, 2, 2};
+const int FACE_SIGN[7] = {0, 1, -1, -1, 1, -1, 1};
+
+// Laplace system for phi^L in Omega_m (S2, S3): matrix in the diagonal format, right-hand side, and the
+// vector of prescribed values (identity rows: Omega_s nodes 0, boundary Omega_m nodes -phi*).
+void assemble_laplace_m(const Grid& g, const uint8_t* solvent, const double* ch, int M, double eps_m,
+                        double* A, double* b) {
+    const int64_t N = g.n();
+    const int64_t off[7] = {0, 1, -1, -(int64_t)g.nx, (int64_t)g.nx, -(int64_t)g.nx * g.ny, (int64_t)g.nx * g.ny};
+    const double c = 1.0 / (g.h * g.h);
+    for (int iz = 0; iz < g.nz; ++iz)
+        for (int iy = 0; iy < g.ny; ++iy)
+            for (int ix = 0; ix < g.nx; ++ix) {
+                int64_t i = ix + (int64_t)g.nx * (iy + (int64_t)g.ny * iz);
+                for (int d = 1; d < 7; ++d) A[d * N + i] = 0.0;
+                if (solvent[i]) { A[i] = 1.0; b[i] = 0.0; continue; }
+                if (on_box_boundary(g, ix, iy, iz)) {
+                    A[i] = 1.0;
+                    b[i] = -coulomb_potential(ch, M, eps_m, ix * g.h, iy * g.h, iz * g.h);
+                    continue;
+                }
+                double diag = 0.0, rhs = 0.0;
+                for (int d = 1; d < 7; ++d) {
+                    int64_t j = i + off[d];
+                    if (!solvent[j]) { A[d * N + i] = -c; diag = diag + c; continue; }
+                    double xf = (ix + 0.5 * FACE_DX[d]) * g.h, yf = (iy + 0.5 * FACE_DY[d]) * g.h,
+                           zf = (iz + 0.5 * FACE_DZ[d]) * g.h;
+                    double gf = -coulomb_potential(ch, M, eps_m, xf, yf, zf);
+                    diag = diag + 2.0 * c;
+                    rhs = rhs + (2.0 * c) * gf;
+                }
+                A[i] = diag;
+                b[i] = rhs;
+            }
+}
+
+// Flux jumps J_f on the interface faces, stored at the Omega_m node: J[(d-1)*N + i] for face d of node i
+// (0 where face d of i is not an interface face).  Box-boundary Omega_m nodes have no rows of their own in
+// the Poisson system beyond what the boundary condition gives, but their interface faces still separate two
+// materials and carry a jump like any other.
+void face_jumps(const Grid& g, const double* eps, const uint8_t* solvent, const double* ch, int M, double eps_m,
+                const double* phiL, double* J) {
+    const int64_t N = g.n();
+    const int64_t off[7] = {0, 1, -1, -(int64_t)g.nx, (int64_t)g.nx, -(int64_t)g.nx * g.ny, (int64_t)g.nx * g.ny};
+    std::fill(J, J + 6 * N, 0.0);
+    for (int iz = 0; iz < g.nz; ++iz)
+        for (int iy = 0; iy < g.ny; ++iy)
+            for (int ix = 0; ix < g.nx; ++ix) {
+                int64_t i = ix + (int64_t)g.nx * (iy + (int64_t)g.ny * iz);
+                if (solvent[i]) continue;
+                bool inside[7] = {true, ix + 1 < g.nx, ix - 1 >= 0, iy - 1 >= 0, iy + 1 < g.ny, iz - 1 >= 0, iz + 1 < g.nz};
+                for (int d = 1; d < 7; ++d) {
+                    if (!inside[d] || !solvent[i + off[d]]) continue;
+                    double xf = (ix + 0.5 * FACE_DX[d]) * g.h, yf = (iy + 0.5 * FACE_DY[d]) * g.h,
+                           zf = (iz + 0.5 * FACE_DZ[d]) * g.h;
+                    double gf = -coulomb_potential(ch, M, eps_m, xf, yf, zf);
+                    double dn_star = FACE_SIGN[d] * coulomb_gradient(ch, M, eps_m, xf, yf, zf, FACE_AXIS[d]);
+                    double dn_L = 2.0 * (gf - phiL[i]) / g.h;
+                    J[(d - 1) * N + i] = eps[i] * (dn_star + dn_L);
+                }
+            }
+}
+
+// b^IF from the jumps: every node gathers the faces it shares with a node of the other kind, d = 1..6.
+void interface_rhs(const Grid& g, const double* eps, const uint8_t* solvent, const double* J, double* b) {
+    const int64_t N = g.n();
+    const int64_t off[7] = {0, 1, -1, -(int64_t)g.nx, (int64_t)g.nx, -(int64_t)g.nx * g.ny, (int64_t)g.nx * g.ny};
+    const int opposite[7] = {0, 2, 1, 4, 3, 6, 5};
+    for (int iz = 0; iz < g.nz; ++iz)
+        for (int iy = 0; iy < g.ny; ++iy)
+            for (int ix = 0; ix < g.nx; ++ix) {
+                int64_t i = ix + (int64_t)g.nx * (iy + (int64_t)g.ny * iz);
+                bool inside[7] = {true, ix + 1 < g.nx, ix - 1 >= 0, iy - 1 >= 0, iy + 1 < g.ny, iz - 1 >= 0, iz + 1 < g.nz};
+                double acc = 0.0;
+                for (int d = 1; d < 7; ++d) {
+                    if (!inside[d]) continue;
+                    int64_t j = i + off[d];
+                    if (solvent[i] == solvent[j]) continue;
+                    // the jump is stored at the Omega_m node of the pair
+                    double Jf = solvent[i] ? J[(opposite[d] - 1) * N + j] : J[(d - 1) * N + i];
+                    acc = acc + (-(eps[i] * Jf) / ((eps[i] + eps[j]) * g.h));
+                }
+                b[i] = acc;
+            }
+}
+
+}  // namespace
+
+// =========================================================================================
 // C interface (ctypes).  All pointers are host pointers.
 // =========================================================================================
 extern "C" {
@@ -508,7 +648,7 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
                  double* phi /* out */, double* psi /* out or null */, double* conc /* out or null */,
                  double* steric /* out or null */,
                  int* outer_iters, int* linear_iters, int* lin_iters_hist, int hist_cap,
-                 double* incr_hist) {
+                 double* incr_hist, const double* fixed_override /* b^IF of the singular-charge model, or null */) {
     Grid g = mk(nx, ny, nz, h, bct, bcv);
     const int64_t N = g.n();
     SpeciesTab sp;
@@ -518,7 +658,8 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
     solvent_mask(N, eps, solv.data());
     std::vector<double> fixed(N, 0.0), A0(7 * N), A1(7 * N), A2(7 * N), b(N);
     std::vector<double> phi0(N, 0.0), Psi(N, 0.0), ph(N), rho(N), sigma(N), S(N);
-    deposit_charges(g, charges, M, fixed.data());
+    if (fixed_override) std::memcpy(fixed.data(), fixed_override, N * sizeof(double));
+    else deposit_charges(g, charges, M, fixed.data());
     int nsolve = 0, total = 0, its = 0;
     double rr, tr;
     auto record = [&](int n) { if (lin_iters_hist && nsolve < hist_cap) lin_iters_hist[nsolve] = n; ++nsolve; total += n; };
@@ -594,6 +735,56 @@ int pfo_pf_residuals(int nx, int ny, int nz, double h, const int* bct, const dou
     bn = norm2(N, b.data());
     *res_pf2 = bn > 0 ? norm2(N, y.data()) / bn : norm2(N, y.data());
     return 0;
+}
+
+// ---- singular-charge decomposition (see the block comment above assemble_laplace_m) -----------------
+double pfo_coulomb_potential(const double* charges, int M, double eps_m, double x, double y, double z) {
+    return coulomb_potential(charges, M, eps_m, x, y, z);
+}
+
+double pfo_coulomb_gradient(const double* charges, int M, double eps_m, double x, double y, double z, int axis) {
+    return coulomb_gradient(charges, M, eps_m, x, y, z, axis);
+}
+
+void pfo_interface_rhs(int nx, int ny, int nz, double h, const double* eps, const uint8_t* solvent,
+                       const double* J, double* b) {
+    int t[6] = {0, 0, 0, 0, 0, 0}; double v[6] = {0, 0, 0, 0, 0, 0};
+    interface_rhs(mk(nx, ny, nz, h, t, v), eps, solvent, J, b);
+}
+
+// Everything that precedes the PF loop in Table 2 step 1 / Table 4 steps 2-3:
+// phi* on the Omega_m nodes, the Laplace solve for phi^L, the flux jumps and b^IF.
+// eps_m = the smallest eps of the map (S4).  Returns the status of the Laplace solve.
+int pfo_singular_setup(int nx, int ny, int nz, double h, const double* eps, const double* charges, int M,
+                       double lin_tol, int lin_maxit,
+                       double* phiL /* N */, double* phistar /* N, 0 on Omega_s */, double* bIF /* N */,
+                       double* Jout /* 6N or null */, int* laplace_iters) {
+    int t[6] = {0, 0, 0, 0, 0, 0}; double v[6] = {0, 0, 0, 0, 0, 0};
+    Grid g = mk(nx, ny, nz, h, t, v);
+    const int64_t N = g.n();
+    std::vector<uint8_t> solv(N);
+    solvent_mask(N, eps, solv.data());
+    double eps_m = eps[0];
+    for (int64_t i = 1; i < N; ++i) eps_m = std::min(eps_m, eps[i]);
+    std::vector<double> A(7 * N), b(N), J(6 * N);
+    assemble_laplace_m(g, solv.data(), charges, M, eps_m, A.data(), b.data());
+    // initial guess: the prescribed values on identity rows, 0 elsewhere (the Krylov vectors then vanish there)
+    for (int64_t i = 0; i < N; ++i) phiL[i] = (A[i] == 1.0 && A[1 * N + i] == 0.0 && A[2 * N + i] == 0.0 &&
+                                               A[3 * N + i] == 0.0 && A[4 * N + i] == 0.0 && A[5 * N + i] == 0.0 &&
+                                               A[6 * N + i] == 0.0) ? b[i] : 0.0;
+    double rr, tr;
+    int rc = bicgstab(g, A.data(), b.data(), phiL, lin_tol, lin_maxit, 1, laplace_iters, &rr, &tr, nullptr);
+    if (rc < 0) return rc;
+    for (int iz = 0; iz < nz; ++iz)
+        for (int iy = 0; iy < ny; ++iy)
+            for (int ix = 0; ix < nx; ++ix) {
+                int64_t i = ix + (int64_t)nx * (iy + (int64_t)ny * iz);
+                phistar[i] = solv[i] ? 0.0 : coulomb_potential(charges, M, eps_m, ix * h, iy * h, iz * h);
+            }
+    face_jumps(g, eps, solv.data(), charges, M, eps_m, phiL, J.data());
+    interface_rhs(g, eps, solv.data(), J.data(), bIF);
+    if (Jout) std::memcpy(Jout, J.data(), 6 * N * sizeof(double));
+    return rc;
 }
 
 // ---- dense LU with partial pivoting (pin for the 8^3 case; no LAPACK) --------------------

@@ -40,6 +40,8 @@ def lib():
         _lib.pfo_kT_over_e_volt.restype = ctypes.c_double
         _lib.pfo_molar_to_per_A3.restype = ctypes.c_double
         _lib.pfo_dot.restype = ctypes.c_double
+        _lib.pfo_coulomb_potential.restype = ctypes.c_double
+        _lib.pfo_coulomb_gradient.restype = ctypes.c_double
     return _lib
 
 
@@ -197,7 +199,8 @@ def fermi_pointwise(valence, bath_molar, radii, phi, solvent=None, water_molar=5
 
 
 def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar, radii, l_c, tol,
-             omega_pf=0.3, lin_tol=1e-10, lin_maxit=10000, max_outer=200, water_molar=55.5, norm=NORM_REL_L2):
+             omega_pf=0.3, lin_tol=1e-10, lin_maxit=10000, max_outer=200, water_molar=55.5, norm=NORM_REL_L2,
+             fixed_override=None):
     """The outer loop of Table 2 / Table 4 (R5)."""
     n = nx * ny * nz
     t, v = _bc(bc_type, bc_value)
@@ -221,7 +224,7 @@ def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar
                             ctypes.c_double(l_c), ctypes.c_double(tol), ctypes.c_double(omega_pf),
                             ctypes.c_double(lin_tol), int(lin_maxit), int(max_outer), int(norm),
                             _d(phi), _d(psi), _d(conc), _d(steric), ctypes.byref(outer), ctypes.byref(lin),
-                            _i(lhist), int(cap), _d(ihist))
+                            _i(lhist), int(cap), _d(ihist), _d(None if fixed_override is None else _f64(fixed_override)))
     return dict(phi=phi, psi=psi, conc=conc, steric=steric, status=st, outer_iters=outer.value,
                 linear_iters=lin.value, lin_iters_hist=lhist[: 2 * outer.value + 1].copy(),
                 incr_hist=ihist[: outer.value].copy())
@@ -243,6 +246,42 @@ def pf_residuals(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_m
                                 int(valence.size), _d(valence), _d(bath), _d(radii), ctypes.c_double(water_molar),
                                 ctypes.c_double(l_c), _d(phi), _d(psi), ctypes.byref(r1), ctypes.byref(r2))
     return dict(status=st, res_pf1=r1.value, res_pf2=r2.value)
+
+
+def coulomb_potential(charges, eps_m, x, y, z) -> float:
+    ch = _f64(charges).reshape(-1, 4)
+    return lib().pfo_coulomb_potential(_d(ch), int(ch.shape[0]), ctypes.c_double(eps_m), ctypes.c_double(x),
+                                       ctypes.c_double(y), ctypes.c_double(z))
+
+
+def coulomb_gradient(charges, eps_m, x, y, z, axis) -> float:
+    ch = _f64(charges).reshape(-1, 4)
+    return lib().pfo_coulomb_gradient(_d(ch), int(ch.shape[0]), ctypes.c_double(eps_m), ctypes.c_double(x),
+                                      ctypes.c_double(y), ctypes.c_double(z), int(axis))
+
+
+def interface_rhs(nx, ny, nz, h, eps, solvent, J) -> np.ndarray:
+    """b^IF from the flux jumps J (6 x N, stored at the Omega_m node of each interface face)."""
+    b = np.zeros(nx * ny * nz)
+    lib().pfo_interface_rhs(nx, ny, nz, ctypes.c_double(h), _d(_f64(eps)),
+                            _u8(np.ascontiguousarray(solvent, dtype=np.uint8)), _d(_f64(J).reshape(-1)), _d(b))
+    return b
+
+
+def singular_setup(nx, ny, nz, h, eps, charges, lin_tol=1e-10, lin_maxit=10000, want_jumps=False):
+    """phi^L, phi* (on Omega_m), b^IF of the singular-charge decomposition (Eqs 5-10)."""
+    n = nx * ny * nz
+    ch = _f64(charges).reshape(-1, 4)
+    phiL, phistar, bIF = np.zeros(n), np.zeros(n), np.zeros(n)
+    J = np.zeros(6 * n) if want_jumps else None
+    it = ctypes.c_int(0)
+    st = lib().pfo_singular_setup(nx, ny, nz, ctypes.c_double(h), _d(_f64(eps)), _d(ch), int(ch.shape[0]),
+                                  ctypes.c_double(lin_tol), int(lin_maxit), _d(phiL), _d(phistar), _d(bIF), _d(J),
+                                  ctypes.byref(it))
+    out = dict(status=st, phiL=phiL, phistar=phistar, bIF=bIF, laplace_iters=it.value)
+    if want_jumps:
+        out["J"] = J.reshape(6, n)
+    return out
 
 
 def dia_to_dense(nx, ny, nz, A) -> np.ndarray:
