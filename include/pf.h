@@ -84,6 +84,15 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
                                      absolute.  With 1, relres_out, true_relres_out and the history are absolute
                                      maximum norms. */
 
+#define PF_OPT_CHARGE_MODEL   14  /* how the fixed point charges enter.  0 (default, reading Q22): trilinear deposition on
+                                     the 8 surrounding nodes.  1: the singular-charge decomposition of Eqs (5)-(10)
+                                     (PAPER.md:85-111): phi = phi~ + phi* + phi^L in Omega_m (the low-eps nodes, Q17),
+                                     phi* the Coulomb sum with eps_m = min eps, phi^L from a Laplace solve in Omega_m run
+                                     inside pf_grid_set_workspace (Table 2 step 1), the charges entering the equations
+                                     for phi~ only through the interface vector b^IF (flux-jump terms of Eqs (17)-(18)).
+                                     pf_solve_pf then returns the total phi.  Needs 3 more workspace vectors; must be
+                                     set before pf_grid_set_workspace; all charges are assumed to lie in Omega_m. */
+
 /* Create a grid: store geometry and boundary conditions, scan eps_map for its palette of distinct
  * values, keep a device copy of the charges.  Assembly itself runs in pf_grid_set_workspace.
  *   eps_map : device, nx*ny*nz doubles, relative permittivity per node; borrowed.
@@ -164,6 +173,9 @@ int pf_grid_profile(pf_grid *g, double *ms_out, long long *launches_out);
 /* Kernel launches issued by the library in this process so far. */
 long long pf_launch_count(void);
 
+/* BiCGSTAB iterations of the Laplace solve for phi^L (charge model 1). */
+int pf_grid_laplace_iters(const pf_grid *g);
+
 /* Number of linear solves of this grid that were repeated by the direct kernels because the tiled kernels met
  * operands outside the range of their branch-free division (reading D4 of DESIGN.md). */
 int pf_grid_fault_repeats(const pf_grid *g);
@@ -183,7 +195,8 @@ int pf_grid_code_layout(const pf_grid *g, int *bits_out, int *pitch_out, size_t 
  * which = 0: Poisson diagonal A0 (N doubles); 1..6: stored off-diagonals A1..A6 (stored variant
  * only); 7: deposited fixed-charge vector (N doubles); 8: Poisson stencil codes (pf_grid_code_layout
  * bytes); 9: PF1 diagonal (N doubles, after a pf_solve_pf); 10: Poisson coefficient table (16 doubles);
- * 11: PF1 stencil codes; 12: PF1 coefficient table; 13: Psi of the last pf_solve_pf (N doubles).
+ * 11: PF1 stencil codes; 12: PF1 coefficient table; 13: Psi of the last pf_solve_pf (N doubles);
+ * 14: phi^L, 15: phi* on Omega_m (N doubles each, charge model 1; with it, 7 is b^IF).
  * Returns PF_ERR_ARG if unavailable. */
 int pf_grid_copy_array(pf_grid *g, int which, void *dst_device);
 

@@ -144,6 +144,12 @@ struct pf_grid {
     cudaStream_t capture_stream;
     int opt_graph;
     int opt_norm;            // 0: relative 2-norm (Q3), 1: the paper's absolute maximum norm
+    int opt_charge_model;    // 0: trilinear deposition (Q22), 1: singular-charge decomposition (Eqs 5-10)
+    int charge_model;        // the model the workspace was laid out and assembled for
+    double *phiL, *phistar, *A0_L;
+    void* code_L;
+    double* ctab_L;
+    int laplace_iters;
     int fault_repeats;       // solves repeated by the direct kernels after a division range fault (D4)
     std::string err;
 };
@@ -166,7 +172,7 @@ int fail(pf_grid* g, int code, const char* fmt, ...) {
         if (e_ != cudaSuccess) return fail((g), PF_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
     } while (0)
 
-int n_vectors(bool stored) { return 19 + (stored ? 12 : 0); }
+int n_vectors(bool stored, int charge_model) { return 19 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0); }
 
 int code_mode_of(const pf_grid* g) { return g->pal.count > PF_MAX_PALETTE ? 0 : (g->pal.count <= 2 ? 1 : 2); }
 int cpitch_of(const pf_grid* g) { return (g->g.nx + 7) & ~7; }
@@ -186,13 +192,16 @@ bool use_tiled(const pf_grid* g) {
     return tma_supported(g->g) && tma_available();
 }
 
-Operator make_op(const pf_grid* g, int which /*0 poisson, 1 pf1, 2 poisson+sigma*/) {
+Operator make_op(const pf_grid* g, int which /*0 poisson, 1 pf1, 2 poisson+sigma, 3 Laplace in Omega_m*/) {
     Operator op;
     std::memset(&op, 0, sizeof(op));
     op.stored = g->stored ? 1 : 0;
     op.code32 = g->code_mode == 2 ? 1 : 0;
     op.cpitch = g->cpitch;
-    if (which == 1) {
+    if (which == 3) {             // always in code form: two coefficient values, 0 and -1/h^2
+        op.stored = 0; op.code32 = 0;
+        op.A0 = g->A0_L; op.code = g->code_L; op.ctab = g->ctab_L;
+    } else if (which == 1) {
         op.A0 = g->A0_pf1; op.code = g->code_pf1; op.ctab = g->ctab_pf1;
         for (int d = 0; d < 6; ++d) op.offd[d] = g->offd_pf1[d];
     } else {
@@ -440,6 +449,8 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
     g->capture_stream = nullptr; g->opt_graph = 1; g->opt_norm = 0;
+    g->opt_charge_model = 0; g->charge_model = 0; g->phiL = g->phistar = g->A0_L = nullptr; g->code_L = nullptr;
+    g->ctab_L = nullptr; g->laplace_iters = 0;
     g->small = nullptr;
     g->charges_dev = nullptr; g->sc = nullptr; g->rb.partial = nullptr; g->rb.ticket = nullptr;
     g->ctab_poisson = g->ctab_pf1 = nullptr; g->dmax_bits = nullptr; g->tma = nullptr;
@@ -462,6 +473,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->dmax_bits = reinterpret_cast<unsigned long long*>(g->small->dev + SS_DMAX);
     g->ctab_poisson = reinterpret_cast<double*>(g->small->dev + SS_CTAB0);
     g->ctab_pf1 = reinterpret_cast<double*>(g->small->dev + SS_CTAB1);
+    g->ctab_L = reinterpret_cast<double*>(g->small->dev + SS_CTAB1 + 128);
     g->rb.partial = reinterpret_cast<dd*>(g->small->dev + SS_PARTIAL);
     g->sc_host[0] = reinterpret_cast<Scalars*>(g->small->host);
     g->sc_host[1] = reinterpret_cast<Scalars*>(g->small->host + 256);
@@ -502,7 +514,8 @@ void pf_grid_destroy(pf_grid* g) {
 size_t pf_grid_workspace_bytes(const pf_grid* g) {
     if (!g) return 0;
     const size_t vec = align_up(sizeof(double) * (size_t)g->g.n, 256);
-    return (size_t)n_vectors(want_stored(g)) * vec + 2 * code_bytes_of(g);
+    const size_t code_l = g->opt_charge_model == 1 ? align_up((size_t)cpitch_of(g) * g->g.ny * g->g.nz * 2, 256) : 0;
+    return (size_t)n_vectors(want_stored(g), g->opt_charge_model) * vec + 2 * code_bytes_of(g) + code_l;
 }
 
 int pf_grid_set_option(pf_grid* g, int key, double value) {
@@ -565,6 +578,11 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
         case PF_OPT_NORM:
             if (iv != 0 && iv != 1) return fail(g, PF_ERR_ARG, "norm must be 0 or 1");
             g->opt_norm = iv; return PF_OK;
+        case PF_OPT_CHARGE_MODEL:
+            if (iv != 0 && iv != 1) return fail(g, PF_ERR_ARG, "charge model must be 0 or 1");
+            if (g->assembled && iv != g->charge_model)
+                return fail(g, PF_ERR_ARG, "set the charge model before pf_grid_set_workspace");
+            g->opt_charge_model = iv; return PF_OK;
         case PF_OPT_GRAPH:
             g->opt_graph = iv != 0; return PF_OK;
         case PF_OPT_KERNELS:
@@ -592,6 +610,8 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     g->t = take(); g->y = take(); g->bw = take(); g->xw = take();
     g->A0 = take(); g->A0_pf1 = take(); g->A0_s = take(); g->fixed = take(); g->psi = take();
     g->phi0 = take(); g->phiw = take(); g->sigma = take(); g->bpf = take();
+    g->charge_model = g->opt_charge_model;
+    if (g->charge_model == 1) { g->phiL = take(); g->phistar = take(); g->A0_L = take(); }
     for (int d = 0; d < 6; ++d) { g->offd[d] = g->stored ? take() : nullptr; }
     for (int d = 0; d < 6; ++d) { g->offd_pf1[d] = g->stored ? take() : nullptr; }
     g->code_mode = code_mode_of(g);
@@ -599,6 +619,7 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     const size_t cb = code_bytes_of(g);
     g->code = cb ? (void*)base : nullptr; base += cb;
     g->code_pf1 = cb ? (void*)base : nullptr; base += cb;
+    if (g->charge_model == 1) { g->code_L = (void*)base; base += align_up((size_t)g->cpitch * g->g.ny * g->g.nz * 2, 256); }
     // rows L1, L2: Poisson operator, coefficient table, fixed charges
     if (cb) PF_CUDA(g, cudaMemsetAsync(g->code, 0, 2 * cb, g->stream));    // padding columns of the code rows
     launch_assemble_poisson(g->stream, g->g, g->h, g->bc, g->eps, g->pal, g->code_mode, g->A0, g->code, g->cpitch,
@@ -608,7 +629,27 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
         build_ctab_poisson(g->pal, g->h, ctab);
         PF_CUDA(g, cudaMemcpyAsync(g->ctab_poisson, ctab, sizeof(ctab), cudaMemcpyHostToDevice, g->stream));
     }
-    launch_deposit(g->stream, g->g, g->h, kappa_angstrom(), g->charges_dev, g->ncharges, g->fixed);
+    if (g->charge_model == 0) {
+        launch_deposit(g->stream, g->g, g->h, kappa_angstrom(), g->charges_dev, g->ncharges, g->fixed);
+    } else {
+        // Table 2 step 1 / Table 4 steps 2-3: phi^L by the Krylov core, then the interface vector b^IF (in `fixed`)
+        if (g->uniform) return fail(g, PF_ERR_ARG, "the singular-charge model needs a map with a low-eps region (Omega_m)");
+        const double kap = kappa_angstrom();
+        double ctab[PF_CTAB] = {0.0};
+        ctab[1] = -(1.0 / (g->h * g->h));
+        PF_CUDA(g, cudaMemcpyAsync(g->ctab_L, ctab, sizeof(ctab), cudaMemcpyHostToDevice, g->stream));
+        PF_CUDA(g, cudaMemsetAsync(g->code_L, 0, align_up((size_t)g->cpitch * g->g.ny * g->g.nz * 2, 256), g->stream));
+        PF_CUDA(g, cudaMemsetAsync(g->p0, 0, vec * 4, g->stream));
+        launch_laplace_m(g->stream, g->g, g->h, g->eps, g->eps_mid, g->eps_min, kap, g->charges_dev, g->ncharges, g->A0_L,
+                         g->code_L, g->cpitch, g->bpf, g->phiL);
+        g->assembled = true;                  // the solver core may run now
+        int rc = bicgstab_device(g, make_op(g, 3), g->bpf, g->phiL, g->opt_lin_tol, g->opt_lin_maxit, &g->laplace_iters,
+                                 nullptr, nullptr);
+        if (rc < 0) { g->assembled = false; return rc; }
+        launch_phistar(g->stream, g->g, g->h, g->eps, g->eps_mid, g->eps_min, kap, g->charges_dev, g->ncharges, g->phistar);
+        launch_interface_rhs(g->stream, g->g, g->h, g->eps, g->eps_mid, g->eps_min, kap, g->charges_dev, g->ncharges,
+                             g->phiL, g->fixed);
+    }
     PF_CUDA(g, cudaMemsetAsync(g->p0, 0, vec * 4, g->stream));   // p0,p1,v0,v1 finite before first use
     PF_CUDA(g, cudaStreamSynchronize(g->stream));
     PF_CUDA(g, cudaGetLastError());
@@ -722,6 +763,7 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
         if (!(d > tol)) { status = PF_OK; break; }
     }
     PF_CUDA(g, cudaMemcpyAsync(phi, phi0, nbytes, cudaMemcpyDeviceToDevice, g->stream));
+    if (g->charge_model == 1) launch_recombine(g->stream, g->g.n, g->phistar, g->phiL, phi);   // Eq (5)
     if (conc || steric)
         launch_fermi(g->stream, g->g, g->bc, sp, g->eps, g->eps_mid, g->uniform, phi0, nullptr, nullptr, steric, conc,
                      nullptr, nullptr, nullptr);
@@ -763,6 +805,8 @@ int pf_grid_profile(pf_grid* g, double* ms_out, long long* launches_out) {
     return PF_OK;
 }
 
+int pf_grid_laplace_iters(const pf_grid* g) { return g ? g->laplace_iters : PF_ERR_ARG; }
+
 int pf_grid_fault_repeats(const pf_grid* g) { return g ? g->fault_repeats : PF_ERR_ARG; }
 
 int pf_grid_stencil(const pf_grid* g) { return g ? (want_stored(g) ? 1 : 2) : PF_ERR_ARG; }
@@ -790,6 +834,8 @@ int pf_grid_copy_array(pf_grid* g, int which, void* dst) {
     else if (which == 10) { src = g->code_mode ? g->ctab_poisson : nullptr; nbytes = sizeof(double) * PF_CTAB; }
     else if (which == 11) { src = (g->pf1_lc == g->pf1_lc) ? g->code_pf1 : nullptr; nbytes = code_bytes_of(g); }
     else if (which == 13) src = (g->pf1_lc == g->pf1_lc) ? g->psi : nullptr;
+    else if (which == 14) src = g->charge_model == 1 ? g->phiL : nullptr;
+    else if (which == 15) src = g->charge_model == 1 ? g->phistar : nullptr;
     else if (which == 12) { src = (g->pf1_lc == g->pf1_lc && g->code_mode) ? g->ctab_pf1 : nullptr; nbytes = sizeof(double) * PF_CTAB; }
     if (!src) return fail(g, PF_ERR_ARG, "array %d is not available", which);
     PF_CUDA(g, cudaMemcpyAsync(dst, src, nbytes, cudaMemcpyDeviceToDevice, g->stream));

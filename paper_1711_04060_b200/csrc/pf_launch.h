@@ -92,6 +92,21 @@ void launch_set_dirichlet(cudaStream_t s, const GridDims& g, const BcDev& bc, do
 // b_work = rhs with Dirichlet values forced.
 void launch_copy_with_dirichlet(cudaStream_t s, const GridDims& g, const BcDev& bc, const double* src, double* dst);
 
+// ---- singular-charge decomposition (pf_singular.cu), Eqs (5)-(10), readings S1-S5 ----------------------
+// Laplace problem for phi^L in Omega_m: diagonal, uint16 stencil codes (table {0, -1/h^2}), right-hand side b
+// and start vector x0 (prescribed values on identity rows).
+void launch_laplace_m(cudaStream_t s, const GridDims& g, double h, const double* eps, double eps_mid, double eps_m,
+                      double kappa, const double* charges_dev, int m, double* A0, void* code, int cpitch, double* b,
+                      double* x0);
+// phi* on the Omega_m nodes (0 on Omega_s).
+void launch_phistar(cudaStream_t s, const GridDims& g, double h, const double* eps, double eps_mid, double eps_m,
+                    double kappa, const double* charges_dev, int m, double* out);
+// b^IF from the flux jumps of the interface faces (c0, d0 of Eqs (17)-(18)).
+void launch_interface_rhs(cudaStream_t s, const GridDims& g, double h, const double* eps, double eps_mid, double eps_m,
+                          double kappa, const double* charges_dev, int m, const double* phiL, double* b);
+// phi := phi + phi* + phi^L.
+void launch_recombine(cudaStream_t s, long long n, const double* phistar, const double* phiL, double* phi);
+
 // ---- pointwise PF kernels (pf_pointwise.cu) ------------------------------------------------
 struct SpeciesDev {
     int K;                              // ions; water is index K

@@ -22,7 +22,8 @@ PF_ERR_ARG, PF_ERR_CUDA, PF_ERR_BREAKDOWN, PF_ERR_NONPHYSICAL, PF_ERR_WORKSPACE 
 PF_BC_DIRICHLET, PF_BC_NEUMANN = 0, 1
 (PF_OPT_STENCIL, PF_OPT_OMEGA_PF, PF_OPT_LINEAR_TOL, PF_OPT_LINEAR_MAXIT, PF_OPT_CHECK_INTERVAL,
  PF_OPT_WATER_MOLAR, PF_OPT_MAX_OUTER, PF_OPT_PRECOND, PF_OPT_HISTORY, PF_OPT_KERNELS, PF_OPT_PROFILE,
- PF_OPT_GRAPH, PF_OPT_NORM) = range(1, 14)
+ PF_OPT_GRAPH, PF_OPT_NORM, PF_OPT_CHARGE_MODEL) = range(1, 15)
+CHARGES_DEPOSITED, CHARGES_SINGULAR = 0, 1
 NORM_REL_L2, NORM_ABS_INF = 0, 1
 STENCIL_AUTO, STENCIL_STORED, STENCIL_ONTHEFLY = 0, 1, 2
 KERNELS_AUTO, KERNELS_DIRECT, KERNELS_TILED = 0, 1, 2
@@ -30,7 +31,7 @@ KERNELS_AUTO, KERNELS_DIRECT, KERNELS_TILED = 0, 1, 2
 EXPORTS = [
     "pf_grid_create", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
     "pf_solve_linear", "pf_solve_linear_host", "pf_solve_pf", "pf_fermi_pointwise", "pf_grid_history",
-    "pf_grid_linear_iters", "pf_grid_increments", "pf_grid_fault_repeats", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_code_layout", "pf_grid_copy_array",
+    "pf_grid_linear_iters", "pf_grid_increments", "pf_grid_fault_repeats", "pf_grid_laplace_iters", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_code_layout", "pf_grid_copy_array",
     "pf_grid_profile", "pf_launch_count", "pf_grid_destroy", "pf_last_error", "pf_version",
 ]
 
@@ -78,6 +79,7 @@ def load():
     L.pf_grid_linear_iters.argtypes = [_vp, _ip, ctypes.c_int]
     L.pf_grid_increments.argtypes = [_vp, _dp, ctypes.c_int]
     L.pf_grid_fault_repeats.argtypes = [_vp]
+    L.pf_grid_laplace_iters.argtypes = [_vp]
     L.pf_grid_stencil.argtypes = [_vp]
     L.pf_grid_palette_size.argtypes = [_vp]
     L.pf_grid_copy_array.argtypes = [_vp, ctypes.c_int, _vp]
@@ -221,6 +223,10 @@ def pf_grid_profile(handle) -> dict:
 
 def pf_launch_count() -> int:
     return int(load().pf_launch_count())
+
+
+def pf_grid_laplace_iters(handle) -> int:
+    return load().pf_grid_laplace_iters(handle)
 
 
 def pf_grid_fault_repeats(handle) -> int:
