@@ -260,6 +260,10 @@ cudaGraphExec_t chunk_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, 
     if (ok) ok = cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess;
     if (graph) cudaGraphDestroy(graph);
     if (!ok) { cudaGetLastError(); g->opt_graph = 0; return nullptr; }
+    if (g->graphs.size() >= 16) {              // callers that keep changing x: drop the oldest graph
+        cudaGraphExecDestroy(g->graphs.front().exec);
+        g->graphs.erase(g->graphs.begin());
+    }
     g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled, chunk, exec});
     return exec;
 }

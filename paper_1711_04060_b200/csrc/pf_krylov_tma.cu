@@ -73,7 +73,6 @@ struct Layout {
     static constexpr int STAGE_BYTES = T::NF * FIELD_BYTES + (T::OWN ? OWN_BYTES : 0) + CODE_BYTES;
     static constexpr int OWN_OFF = T::NF * FIELD_BYTES;
     static constexpr int CODE_OFF = OWN_OFF + (T::OWN ? OWN_BYTES : 0);
-    static constexpr int U_BYTES = BX * BY * 8;                     // one buffer of u
     static constexpr int U_OFF = T::STAGES * STAGE_BYTES;
     static constexpr int CTAB_OFF = U_OFF + NU * FIELD_BYTES;
     static constexpr int SCRATCH_OFF = CTAB_OFF + PF_CTAB * 8;
