@@ -329,12 +329,21 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     *reinterpret_cast<double2*>(kv.p_out + own_off + plane * z) = make_double2(up.n[0], up.n[1]);
                 if (to_shared) *reinterpret_cast<double2*>(u_buf(k) + pair_box) = make_double2(up.u[0], up.u[1]);
             };
+            double pa[2] = {0.0, 0.0}, pb[2] = {0.0, 0.0};   // operands of the deferred inner products (zeros add nothing)
             auto step = [&](int z, const Slot& dn, const Slot& c, Slot& up) {
                 const int k = z - z0 + 1;                               // load-sequence index of plane z
                 const long long i = own_off + plane * z;
                 const double* u_s = u_buf(k);
                 wait_ready(k);
                 load_slot(k + 1, up, true);
+                // inner products of the PREVIOUS plane: a third independent chain beside the divisions of plane
+                // z+1 and the 7-point sums of plane z
+                if (MODE == MODE_K1) {
+                    dd_fma(q[0], pa[0], pb[0]); dd_fma(q[1], pa[1], pb[1]);
+                } else if (MODE == MODE_K2) {
+                    dd_fma(q[0], pa[0], pb[0]); dd_fma(q[0], pa[1], pb[1]);
+                    dd_fma(q[1], pa[0], pa[0]); dd_fma(q[1], pa[1], pa[1]);
+                }
                 const double2 us = *reinterpret_cast<const double2*>(u_s + pair_box - BX);
                 const double2 un = *reinterpret_cast<const double2*>(u_s + pair_box + BX);
                 const double uw = u_s[pair_box - 1], ue = u_s[pair_box + 2];
@@ -370,11 +379,10 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 out[1] = add(out[1], mul(c5[1], up.u[1]));
                 if (MODE == MODE_K1) {
                     if (pair_ok) *reinterpret_cast<double2*>(kv.v_out + i) = make_double2(out[0], out[1]);
-                    dd_fma(q[0], c.w.x, out[0]); dd_fma(q[1], c.w.y, out[1]);
+                    pa[0] = c.w.x; pa[1] = c.w.y; pb[0] = out[0]; pb[1] = out[1];      // r~ . v', next step
                 } else if (MODE == MODE_K2) {
                     if (pair_ok) *reinterpret_cast<double2*>(kv.t + i) = make_double2(out[0], out[1]);
-                    dd_fma(q[0], out[0], c.n[0]); dd_fma(q[0], out[1], c.n[1]);
-                    dd_fma(q[1], out[0], out[0]); dd_fma(q[1], out[1], out[1]);
+                    pa[0] = out[0]; pa[1] = out[1]; pb[0] = c.n[0]; pb[1] = c.n[1];    // t . s and t . t, next step
                 } else {
                     const double r0 = sub(c.w.x, out[0]), r1 = sub(c.w.y, out[1]);
                     if (MODE == MODE_R0) {
@@ -400,6 +408,12 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 step(z + 1, s1, s2, s0);
                 if (z + 2 >= z1) break;
                 step(z + 2, s2, s0, s1);
+            }
+            if (MODE == MODE_K1) {                           // the last plane's inner products
+                dd_fma(q[0], pa[0], pb[0]); dd_fma(q[1], pa[1], pb[1]);
+            } else if (MODE == MODE_K2) {
+                dd_fma(q[0], pa[0], pb[0]); dd_fma(q[0], pa[1], pb[1]);
+                dd_fma(q[1], pa[0], pa[0]); dd_fma(q[1], pa[1], pa[1]);
             }
         }
     }
