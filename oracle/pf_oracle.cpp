@@ -30,7 +30,9 @@
 //                   saturation C_k < 1/v_k; radii->0 => Boltzmann
 //   outer loop    : l_c=0 + steric off => nonlinear PB (Gouy-Chapman closed form in 1-D);
 //                   independence of omega_PF; fixed-point residuals of PF1/PF2 at convergence
-//   full PF, l_c>0, unequal radii, 3-D: PARITY UNPINNED beyond the reductions above.
+//                   l_c > 0 coupling: closed form of the discrete split system for a sine-mode source
+//   full PF with l_c>0, steric term and strong nonlinearity together, 3-D: PARITY UNPINNED as a whole
+//                   (each ingredient is pinned above).
 //   singular charges (Eqs 5-10): Coulomb sums vs numpy; 1-D closed form with a prescribed flux jump (c0, d0 of
 //                   Eqs 17-18); discrete Gauss law sum b^IF h^3 = kappa sum q; harmonic phi^L; Born ion;
 //                   agreement with the independent deposition model in the solvent (tests/test_oracle_singular.py)

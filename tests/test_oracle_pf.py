@@ -145,3 +145,38 @@ def test_initial_guess_is_linear_poisson(oracle):
     lin = oracle.solve_linear(n, n, n, h, bt, bv, eps, fixed, tol=1e-12)
     assert r["status"] == 1 and r["outer_iters"] == 0
     assert np.array_equal(r["phi"], lin["x"])
+
+
+def test_split_system_sine_mode_closed_form(oracle):
+    """Pins the l_c > 0 path (PF1/PF2 coupling of Eqs (12)-(14), sign and size of the l_c^2 term, kappa, Psi = 0
+    on the whole box boundary) by the closed form of the DISCRETE split system: uniform eps, phi = Psi = 0 on all
+    faces, no steric term, a weak source f = F sin sin sin (an eigenfunction of the 7-point Laplacian with
+    eigenvalue -mu, mu = (12/h^2) sin^2(pi h/2L)).  With rho ~ -2 C^B phi (1:1 electrolyte, |phi| ~ 1e-3):
+        PF2 fixed point:  eps mu phi = -eps Psi + f,     PF1:  eps (l_c^2 mu + 1) Psi = 2 kappa C^B phi
+        =>  phi = f (l_c^2 mu + 1) / (eps l_c^2 mu^2 + eps mu + 2 kappa C^B),   Psi = (f - eps mu phi)/eps.
+    The eps l_c^2 mu^2 term is the fourth-order operator of Eq (2)."""
+    n, h, lc, eps_w = 21, 0.5, 1.2, 78.5
+    L = (n - 1) * h
+    ax = np.sin(np.pi * np.arange(n) * h / L)
+    mode = (ax[:, None, None] * ax[None, :, None] * ax[None, None, :]).reshape(-1)
+    mu = 12.0 / h ** 2 * np.sin(np.pi * h / (2 * L)) ** 2
+    cb = 0.1 * oracle.molar_to_per_A3()
+    denom = eps_w * lc ** 2 * mu ** 2 + eps_w * mu + 2 * oracle.kappa() * cb
+    F = 1e-3 * denom / (lc ** 2 * mu + 1)                    # so that the peak potential is 1e-3 kT/e
+    eps = np.full(n ** 3, eps_w)
+    bt, bv = [D] * 6, [0.0] * 6
+    r = oracle.solve_pf(n, n, n, h, bt, bv, eps, np.zeros((0, 4)), [1.0, -1.0], [0.1, 0.1], [0.0, 0.0, 0.0], lc, 1e-14,
+                        lin_tol=1e-13, max_outer=400, fixed_override=F * mode)
+    assert r["status"] == 0
+    phi_exact = 1e-3 * mode
+    psi_exact = (F * mode - eps_w * mu * phi_exact) / eps_w
+    # nonlinearity of sinh at 1e-3 is 2e-7 relative; everything else is solver tolerance
+    assert np.abs(r["phi"] - phi_exact).max() < 1e-6 * 1e-3
+    assert np.abs(r["psi"] - psi_exact).max() < 1e-6 * np.abs(psi_exact).max()
+    # the l_c term matters: without it the amplitude would differ by far more than the tolerance
+    no_lc = F / (eps_w * mu + 2 * oracle.kappa() * cb)
+    assert abs(no_lc - 1e-3) > 1e-2 * 1e-3
+    # same closed form with l_c = 0 (PF reduces to linearised Poisson-Boltzmann, PAPER.md:28)
+    r0 = oracle.solve_pf(n, n, n, h, bt, bv, eps, np.zeros((0, 4)), [1.0, -1.0], [0.1, 0.1], [0.0, 0.0, 0.0], 0.0, 1e-14,
+                         lin_tol=1e-13, max_outer=400, fixed_override=F * mode)
+    assert np.abs(r0["phi"] - no_lc * mode).max() < 1e-6 * no_lc
