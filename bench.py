@@ -182,6 +182,13 @@ def run_b200(args):
 
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the library has no CPU fallback")
+    from paper_1711_04060_b200 import build as _build
+    if int(os.environ.get("LOCAL_RANK", "0")) == 0:
+        _build.build()          # no-op when the in-tree library is up to date
+    else:                       # the other ranks wait for rank 0's build
+        t_wait = time.time()
+        while _build._stale() and time.time() - t_wait < 600:
+            time.sleep(1.0)
     pf.load()
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))

@@ -18,7 +18,8 @@ from paper_1711_04060_b200 import workloads as wl  # noqa: E402
 def pf():
     if not torch.cuda.is_available():
         pytest.skip("needs a CUDA device")
-    from paper_1711_04060_b200 import pf as _pf
+    from paper_1711_04060_b200 import build as _build, pf as _pf
+    _build.build()      # no-op when libpf_b200.so is newer than its sources; needs nvcc otherwise
     _pf.load()
     return _pf
 
