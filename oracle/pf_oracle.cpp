@@ -63,6 +63,10 @@ struct Grid {
     double h;
     int bc_type[6];
     double bc_value[6];
+    // Omega_f (readings F1-F3): nodes whose potential is prescribed by an atomic model the
+    // caller brings.  fix_mask[i] != 0 => phi_i = fix_val[i] (an interior Dirichlet node).  Null = no such nodes.
+    const uint8_t* fix_mask = nullptr;
+    const double* fix_val = nullptr;
     int64_t n() const { return (int64_t)nx * ny * nz; }
 };
 
@@ -100,7 +104,7 @@ void assemble_poisson(const Grid& g, const double* eps, const double* sigma, dou
         for (int iy = 0; iy < g.ny; ++iy)
             for (int ix = 0; ix < g.nx; ++ix) {
                 int64_t i = ix + (int64_t)g.nx * (iy + (int64_t)g.ny * iz);
-                if (dirichlet_face(g, ix, iy, iz) >= 0) {
+                if (dirichlet_face(g, ix, iy, iz) >= 0 || (g.fix_mask && g.fix_mask[i])) {   // Q20, F2
                     A[i] = 1.0;
                     for (int d = 1; d < 7; ++d) A[d * N + i] = 0.0;
                     continue;
@@ -194,7 +198,9 @@ void set_dirichlet(const Grid& g, double* x) {
         for (int iy = 0; iy < g.ny; ++iy)
             for (int ix = 0; ix < g.nx; ++ix) {
                 int f = dirichlet_face(g, ix, iy, iz);
-                if (f >= 0) x[ix + (int64_t)g.nx * (iy + (int64_t)g.ny * iz)] = g.bc_value[f];
+                int64_t i = ix + (int64_t)g.nx * (iy + (int64_t)g.ny * iz);
+                if (f >= 0) x[i] = g.bc_value[f];
+                else if (g.fix_mask && g.fix_mask[i]) x[i] = g.fix_val[i];
             }
 }
 
@@ -570,15 +576,18 @@ double pfo_kappa(void) { return kappa_angstrom(); }
 double pfo_kT_over_e_volt(void) { return K_B * T_ABS / E_CH; }
 double pfo_molar_to_per_A3(void) { return AVOGADRO_PER_A3; }
 
-static Grid mk(int nx, int ny, int nz, double h, const int* bct, const double* bcv) {
+static Grid mk(int nx, int ny, int nz, double h, const int* bct, const double* bcv,
+               const uint8_t* fix_mask = nullptr, const double* fix_val = nullptr) {
     Grid g; g.nx = nx; g.ny = ny; g.nz = nz; g.h = h;
     for (int f = 0; f < 6; ++f) { g.bc_type[f] = bct[f]; g.bc_value[f] = bcv[f]; }
+    g.fix_mask = fix_mask; g.fix_val = fix_val;
     return g;
 }
 
 void pfo_assemble_poisson(int nx, int ny, int nz, double h, const int* bct, const double* bcv,
-                          const double* eps, const double* sigma, double* A) {
-    assemble_poisson(mk(nx, ny, nz, h, bct, bcv), eps, sigma, A);
+                          const double* eps, const double* sigma, double* A,
+                          const uint8_t* fix_mask, const double* fix_val) {
+    assemble_poisson(mk(nx, ny, nz, h, bct, bcv, fix_mask, fix_val), eps, sigma, A);
 }
 
 void pfo_assemble_pf1(int nx, int ny, int nz, double h, const int* bct, const double* bcv,
@@ -595,8 +604,9 @@ void pfo_dia_spmv(int nx, int ny, int nz, const double* A, const double* x, doub
 
 double pfo_dot(int64_t N, const double* a, const double* b) { return dot(N, a, b); }
 
-void pfo_set_dirichlet(int nx, int ny, int nz, const int* bct, const double* bcv, double* x) {
-    set_dirichlet(mk(nx, ny, nz, 1.0, bct, bcv), x);
+void pfo_set_dirichlet(int nx, int ny, int nz, const int* bct, const double* bcv, double* x,
+                       const uint8_t* fix_mask, const double* fix_val) {
+    set_dirichlet(mk(nx, ny, nz, 1.0, bct, bcv, fix_mask, fix_val), x);
 }
 
 void pfo_deposit_charges(int nx, int ny, int nz, double h, const double* charges, int M, double* b) {
@@ -617,8 +627,9 @@ int pfo_bicgstab(int nx, int ny, int nz, const double* A, const double* b, doubl
 int pfo_solve_linear(int nx, int ny, int nz, double h, const int* bct, const double* bcv,
                      const double* eps, const double* sigma, const double* rhs, double* x,
                      double tol, int maxit, int precond, int* iters, double* relres,
-                     double* true_relres, double* hist, int norm_mode) {
-    Grid g = mk(nx, ny, nz, h, bct, bcv);
+                     double* true_relres, double* hist, int norm_mode,
+                     const uint8_t* fix_mask, const double* fix_val) {
+    Grid g = mk(nx, ny, nz, h, bct, bcv, fix_mask, fix_val);
     const int64_t N = g.n();
     std::vector<double> A(7 * N), b(rhs, rhs + N);
     assemble_poisson(g, eps, sigma, A.data());
@@ -650,14 +661,18 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
                  double* phi /* out */, double* psi /* out or null */, double* conc /* out or null */,
                  double* steric /* out or null */,
                  int* outer_iters, int* linear_iters, int* lin_iters_hist, int hist_cap,
-                 double* incr_hist, const double* fixed_override /* b^IF of the singular-charge model, or null */) {
-    Grid g = mk(nx, ny, nz, h, bct, bcv);
+                 double* incr_hist, const double* fixed_override /* b^IF of the singular-charge model, or null */,
+                 const uint8_t* fix_mask, const double* fix_val /* Omega_f, or null */) {
+    Grid g = mk(nx, ny, nz, h, bct, bcv, fix_mask, fix_val);
     const int64_t N = g.n();
     SpeciesTab sp;
     int rc = make_species(K, valence, bath_molar, radii, water_molar, sp);
     if (rc) return rc;
     std::vector<uint8_t> solv(N);
     solvent_mask(N, eps, solv.data());
+    // F2, F3: in Omega_f neither Eq (1) nor PF1 applies: treat its nodes like non-solvent ones (C = rho = sigma = 0,
+    // Psi = 0); their PF2 rows are the identity rows that assemble_poisson and set_dirichlet produce
+    if (fix_mask) for (int64_t i = 0; i < N; ++i) if (fix_mask[i]) solv[i] = 0;
     std::vector<double> fixed(N, 0.0), A0(7 * N), A1(7 * N), A2(7 * N), b(N);
     std::vector<double> phi0(N, 0.0), Psi(N, 0.0), ph(N), rho(N), sigma(N), S(N);
     if (fixed_override) std::memcpy(fixed.data(), fixed_override, N * sizeof(double));

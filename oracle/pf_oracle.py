@@ -83,14 +83,27 @@ def dot(a, b) -> float:
     return lib().pfo_dot(ctypes.c_int64(a.size), _d(a), _d(b))
 
 
-def assemble_poisson(nx, ny, nz, h, bc_type, bc_value, eps, sigma=None) -> np.ndarray:
+def _fix(fixed_nodes, n):
+    """(mask uint8[n], values float64[n]) of Omega_f from (indices, values), or (None, None)."""
+    if fixed_nodes is None:
+        return None, None
+    idx, val = fixed_nodes
+    mask = np.zeros(n, dtype=np.uint8)
+    vals = np.zeros(n)
+    mask[np.asarray(idx, dtype=np.int64)] = 1
+    vals[np.asarray(idx, dtype=np.int64)] = np.asarray(val, dtype=np.float64)
+    return mask, vals
+
+
+def assemble_poisson(nx, ny, nz, h, bc_type, bc_value, eps, sigma=None, fixed_nodes=None) -> np.ndarray:
     """Rows of -div(eps grad u) + sigma u in the paper's A0..A6 format; returns (7, N)."""
     n = nx * ny * nz
     t, v = _bc(bc_type, bc_value)
     eps = _f64(eps)
     sigma = None if sigma is None else _f64(sigma)
     A = np.empty((7, n), dtype=np.float64)
-    lib().pfo_assemble_poisson(nx, ny, nz, ctypes.c_double(h), _i(t), _d(v), _d(eps), _d(sigma), _d(A))
+    fm, fv = _fix(fixed_nodes, n)
+    lib().pfo_assemble_poisson(nx, ny, nz, ctypes.c_double(h), _i(t), _d(v), _d(eps), _d(sigma), _d(A), _u8(fm), _d(fv))
     return A
 
 
@@ -120,10 +133,11 @@ def dia_spmv(nx, ny, nz, A, x) -> np.ndarray:
     return y
 
 
-def set_dirichlet(nx, ny, nz, bc_type, bc_value, x) -> np.ndarray:
+def set_dirichlet(nx, ny, nz, bc_type, bc_value, x, fixed_nodes=None) -> np.ndarray:
     t, v = _bc(bc_type, bc_value)
     x = _f64(x).copy()
-    lib().pfo_set_dirichlet(nx, ny, nz, _i(t), _d(v), _d(x))
+    fm, fv = _fix(fixed_nodes, nx * ny * nz)
+    lib().pfo_set_dirichlet(nx, ny, nz, _i(t), _d(v), _d(x), _u8(fm), _d(fv))
     return x
 
 
@@ -157,7 +171,7 @@ def bicgstab(nx, ny, nz, A, b, x0=None, tol=1e-10, maxit=10000, precond=True, hi
 
 
 def solve_linear(nx, ny, nz, h, bc_type, bc_value, eps, rhs, x0=None, sigma=None, tol=1e-10,
-                 maxit=10000, precond=True, history=False, norm=NORM_REL_L2):
+                 maxit=10000, precond=True, history=False, norm=NORM_REL_L2, fixed_nodes=None):
     """What pf_solve_linear computes: the grid's Poisson operator, Dirichlet data forced."""
     n = nx * ny * nz
     t, v = _bc(bc_type, bc_value)
@@ -169,9 +183,11 @@ def solve_linear(nx, ny, nz, h, bc_type, bc_value, eps, rhs, x0=None, sigma=None
     rr = ctypes.c_double(0)
     tr = ctypes.c_double(0)
     hist = np.full(maxit + 1, np.nan) if history else None
+    fm, fv = _fix(fixed_nodes, n)
     st = lib().pfo_solve_linear(nx, ny, nz, ctypes.c_double(h), _i(t), _d(v), _d(eps), _d(sigma), _d(rhs),
                                 _d(x), ctypes.c_double(tol), int(maxit), int(bool(precond)),
-                                ctypes.byref(it), ctypes.byref(rr), ctypes.byref(tr), _d(hist), int(norm))
+                                ctypes.byref(it), ctypes.byref(rr), ctypes.byref(tr), _d(hist), int(norm),
+                                _u8(fm), _d(fv))
     out = dict(x=x, status=st, iters=it.value, relres=rr.value, true_relres=tr.value)
     if history:
         out["hist"] = hist[: it.value + 1]
@@ -200,7 +216,7 @@ def fermi_pointwise(valence, bath_molar, radii, phi, solvent=None, water_molar=5
 
 def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar, radii, l_c, tol,
              omega_pf=0.3, lin_tol=1e-10, lin_maxit=10000, max_outer=200, water_molar=55.5, norm=NORM_REL_L2,
-             fixed_override=None):
+             fixed_override=None, fixed_nodes=None):
     """The outer loop of Table 2 / Table 4 (R5)."""
     n = nx * ny * nz
     t, v = _bc(bc_type, bc_value)
@@ -219,12 +235,14 @@ def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar
     cap = 2 * max_outer + 1
     lhist = np.zeros(cap, dtype=np.int32)
     ihist = np.zeros(max_outer, dtype=np.float64)
+    fm, fv = _fix(fixed_nodes, n)
     st = lib().pfo_solve_pf(nx, ny, nz, ctypes.c_double(h), _i(t), _d(v), _d(eps), _d(ch), int(ch.shape[0]),
                             int(K), _d(valence), _d(bath), _d(radii), ctypes.c_double(water_molar),
                             ctypes.c_double(l_c), ctypes.c_double(tol), ctypes.c_double(omega_pf),
                             ctypes.c_double(lin_tol), int(lin_maxit), int(max_outer), int(norm),
                             _d(phi), _d(psi), _d(conc), _d(steric), ctypes.byref(outer), ctypes.byref(lin),
-                            _i(lhist), int(cap), _d(ihist), _d(None if fixed_override is None else _f64(fixed_override)))
+                            _i(lhist), int(cap), _d(ihist), _d(None if fixed_override is None else _f64(fixed_override)),
+                            _u8(fm), _d(fv))
     return dict(phi=phi, psi=psi, conc=conc, steric=steric, status=st, outer_iters=outer.value,
                 linear_iters=lin.value, lin_iters_hist=lhist[: 2 * outer.value + 1].copy(),
                 incr_hist=ihist[: outer.value].copy())
