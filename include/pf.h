@@ -104,6 +104,14 @@ int pf_grid_create(pf_grid **out, int nx, int ny, int nz, double h,
                    const double *eps_map, const pf_charge *charges, int ncharges,
                    const pf_bc *bc, void *cuda_stream);
 
+/* Omega_f (readings F1-F3 of DESIGN.md): `count` nodes whose potential an atomic model
+ * prescribes.  idx_host[k] is the linear index of a node, val_host[k] its potential in k_B T/e; both host, copied.
+ * These nodes become interior Dirichlet nodes of every system built on the grid (identity rows, neighbours keep
+ * their coupling, Q20), carry Psi = 0 in PF1, and are excluded from the Fermi distribution (C_k = 0 there).
+ * Must be called before pf_grid_workspace_bytes / pf_grid_set_workspace (one more workspace vector); count = 0
+ * removes them.  Errors: PF_ERR_ARG (index outside the grid, NaN value, called after assembly). */
+int pf_grid_set_fixed_nodes(pf_grid *g, const long long *idx_host, const double *val_host, int count);
+
 /* Bytes of device scratch the grid needs with its current options (stencil variant). */
 size_t pf_grid_workspace_bytes(const pf_grid *g);
 

@@ -150,6 +150,10 @@ struct pf_grid {
     void* code_L;
     double* ctab_L;
     int laplace_iters;
+    // Omega_f: nodes with prescribed potential (readings F1-F3); fixv lives in the workspace
+    std::vector<long long> fix_idx;
+    std::vector<double> fix_val;
+    double* fixv;
     int fault_repeats;       // solves repeated by the direct kernels after a division range fault (D4)
     std::string err;
 };
@@ -172,7 +176,9 @@ int fail(pf_grid* g, int code, const char* fmt, ...) {
         if (e_ != cudaSuccess) return fail((g), PF_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
     } while (0)
 
-int n_vectors(bool stored, int charge_model) { return 19 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0); }
+int n_vectors(bool stored, int charge_model, bool fixed_nodes) {
+    return 19 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0) + (fixed_nodes ? 1 : 0);
+}
 
 int code_mode_of(const pf_grid* g) { return g->pal.count > PF_MAX_PALETTE ? 0 : (g->pal.count <= 2 ? 1 : 2); }
 int cpitch_of(const pf_grid* g) { return (g->g.nx + 7) & ~7; }
@@ -454,7 +460,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
     g->capture_stream = nullptr; g->opt_graph = 1; g->opt_norm = 0;
     g->opt_charge_model = 0; g->charge_model = 0; g->phiL = g->phistar = g->A0_L = nullptr; g->code_L = nullptr;
-    g->ctab_L = nullptr; g->laplace_iters = 0;
+    g->ctab_L = nullptr; g->laplace_iters = 0; g->fixv = nullptr; g->bc.fixv = nullptr;
     g->small = nullptr;
     g->charges_dev = nullptr; g->sc = nullptr; g->rb.partial = nullptr; g->rb.ticket = nullptr;
     g->ctab_poisson = g->ctab_pf1 = nullptr; g->dmax_bits = nullptr; g->tma = nullptr;
@@ -519,7 +525,7 @@ size_t pf_grid_workspace_bytes(const pf_grid* g) {
     if (!g) return 0;
     const size_t vec = align_up(sizeof(double) * (size_t)g->g.n, 256);
     const size_t code_l = g->opt_charge_model == 1 ? align_up((size_t)cpitch_of(g) * g->g.ny * g->g.nz * 2, 256) : 0;
-    return (size_t)n_vectors(want_stored(g), g->opt_charge_model) * vec + 2 * code_bytes_of(g) + code_l;
+    return (size_t)n_vectors(want_stored(g), g->opt_charge_model, !g->fix_idx.empty()) * vec + 2 * code_bytes_of(g) + code_l;
 }
 
 int pf_grid_set_option(pf_grid* g, int key, double value) {
@@ -616,6 +622,7 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     g->phi0 = take(); g->phiw = take(); g->sigma = take(); g->bpf = take();
     g->charge_model = g->opt_charge_model;
     if (g->charge_model == 1) { g->phiL = take(); g->phistar = take(); g->A0_L = take(); }
+    g->fixv = g->fix_idx.empty() ? nullptr : take();
     for (int d = 0; d < 6; ++d) { g->offd[d] = g->stored ? take() : nullptr; }
     for (int d = 0; d < 6; ++d) { g->offd_pf1[d] = g->stored ? take() : nullptr; }
     g->code_mode = code_mode_of(g);
@@ -624,6 +631,14 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     g->code = cb ? (void*)base : nullptr; base += cb;
     g->code_pf1 = cb ? (void*)base : nullptr; base += cb;
     if (g->charge_model == 1) { g->code_L = (void*)base; base += align_up((size_t)g->cpitch * g->g.ny * g->g.nz * 2, 256); }
+    g->bc.fixv = g->fixv;
+    if (g->fixv) {            // Omega_f: NaN = free node, then the prescribed values (r, r~ serve as staging)
+        const int cnt = (int)g->fix_idx.size();
+        PF_CUDA(g, cudaMemsetAsync(g->fixv, 0xFF, sizeof(double) * (size_t)g->g.n, g->stream));
+        PF_CUDA(g, cudaMemcpyAsync(g->rt, g->fix_idx.data(), sizeof(long long) * cnt, cudaMemcpyHostToDevice, g->stream));
+        PF_CUDA(g, cudaMemcpyAsync(g->r, g->fix_val.data(), sizeof(double) * cnt, cudaMemcpyHostToDevice, g->stream));
+        launch_scatter_fixed(g->stream, reinterpret_cast<const long long*>(g->rt), g->r, cnt, g->fixv);
+    }
     // rows L1, L2: Poisson operator, coefficient table, fixed charges
     if (cb) PF_CUDA(g, cudaMemsetAsync(g->code, 0, 2 * cb, g->stream));    // padding columns of the code rows
     launch_assemble_poisson(g->stream, g->g, g->h, g->bc, g->eps, g->pal, g->code_mode, g->A0, g->code, g->cpitch,
@@ -717,7 +732,7 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
     if (rc) return rc;
     const size_t nbytes = sizeof(double) * (size_t)g->g.n;
     if (!(g->pf1_lc == l_c)) {      // row N2: PF1 operator, once per (grid, l_c)
-        launch_assemble_pf1(g->stream, g->g, g->h, l_c, g->eps, g->eps_mid, g->uniform, g->pal, g->code_mode, g->A0_pf1,
+        launch_assemble_pf1(g->stream, g->g, g->h, l_c, g->bc, g->eps, g->eps_mid, g->uniform, g->pal, g->code_mode, g->A0_pf1,
                             g->code_pf1, g->cpitch, g->offd_pf1);
         if (g->code_mode) {
             double ctab[PF_CTAB];
@@ -806,6 +821,20 @@ long long pf_launch_count(void) { return pf::g_launch_count; }
 int pf_grid_profile(pf_grid* g, double* ms_out, long long* launches_out) {
     if (!g || !ms_out || !launches_out) return PF_ERR_ARG;
     for (int j = 0; j < 3; ++j) { ms_out[j] = g->prof_ms[j]; launches_out[j] = g->prof_launches[j]; }
+    return PF_OK;
+}
+
+int pf_grid_set_fixed_nodes(pf_grid* g, const long long* idx_host, const double* val_host, int count) {
+    if (!g) return PF_ERR_ARG;
+    if (g->assembled) return fail(g, PF_ERR_ARG, "set the fixed nodes before pf_grid_set_workspace");
+    if (count < 0 || (count > 0 && (!idx_host || !val_host))) return fail(g, PF_ERR_ARG, "bad fixed-node list");
+    if ((long long)count > g->g.n) return fail(g, PF_ERR_ARG, "more fixed nodes than grid nodes");
+    for (int k = 0; k < count; ++k) {
+        if (idx_host[k] < 0 || idx_host[k] >= g->g.n) return fail(g, PF_ERR_ARG, "fixed node %d is outside the grid", k);
+        if (!(val_host[k] == val_host[k])) return fail(g, PF_ERR_ARG, "fixed node %d has a NaN value", k);
+    }
+    g->fix_idx.assign(idx_host, idx_host + count);
+    g->fix_val.assign(val_host, val_host + count);
     return PF_OK;
 }
 

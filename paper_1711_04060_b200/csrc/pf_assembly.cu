@@ -109,7 +109,7 @@ k_assemble_poisson(GridDims g, double h, BcDev bc, const double* __restrict__ ep
         decode(g, i, ix, iy, iz);
         const long long k = ix + (long long)cpitch * (iy + (long long)g.ny * iz);
         const double ei = eps[i];
-        const bool ident = dirichlet_face(g, bc, ix, iy, iz) >= 0;
+        const bool ident = dirichlet_face(g, bc, ix, iy, iz) >= 0 || is_fixed_node(bc, i);   // Q20, F2
         if (ident) {
             A0[i] = 1.0;
             store_code(code, code_mode, k, 0u);
@@ -138,7 +138,7 @@ k_assemble_poisson(GridDims g, double h, BcDev bc, const double* __restrict__ ep
 }
 
 __global__ void __launch_bounds__(ASM_THREADS)
-k_assemble_pf1(GridDims g, double h, double lc, const double* __restrict__ eps, double eps_mid, bool uniform,
+k_assemble_pf1(GridDims g, double h, double lc, BcDev bc, const double* __restrict__ eps, double eps_mid, bool uniform,
                Palette pal, int code_mode, double* __restrict__ A0, void* __restrict__ code, int cpitch, double* o0,
                double* o1, double* o2, double* o3, double* o4, double* o5) {
     double* offd[6] = {o0, o1, o2, o3, o4, o5};
@@ -152,7 +152,7 @@ k_assemble_pf1(GridDims g, double h, double lc, const double* __restrict__ eps, 
         const double ei = eps[i];
         const bool boundary = ix == 0 || ix == g.nx - 1 || iy == 0 || iy == g.ny - 1 || iz == 0 || iz == g.nz - 1;
         const bool solvent = uniform || ei > eps_mid;           // Q17
-        const bool ident = boundary || !solvent;                // Q15
+        const bool ident = boundary || !solvent || is_fixed_node(bc, i);   // Q15, F2
         if (ident) {
             A0[i] = 1.0;
             store_code(code, code_mode, k, 0u);
@@ -242,6 +242,7 @@ k_set_dirichlet(GridDims g, BcDev bc, const double* __restrict__ src, double* __
         decode(g, i, ix, iy, iz);
         const int f = dirichlet_face(g, bc, ix, iy, iz);
         if (f >= 0) dst[i] = bc.value[f];
+        else if (is_fixed_node(bc, i)) dst[i] = bc.fixv[i];
         else if (src != dst) dst[i] = src[i];
     }
 }
@@ -289,11 +290,23 @@ void launch_assemble_poisson(cudaStream_t s, const GridDims& g, double h, const 
                                                                 offd[1], offd[2], offd[3], offd[4], offd[5]);
 }
 
-void launch_assemble_pf1(cudaStream_t s, const GridDims& g, double h, double lc, const double* eps, double eps_mid,
-                         bool uniform, const Palette& pal, int code_mode, double* A0, void* code, int cpitch,
-                         double* const offd[6]) {
+__global__ void k_scatter_fixed(const long long* __restrict__ idx, const double* __restrict__ val, int count,
+                                double* __restrict__ fixv) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < count) fixv[idx[k]] = val[k];
+}
+
+void launch_scatter_fixed(cudaStream_t s, const long long* idx_dev, const double* val_dev, int count, double* fixv) {
+    if (count <= 0) return;
     ++g_launch_count;
-    k_assemble_pf1<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, h, lc, eps, eps_mid, uniform, pal, code_mode, A0, code,
+    k_scatter_fixed<<<(count + 255) / 256, 256, 0, s>>>(idx_dev, val_dev, count, fixv);
+}
+
+void launch_assemble_pf1(cudaStream_t s, const GridDims& g, double h, double lc, const BcDev& bc, const double* eps,
+                         double eps_mid, bool uniform, const Palette& pal, int code_mode, double* A0, void* code,
+                         int cpitch, double* const offd[6]) {
+    ++g_launch_count;
+    k_assemble_pf1<<<asm_blocks(g.n), ASM_THREADS, 0, s>>>(g, h, lc, bc, eps, eps_mid, uniform, pal, code_mode, A0, code,
                                                             cpitch, offd[0], offd[1], offd[2], offd[3], offd[4], offd[5]);
 }
 

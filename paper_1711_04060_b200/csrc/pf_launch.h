@@ -59,7 +59,12 @@ void launch_k2_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv,
                    int parity);
 
 // ---- assembly (pf_assembly.cu) ----------------------------------------------------------------
-struct BcDev { int type[6]; double value[6]; };
+// Boundary data handed to the assembly and pointwise kernels: the six box faces, and Omega_f (PAPER.md:213,
+// 224-226; readings F1-F3): fixv[i] = prescribed potential of node i, NaN where the node is free; null = none.
+struct BcDev { int type[6]; double value[6]; const double* fixv; };
+__host__ __device__ inline bool is_fixed_node(const BcDev& bc, long long i) {
+    return bc.fixv != nullptr && bc.fixv[i] == bc.fixv[i];
+}
 
 struct Palette {
     int count;                         // distinct eps values found (PF_MAX_PALETTE+1 = overflow)
@@ -77,9 +82,11 @@ void launch_assemble_poisson(cudaStream_t s, const GridDims& g, double h, const 
                              double* const offd[6] /* entries null unless stored */);
 // PF1 operator eps(l_c^2 Lap - 1), sign flipped (Eq (12)), identity rows on the
 // box boundary and outside the solvent (Q15).
-void launch_assemble_pf1(cudaStream_t s, const GridDims& g, double h, double lc, const double* eps, double eps_mid,
-                         bool uniform, const Palette& pal, int code_mode, double* A0, void* code, int cpitch,
-                         double* const offd[6]);
+void launch_assemble_pf1(cudaStream_t s, const GridDims& g, double h, double lc, const BcDev& bc, const double* eps,
+                         double eps_mid, bool uniform, const Palette& pal, int code_mode, double* A0, void* code,
+                         int cpitch, double* const offd[6]);
+// fixv[idx[k]] = val[k] (fixv pre-filled with NaN).
+void launch_scatter_fixed(cudaStream_t s, const long long* idx_dev, const double* val_dev, int count, double* fixv);
 // Coefficient tables of the on-the-fly variant (host side; PF_CTAB doubles each).
 void build_ctab_poisson(const Palette& pal, double h, double* ctab_host);
 void build_ctab_pf1(const Palette& pal, double h, double lc, double* ctab_host);

@@ -51,7 +51,8 @@ k_fermi(GridDims g, BcDev bc, SpeciesDev sp, const double* __restrict__ eps, dou
     const int K = sp.K;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
-        const bool solvent = uniform || eps[i] > eps_mid;     // Q17; Eq (1) lives in Omega_s only
+        // Q17; Eq (1) lives in Omega_s only, and not in Omega_f (F3)
+        const bool solvent = (uniform || eps[i] > eps_mid) && !is_fixed_node(bc, i);
         double S = 0.0, rho = 0.0, sig = 0.0;
         double c[PF_MAX_SPECIES];
 #pragma unroll
@@ -102,7 +103,7 @@ k_fermi(GridDims g, BcDev bc, SpeciesDev sp, const double* __restrict__ eps, dou
                 if (k <= K) conc[(long long)k * g.n + i] = c[k];
         }
         if (b1) b1[i] = (!solvent || on_boundary(g, i)) ? 0.0 : -(sp.kappa * rho);
-        if (a2) a2[i] = dirichlet_face_pw(g, bc, i) >= 0 ? a0[i] : add(a0[i], sig);   // identity rows stay identity
+        if (a2) a2[i] = (dirichlet_face_pw(g, bc, i) >= 0 || is_fixed_node(bc, i)) ? a0[i] : add(a0[i], sig);   // identity rows stay identity
     }
 }
 
@@ -116,6 +117,7 @@ k_rhs_pf2(GridDims g, BcDev bc, const double* __restrict__ eps, double eps_mid, 
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
         const int f = dirichlet_face_pw(g, bc, i);
         if (f >= 0) { b[i] = bc.value[f]; continue; }
+        if (is_fixed_node(bc, i)) { b[i] = bc.fixv[i]; continue; }
         const double e = eps[i];
         const bool solvent = uniform || e > eps_mid;
         const double addv = solvent ? add(-mul(e, psi[i]), mul(sigma[i], phi0[i])) : 0.0;
@@ -148,7 +150,7 @@ k_diag_plus_sigma(GridDims g, BcDev bc, const double* __restrict__ a0, const dou
                   double* __restrict__ a2) {
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride)
-        a2[i] = dirichlet_face_pw(g, bc, i) >= 0 ? a0[i] : add(a0[i], sigma[i]);
+        a2[i] = (dirichlet_face_pw(g, bc, i) >= 0 || is_fixed_node(bc, i)) ? a0[i] : add(a0[i], sigma[i]);
 }
 
 void launch_diag_plus_sigma(cudaStream_t s, const GridDims& g, const BcDev& bc, const double* a0, const double* sigma,

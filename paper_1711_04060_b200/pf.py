@@ -29,7 +29,7 @@ STENCIL_AUTO, STENCIL_STORED, STENCIL_ONTHEFLY = 0, 1, 2
 KERNELS_AUTO, KERNELS_DIRECT, KERNELS_TILED = 0, 1, 2
 
 EXPORTS = [
-    "pf_grid_create", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
+    "pf_grid_create", "pf_grid_set_fixed_nodes", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
     "pf_solve_linear", "pf_solve_linear_host", "pf_solve_pf", "pf_fermi_pointwise", "pf_grid_history",
     "pf_grid_linear_iters", "pf_grid_increments", "pf_grid_fault_repeats", "pf_grid_laplace_iters", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_code_layout", "pf_grid_copy_array",
     "pf_grid_profile", "pf_launch_count", "pf_grid_destroy", "pf_last_error", "pf_version",
@@ -66,6 +66,7 @@ def load():
     L.pf_grid_create.argtypes = [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
                                  _vp, ctypes.POINTER(pf_charge), ctypes.c_int, ctypes.POINTER(pf_bc), _vp]
     L.pf_grid_create.restype = ctypes.c_int
+    L.pf_grid_set_fixed_nodes.argtypes = [_vp, ctypes.POINTER(ctypes.c_longlong), _dp, ctypes.c_int]
     L.pf_grid_workspace_bytes.argtypes = [_vp]
     L.pf_grid_workspace_bytes.restype = ctypes.c_size_t
     L.pf_grid_set_workspace.argtypes = [_vp, _vp, ctypes.c_size_t]
@@ -137,6 +138,16 @@ def pf_grid_create(nx: int, ny: int, nz: int, h: float, eps_map: torch.Tensor, c
                           ctypes.byref(bc), _vp(s))
     _check(None, rc)
     return handle
+
+
+def pf_grid_set_fixed_nodes(handle, idx, val) -> None:
+    """Omega_f: nodes (linear indices) whose potential is prescribed; call before pf_grid_set_workspace."""
+    idx = np.ascontiguousarray(np.asarray(idx, dtype=np.int64).reshape(-1))
+    val = _host_doubles(val)
+    if idx.size != val.size:
+        raise ValueError("idx and val need the same length")
+    _check(handle, load().pf_grid_set_fixed_nodes(handle, idx.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong)),
+                                                  val.ctypes.data_as(_dp), int(idx.size)))
 
 
 def pf_grid_workspace_bytes(handle) -> int:
@@ -282,7 +293,7 @@ class Grid:
     """Owns a pf_grid handle, the borrowed eps tensor and the torch-allocated workspace."""
 
     def __init__(self, nx, ny, nz, h, eps, charges, bc_type, bc_value, stencil=STENCIL_AUTO, kernels=KERNELS_AUTO,
-                 options: Optional[dict] = None, stream: Optional[torch.cuda.Stream] = None):
+                 options: Optional[dict] = None, stream: Optional[torch.cuda.Stream] = None, fixed_nodes=None):
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: paper_1711_04060_b200 has no CPU fallback")
         self.nx, self.ny, self.nz, self.h = nx, ny, nz, h
@@ -294,6 +305,8 @@ class Grid:
             pf_grid_set_option(self.handle, PF_OPT_KERNELS, kernels)
         for k, v in (options or {}).items():
             pf_grid_set_option(self.handle, k, v)
+        if fixed_nodes is not None:
+            pf_grid_set_fixed_nodes(self.handle, fixed_nodes[0], fixed_nodes[1])
         self.workspace = torch.empty(pf_grid_workspace_bytes(self.handle), dtype=torch.uint8, device="cuda")
         pf_grid_set_workspace(self.handle, self.workspace)
 
