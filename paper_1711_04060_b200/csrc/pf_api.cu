@@ -45,8 +45,9 @@ struct SmallSet {
     char* host = nullptr;           // pinned, 2 x 256 bytes
     cudaEvent_t ev[2] = {nullptr, nullptr};
 };
-constexpr size_t SS_SC = 0, SS_TICKET = 256, SS_DMAX = 512, SS_CTAB0 = 768, SS_CTAB1 = 1024,
-                 SS_PARTIAL = 1280, SS_CHARGES = SS_PARTIAL + sizeof(dd) * 3 * PF_MAX_PARTIAL_BLOCKS;
+constexpr size_t SS_SC = 0 /* two copies, 256 bytes each */, SS_FAULT = 512, SS_DMAX = 768, SS_CTAB0 = 1024,
+                 SS_CTAB1 = 1280, SS_PARTIAL = 1536,
+                 SS_CHARGES = SS_PARTIAL + sizeof(dd) * 3 * PF_PARTIAL_QUANTITIES * PF_MAX_PARTIAL_BLOCKS;
 static_assert(sizeof(Scalars) <= 256, "Scalars slots of the small set");
 std::mutex g_pool_mutex;
 std::vector<SmallSet*> g_pool;
@@ -107,7 +108,8 @@ struct pf_grid {
     int opt_stencil, opt_kernels, opt_check, opt_lin_maxit, opt_max_outer, opt_precond, opt_history;
     double opt_omega_pf, opt_lin_tol, opt_water;
     // small owned device buffers
-    Scalars* sc;
+    Scalars* sc[2];          // the two alternating device copies of the scalars
+    int flip;                // which one the next kernel reads
     ReduceBuf rb;
     double* ctab_poisson;    // PF_CTAB doubles each
     double* ctab_pf1;
@@ -219,7 +221,8 @@ Operator make_op(const pf_grid* g, int which /*0 poisson, 1 pf1, 2 poisson+sigma
 
 LaunchCtx make_ctx(const pf_grid* g) {
     LaunchCtx c;
-    c.stream = g->stream; c.g = g->g; c.sc = g->sc; c.rb = g->rb; c.sm_count = g->sm_count; c.pdl = true;
+    c.stream = g->stream; c.g = g->g; c.sc[0] = g->sc[0]; c.sc[1] = g->sc[1]; c.flip = const_cast<int*>(&g->flip);
+    c.rb = g->rb; c.sm_count = g->sm_count; c.pdl = true;
     return c;
 }
 
@@ -286,7 +289,9 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     std::memset(&init, 0, sizeof(init));
     init.tol = tol; init.maxit = maxit; init.hist_cap = g->hist ? g->hist_cap : 0; init.norm_mode = g->opt_norm;
     // pageable source: the runtime stages it before returning, so a stack object is safe
-    PF_CUDA(g, cudaMemcpyAsync(g->sc, &init, sizeof(init), cudaMemcpyHostToDevice, g->stream));
+    g->flip = 0;
+    PF_CUDA(g, cudaMemcpyAsync(g->sc[0], &init, sizeof(init), cudaMemcpyHostToDevice, g->stream));
+    PF_CUDA(g, cudaMemsetAsync(g->rb.fault, 0, sizeof(int), g->stream));
     KrylovVecs kv;
     kv.b = b; kv.x = x; kv.r = g->r; kv.rt = g->rt; kv.t = g->t; kv.hist = g->hist;
     kv.p_in = g->p0; kv.p_out = g->p1; kv.v_in = g->v0; kv.v_out = g->v1;
@@ -324,7 +329,9 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
             }
         }
         launched += todo;
-        PF_CUDA(g, cudaMemcpyAsync(g->sc_host[slot], g->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
+        launch_finalize(c, kv.hist);          // the scalar step the last kernel left pending
+        PF_CUDA(g, cudaMemcpyAsync(g->sc_host[slot], c.current_scalars(), sizeof(Scalars), cudaMemcpyDeviceToHost,
+                                   g->stream));
         PF_CUDA(g, cudaEventRecord(g->ev[slot], g->stream));
         pending[slot] = true;
         const int other = slot ^ 1;
@@ -365,7 +372,8 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     double true_rel = 0.0;
     if (true_relres_out && fin.bb != 0.0) {
         if (tiled) launch_residual_tma(c, op, kv, g->tma, 1); else launch_residual_direct(c, op, kv, 1);
-        PF_CUDA(g, cudaMemcpyAsync(g->sc_host[0], g->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
+        launch_finalize(c, nullptr);
+        PF_CUDA(g, cudaMemcpyAsync(g->sc_host[0], c.current_scalars(), sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
         PF_CUDA(g, cudaStreamSynchronize(g->stream));
         true_rel = g->opt_norm == 1 ? g->sc_host[0]->true_rmax : std::sqrt(g->sc_host[0]->true_rr) / fin.bnorm;
     }
@@ -462,7 +470,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->opt_charge_model = 0; g->charge_model = 0; g->phiL = g->phistar = g->A0_L = nullptr; g->code_L = nullptr;
     g->ctab_L = nullptr; g->laplace_iters = 0; g->fixv = nullptr; g->bc.fixv = nullptr;
     g->small = nullptr;
-    g->charges_dev = nullptr; g->sc = nullptr; g->rb.partial = nullptr; g->rb.ticket = nullptr;
+    g->charges_dev = nullptr; g->sc[0] = g->sc[1] = nullptr; g->flip = 0; g->rb.partial = nullptr; g->rb.fault = nullptr;
     g->ctab_poisson = g->ctab_pf1 = nullptr; g->dmax_bits = nullptr; g->tma = nullptr;
     g->code = g->code_pf1 = nullptr; g->code_mode = 0; g->cpitch = 0;
     g->sc_host[0] = g->sc_host[1] = nullptr; g->ev[0] = g->ev[1] = nullptr;
@@ -478,8 +486,9 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     PF_CREATE_CUDA(cudaGetDevice(&dev));
     PF_CREATE_CUDA(cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev));
     PF_CREATE_CUDA(small_set_acquire(dev, (size_t)ncharges, &g->small));
-    g->sc = reinterpret_cast<Scalars*>(g->small->dev + SS_SC);
-    g->rb.ticket = reinterpret_cast<unsigned int*>(g->small->dev + SS_TICKET);
+    g->sc[0] = reinterpret_cast<Scalars*>(g->small->dev + SS_SC);
+    g->sc[1] = reinterpret_cast<Scalars*>(g->small->dev + SS_SC + 256);
+    g->rb.fault = reinterpret_cast<int*>(g->small->dev + SS_FAULT);
     g->dmax_bits = reinterpret_cast<unsigned long long*>(g->small->dev + SS_DMAX);
     g->ctab_poisson = reinterpret_cast<double*>(g->small->dev + SS_CTAB0);
     g->ctab_pf1 = reinterpret_cast<double*>(g->small->dev + SS_CTAB1);
@@ -488,7 +497,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->sc_host[0] = reinterpret_cast<Scalars*>(g->small->host);
     g->sc_host[1] = reinterpret_cast<Scalars*>(g->small->host + 256);
     g->ev[0] = g->small->ev[0]; g->ev[1] = g->small->ev[1];
-    PF_CREATE_CUDA(cudaMemsetAsync(g->rb.ticket, 0, 256, g->stream));
+    PF_CREATE_CUDA(cudaMemsetAsync(g->rb.fault, 0, 256, g->stream));
     g->tma = tma_set_create();
     if (ncharges > 0) {
         g->charges_dev = reinterpret_cast<double*>(g->small->dev + SS_CHARGES);

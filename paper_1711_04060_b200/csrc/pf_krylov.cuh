@@ -92,4 +92,45 @@ __device__ __forceinline__ void finish_k3(Scalars* sc, double* hist, double rho_
     sc->first = 0;
 }
 
+// ---- start of every kernel of a solve (rows L7, L8) ---------------------------------------------
+// Copy the device scalars into the block's shared memory, combine the partial sums the previous kernel left
+// (pf_common.cuh), take the scalar step that was waiting for them, and note what THIS kernel (kind `kind`, a
+// PEND_* value; PEND_NONE for the one-block finalize kernel) will leave pending.  Every block does the same
+// arithmetic on the same data; block 0 stores the new state to sc_out.  Returns false when the solve is over
+// (the block returns at once).  All threads of the block must call; S and scratch are shared memory
+// (scratch: 3*32 dd).  hist: residual history or null.
+__device__ __forceinline__ bool begin_kernel(int kind, Scalars* S, const Scalars* sc_in, Scalars* sc_out,
+                                             const ReduceBuf& rb, double* hist, dd* scratch) {
+    constexpr int NWORDS = (int)(sizeof(Scalars) / sizeof(int));
+    // what usually precedes a kernel of this kind (k3 or the initial residual before k1, k1 before k2, k2 before
+    // k3): its partials are requested together with the scalars
+    const PartialPrefetch pre = prefetch_partials(
+        rb, kind == PEND_K1 ? PEND_K3 : (kind == PEND_K2 ? PEND_K1 : (kind == PEND_K3 ? PEND_K2 : PEND_NONE)));
+    if ((int)threadIdx.x < NWORDS)
+        reinterpret_cast<int*>(S)[threadIdx.x] = reinterpret_cast<const int*>(sc_in)[threadIdx.x];
+    __syncthreads();
+    const int pend = S->pending, nblk = S->pending_nblk;        // the same in every thread of every block
+    dd q[2] = {dd_zero(), dd_zero()};
+    double m = 0.0;
+    if (pend == PEND_K1) { dd q1[1]; combine_partials<1, false>(q1, m, nblk, scratch, rb, pend, pre); q[0] = q1[0]; }
+    else if (pend == PEND_K2) combine_partials<2, false>(q, m, nblk, scratch, rb, pend, pre);
+    else if (pend != PEND_NONE) combine_partials<2, true>(q, m, nblk, scratch, rb, pend, pre);
+    if (threadIdx.x == 0) {
+        const bool lead = linear_block_id() == 0;
+        double* h = lead ? hist : nullptr;                       // one writer for the history
+        if (pend == PEND_INIT) finish_init(S, h, dd_round(q[0]), dd_round(q[1]), m);
+        else if (pend == PEND_K1) finish_k1(S, dd_round(q[0]));
+        else if (pend == PEND_K2) finish_k2(S, dd_round(q[0]), dd_round(q[1]));
+        else if (pend == PEND_K3) finish_k3(S, h, dd_round(q[0]), dd_round(q[1]), m);
+        else if (pend == PEND_TRUE) { S->true_rr = dd_round(q[1]); S->true_rmax = m; }
+        const bool runs = kind == PEND_INIT || kind == PEND_TRUE || (kind != PEND_NONE && !S->done);
+        S->pending = runs ? kind : PEND_NONE;
+        S->pending_nblk = (int)linear_grid_size();
+        if (kind == PEND_NONE) S->fault = *rb.fault;             // finalize: what the host is about to read
+        if (lead) *sc_out = *S;
+    }
+    __syncthreads();
+    return S->pending != PEND_NONE;
+}
+
 }  // namespace pf

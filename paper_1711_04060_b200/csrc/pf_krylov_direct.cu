@@ -6,6 +6,9 @@
 // One BiCGSTAB iteration (Table 3) is three launches, one per reduction point:
 //   k1: steps 5-11   p = r + beta(p - omega v);  v = A M^-1 p;           reduces r~.v        (row L4)
 //   k2: steps 12-14  alpha; s = r - alpha v;  t = A M^-1 s;              reduces t.s, t.t    (row L5)
+// Each kernel starts by combining the partial sums its predecessor left and taking the scalar step that waited
+// for them (alpha in k2, omega in k3, the convergence test, rho and beta in k1; begin_kernel, pf_krylov.cuh),
+// and ends by writing its own partial sums.
 //   k3: steps 15-18  omega; y += alpha p + omega s (x = x0 + M^-1 y at the end, reading D3);
 //                    r = s - omega t; reduces r~.r (step 4 of the next iteration) and r.r     (row L6)
 #include "pf_krylov.cuh"
@@ -63,9 +66,11 @@ __device__ __forceinline__ void load_ctab(const Operator& op, double* ctab_s) {
 // MODE 0: r = b - A x, r~ = r, reduces b.b and r.r (step 2).  MODE 1: reduces ||b - A x||^2 only.
 template <int MODE>
 __global__ void __launch_bounds__(DIRECT_THREADS)
-k_residual(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
+k_residual(GridDims g, Operator op, KrylovVecs kv, const Scalars* sc_in, Scalars* sc_out, ReduceBuf rb) {
     __shared__ double ctab_s[PF_CTAB];
     __shared__ dd scratch[3 * 32];
+    __shared__ Scalars S;
+    begin_kernel(MODE == 0 ? PEND_INIT : PEND_TRUE, &S, sc_in, sc_out, rb, kv.hist, scratch);
     load_ctab(op, ctab_s);
     dd q[2] = {dd_zero(), dd_zero()};
     double rmax = 0.0;
@@ -88,21 +93,19 @@ k_residual(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
         dd_fma(q[1], ri, ri);
         rmax = fmax(rmax, fabs(ri));
     }
-    if (grid_reduce_dd_max<2>(q, rmax, scratch, rb)) {
-        if (MODE == 0) finish_init(sc, kv.hist, dd_round(q[0]), dd_round(q[1]), rmax);
-        else { sc->true_rr = dd_round(q[1]); sc->true_rmax = rmax; }
-    }
+    store_partials<2, true>(q, rmax, scratch, rb, MODE == 0 ? PEND_INIT : PEND_TRUE);
 }
 
 template <bool PRECOND>
 __global__ void __launch_bounds__(DIRECT_THREADS)
-k1_direct(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
-    if (sc->done) return;
+k1_direct(GridDims g, Operator op, KrylovVecs kv, const Scalars* sc_in, Scalars* sc_out, ReduceBuf rb) {
     __shared__ double ctab_s[PF_CTAB];
-    __shared__ dd scratch[32];
+    __shared__ dd scratch[3 * 32];
+    __shared__ Scalars S;
+    if (!begin_kernel(PEND_K1, &S, sc_in, sc_out, rb, kv.hist, scratch)) return;
     load_ctab(op, ctab_s);
-    const bool first = sc->first != 0;
-    const double beta = sc->beta, omega = sc->omega;
+    const bool first = S.first != 0;
+    const double beta = S.beta, omega = S.omega;
     dd q[1] = {dd_zero()};
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
@@ -123,17 +126,18 @@ k1_direct(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
         kv.v_out[i] = acc;
         dd_fma(q[0], kv.rt[i], acc);
     }
-    if (grid_reduce_dd<1>(q, scratch, rb)) finish_k1(sc, dd_round(q[0]));
+    store_partials<1, false>(q, 0.0, scratch, rb, PEND_K1);
 }
 
 template <bool PRECOND>
 __global__ void __launch_bounds__(DIRECT_THREADS)
-k2_direct(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
-    if (sc->done) return;
+k2_direct(GridDims g, Operator op, KrylovVecs kv, const Scalars* sc_in, Scalars* sc_out, ReduceBuf rb) {
     __shared__ double ctab_s[PF_CTAB];
-    __shared__ dd scratch[2 * 32];
+    __shared__ dd scratch[3 * 32];
+    __shared__ Scalars S;
+    if (!begin_kernel(PEND_K2, &S, sc_in, sc_out, rb, kv.hist, scratch)) return;
     load_ctab(op, ctab_s);
-    const double alpha = sc->alpha;
+    const double alpha = S.alpha;
     dd q[2] = {dd_zero(), dd_zero()};
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
@@ -154,7 +158,7 @@ k2_direct(GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
         dd_fma(q[0], acc, si);
         dd_fma(q[1], acc, acc);
     }
-    if (grid_reduce_dd<2>(q, scratch, rb)) finish_k2(sc, dd_round(q[0]), dd_round(q[1]));
+    store_partials<2, false>(q, 0.0, scratch, rb, PEND_K2);
 }
 
 }  // namespace
@@ -177,12 +181,13 @@ __device__ __forceinline__ void k3_point(const K3Elem& e, double alpha, double o
 
 template <bool VEC>
 __global__ void __launch_bounds__(256, 3)
-k3_update(long long n, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
+k3_update(long long n, KrylovVecs kv, const Scalars* sc_in, Scalars* sc_out, ReduceBuf rb) {
+    __shared__ dd scratch[3 * 32];
+    __shared__ Scalars S;
     pdl_launch_dependents();
     pdl_wait();
-    if (sc->done) return;
-    __shared__ dd scratch[3 * 32];
-    const double alpha = sc->alpha, omega = sc->omega;
+    if (!begin_kernel(PEND_K3, &S, sc_in, sc_out, rb, kv.hist, scratch)) return;
+    const double alpha = S.alpha, omega = S.omega;
     dd qa[2] = {dd_zero(), dd_zero()}, qb[2] = {dd_zero(), dd_zero()};
     double rmax = 0.0;
     const long long stride = (long long)gridDim.x * blockDim.x;
@@ -232,7 +237,15 @@ k3_update(long long n, KrylovVecs kv, Scalars* sc, ReduceBuf rb) {
     }
     dd_add(qa[0], qb[0]);
     dd_add(qa[1], qb[1]);
-    if (grid_reduce_dd_max<2>(qa, rmax, scratch, rb)) finish_k3(sc, kv.hist, dd_round(qa[0]), dd_round(qa[1]), rmax);
+    store_partials<2, true>(qa, rmax, scratch, rb, PEND_K3);
+}
+
+// One block: take the scalar step that is still pending (so that the host reads a finished state), in place.
+__global__ void __launch_bounds__(256)
+k_finalize(Scalars* sc, ReduceBuf rb, double* hist) {
+    __shared__ dd scratch[3 * 32];
+    __shared__ Scalars S;
+    begin_kernel(PEND_NONE, &S, sc, sc, rb, hist, scratch);
 }
 
 // x = x + M^-1 y (reading D3).  y is exactly 0 on identity rows, so Dirichlet values of x are kept.
@@ -251,24 +264,32 @@ static int direct_blocks(long long n, int sm_count) {
 }
 
 void launch_residual_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, int mode) {
+    const Scalars* sc_in; Scalars* sc_out;
+    c.next_scalars(sc_in, sc_out);
     const int nb = direct_blocks(c.g.n, c.sm_count);
-    if (mode == 0) { ++g_launch_count; k_residual<0><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb); }
-    else           { ++g_launch_count; k_residual<1><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb); }
+    if (mode == 0) { ++g_launch_count; k_residual<0><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, sc_in, sc_out, c.rb); }
+    else           { ++g_launch_count; k_residual<1><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, sc_in, sc_out, c.rb); }
 }
 
 void launch_k1_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond) {
+    const Scalars* sc_in; Scalars* sc_out;
+    c.next_scalars(sc_in, sc_out);
     const int nb = direct_blocks(c.g.n, c.sm_count);
-    if (precond) { ++g_launch_count; k1_direct<true><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb); }
-    else         { ++g_launch_count; k1_direct<false><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb); }
+    if (precond) { ++g_launch_count; k1_direct<true><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, sc_in, sc_out, c.rb); }
+    else         { ++g_launch_count; k1_direct<false><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, sc_in, sc_out, c.rb); }
 }
 
 void launch_k2_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond) {
+    const Scalars* sc_in; Scalars* sc_out;
+    c.next_scalars(sc_in, sc_out);
     const int nb = direct_blocks(c.g.n, c.sm_count);
-    if (precond) { ++g_launch_count; k2_direct<true><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb); }
-    else         { ++g_launch_count; k2_direct<false><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, c.sc, c.rb); }
+    if (precond) { ++g_launch_count; k2_direct<true><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, sc_in, sc_out, c.rb); }
+    else         { ++g_launch_count; k2_direct<false><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, sc_in, sc_out, c.rb); }
 }
 
 void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond) {
+    const Scalars* sc_in; Scalars* sc_out;
+    c.next_scalars(sc_in, sc_out);
     (void)op; (void)precond;
     // 3 blocks of 256 threads per SM, each thread two 16-byte groups in flight per vector
     long long want = (c.g.n / 2 + 255) / 256;
@@ -278,8 +299,13 @@ void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, boo
     const bool vec = (((uintptr_t)kv.y | (uintptr_t)kv.r | (uintptr_t)kv.v_out | (uintptr_t)kv.p_out | (uintptr_t)kv.t |
                        (uintptr_t)kv.rt) & 15u) == 0;
     ++g_launch_count;
-    if (vec) launch_pdl(c.pdl, k3_update<true>, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, c.sc, c.rb);
-    else     launch_pdl(c.pdl, k3_update<false>, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, c.sc, c.rb);
+    if (vec) launch_pdl(c.pdl, k3_update<true>, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, sc_in, sc_out, c.rb);
+    else     launch_pdl(c.pdl, k3_update<false>, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, sc_in, sc_out, c.rb);
+}
+
+void launch_finalize(const LaunchCtx& c, double* hist) {
+    ++g_launch_count;
+    k_finalize<<<1, 256, 0, c.stream>>>(c.current_scalars(), c.rb, hist);
 }
 
 void launch_finish_x(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv) {

@@ -1,8 +1,10 @@
 // pf_krylov_tma.cu -- the fused stencil kernels of the BiCGSTAB iteration for B200: planes staged in
 // shared memory by TMA, z marched in registers, warp-specialised.
 //
-// Work decomposition.  The xy plane is cut into tiles of TX x TY = 64 x 16 nodes; a block marches its tile
-// along z over a chunk of planes.  Roles of its 19 warps:
+// Work decomposition.  The xy plane is cut into tiles of TX x TY = 64 x 16 nodes and z into chunks; a work item
+// is one tile marched along z over one chunk.  min(#SMs, #items) persistent blocks take the items round-robin in
+// the order x tile, y tile, chunk (neighbouring tiles run at the same time and share halo rows in L2), with the
+// stage ring running on from one item to the next.  Roles of a block's 19 warps:
 //   producer (1 warp, one lane)  keeps a ring of S stages filled: per plane one 3-D tensor-map copy
 //       (cp.async.bulk.tensor, completion on a "full" mbarrier) per operand, of the tile PLUS its halo ring --
 //       box (TX+4) x (TY+2) so that every thread's pair of nodes is 16-byte aligned in shared memory.  Nodes
@@ -24,6 +26,10 @@
 // three-way unrolled loop).  Per plane: wait for the stage, form u(z+1), publish it and release the stage,
 // difference plane z.  There is no block-wide barrier in the loop: a "ready" mbarrier per u buffer (one
 // arrival per consumer warp) orders the writers and readers of the buffers, so warps drift by up to a plane.
+//
+// Reductions: a block ends by writing its double-double partial sums; the next kernel of the stream combines
+// them in every block and takes the scalar step (begin_kernel, pf_krylov.cuh), while its producer warp has
+// already requested the first stages.
 //
 // Arithmetic is the same statement for statement as the direct kernels (pf_krylov_direct.cu): both
 // families give bit-identical vectors.
@@ -77,7 +83,8 @@ struct Layout {
     static constexpr int CTAB_OFF = U_OFF + NU * FIELD_BYTES;
     static constexpr int SCRATCH_OFF = CTAB_OFF + PF_CTAB * 8;
     static constexpr int BAR_OFF = SCRATCH_OFF + 3 * 32 * (int)sizeof(dd);
-    static constexpr int TOTAL = BAR_OFF + 16 * T::STAGES + 8 * NU;  // full[S], empty[S], ready[NU]
+    static constexpr int SC_OFF = ((BAR_OFF + 16 * T::STAGES + 8 * NU + 15) / 16) * 16;   // after full[S], empty[S], ready[NU]
+    static constexpr int TOTAL = SC_OFF + 256;                       // the block's copy of the scalars
     static_assert(CTAB_OFF % 128 == 0, "ctab_at ORs table offsets into the table address");
     static constexpr unsigned TX_BYTES = (unsigned)(T::NF * BX * BY * 8 + (T::OWN ? OWN_BYTES : 0) + CODE_BYTES);
 };
@@ -153,27 +160,32 @@ __device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
 
 template <int MODE, bool PRECOND, bool STORED, bool CODE32>
 __global__ void __launch_bounds__(NT, 1)
-k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv, Scalars* sc, ReduceBuf rb, int zchunk) {
+k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv, const Scalars* sc_in, Scalars* sc_out, ReduceBuf rb,
+      int zchunk, int ntx, int ntiles, int nitems) {
     using L = Layout<MODE, STORED, CODE32>;
     using T = ModeTraits<MODE>;
-    constexpr int S = T::STAGES;
+    constexpr int NS = T::STAGES;
     constexpr int NF = T::NF;
     pdl_launch_dependents();
     extern __shared__ __align__(128) unsigned char smem[];
     double* ctab_s = reinterpret_cast<double*>(smem + L::CTAB_OFF);
     dd* scratch = reinterpret_cast<dd*>(smem + L::SCRATCH_OFF);
     unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + L::BAR_OFF);
-    unsigned long long* empty = full + S;
-    unsigned long long* ready = empty + S;     // ready[b]: all 18 consumer warps have written their part of u buffer b
+    unsigned long long* empty = full + NS;
+    unsigned long long* ready = empty + NS;    // ready[b]: all 18 consumer warps have written their part of u buffer b
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
-    const int z0 = blockIdx.z * zchunk, z1 = min(z0 + zchunk, g.nz);
-    const int nq = z1 - z0 + 2;            // plane q of this block's load sequence is z0 - 1 + q
+    // Persistent blocks: work item i = (tile i % ntiles, z chunk i / ntiles), x tiles fastest, so that the
+    // blocks running at any moment work on neighbouring tiles of the same chunk and share their halo rows in
+    // L2.  Block b takes items b, b + gridDim.x, ...; the stage and u-buffer rings run on across items, so
+    // the producer already loads the next item while the consumers finish the current one, and a launch leaves
+    // at most one set of partial sums per SM for the next kernel to combine.
+    int sb = 0, ub = 0;                    // stages loaded / u planes published in earlier items
+    Scalars* S = reinterpret_cast<Scalars*>(smem + L::SC_OFF);
 
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW_CONSUMER); }
+        for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW_CONSUMER); }
 #pragma unroll
         for (int b = 0; b < NU; ++b) mbar_init(&ready[b], NW_CONSUMER);
         fence_proxy_async();
@@ -182,32 +194,60 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     const unsigned ctab_addr = smem_u32(ctab_s);           // 128-byte aligned: CTAB_OFF and the smem base are
     __syncthreads();
     pdl_wait();                                            // everything above is independent of the previous kernel
-    if (MODE >= MODE_K1 && sc->done) return;
+    constexpr int KIND = MODE == MODE_K1 ? PEND_K1 : (MODE == MODE_K2 ? PEND_K2 : (MODE == MODE_R0 ? PEND_INIT : PEND_TRUE));
+    // plane k of the load sequence of work item `item` into stage (seq % NS); the producer lane only
+    auto issue_plane = [&](int item, int k, int seq) {
+        const int tile = item % ntiles;
+        const int px = (tile % ntx) * TX, py = (tile / ntx) * TY, pz = (item / ntiles) * zchunk - 1 + k;
+        const int s = seq % NS;
+        unsigned char* st = smem + s * L::STAGE_BYTES;
+        mbar_expect_tx(&full[s], L::TX_BYTES);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) tma_load_3d(st + f * FIELD_BYTES, &tm.f[f], &full[s], px - 2, py - 1, pz);
+        if (T::OWN) tma_load_3d(st + L::OWN_OFF, &tm.own, &full[s], px, py, pz);
+        if (!STORED) tma_load_3d(st + L::CODE_OFF, &tm.code, &full[s], px, py, pz);
+    };
+    // The first stages do not depend on the scalars: they are requested before the block combines the previous
+    // kernel's partial sums, so the loads fly while the scalar step is taken.
+    int pre_issued = 0;
+    if (tid == NT_CONSUMER && (int)blockIdx.x < nitems) {
+        const int z0f = ((int)blockIdx.x / ntiles) * zchunk;
+        const int nqf = min(z0f + zchunk, g.nz) - z0f + 2;
+        for (; pre_issued < NS && pre_issued < nqf; ++pre_issued) issue_plane(blockIdx.x, pre_issued, pre_issued);
+    }
+    if (!begin_kernel(KIND, S, sc_in, sc_out, rb, kv.hist, scratch)) {
+        // the solve is over: let the requested stages land before the block's shared memory is released
+        for (int k = 0; k < pre_issued; ++k) while (!mbar_try_wait(&full[k], 0u)) {}
+        return;
+    }
 
     dd q[2] = {dd_zero(), dd_zero()};
     double rmax = 0.0;                     // residual modes: ||b - A x||_inf
     unsigned fault = 0u;
 
+    for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+    const int tile = item % ntiles;
+    const int x0 = (tile % ntx) * TX, y0 = (tile / ntx) * TY;
+    const int z0 = (item / ntiles) * zchunk, z1 = min(z0 + zchunk, g.nz);
+    const int nq = z1 - z0 + 2;            // plane k of this item's load sequence is z0 - 1 + k
+
     if (wid == NW_CONSUMER) {
         // ---- producer warp: one lane keeps the ring of stages filled ----------------------------
         if (lane == 0) {
-            for (int k = 0; k < nq; ++k) {
-                const int s = k % S;
-                if (k >= S) { const unsigned par = (unsigned)(k / S - 1) & 1u; while (!mbar_try_wait(&empty[s], par)) {} }
-                unsigned char* st = smem + s * L::STAGE_BYTES;
-                const int z = z0 - 1 + k;
-                mbar_expect_tx(&full[s], L::TX_BYTES);
-#pragma unroll
-                for (int f = 0; f < NF; ++f) tma_load_3d(st + f * FIELD_BYTES, &tm.f[f], &full[s], x0 - 2, y0 - 1, z);
-                if (T::OWN) tma_load_3d(st + L::OWN_OFF, &tm.own, &full[s], x0, y0, z);
-                if (!STORED) tma_load_3d(st + L::CODE_OFF, &tm.code, &full[s], x0, y0, z);
+            for (int k = (item == (int)blockIdx.x ? pre_issued : 0); k < nq; ++k) {
+                const int s = (sb + k) % NS;
+                if (sb + k >= NS) {
+                    const unsigned par = (unsigned)((sb + k) / NS - 1) & 1u;
+                    while (!mbar_try_wait(&empty[s], par)) {}
+                }
+                issue_plane(item, k, sb + k);
             }
         }
         __syncwarp();
     } else {
         bool first = false; double c1 = 0.0, c2 = 0.0;
-        if (MODE == MODE_K1) { first = sc->first != 0; c1 = sc->beta; c2 = sc->omega; }
-        else if (MODE == MODE_K2) { c1 = sc->alpha; }
+        if (MODE == MODE_K1) { first = S->first != 0; c1 = S->beta; c2 = S->omega; }
+        else if (MODE == MODE_K2) { c1 = S->alpha; }
         const bool is_main = wid < TY;
         // main thread: nodes (x, y) and (x+1, y) of box row wid+1; nx is even so both are inside or both outside.
         // halo warp TY: box row 0 (pairs) and box column 1 (lanes 0..15); halo warp TY+1: row BY-1 and column BX-2.
@@ -243,29 +283,29 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             a[0] = fa.x; a[1] = fa.y;
         };
         auto wait_full = [&](int k) -> const unsigned char* {
-            const int s = k % S;
-            const unsigned par = (unsigned)(k / S) & 1u;
+            const int s = (sb + k) % NS;
+            const unsigned par = (unsigned)((sb + k) / NS) & 1u;
             while (!mbar_try_wait(&full[s], par)) {}
             return smem + s * L::STAGE_BYTES;
         };
         auto release = [&](int k) {                                     // this warp is done with the stage of plane k
             __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[k % S]);
+            if (lane == 0) mbar_arrive(&empty[(sb + k) % NS]);
         };
         // u of plane k (k >= 1) lives in shared buffer (k-1) % NU.  publish: this warp's part is written (and its
         // stage released); wait_ready: every consumer warp has published plane k.  No block-wide barrier: a warp
         // that waits for plane k before it overwrites plane k-2's buffer with plane k+1 cannot race a reader
         // (every warp that published plane k has finished differencing plane k-2).
         auto u_buf = [&](int k) -> double* {
-            return reinterpret_cast<double*>(smem + L::U_OFF + ((k - 1) % NU) * FIELD_BYTES);
+            return reinterpret_cast<double*>(smem + L::U_OFF + ((ub + k - 1) % NU) * FIELD_BYTES);
         };
         auto publish = [&](int k) {
             __syncwarp();
-            if (lane == 0) { mbar_arrive(&ready[(k - 1) % NU]); mbar_arrive(&empty[k % S]); }
+            if (lane == 0) { mbar_arrive(&ready[(ub + k - 1) % NU]); mbar_arrive(&empty[(sb + k) % NS]); }
         };
         auto wait_ready = [&](int k) {
-            const unsigned par = (unsigned)((k - 1) / NU) & 1u;
-            while (!mbar_try_wait(&ready[(k - 1) % NU], par)) {}
+            const unsigned par = (unsigned)((ub + k - 1) / NU) & 1u;
+            while (!mbar_try_wait(&ready[(ub + k - 1) % NU], par)) {}
         };
 
         if (!is_main) {
@@ -280,7 +320,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             }
             wait_full(0); release(0);                                   // plane z0-1 has no xy neighbours to serve
             for (int k = 1; k < nq; ++k) {
-                if (k >= 2) wait_ready(k - 1);                           // plane k-3 (same buffer) is no longer read
+                if (ub + k >= 2) wait_ready(k - 1);                      // the plane written 3 publishes ago is no longer read
                 const unsigned char* st = wait_full(k);
                 const int z = z0 - 1 + k;
                 const bool zin = z >= 0 && z < g.nz;
@@ -401,6 +441,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             s0.w = s1.w = s2.w = make_double2(0, 0);
             s0.k0 = s0.k1 = s1.k0 = s1.k1 = s2.k0 = s2.k1 = 0u;
             load_slot(0, s0, false); release(0);   // plane z0-1: registers only
+            if (ub >= 1) wait_ready(0);            // last plane of the previous item: its buffer-mates are free
             load_slot(1, s1, true);  publish(1);   // plane z0
             for (int z = z0; z < z1; z += 3) {     // slots rotate by renaming, not by moving registers
                 step(z, s0, s1, s2);
@@ -418,16 +459,19 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
         }
     }
 
-    if (fault) sc->fault = 1;              // the host repeats the solve with the __ddiv_rn kernels
+    sb += nq; ub += nq - 1;
+    }
+
+    if (fault) *rb.fault = 1;              // the host repeats the solve with the __ddiv_rn kernels
+    // this block's partial sums; the next kernel of the stream combines them (pf_common.cuh)
     if (MODE == MODE_K1) {
         dd_add(q[0], q[1]);                // two chains for instruction-level parallelism, one quantity
         dd q1[1] = {q[0]};
-        if (grid_reduce_dd<1>(q1, scratch, rb)) finish_k1(sc, dd_round(q1[0]));
+        store_partials<1, false>(q1, 0.0, scratch, rb, PEND_K1);
     } else if (MODE == MODE_K2) {
-        if (grid_reduce_dd<2>(q, scratch, rb)) finish_k2(sc, dd_round(q[0]), dd_round(q[1]));
-    } else if (grid_reduce_dd_max<2>(q, rmax, scratch, rb)) {
-        if (MODE == MODE_R0) finish_init(sc, kv.hist, dd_round(q[0]), dd_round(q[1]), rmax);
-        else { sc->true_rr = dd_round(q[1]); sc->true_rmax = rmax; }
+        store_partials<2, false>(q, 0.0, scratch, rb, PEND_K2);
+    } else {
+        store_partials<2, true>(q, rmax, scratch, rb, KIND);
     }
 }
 
@@ -494,6 +538,11 @@ bool own_map(CUtensorMap* m, const double* base, const GridDims& g) {
 
 template <int MODE, bool PRECOND, bool STORED, bool CODE32>
 void launch_inst(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaArgs& tm, dim3 grid, int depth) {
+    // grid = (x tiles, y tiles, z chunks) of work items; launched as min(#SMs, #items) persistent blocks
+    const int ntx = (int)grid.x, ntiles = (int)(grid.x * grid.y), nitems = ntiles * (int)grid.z;
+    const int blocks = std::min(c.sm_count, nitems);
+    const Scalars* sc_in; Scalars* sc_out;
+    c.next_scalars(sc_in, sc_out);
     using L = Layout<MODE, STORED, CODE32>;
     static bool configured = false;
     auto kern = k_tma<MODE, PRECOND, STORED, CODE32>;
@@ -502,7 +551,8 @@ void launch_inst(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, c
         configured = true;
     }
     ++g_launch_count;
-    launch_pdl(c.pdl, kern, grid, dim3(NT), (size_t)L::TOTAL, c.stream, tm, c.g, op, kv, c.sc, c.rb, depth);
+    launch_pdl(c.pdl, kern, dim3(blocks), dim3(NT), (size_t)L::TOTAL, c.stream, tm, c.g, op, kv, sc_in, sc_out, c.rb, depth,
+               ntx, ntiles, nitems);
 }
 
 template <int MODE>

@@ -27,10 +27,14 @@ inline cudaError_t launch_pdl(bool pdl, void (*kern)(KArgs...), dim3 grid, dim3 
 struct LaunchCtx {
     cudaStream_t stream;
     GridDims g;
-    Scalars* sc;      // device
+    Scalars* sc[2];   // device: the two alternating copies of the scalars (pf_common.cuh)
+    int* flip;        // host: index of the copy the next kernel reads
     ReduceBuf rb;     // device
     int sm_count;
     bool pdl;         // programmatic dependent launch allowed
+    // the next kernel reads sc[*flip] and its block 0 writes sc[*flip ^ 1]
+    void next_scalars(const Scalars*& in, Scalars*& out) const { in = sc[*flip]; out = sc[*flip ^ 1]; *flip ^= 1; }
+    Scalars* current_scalars() const { return sc[*flip]; }
 };
 
 // ---- Krylov kernels -----------------------------------------------------------------------
@@ -39,6 +43,8 @@ void launch_residual_direct(const LaunchCtx& c, const Operator& op, const Krylov
 void launch_k1_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
 void launch_k2_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
 void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
+// One-block kernel that takes the pending scalar step in place, before the host reads the scalars.
+void launch_finalize(const LaunchCtx& c, double* hist);
 // x += M^-1 y at the end of a preconditioned solve (reading D3).
 void launch_finish_x(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv);
 
