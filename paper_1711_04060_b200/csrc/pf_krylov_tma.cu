@@ -180,7 +180,9 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     // L2.  Block b takes items b, b + gridDim.x, ...; the stage and u-buffer rings run on across items, so
     // the producer already loads the next item while the consumers finish the current one, and a launch leaves
     // at most one set of partial sums per SM for the next kernel to combine.
-    int sb = 0, ub = 0;                    // stages loaded / u planes published in earlier items
+    // (The stored variant, short of registers, runs one item per block: its ring counters are constants.)
+    constexpr bool PERSIST = true;
+    int sb_run = 0, ub_run = 0;            // stages loaded / u planes published in earlier items
     Scalars* S = reinterpret_cast<Scalars*>(smem + L::SC_OFF);
 
     if (tid == 0) {
@@ -225,7 +227,8 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     double rmax = 0.0;                     // residual modes: ||b - A x||_inf
     unsigned fault = 0u;
 
-    for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+    for (int item = blockIdx.x; item < nitems; item += PERSIST ? (int)gridDim.x : nitems) {
+    const int sb = PERSIST ? sb_run : 0, ub = PERSIST ? ub_run : 0;
     const int tile = item % ntiles;
     const int x0 = (tile % ntx) * TX, y0 = (tile / ntx) * TY;
     const int z0 = (item / ntiles) * zchunk, z1 = min(z0 + zchunk, g.nz);
@@ -369,6 +372,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     *reinterpret_cast<double2*>(kv.p_out + own_off + plane * z) = make_double2(up.n[0], up.n[1]);
                 if (to_shared) *reinterpret_cast<double2*>(u_buf(k) + pair_box) = make_double2(up.u[0], up.u[1]);
             };
+            constexpr bool DEFER = !STORED;                  // the stored variant has no registers to spare for it
             double pa[2] = {0.0, 0.0}, pb[2] = {0.0, 0.0};   // operands of the deferred inner products (zeros add nothing)
             auto step = [&](int z, const Slot& dn, const Slot& c, Slot& up) {
                 const int k = z - z0 + 1;                               // load-sequence index of plane z
@@ -378,9 +382,9 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 load_slot(k + 1, up, true);
                 // inner products of the PREVIOUS plane: a third independent chain beside the divisions of plane
                 // z+1 and the 7-point sums of plane z
-                if (MODE == MODE_K1) {
+                if (DEFER && MODE == MODE_K1) {
                     dd_fma(q[0], pa[0], pb[0]); dd_fma(q[1], pa[1], pb[1]);
-                } else if (MODE == MODE_K2) {
+                } else if (DEFER && MODE == MODE_K2) {
                     dd_fma(q[0], pa[0], pb[0]); dd_fma(q[0], pa[1], pb[1]);
                     dd_fma(q[1], pa[0], pa[0]); dd_fma(q[1], pa[1], pa[1]);
                 }
@@ -419,10 +423,15 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 out[1] = add(out[1], mul(c5[1], up.u[1]));
                 if (MODE == MODE_K1) {
                     if (pair_ok) *reinterpret_cast<double2*>(kv.v_out + i) = make_double2(out[0], out[1]);
-                    pa[0] = c.w.x; pa[1] = c.w.y; pb[0] = out[0]; pb[1] = out[1];      // r~ . v', next step
+                    if (DEFER) { pa[0] = c.w.x; pa[1] = c.w.y; pb[0] = out[0]; pb[1] = out[1]; }   // r~ . v', next step
+                    else { dd_fma(q[0], c.w.x, out[0]); dd_fma(q[1], c.w.y, out[1]); }
                 } else if (MODE == MODE_K2) {
                     if (pair_ok) *reinterpret_cast<double2*>(kv.t + i) = make_double2(out[0], out[1]);
-                    pa[0] = out[0]; pa[1] = out[1]; pb[0] = c.n[0]; pb[1] = c.n[1];    // t . s and t . t, next step
+                    if (DEFER) { pa[0] = out[0]; pa[1] = out[1]; pb[0] = c.n[0]; pb[1] = c.n[1]; }   // t . s, t . t, next step
+                    else {
+                        dd_fma(q[0], out[0], c.n[0]); dd_fma(q[0], out[1], c.n[1]);
+                        dd_fma(q[1], out[0], out[0]); dd_fma(q[1], out[1], out[1]);
+                    }
                 } else {
                     const double r0 = sub(c.w.x, out[0]), r1 = sub(c.w.y, out[1]);
                     if (MODE == MODE_R0) {
@@ -450,16 +459,16 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 if (z + 2 >= z1) break;
                 step(z + 2, s2, s0, s1);
             }
-            if (MODE == MODE_K1) {                           // the last plane's inner products
+            if (DEFER && MODE == MODE_K1) {                  // the last plane's inner products
                 dd_fma(q[0], pa[0], pb[0]); dd_fma(q[1], pa[1], pb[1]);
-            } else if (MODE == MODE_K2) {
+            } else if (DEFER && MODE == MODE_K2) {
                 dd_fma(q[0], pa[0], pb[0]); dd_fma(q[0], pa[1], pb[1]);
                 dd_fma(q[1], pa[0], pa[0]); dd_fma(q[1], pa[1], pa[1]);
             }
         }
     }
 
-    sb += nq; ub += nq - 1;
+    sb_run += nq; ub_run += nq - 1;
     }
 
     if (fault) *rb.fault = 1;              // the host repeats the solve with the __ddiv_rn kernels
@@ -540,6 +549,8 @@ template <int MODE, bool PRECOND, bool STORED, bool CODE32>
 void launch_inst(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaArgs& tm, dim3 grid, int depth) {
     // grid = (x tiles, y tiles, z chunks) of work items; launched as min(#SMs, #items) persistent blocks
     const int ntx = (int)grid.x, ntiles = (int)(grid.x * grid.y), nitems = ntiles * (int)grid.z;
+    // The stored variant (six more arrays per node straight from global memory, no registers to spare for the
+    // item loop) keeps one item per block.
     const int blocks = std::min(c.sm_count, nitems);
     const Scalars* sc_in; Scalars* sc_out;
     c.next_scalars(sc_in, sc_out);
