@@ -307,14 +307,16 @@ def run_b200(args):
         dom = max(kernels_rep, key=lambda k: kernels_rep[k]["avg_ms"] * kernels_rep[k]["launches"])
         iter_ms = sum(kernels_rep[k]["avg_ms"] for k in kernels_rep)
         iter_bytes = sum(bpu.values()) * n
+        # DRAM bytes per launch from the committed ncu --set full capture (profiles/traffic.csv: stencil,n,kernel,bytes)
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(tpath):
-            try:
-                with open(tpath) as f:
-                    traffic = json.load(f).get(f"{args.stencil}_{args.n}", {}).get(dom)
-            except Exception:
-                traffic = None
+        try:
+            with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+                for row in f:
+                    c = [x.strip() for x in row.split(",")]
+                    if len(c) >= 4 and c[0] == args.stencil and c[1] == str(args.n) and c[2] == dom:
+                        traffic = int(c[3])
+        except (OSError, ValueError):
+            traffic = None
         roofline = {"bound": "hbm", "kernel": {"k1": "k1 (p-update + matvec + r~.v)", "k2": "k2 (s-update + matvec + t.s,t.t)",
                                                 "k3": "k3 (x,r update + r~.r, r.r)"}[dom],
                     "achieved": kernels_rep[dom]["gbs"], "peak": peak, "unit": "GB/s",
