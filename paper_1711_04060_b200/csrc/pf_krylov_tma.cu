@@ -81,7 +81,11 @@ struct Layout {
     static constexpr int CODE_OFF = OWN_OFF + (T::OWN ? OWN_BYTES : 0);
     static constexpr int U_OFF = T::STAGES * STAGE_BYTES;
     static constexpr int CTAB_OFF = U_OFF + NU * FIELD_BYTES;
-    static constexpr int SCRATCH_OFF = CTAB_OFF + PF_CTAB * 8;
+    // 2-bit codes: the coefficients of three faces at once from a 64-entry table of 32-byte entries, placed at
+    // the first 2048-byte boundary inside a 4 KB region (its address is ORed with the entry offset)
+    static constexpr int T3_OFF = CTAB_OFF + PF_CTAB * 8;
+    static constexpr int T3_BYTES = (STORED || CODE32) ? 0 : 4096;
+    static constexpr int SCRATCH_OFF = T3_OFF + T3_BYTES;
     static constexpr int BAR_OFF = SCRATCH_OFF + 3 * 32 * (int)sizeof(dd);
     static constexpr int SC_OFF = ((BAR_OFF + 16 * T::STAGES + 8 * NU + 15) / 16) * 16;   // after full[S], empty[S], ready[NU]
     static constexpr int TOTAL = SC_OFF + 256;                       // the block's copy of the scalars
@@ -146,6 +150,16 @@ __device__ __forceinline__ double ctab_at(unsigned ctab_addr, unsigned w0, unsig
     return c;
 }
 
+// 2-bit codes: the coefficients of faces 3g+1 .. 3g+3 (g = 0, 1) of node e of the thread's code word, from the
+// table whose entry i holds ctab[i & 3], ctab[(i >> 2) & 3], ctab[(i >> 4) & 3]: one shift, one logic operation
+// (mask the six code bits, scaled by 32, and OR in the 2048-byte aligned table address), two loads.
+__device__ __forceinline__ void ctab3_at(unsigned t3_addr, unsigned w0, int e, int g, double (&c)[3]) {
+    const int sh = 16 * e + 6 * g - 5;
+    const unsigned off = ((sh >= 0 ? (w0 >> sh) : (w0 << -sh)) & 0x7e0u) | t3_addr;
+    asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(c[0]), "=d"(c[1]) : "r"(off));
+    asm("ld.shared.f64 %0, [%1+16];" : "=d"(c[2]) : "r"(off));
+}
+
 // Registers of one plane of a main thread: u at its two nodes, the numerators (p' or s), the diagonal,
 // the own-only operand (r~ or b) and the stencil code word(s).
 struct Slot {
@@ -193,6 +207,14 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
         fence_proxy_async();
     }
     if (!STORED && tid < PF_CTAB) ctab_s[tid] = op.ctab[tid];
+    unsigned t3_addr = 0u;
+    if (!STORED && !CODE32) {
+        unsigned char* region = smem + L::T3_OFF;
+        const unsigned a = smem_u32(region);
+        t3_addr = (a + 2047u) & ~2047u;
+        double* T3 = reinterpret_cast<double*>(region + (t3_addr - a));
+        if (tid < 256) T3[tid] = (tid & 3) < 3 ? op.ctab[((tid >> 2) >> (2 * (tid & 3))) & 3] : 0.0;
+    }
     const unsigned ctab_addr = smem_u32(ctab_s);           // 128-byte aligned: CTAB_OFF and the smem base are
     __syncthreads();
     pdl_wait();                                            // everything above is independent of the previous kernel
@@ -404,10 +426,14 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     if (STORED) {
 #pragma unroll
                         for (int d = 0; d < 6; ++d) cc[d] = e == 0 ? cf[d].x : cf[d].y;
-                    } else {
+                    } else if (CODE32) {
 #pragma unroll
                         for (int d = 0; d < 6; ++d)
                             cc[d] = ctab_at<CODE32>(ctab_addr, c.k0, c.k1, e, d);
+                    } else {
+                        double c3[3];
+                        ctab3_at(t3_addr, c.k0, e, 0, c3); cc[0] = c3[0]; cc[1] = c3[1]; cc[2] = c3[2];
+                        ctab3_at(t3_addr, c.k0, e, 1, c3); cc[3] = c3[0]; cc[4] = c3[1]; cc[5] = c3[2];
                     }
                     double acc = mul(c.a[e], c.u[e]);
                     acc = add(acc, mul(cc[0], e == 0 ? c.u[1] : ue));
