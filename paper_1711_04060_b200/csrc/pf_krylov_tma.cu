@@ -195,7 +195,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     // the producer already loads the next item while the consumers finish the current one, and a launch leaves
     // at most one set of partial sums per SM for the next kernel to combine.
     // (The stored variant, short of registers, runs one item per block: its ring counters are constants.)
-    constexpr bool PERSIST = true;
+    constexpr bool PERSIST = !STORED;
     int sb_run = 0, ub_run = 0;            // stages loaded / u planes published in earlier items
     Scalars* S = reinterpret_cast<Scalars*>(smem + L::SC_OFF);
 
@@ -577,7 +577,7 @@ void launch_inst(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, c
     const int ntx = (int)grid.x, ntiles = (int)(grid.x * grid.y), nitems = ntiles * (int)grid.z;
     // The stored variant (six more arrays per node straight from global memory, no registers to spare for the
     // item loop) keeps one item per block.
-    const int blocks = std::min(c.sm_count, nitems);
+    const int blocks = STORED ? nitems : std::min(c.sm_count, nitems);
     const Scalars* sc_in; Scalars* sc_out;
     c.next_scalars(sc_in, sc_out);
     using L = Layout<MODE, STORED, CODE32>;
