@@ -69,8 +69,11 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
                                      last linear solve (up to that many entries); see pf_grid_history */
 #define PF_OPT_KERNELS        10  /* 0 = auto, 1 = direct (one thread per node, neighbours through L1/L2),
                                      2 = tiled (planes staged in shared memory by TMA, z-marched; needs an
-                                     even nx >= 32, ny >= 16, nz >= 8 and 16-byte aligned vectors).  Same
-                                     arithmetic, bit-identical vectors. */
+                                     even nx >= 32, ny >= 16, nz >= 8 and 16-byte aligned vectors),
+                                     3 = cooperative (a whole solve in one persistent kernel, one brick of
+                                     the box per SM with its vectors in shared memory, three grid-wide
+                                     barriers per iteration; needs the on-the-fly stencil and a grid of at
+                                     most about 72^3 nodes).  Same arithmetic, bit-identical vectors. */
 
 #define PF_OPT_PROFILE        11  /* n > 0: bracket the three kernels of the first n iterations of every
                                      linear solve with CUDA events and accumulate their durations

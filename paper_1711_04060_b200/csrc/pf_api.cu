@@ -45,6 +45,8 @@ struct SmallSet {
     char* host = nullptr;           // pinned, 2 x 256 bytes
     cudaEvent_t ev[2] = {nullptr, nullptr};
 };
+constexpr long long COOP_AUTO_MAX_N = 64ll * 64 * 64;     // largest grid the cooperative solver is chosen for by itself
+                                                          // (measured: 1.1x at 64^3 to 1.7x at 32^3 over the next best family)
 constexpr size_t SS_SC = 0 /* two copies, 256 bytes each */, SS_FAULT = 512, SS_DMAX = 768, SS_CTAB0 = 1024,
                  SS_CTAB1 = 1280, SS_PARTIAL = 1536,
                  SS_CHARGES = SS_PARTIAL + sizeof(dd) * 3 * PF_PARTIAL_QUANTITIES * PF_MAX_PARTIAL_BLOCKS;
@@ -105,6 +107,8 @@ struct pf_grid {
     SmallSet* small;         // recycled small buffers; the pointers below point into it
     double* charges_dev;
     // options
+    int coop_state;            // 0 not planned yet, 1 plan valid, -1 not applicable
+    CoopPlan coop;
     int opt_stencil, opt_kernels, opt_check, opt_lin_maxit, opt_max_outer, opt_precond, opt_history;
     double opt_omega_pf, opt_lin_tol, opt_water;
     // small owned device buffers
@@ -200,6 +204,21 @@ bool use_tiled(const pf_grid* g) {
     return tma_supported(g->g) && tma_available();
 }
 
+// The cooperative single-kernel solver: asked for (PF_OPT_KERNELS = 3), or chosen on small grids.
+bool use_coop(pf_grid* g, const Operator& op, CoopPlan* plan) {
+    if (g->opt_kernels != 3 && g->opt_kernels != 0) return false;
+    if (op.stored) return false;
+    if (g->coop_state == 0) {
+        const size_t cap = coop_smem_cap();
+        g->coop_state = (cap > 0 && coop_plan(g->g, op, g->sm_count, cap, &g->coop)) ? 1 : -1;
+    }
+    if (g->coop_state < 0) return false;
+    // auto: small grids only; a per-kernel profile needs the three-kernel families
+    if (g->opt_kernels == 0 && (g->opt_profile || g->g.n > COOP_AUTO_MAX_N)) return false;
+    *plan = g->coop;
+    return true;
+}
+
 Operator make_op(const pf_grid* g, int which /*0 poisson, 1 pf1, 2 poisson+sigma, 3 Laplace in Omega_m*/) {
     Operator op;
     std::memset(&op, 0, sizeof(op));
@@ -277,6 +296,30 @@ cudaGraphExec_t chunk_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, 
     return exec;
 }
 
+// Tail of a linear solve: Q3, the true residual of the returned x (row L8) and the outputs.
+int finish_solve(pf_grid* g, const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, Scalars fin, bool tiled,
+                 int* iters_out, double* relres_out, double* true_relres_out) {
+    double* x = kv.x;
+    if (!fin.done) { fin.status = PF_NOT_CONVERGED; }
+    if (fin.bb == 0.0) PF_CUDA(g, cudaMemsetAsync(x, 0, sizeof(double) * g->g.n, g->stream));   // Q3
+    double true_rel = 0.0;
+    if (true_relres_out && fin.bb != 0.0) {
+        if (tiled) launch_residual_tma(c, op, kv, g->tma, 1); else launch_residual_direct(c, op, kv, 1);
+        launch_finalize(c, nullptr);
+        PF_CUDA(g, cudaMemcpyAsync(g->sc_host[0], c.current_scalars(), sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
+        PF_CUDA(g, cudaStreamSynchronize(g->stream));
+        true_rel = g->opt_norm == 1 ? g->sc_host[0]->true_rmax : std::sqrt(g->sc_host[0]->true_rr) / fin.bnorm;
+    }
+    PF_CUDA(g, cudaGetLastError());
+    g->last_iters = fin.it;
+    if (iters_out) *iters_out = fin.it;
+    if (relres_out) *relres_out = fin.bb == 0.0 ? 0.0 : fin.rnorm / fin.bnorm;
+    if (true_relres_out) *true_relres_out = true_rel;
+    if (fin.status == PF_ERR_BREAKDOWN) return fail(g, PF_ERR_BREAKDOWN, "BiCGSTAB breakdown at iteration %d", fin.it);
+    return fin.status;
+}
+
+
 // ---- Table 3 on the device ----------------------------------------------------------------
 // b: device N with Dirichlet values already forced; x: device N, in/out, Dirichlet values forced.
 int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, double tol, int maxit,
@@ -305,6 +348,23 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     }
     if (g->opt_kernels == 2 && allow_tiled && !tiled)
         return fail(g, PF_ERR_ARG, "tiled kernels need 16-byte aligned vectors");
+    // Small grids: the whole solve in one cooperative kernel (pf_krylov_coop.cu)
+    CoopPlan plan;
+    const bool coop = allow_tiled && use_coop(g, op, &plan);
+    if (g->opt_kernels == 3 && allow_tiled && !coop)
+        return fail(g, PF_ERR_ARG, "the cooperative kernel needs an operator in code form and a grid whose bricks "
+                                   "fit the shared memory of the SMs (about <= 72^3)");
+    if (coop) {
+        Scalars fin;
+        PF_CUDA(g, launch_solve_coop(c, op, kv, precond, plan));
+        PF_CUDA(g, cudaMemcpyAsync(g->sc_host[0], c.current_scalars(), sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
+        PF_CUDA(g, cudaMemcpyAsync(g->sc_host[1], g->rb.fault, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
+        PF_CUDA(g, cudaStreamSynchronize(g->stream));
+        if (*reinterpret_cast<const int*>(g->sc_host[1]) != 0)
+            return fail(g, PF_ERR_CUDA, "cooperative solve: a grid-wide barrier timed out");
+        fin = *g->sc_host[0];
+        return finish_solve(g, c, op, kv, fin, false, iters_out, relres_out, true_relres_out);
+    }
     if (tiled) launch_residual_tma(c, op, kv, g->tma, 0); else launch_residual_direct(c, op, kv, 0);
 
     const int chunk = g->opt_check < 1 ? 1 : g->opt_check;
@@ -367,23 +427,7 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
                 }
             }
     }
-    if (!fin.done) { fin.status = PF_NOT_CONVERGED; }
-    if (fin.bb == 0.0) PF_CUDA(g, cudaMemsetAsync(x, 0, sizeof(double) * g->g.n, g->stream));   // Q3
-    double true_rel = 0.0;
-    if (true_relres_out && fin.bb != 0.0) {
-        if (tiled) launch_residual_tma(c, op, kv, g->tma, 1); else launch_residual_direct(c, op, kv, 1);
-        launch_finalize(c, nullptr);
-        PF_CUDA(g, cudaMemcpyAsync(g->sc_host[0], c.current_scalars(), sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
-        PF_CUDA(g, cudaStreamSynchronize(g->stream));
-        true_rel = g->opt_norm == 1 ? g->sc_host[0]->true_rmax : std::sqrt(g->sc_host[0]->true_rr) / fin.bnorm;
-    }
-    PF_CUDA(g, cudaGetLastError());
-    g->last_iters = fin.it;
-    if (iters_out) *iters_out = fin.it;
-    if (relres_out) *relres_out = fin.bb == 0.0 ? 0.0 : fin.rnorm / fin.bnorm;
-    if (true_relres_out) *true_relres_out = true_rel;
-    if (fin.status == PF_ERR_BREAKDOWN) return fail(g, PF_ERR_BREAKDOWN, "BiCGSTAB breakdown at iteration %d", fin.it);
-    return fin.status;
+    return finish_solve(g, c, op, kv, fin, tiled, iters_out, relres_out, true_relres_out);
 }
 
 int check_ready(pf_grid* g) {
@@ -458,6 +502,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->stream = (cudaStream_t)cuda_stream;
     g->eps = eps_map;
     g->ncharges = ncharges;
+    g->coop_state = 0;
     g->opt_stencil = 0; g->opt_kernels = 0; g->opt_check = 16; g->opt_lin_maxit = 10000; g->opt_max_outer = 1000;
     g->opt_precond = 1; g->opt_history = 0;
     g->opt_omega_pf = 0.3; g->opt_lin_tol = 1e-10; g->opt_water = 55.5;
@@ -605,7 +650,7 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
         case PF_OPT_GRAPH:
             g->opt_graph = iv != 0; return PF_OK;
         case PF_OPT_KERNELS:
-            if (iv < 0 || iv > 2) return fail(g, PF_ERR_ARG, "kernels must be 0, 1 or 2");
+            if (iv < 0 || iv > 3) return fail(g, PF_ERR_ARG, "kernels must be 0, 1, 2 or 3");
             if (iv == 2 && !(tma_supported(g->g) && tma_available()))
                 return fail(g, PF_ERR_ARG, "the tiled kernels need an even nx >= 32, ny >= 16, nz >= 8");
             g->opt_kernels = iv; return PF_OK;

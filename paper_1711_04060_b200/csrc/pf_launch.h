@@ -64,6 +64,15 @@ void launch_k1_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv,
 void launch_k2_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond,
                    int parity);
 
+// Cooperative family (pf_krylov_coop.cu): one persistent kernel per solve, one brick of the box per block, the
+// brick's vectors in shared memory.  For grids small enough that a brick fits one SM (about <= 72^3) and
+// operators in code form.
+struct CoopPlan { int nbx, nby, nbz, vmax, hmax, nhmax, threads; size_t smem; };
+size_t coop_smem_cap();        // usable dynamic shared memory per block, 0 if cooperative launch is unsupported
+bool coop_plan(const GridDims& g, const Operator& op, int max_blocks, size_t smem_cap, CoopPlan* out);
+cudaError_t launch_solve_coop(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond,
+                              const CoopPlan& plan);
+
 // ---- assembly (pf_assembly.cu) ----------------------------------------------------------------
 // Boundary data handed to the assembly and pointwise kernels: the six box faces, and Omega_f (PAPER.md:213,
 // 224-226; readings F1-F3): fixv[i] = prescribed potential of node i, NaN where the node is free; null = none.

@@ -26,7 +26,7 @@ PF_BC_DIRICHLET, PF_BC_NEUMANN = 0, 1
 CHARGES_DEPOSITED, CHARGES_SINGULAR = 0, 1
 NORM_REL_L2, NORM_ABS_INF = 0, 1
 STENCIL_AUTO, STENCIL_STORED, STENCIL_ONTHEFLY = 0, 1, 2
-KERNELS_AUTO, KERNELS_DIRECT, KERNELS_TILED = 0, 1, 2
+KERNELS_AUTO, KERNELS_DIRECT, KERNELS_TILED, KERNELS_COOP = 0, 1, 2, 3
 
 EXPORTS = [
     "pf_grid_create", "pf_grid_set_fixed_nodes", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
