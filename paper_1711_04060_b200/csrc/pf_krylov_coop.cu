@@ -14,12 +14,18 @@
 //     halo nodes from them.  p and v alternate between two global buffers, r is only written in a phase in
 //     which no block reads halos, so no exchange barrier is needed: three grid-wide barriers per iteration,
 //     one per reduction point.
-//   * the inner products.  Barrier and reduction are one step (sync_reduce): a block publishes its
-//     double-double partial sums and a generation flag; thread b of every block waits for block b's flag and
-//     takes its partials; every block then sums them in the same order and takes the same scalar step
-//     (alpha, omega, beta, the convergence test), so all blocks leave the loop in the same iteration.
-// A wait is bounded: a block that does not see a flag within about a second sets the abort flag and leaves
+//   * the inner products.  Barrier and reduction are one step (sync_reduce): a block writes its double-double
+//     partial sums to its record, thread 0 adds 1 to an arrival counter (after a fence) and waits until the
+//     counter shows that all blocks of this generation have arrived; then thread b of every block takes block
+//     b's record, and every block sums the records in the same order and takes the same scalar step (alpha,
+//     omega, beta, the convergence test), so all blocks leave the loop in the same iteration.
+// A wait is bounded: a block that does not see the arrivals within about a second sets the abort flag and leaves
 // (the host reports PF_ERR_CUDA); the cooperative launch makes that unreachable in normal operation.
+//
+// Measured (B200, profiles/r1_coop.md): a barrier-reduction costs about 3.5 us (two block-wide double-double
+// trees, a fence, the atomic round trip, the record reads), so an iteration costs 13.5 us at 32^3 and 23 us at
+// 64^3 against 23 / 25.6 us for three launches; a flag per block polled by all blocks was 2x slower (hot lines),
+// cooperative_groups' grid.sync() alone costs 1.2 us.
 #include <algorithm>
 #include <cstring>
 #include "pf_krylov.cuh"
@@ -380,7 +386,8 @@ bool coop_plan(const GridDims& g, const Operator& op, int max_blocks, size_t sme
                 const size_t smem = coop_smem_bytes(V, H, nh);
                 if (smem > smem_cap || H > 65535) continue;
                 // a halo node costs about as much as an own node in each of the two matvec phases
-                const double cost = V + 0.7 * nh;
+                // (ties: the longest bricks along x, the contiguous direction)
+                const double cost = V + 0.7 * nh + 1e-3 * nbx;
                 if (cost < best) {
                     best = cost;
                     out->nbx = nbx; out->nby = nby; out->nbz = nbz;
