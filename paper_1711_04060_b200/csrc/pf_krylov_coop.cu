@@ -63,83 +63,6 @@ __device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long
     return v;
 }
 
-// Block-wide sum of NQ <= 2 double-double values (and maximum of non-negative doubles), results in thread 0.
-// The fp64 pipe adds 16 lanes per clock and SM quarter, so a shuffle tree over double-doubles is bound by
-// instruction count, not latency: two sums share one tree (after the first exchange the lower half-warp carries
-// the first sum and the upper one the second), warps that hold no values skip the first level, and the maximum
-// goes through the integer warp reduction.  scratch: 2*32 dd, mxs: 32 doubles; all threads of the block call;
-// only the first `active` warps hold values.
-__device__ __forceinline__ dd dd_shfl_xor(const dd& a, int mask) {
-    dd r;
-    r.hi = __shfl_xor_sync(0xffffffffu, a.hi, mask);
-    r.lo = __shfl_xor_sync(0xffffffffu, a.lo, mask);
-    return r;
-}
-__device__ __forceinline__ dd dd_shfl_down16(const dd& a, int delta) {
-    dd r;
-    r.hi = __shfl_down_sync(0xffffffffu, a.hi, delta, 16);
-    r.lo = __shfl_down_sync(0xffffffffu, a.lo, delta, 16);
-    return r;
-}
-// Maximum of non-negative doubles over a warp: their bit patterns order like the values.
-__device__ __forceinline__ double warp_max_nonneg(double m) {
-    const unsigned hi = (unsigned)__double2hiint(m), lo = (unsigned)__double2loint(m);
-    const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
-    const unsigned ml = __reduce_max_sync(0xffffffffu, hi == mh ? lo : 0u);
-    return __hiloint2double((int)mh, (int)ml);
-}
-// One warp: sums of q over the lanes.  NQ = 2: q[0] total in lane 0, q[1] total in lane 16 (returned in x).
-template <int NQ>
-__device__ __forceinline__ dd warp_sum_packed(const dd (&q)[NQ], int lane) {
-    dd x;
-    if (NQ == 2) {
-        const bool up = (lane & 16) != 0;
-        const dd send = up ? q[0] : q[NQ - 1];
-        x = up ? q[NQ - 1] : q[0];
-        dd_add(x, dd_shfl_xor(send, 16));
-#pragma unroll
-        for (int d = 8; d > 0; d >>= 1) dd_add(x, dd_shfl_down16(x, d));
-    } else {
-        x = q[0];
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) dd_add(x, dd_shfl_down(x, d));
-    }
-    return x;
-}
-template <int NQ, bool MAX>
-__device__ __forceinline__ void block_reduce_packed(dd (&q)[NQ], double& m, dd* scratch, double* mxs, int active) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (warp < active) {
-        const dd x = warp_sum_packed<NQ>(q, lane);
-        if (NQ == 2) { if ((lane & 15) == 0) scratch[(lane >> 4) * 32 + warp] = x; }
-        else if (lane == 0) scratch[warp] = x;
-        if (MAX) { const double wm = warp_max_nonneg(m); if (lane == 0) mxs[warp] = wm; }
-    }
-    __syncthreads();
-    if (warp == 0) {
-        dd w[NQ];
-        if (NQ == 2) {              // lane (k, j): entries j and j + 16 of sum k
-            const int k = lane >> 4, j = lane & 15;
-            dd a = j < active ? scratch[k * 32 + j] : dd_zero();
-            const dd b = j + 16 < active ? scratch[k * 32 + j + 16] : dd_zero();
-            dd_add(a, b);
-#pragma unroll
-            for (int d = 8; d > 0; d >>= 1) dd_add(a, dd_shfl_down16(a, d));
-            w[0] = a;
-            w[NQ - 1].hi = __shfl_sync(0xffffffffu, a.hi, 16);
-            w[NQ - 1].lo = __shfl_sync(0xffffffffu, a.lo, 16);
-        } else {
-            dd a = lane < active ? scratch[lane] : dd_zero();
-#pragma unroll
-            for (int d = 16; d > 0; d >>= 1) dd_add(a, dd_shfl_down(a, d));
-            w[0] = a;
-        }
-#pragma unroll
-        for (int k = 0; k < NQ; ++k) q[k] = w[k];
-        if (MAX) m = warp_max_nonneg(lane < active ? mxs[lane] : 0.0);
-    }
-}
-
 // Grid-wide barrier + reduction.  In: this thread's sums q (and maximum m).  Out (thread 0): totals over all
 // blocks, the same bits in every block.  Returns false if the wait timed out.  Every global write the block
 // made before the call is visible to every block after it.  One arrival counter (thread 0 of a block adds 1 and
@@ -149,7 +72,8 @@ __device__ __forceinline__ bool sync_reduce(dd (&q)[NQ], double& m, unsigned gen
     const int nblk = (int)gridDim.x;
     __shared__ int ok_s;
     double* mxs = reinterpret_cast<double*>(scratch + 2 * 32);
-    block_reduce_packed<NQ, MAX>(q, m, scratch, mxs, (int)(blockDim.x >> 5));
+    block_reduce_dd<NQ>(q, scratch);
+    if (MAX) m = block_reduce_max(m, mxs);
     if (threadIdx.x == 0) {
         dd* rec = a.rec + ((size_t)(gen & 3u) * COOP_MAX_BLOCKS + blockIdx.x) * 3;
 #pragma unroll
@@ -179,7 +103,8 @@ __device__ __forceinline__ bool sync_reduce(dd (&q)[NQ], double& m, unsigned gen
         for (int k = 0; k < NQ; ++k) { dd part; part.hi = w[k].x; part.lo = w[k].y; dd_add(q[k], part); }
         if (MAX) m = fmax(m, w[NQ].x);
     }
-    block_reduce_packed<NQ, MAX>(q, m, scratch, mxs, (nblk + 31) >> 5);     // thread b holds block b's record
+    block_reduce_dd<NQ>(q, scratch, (nblk + 31) >> 5);     // thread b holds block b's record
+    if (MAX) m = block_reduce_max(m, mxs, (nblk + 31) >> 5);
     return true;
 }
 
