@@ -191,6 +191,15 @@ int pf_grid_laplace_iters(const pf_grid *g);
  * operands outside the range of their branch-free division (reading D4 of DESIGN.md). */
 int pf_grid_fault_repeats(const pf_grid *g);
 
+/* Decomposition the cooperative kernel (PF_OPT_KERNELS = 3; pf_krylov_coop.cu) would use for an nx x ny x nz box
+ * on a device with max_blocks SMs and smem_cap bytes of dynamic shared memory per block: one brick per block,
+ * brick k of nb along an axis of n nodes = nodes floor(k n/nb) .. floor((k+1) n/nb) - 1.  Host arithmetic only
+ * (no device is touched).  out (host, 8 ints): bricks per direction nbx, nby, nbz; array extents of the largest
+ * brick: own nodes (rounded up to even), nodes with one halo layer, halo nodes; threads per block; bytes of
+ * dynamic shared memory.  Returns PF_OK, or PF_ERR_ARG when no decomposition fits (the solver then uses the
+ * three-kernel families) or an argument is invalid. */
+int pf_coop_plan(int nx, int ny, int nz, int max_blocks, size_t smem_cap, int *out);
+
 /* Introspection used by the tests: 1 = stored, 2 = on-the-fly; number of palette entries. */
 int pf_grid_stencil(const pf_grid *g);
 int pf_grid_palette_size(const pf_grid *g);

@@ -899,6 +899,19 @@ int pf_grid_laplace_iters(const pf_grid* g) { return g ? g->laplace_iters : PF_E
 
 int pf_grid_fault_repeats(const pf_grid* g) { return g ? g->fault_repeats : PF_ERR_ARG; }
 
+int pf_coop_plan(int nx, int ny, int nz, int max_blocks, size_t smem_cap, int* out) {
+    if (!out || nx < 3 || ny < 3 || nz < 3 || max_blocks < 1) return PF_ERR_ARG;
+    GridDims gd;
+    gd.nx = nx; gd.ny = ny; gd.nz = nz; gd.n = (long long)nx * ny * nz;
+    Operator op;
+    std::memset(&op, 0, sizeof(op));
+    CoopPlan plan;
+    if (!coop_plan(gd, op, max_blocks, smem_cap, &plan)) return PF_ERR_ARG;
+    out[0] = plan.nbx; out[1] = plan.nby; out[2] = plan.nbz; out[3] = plan.vmax; out[4] = plan.hmax;
+    out[5] = plan.nhmax; out[6] = plan.threads; out[7] = (int)plan.smem;
+    return PF_OK;
+}
+
 int pf_grid_stencil(const pf_grid* g) { return g ? (want_stored(g) ? 1 : 2) : PF_ERR_ARG; }
 int pf_grid_palette_size(const pf_grid* g) { return g ? g->pal.count : PF_ERR_ARG; }
 

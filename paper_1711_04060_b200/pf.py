@@ -32,7 +32,7 @@ EXPORTS = [
     "pf_grid_create", "pf_grid_set_fixed_nodes", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
     "pf_solve_linear", "pf_solve_linear_host", "pf_solve_pf", "pf_fermi_pointwise", "pf_grid_history",
     "pf_grid_linear_iters", "pf_grid_increments", "pf_grid_fault_repeats", "pf_grid_laplace_iters", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_code_layout", "pf_grid_copy_array",
-    "pf_grid_profile", "pf_launch_count", "pf_grid_destroy", "pf_last_error", "pf_version",
+    "pf_grid_profile", "pf_launch_count", "pf_coop_plan", "pf_grid_destroy", "pf_last_error", "pf_version",
 ]
 
 
@@ -87,6 +87,7 @@ def load():
     L.pf_grid_code_layout.argtypes = [_vp, _ip, _ip, ctypes.POINTER(ctypes.c_size_t)]
     L.pf_grid_profile.argtypes = [_vp, _dp, ctypes.POINTER(ctypes.c_longlong)]
     L.pf_launch_count.restype = ctypes.c_longlong
+    L.pf_coop_plan.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_size_t, _ip]
     L.pf_grid_destroy.argtypes = [_vp]
     L.pf_grid_destroy.restype = None
     L.pf_last_error.argtypes = [_vp]
@@ -234,6 +235,15 @@ def pf_grid_profile(handle) -> dict:
 
 def pf_launch_count() -> int:
     return int(load().pf_launch_count())
+
+
+def pf_coop_plan(nx: int, ny: int, nz: int, max_blocks: int = 148, smem_cap: int = 228352) -> Optional[dict]:
+    """Brick decomposition of the cooperative kernel (host arithmetic only); None when none fits."""
+    out = (ctypes.c_int * 8)()
+    if load().pf_coop_plan(nx, ny, nz, max_blocks, smem_cap, out) != PF_OK:
+        return None
+    keys = ("nbx", "nby", "nbz", "vmax", "hmax", "nhmax", "threads", "smem")
+    return dict(zip(keys, list(out)))
 
 
 def pf_grid_laplace_iters(handle) -> int:
