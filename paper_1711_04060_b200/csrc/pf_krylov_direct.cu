@@ -1,7 +1,8 @@
 // pf_krylov_direct.cu -- "direct" Krylov kernels: one thread per node in a grid-stride loop,
 // neighbours fetched straight from global memory through L1/L2.  Same arithmetic, statement for
-// statement, as the tiled kernels (pf_krylov_tiled.cu); this variant is the simple one the tiled
-// kernels are tested against, and the one used for grids too small to fill the tiles.
+// statement, as the tiled kernels (pf_krylov_tma.cu) and the cooperative kernel (pf_krylov_coop.cu);
+// this variant is the simple one the other two are tested against, and the one used for grids too
+// small to fill the tiles when the cooperative kernel does not apply.
 //
 // One BiCGSTAB iteration (Table 3) is three launches, one per reduction point:
 //   k1: steps 5-11   p = r + beta(p - omega v);  v = A M^-1 p;           reduces r~.v        (row L4)
