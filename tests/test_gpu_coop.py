@@ -144,3 +144,21 @@ def test_coop_not_applicable(pf):
     with pytest.raises(pf.PFError):
         g.solve_linear(w.rhs, maxit=5)
     g.close()
+
+
+def test_coop_random_shapes_repeatable(pf):
+    """Twelve seeded random box shapes, each solved three times by the cooperative kernel: every run gives the bits
+    of the one-thread-per-node kernels (a race in the barrier or in the halo reads would show up as a run-to-run
+    difference)."""
+    rng = np.random.default_rng(123)
+    for trial in range(12):
+        nx, ny, nz = (int(v) for v in rng.integers(3, 64, size=3))
+        w = ragged_workload(nx=nx, ny=ny, nz=nz, seed=1000 + trial)
+        ref = _solve(pf, w, pf.KERNELS_DIRECT, maxit=300)
+        g = pf.Grid.from_workload(w, stencil=2, kernels=pf.KERNELS_COOP, options={pf.PF_OPT_HISTORY: 4096})
+        for _ in range(3):
+            x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+            out = g.solve_linear(w.rhs, x=x, tol=1e-10, maxit=300)
+            assert out["iters"] == ref["iters"] and torch.equal(out["x"], ref["x"]), (nx, ny, nz)
+            assert np.array_equal(g.history(4096), ref["hist"])
+        g.close()
