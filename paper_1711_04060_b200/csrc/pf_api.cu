@@ -357,9 +357,24 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     if (g->opt_kernels == 3 && allow_tiled && !coop)
         return fail(g, PF_ERR_ARG, "the cooperative kernel needs an operator in code form and a grid whose bricks "
                                    "fit the shared memory of the SMs (about <= 72^3)");
+    bool coop_launched = false;
     if (coop) {
+        const int flip0 = g->flip;
+        const cudaError_t le = launch_solve_coop(c, op, kv, precond, plan);
+        if (le == cudaSuccess) {
+            coop_launched = true;
+        } else if (g->opt_kernels == 0) {
+            // chosen automatically, but the device cannot hold the grid right now (e.g. fewer SMs available to this
+            // context than the plan assumed): not an error, the three-kernel families take over for this grid
+            cudaGetLastError();
+            g->coop_state = -1;
+            g->flip = flip0;
+        } else {
+            return fail(g, PF_ERR_CUDA, "cooperative launch: %s", cudaGetErrorString(le));
+        }
+    }
+    if (coop_launched) {
         Scalars fin;
-        PF_CUDA(g, launch_solve_coop(c, op, kv, precond, plan));
         PF_CUDA(g, cudaMemcpyAsync(g->sc_host[0], c.current_scalars(), sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
         PF_CUDA(g, cudaMemcpyAsync(g->sc_host[1], g->rb.fault, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
         PF_CUDA(g, cudaStreamSynchronize(g->stream));

@@ -382,8 +382,9 @@ cudaError_t launch_solve_coop(const LaunchCtx& c, const Operator& op, const Kryl
     e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem);
     if (e != cudaSuccess) return e;
     void* args[] = {&a};
-    ++g_launch_count;
-    return cudaLaunchCooperativeKernel(fn, dim3(nblk), dim3(plan.threads), args, plan.smem, c.stream);
+    e = cudaLaunchCooperativeKernel(fn, dim3(nblk), dim3(plan.threads), args, plan.smem, c.stream);
+    if (e == cudaSuccess) ++g_launch_count;
+    return e;
 }
 
 }  // namespace pf
