@@ -107,6 +107,11 @@ struct pf_grid {
     SmallSet* small;         // recycled small buffers; the pointers below point into it
     double* charges_dev;
     // options
+    // Odd nx: the tiled kernels need an even row length, so the Krylov layer can work on the box widened by one
+    // column of identity rows (gk); A0p, bp, xp are the widened copies of the diagonal, right-hand side and iterate
+    GridDims gk;
+    bool padx;
+    double *A0p, *bp, *xp;
     int coop_state;            // 0 not planned yet, 1 plan valid, -1 not applicable
     CoopPlan coop;
     int opt_stencil, opt_kernels, opt_check, opt_lin_maxit, opt_max_outer, opt_precond, opt_history;
@@ -182,8 +187,8 @@ int fail(pf_grid* g, int code, const char* fmt, ...) {
         if (e_ != cudaSuccess) return fail((g), PF_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
     } while (0)
 
-int n_vectors(bool stored, int charge_model, bool fixed_nodes) {
-    return 19 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0) + (fixed_nodes ? 1 : 0);
+int n_vectors(bool stored, int charge_model, bool fixed_nodes, bool padx) {
+    return 19 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0) + (fixed_nodes ? 1 : 0) + (padx ? 3 : 0);
 }
 
 int code_mode_of(const pf_grid* g) { return g->pal.count > PF_MAX_PALETTE ? 0 : (g->pal.count <= 2 ? 1 : 2); }
@@ -199,12 +204,12 @@ bool want_stored(const pf_grid* g) {
     return g->pal.count > PF_MAX_PALETTE;
 }
 
-bool use_tiled(const pf_grid* g) {
+bool use_tiled(const pf_grid* g, const GridDims& dims) {
     if (g->opt_kernels == 1) return false;
     // auto: below about 40^3 a launch of the one-thread-per-node kernels is shorter than one of the tiled kernels
     // (16.7 against 22.2 us per iteration at 32^3, 49 against 24 at 64^3)
-    if (g->opt_kernels == 0 && g->g.n < 70000) return false;
-    return tma_supported(g->g) && tma_available();
+    if (g->opt_kernels == 0 && dims.n < 70000) return false;
+    return tma_supported(dims) && tma_available();
 }
 
 // The cooperative single-kernel solver: asked for (PF_OPT_KERNELS = 3), or chosen on small grids.
@@ -267,7 +272,7 @@ void enqueue_iteration(const LaunchCtx& c, const Operator& op, KrylovVecs& kv, c
 // (operator, vectors, kernel family) and replayed.  Returns null when graphs do not apply.
 cudaGraphExec_t chunk_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool tiled,
                             bool precond, int chunk) {
-    if (!g->opt_graph || g->opt_profile || (chunk & 1) || g->g.n > (1ll << 22)) return nullptr;
+    if (!g->opt_graph || g->opt_profile || (chunk & 1) || c.g.n > (1ll << 22)) return nullptr;
     for (const auto& cg : g->graphs)
         if (cg.a0 == op.A0 && cg.code == op.code && cg.b == kv.b && cg.x == kv.x && cg.y == kv.y && cg.hist == kv.hist &&
             cg.precond == (int)precond && cg.tiled == (int)tiled && cg.chunk == chunk)
@@ -304,7 +309,7 @@ int finish_solve(pf_grid* g, const LaunchCtx& c, const Operator& op, const Krylo
                  int* iters_out, double* relres_out, double* true_relres_out) {
     double* x = kv.x;
     if (!fin.done) { fin.status = PF_NOT_CONVERGED; }
-    if (fin.bb == 0.0) PF_CUDA(g, cudaMemsetAsync(x, 0, sizeof(double) * g->g.n, g->stream));   // Q3
+    if (fin.bb == 0.0) PF_CUDA(g, cudaMemsetAsync(x, 0, sizeof(double) * c.g.n, g->stream));   // Q3
     double true_rel = 0.0;
     if (true_relres_out && fin.bb != 0.0) {
         if (tiled) launch_residual_tma(c, op, kv, g->tma, 1); else launch_residual_direct(c, op, kv, 1);
@@ -324,12 +329,14 @@ int finish_solve(pf_grid* g, const LaunchCtx& c, const Operator& op, const Krylo
 
 
 // ---- Table 3 on the device ----------------------------------------------------------------
-// b: device N with Dirichlet values already forced; x: device N, in/out, Dirichlet values forced.
-int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, double tol, int maxit,
-                    int* iters_out, double* relres_out, double* true_relres_out, bool allow_tiled = true) {
+// b: device, dims.n entries with Dirichlet values already forced; x: device, in/out, Dirichlet values forced.
+// dims: the grid's box, or the box widened by one column of identity rows (bicgstab_device below).
+int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const double* b, double* x, double tol, int maxit,
+                  int* iters_out, double* relres_out, double* true_relres_out, bool allow_tiled, bool allow_coop) {
     if (maxit < 0) return fail(g, PF_ERR_ARG, "maxit < 0");
     if (!(tol >= 0.0)) return fail(g, PF_ERR_ARG, "tol must be >= 0");
-    const LaunchCtx c = make_ctx(g);
+    LaunchCtx c = make_ctx(g);
+    c.g = dims;
     const bool precond = g->opt_precond != 0;
     Scalars init;
     std::memset(&init, 0, sizeof(init));
@@ -343,17 +350,18 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     kv.p_in = g->p0; kv.p_out = g->p1; kv.v_in = g->v0; kv.v_out = g->v1;
     // D3: with the Jacobi preconditioner step 16 accumulates y = sum(alpha p + omega s); x = x0 + M^-1 y at the end
     kv.y = precond ? g->y : x;
-    if (precond) PF_CUDA(g, cudaMemsetAsync(g->y, 0, sizeof(double) * g->g.n, g->stream));
-    bool tiled = allow_tiled && use_tiled(g) && tma_pointers_ok(kv, op);
-    if (tiled && !tma_set_build(g->tma, g->g, op, kv)) {
+    if (precond) PF_CUDA(g, cudaMemsetAsync(g->y, 0, sizeof(double) * dims.n, g->stream));
+    bool tiled = allow_tiled && use_tiled(g, dims) && tma_pointers_ok(kv, op);
+    if (tiled && !tma_set_build(g->tma, dims, op, kv)) {
         if (g->opt_kernels == 2) return fail(g, PF_ERR_CUDA, "tensor-map encoding failed");
         tiled = false;
     }
     if (g->opt_kernels == 2 && allow_tiled && !tiled)
-        return fail(g, PF_ERR_ARG, "tiled kernels need 16-byte aligned vectors");
+        return fail(g, PF_ERR_ARG, "the tiled kernels need 16-byte aligned vectors and an even nx (an odd nx only with "
+                                   "the on-the-fly stencil)");
     // Small grids: the whole solve in one cooperative kernel (pf_krylov_coop.cu)
     CoopPlan plan;
-    const bool coop = allow_tiled && use_coop(g, op, &plan);
+    const bool coop = allow_tiled && allow_coop && use_coop(g, op, &plan);
     if (g->opt_kernels == 3 && allow_tiled && !coop)
         return fail(g, PF_ERR_ARG, "the cooperative kernel needs an operator in code form and a grid whose bricks "
                                    "fit the shared memory of the SMs (about <= 72^3)");
@@ -431,7 +439,7 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
         // not been touched yet (D3), so the solve is simply repeated with the kernels that use __ddiv_rn
         PF_CUDA(g, cudaStreamSynchronize(g->stream));
         ++g->fault_repeats;
-        return bicgstab_device(g, op, b, x, tol, maxit, iters_out, relres_out, true_relres_out, false);
+        return bicgstab_core(g, dims, op, b, x, tol, maxit, iters_out, relres_out, true_relres_out, false, false);
     }
     if (precond) launch_finish_x(c, op, kv);
     PF_CUDA(g, cudaStreamSynchronize(g->stream));
@@ -446,6 +454,30 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
             }
     }
     return finish_solve(g, c, op, kv, fin, tiled, iters_out, relres_out, true_relres_out);
+}
+
+// A linear solve of the grid.  Odd nx (rows of an odd number of doubles cannot be described to the TMA unit, whose
+// strides are multiples of 16 bytes): where the tiled kernels would otherwise apply, the system is embedded in the
+// box widened by one column x = nx of identity rows (diagonal 1, stencil code 0, b = x = 0): the extra unknowns are
+// decoupled and exactly 0 in every vector, so they add exact zeros to the inner products and the iterates of the
+// real unknowns keep their bits.  Costs eight vector passes per solve (about half an iteration).
+int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, double tol, int maxit,
+                    int* iters_out, double* relres_out, double* true_relres_out) {
+    CoopPlan plan;
+    const bool widen = g->padx && !op.stored && g->opt_kernels != 1 && g->opt_kernels != 3 && use_tiled(g, g->gk) &&
+                       !use_coop(g, op, &plan);
+    if (!widen)
+        return bicgstab_core(g, g->g, op, b, x, tol, maxit, iters_out, relres_out, true_relres_out, true, true);
+    launch_widen(g->stream, g->g, op.A0, g->A0p, 1.0);
+    launch_widen(g->stream, g->g, b, g->bp, 0.0);
+    launch_widen(g->stream, g->g, x, g->xp, 0.0);
+    Operator opk = op;
+    opk.A0 = g->A0p;
+    const int rc = bicgstab_core(g, g->gk, opk, g->bp, g->xp, tol, maxit, iters_out, relres_out, true_relres_out, true, false);
+    if (rc == PF_ERR_CUDA || rc == PF_ERR_ARG) return rc;
+    launch_narrow(g->stream, g->g, g->xp, x);
+    PF_CUDA(g, cudaGetLastError());
+    return rc;
 }
 
 int check_ready(pf_grid* g) {
@@ -515,6 +547,8 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     }
     pf_grid* g = new pf_grid();
     g->g.nx = nx; g->g.ny = ny; g->g.nz = nz; g->g.n = (long long)nx * ny * nz;
+    g->gk = g->g; g->padx = (nx & 1) != 0; g->A0p = g->bp = g->xp = nullptr;
+    if (g->padx) { g->gk.nx = nx + 1; g->gk.n = (long long)(nx + 1) * ny * nz; }
     g->h = h;
     for (int f = 0; f < 6; ++f) { g->bc.type[f] = bc->type[f]; g->bc.value[f] = bc->value[f]; }
     g->stream = (cudaStream_t)cuda_stream;
@@ -595,9 +629,9 @@ void pf_grid_destroy(pf_grid* g) {
 
 size_t pf_grid_workspace_bytes(const pf_grid* g) {
     if (!g) return 0;
-    const size_t vec = align_up(sizeof(double) * (size_t)g->g.n, 256);
+    const size_t vec = align_up(sizeof(double) * (size_t)g->gk.n, 256);
     const size_t code_l = g->opt_charge_model == 1 ? align_up((size_t)cpitch_of(g) * g->g.ny * g->g.nz * 2, 256) : 0;
-    return (size_t)n_vectors(want_stored(g), g->opt_charge_model, !g->fix_idx.empty()) * vec + 2 * code_bytes_of(g) + code_l;
+    return (size_t)n_vectors(want_stored(g), g->opt_charge_model, !g->fix_idx.empty(), g->padx) * vec + 2 * code_bytes_of(g) + code_l;
 }
 
 int pf_grid_set_option(pf_grid* g, int key, double value) {
@@ -669,8 +703,8 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
             g->opt_graph = iv != 0; return PF_OK;
         case PF_OPT_KERNELS:
             if (iv < 0 || iv > 3) return fail(g, PF_ERR_ARG, "kernels must be 0, 1, 2 or 3");
-            if (iv == 2 && !(tma_supported(g->g) && tma_available()))
-                return fail(g, PF_ERR_ARG, "the tiled kernels need an even nx >= 32, ny >= 16, nz >= 8");
+            if (iv == 2 && !(tma_supported(g->gk) && tma_available()))
+                return fail(g, PF_ERR_ARG, "the tiled kernels need nx >= 32, ny >= 16, nz >= 8");
             g->opt_kernels = iv; return PF_OK;
         default:
             return fail(g, PF_ERR_ARG, "unknown option key %d", key);
@@ -685,7 +719,7 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     if (bytes < need) return fail(g, PF_ERR_WORKSPACE, "workspace has %zu bytes, %zu needed", bytes, need);
     g->stored = want_stored(g);
     g->ws = dev_ptr; g->ws_bytes = bytes;
-    const size_t vec = align_up(sizeof(double) * (size_t)g->g.n, 256);
+    const size_t vec = align_up(sizeof(double) * (size_t)g->gk.n, 256);     // every vector has room for the widened box
     char* base = (char*)dev_ptr;
     auto take = [&]() { double* p = (double*)base; base += vec; return p; };
     g->r = take(); g->rt = take(); g->p0 = take(); g->p1 = take(); g->v0 = take(); g->v1 = take();
@@ -695,6 +729,7 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     g->charge_model = g->opt_charge_model;
     if (g->charge_model == 1) { g->phiL = take(); g->phistar = take(); g->A0_L = take(); }
     g->fixv = g->fix_idx.empty() ? nullptr : take();
+    if (g->padx) { g->A0p = take(); g->bp = take(); g->xp = take(); }
     for (int d = 0; d < 6; ++d) { g->offd[d] = g->stored ? take() : nullptr; }
     for (int d = 0; d < 6; ++d) { g->offd_pf1[d] = g->stored ? take() : nullptr; }
     g->code_mode = code_mode_of(g);

@@ -257,6 +257,40 @@ k_finish_x(long long n, const double* __restrict__ A0, const double* __restrict_
         x[i] = add(x[i], dvd(y[i], A0[i]));
 }
 
+// Rows of nx doubles <-> rows of nx + 1 doubles (odd nx, pf_api.cu bicgstab_device).
+__global__ void __launch_bounds__(256)
+k_widen(int nx, long long rows, const double* __restrict__ src, double* __restrict__ dst, double fill) {
+    const long long total = rows * (nx + 1);
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) {
+        const long long row = k / (nx + 1);
+        const int ix = (int)(k - row * (nx + 1));
+        dst[k] = ix < nx ? src[row * nx + ix] : fill;
+    }
+}
+__global__ void __launch_bounds__(256)
+k_narrow(int nx, long long rows, const double* __restrict__ src, double* __restrict__ dst) {
+    const long long total = rows * nx;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += stride) {
+        const long long row = k / nx;
+        dst[k] = src[k + row];
+    }
+}
+
+void launch_widen(cudaStream_t s, const GridDims& g, const double* src, double* dst, double fill) {
+    const long long rows = (long long)g.ny * g.nz;
+    const long long want = (rows * (g.nx + 1) + 255) / 256;
+    ++g_launch_count;
+    k_widen<<<(int)(want < 4736 ? want : 4736), 256, 0, s>>>(g.nx, rows, src, dst, fill);
+}
+void launch_narrow(cudaStream_t s, const GridDims& g, const double* src, double* dst) {
+    const long long rows = (long long)g.ny * g.nz;
+    const long long want = (rows * g.nx + 255) / 256;
+    ++g_launch_count;
+    k_narrow<<<(int)(want < 4736 ? want : 4736), 256, 0, s>>>(g.nx, rows, src, dst);
+}
+
 static int direct_blocks(long long n, int sm_count) {
     long long want = (n + DIRECT_THREADS - 1) / DIRECT_THREADS;
     long long cap = (long long)sm_count * 8;

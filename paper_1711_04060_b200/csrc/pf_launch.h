@@ -37,6 +37,10 @@ struct LaunchCtx {
     Scalars* current_scalars() const { return sc[*flip]; }
 };
 
+// dst (rows of g.nx + 1 doubles) = src (rows of g.nx doubles) with `fill` in the extra column, and back.
+void launch_widen(cudaStream_t s, const GridDims& g, const double* src, double* dst, double fill);
+void launch_narrow(cudaStream_t s, const GridDims& g, const double* src, double* dst);
+
 // ---- Krylov kernels -----------------------------------------------------------------------
 // mode 0: r = b - A x, r~ = r, ||b||, ||r|| (Table 3 step 2); mode 1: ||b - A x||^2 only.
 void launch_residual_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, int mode);

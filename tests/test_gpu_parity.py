@@ -402,3 +402,61 @@ def test_pf_paper_parameters(pf, oracle):
     assert np.max(np.abs(np.array(out["lin_iters_hist"]) - ref["lin_iters_hist"])) <= 10
     assert rel_l2(out["phi"].cpu().numpy(), ref["phi"]) <= 1e-7
     assert np.allclose(out["incr_hist"], ref["incr_hist"], rtol=1e-4, atol=0)
+
+
+# ---- odd nx: the tiled kernels on the box widened by one column of identity rows ---------------------------
+
+@pytest.mark.parametrize("shape", [(33, 16, 8), (65, 17, 9), (131, 33, 21), (97, 48, 64)])
+def test_tiled_kernels_odd_nx(pf, oracle, shape):
+    """An odd nx cannot be described to the TMA unit; the solve is embedded in the box with one more column of
+    decoupled identity rows.  Same bits as the one-thread-per-node kernels on the original box:
+    iterate, residual history, true residual; with a warm start and a sigma shift as well."""
+    nx, ny, nz = shape
+    w = ragged_workload(nx=nx, ny=ny, nz=nz, seed=77 + nx)
+    rng = wl.SplitMix64(5)
+    sigma = np.array([rng.uniform_range(0.0, 3.0) for _ in range(w.n)])
+    x0 = np.array([rng.uniform_range(-1.0, 1.0) for _ in range(w.n)])
+    for sg, start in ((None, None), (sigma, x0)):
+        res = []
+        for kernels in (1, 2):
+            g = pf.Grid.from_workload(w, stencil=2, kernels=kernels, options={pf.PF_OPT_HISTORY: 64})
+            x = torch.zeros(w.n, dtype=torch.float64, device="cuda") if start is None else torch.tensor(start, device="cuda")
+            out = g.solve_linear(w.rhs, x=x, tol=0.0, maxit=30, sigma=None if sg is None else torch.tensor(sg, device="cuda"))
+            res.append((out["x"].clone(), g.history(64), out["true_relres"], out["iters"]))
+            g.close()
+        assert torch.equal(res[0][0], res[1][0]), shape
+        assert np.array_equal(res[0][1], res[1][1]) and res[0][2] == res[1][2] and res[0][3] == res[1][3] == 30
+    ref = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, w.rhs, tol=1e-10)
+    g = pf.Grid.from_workload(w, stencil=2, kernels=2)
+    out = g.solve_linear(w.rhs, tol=1e-10)
+    g.close()
+    assert out["status"] == 0 and abs(out["iters"] - ref["iters"]) <= max(1, 0.02 * ref["iters"])
+    assert out["true_relres"] <= 1.05e-10 and rel_l2(out["x"].cpu().numpy(), ref["x"]) <= 1e-9
+
+
+def test_odd_nx_auto_and_pf(pf):
+    """Auto mode on a large odd-nx box takes the widened tiled path (same bits as the direct kernels); b = 0 gives
+    x = 0; a PF solve on an odd-nx box is the same with both families."""
+    w = ragged_workload(nx=129, ny=96, nz=80, seed=3)
+    res = []
+    for kernels in (1, 0):
+        g = pf.Grid.from_workload(w, stencil=2, kernels=kernels)
+        out = g.solve_linear(w.rhs, tol=0.0, maxit=12)
+        res.append(out["x"].clone())
+        g.close()
+    assert torch.equal(res[0], res[1])
+    w0 = ragged_workload(nx=65, ny=40, nz=37, seed=4, mixed_bc=False)
+    g = pf.Grid.from_workload(w0, stencil=2, kernels=2)
+    x = torch.ones(w0.n, dtype=torch.float64, device="cuda")
+    z = g.solve_linear(np.zeros(w0.n), x=x)                       # Q3 through the widened path
+    assert z["status"] == 0 and z["iters"] == 0 and float(x.abs().max()) == 0.0
+    g.close()
+    w = wl.config0(n=33)
+    sp = w.species
+    out = []
+    for kernels in (1, 2):
+        g = pf.Grid.from_workload(w, stencil=2, kernels=kernels)
+        out.append(g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, 1e-6))
+        g.close()
+    assert out[0]["outer_iters"] == out[1]["outer_iters"] and out[0]["lin_iters_hist"] == out[1]["lin_iters_hist"]
+    assert torch.equal(out[0]["phi"], out[1]["phi"])
