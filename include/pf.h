@@ -68,8 +68,10 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
 #define PF_OPT_HISTORY         9  /* >0: keep the relative residual of every BiCGSTAB iteration of the
                                      last linear solve (up to that many entries); see pf_grid_history */
 #define PF_OPT_KERNELS        10  /* 0 = auto, 1 = direct (one thread per node, neighbours through L1/L2),
-                                     2 = tiled (planes staged in shared memory by TMA, z-marched; needs an
-                                     even nx >= 32, ny >= 16, nz >= 8 and 16-byte aligned vectors),
+                                     2 = tiled (planes staged in shared memory by TMA, z-marched; needs
+                                     nx >= 32, ny >= 16, nz >= 8, 16-byte aligned vectors, and for an odd nx
+                                     the on-the-fly stencil: the solve then runs on the box widened by one
+                                     column of decoupled identity rows),
                                      3 = cooperative (a whole solve in one persistent kernel, one brick of
                                      the box per SM with its vectors in shared memory, three grid-wide
                                      barriers per iteration; needs the on-the-fly stencil and a grid of at
