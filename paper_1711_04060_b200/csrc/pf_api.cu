@@ -603,7 +603,8 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     }
     PF_CREATE_CUDA(scan_eps(g->stream, g->g.n, eps_map, g->dmax_bits, &g->pal, &g->eps_min, &g->eps_max));
 #undef PF_CREATE_CUDA
-    if (!(g->eps_min > 0.0) || !std::isfinite(g->eps_max)) {
+    // (the scan orders bit patterns: a negative entry shows up as a 'maximum' below the minimum)
+    if (!(g->eps_min > 0.0) || !std::isfinite(g->eps_max) || !(g->eps_max >= g->eps_min)) {
         int rc = fail(nullptr, PF_ERR_ARG, "eps_map must be finite and > 0 (range %g..%g)", g->eps_min, g->eps_max);
         pf_grid_destroy(g);
         return rc;

@@ -32,26 +32,39 @@ struct ScanBuf {
     int overflow;
 };
 
-__global__ void k_scan_eps(long long n, const double* __restrict__ eps, ScanBuf* sb) {
+// Distinct values (up to PF_MAX_PALETTE + 1, then overflow), minimum and maximum of eps.  A thread keeps the
+// values it has met in registers and goes to the shared table only for a value that is new to it, so the scan
+// runs at memory speed (one 8-byte load and a few compares per node).
+__global__ void __launch_bounds__(ASM_THREADS) k_scan_eps(long long n, const double* __restrict__ eps, ScanBuf* sb) {
     unsigned long long lo = ~0ull, hi = 0ull;
+    unsigned long long known[PF_MAX_PALETTE + 1];
+    int nknown = 0;
+    bool lost = false;                  // more distinct values than the table holds
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
         const unsigned long long bits = (unsigned long long)__double_as_longlong(eps[i]);
         lo = bits < lo ? bits : lo;
         hi = bits > hi ? bits : hi;
-        bool found = false;
+        bool seen = lost;
+#pragma unroll
+        for (int k = 0; k <= PF_MAX_PALETTE; ++k) seen = seen || (k < nknown && known[k] == bits);
+        if (seen) continue;
+        bool found = false;                 // new to this thread: look in the shared table, claim a free slot if absent
         int k = 0;
         for (; k <= PF_MAX_PALETTE; ++k) {
             const unsigned long long v = ((volatile unsigned long long*)sb->tab)[k];
             if (v == bits) { found = true; break; }
             if (v == 0ull) break;
         }
-        if (found) continue;
-        for (; k <= PF_MAX_PALETTE; ++k) {
+        for (; !found && k <= PF_MAX_PALETTE; ++k) {
             const unsigned long long old = atomicCAS(&sb->tab[k], 0ull, bits);
-            if (old == 0ull || old == bits) { found = true; break; }
+            if (old == 0ull || old == bits) found = true;
         }
-        if (!found) sb->overflow = 1;
+        if (!found) { sb->overflow = 1; lost = true; continue; }
+#pragma unroll
+        for (int k = 0; k <= PF_MAX_PALETTE; ++k)
+            if (k == nknown) known[k] = bits;
+        ++nknown;
     }
     for (int d = 16; d > 0; d >>= 1) {
         unsigned long long a = __shfl_xor_sync(0xffffffffu, lo, d), b = __shfl_xor_sync(0xffffffffu, hi, d);
@@ -103,6 +116,14 @@ k_assemble_poisson(GridDims g, double h, BcDev bc, const double* __restrict__ ep
     const long long off[6] = {1, -1, -(long long)g.nx, (long long)g.nx, -(long long)g.nx * g.ny,
                               (long long)g.nx * g.ny};
     const int fbits = code_mode == 2 ? 4 : 2;
+    // With a palette the map has at most ten distinct face coefficients: each block forms them once (the same
+    // expression, so the same bits, as a node would) instead of two divisions per face and node.
+    __shared__ double pair_coeff[PF_CTAB];
+    if (code_mode && (int)threadIdx.x < pal.count * pal.count) {
+        const int a = threadIdx.x / pal.count, b = threadIdx.x % pal.count;
+        if (a <= b) pair_coeff[pair_index(a, b, pal.count)] = face_coeff(pal.value[a], pal.value[b], hh);
+    }
+    __syncthreads();
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
         int ix, iy, iz;
@@ -126,9 +147,14 @@ k_assemble_poisson(GridDims g, double h, BcDev bc, const double* __restrict__ ep
             double c = 0.0;
             if (in[d]) {
                 const double en = eps[i + off[d]];
-                c = face_coeff(ei, en, hh);
+                if (code_mode) {
+                    const int pj = pair_index(pi, palette_index(pal, en), pal.count);
+                    c = pair_coeff[pj];
+                    cw |= (unsigned int)pj << (fbits * d);
+                } else {
+                    c = face_coeff(ei, en, hh);
+                }
                 diag = add(diag, c);
-                if (code_mode) cw |= (unsigned int)pair_index(pi, palette_index(pal, en), pal.count) << (fbits * d);
             }
             if (offd[d]) offd[d][i] = in[d] ? -c : 0.0;
         }

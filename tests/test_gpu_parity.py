@@ -460,3 +460,24 @@ def test_odd_nx_auto_and_pf(pf):
         g.close()
     assert out[0]["outer_iters"] == out[1]["outer_iters"] and out[0]["lin_iters_hist"] == out[1]["lin_iters_hist"]
     assert torch.equal(out[0]["phi"], out[1]["phi"])
+
+
+def test_eps_scan(pf):
+    """The scan of the permittivity map: palette sizes 1..5+ with the values scattered so that every thread meets
+    them in a different order; maps with a negative, zero, NaN or infinite entry are rejected at grid creation."""
+    w = ragged_workload(nx=40, ny=33, nz=21, seed=13)
+    rng = np.random.default_rng(5)
+    vals = [2.0, 4.5, 20.0, 78.5, 80.0, 33.0]
+    for count in range(1, 7):
+        w.eps = rng.choice(vals[:count], size=w.n)
+        w.eps[: count] = vals[:count]                       # every value present
+        g = pf.Grid.from_workload(w)
+        assert pf.pf_grid_palette_size(g.handle) == min(count, 5), count      # 5 = "more than four"
+        assert pf.pf_grid_stencil(g.handle) == (2 if count <= 4 else 1)
+        g.close()
+    for bad in (-2.0, 0.0, float("nan"), float("inf")):
+        w.eps = np.full(w.n, 2.0)
+        w.eps[w.n // 3] = bad
+        with pytest.raises(pf.PFError) as e:
+            pf.Grid.from_workload(w)
+        assert e.value.code == pf.PF_ERR_ARG, bad
