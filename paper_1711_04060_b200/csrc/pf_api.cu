@@ -112,6 +112,7 @@ struct pf_grid {
     GridDims gk;
     bool padx;
     double *A0p, *bp, *xp;
+    double* offdp[6];          // stored variant: the six off-diagonals in the widened layout
     int coop_state;            // 0 not planned yet, 1 plan valid, -1 not applicable
     CoopPlan coop;
     int opt_stencil, opt_kernels, opt_check, opt_lin_maxit, opt_max_outer, opt_precond, opt_history;
@@ -188,7 +189,7 @@ int fail(pf_grid* g, int code, const char* fmt, ...) {
     } while (0)
 
 int n_vectors(bool stored, int charge_model, bool fixed_nodes, bool padx) {
-    return 19 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0) + (fixed_nodes ? 1 : 0) + (padx ? 3 : 0);
+    return 19 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0) + (fixed_nodes ? 1 : 0) + (padx ? 3 + (stored ? 6 : 0) : 0);
 }
 
 int code_mode_of(const pf_grid* g) { return g->pal.count > PF_MAX_PALETTE ? 0 : (g->pal.count <= 2 ? 1 : 2); }
@@ -460,12 +461,13 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
 // strides are multiples of 16 bytes): where the tiled kernels would otherwise apply, the system is embedded in the
 // box widened by one column x = nx of identity rows (diagonal 1, stencil code 0, b = x = 0): the extra unknowns are
 // decoupled and exactly 0 in every vector, so they add exact zeros to the inner products and the iterates of the
-// real unknowns keep their bits.  Costs eight vector passes per solve (about half an iteration).
+// real unknowns keep their bits.  Costs eight vector passes per solve (about half an iteration; twelve more with
+// stored coefficients).
 int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, double tol, int maxit,
                     int* iters_out, double* relres_out, double* true_relres_out) {
     CoopPlan plan;
-    const bool widen = g->padx && !op.stored && g->opt_kernels != 1 && g->opt_kernels != 3 && use_tiled(g, g->gk) &&
-                       !use_coop(g, op, &plan);
+    const bool widen = g->padx && (!op.stored || g->offdp[0]) && g->opt_kernels != 1 && g->opt_kernels != 3 &&
+                       use_tiled(g, g->gk) && !use_coop(g, op, &plan);
     if (!widen)
         return bicgstab_core(g, g->g, op, b, x, tol, maxit, iters_out, relres_out, true_relres_out, true, true);
     launch_widen(g->stream, g->g, op.A0, g->A0p, 1.0);
@@ -473,6 +475,8 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
     launch_widen(g->stream, g->g, x, g->xp, 0.0);
     Operator opk = op;
     opk.A0 = g->A0p;
+    if (op.stored)
+        for (int d = 0; d < 6; ++d) { launch_widen(g->stream, g->g, op.offd[d], g->offdp[d], 0.0); opk.offd[d] = g->offdp[d]; }
     const int rc = bicgstab_core(g, g->gk, opk, g->bp, g->xp, tol, maxit, iters_out, relres_out, true_relres_out, true, false);
     if (rc == PF_ERR_CUDA || rc == PF_ERR_ARG) return rc;
     launch_narrow(g->stream, g->g, g->xp, x);
@@ -548,6 +552,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     pf_grid* g = new pf_grid();
     g->g.nx = nx; g->g.ny = ny; g->g.nz = nz; g->g.n = (long long)nx * ny * nz;
     g->gk = g->g; g->padx = (nx & 1) != 0; g->A0p = g->bp = g->xp = nullptr;
+    for (int d = 0; d < 6; ++d) g->offdp[d] = nullptr;
     if (g->padx) { g->gk.nx = nx + 1; g->gk.n = (long long)(nx + 1) * ny * nz; }
     g->h = h;
     for (int f = 0; f < 6; ++f) { g->bc.type[f] = bc->type[f]; g->bc.value[f] = bc->value[f]; }
@@ -731,6 +736,7 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     if (g->charge_model == 1) { g->phiL = take(); g->phistar = take(); g->A0_L = take(); }
     g->fixv = g->fix_idx.empty() ? nullptr : take();
     if (g->padx) { g->A0p = take(); g->bp = take(); g->xp = take(); }
+    for (int d = 0; d < 6; ++d) g->offdp[d] = (g->padx && g->stored) ? take() : nullptr;
     for (int d = 0; d < 6; ++d) { g->offd[d] = g->stored ? take() : nullptr; }
     for (int d = 0; d < 6; ++d) { g->offd_pf1[d] = g->stored ? take() : nullptr; }
     g->code_mode = code_mode_of(g);

@@ -416,10 +416,10 @@ def test_tiled_kernels_odd_nx(pf, oracle, shape):
     rng = wl.SplitMix64(5)
     sigma = np.array([rng.uniform_range(0.0, 3.0) for _ in range(w.n)])
     x0 = np.array([rng.uniform_range(-1.0, 1.0) for _ in range(w.n)])
-    for sg, start in ((None, None), (sigma, x0)):
+    for sg, start, stencil in ((None, None, 2), (sigma, x0, 2), (sigma, None, 1)):     # 1: stored coefficients
         res = []
         for kernels in (1, 2):
-            g = pf.Grid.from_workload(w, stencil=2, kernels=kernels, options={pf.PF_OPT_HISTORY: 64})
+            g = pf.Grid.from_workload(w, stencil=stencil, kernels=kernels, options={pf.PF_OPT_HISTORY: 64})
             x = torch.zeros(w.n, dtype=torch.float64, device="cuda") if start is None else torch.tensor(start, device="cuda")
             out = g.solve_linear(w.rhs, x=x, tol=0.0, maxit=30, sigma=None if sg is None else torch.tensor(sg, device="cuda"))
             res.append((out["x"].clone(), g.history(64), out["true_relres"], out["iters"]))
