@@ -797,10 +797,21 @@ int pf_solve_linear(pf_grid* g, const double* rhs, double* x, const double* sigm
     if (rc) return rc;
     if (!rhs || !x) return fail(g, PF_ERR_ARG, "rhs and x must not be NULL");
     launch_copy_with_dirichlet(g->stream, g->g, g->bc, rhs, g->bw);   // Q20
-    launch_set_dirichlet(g->stream, g->g, g->bc, x);                   // Q4
+    // an iterate that is not 16-byte aligned (a view into a larger array) would keep the solve off the tiled
+    // kernels: it is solved in the workspace copy instead
+    double* xs = x;
+    const size_t nbytes = sizeof(double) * (size_t)g->g.n;
+    if (((uintptr_t)x & 15u) != 0 && x != g->xw) {
+        PF_CUDA(g, cudaMemcpyAsync(g->xw, x, nbytes, cudaMemcpyDeviceToDevice, g->stream));
+        xs = g->xw;
+    }
+    launch_set_dirichlet(g->stream, g->g, g->bc, xs);                  // Q4
     int which = 0;
     if (sigma) { launch_diag_plus_sigma(g->stream, g->g, g->bc, g->A0, sigma, g->A0_s); which = 2; }
-    return bicgstab_device(g, make_op(g, which), g->bw, x, tol, maxit, iters_out, relres_out, true_relres_out);
+    rc = bicgstab_device(g, make_op(g, which), g->bw, xs, tol, maxit, iters_out, relres_out, true_relres_out);
+    if (xs != x && rc != PF_ERR_CUDA && rc != PF_ERR_ARG)
+        PF_CUDA(g, cudaMemcpyAsync(x, xs, nbytes, cudaMemcpyDeviceToDevice, g->stream));
+    return rc;
 }
 
 int pf_solve_linear_host(pf_grid* g, const double* rhs_host, double* x_host, const double* sigma, double tol,

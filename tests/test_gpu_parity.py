@@ -481,3 +481,22 @@ def test_eps_scan(pf):
         with pytest.raises(pf.PFError) as e:
             pf.Grid.from_workload(w)
         assert e.value.code == pf.PF_ERR_ARG, bad
+
+
+def test_linear_unaligned_views(pf):
+    """rhs, x and sigma given as views that start 8 bytes into a larger allocation: same bits as with aligned
+    tensors (the iterate is solved in the workspace copy so that the tiled kernels still apply)."""
+    w = ragged_workload(nx=70, ny=37, nz=19, seed=9)
+    rng = wl.SplitMix64(8)
+    sigma = np.array([rng.uniform_range(0.0, 2.0) for _ in range(w.n)])
+    g = pf.Grid.from_workload(w, stencil=2, kernels=2)
+    ref = g.solve_linear(w.rhs, tol=0.0, maxit=20, sigma=torch.tensor(sigma, device="cuda"))
+    big = [torch.zeros(w.n + 1, dtype=torch.float64, device="cuda") for _ in range(3)]
+    rhs_v, x_v, sg_v = (b[1:] for b in big)
+    assert rhs_v.data_ptr() % 16 == 8
+    rhs_v.copy_(torch.tensor(w.rhs)); sg_v.copy_(torch.tensor(sigma))
+    out = pf.pf_solve_linear(g.handle, w.n, rhs_v, x_v, 0.0, 20, sigma=sg_v)
+    assert out["iters"] == 20 and out["true_relres"] == ref["true_relres"]
+    assert torch.equal(x_v, ref["x"])
+    assert pf.pf_grid_fault_repeats(g.handle) == 0
+    g.close()
