@@ -38,6 +38,7 @@
 
 #include <cuda.h>      // CUtensorMap and its enums (types only; the encoder is fetched at run time)
 #include <algorithm>
+#include <type_traits>
 #include <cstring>
 
 namespace pf {
@@ -375,7 +376,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             // one basic block: the divisions of plane z+1 and the stencil chain of plane z are independent and
             // get interleaved by the scheduler.  Nodes outside the grid see zero operands and zero codes, give
             // exact zeros and add nothing to the inner products; only their stores are predicated.
-            auto load_slot = [&](int k, Slot& up, bool to_shared) {
+            auto load_slot = [&](int k, Slot& up, bool to_shared, double* u_dst = nullptr) {
                 const unsigned char* st = wait_full(k);
                 const int z = z0 - 1 + k;
                 const bool ok = pair_ok && z >= 0 && z < g.nz;
@@ -392,16 +393,33 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 }
                 if (MODE == MODE_K1 && ok && z >= z0 && z < z1)         // p' is an output of steps 5-9
                     *reinterpret_cast<double2*>(kv.p_out + own_off + plane * z) = make_double2(up.n[0], up.n[1]);
-                if (to_shared) *reinterpret_cast<double2*>(u_buf(k) + pair_box) = make_double2(up.u[0], up.u[1]);
+                if (to_shared)
+                    *reinterpret_cast<double2*>((u_dst ? u_dst : u_buf(k)) + pair_box) = make_double2(up.u[0], up.u[1]);
             };
             constexpr bool DEFER = !STORED;                  // the stored variant has no registers to spare for it
             double pa[2] = {0.0, 0.0}, pb[2] = {0.0, 0.0};   // operands of the deferred inner products (zeros add nothing)
-            auto step = [&](int z, const Slot& dn, const Slot& c, Slot& up) {
+            // The loop below is unrolled three ways and NU = 3, so the u buffer of plane z0 + 3m + J is a fixed
+            // rotation J of the item's first one and the parity of its `ready` barrier a fixed bit xor (m & 1):
+            // three pointers and three bits per item instead of a division by 3 per plane and use.
+            static_assert(NU == 3, "the rotation below is written for three u buffers");
+            const int ub3 = ub % NU;
+            int bj[3];                                                  // buffer of rotation j
+            unsigned pbits = 0u;                                        // bit j: parity of rotation j at m = 0
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                bj[j] = ub3 + j >= NU ? ub3 + j - NU : ub3 + j;
+                pbits |= ((unsigned)(ub / NU + (ub3 + j >= NU ? 1 : 0)) & 1u) << j;
+            }
+            unsigned mp = 0u;                                           // (z - z0) / 3 & 1
+            auto U = [&](int j) { return reinterpret_cast<double*>(smem + L::U_OFF + bj[j] * FIELD_BYTES); };
+            auto R = [&](int j) { return &ready[bj[j]]; };
+            auto step = [&](auto Jc, int z, const Slot& dn, const Slot& c, Slot& up) {
+                constexpr int J = decltype(Jc)::value, J1 = (J + 1) % 3;
                 const int k = z - z0 + 1;                               // load-sequence index of plane z
                 const long long i = own_off + plane * z;
-                const double* u_s = u_buf(k);
-                wait_ready(k);
-                load_slot(k + 1, up, true);
+                const double* u_s = U(J);                               // == u_buf(k)
+                { const unsigned par = ((pbits >> J) & 1u) ^ mp; while (!mbar_try_wait(R(J), par)) {} }   // == wait_ready(k)
+                load_slot(k + 1, up, true, U(J1));
                 // inner products of the PREVIOUS plane: a third independent chain beside the divisions of plane
                 // z+1 and the 7-point sums of plane z
                 if (DEFER && MODE == MODE_K1) {
@@ -444,7 +462,8 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     out[e] = acc;
                     c5[e] = cc[5];
                 }
-                publish(k + 1);                                         // u(z+1) is in shared memory
+                __syncwarp();                                           // == publish(k + 1): u(z+1) is in shared memory
+                if (lane == 0) { mbar_arrive(R(J1)); mbar_arrive(&empty[(sb + k + 1) % NS]); }
                 out[0] = add(out[0], mul(c5[0], up.u[0]));
                 out[1] = add(out[1], mul(c5[1], up.u[1]));
                 if (MODE == MODE_K1) {
@@ -479,11 +498,12 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             if (ub >= 1) wait_ready(0);            // last plane of the previous item: its buffer-mates are free
             load_slot(1, s1, true);  publish(1);   // plane z0
             for (int z = z0; z < z1; z += 3) {     // slots rotate by renaming, not by moving registers
-                step(z, s0, s1, s2);
+                step(std::integral_constant<int, 0>{}, z, s0, s1, s2);
                 if (z + 1 >= z1) break;
-                step(z + 1, s1, s2, s0);
+                step(std::integral_constant<int, 1>{}, z + 1, s1, s2, s0);
                 if (z + 2 >= z1) break;
-                step(z + 2, s2, s0, s1);
+                step(std::integral_constant<int, 2>{}, z + 2, s2, s0, s1);
+                mp ^= 1u;
             }
             if (DEFER && MODE == MODE_K1) {                  // the last plane's inner products
                 dd_fma(q[0], pa[0], pb[0]); dd_fma(q[1], pa[1], pb[1]);
