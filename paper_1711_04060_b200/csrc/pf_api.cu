@@ -358,8 +358,7 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
         tiled = false;
     }
     if (g->opt_kernels == 2 && allow_tiled && !tiled)
-        return fail(g, PF_ERR_ARG, "the tiled kernels need 16-byte aligned vectors and an even nx (an odd nx only with "
-                                   "the on-the-fly stencil)");
+        return fail(g, PF_ERR_ARG, "the tiled kernels need 16-byte aligned vectors");
     // Small grids: the whole solve in one cooperative kernel (pf_krylov_coop.cu)
     CoopPlan plan;
     const bool coop = allow_tiled && allow_coop && use_coop(g, op, &plan);

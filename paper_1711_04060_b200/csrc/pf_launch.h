@@ -53,7 +53,8 @@ void launch_finalize(const LaunchCtx& c, double* hist);
 void launch_finish_x(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv);
 
 // Tiled family (pf_krylov_tma.cu): TMA-staged planes, z-marched.  Needs an even nx (16-byte row
-// strides) and 16-byte aligned vectors; tma_supported() says whether the grid qualifies.
+// strides; the driver widens an odd-nx box by one column of identity rows, pf_api.cu bicgstab_device) and
+// 16-byte aligned vectors; tma_supported() says whether the grid qualifies.
 struct TmaSet;                                   // tensor maps of one solve (opaque here)
 bool tma_available();                            // driver entry point for tensor-map encoding found
 bool tma_supported(const GridDims& g);
