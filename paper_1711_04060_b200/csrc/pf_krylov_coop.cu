@@ -22,9 +22,9 @@
 // A wait is bounded: a block that does not see the arrivals within about a second sets the abort flag and leaves
 // (the host reports PF_ERR_CUDA); the cooperative launch makes that unreachable in normal operation.
 //
-// Measured (B200, profiles/r1_coop.md): a barrier-reduction costs about 3.5 us (two block-wide double-double
-// trees, a fence, the atomic round trip, the record reads), so an iteration costs 13.5 us at 32^3 and 23 us at
-// 64^3 against 23 / 25.6 us for three launches; a flag per block polled by all blocks was 2x slower (hot lines),
+// Measured (B200, profiles/r1_coop.md): a barrier-reduction costs 2.5-3.5 us (two block-wide double-double
+// trees, a fence, the atomic round trip, the record reads), so an iteration costs 12 us at 32^3 and 19 us at
+// 64^3 against 16-22 / 24 us for three launches; a flag per block polled by all blocks was 2x slower (hot lines),
 // cooperative_groups' grid.sync() alone costs 1.2 us.
 #include <algorithm>
 #include <cstring>
