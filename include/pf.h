@@ -61,7 +61,7 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
 #define PF_OPT_LINEAR_TOL      3  /* relative tolerance of the solves inside pf_solve_pf; default 1e-10 */
 #define PF_OPT_LINEAR_MAXIT    4  /* their iteration cap; default 10000 */
 #define PF_OPT_CHECK_INTERVAL  5  /* BiCGSTAB iterations enqueued between two host polls of the
-                                     device-side convergence flag; default 16; >= 1 */
+                                     device-side convergence flag (PF_OPT_GRAPH 0 and 1); default 16; >= 1 */
 #define PF_OPT_WATER_MOLAR     6  /* bath concentration of water, mol/L; default 55.5 (Q12) */
 #define PF_OPT_MAX_OUTER       7  /* cap on outer (Newton) iterations; default 1000 */
 #define PF_OPT_PRECOND         8  /* 1 = Jacobi M = diag(A) (default, reading Q2); 0 = M = I, Table 3 verbatim */
@@ -81,8 +81,13 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
                                      linear solve with CUDA events and accumulate their durations
                                      (pf_grid_profile); setting it resets the sums; 0 = off */
 
-#define PF_OPT_GRAPH          12  /* 1 (default): on grids of up to 2^22 unknowns, which are bound by launch latency,
-                                     replay each polling chunk of iterations as one CUDA graph; 0 = plain launches */
+#define PF_OPT_GRAPH          12  /* how the iterations of a linear solve reach the GPU (three-kernel families).
+                                     2 (default): one CUDA graph launch per solve whose WHILE conditional node repeats
+                                     a body of 8 or 16 iterations on the device until the solve is over (converged, maxit,
+                                     breakdown); the host does not poll.  1: each polling chunk of
+                                     PF_OPT_CHECK_INTERVAL iterations is replayed as one CUDA graph, the host polls the
+                                     device-side flag between chunks.  0: plain stream launches, polled.  All three give
+                                     the same bits.  2 falls back to 1, and 1 to 0, if the graph cannot be built. */
 
 #define PF_OPT_NORM           13  /* stopping test of every linear solve.  0 (default, reading Q3): ||r||_2 <= tol ||b||_2;
                                      1: the paper's own test, Table 3 steps 18-19: ||r||_inf < tol,

@@ -45,6 +45,11 @@ struct SmallSet {
     char* host = nullptr;           // pinned, 2 x 256 bytes
     cudaEvent_t ev[2] = {nullptr, nullptr};
 };
+// Iterations per turn of the device-side loop (even: the (p, v) double buffers are back in place).  A turn costs 6-7 us
+// (the body drains, the condition is read, the body is launched again), the kernels that return at once after
+// the end of the solve 1.5-8 us each: short solves (the inner solves of a PF iteration, 40-100 iterations) want the
+// short body, long ones the long body.  The choice follows the previous solve with the same operator.
+constexpr int LOOP_BODY_SHORT = 8, LOOP_BODY_LONG = 16, LOOP_LONG_SOLVE = 192;
 constexpr long long COOP_AUTO_MAX_N = 64ll * 64 * 64;     // largest grid the cooperative solver is chosen for by itself
                                                           // (measured: 1.1x at 64^3 to 1.7x at 32^3 over the next best family)
 constexpr size_t SS_SC = 0 /* two copies, 256 bytes each */, SS_FAULT = 512, SS_DMAX = 768, SS_CTAB0 = 1024,
@@ -153,6 +158,7 @@ struct pf_grid {
     // CUDA graphs of one polling chunk of iterations, for grids small enough to be launch-bound
     struct ChunkGraph { const void *a0, *code, *b, *x, *y, *hist; int precond, tiled, chunk; cudaGraphExec_t exec; };
     std::vector<ChunkGraph> graphs;
+    std::vector<std::pair<const void*, int>> solve_len;     // iterations of the last solve per operator (by its A0)
     cudaStream_t capture_stream;
     int opt_graph;
     int opt_norm;            // 0: relative 2-norm (Q3), 1: the paper's absolute maximum norm
@@ -306,6 +312,61 @@ cudaGraphExec_t chunk_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, 
     return exec;
 }
 
+// The whole iteration loop on the device: a graph whose only node is a WHILE conditional node with a body of `body`
+// iterations (an even number).  Every kernel of the body, once it has taken the scalar step its predecessor left
+// pending, sets the node's condition to "the solve is not over" (begin_kernel, ReduceBuf::more), so the device
+// repeats the body until the state says done (converged, maxit, breakdown) and the kernels of at most one more
+// body return at once: no host poll, no chunk enqueued ahead.  A loop turn costs 1 us with empty kernels and 6-7 us
+// with these (B200, driver 580; profiles/r1_v8_loop.md).  Cached like the chunk graphs (chunk = -body).  Null when it cannot be built.
+cudaGraphExec_t loop_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool tiled,
+                           bool precond, int body) {
+    if (g->opt_graph != 2 || (body & 1) || body < 2) return nullptr;
+    for (const auto& cg : g->graphs)
+        if (cg.a0 == op.A0 && cg.code == op.code && cg.b == kv.b && cg.x == kv.x && cg.y == kv.y && cg.hist == kv.hist &&
+            cg.precond == (int)precond && cg.tiled == (int)tiled && cg.chunk == -body)
+            return cg.exec;
+    if (!g->capture_stream &&
+        cudaStreamCreateWithFlags(&g->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError(); g->opt_graph = 1; return nullptr;
+    }
+    LaunchCtx cc = c;
+    cc.stream = g->capture_stream; cc.pdl = false;
+    KrylovVecs kc = kv;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    const long long launches0 = pf::g_launch_count;
+    cudaGraphConditionalHandle more;
+    bool ok = cudaGraphCreate(&graph, 0) == cudaSuccess &&
+              cudaGraphConditionalHandleCreate(&more, graph, 1, cudaGraphCondAssignDefault) == cudaSuccess;
+    if (ok) {
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = more;
+        np.conditional.type = cudaGraphCondTypeWhile;
+        np.conditional.size = 1;
+        cudaGraphNode_t node;
+        ok = cudaGraphAddNode(&node, graph, nullptr, 0, &np) == cudaSuccess;
+        if (ok) ok = cudaStreamBeginCaptureToGraph(cc.stream, np.conditional.phGraph_out[0], nullptr, nullptr, 0,
+                                                   cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+        if (ok) {
+            cc.rb.more = (unsigned long long)more;
+            for (int k = 0; k < body; ++k) enqueue_iteration(cc, op, kc, g->tma, tiled, precond, k & 1, nullptr);
+            cudaGraph_t captured = nullptr;
+            ok = cudaStreamEndCapture(cc.stream, &captured) == cudaSuccess;
+        }
+    }
+    pf::g_launch_count = launches0;            // nothing ran; the kernels of a loop are counted after the solve
+    if (ok) ok = cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess;
+    if (graph) cudaGraphDestroy(graph);
+    if (!ok) { cudaGetLastError(); g->opt_graph = 1; return nullptr; }     // back to polled chunk replays
+    if (g->graphs.size() >= 16) {
+        cudaGraphExecDestroy(g->graphs.front().exec);
+        g->graphs.erase(g->graphs.begin());
+    }
+    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled, -body, exec});
+    return exec;
+}
+
 // Tail of a linear solve: Q3, the true residual of the returned x (row L8) and the outputs.
 int finish_solve(pf_grid* g, const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, Scalars fin, bool tiled,
                  int* iters_out, double* relres_out, double* true_relres_out) {
@@ -402,6 +463,37 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
     std::memset(&fin, 0, sizeof(fin));
     // Pipelined polling: enqueue chunk k+1 before waiting for the flag copy of chunk k, so the GPU
     // never idles on the host; kernels launched after convergence return at once (sc->done).
+    // Device-side loop (PF_OPT_GRAPH = 2): the iterations that are bracketed by profiling events are launched one by
+    // one, all others run as ONE graph launch whose WHILE node repeats a body of LOOP_BODY iterations until the
+    // device-side state says done; the host only waits for the final scalars.
+    const int nprof_all = g->opt_profile ? std::min(maxit & ~1, ((int)(g->prof_ev.size() / 4) + 1) & ~1) : 0;
+    int* prev_len = nullptr;
+    for (auto& e : g->solve_len) if (e.first == op.A0) prev_len = &e.second;
+    if (!prev_len) {
+        if (g->solve_len.size() >= 8) g->solve_len.erase(g->solve_len.begin());
+        g->solve_len.push_back({op.A0, LOOP_LONG_SOLVE});
+        prev_len = &g->solve_len.back().second;
+    }
+    const int LOOP_BODY = std::min(maxit, *prev_len) >= LOOP_LONG_SOLVE ? LOOP_BODY_LONG : LOOP_BODY_SHORT;
+    cudaGraphExec_t loop = (g->opt_graph == 2 && maxit - nprof_all > 0)
+                               ? loop_graph(g, c, op, kv, tiled, precond, LOOP_BODY) : nullptr;
+    if (loop) {
+        for (int k = 0; k < nprof_all; ++k) {
+            const bool prof = (size_t)(4 * k + 3) < g->prof_ev.size();
+            enqueue_iteration(c, op, kv, g->tma, tiled, precond, k & 1, prof ? &g->prof_ev[4 * k] : nullptr);
+        }
+        PF_CUDA(g, cudaGraphLaunch(loop, g->stream));
+        launch_finalize(c, kv.hist);          // the scalar step the last kernel left pending
+        PF_CUDA(g, cudaMemcpyAsync(g->sc_host[0], c.current_scalars(), sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
+        PF_CUDA(g, cudaStreamSynchronize(g->stream));
+        fin = *g->sc_host[0];
+        // kernels the loop ran: whole bodies of 3 per iteration; the body in which the last iteration ran is the last
+        // one unless that iteration was the body's last (its k3's step is then taken by the next body's first kernel)
+        const int in_loop = std::max(fin.it - nprof_all, 0);
+        pf::g_launch_count += 3ll * LOOP_BODY * (in_loop / LOOP_BODY + 1);
+        *prev_len = fin.it;
+        done = true;
+    }
     while (!done) {
         int todo = std::min(chunk, maxit - launched);
         // iterations that are bracketed by profiling events are launched one by one (an even number of them, so
@@ -573,11 +665,11 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->opt_profile = 0; g->prof_ms[0] = g->prof_ms[1] = g->prof_ms[2] = 0.0;
     g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
-    g->capture_stream = nullptr; g->opt_graph = 1; g->opt_norm = 0;
+    g->capture_stream = nullptr; g->opt_graph = 2; g->opt_norm = 0;
     g->opt_charge_model = 0; g->charge_model = 0; g->phiL = g->phistar = g->A0_L = nullptr; g->code_L = nullptr;
     g->ctab_L = nullptr; g->laplace_iters = 0; g->fixv = nullptr; g->bc.fixv = nullptr;
     g->small = nullptr;
-    g->charges_dev = nullptr; g->sc[0] = g->sc[1] = nullptr; g->flip = 0; g->rb.partial = nullptr; g->rb.fault = nullptr;
+    g->charges_dev = nullptr; g->sc[0] = g->sc[1] = nullptr; g->flip = 0; g->rb.partial = nullptr; g->rb.fault = nullptr; g->rb.more = 0;
     g->ctab_poisson = g->ctab_pf1 = nullptr; g->dmax_bits = nullptr; g->tma = nullptr;
     g->code = g->code_pf1 = nullptr; g->code_mode = 0; g->cpitch = 0;
     g->sc_host[0] = g->sc_host[1] = nullptr; g->ev[0] = g->ev[1] = nullptr;
@@ -711,7 +803,8 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
                 return fail(g, PF_ERR_ARG, "set the charge model before pf_grid_set_workspace");
             g->opt_charge_model = iv; return PF_OK;
         case PF_OPT_GRAPH:
-            g->opt_graph = iv != 0; return PF_OK;
+            if (iv < 0 || iv > 2) return fail(g, PF_ERR_ARG, "graph must be 0, 1 or 2");
+            g->opt_graph = iv; return PF_OK;
         case PF_OPT_KERNELS:
             if (iv < 0 || iv > 3) return fail(g, PF_ERR_ARG, "kernels must be 0, 1, 2 or 3");
             if (iv == 2 && !(tma_supported(g->gk) && tma_available()))

@@ -128,6 +128,8 @@ __device__ __forceinline__ bool begin_kernel(int kind, Scalars* S, const Scalars
         S->pending_nblk = (int)linear_grid_size();
         if (kind == PEND_NONE) S->fault = *rb.fault;             // finalize: what the host is about to read
         if (lead) *sc_out = *S;
+        // body of a device-side loop: the last kernel of the body that knows decides whether there is another turn
+        if (lead && rb.more && kind != PEND_NONE) cudaGraphSetConditional((cudaGraphConditionalHandle)rb.more, S->done ? 0u : 1u);
     }
     __syncthreads();
     return S->pending != PEND_NONE;

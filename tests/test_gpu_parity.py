@@ -500,3 +500,62 @@ def test_linear_unaligned_views(pf):
     assert torch.equal(x_v, ref["x"])
     assert pf.pf_grid_fault_repeats(g.handle) == 0
     g.close()
+
+
+@pytest.mark.parametrize("kernels", [1, 2])
+def test_device_loop_equals_polled_launches(pf, kernels):
+    """PF_OPT_GRAPH 0 (stream launches, host polls), 1 (graph replays of polling chunks) and 2 (one graph whose WHILE
+    node repeats the iterations on the device until the solve is over) run the same kernels on the same state: same
+    iterate, residual history, iteration count and status -- for solves that end inside a loop body, at its last
+    iteration, at maxit (odd and even, below and above one body), before the first iteration, and with the first
+    iterations bracketed by profiling events."""
+    w = ragged_workload(nx=66, ny=35, nz=23, seed=77)
+    cases = [dict(tol=1e-10, maxit=10000), dict(tol=0.0, maxit=1), dict(tol=0.0, maxit=7), dict(tol=0.0, maxit=8),
+             dict(tol=0.0, maxit=16), dict(tol=0.0, maxit=21), dict(tol=1e-3, maxit=10000), dict(tol=1e30, maxit=10)]
+    res = {}
+    for mode in (0, 1, 2):
+        g = pf.Grid.from_workload(w, kernels=kernels, options={pf.PF_OPT_GRAPH: mode, pf.PF_OPT_HISTORY: 512})
+        res[mode] = []
+        for c in cases:
+            out = g.solve_linear(w.rhs, **c)
+            res[mode].append((out["x"].clone(), g.history(512), out["iters"], out["status"], out["true_relres"]))
+        g.set_option(pf.PF_OPT_PROFILE, 3)           # four iterations launched one by one, the rest in the loop
+        out = g.solve_linear(w.rhs, tol=1e-10)
+        res[mode].append((out["x"].clone(), g.history(512), out["iters"], out["status"], out["true_relres"]))
+        g.close()
+    assert res[0][0][3] == 0 and res[0][0][2] > 16       # the converged case runs over several bodies
+    # every iteration count 9..24 ends somewhere else in a body of 8 and in a polling chunk of 16
+    for k, ref in enumerate(res[0]):
+        for mode in (1, 2):
+            got = res[mode][k]
+            assert torch.equal(got[0], ref[0]), (mode, k)
+            assert np.array_equal(got[1], ref[1]) and got[2:] == ref[2:], (mode, k)
+
+
+def test_device_loop_every_exit_position(pf):
+    """The solve ends at every position of a loop body: maxit = 9..25 with tol = 0, and tolerances that stop the
+    solve at consecutive iteration counts; the launch counter follows the bodies that ran."""
+    w = ragged_workload(nx=40, ny=24, nz=16, seed=78)
+    g1 = pf.Grid.from_workload(w, kernels=2, options={pf.PF_OPT_GRAPH: 1, pf.PF_OPT_HISTORY: 64})
+    g2 = pf.Grid.from_workload(w, kernels=2, options={pf.PF_OPT_GRAPH: 2, pf.PF_OPT_HISTORY: 64})
+    fixed = set()
+    for maxit in range(9, 26):
+        a = g1.solve_linear(w.rhs, tol=0.0, maxit=maxit)
+        n0 = pf.pf_launch_count()
+        b = g2.solve_linear(w.rhs, tol=0.0, maxit=maxit, true_residual=False)
+        launched = pf.pf_launch_count() - n0
+        assert a["iters"] == b["iters"] == maxit and torch.equal(a["x"], b["x"]), maxit
+        # whole bodies of 8 iterations (one more when the last iteration closes a body) + the solve's fixed launches
+        # (Dirichlet values into b and x, residual kernel, finalize, x = x0 + M^-1 y)
+        fixed.add(launched - 24 * (maxit // 8 + 1))
+    assert len(fixed) == 1 and 3 <= fixed.pop() <= 8
+    hist = g1.history(64)
+    hist = hist[np.isfinite(hist)]
+    for it in range(10, 19):                       # stop right after iteration `it`
+        tol = float(np.sqrt(hist[it] * hist[it - 1])) if hist[it] < hist[it - 1] else None
+        if tol is None:
+            continue
+        a = g1.solve_linear(w.rhs, tol=tol)
+        b = g2.solve_linear(w.rhs, tol=tol)
+        assert a["iters"] == b["iters"] and a["status"] == b["status"] == 0 and torch.equal(a["x"], b["x"]), it
+    g1.close(); g2.close()
