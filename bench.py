@@ -50,6 +50,12 @@ def parse():
                          "(100 fixed iterations + one PF pass, BASELINE.json configs[4])")
     ap.add_argument("--stencil", choices=["onthefly", "stored"], default="onthefly")
     ap.add_argument("--kernels", choices=["auto", "direct", "tiled"], default="auto")
+    ap.add_argument("--launch-mode", choices=["auto", "loop", "chunks", "stream"], default="auto",
+                    help="how the iterations reach the GPU (PF_OPT_GRAPH): auto = library default (device-side loop for "
+                         "short solves, polled graph replays for long ones); loop = one graph per solve whose WHILE "
+                         "node repeats the iterations on the device; chunks = graph replays of 16 iterations polled "
+                         "by the host (ncu does not profile kernel nodes of graphs with conditional nodes: launch "
+                         "lists are taken with this mode); stream = plain launches")
     ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -230,6 +236,7 @@ def run_b200(args):
         pf.pf_grid_set_option(h, pf.PF_OPT_STENCIL, stencil)
         if kernels:
             pf.pf_grid_set_option(h, pf.PF_OPT_KERNELS, kernels)
+        pf.pf_grid_set_option(h, pf.PF_OPT_GRAPH, {"auto": 3, "loop": 2, "chunks": 1, "stream": 0}[args.launch_mode])
         pf.pf_grid_set_option(h, pf.PF_OPT_LINEAR_TOL, 0.0)
         pf.pf_grid_set_option(h, pf.PF_OPT_LINEAR_MAXIT, PF_INNER_ITERS)
         pf.pf_grid_set_option(h, pf.PF_OPT_MAX_OUTER, 1)
@@ -344,7 +351,7 @@ def run_b200(args):
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": f"{wdesc}; step = assembly + {lin_iters} fixed Jacobi-BiCGSTAB iterations + "
                                        f"one PF outer pass with 3x{PF_INNER_ITERS} inner iterations",
-                           "stencil": args.stencil, "kernels": args.kernels, "unknowns": n,
+                           "stencil": args.stencil, "kernels": args.kernels, "launch_mode": args.launch_mode, "unknowns": n,
                            "iterations_per_step": step_iters, "parallelism": "replicas only" if world > 1 else "1 GPU",
                            "l2": "inputs larger than L2 (working set %.1f GB)" % (ws.numel() / 1e9)},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,

@@ -82,12 +82,16 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
                                      (pf_grid_profile); setting it resets the sums; 0 = off */
 
 #define PF_OPT_GRAPH          12  /* how the iterations of a linear solve reach the GPU (three-kernel families).
-                                     2 (default): one CUDA graph launch per solve whose WHILE conditional node repeats
-                                     a body of 8 or 16 iterations on the device until the solve is over (converged, maxit,
-                                     breakdown); the host does not poll.  1: each polling chunk of
-                                     PF_OPT_CHECK_INTERVAL iterations is replayed as one CUDA graph, the host polls the
-                                     device-side flag between chunks.  0: plain stream launches, polled.  All three give
-                                     the same bits.  2 falls back to 1, and 1 to 0, if the graph cannot be built. */
+                                     0: plain stream launches; the host polls the device-side flag every
+                                     PF_OPT_CHECK_INTERVAL iterations.  1: each polling chunk is replayed as one CUDA
+                                     graph.  2: device-side loop -- one CUDA graph launch per solve whose WHILE
+                                     conditional node repeats a body of 8 or 16 iterations until the solve is over
+                                     (converged, breakdown) or the whole bodies below maxit are done; the host does not
+                                     poll; the fewer-than-a-body iterations up to maxit follow as stream launches.
+                                     3 (default): 2 for solves expected to take fewer than 192 iterations (by the
+                                     previous solve with the same operator, e.g. the inner solves of pf_solve_pf),
+                                     1 for longer ones.  All give the same bits.  2 falls back to 1, and 1 to 0, if a
+                                     graph cannot be built. */
 
 #define PF_OPT_NORM           13  /* stopping test of every linear solve.  0 (default, reading Q3): ||r||_2 <= tol ||b||_2;
                                      1: the paper's own test, Table 3 steps 18-19: ||r||_inf < tol,

@@ -313,14 +313,14 @@ cudaGraphExec_t chunk_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, 
 }
 
 // The whole iteration loop on the device: a graph whose only node is a WHILE conditional node with a body of `body`
-// iterations (an even number).  Every kernel of the body, once it has taken the scalar step its predecessor left
-// pending, sets the node's condition to "the solve is not over" (begin_kernel, ReduceBuf::more), so the device
+// iterations (an even number).  The k3 of every iteration, once it has taken the scalar step its predecessor left
+// pending, sets the node's condition to "the solve is not over" (begin_kernel<true>, ReduceBuf::more), so the device
 // repeats the body until the state says done (converged, maxit, breakdown) and the kernels of at most one more
 // body return at once: no host poll, no chunk enqueued ahead.  A loop turn costs 1 us with empty kernels and 6-7 us
 // with these (B200, driver 580; profiles/r1_v8_loop.md).  Cached like the chunk graphs (chunk = -body).  Null when it cannot be built.
 cudaGraphExec_t loop_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool tiled,
                            bool precond, int body) {
-    if (g->opt_graph != 2 || (body & 1) || body < 2) return nullptr;
+    if (g->opt_graph < 2 || (body & 1) || body < 2) return nullptr;
     for (const auto& cg : g->graphs)
         if (cg.a0 == op.A0 && cg.code == op.code && cg.b == kv.b && cg.x == kv.x && cg.y == kv.y && cg.hist == kv.hist &&
             cg.precond == (int)precond && cg.tiled == (int)tiled && cg.chunk == -body)
@@ -404,6 +404,24 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
     Scalars init;
     std::memset(&init, 0, sizeof(init));
     init.tol = tol; init.maxit = maxit; init.hist_cap = g->hist ? g->hist_cap : 0; init.norm_mode = g->opt_norm;
+    // How the iterations reach the GPU (PF_OPT_GRAPH).  The iterations that are bracketed by profiling events are
+    // launched one by one (an even number of them); of the others, a device-side loop runs the whole bodies that fit
+    // below maxit and the rest follows as stream launches.  Auto: the loop for solves expected to be short (the inner
+    // solves of a PF iteration: what counts is what is left behind after convergence), polled graph replays for long
+    // ones (what counts is the cost per iteration); the expectation is the previous solve with the same operator.
+    const int nprof_all = g->opt_profile ? std::min(maxit & ~1, ((int)(g->prof_ev.size() / 4) + 1) & ~1) : 0;
+    int* prev_len = nullptr;
+    for (auto& e : g->solve_len) if (e.first == op.A0) prev_len = &e.second;
+    if (!prev_len) {
+        if (g->solve_len.size() >= 8) g->solve_len.erase(g->solve_len.begin());
+        g->solve_len.push_back({op.A0, LOOP_LONG_SOLVE});
+        prev_len = &g->solve_len.back().second;
+    }
+    const bool expect_long = std::min(maxit, *prev_len) >= LOOP_LONG_SOLVE;
+    const int LOOP_BODY = expect_long ? LOOP_BODY_LONG : LOOP_BODY_SHORT;
+    const int loop_end = nprof_all + (maxit - nprof_all) / LOOP_BODY * LOOP_BODY;
+    const bool want_loop = (g->opt_graph == 2 || (g->opt_graph == 3 && !expect_long)) && loop_end > nprof_all;
+    init.loop_end = loop_end;
     // pageable source: the runtime stages it before returning, so a stack object is safe
     g->flip = 0;
     PF_CUDA(g, cudaMemcpyAsync(g->sc[0], &init, sizeof(init), cudaMemcpyHostToDevice, g->stream));
@@ -463,35 +481,25 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
     std::memset(&fin, 0, sizeof(fin));
     // Pipelined polling: enqueue chunk k+1 before waiting for the flag copy of chunk k, so the GPU
     // never idles on the host; kernels launched after convergence return at once (sc->done).
-    // Device-side loop (PF_OPT_GRAPH = 2): the iterations that are bracketed by profiling events are launched one by
-    // one, all others run as ONE graph launch whose WHILE node repeats a body of LOOP_BODY iterations until the
-    // device-side state says done; the host only waits for the final scalars.
-    const int nprof_all = g->opt_profile ? std::min(maxit & ~1, ((int)(g->prof_ev.size() / 4) + 1) & ~1) : 0;
-    int* prev_len = nullptr;
-    for (auto& e : g->solve_len) if (e.first == op.A0) prev_len = &e.second;
-    if (!prev_len) {
-        if (g->solve_len.size() >= 8) g->solve_len.erase(g->solve_len.begin());
-        g->solve_len.push_back({op.A0, LOOP_LONG_SOLVE});
-        prev_len = &g->solve_len.back().second;
-    }
-    const int LOOP_BODY = std::min(maxit, *prev_len) >= LOOP_LONG_SOLVE ? LOOP_BODY_LONG : LOOP_BODY_SHORT;
-    cudaGraphExec_t loop = (g->opt_graph == 2 && maxit - nprof_all > 0)
-                               ? loop_graph(g, c, op, kv, tiled, precond, LOOP_BODY) : nullptr;
+    cudaGraphExec_t loop = want_loop ? loop_graph(g, c, op, kv, tiled, precond, LOOP_BODY) : nullptr;
     if (loop) {
         for (int k = 0; k < nprof_all; ++k) {
             const bool prof = (size_t)(4 * k + 3) < g->prof_ev.size();
             enqueue_iteration(c, op, kv, g->tma, tiled, precond, k & 1, prof ? &g->prof_ev[4 * k] : nullptr);
         }
         PF_CUDA(g, cudaGraphLaunch(loop, g->stream));
+        for (int k = loop_end; k < maxit; ++k)      // fewer than a body; they return at once if the solve is over
+            enqueue_iteration(c, op, kv, g->tma, tiled, precond, k & 1, nullptr);
         launch_finalize(c, kv.hist);          // the scalar step the last kernel left pending
         PF_CUDA(g, cudaMemcpyAsync(g->sc_host[0], c.current_scalars(), sizeof(Scalars), cudaMemcpyDeviceToHost, g->stream));
         PF_CUDA(g, cudaStreamSynchronize(g->stream));
         fin = *g->sc_host[0];
-        // kernels the loop ran: whole bodies of 3 per iteration; the body in which the last iteration ran is the last
-        // one unless that iteration was the body's last (its k3's step is then taken by the next body's first kernel)
-        const int in_loop = std::max(fin.it - nprof_all, 0);
-        pf::g_launch_count += 3ll * LOOP_BODY * (in_loop / LOOP_BODY + 1);
-        *prev_len = fin.it;
+        // kernels the loop ran: whole bodies of 3 per iteration, up to loop_end; if the solve ended before that, the
+        // body in which its last iteration ran is the last one unless that iteration was the body's last (its k3's
+        // step is then taken by the next body's first kernel)
+        const int bodies = fin.it >= loop_end ? (loop_end - nprof_all) / LOOP_BODY
+                                              : std::max(fin.it - nprof_all, 0) / LOOP_BODY + 1;
+        pf::g_launch_count += 3ll * LOOP_BODY * bodies;
         done = true;
     }
     while (!done) {
@@ -532,6 +540,7 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
         }
         slot ^= 1;
     }
+    *prev_len = fin.it;
     if (tiled && fin.fault) {
         // operands outside the range of the tiled kernels' branch-free division (pf_common.cuh dvd_nb): x has
         // not been touched yet (D3), so the solve is simply repeated with the kernels that use __ddiv_rn
@@ -665,7 +674,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->opt_profile = 0; g->prof_ms[0] = g->prof_ms[1] = g->prof_ms[2] = 0.0;
     g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
-    g->capture_stream = nullptr; g->opt_graph = 2; g->opt_norm = 0;
+    g->capture_stream = nullptr; g->opt_graph = 3; g->opt_norm = 0;
     g->opt_charge_model = 0; g->charge_model = 0; g->phiL = g->phistar = g->A0_L = nullptr; g->code_L = nullptr;
     g->ctab_L = nullptr; g->laplace_iters = 0; g->fixv = nullptr; g->bc.fixv = nullptr;
     g->small = nullptr;
@@ -803,7 +812,7 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
                 return fail(g, PF_ERR_ARG, "set the charge model before pf_grid_set_workspace");
             g->opt_charge_model = iv; return PF_OK;
         case PF_OPT_GRAPH:
-            if (iv < 0 || iv > 2) return fail(g, PF_ERR_ARG, "graph must be 0, 1 or 2");
+            if (iv < 0 || iv > 3) return fail(g, PF_ERR_ARG, "graph must be 0, 1, 2 or 3");
             g->opt_graph = iv; return PF_OK;
         case PF_OPT_KERNELS:
             if (iv < 0 || iv > 3) return fail(g, PF_ERR_ARG, "kernels must be 0, 1, 2 or 3");

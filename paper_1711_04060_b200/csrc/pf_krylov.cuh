@@ -99,6 +99,10 @@ __device__ __forceinline__ void finish_k3(Scalars* sc, double* hist, double rho_
 // arithmetic on the same data; block 0 stores the new state to sc_out.  Returns false when the solve is over
 // (the block returns at once).  All threads of the block must call; S and scratch are shared memory
 // (scratch: 3*32 dd).  hist: residual history or null.
+// LOOP: the kernel is the one of a loop body that keeps the condition of the body's WHILE node up to date
+// (pf_api.cu loop_graph; only k3 is compiled that way -- Nsight Compute does not profile kernel nodes that can set
+// conditional handles, in graphs of any kind, so every other kernel stays free of the call).
+template <bool LOOP = false>
 __device__ __forceinline__ bool begin_kernel(int kind, Scalars* S, const Scalars* sc_in, Scalars* sc_out,
                                              const ReduceBuf& rb, double* hist, dd* scratch) {
     constexpr int NWORDS = (int)(sizeof(Scalars) / sizeof(int));
@@ -128,8 +132,14 @@ __device__ __forceinline__ bool begin_kernel(int kind, Scalars* S, const Scalars
         S->pending_nblk = (int)linear_grid_size();
         if (kind == PEND_NONE) S->fault = *rb.fault;             // finalize: what the host is about to read
         if (lead) *sc_out = *S;
-        // body of a device-side loop: the last kernel of the body that knows decides whether there is another turn
-        if (lead && rb.more && kind != PEND_NONE) cudaGraphSetConditional((cudaGraphConditionalHandle)rb.more, S->done ? 0u : 1u);
+        // body of a device-side loop: is there another turn?  Not when the solve is over (known with a lag of one
+        // iteration: the k1 of iteration i + 1 takes the step that ends iteration i), nor when this k3 closes the
+        // last iteration the loop is meant to run (the whole bodies that fit below maxit), whatever its sums turn
+        // out to be.
+        if (LOOP && lead && rb.more) {
+            const bool last = S->it + 1 >= S->loop_end;
+            cudaGraphSetConditional((cudaGraphConditionalHandle)rb.more, (S->done || last) ? 0u : 1u);
+        }
     }
     __syncthreads();
     return S->pending != PEND_NONE;

@@ -180,14 +180,14 @@ __device__ __forceinline__ void k3_point(const K3Elem& e, double alpha, double o
     rmax = fmax(rmax, fabs(r_new));          // ||r||_inf of Table 3 step 18
 }
 
-template <bool VEC>
+template <bool VEC, bool LOOP>
 __global__ void __launch_bounds__(256, 3)
 k3_update(long long n, KrylovVecs kv, const Scalars* sc_in, Scalars* sc_out, ReduceBuf rb) {
     __shared__ dd scratch[3 * 32];
     __shared__ Scalars S;
     pdl_launch_dependents();
     pdl_wait();
-    if (!begin_kernel(PEND_K3, &S, sc_in, sc_out, rb, kv.hist, scratch)) return;
+    if (!begin_kernel<LOOP>(PEND_K3, &S, sc_in, sc_out, rb, kv.hist, scratch)) return;
     const double alpha = S.alpha, omega = S.omega;
     dd qa[2] = {dd_zero(), dd_zero()}, qb[2] = {dd_zero(), dd_zero()};
     double rmax = 0.0;
@@ -334,8 +334,10 @@ void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, boo
     const bool vec = (((uintptr_t)kv.y | (uintptr_t)kv.r | (uintptr_t)kv.v_out | (uintptr_t)kv.p_out | (uintptr_t)kv.t |
                        (uintptr_t)kv.rt) & 15u) == 0;
     ++g_launch_count;
-    if (vec) launch_pdl(c.pdl, k3_update<true>, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, sc_in, sc_out, c.rb);
-    else     launch_pdl(c.pdl, k3_update<false>, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, sc_in, sc_out, c.rb);
+    // inside the body of a device-side loop (c.rb.more) the instance that sets the loop condition
+    auto kern = c.rb.more ? (vec ? k3_update<true, true> : k3_update<false, true>)
+                          : (vec ? k3_update<true, false> : k3_update<false, false>);
+    launch_pdl(c.pdl, kern, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, sc_in, sc_out, c.rb);
 }
 
 void launch_finalize(const LaunchCtx& c, double* hist) {

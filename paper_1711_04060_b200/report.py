@@ -1,6 +1,7 @@
 """Report table of BASELINE.md section 4: one row per config x stencil variant, GPU next to the CPU oracle.
 
     python -m paper_1711_04060_b200.report [--out gpurun_out/report.md] [--skip-512]
+    python -m paper_1711_04060_b200.report --launch-ab [--out gpurun_out/launch_ab.md]     (PF_OPT_GRAPH 0 / 1 / 2 / 3)
 
 Needs a CUDA device (the GPU columns) and builds the oracle for the CPU columns; the oracle is only ever
 run where it finishes in about a minute (full solves up to 64^3, a few iterations beyond).
@@ -115,14 +116,69 @@ def pf_row(name, w, oracle, oracle_full: bool):
                 pft=f"{tg:.2f} s / {to:.0f} s" if to else f"{tg:.2f} s / n/a")
 
 
+def launch_mode_ab(out_path):
+    """PF_OPT_GRAPH 0 / 1 / 2 / 3 (stream launches and graph replays polled by the host, device-side loop, auto) side by side:
+    whole-solve CUDA-event times of linear solves of configs 2 and 3 and wall time of config 2's PF solve, each the
+    best of three, modes interleaved; checks that the three modes return the same bits."""
+    lines = ["| workload | iterations | mode 0 (stream, polled) | mode 1 (graph chunks, polled) | mode 2 (device loop) | mode 3 (auto, default) | same bits |",
+             "|---|---:|---:|---:|---:|---:|---|"]
+    for name, w in (("config 2, 128^3", wl.config2()), ("config 2 at 192^3", wl.config2(n=192)),
+                    ("config 3, 256^3", wl.config3())):
+        rhs = torch.from_numpy(np.random.default_rng(3).standard_normal(w.n)).cuda()
+        for tol, maxit in ((0.0, 200), (1e-10, 10000)):
+            best, xs, its = {}, {}, {}
+            for rep in range(3):
+                for mode in (0, 1, 2, 3):
+                    g = pf.Grid.from_workload(w, options={pf.PF_OPT_GRAPH: mode})
+                    x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+                    for _ in range(2):
+                        x.zero_()
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        torch.cuda.synchronize()
+                        e0.record()
+                        out = pf.pf_solve_linear(g.handle, w.n, rhs, x, tol, maxit, true_residual=False)
+                        e1.record()
+                        torch.cuda.synchronize()
+                    best[mode] = min(best.get(mode, 1e30), e0.elapsed_time(e1))
+                    xs[mode], its[mode] = x.clone(), out["iters"]
+                    g.close()
+            same = all(torch.equal(xs[0], xs[m]) and its[0] == its[m] for m in (1, 2, 3))
+            lines.append(f"| {name}, linear, tol {tol:g} | {its[2]} | {best[0]:.2f} ms | {best[1]:.2f} ms | {best[2]:.2f} ms | {best[3]:.2f} ms | {same} |")
+    w = wl.config2()
+    sp = w.species
+    best, phis, its = {}, {}, {}
+    for rep in range(2):
+        for mode in (0, 1, 2, 3):
+            g = pf.Grid.from_workload(w, options={pf.PF_OPT_GRAPH: mode})
+            g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol, want_conc=False)   # warm-up
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            out = g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol, want_conc=False)
+            torch.cuda.synchronize()
+            best[mode] = min(best.get(mode, 1e30), time.perf_counter() - t0)
+            phis[mode], its[mode] = out["phi"].clone(), (out["outer_iters"], out["linear_iters"])
+            g.close()
+    same = all(torch.equal(phis[0], phis[m]) and its[0] == its[m] for m in (1, 2, 3))
+    lines.append(f"| config 2, 128^3, PF solve | {its[2][0]} outer, {its[2][1]} linear | {best[0]:.3f} s | {best[1]:.3f} s | {best[2]:.3f} s | {best[3]:.3f} s | {same} |")
+    text = "\n".join(lines) + "\n"
+    os.makedirs(os.path.dirname(out_path), exist_ok=True)
+    with open(out_path, "w") as f:
+        f.write(text)
+    print(text)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "report.md"))
     ap.add_argument("--skip-512", action="store_true")
+    ap.add_argument("--launch-ab", action="store_true", help="only the A/B table of the launch modes (PF_OPT_GRAPH)")
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise RuntimeError("report needs a CUDA device")
     pf.load()
+    if args.launch_ab:
+        launch_mode_ab(args.out)
+        return
     from oracle import pf_oracle as oracle
     oracle.build()
     peak = measured_peak()

@@ -504,8 +504,9 @@ def test_linear_unaligned_views(pf):
 
 @pytest.mark.parametrize("kernels", [1, 2])
 def test_device_loop_equals_polled_launches(pf, kernels):
-    """PF_OPT_GRAPH 0 (stream launches, host polls), 1 (graph replays of polling chunks) and 2 (one graph whose WHILE
-    node repeats the iterations on the device until the solve is over) run the same kernels on the same state: same
+    """PF_OPT_GRAPH 0 (stream launches, host polls), 1 (graph replays of polling chunks), 2 (one graph whose WHILE
+    node repeats the iterations on the device until the solve is over) and 3 (2 or 1 by the expected length of the
+    solve) run the same kernels on the same state: same
     iterate, residual history, iteration count and status -- for solves that end inside a loop body, at its last
     iteration, at maxit (odd and even, below and above one body), before the first iteration, and with the first
     iterations bracketed by profiling events."""
@@ -513,7 +514,7 @@ def test_device_loop_equals_polled_launches(pf, kernels):
     cases = [dict(tol=1e-10, maxit=10000), dict(tol=0.0, maxit=1), dict(tol=0.0, maxit=7), dict(tol=0.0, maxit=8),
              dict(tol=0.0, maxit=16), dict(tol=0.0, maxit=21), dict(tol=1e-3, maxit=10000), dict(tol=1e30, maxit=10)]
     res = {}
-    for mode in (0, 1, 2):
+    for mode in (0, 1, 2, 3):
         g = pf.Grid.from_workload(w, kernels=kernels, options={pf.PF_OPT_GRAPH: mode, pf.PF_OPT_HISTORY: 512})
         res[mode] = []
         for c in cases:
@@ -526,7 +527,7 @@ def test_device_loop_equals_polled_launches(pf, kernels):
     assert res[0][0][3] == 0 and res[0][0][2] > 16       # the converged case runs over several bodies
     # every iteration count 9..24 ends somewhere else in a body of 8 and in a polling chunk of 16
     for k, ref in enumerate(res[0]):
-        for mode in (1, 2):
+        for mode in (1, 2, 3):
             got = res[mode][k]
             assert torch.equal(got[0], ref[0]), (mode, k)
             assert np.array_equal(got[1], ref[1]) and got[2:] == ref[2:], (mode, k)
@@ -545,9 +546,10 @@ def test_device_loop_every_exit_position(pf):
         b = g2.solve_linear(w.rhs, tol=0.0, maxit=maxit, true_residual=False)
         launched = pf.pf_launch_count() - n0
         assert a["iters"] == b["iters"] == maxit and torch.equal(a["x"], b["x"]), maxit
-        # whole bodies of 8 iterations (one more when the last iteration closes a body) + the solve's fixed launches
-        # (Dirichlet values into b and x, residual kernel, finalize, x = x0 + M^-1 y)
-        fixed.add(launched - 24 * (maxit // 8 + 1))
+        # the whole bodies of 8 iterations below maxit in the loop, the rest as stream launches: nothing runs
+        # beyond iteration maxit; + the solve's fixed launches (Dirichlet values into b and x, residual kernel,
+        # finalize, x = x0 + M^-1 y)
+        fixed.add(launched - 3 * maxit)
     assert len(fixed) == 1 and 3 <= fixed.pop() <= 8
     hist = g1.history(64)
     hist = hist[np.isfinite(hist)]
