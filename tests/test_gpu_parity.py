@@ -561,3 +561,21 @@ def test_device_loop_every_exit_position(pf):
         b = g2.solve_linear(w.rhs, tol=tol)
         assert a["iters"] == b["iters"] and a["status"] == b["status"] == 0 and torch.equal(a["x"], b["x"]), it
     g1.close(); g2.close()
+
+
+def test_device_loop_pf_and_odd_nx(pf):
+    """A whole PF solve (three operators, warm starts, sigma diagonal; tiled kernels, and the widened box of an odd
+    nx) gives the same bits, outer and linear iteration counts whether its inner solves run as polled launches,
+    in the device-side loop or in the mode the library picks by itself; stored coefficients included."""
+    for w, stencil in ((wl.config2(n=40, volt_mv=50.0), 2), (wl.config0(n=33), 2), (wl.config0(n=34), 1)):
+        sp = w.species
+        out = {}
+        for mode in (0, 2, 3):
+            g = pf.Grid.from_workload(w, stencil=stencil, kernels=2, options={pf.PF_OPT_GRAPH: mode})
+            out[mode] = g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, 1e-6)
+            g.close()
+        for mode in (2, 3):
+            assert out[mode]["status"] == out[0]["status"] == 0
+            assert out[mode]["outer_iters"] == out[0]["outer_iters"]
+            assert out[mode]["lin_iters_hist"] == out[0]["lin_iters_hist"], (w.name, mode)
+            assert torch.equal(out[mode]["phi"], out[0]["phi"]) and torch.equal(out[mode]["conc"], out[0]["conc"])
