@@ -107,6 +107,11 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
                                      pf_solve_pf then returns the total phi.  Needs 3 more workspace vectors; must be
                                      set before pf_grid_set_workspace; all charges are assumed to lie in Omega_m. */
 
+#define PF_OPT_DIAG_FROM_CODE 15  /* 1: in Poisson solves without sigma (pf_solve_linear, the initial guess of
+                                     pf_solve_pf) with 2-byte stencil codes, the tiled kernel of row L4 forms the
+                                     diagonal A0 = sum of the six face coefficients from the code instead of reading
+                                     it (8 bytes per unknown less; same bits).  0: A0 is read. */
+
 /* Create a grid: store geometry and boundary conditions, scan eps_map for its palette of distinct
  * values, keep a device copy of the charges.  Assembly itself runs in pf_grid_set_workspace.
  *   eps_map : device, nx*ny*nz doubles, relative permittivity per node; borrowed.

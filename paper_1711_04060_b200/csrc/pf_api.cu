@@ -161,6 +161,7 @@ struct pf_grid {
     std::vector<std::pair<const void*, int>> solve_len;     // iterations of the last solve per operator (by its A0)
     cudaStream_t capture_stream;
     int opt_graph;
+    int opt_diag_code;       // k1 forms the Poisson diagonal from the stencil codes (PF_OPT_DIAG_FROM_CODE)
     int opt_norm;            // 0: relative 2-norm (Q3), 1: the paper's absolute maximum norm
     int opt_charge_model;    // 0: trilinear deposition (Q22), 1: singular-charge decomposition (Eqs 5-10)
     int charge_model;        // the model the workspace was laid out and assembled for
@@ -248,6 +249,7 @@ Operator make_op(const pf_grid* g, int which /*0 poisson, 1 pf1, 2 poisson+sigma
         for (int d = 0; d < 6; ++d) op.offd[d] = g->offd_pf1[d];
     } else {
         op.A0 = which == 2 ? g->A0_s : g->A0; op.code = g->code; op.ctab = g->ctab_poisson;
+        op.diag_code = (which == 0 && g->opt_diag_code && !op.stored && !op.code32) ? 1 : 0;
         for (int d = 0; d < 6; ++d) op.offd[d] = g->offd[d];
     }
     return op;
@@ -283,7 +285,7 @@ cudaGraphExec_t chunk_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, 
     if (!g->opt_graph || (chunk & 1)) return nullptr;
     for (const auto& cg : g->graphs)
         if (cg.a0 == op.A0 && cg.code == op.code && cg.b == kv.b && cg.x == kv.x && cg.y == kv.y && cg.hist == kv.hist &&
-            cg.precond == (int)precond && cg.tiled == (int)tiled && cg.chunk == chunk)
+            cg.precond == (int)precond && cg.tiled == ((int)tiled | (op.diag_code ? 2 : 0)) && cg.chunk == chunk)
             return cg.exec;
     if (!g->capture_stream &&
         cudaStreamCreateWithFlags(&g->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
@@ -308,7 +310,7 @@ cudaGraphExec_t chunk_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, 
         cudaGraphExecDestroy(g->graphs.front().exec);
         g->graphs.erase(g->graphs.begin());
     }
-    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled, chunk, exec});
+    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled | (op.diag_code ? 2 : 0), chunk, exec});
     return exec;
 }
 
@@ -323,7 +325,7 @@ cudaGraphExec_t loop_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, c
     if (g->opt_graph < 2 || (body & 1) || body < 2) return nullptr;
     for (const auto& cg : g->graphs)
         if (cg.a0 == op.A0 && cg.code == op.code && cg.b == kv.b && cg.x == kv.x && cg.y == kv.y && cg.hist == kv.hist &&
-            cg.precond == (int)precond && cg.tiled == (int)tiled && cg.chunk == -body)
+            cg.precond == (int)precond && cg.tiled == ((int)tiled | (op.diag_code ? 2 : 0)) && cg.chunk == -body)
             return cg.exec;
     if (!g->capture_stream &&
         cudaStreamCreateWithFlags(&g->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
@@ -363,7 +365,7 @@ cudaGraphExec_t loop_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, c
         cudaGraphExecDestroy(g->graphs.front().exec);
         g->graphs.erase(g->graphs.begin());
     }
-    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled, -body, exec});
+    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled | (op.diag_code ? 2 : 0), -body, exec});
     return exec;
 }
 
@@ -674,7 +676,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->opt_profile = 0; g->prof_ms[0] = g->prof_ms[1] = g->prof_ms[2] = 0.0;
     g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
-    g->capture_stream = nullptr; g->opt_graph = 3; g->opt_norm = 0;
+    g->capture_stream = nullptr; g->opt_graph = 3; g->opt_diag_code = 0; g->opt_norm = 0;
     g->opt_charge_model = 0; g->charge_model = 0; g->phiL = g->phistar = g->A0_L = nullptr; g->code_L = nullptr;
     g->ctab_L = nullptr; g->laplace_iters = 0; g->fixv = nullptr; g->bc.fixv = nullptr;
     g->small = nullptr;
@@ -811,6 +813,8 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
             if (g->assembled && iv != g->charge_model)
                 return fail(g, PF_ERR_ARG, "set the charge model before pf_grid_set_workspace");
             g->opt_charge_model = iv; return PF_OK;
+        case PF_OPT_DIAG_FROM_CODE:
+            g->opt_diag_code = iv != 0; return PF_OK;
         case PF_OPT_GRAPH:
             if (iv < 0 || iv > 3) return fail(g, PF_ERR_ARG, "graph must be 0, 1, 2 or 3");
             g->opt_graph = iv; return PF_OK;

@@ -57,15 +57,20 @@ constexpr int OWN_BYTES = TX * TY * 8;                            // 8192
 constexpr int NU = 3;                    // shared buffers of u (planes k, k+1 live, k+2 being written)
 static_assert(TY <= 32, "one halo column node per lane of a halo warp");
 
-enum { MODE_R0 = 0, MODE_R1 = 1, MODE_K1 = 2, MODE_K2 = 3 };
+enum { MODE_R0 = 0, MODE_R1 = 1, MODE_K1 = 2, MODE_K2 = 3, MODE_K1D = 4 };
+// MODE_K1D: k1 for operators whose diagonal is the sum of their face coefficients (Poisson without sigma): A0 is
+// not read but formed from the stencil code, whose box then covers the halo ring too.
+constexpr int CXO = 8;                   // code box with halo: starts CXO nodes left of the tile (the TMA unit wants the
+constexpr int BXC = TX + 2 * CXO;        // box to start on a 16-byte boundary of the row: 8 two-byte entries), rows of 160 bytes
 
 template <int MODE> struct ModeTraits;
 template <> struct ModeTraits<MODE_R0> { static constexpr int NF = 2; static constexpr bool OWN = true;  static constexpr int STAGES = 4; };
 template <> struct ModeTraits<MODE_R1> { static constexpr int NF = 2; static constexpr bool OWN = true;  static constexpr int STAGES = 4; };
 template <> struct ModeTraits<MODE_K1> { static constexpr int NF = 4; static constexpr bool OWN = true;  static constexpr int STAGES = 3; };
+template <> struct ModeTraits<MODE_K1D> { static constexpr int NF = 3; static constexpr bool OWN = true; static constexpr int STAGES = 3; };
 template <> struct ModeTraits<MODE_K2> { static constexpr int NF = 3; static constexpr bool OWN = false; static constexpr int STAGES = 4; };
 
-// Halo fields in stage order.  K1: r, p, v, A0.  K2: r, v, A0.  R0/R1: x, A0.
+// Halo fields in stage order.  K1: r, p, v, A0.  K1D: r, p, v.  K2: r, v, A0.  R0/R1: x, A0.
 // Own-only field (tile without halo): K1: r~;  R0/R1: b.
 struct TmaArgs {
     CUtensorMap f[4];
@@ -76,7 +81,9 @@ struct TmaArgs {
 template <int MODE, bool STORED, bool CODE32>
 struct Layout {
     using T = ModeTraits<MODE>;
-    static constexpr int CODE_BYTES = STORED ? 0 : TX * TY * (CODE32 ? 4 : 2);
+    static constexpr bool DIAG = MODE == MODE_K1D;
+    static constexpr int CODE_TX = DIAG ? BXC * BY * 2 : TX * TY * (CODE32 ? 4 : 2);   // bytes the TMA unit delivers
+    static constexpr int CODE_BYTES = STORED ? 0 : ((CODE_TX + 127) / 128) * 128;
     static constexpr int STAGE_BYTES = T::NF * FIELD_BYTES + (T::OWN ? OWN_BYTES : 0) + CODE_BYTES;
     static constexpr int OWN_OFF = T::NF * FIELD_BYTES;
     static constexpr int CODE_OFF = OWN_OFF + (T::OWN ? OWN_BYTES : 0);
@@ -86,12 +93,15 @@ struct Layout {
     // the first 2048-byte boundary inside a 4 KB region (its address is ORed with the entry offset)
     static constexpr int T3_OFF = CTAB_OFF + PF_CTAB * 8;
     static constexpr int T3_BYTES = (STORED || CODE32) ? 0 : 4096;
-    static constexpr int SCRATCH_OFF = T3_OFF + T3_BYTES;
+    // MODE_K1D: the diagonal as a function of the 12-bit code of a node, 4096 doubles, built by the block at its start
+    static constexpr int DTAB_OFF = T3_OFF + T3_BYTES;
+    static constexpr int DTAB_BYTES = DIAG ? 4096 * 8 : 0;
+    static constexpr int SCRATCH_OFF = DTAB_OFF + DTAB_BYTES;
     static constexpr int BAR_OFF = SCRATCH_OFF + 3 * 32 * (int)sizeof(dd);
     static constexpr int SC_OFF = ((BAR_OFF + 16 * T::STAGES + 8 * NU + 15) / 16) * 16;   // after full[S], empty[S], ready[NU]
     static constexpr int TOTAL = SC_OFF + 256;                       // the block's copy of the scalars
     static_assert(CTAB_OFF % 128 == 0, "ctab_at ORs table offsets into the table address");
-    static constexpr unsigned TX_BYTES = (unsigned)(T::NF * BX * BY * 8 + (T::OWN ? OWN_BYTES : 0) + CODE_BYTES);
+    static constexpr unsigned TX_BYTES = (unsigned)(T::NF * BX * BY * 8 + (T::OWN ? OWN_BYTES : 0) + (STORED ? 0 : CODE_TX));
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -127,7 +137,7 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
 template <int MODE, bool PRECOND>
 __device__ __forceinline__ double u_of(double r, double p, double v, double a, bool first, double c1, double c2,
                                        double& numer, unsigned& fault) {
-    if (MODE == MODE_K1) numer = p_new_at<PRECOND>(first, c1, c2, r, p, v);
+    if (MODE == MODE_K1 || MODE == MODE_K1D) numer = p_new_at<PRECOND>(first, c1, c2, r, p, v);
     else if (MODE == MODE_K2) numer = s_at(c1, r, v);
     else { numer = r; return r; }    // residual modes: the field is x itself (passed in r)
     return PRECOND ? dvd_nb(numer, a, fault) : numer;   // == jacobi<PRECOND>(numer, a) of the direct kernels
@@ -161,6 +171,23 @@ __device__ __forceinline__ void ctab3_at(unsigned t3_addr, unsigned w0, int e, i
     asm("ld.shared.f64 %0, [%1+16];" : "=d"(c[2]) : "r"(off));
 }
 
+// MODE_K1D: the diagonal of a node as a function of its 12-bit code (six 2-bit fields).  The Poisson assembly adds
+// the six face coefficients in the order of the fields, starting from 0.0, and the table holds their negatives, so
+// the negated sum of the table entries has the same bits; rows without a face (code 0) are the identity rows,
+// diagonal 1.  Every block tabulates the 4096 values once at its start (ctab: the 16-entry coefficient table).
+__device__ __forceinline__ double diag_of_code12(const double* ctab, unsigned code) {
+    double sacc = 0.0;
+#pragma unroll
+    for (int d = 0; d < 6; ++d) sacc = add(sacc, ctab[(code >> (2 * d)) & 3u]);
+    return code == 0u ? 1.0 : -sacc;
+}
+__device__ __forceinline__ double dtab_at(unsigned dtab_addr, unsigned w0, int e) {
+    const unsigned off = (e ? (w0 >> 13) & 0x7ff8u : (w0 << 3) & 0x7ff8u) + dtab_addr;
+    double a;
+    asm("ld.shared.f64 %0, [%1];" : "=d"(a) : "r"(off));
+    return a;
+}
+
 // Registers of one plane of a main thread: u at its two nodes, the numerators (p' or s), the diagonal,
 // the own-only operand (r~ or b) and the stencil code word(s).
 struct Slot {
@@ -181,6 +208,9 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     using T = ModeTraits<MODE>;
     constexpr int NS = T::STAGES;
     constexpr int NF = T::NF;
+    constexpr bool DIAG = MODE == MODE_K1D;          // k1 with the diagonal formed from the codes
+    constexpr bool K1 = MODE == MODE_K1 || DIAG;
+    static_assert(!DIAG || (!STORED && !CODE32), "the diagonal is formed from 2-bit codes");
     pdl_launch_dependents();
     extern __shared__ __align__(128) unsigned char smem[];
     double* ctab_s = reinterpret_cast<double*>(smem + L::CTAB_OFF);
@@ -218,8 +248,15 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     }
     const unsigned ctab_addr = smem_u32(ctab_s);           // 128-byte aligned: CTAB_OFF and the smem base are
     __syncthreads();
+    unsigned dtab_addr = 0u;
+    if (DIAG) {
+        double* dtab = reinterpret_cast<double*>(smem + L::DTAB_OFF);
+        dtab_addr = smem_u32(dtab);
+        for (int k = tid; k < 4096; k += blockDim.x) dtab[k] = diag_of_code12(ctab_s, (unsigned)k);
+        __syncthreads();
+    }
     pdl_wait();                                            // everything above is independent of the previous kernel
-    constexpr int KIND = MODE == MODE_K1 ? PEND_K1 : (MODE == MODE_K2 ? PEND_K2 : (MODE == MODE_R0 ? PEND_INIT : PEND_TRUE));
+    constexpr int KIND = K1 ? PEND_K1 : (MODE == MODE_K2 ? PEND_K2 : (MODE == MODE_R0 ? PEND_INIT : PEND_TRUE));
     // plane k of the load sequence of work item `item` into stage (seq % NS); the producer lane only
     auto issue_plane = [&](int item, int k, int seq) {
         const int tile = item % ntiles;
@@ -230,7 +267,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
 #pragma unroll
         for (int f = 0; f < NF; ++f) tma_load_3d(st + f * FIELD_BYTES, &tm.f[f], &full[s], px - 2, py - 1, pz);
         if (T::OWN) tma_load_3d(st + L::OWN_OFF, &tm.own, &full[s], px, py, pz);
-        if (!STORED) tma_load_3d(st + L::CODE_OFF, &tm.code, &full[s], px, py, pz);
+        if (!STORED) tma_load_3d(st + L::CODE_OFF, &tm.code, &full[s], DIAG ? px - CXO : px, DIAG ? py - 1 : py, pz);
     };
     // The first stages do not depend on the scalars: they are requested before the block combines the previous
     // kernel's partial sums, so the loads fly while the scalar step is taken.
@@ -272,7 +309,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
         __syncwarp();
     } else {
         bool first = false; double c1 = 0.0, c2 = 0.0;
-        if (MODE == MODE_K1) { first = S->first != 0; c1 = S->beta; c2 = S->omega; }
+        if (K1) { first = S->first != 0; c1 = S->beta; c2 = S->omega; }
         else if (MODE == MODE_K2) { c1 = S->alpha; }
         const bool is_main = wid < TY;
         // main thread: nodes (x, y) and (x+1, y) of box row wid+1; nx is even so both are inside or both outside.
@@ -284,6 +321,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
         const long long own_off = x + (long long)g.nx * y;
         const int pair_box = brow * BX + 2 + 2 * lane;                 // element offset in a halo box
         const int own_tile = (brow - 1) * TX + 2 * lane;               // element offset in an own-only box (main)
+        const int pair_code = brow * BXC + CXO + 2 * lane;               // MODE_K1D: element offset in the code box with halo
 
         // operands of the thread's pair of nodes in plane z0-1+k -> u, numerator, diagonal
         auto form_pair = [&](const unsigned char* st, bool ok, double (&u)[2], double (&n)[2], double (&a)[2]) {
@@ -293,7 +331,12 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             const double* F3 = reinterpret_cast<const double*>(st + 3 * FIELD_BYTES);
             double2 fr = *reinterpret_cast<const double2*>(F0 + pair_box), fp = make_double2(0, 0),
                     fv = make_double2(0, 0), fa;
-            if (MODE == MODE_K1) {
+            if (DIAG) {
+                fp = *reinterpret_cast<const double2*>(F1 + pair_box);
+                fv = *reinterpret_cast<const double2*>(F2 + pair_box);
+                const unsigned cw = *reinterpret_cast<const unsigned*>(st + L::CODE_OFF + 2 * pair_code);
+                fa = make_double2(dtab_at(dtab_addr, cw, 0), dtab_at(dtab_addr, cw, 1));
+            } else if (MODE == MODE_K1) {
                 fp = *reinterpret_cast<const double2*>(F1 + pair_box);
                 fv = *reinterpret_cast<const double2*>(F2 + pair_box);
                 fa = *reinterpret_cast<const double2*>(F3 + pair_box);
@@ -360,7 +403,13 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     const double* F2 = reinterpret_cast<const double*>(st + 2 * FIELD_BYTES);
                     const double* F3 = reinterpret_cast<const double*>(st + 3 * FIELD_BYTES);
                     double hr = F0[col_box], hp = 0.0, hv = 0.0, ha;
-                    if (MODE == MODE_K1) { hp = F1[col_box]; hv = F2[col_box]; ha = F3[col_box]; }
+                    if (DIAG) {
+                        hp = F1[col_box]; hv = F2[col_box];
+                        const int hxc = (wid == TY ? 1 : BX - 2) + CXO - 2; // the code box starts CXO - 2 columns further left
+                        const unsigned cw = *reinterpret_cast<const unsigned short*>(st + L::CODE_OFF + 2 * ((1 + lane) * BXC + hxc));
+                        ha = dtab_at(dtab_addr, cw, 0);
+                    }
+                    else if (MODE == MODE_K1) { hp = F1[col_box]; hv = F2[col_box]; ha = F3[col_box]; }
                     else if (MODE == MODE_K2) { hv = F1[col_box]; ha = F2[col_box]; }
                     else ha = 1.0;
                     if (!(col_ok && zin)) ha = 1.0;
@@ -387,11 +436,13 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     if (CODE32) {
                         const uint2 cw = *reinterpret_cast<const uint2*>(st + L::CODE_OFF + 4 * own_tile);
                         up.k0 = cw.x; up.k1 = cw.y;
+                    } else if (DIAG) {
+                        up.k0 = *reinterpret_cast<const unsigned*>(st + L::CODE_OFF + 2 * pair_code);
                     } else {
                         up.k0 = *reinterpret_cast<const unsigned*>(st + L::CODE_OFF + 2 * own_tile);
                     }
                 }
-                if (MODE == MODE_K1 && ok && z >= z0 && z < z1)         // p' is an output of steps 5-9
+                if (K1 && ok && z >= z0 && z < z1)                      // p' is an output of steps 5-9
                     *reinterpret_cast<double2*>(kv.p_out + own_off + plane * z) = make_double2(up.n[0], up.n[1]);
                 if (to_shared)
                     *reinterpret_cast<double2*>((u_dst ? u_dst : u_buf(k)) + pair_box) = make_double2(up.u[0], up.u[1]);
@@ -422,7 +473,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 load_slot(k + 1, up, true, U(J1));
                 // inner products of the PREVIOUS plane: a third independent chain beside the divisions of plane
                 // z+1 and the 7-point sums of plane z
-                if (DEFER && MODE == MODE_K1) {
+                if (DEFER && K1) {
                     dd_fma(q[0], pa[0], pb[0]); dd_fma(q[1], pa[1], pb[1]);
                 } else if (DEFER && MODE == MODE_K2) {
                     dd_fma(q[0], pa[0], pb[0]); dd_fma(q[0], pa[1], pb[1]);
@@ -466,7 +517,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 if (lane == 0) { mbar_arrive(R(J1)); mbar_arrive(&empty[(sb + k + 1) % NS]); }
                 out[0] = add(out[0], mul(c5[0], up.u[0]));
                 out[1] = add(out[1], mul(c5[1], up.u[1]));
-                if (MODE == MODE_K1) {
+                if (K1) {
                     if (pair_ok) *reinterpret_cast<double2*>(kv.v_out + i) = make_double2(out[0], out[1]);
                     if (DEFER) { pa[0] = c.w.x; pa[1] = c.w.y; pb[0] = out[0]; pb[1] = out[1]; }   // r~ . v', next step
                     else { dd_fma(q[0], c.w.x, out[0]); dd_fma(q[1], c.w.y, out[1]); }
@@ -505,7 +556,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 step(std::integral_constant<int, 2>{}, z + 2, s2, s0, s1);
                 mp ^= 1u;
             }
-            if (DEFER && MODE == MODE_K1) {                  // the last plane's inner products
+            if (DEFER && K1) {                               // the last plane's inner products
                 dd_fma(q[0], pa[0], pb[0]); dd_fma(q[1], pa[1], pb[1]);
             } else if (DEFER && MODE == MODE_K2) {
                 dd_fma(q[0], pa[0], pb[0]); dd_fma(q[0], pa[1], pb[1]);
@@ -519,7 +570,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
 
     if (fault) *rb.fault = 1;              // the host repeats the solve with the __ddiv_rn kernels
     // this block's partial sums; the next kernel of the stream combines them (pf_common.cuh)
-    if (MODE == MODE_K1) {
+    if (K1) {
         dd_add(q[0], q[1]);                // two chains for instruction-level parallelism, one quantity
         dd q1[1] = {q[0]};
         store_partials<1, false>(q1, 0.0, scratch, rb, PEND_K1);
@@ -636,7 +687,8 @@ void launch_mode(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, c
 // Tensor maps of one solve: every vector a kernel reads through TMA.
 struct TmaSet {
     CUtensorMap r, p[2], v[2], a0, rt, x, b, code;
-    bool have_code;
+    CUtensorMap codeh;       // 2-byte codes with the halo ring (MODE_K1D)
+    bool have_code, have_codeh;
 };
 
 bool tma_available() { return encoder() != nullptr; }
@@ -664,6 +716,8 @@ bool tma_set_build(TmaSet* t, const GridDims& g, const Operator& op, const Krylo
                        : make_map(&t->code, op.code, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, g, op.cpitch, TX, TY);
         t->have_code = ok;
     }
+    t->have_codeh = ok && !op.stored && !op.code32 && op.diag_code &&
+                    make_map(&t->codeh, op.code, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, g, op.cpitch, BXC, BY);
     return ok;
 }
 
@@ -678,6 +732,16 @@ void launch_k1_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv,
                    int parity) {
     TmaArgs a;
     std::memset(&a, 0, sizeof(a));
+    if (t->have_codeh) {     // the diagonal is the sum of the face coefficients: formed from the codes, A0 not read
+        a.f[0] = t->r; a.f[1] = t->p[parity]; a.f[2] = t->v[parity]; a.own = t->rt; a.code = t->codeh;
+        const int tx = (c.g.nx + TX - 1) / TX, tyb = (c.g.ny + TY - 1) / TY;
+        const int chunks = choose_zchunks(c.g, tx * tyb, c.sm_count);
+        const int depth = (c.g.nz + chunks - 1) / chunks;
+        dim3 grid(tx, tyb, (c.g.nz + depth - 1) / depth);
+        if (precond) launch_inst<MODE_K1D, true, false, false>(c, op, kv, a, grid, depth);
+        else         launch_inst<MODE_K1D, false, false, false>(c, op, kv, a, grid, depth);
+        return;
+    }
     a.f[0] = t->r; a.f[1] = t->p[parity]; a.f[2] = t->v[parity]; a.f[3] = t->a0; a.own = t->rt; a.code = t->code;
     launch_mode<MODE_K1>(c, op, kv, a, precond);
 }
