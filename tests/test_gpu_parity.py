@@ -579,3 +579,26 @@ def test_device_loop_pf_and_odd_nx(pf):
             assert out[mode]["outer_iters"] == out[0]["outer_iters"]
             assert out[mode]["lin_iters_hist"] == out[0]["lin_iters_hist"], (w.name, mode)
             assert torch.equal(out[mode]["phi"], out[0]["phi"]) and torch.equal(out[mode]["conc"], out[0]["conc"])
+
+
+@pytest.mark.parametrize("shape", [(32, 16, 8), (34, 17, 9), (130, 33, 21), (96, 48, 64), (65, 17, 9)])
+def test_diagonal_from_codes(pf, shape):
+    """PF_OPT_DIAG_FROM_CODE: the tiled k1 that takes the Poisson diagonal from the table indexed by the node's
+    stencil code (identity rows, Neumann and Dirichlet faces, partial tiles, the widened box of an odd nx) gives the
+    bits of the k1 that reads A0, with and without the Jacobi preconditioner; a solve with a sigma diagonal and the
+    PF operators keep reading A0 and are unchanged."""
+    nx, ny, nz = shape
+    w = ragged_workload(nx=nx, ny=ny, nz=nz, seed=11 + nx, mixed_bc=(nx % 3 != 0))
+    sigma = torch.rand(w.n, dtype=torch.float64, device="cuda")
+    for precond in (1, 0):
+        res = []
+        for diag in (0, 1):
+            g = pf.Grid.from_workload(w, stencil=2, kernels=2, options={pf.PF_OPT_DIAG_FROM_CODE: diag,
+                                                                       pf.PF_OPT_PRECOND: precond, pf.PF_OPT_HISTORY: 64})
+            out = g.solve_linear(w.rhs, tol=0.0, maxit=25)
+            h = g.history(26)
+            outs = g.solve_linear(w.rhs, tol=0.0, maxit=9, sigma=sigma)
+            res.append((out["x"].clone(), h, out["true_relres"], outs["x"].clone()))
+            g.close()
+        assert torch.equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1]), (shape, precond)
+        assert res[0][2] == res[1][2] and torch.equal(res[0][3], res[1][3]), (shape, precond)
