@@ -36,9 +36,12 @@ extern "C" {
 
 #define PF_OK                0
 #define PF_NOT_CONVERGED     1   /* maxit (or max outer iterations) reached; outputs hold the last iterate */
+#define PF_INNER_NOT_CONVERGED 2 /* pf_solve_pf: the increment met the tolerance, but at least one of the linear solves
+                                    stopped at PF_OPT_LINEAR_MAXIT and its last iterate was used as it stood */
 #define PF_ERR_ARG          -1
 #define PF_ERR_CUDA         -2
-#define PF_ERR_BREAKDOWN    -3   /* rho = 0, r~.v = 0 or omega = 0 before convergence (reading Q5) */
+#define PF_ERR_BREAKDOWN    -3   /* rho = 0, r~.v = 0 or omega = 0 before convergence (reading Q5); a reduced scalar or
+                                    the potential increment is not finite (NaN/inf input, divergence; reading D7) */
 #define PF_ERR_NONPHYSICAL  -4   /* bath not neutral or Gamma^B <= 0 (reading Q26) */
 #define PF_ERR_WORKSPACE    -5   /* workspace missing or too small */
 
@@ -136,7 +139,8 @@ size_t pf_grid_workspace_bytes(const pf_grid *g);
 
 /* Hand the grid its scratch (device, 256-byte aligned, >= pf_grid_workspace_bytes) and run the
  * operator assembly (rows L1, L2 of DESIGN.md): node classes, diagonals, optionally the stored
- * off-diagonals, the deposited fixed-charge right-hand side (reading R2). */
+ * off-diagonals, the deposited fixed-charge right-hand side (reading R2).  With charge model 1 the Laplace solve for
+ * phi^L runs here; PF_NOT_CONVERGED is returned (the grid stays usable) when it stopped at PF_OPT_LINEAR_MAXIT. */
 int pf_grid_set_workspace(pf_grid *g, void *dev_ptr, size_t bytes);
 
 int pf_grid_set_option(pf_grid *g, int key, double value);
@@ -169,7 +173,7 @@ int pf_solve_linear_host(pf_grid *g, const double *rhs_host, double *x_host, con
  *   conc   : device (K+1)*N or NULL, out: C_k at the final phi (species-major), 0 outside the solvent.
  *   steric : device N or NULL, out: S^trc at the final phi.
  *   outer_iters_out, linear_iters_out (sum over all linear solves): host, may be NULL.
- * Returns PF_OK, PF_NOT_CONVERGED, or an error. */
+ * Returns PF_OK, PF_NOT_CONVERGED (outer cap reached), PF_INNER_NOT_CONVERGED, or an error. */
 int pf_solve_pf(pf_grid *g, int nions, const double *valence, const double *bath_conc,
                 const double *radii, double l_c, double tol,
                 double *phi, double *conc, double *steric,
@@ -191,50 +195,6 @@ int pf_grid_linear_iters(pf_grid *g, int *iters_host, int cap);
 /* ||Phi - Phi0||_inf (after relaxation, Table 2 step 5) of every outer iteration of the last pf_solve_pf.
  * Returns the number of entries written (<= cap). */
 int pf_grid_increments(pf_grid *g, double *incr_host, int cap);
-
-/* Accumulated device time (ms) and launch count of the three per-iteration kernels since
- * PF_OPT_PROFILE was set: index 0 = p-update + matvec + r~.v (row L4), 1 = s-update + matvec + t.s,
- * t.t (row L5), 2 = x, r update + r~.r, r.r (row L6).  ms_out, launches_out: host, 3 entries. */
-int pf_grid_profile(pf_grid *g, double *ms_out, long long *launches_out);
-
-/* Kernel launches issued by the library in this process so far. */
-long long pf_launch_count(void);
-
-/* BiCGSTAB iterations of the Laplace solve for phi^L (charge model 1). */
-int pf_grid_laplace_iters(const pf_grid *g);
-
-/* Number of linear solves of this grid that were repeated by the direct kernels because the tiled kernels met
- * operands outside the range of their branch-free division (reading D4 of DESIGN.md). */
-int pf_grid_fault_repeats(const pf_grid *g);
-
-/* Decomposition the cooperative kernel (PF_OPT_KERNELS = 3; pf_krylov_coop.cu) would use for an nx x ny x nz box
- * on a device with max_blocks SMs and smem_cap bytes of dynamic shared memory per block: one brick per block,
- * brick k of nb along an axis of n nodes = nodes floor(k n/nb) .. floor((k+1) n/nb) - 1.  Host arithmetic only
- * (no device is touched).  out (host, 8 ints): bricks per direction nbx, nby, nbz; array extents of the largest
- * brick: own nodes (rounded up to even), nodes with one halo layer, halo nodes; threads per block; bytes of
- * dynamic shared memory.  Returns PF_OK, or PF_ERR_ARG when no decomposition fits (the solver then uses the
- * three-kernel families) or an argument is invalid. */
-int pf_coop_plan(int nx, int ny, int nz, int max_blocks, size_t smem_cap, int *out);
-
-/* Introspection used by the tests: 1 = stored, 2 = on-the-fly; number of palette entries. */
-int pf_grid_stencil(const pf_grid *g);
-int pf_grid_palette_size(const pf_grid *g);
-
-/* Layout of the stencil codes of the on-the-fly variant: bits per code (16: six 2-bit fields, 32: six
- * 4-bit fields, 0: none -- more than 4 distinct eps values), row pitch in codes (nx rounded up to 8;
- * code of node (ix,iy,iz) at ix + pitch*(iy + ny*iz)), bytes of one code array.  Field d-1 (d = 1..6 in
- * the order east, west, south, north, down, up of PAPER.md:219) indexes the coefficient table; index 0
- * is the coefficient 0.  Out-pointers: host, may be NULL. */
-int pf_grid_code_layout(const pf_grid *g, int *bits_out, int *pitch_out, size_t *bytes_out);
-
-/* Copy an assembled array into caller memory (device), for the assembly parity tests (rows L1/L2):
- * which = 0: Poisson diagonal A0 (N doubles); 1..6: stored off-diagonals A1..A6 (stored variant
- * only); 7: deposited fixed-charge vector (N doubles); 8: Poisson stencil codes (pf_grid_code_layout
- * bytes); 9: PF1 diagonal (N doubles, after a pf_solve_pf); 10: Poisson coefficient table (16 doubles);
- * 11: PF1 stencil codes; 12: PF1 coefficient table; 13: Psi of the last pf_solve_pf (N doubles);
- * 14: phi^L, 15: phi* on Omega_m (N doubles each, charge model 1; with it, 7 is b^IF).
- * Returns PF_ERR_ARG if unavailable. */
-int pf_grid_copy_array(pf_grid *g, int which, void *dst_device);
 
 void pf_grid_destroy(pf_grid *g);
 const char *pf_last_error(const pf_grid *g);   /* g may be NULL: last error of pf_grid_create */

@@ -186,9 +186,14 @@ double dot(int64_t N, const double* a, const double* b) {
 double norm2(int64_t N, const double* a) { return std::sqrt(dot(N, a, a)); }
 
 // K4: maximum norm (Table 3 step 18).
+// A NaN entry makes the norm NaN (std::max would drop it: every comparison with a NaN is false).
 double norm_inf(int64_t N, const double* a) {
     double m = 0.0;
-    for (int64_t i = 0; i < N; ++i) m = std::max(m, std::fabs(a[i]));
+    for (int64_t i = 0; i < N; ++i) {
+        double v = std::fabs(a[i]);
+        if (std::isnan(v) || v > m) m = v;
+        if (std::isnan(m)) break;
+    }
     return m;
 }
 
@@ -210,6 +215,8 @@ void set_dirichlet(const Grid& g, double* x) {
 // is Table 3 verbatim.  Stopping on the recurrence residual: norm_mode 0 (Q3, BASELINE): ||r||_2 <= tol*||b||_2;
 // norm_mode 1 (the paper's own test, Table 3 steps 18-19): ||r||_inf < tol, absolute.
 // In mode 1 relres_out, true_relres_out and hist carry the absolute maximum norms.
+// Reading D7: a scalar that is not finite (||b||, ||r||, rho, r~.v, t.s, t.t) is a breakdown (-3);
+// Table 3 is silent, and a NaN would otherwise fail "== 0" and never pass the convergence test.
 int bicgstab(const Grid& g, const double* A, const double* b, double* x, double tol, int maxit,
              int precond, int* iters_out, double* relres_out, double* true_relres_out,
              double* hist /* maxit+1 or null */, int norm_mode = 0) {
@@ -234,13 +241,14 @@ int bicgstab(const Grid& g, const double* A, const double* b, double* x, double 
     if (hist) hist[0] = rnorm / scale;
     int status = 1;
     double rho_old = 1.0, alpha = 1.0, omega = 1.0;
-    if (converged(rnorm)) status = 0;       // warm start already converged (DESIGN reading D1)
+    if (!std::isfinite(bnorm) || !std::isfinite(rnorm)) status = -3;                  // D7
+    else if (converged(rnorm)) status = 0;  // warm start already converged (DESIGN reading D1)
     int it = 0;
     while (status == 1 && it < maxit) {
         ++it;
         // step 4
         double rho = dot(N, rt.data(), r.data());
-        if (rho == 0.0) { status = -3; --it; break; }
+        if (rho == 0.0 || !std::isfinite(rho)) { status = -3; --it; break; }
         // steps 5-10
         if (it == 1) {
             p = r;
@@ -253,7 +261,7 @@ int bicgstab(const Grid& g, const double* A, const double* b, double* x, double 
         dia_spmv(g, A, ph.data(), v.data());
         // step 12
         double rtv = dot(N, rt.data(), v.data());
-        if (rtv == 0.0) { status = -3; --it; break; }
+        if (rtv == 0.0 || !std::isfinite(rtv)) { status = -3; --it; break; }
         alpha = rho / rtv;
         // step 13
         for (int64_t i = 0; i < N; ++i) s[i] = r[i] - alpha * v[i];
@@ -264,6 +272,7 @@ int bicgstab(const Grid& g, const double* A, const double* b, double* x, double 
         double ts = dot(N, t.data(), s.data());
         double tt = dot(N, t.data(), t.data());
         omega = (tt == 0.0) ? 0.0 : ts / tt;   // Q5
+        if (!std::isfinite(ts) || !std::isfinite(tt)) { status = -3; --it; break; }   // D7
         // step 16
         for (int64_t i = 0; i < N; ++i) x[i] = x[i] + alpha * ph[i] + omega * sh[i];
         // step 17
@@ -272,6 +281,7 @@ int bicgstab(const Grid& g, const double* A, const double* b, double* x, double 
         rnorm = measure(r.data());
         if (hist) hist[it] = rnorm / scale;
         rho_old = rho;
+        if (!std::isfinite(rnorm)) { status = -3; break; }                            // D7
         if (converged(rnorm)) { status = 0; break; }
         if (omega == 0.0) { status = -3; break; }
     }
@@ -650,7 +660,8 @@ int pfo_fermi_pointwise(int K, const double* valence, const double* bath_molar, 
 }
 
 // ---- R5: the outer loop, Table 2 steps 2-5 / Table 4 steps 4-7 ----
-// Returns 0 converged, 1 max_outer reached, <0 error.  lin_iters_hist (may be null) receives the
+// Returns 0 converged, 1 max_outer reached, 2 converged on the increment although at least one linear solve stopped
+// at lin_maxit, <0 error (-3: breakdown of a linear solve or a non-finite increment, D7).  lin_iters_hist (may be null) receives the
 // BiCGSTAB iteration count of every linear solve in call order (initial guess, then PF1, PF2, ...),
 // up to hist_cap entries; incr_hist the increment ||phi - phi0||_inf of every outer iteration.
 int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double* bcv,
@@ -679,6 +690,7 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
     else deposit_charges(g, charges, M, fixed.data());
     int nsolve = 0, total = 0, its = 0;
     double rr, tr;
+    bool inner_maxit = false;     // a linear solve stopped at lin_maxit (status 1): its last iterate is used as it stands
     auto record = [&](int n) { if (lin_iters_hist && nsolve < hist_cap) lin_iters_hist[nsolve] = n; ++nsolve; total += n; };
     // step 2 / 4: initial guess, PF2 with rho' = Psi = 0
     assemble_poisson(g, eps, nullptr, A0.data());
@@ -687,6 +699,7 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
     rc = bicgstab(g, A0.data(), b.data(), phi0.data(), lin_tol, lin_maxit, 1, &its, &rr, &tr, nullptr, norm_mode);
     record(its);
     if (rc < 0) return rc;
+    inner_maxit |= rc == 1;
     assemble_pf1(g, eps, solv.data(), lc, A1.data());
     int status = 1, outer = 0;
     while (outer < max_outer) {
@@ -697,6 +710,7 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
         rc = bicgstab(g, A1.data(), b.data(), Psi.data(), lin_tol, lin_maxit, 1, &its, &rr, &tr, nullptr, norm_mode);
         record(its);
         if (rc < 0) return rc;
+        inner_maxit |= rc == 1;
         // step 4 / 6: PF2 -> phi (warm start: phi0)
         assemble_poisson(g, eps, sigma.data(), A2.data());
         rhs_pf2(g, eps, solv.data(), Psi.data(), sigma.data(), phi0.data(), fixed.data(), b.data());
@@ -704,13 +718,13 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
         rc = bicgstab(g, A2.data(), b.data(), ph.data(), lin_tol, lin_maxit, 1, &its, &rr, &tr, nullptr, norm_mode);
         record(its);
         if (rc < 0) return rc;
+        inner_maxit |= rc == 1;
         // step 5 / 7: relax, then test the increment (Q8, Q9)
-        double d = 0.0;
-        for (int64_t i = 0; i < N; ++i) {
-            ph[i] = omega_pf * phi0[i] + (1.0 - omega_pf) * ph[i];
-            d = std::max(d, std::fabs(ph[i] - phi0[i]));
-        }
+        for (int64_t i = 0; i < N; ++i) ph[i] = omega_pf * phi0[i] + (1.0 - omega_pf) * ph[i];
+        for (int64_t i = 0; i < N; ++i) b[i] = ph[i] - phi0[i];
+        double d = norm_inf(N, b.data());
         if (incr_hist) incr_hist[outer - 1] = d;
+        if (!std::isfinite(d)) return -3;                  // D7: a NaN fails "d > tol" and would read as converged
         phi0 = ph;
         if (!(d > tol)) { status = 0; break; }
     }
@@ -719,6 +733,7 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
     if (conc || steric) fermi_field(sp, N, phi0.data(), solv.data(), nullptr, nullptr, steric, conc);
     *outer_iters = outer;
     *linear_iters = total;
+    if (status == 0 && inner_maxit) return 2;    // converged on the increment, but an inner solve was cut off
     return status;
 }
 

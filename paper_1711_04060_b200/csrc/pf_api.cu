@@ -1,7 +1,8 @@
-// pf_api.cu -- the C ABI of include/pf.h and the host-side solver driver: launch sequencing of the
+// pf_api.cu -- the C ABI of include/pf.h (+ the introspection calls of include/pf_debug.h) and the host-side solver driver: launch sequencing of the
 // three-kernel BiCGSTAB iteration, device-resident scalars, pipelined polling of the device-side
 // convergence flag (row L8), and the PF outer loop (rows N1-N5).
 #include "../../include/pf.h"
+#include "../../include/pf_debug.h"
 #include "pf_launch.h"
 
 #include <cmath>
@@ -15,6 +16,7 @@
 using namespace pf;
 
 long long pf::g_launch_count = 0;
+thread_local cudaError_t pf::g_launch_error = cudaSuccess;
 
 namespace {
 
@@ -103,7 +105,7 @@ struct pf_grid {
     double h;
     BcDev bc;
     cudaStream_t stream;
-    int sm_count;
+    int sm_count, device;
     const double* eps;
     Palette pal;
     double eps_min, eps_max, eps_mid;
@@ -174,6 +176,7 @@ struct pf_grid {
     std::vector<double> fix_val;
     double* fixv;
     int fault_repeats;       // solves repeated by the direct kernels after a division range fault (D4)
+    std::vector<const void*> fault_ops;   // operators (by their A0) whose tiled solve faulted: they go straight to the direct family
     std::string err;
 };
 
@@ -258,7 +261,7 @@ Operator make_op(const pf_grid* g, int which /*0 poisson, 1 pf1, 2 poisson+sigma
 LaunchCtx make_ctx(const pf_grid* g) {
     LaunchCtx c;
     c.stream = g->stream; c.g = g->g; c.sc[0] = g->sc[0]; c.sc[1] = g->sc[1]; c.flip = const_cast<int*>(&g->flip);
-    c.rb = g->rb; c.sm_count = g->sm_count; c.pdl = true;
+    c.rb = g->rb; c.sm_count = g->sm_count; c.device = g->device; c.pdl = true;
     return c;
 }
 
@@ -402,6 +405,9 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
     if (!(tol >= 0.0)) return fail(g, PF_ERR_ARG, "tol must be >= 0");
     LaunchCtx c = make_ctx(g);
     c.g = dims;
+    pf::g_launch_error = cudaSuccess;
+    bool op_faulted = false;      // an earlier tiled solve with this operator left dvd_nb's range (D4)
+    for (const void* f : g->fault_ops) op_faulted |= f == op.A0;
     const bool precond = g->opt_precond != 0;
     Scalars init;
     std::memset(&init, 0, sizeof(init));
@@ -434,12 +440,12 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
     // D3: with the Jacobi preconditioner step 16 accumulates y = sum(alpha p + omega s); x = x0 + M^-1 y at the end
     kv.y = precond ? g->y : x;
     if (precond) PF_CUDA(g, cudaMemsetAsync(g->y, 0, sizeof(double) * dims.n, g->stream));
-    bool tiled = allow_tiled && use_tiled(g, dims) && tma_pointers_ok(kv, op);
+    bool tiled = allow_tiled && !op_faulted && use_tiled(g, dims) && tma_pointers_ok(kv, op);
     if (tiled && !tma_set_build(g->tma, dims, op, kv)) {
         if (g->opt_kernels == 2) return fail(g, PF_ERR_CUDA, "tensor-map encoding failed");
         tiled = false;
     }
-    if (g->opt_kernels == 2 && allow_tiled && !tiled)
+    if (g->opt_kernels == 2 && allow_tiled && !op_faulted && !tiled)
         return fail(g, PF_ERR_ARG, "the tiled kernels need 16-byte aligned vectors");
     // Small grids: the whole solve in one cooperative kernel (pf_krylov_coop.cu)
     CoopPlan plan;
@@ -543,11 +549,18 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
         slot ^= 1;
     }
     *prev_len = fin.it;
+    if (pf::g_launch_error != cudaSuccess) {
+        const cudaError_t le = pf::g_launch_error;
+        pf::g_launch_error = cudaSuccess;
+        cudaGetLastError();
+        return fail(g, PF_ERR_CUDA, "kernel launch: %s", cudaGetErrorString(le));
+    }
     if (tiled && fin.fault) {
         // operands outside the range of the tiled kernels' branch-free division (pf_common.cuh dvd_nb): x has
         // not been touched yet (D3), so the solve is simply repeated with the kernels that use __ddiv_rn
         PF_CUDA(g, cudaStreamSynchronize(g->stream));
         ++g->fault_repeats;
+        if (g->fault_ops.size() < 16) g->fault_ops.push_back(op.A0);    // later solves with it skip the tiled family
         return bicgstab_core(g, dims, op, b, x, tol, maxit, iters_out, relres_out, true_relres_out, false, false);
     }
     if (precond) launch_finish_x(c, op, kv);
@@ -694,6 +707,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
         }                                                                                            \
     } while (0)
     PF_CREATE_CUDA(cudaGetDevice(&dev));
+    g->device = dev;
     PF_CREATE_CUDA(cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev));
     PF_CREATE_CUDA(small_set_acquire(dev, (size_t)ncharges, &g->small));
     g->sc[0] = reinterpret_cast<Scalars*>(g->small->dev + SS_SC);
@@ -836,6 +850,15 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     if (bytes < need) return fail(g, PF_ERR_WORKSPACE, "workspace has %zu bytes, %zu needed", bytes, need);
     g->stored = want_stored(g);
     g->ws = dev_ptr; g->ws_bytes = bytes;
+    bool laplace_maxit = false;
+    // everything that was derived from an earlier workspace: cached graphs (they bake in the vector, scalar and
+    // partial-sum pointers and the tensor maps), expected solve lengths, the cooperative plan, faulted operators
+    cudaStreamSynchronize(g->stream);
+    for (auto& cg : g->graphs) cudaGraphExecDestroy(cg.exec);
+    g->graphs.clear();
+    g->solve_len.clear();
+    g->fault_ops.clear();
+    g->coop_state = 0;
     const size_t vec = align_up(sizeof(double) * (size_t)g->gk.n, 256);     // every vector has room for the widened box
     char* base = (char*)dev_ptr;
     auto take = [&]() { double* p = (double*)base; base += vec; return p; };
@@ -890,6 +913,7 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
         int rc = bicgstab_device(g, make_op(g, 3), g->bpf, g->phiL, g->opt_lin_tol, g->opt_lin_maxit, &g->laplace_iters,
                                  nullptr, nullptr);
         if (rc < 0) { g->assembled = false; return rc; }
+        laplace_maxit = rc == PF_NOT_CONVERGED;
         launch_phistar(g->stream, g->g, g->h, g->eps, g->eps_mid, g->eps_min, kap, g->charges_dev, g->ncharges, g->phistar);
         launch_interface_rhs(g->stream, g->g, g->h, g->eps, g->eps_mid, g->eps_min, kap, g->charges_dev, g->ncharges,
                              g->phiL, g->fixed);
@@ -899,6 +923,10 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     PF_CUDA(g, cudaGetLastError());
     g->pf1_lc = std::nan("");
     g->assembled = true;
+    if (laplace_maxit) {
+        g->err = "the Laplace solve for phi^L stopped at PF_OPT_LINEAR_MAXIT: b^IF was built from an unconverged phi^L";
+        return PF_NOT_CONVERGED;
+    }
     return PF_OK;
 }
 
@@ -980,6 +1008,7 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
     g->lin_iters.clear();
     g->increments.clear();
     int total = 0, its = 0;
+    bool inner_maxit = false;      // a linear solve stopped at its iteration cap: its result was used as it stood
     // row N4 (Table 2 step 2): initial guess from PF2 with rho' = Psi = 0
     launch_copy_with_dirichlet(g->stream, g->g, g->bc, g->fixed, g->bpf);
     PF_CUDA(g, cudaMemsetAsync(g->phi0, 0, nbytes, g->stream));
@@ -987,6 +1016,7 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
     rc = bicgstab_device(g, make_op(g, 0), g->bpf, g->phi0, g->opt_lin_tol, g->opt_lin_maxit, &its, nullptr, nullptr);
     g->lin_iters.push_back(its); total += its;
     if (rc < 0) return rc;
+    inner_maxit |= rc == PF_NOT_CONVERGED;
     PF_CUDA(g, cudaMemsetAsync(g->psi, 0, nbytes, g->stream));
     int status = PF_NOT_CONVERGED, outer = 0;
     double* phi0 = g->phi0;
@@ -1000,12 +1030,14 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
         rc = bicgstab_device(g, make_op(g, 1), g->bpf, g->psi, g->opt_lin_tol, g->opt_lin_maxit, &its, nullptr, nullptr);
         g->lin_iters.push_back(its); total += its;
         if (rc < 0) return rc;
+        inner_maxit |= rc == PF_NOT_CONVERGED;
         // row N3 (step 4): PF2 -> phi, warm start from phi0
         launch_rhs_pf2(g->stream, g->g, g->bc, g->eps, g->eps_mid, g->uniform, g->psi, g->sigma, phi0, g->fixed, g->bpf);
         PF_CUDA(g, cudaMemcpyAsync(phiw, phi0, nbytes, cudaMemcpyDeviceToDevice, g->stream));
         rc = bicgstab_device(g, make_op(g, 2), g->bpf, phiw, g->opt_lin_tol, g->opt_lin_maxit, &its, nullptr, nullptr);
         g->lin_iters.push_back(its); total += its;
         if (rc < 0) return rc;
+        inner_maxit |= rc == PF_NOT_CONVERGED;
         // row N5 (step 5): relax, then test the increment
         launch_relax(g->stream, g->g.n, g->opt_omega_pf, phi0, phiw, g->dmax_bits);
         unsigned long long bits = 0;
@@ -1014,6 +1046,8 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
         double d;
         std::memcpy(&d, &bits, sizeof(d));
         g->increments.push_back(d);
+        if (!std::isfinite(d))          // reading D7: a NaN fails "d > tol" and would otherwise read as converged
+            return fail(g, PF_ERR_BREAKDOWN, "non-finite potential increment in outer iteration %d", outer);
         std::swap(phi0, phiw);
         if (!(d > tol)) { status = PF_OK; break; }
     }
@@ -1026,6 +1060,10 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
     PF_CUDA(g, cudaGetLastError());
     if (outer_iters_out) *outer_iters_out = outer;
     if (linear_iters_out) *linear_iters_out = total;
+    if (status == PF_OK && inner_maxit) {
+        g->err = "the increment met the tolerance, but at least one linear solve stopped at PF_OPT_LINEAR_MAXIT";
+        return PF_INNER_NOT_CONVERGED;
+    }
     return status;
 }
 

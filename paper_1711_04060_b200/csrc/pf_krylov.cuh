@@ -1,6 +1,7 @@
-// pf_krylov.cuh -- pieces shared by the direct and the tiled Krylov kernels: the elementwise
-// statements of Table 3 (reading R3) and the scalar work that thread 0 of the
-// last block does at each of the three reduction points of an iteration (rows L4-L8).
+// pf_krylov.cuh -- pieces shared by the direct, the tiled and the cooperative Krylov kernels: the elementwise
+// statements of Table 3 (reading R3) and the scalar work at each of the three reduction
+// points of an iteration (rows L4-L8), taken by thread 0 of EVERY block at the start of the next kernel
+// (begin_kernel below: same data, same order, same bits in all blocks; block 0 stores the new state).
 #pragma once
 #include "pf_common.cuh"
 
@@ -34,7 +35,7 @@ __device__ __forceinline__ double s_at(double alpha, double r, double v) { retur
 template <bool PRECOND>
 __device__ __forceinline__ double jacobi(double u, double a0) { return PRECOND ? dvd(u, a0) : u; }
 
-// ---- reduction-point epilogues (thread 0 of the last block only) ------------------------------
+// ---- reduction-point epilogues (the scalar steps; thread 0 of every block, see begin_kernel) -----
 
 // After r0 = b - A x0 (step 2): ||b||, ||r0||, rho_0 = r~.r0 = r0.r0, early exits.
 // norm_mode 1 (Table 3 steps 18-19 as written): the measure is ||r||_inf, absolute, the test
@@ -43,12 +44,22 @@ __device__ __forceinline__ bool converged(const Scalars* sc) {
     return sc->norm_mode == 1 ? sc->rnorm < sc->tol : sc->rnorm <= mul(sc->tol, sc->bnorm);
 }
 
+// Reading D7: a reduced scalar that is not finite (NaN or infinite right-hand side, overflow of a
+// diverging iterate) ends the solve as a breakdown -- a NaN fails every comparison, so without this test it would
+// pass "rho == 0" and never pass the convergence test, and with the maximum norm it could even look converged.
+__device__ __forceinline__ bool finite2(double a, double b) { return isfinite(a) && isfinite(b); }
+
 __device__ __forceinline__ void finish_init(Scalars* sc, double* hist, double bb, double rr, double rmax) {
     sc->bb = bb; sc->rr = rr; sc->rmax = rmax;
     sc->bnorm = sc->norm_mode == 1 ? 1.0 : __dsqrt_rn(bb);
     sc->rnorm = sc->norm_mode == 1 ? rmax : __dsqrt_rn(rr);
     sc->it = 0; sc->first = 1; sc->done = 0; sc->status = 1;
     sc->rho = rr; sc->rho_old = 1.0; sc->alpha = 1.0; sc->omega = 1.0; sc->beta = 0.0;
+    if (!finite2(bb, sc->rnorm)) {                      // D7
+        sc->done = 1; sc->status = -3;
+        if (hist && sc->hist_cap > 0) hist[0] = sc->rnorm;
+        return;
+    }
     if (bb == 0.0) {                       // Q3: b = 0 => x = 0, no iterations (host zeroes x)
         sc->done = 1; sc->status = 0; sc->rnorm = 0.0; sc->bnorm = 0.0;
         if (hist && sc->hist_cap > 0) hist[0] = 0.0;
@@ -63,7 +74,7 @@ __device__ __forceinline__ void finish_init(Scalars* sc, double* hist, double bb
 // After v = A M^-1 p (step 11): alpha = rho/(r~.v) (step 12).
 __device__ __forceinline__ void finish_k1(Scalars* sc, double rtv) {
     sc->rtv = rtv;
-    if (rtv == 0.0) { sc->done = 1; sc->status = -3; return; }
+    if (rtv == 0.0 || !isfinite(rtv)) { sc->done = 1; sc->status = -3; return; }     // Q5, D7
     sc->alpha = dvd(sc->rho, rtv);
 }
 
@@ -71,6 +82,7 @@ __device__ __forceinline__ void finish_k1(Scalars* sc, double rtv) {
 __device__ __forceinline__ void finish_k2(Scalars* sc, double ts, double tt) {
     sc->ts = ts; sc->tt = tt;
     sc->omega = (tt == 0.0) ? 0.0 : dvd(ts, tt);
+    if (!finite2(ts, tt)) { sc->done = 1; sc->status = -3; }                          // D7
 }
 
 // After the x and r updates (steps 16-17): ||r|| test (steps 18-20), then rho and beta of the next
@@ -83,11 +95,12 @@ __device__ __forceinline__ void finish_k3(Scalars* sc, double* hist, double rho_
     if (hist && it < sc->hist_cap) hist[it] = dvd(sc->rnorm, sc->bnorm);
     const double rho_old = sc->rho;
     sc->rho_old = rho_old;
+    if (!isfinite(sc->rnorm)) { sc->done = 1; sc->status = -3; return; }              // D7
     if (converged(sc)) { sc->done = 1; sc->status = 0; return; }
     if (sc->omega == 0.0) { sc->done = 1; sc->status = -3; return; }
     if (it >= sc->maxit) { sc->done = 1; sc->status = 1; return; }
     sc->rho = rho_new;
-    if (rho_new == 0.0) { sc->done = 1; sc->status = -3; return; }
+    if (rho_new == 0.0 || !isfinite(rho_new)) { sc->done = 1; sc->status = -3; return; }     // Q5, D7
     sc->beta = mul(dvd(rho_new, rho_old), dvd(sc->alpha, sc->omega));   // step 8
     sc->first = 0;
 }
@@ -112,6 +125,8 @@ __device__ __forceinline__ bool begin_kernel(int kind, Scalars* S, const Scalars
         rb, kind == PEND_K1 ? PEND_K3 : (kind == PEND_K2 ? PEND_K1 : (kind == PEND_K3 ? PEND_K2 : PEND_NONE)));
     if ((int)threadIdx.x < NWORDS)
         reinterpret_cast<int*>(S)[threadIdx.x] = reinterpret_cast<const int*>(sc_in)[threadIdx.x];
+    // a division range fault raised by an earlier kernel of this solve (dvd_nb, reading D4): requested with the scalars
+    const int faulted = threadIdx.x == 0 ? *rb.fault : 0;
     __syncthreads();
     const int pend = S->pending, nblk = S->pending_nblk;        // the same in every thread of every block
     dd q[2] = {dd_zero(), dd_zero()};
@@ -127,10 +142,15 @@ __device__ __forceinline__ bool begin_kernel(int kind, Scalars* S, const Scalars
         else if (pend == PEND_K2) finish_k2(S, dd_round(q[0]), dd_round(q[1]));
         else if (pend == PEND_K3) finish_k3(S, h, dd_round(q[0]), dd_round(q[1]), m);
         else if (pend == PEND_TRUE) { S->true_rr = dd_round(q[1]); S->true_rmax = m; }
+        // the iterates are invalid from the faulting kernel on: stop here (status stays PF_NOT_CONVERGED) instead of
+        // iterating on them up to maxit; the host repeats the solve with the __ddiv_rn kernels (x is untouched, D3).
+        // Blocks of one launch may disagree for one kernel (a block of THIS launch can raise the flag while others
+        // read it); what they compute is discarded anyway, and the next launch sees done in every block.
+        if (faulted && kind != PEND_INIT && kind != PEND_TRUE) { S->done = 1; S->fault = 1; }
         const bool runs = kind == PEND_INIT || kind == PEND_TRUE || (kind != PEND_NONE && !S->done);
         S->pending = runs ? kind : PEND_NONE;
         S->pending_nblk = (int)linear_grid_size();
-        if (kind == PEND_NONE) S->fault = *rb.fault;             // finalize: what the host is about to read
+        if (kind == PEND_NONE) S->fault = faulted;               // finalize: what the host is about to read
         if (lead) *sc_out = *S;
         // body of a device-side loop: is there another turn?  Not when the solve is over (known with a lag of one
         // iteration: the k1 of iteration i + 1 takes the step that ends iteration i), nor when this k3 closes the

@@ -101,7 +101,7 @@ __device__ __forceinline__ bool sync_reduce(dd (&q)[NQ], double& m, unsigned gen
         for (int k = 0; k < NQ + (MAX ? 1 : 0); ++k) w[k] = __ldcg(rec + k);
 #pragma unroll
         for (int k = 0; k < NQ; ++k) { dd part; part.hi = w[k].x; part.lo = w[k].y; dd_add(q[k], part); }
-        if (MAX) m = fmax(m, w[NQ].x);
+        if (MAX) m = max_abs(m, w[NQ].x);
     }
     block_reduce_dd<NQ>(q, scratch, (nblk + 31) >> 5);     // thread b holds block b's record
     if (MAX) m = block_reduce_max(m, mxs, (nblk + 31) >> 5);
@@ -216,7 +216,7 @@ __global__ void __launch_bounds__(COOP_MAX_THREADS, 1) k_solve_coop(const CoopAr
             kv.r[gi] = ri;
             dd_fma(q[0], bi, bi);
             dd_fma(q[1], ri, ri);
-            rmax = fmax(rmax, fabs(ri));
+            rmax = max_abs(rmax, ri);
         }
         if (!sync_reduce<2, true>(q, rmax, ++gen, a, scratch)) return;
         if (tid == 0) finish_init(&S, hist, dd_round(q[0]), dd_round(q[1]), rmax);
@@ -285,6 +285,7 @@ __global__ void __launch_bounds__(COOP_MAX_THREADS, 1) k_solve_coop(const CoopAr
             if (!sync_reduce<2, false>(q, m, ++gen, a, scratch)) return;
             if (tid == 0) finish_k2(&S, dd_round(q[0]), dd_round(q[1]));
             __syncthreads();
+            if (S.done) break;            // non-finite t.s or t.t (reading D7)
         }
         {   // steps 15-18: y += alpha p + omega s (reading D3); r = s - omega t; r~.r, r.r, ||r||_inf
             const double alpha = S.alpha, omega = S.omega;
@@ -298,7 +299,7 @@ __global__ void __launch_bounds__(COOP_MAX_THREADS, 1) k_solve_coop(const CoopAr
                 kv.r[B.gidx[e]] = rn;
                 dd_fma(q[0], B.rt[e], rn);
                 dd_fma(q[1], rn, rn);
-                rmax = fmax(rmax, fabs(rn));
+                rmax = max_abs(rmax, rn);
             }
             if (!sync_reduce<2, true>(q, rmax, ++gen, a, scratch)) return;
             if (tid == 0) finish_k3(&S, hist, dd_round(q[0]), dd_round(q[1]), rmax);

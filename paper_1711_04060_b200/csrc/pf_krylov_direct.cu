@@ -92,7 +92,7 @@ k_residual(GridDims g, Operator op, KrylovVecs kv, const Scalars* sc_in, Scalars
             dd_fma(q[0], bi, bi);
         }
         dd_fma(q[1], ri, ri);
-        rmax = fmax(rmax, fabs(ri));
+        rmax = max_abs(rmax, ri);
     }
     store_partials<2, true>(q, rmax, scratch, rb, MODE == 0 ? PEND_INIT : PEND_TRUE);
 }
@@ -177,7 +177,7 @@ __device__ __forceinline__ void k3_point(const K3Elem& e, double alpha, double o
     r_new = sub(s, mul(omega, e.t));                              // step 17
     dd_fma(q0, e.rt, r_new);
     dd_fma(q1, r_new, r_new);
-    rmax = fmax(rmax, fabs(r_new));          // ||r||_inf of Table 3 step 18
+    rmax = max_abs(rmax, r_new);             // ||r||_inf of Table 3 step 18 (a NaN is kept)
 }
 
 template <bool VEC, bool LOOP>
@@ -337,7 +337,7 @@ void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, boo
     // inside the body of a device-side loop (c.rb.more) the instance that sets the loop condition
     auto kern = c.rb.more ? (vec ? k3_update<true, true> : k3_update<false, true>)
                           : (vec ? k3_update<true, false> : k3_update<false, false>);
-    launch_pdl(c.pdl, kern, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, sc_in, sc_out, c.rb);
+    note_launch(launch_pdl(c.pdl, kern, dim3(nb), dim3(256), 0, c.stream, c.g.n, kv, sc_in, sc_out, c.rb));
 }
 
 void launch_finalize(const LaunchCtx& c, double* hist) {

@@ -38,6 +38,7 @@
 
 #include <cuda.h>      // CUtensorMap and its enums (types only; the encoder is fetched at run time)
 #include <algorithm>
+#include <atomic>
 #include <type_traits>
 #include <cstring>
 
@@ -538,7 +539,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                         dd_fma(q[0], c.w.x, c.w.x); dd_fma(q[0], c.w.y, c.w.y);
                     }
                     dd_fma(q[1], r0, r0); dd_fma(q[1], r1, r1);
-                    rmax = fmax(rmax, fmax(fabs(r0), fabs(r1)));
+                    rmax = max_abs(max_abs(rmax, r0), r1);
                 }
             };
 
@@ -652,15 +653,16 @@ void launch_inst(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, c
     const Scalars* sc_in; Scalars* sc_out;
     c.next_scalars(sc_in, sc_out);
     using L = Layout<MODE, STORED, CODE32>;
-    static bool configured = false;
+    static std::atomic<unsigned long long> configured{0ull};      // bit d: the attribute is set on device d
     auto kern = k_tma<MODE, PRECOND, STORED, CODE32>;
-    if (!configured) {
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L::TOTAL);
-        configured = true;
+    const unsigned long long bit = 1ull << (c.device & 63);
+    if (c.device >= 64 || !(configured.load(std::memory_order_relaxed) & bit)) {
+        note_launch(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L::TOTAL));
+        configured.fetch_or(bit, std::memory_order_relaxed);
     }
     ++g_launch_count;
-    launch_pdl(c.pdl, kern, dim3(blocks), dim3(NT), (size_t)L::TOTAL, c.stream, tm, c.g, op, kv, sc_in, sc_out, c.rb, depth,
-               ntx, ntiles, nitems);
+    note_launch(launch_pdl(c.pdl, kern, dim3(blocks), dim3(NT), (size_t)L::TOTAL, c.stream, tm, c.g, op, kv, sc_in, sc_out,
+                           c.rb, depth, ntx, ntiles, nitems));
 }
 
 template <int MODE>

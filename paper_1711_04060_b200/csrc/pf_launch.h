@@ -8,6 +8,10 @@ namespace pf {
 
 // Kernel launches issued by this library since load (bench.py reports the difference over the timed region).
 extern long long g_launch_count;
+// First error a kernel launch of this thread returned since the driver last cleared it (pf_api.cu checks it after
+// it has enqueued the iterations of a solve, so a failed launch is reported where it happened).
+extern thread_local cudaError_t g_launch_error;
+inline void note_launch(cudaError_t e) { if (e != cudaSuccess && g_launch_error == cudaSuccess) g_launch_error = e; }
 
 // Launch with programmatic dependent launch allowed: the grid may be scheduled while the preceding kernel of
 // the stream drains (its blocks run their prologue on SMs that are already free); the kernel itself calls
@@ -31,6 +35,7 @@ struct LaunchCtx {
     int* flip;        // host: index of the copy the next kernel reads
     ReduceBuf rb;     // device
     int sm_count;
+    int device;       // CUDA device of the grid (per-device kernel attributes)
     bool pdl;         // programmatic dependent launch allowed
     // the next kernel reads sc[*flip] and its block 0 writes sc[*flip ^ 1]
     void next_scalars(const Scalars*& in, Scalars*& out) const { in = sc[*flip]; out = sc[*flip ^ 1]; *flip ^= 1; }

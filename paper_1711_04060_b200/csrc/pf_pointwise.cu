@@ -135,10 +135,11 @@ k_relax(long long n, double w, double w1, const double* __restrict__ phi0, doubl
         const double p0 = phi0[i];
         const double pn = add(mul(w, p0), mul(w1, phi[i]));
         phi[i] = pn;
-        d = fmax(d, fabs(sub(pn, p0)));
+        d = max_abs(d, sub(pn, p0));
     }
-    for (int s = 16; s > 0; s >>= 1) d = fmax(d, __shfl_xor_sync(0xffffffffu, d, s));
-    // d >= 0: the bit pattern orders like the value.  NaN (a diverged solve) has the largest pattern.
+    // d >= 0 or NaN: the bit pattern orders like the value and a NaN (a diverged solve) has the largest pattern, so
+    // every level of the reduction keeps it (max_abs, pf_common.cuh); the host turns it into PF_ERR_BREAKDOWN
+    for (int s = 16; s > 0; s >>= 1) d = max_abs(d, __shfl_xor_sync(0xffffffffu, d, s));
     if ((threadIdx.x & 31) == 0) atomicMax(dmax_bits, (unsigned long long)__double_as_longlong(d));
 }
 

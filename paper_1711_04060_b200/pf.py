@@ -17,7 +17,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpf_b200.so")
 
-PF_OK, PF_NOT_CONVERGED = 0, 1
+PF_OK, PF_NOT_CONVERGED, PF_INNER_NOT_CONVERGED = 0, 1, 2
 PF_ERR_ARG, PF_ERR_CUDA, PF_ERR_BREAKDOWN, PF_ERR_NONPHYSICAL, PF_ERR_WORKSPACE = -1, -2, -3, -4, -5
 PF_BC_DIRICHLET, PF_BC_NEUMANN = 0, 1
 (PF_OPT_STENCIL, PF_OPT_OMEGA_PF, PF_OPT_LINEAR_TOL, PF_OPT_LINEAR_MAXIT, PF_OPT_CHECK_INTERVAL,

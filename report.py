@@ -1,10 +1,11 @@
 """Report table of BASELINE.md section 4: one row per config x stencil variant, GPU next to the CPU oracle.
 
-    python -m paper_1711_04060_b200.report [--out gpurun_out/report.md] [--skip-512]
-    python -m paper_1711_04060_b200.report --launch-ab [--out gpurun_out/launch_ab.md]     (PF_OPT_GRAPH 0 / 1 / 2 / 3)
+    python report.py [--out gpurun_out/report.md] [--skip-512]
+    python report.py --launch-ab [--out gpurun_out/launch_ab.md]     (PF_OPT_GRAPH 0 / 1 / 2 / 3)
 
 Needs a CUDA device (the GPU columns) and builds the oracle for the CPU columns; the oracle is only ever
 run where it finishes in about a minute (full solves up to 64^3, a few iterations beyond).
+A measurement script beside bench.py, not part of the product package: paper_1711_04060_b200/ never imports oracle/.
 """
 from __future__ import annotations
 
@@ -16,7 +17,7 @@ import time
 import numpy as np
 import torch
 
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 

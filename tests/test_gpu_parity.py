@@ -229,6 +229,43 @@ def test_linear_degenerate_cases(pf, oracle):
     g.close()
 
 
+@pytest.mark.parametrize("kernels", [1, 2, 3])
+@pytest.mark.parametrize("norm", [0, 1])
+@pytest.mark.parametrize("bad", ["nan", "overflow"])
+def test_non_finite_input_is_a_breakdown_not_a_success(pf, oracle, kernels, norm, bad):
+    """Reading D7: a NaN (or a sum of squares that overflows) fails every comparison, so it must not pass the
+    maximum-norm stopping test as 'converged' nor run silently to maxit: all three kernel families and the oracle
+    report a breakdown after zero iterations."""
+    w = ragged_workload(nx=64, ny=32, nz=16, seed=4, mixed_bc=False)      # fits tiled and cooperative kernels
+    rhs = w.rhs.copy()
+    rhs[5 + w.nx * (7 + w.ny * 8)] = np.nan if bad == "nan" else 1e200     # interior node; 1e200^2 overflows: ||b|| = inf
+    ref = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, rhs, tol=1e-6, maxit=50, norm=norm)
+    assert ref["status"] == -3 and ref["iters"] == 0
+    g = pf.Grid.from_workload(w, kernels=kernels, options={pf.PF_OPT_NORM: norm})
+    with pytest.raises(pf.PFError) as e:
+        g.solve_linear(rhs, tol=1e-6, maxit=50)
+    assert e.value.code == pf.PF_ERR_BREAKDOWN
+    # the grid stays usable
+    out = g.solve_linear(w.rhs, tol=1e-8 if norm == 0 else 1e-6)
+    assert out["status"] == 0
+    g.close()
+
+
+def test_pf_reports_cut_off_inner_solves(pf, oracle):
+    """pf_solve_pf whose increment meets a loose tolerance while every linear solve stopped at its cap returns
+    PF_INNER_NOT_CONVERGED (2), like the oracle, not PF_OK."""
+    w = wl.config0(n=24)
+    sp = w.species
+    ref = oracle.solve_pf(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, w.charges, sp.valence, sp.bath_molar,
+                          sp.radii, w.l_c, 1e3, lin_maxit=3, max_outer=5)
+    g = pf.Grid.from_workload(w, options={pf.PF_OPT_LINEAR_MAXIT: 3, pf.PF_OPT_MAX_OUTER: 5})
+    out = g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, 1e3)
+    g.close()
+    assert ref["status"] == 2 and out["status"] == pf.PF_INNER_NOT_CONVERGED
+    assert out["outer_iters"] == ref["outer_iters"] == 1 and out["linear_iters"] == ref["linear_iters"] == 9
+    assert rel_l2(out["phi"].cpu().numpy(), ref["phi"]) <= 1e-12
+
+
 def test_linear_host_buffers(pf, oracle):
     w = ragged_workload()
     ref = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, w.rhs, tol=1e-10)

@@ -265,3 +265,22 @@ def test_paper_stopping_test_max_norm(oracle):
     # the L2-relative mode on the same system stops elsewhere: the modes are really different tests
     out2 = oracle.bicgstab(n, n, n, A, b, tol=tol, maxit=400, precond=False)
     assert out2["status"] == 0 and out2["relres"] <= tol
+
+
+@pytest.mark.parametrize("norm", [0, 1])
+@pytest.mark.parametrize("bad", [float("nan"), 1e200, float("inf")])
+def test_non_finite_right_hand_side_is_a_breakdown(oracle, norm, bad):
+    """Reading D7: Table 3 is silent about non-finite data.  A NaN fails every comparison: it would pass neither
+    'rho == 0' nor the convergence test (and std::max drops it from a maximum norm, which then looks converged), so
+    the solver must stop with the breakdown status after zero iterations instead of returning 0 or running to maxit."""
+    n = 10
+    rng = np.random.default_rng(1)
+    eps = np.where(rng.random(n ** 3) < 0.3, 2.0, 80.0)
+    rhs = rng.standard_normal(n ** 3)
+    rhs[5 + n * (4 + n * 6)] = bad             # an interior node (boundary entries of rhs are ignored, Q20)
+    out = oracle.solve_linear(n, n, n, 0.5, np.zeros(6, dtype=np.int32), np.zeros(6), eps, rhs, tol=1e-6, maxit=40, norm=norm)
+    assert out["status"] == -3 and out["iters"] == 0
+    # and the same system with finite data still converges
+    rhs[5 + n * (4 + n * 6)] = 1.0
+    out = oracle.solve_linear(n, n, n, 0.5, np.zeros(6, dtype=np.int32), np.zeros(6), eps, rhs, tol=1e-6, maxit=400, norm=norm)
+    assert out["status"] == 0
