@@ -295,6 +295,120 @@ int bicgstab(const Grid& g, const double* A, const double* b, double* x, double 
     return status;
 }
 
+// ---- Merged BiCGSTAB: two reduction points per iteration (SURVEY.md section 8(d) "fully merged", 8(f) #3) --------
+// The same Krylov method as Table 3 with the Jacobi step of R3, rearranged so that an iteration has two
+// synchronisation points instead of three (PAPER.md:279 names inner products and synchronisation as where the
+// solver's time goes).  Reading M1: from r_i = s - omega t and s = r_{i-1} - alpha v,
+//     rho_i = r~.r_i = (r~.r_{i-1} - alpha r~.v) - omega r~.t ,
+// a combination of inner products that are all known as soon as omega is: r~.t is reduced together with t.s and
+// t.t, and r~.r_{i-1} together with r~.v and ||r_{i-1}|| one synchronisation earlier.  beta and the next p then need
+// no reduction of their own:
+//     start   r0 = b - A x0; r~ = r0; rho_0 = rhat_0 = r~.r0; p = r0; v = A M^-1 p;                 [r~.v]
+//     i >= 1  alpha = rho_{i-1}/(r~.v); s = r - alpha v; t = A M^-1 s;                              [t.s, t.t, r~.t]
+//             omega = t.s/t.t; x += alpha M^-1 p + omega M^-1 s; r = s - omega t;
+//             rho_i = (rhat_{i-1} - alpha (r~.v)) - omega (r~.t); beta = (rho_i/rho_{i-1})(alpha/omega);
+//             p = r + beta (p - omega v); v = A M^-1 p;                                             [r~.v, rhat_i = r~.r, ||r||]
+//             stop if ||r|| meets the test.
+// SURVEY 8(d) drops the bracket (it vanishes in exact arithmetic by the choice of alpha, leaving rho_i = -omega r~.t).
+// In floating point it must stay: without it the rounding error of rho is never corrected, stays at eps |r~| |r_0|
+// while |r_i| shrinks, and the recurrence stalls near a relative residual of 1e-6..1e-8 (measured with this oracle
+// before the term was restored; tests/test_oracle_merged.py::test_merged_rho_identity_in_the_recurrence).  With it,
+// rho_i differs from the directly reduced r~.r_i only by the rounding of s, r and three scalar operations.
+// The iterates equal Table 3's in exact arithmetic; iteration paths separate from bicgstab() after O(100) iterations
+// like those of any two roundings of the method.  Every elementwise statement is rounded as
+// written; inner products through dot().  The test on ||r|| is made before the next p and v are formed (they are
+// not needed when it passes); statuses, breakdown tests (Q5, D7) and outputs as bicgstab().
+// rho_rec (maxit+1 or null) receives the rho_i the recurrence used, rho_direct (maxit+1 or null) the directly
+// reduced r~.r_i: the pin of the identity compares them.
+int bicgstab_merged(const Grid& g, const double* A, const double* b, double* x, double tol, int maxit,
+                    int precond, int* iters_out, double* relres_out, double* true_relres_out,
+                    double* hist /* maxit+1 or null */, int norm_mode, double* rho_rec, double* rho_direct) {
+    const int64_t N = g.n();
+    std::vector<double> r(N), rt(N), p(N), v(N), s(N), t(N), ph(N), sh(N);
+    *iters_out = 0;
+    double bnorm = norm2(N, b);
+    if (bnorm == 0.0) {  // Q3
+        std::fill(x, x + N, 0.0);
+        if (relres_out) *relres_out = 0.0;
+        if (true_relres_out) *true_relres_out = 0.0;
+        return 0;
+    }
+    dia_spmv(g, A, x, r.data());
+    for (int64_t i = 0; i < N; ++i) r[i] = b[i] - r[i];
+    rt = r;
+    auto measure = [&](const double* u) { return norm_mode == 1 ? norm_inf(N, u) : norm2(N, u); };
+    auto converged = [&](double rn) { return norm_mode == 1 ? rn < tol : rn <= tol * bnorm; };
+    const double scale = norm_mode == 1 ? 1.0 : bnorm;
+    double rnorm = measure(r.data());
+    if (hist) hist[0] = rnorm / scale;
+    int status = 1;
+    if (!std::isfinite(bnorm) || !std::isfinite(rnorm)) status = -3;                  // D7
+    else if (converged(rnorm)) status = 0;                                            // D1
+    double rho = dot(N, rt.data(), r.data());                                         // rho_0
+    double rhat = rho;                                                                // r~.r of the current iterate
+    if (rho_direct) rho_direct[0] = rho;
+    if (rho_rec) rho_rec[0] = rho;
+    int it = 0;
+    double rtv = 0.0;
+    if (status == 1 && maxit > 0) {
+        if (rho == 0.0 || !std::isfinite(rho)) status = -3;
+        else {
+            p = r;
+            for (int64_t i = 0; i < N; ++i) ph[i] = precond ? p[i] / A[i] : p[i];
+            dia_spmv(g, A, ph.data(), v.data());
+            rtv = dot(N, rt.data(), v.data());
+        }
+    }
+    while (status == 1 && it < maxit) {
+        ++it;
+        if (rtv == 0.0 || !std::isfinite(rtv)) { status = -3; --it; break; }
+        double alpha = rho / rtv;
+        for (int64_t i = 0; i < N; ++i) s[i] = r[i] - alpha * v[i];
+        for (int64_t i = 0; i < N; ++i) sh[i] = precond ? s[i] / A[i] : s[i];
+        dia_spmv(g, A, sh.data(), t.data());
+        double ts = dot(N, t.data(), s.data());
+        double tt = dot(N, t.data(), t.data());
+        double rtt = dot(N, rt.data(), t.data());
+        double omega = (tt == 0.0) ? 0.0 : ts / tt;                                   // Q5
+        if (!std::isfinite(ts) || !std::isfinite(tt)) { status = -3; --it; break; }   // D7
+        for (int64_t i = 0; i < N; ++i) x[i] = x[i] + alpha * ph[i] + omega * sh[i];
+        for (int64_t i = 0; i < N; ++i) r[i] = s[i] - omega * t[i];
+        rnorm = measure(r.data());
+        if (hist) hist[it] = rnorm / scale;
+        double rho_new = (rhat - alpha * rtv) - omega * rtt;                          // M1
+        rhat = dot(N, rt.data(), r.data());                                           // reduced with r~.v and ||r||
+        if (rho_direct) rho_direct[it] = rhat;
+        if (rho_rec) rho_rec[it] = rho_new;
+        if (!std::isfinite(rnorm)) { status = -3; break; }                            // D7
+        if (converged(rnorm)) { status = 0; break; }
+        if (omega == 0.0) { status = -3; break; }
+        if (it >= maxit) break;
+        if (rho_new == 0.0 || !std::isfinite(rho_new)) { status = -3; break; }
+        double beta = (rho_new / rho) * (alpha / omega);
+        rho = rho_new;
+        for (int64_t i = 0; i < N; ++i) p[i] = r[i] + beta * (p[i] - omega * v[i]);
+        for (int64_t i = 0; i < N; ++i) ph[i] = precond ? p[i] / A[i] : p[i];
+        dia_spmv(g, A, ph.data(), v.data());
+        rtv = dot(N, rt.data(), v.data());
+    }
+    *iters_out = it;
+    if (relres_out) *relres_out = rnorm / scale;
+    if (true_relres_out) {
+        dia_spmv(g, A, x, t.data());
+        for (int64_t i = 0; i < N; ++i) t[i] = b[i] - t[i];
+        *true_relres_out = measure(t.data()) / scale;
+    }
+    return status;
+}
+
+// solver 0: Table 3 (bicgstab); 1: the merged two-reduction form (bicgstab_merged).
+int krylov(int solver, const Grid& g, const double* A, const double* b, double* x, double tol, int maxit,
+           int precond, int* iters_out, double* relres_out, double* true_relres_out, double* hist, int norm_mode) {
+    return solver == 1 ? bicgstab_merged(g, A, b, x, tol, maxit, precond, iters_out, relres_out, true_relres_out, hist,
+                                         norm_mode, nullptr, nullptr)
+                       : bicgstab(g, A, b, x, tol, maxit, precond, iters_out, relres_out, true_relres_out, hist, norm_mode);
+}
+
 // ---- R2: fixed point charges, trilinear deposition (Eq (3)) ----------------
 // b_i += kappa q w_i / h^3 over the 8 corners of the cell containing the charge.
 void deposit_charges(const Grid& g, const double* ch /* M x 4 */, int M, double* b) {
@@ -632,20 +746,28 @@ int pfo_bicgstab(int nx, int ny, int nz, const double* A, const double* b, doubl
                     norm_mode);
 }
 
+int pfo_bicgstab_merged(int nx, int ny, int nz, const double* A, const double* b, double* x, double tol,
+                        int maxit, int precond, int* iters, double* relres, double* true_relres, double* hist,
+                        int norm_mode, double* rho_rec, double* rho_direct) {
+    int t[6] = {0, 0, 0, 0, 0, 0}; double v[6] = {0, 0, 0, 0, 0, 0};
+    return bicgstab_merged(mk(nx, ny, nz, 1.0, t, v), A, b, x, tol, maxit, precond, iters, relres, true_relres, hist,
+                           norm_mode, rho_rec, rho_direct);
+}
+
 // The library-level call the GPU path mirrors (pf_solve_linear): Poisson operator of the grid,
 // Dirichlet values forced into rhs and x0 (Q4, Q20).
 int pfo_solve_linear(int nx, int ny, int nz, double h, const int* bct, const double* bcv,
                      const double* eps, const double* sigma, const double* rhs, double* x,
                      double tol, int maxit, int precond, int* iters, double* relres,
                      double* true_relres, double* hist, int norm_mode,
-                     const uint8_t* fix_mask, const double* fix_val) {
+                     const uint8_t* fix_mask, const double* fix_val, int solver /* 0 Table 3, 1 merged */) {
     Grid g = mk(nx, ny, nz, h, bct, bcv, fix_mask, fix_val);
     const int64_t N = g.n();
     std::vector<double> A(7 * N), b(rhs, rhs + N);
     assemble_poisson(g, eps, sigma, A.data());
     set_dirichlet(g, b.data());
     set_dirichlet(g, x);
-    return bicgstab(g, A.data(), b.data(), x, tol, maxit, precond, iters, relres, true_relres, hist, norm_mode);
+    return krylov(solver, g, A.data(), b.data(), x, tol, maxit, precond, iters, relres, true_relres, hist, norm_mode);
 }
 
 int pfo_fermi_pointwise(int K, const double* valence, const double* bath_molar, const double* radii,
@@ -673,7 +795,8 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
                  double* steric /* out or null */,
                  int* outer_iters, int* linear_iters, int* lin_iters_hist, int hist_cap,
                  double* incr_hist, const double* fixed_override /* b^IF of the singular-charge model, or null */,
-                 const uint8_t* fix_mask, const double* fix_val /* Omega_f, or null */) {
+                 const uint8_t* fix_mask, const double* fix_val /* Omega_f, or null */,
+                 int solver /* linear solver of every step: 0 Table 3, 1 merged */) {
     Grid g = mk(nx, ny, nz, h, bct, bcv, fix_mask, fix_val);
     const int64_t N = g.n();
     SpeciesTab sp;
@@ -696,7 +819,7 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
     assemble_poisson(g, eps, nullptr, A0.data());
     b = fixed; set_dirichlet(g, b.data());
     set_dirichlet(g, phi0.data());
-    rc = bicgstab(g, A0.data(), b.data(), phi0.data(), lin_tol, lin_maxit, 1, &its, &rr, &tr, nullptr, norm_mode);
+    rc = krylov(solver, g, A0.data(), b.data(), phi0.data(), lin_tol, lin_maxit, 1, &its, &rr, &tr, nullptr, norm_mode);
     record(its);
     if (rc < 0) return rc;
     inner_maxit |= rc == 1;
@@ -707,7 +830,7 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
         fermi_field(sp, N, phi0.data(), solv.data(), rho.data(), sigma.data(), S.data(), nullptr);
         // step 3 / 5: PF1 -> Psi (warm start: previous Psi)
         rhs_pf1(g, solv.data(), rho.data(), b.data());
-        rc = bicgstab(g, A1.data(), b.data(), Psi.data(), lin_tol, lin_maxit, 1, &its, &rr, &tr, nullptr, norm_mode);
+        rc = krylov(solver, g, A1.data(), b.data(), Psi.data(), lin_tol, lin_maxit, 1, &its, &rr, &tr, nullptr, norm_mode);
         record(its);
         if (rc < 0) return rc;
         inner_maxit |= rc == 1;
@@ -715,7 +838,7 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
         assemble_poisson(g, eps, sigma.data(), A2.data());
         rhs_pf2(g, eps, solv.data(), Psi.data(), sigma.data(), phi0.data(), fixed.data(), b.data());
         ph = phi0;
-        rc = bicgstab(g, A2.data(), b.data(), ph.data(), lin_tol, lin_maxit, 1, &its, &rr, &tr, nullptr, norm_mode);
+        rc = krylov(solver, g, A2.data(), b.data(), ph.data(), lin_tol, lin_maxit, 1, &its, &rr, &tr, nullptr, norm_mode);
         record(its);
         if (rc < 0) return rc;
         inner_maxit |= rc == 1;

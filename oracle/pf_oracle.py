@@ -149,6 +149,7 @@ def deposit_charges(nx, ny, nz, h, charges) -> np.ndarray:
 
 
 NORM_REL_L2, NORM_ABS_INF = 0, 1     # stopping test: BASELINE's relative 2-norm / the paper's absolute maximum norm
+SOLVER_TABLE3, SOLVER_MERGED = 0, 1  # Table 3 as written / the merged two-reduction rearrangement (reading M1)
 
 
 def bicgstab(nx, ny, nz, A, b, x0=None, tol=1e-10, maxit=10000, precond=True, history=False, norm=NORM_REL_L2):
@@ -170,9 +171,37 @@ def bicgstab(nx, ny, nz, A, b, x0=None, tol=1e-10, maxit=10000, precond=True, hi
     return out
 
 
+def bicgstab_merged(nx, ny, nz, A, b, x0=None, tol=1e-10, maxit=10000, precond=True, history=False, norm=NORM_REL_L2,
+                    rho_direct=False):
+    """The merged two-reduction BiCGSTAB (reading M1; SURVEY 8(d) "fully merged").  Same outputs as bicgstab();
+    with rho_direct=True also out["rho_rec"][i] = the rho_i the recurrence used, (rhat_{i-1} - alpha r~.v) - omega r~.t,
+    and out["rho_direct"][i] = the directly reduced r~.r_i of every iterate."""
+    A = _f64(A)
+    b = _f64(b)
+    n = nx * ny * nz
+    x = np.zeros(n) if x0 is None else _f64(x0).copy()
+    it = ctypes.c_int(0)
+    rr = ctypes.c_double(0)
+    tr = ctypes.c_double(0)
+    hist = np.full(maxit + 1, np.nan) if history else None
+    rd = np.full(maxit + 1, np.nan) if rho_direct else None
+    rc = np.full(maxit + 1, np.nan) if rho_direct else None
+    st = lib().pfo_bicgstab_merged(nx, ny, nz, _d(A), _d(b), _d(x), ctypes.c_double(tol), int(maxit),
+                                   int(bool(precond)), ctypes.byref(it), ctypes.byref(rr), ctypes.byref(tr), _d(hist),
+                                   int(norm), _d(rc), _d(rd))
+    out = dict(x=x, status=st, iters=it.value, relres=rr.value, true_relres=tr.value)
+    if history:
+        out["hist"] = hist[: it.value + 1]
+    if rho_direct:
+        out["rho_direct"] = rd[: it.value + 1]
+        out["rho_rec"] = rc[: it.value + 1]
+    return out
+
+
 def solve_linear(nx, ny, nz, h, bc_type, bc_value, eps, rhs, x0=None, sigma=None, tol=1e-10,
-                 maxit=10000, precond=True, history=False, norm=NORM_REL_L2, fixed_nodes=None):
-    """What pf_solve_linear computes: the grid's Poisson operator, Dirichlet data forced."""
+                 maxit=10000, precond=True, history=False, norm=NORM_REL_L2, fixed_nodes=None, solver=SOLVER_TABLE3):
+    """What pf_solve_linear computes: the grid's Poisson operator, Dirichlet data forced.
+    solver: SOLVER_TABLE3 (Table 3 of the paper) or SOLVER_MERGED (the two-reduction rearrangement, reading M1)."""
     n = nx * ny * nz
     t, v = _bc(bc_type, bc_value)
     eps = _f64(eps)
@@ -187,7 +216,7 @@ def solve_linear(nx, ny, nz, h, bc_type, bc_value, eps, rhs, x0=None, sigma=None
     st = lib().pfo_solve_linear(nx, ny, nz, ctypes.c_double(h), _i(t), _d(v), _d(eps), _d(sigma), _d(rhs),
                                 _d(x), ctypes.c_double(tol), int(maxit), int(bool(precond)),
                                 ctypes.byref(it), ctypes.byref(rr), ctypes.byref(tr), _d(hist), int(norm),
-                                _u8(fm), _d(fv))
+                                _u8(fm), _d(fv), int(solver))
     out = dict(x=x, status=st, iters=it.value, relres=rr.value, true_relres=tr.value)
     if history:
         out["hist"] = hist[: it.value + 1]
@@ -216,7 +245,7 @@ def fermi_pointwise(valence, bath_molar, radii, phi, solvent=None, water_molar=5
 
 def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar, radii, l_c, tol,
              omega_pf=0.3, lin_tol=1e-10, lin_maxit=10000, max_outer=200, water_molar=55.5, norm=NORM_REL_L2,
-             fixed_override=None, fixed_nodes=None):
+             fixed_override=None, fixed_nodes=None, solver=SOLVER_TABLE3):
     """The outer loop of Table 2 / Table 4 (R5)."""
     n = nx * ny * nz
     t, v = _bc(bc_type, bc_value)
@@ -242,7 +271,7 @@ def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar
                             ctypes.c_double(lin_tol), int(lin_maxit), int(max_outer), int(norm),
                             _d(phi), _d(psi), _d(conc), _d(steric), ctypes.byref(outer), ctypes.byref(lin),
                             _i(lhist), int(cap), _d(ihist), _d(None if fixed_override is None else _f64(fixed_override)),
-                            _u8(fm), _d(fv))
+                            _u8(fm), _d(fv), int(solver))
     return dict(phi=phi, psi=psi, conc=conc, steric=steric, status=st, outer_iters=outer.value,
                 linear_iters=lin.value, lin_iters_hist=lhist[: 2 * outer.value + 1].copy(),
                 incr_hist=ihist[: outer.value].copy())
