@@ -115,6 +115,15 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
                                      diagonal A0 = sum of the six face coefficients from the code instead of reading
                                      it (8 bytes per unknown less; same bits).  0: A0 is read. */
 
+#define PF_OPT_SOLVER         16  /* 0 (default): BiCGSTAB as Table 3 writes it, three kernels and three reduction points per
+                                     iteration.  1: the merged recurrence (SURVEY 8(d) "fully merged"; reading M1 of
+                                     DESIGN.md): rho_i = (r~.r_{i-1} - alpha r~.v) - omega r~.t, two kernels and two
+                                     reduction points per iteration (s, t = A M^-1 s | r, x, p, v = A M^-1 p fused), fewer
+                                     bytes per unknown.  The same method; iterates differ from Table 3's in rounding,
+                                     so its parity reference is the oracle's bicgstab_merged().  Applies to every linear
+                                     solve of the grid, those inside pf_solve_pf included.  Direct and tiled kernel families
+                                     (tiled: on-the-fly stencil); the cooperative kernel implements Table 3 only. */
+
 /* Create a grid: store geometry and boundary conditions, scan eps_map for its palette of distinct
  * values, keep a device copy of the charges.  Assembly itself runs in pf_grid_set_workspace.
  *   eps_map : device, nx*ny*nz doubles, relative permittivity per node; borrowed.

@@ -142,7 +142,7 @@ struct pf_grid {
     bool stored;
     bool assembled;
     double pf1_lc;           // l_c the PF1 operator was assembled for (NaN = none)
-    double *r, *rt, *p0, *p1, *v0, *v1, *t, *y, *bw, *xw;
+    double *r, *r1, *rt, *p0, *p1, *v0, *v1, *t, *y, *bw, *xw;      // r1: second residual buffer of the merged solver
     double *A0, *A0_pf1, *A0_s, *fixed, *psi, *phi0, *phiw, *sigma, *bpf;
     void *code, *code_pf1;   // stencil codes of the on-the-fly variant (pf_common.cuh Operator)
     int code_mode;           // 0 none (palette overflow), 1 uint16, 2 uint32
@@ -165,6 +165,7 @@ struct pf_grid {
     int opt_graph;
     int opt_diag_code;       // k1 forms the Poisson diagonal from the stencil codes (PF_OPT_DIAG_FROM_CODE)
     int opt_norm;            // 0: relative 2-norm (Q3), 1: the paper's absolute maximum norm
+    int opt_solver;          // 0: Table 3 (three kernels per iteration), 1: merged recurrence (two; reading M1)
     int opt_charge_model;    // 0: trilinear deposition (Q22), 1: singular-charge decomposition (Eqs 5-10)
     int charge_model;        // the model the workspace was laid out and assembled for
     double *phiL, *phistar, *A0_L;
@@ -199,7 +200,7 @@ int fail(pf_grid* g, int code, const char* fmt, ...) {
     } while (0)
 
 int n_vectors(bool stored, int charge_model, bool fixed_nodes, bool padx) {
-    return 19 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0) + (fixed_nodes ? 1 : 0) + (padx ? 3 + (stored ? 6 : 0) : 0);
+    return 20 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0) + (fixed_nodes ? 1 : 0) + (padx ? 3 + (stored ? 6 : 0) : 0);
 }
 
 int code_mode_of(const pf_grid* g) { return g->pal.count > PF_MAX_PALETTE ? 0 : (g->pal.count <= 2 ? 1 : 2); }
@@ -261,13 +262,26 @@ Operator make_op(const pf_grid* g, int which /*0 poisson, 1 pf1, 2 poisson+sigma
 LaunchCtx make_ctx(const pf_grid* g) {
     LaunchCtx c;
     c.stream = g->stream; c.g = g->g; c.sc[0] = g->sc[0]; c.sc[1] = g->sc[1]; c.flip = const_cast<int*>(&g->flip);
-    c.rb = g->rb; c.sm_count = g->sm_count; c.device = g->device; c.pdl = true;
+    c.rb = g->rb; c.sm_count = g->sm_count; c.device = g->device; c.pdl = true; c.solver = g->opt_solver;
     return c;
 }
 
 // One BiCGSTAB iteration = three launches (rows L4, L5, L6).  kv's (p, v) buffers are swapped on return.
+// Merged solver (c.solver = 1): two launches (K2M, K31); the current (p, v) pair is (kv.p_in, kv.v_in), K31 writes the
+// other pair and the other r buffer, which become current on return.  The events bracket k1 (nothing), K2M, K31.
 void enqueue_iteration(const LaunchCtx& c, const Operator& op, KrylovVecs& kv, const TmaSet* tma, bool tiled,
                        bool precond, int parity, cudaEvent_t* pe) {
+    if (c.solver == 1) {
+        if (pe) { cudaEventRecord(pe[0], c.stream); cudaEventRecord(pe[1], c.stream); }
+        if (tiled) launch_k2m_tma(c, op, kv, tma, precond, parity); else launch_k2m_direct(c, op, kv, precond);
+        if (pe) cudaEventRecord(pe[2], c.stream);
+        if (tiled) launch_k31_tma(c, op, kv, tma, precond, parity); else launch_k31_direct(c, op, kv, precond);
+        if (pe) cudaEventRecord(pe[3], c.stream);
+        std::swap(kv.p_in, kv.p_out);
+        std::swap(kv.v_in, kv.v_out);
+        std::swap(kv.r, kv.r_out);
+        return;
+    }
     if (pe) cudaEventRecord(pe[0], c.stream);
     if (tiled) launch_k1_tma(c, op, kv, tma, precond, parity); else launch_k1_direct(c, op, kv, precond);
     if (pe) cudaEventRecord(pe[1], c.stream);
@@ -288,7 +302,7 @@ cudaGraphExec_t chunk_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, 
     if (!g->opt_graph || (chunk & 1)) return nullptr;
     for (const auto& cg : g->graphs)
         if (cg.a0 == op.A0 && cg.code == op.code && cg.b == kv.b && cg.x == kv.x && cg.y == kv.y && cg.hist == kv.hist &&
-            cg.precond == (int)precond && cg.tiled == ((int)tiled | (op.diag_code ? 2 : 0)) && cg.chunk == chunk)
+            cg.precond == (int)precond && cg.tiled == ((int)tiled | (op.diag_code ? 2 : 0) | (c.solver ? 4 : 0)) && cg.chunk == chunk)
             return cg.exec;
     if (!g->capture_stream &&
         cudaStreamCreateWithFlags(&g->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
@@ -313,7 +327,7 @@ cudaGraphExec_t chunk_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, 
         cudaGraphExecDestroy(g->graphs.front().exec);
         g->graphs.erase(g->graphs.begin());
     }
-    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled | (op.diag_code ? 2 : 0), chunk, exec});
+    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled | (op.diag_code ? 2 : 0) | (c.solver ? 4 : 0), chunk, exec});
     return exec;
 }
 
@@ -328,7 +342,7 @@ cudaGraphExec_t loop_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, c
     if (g->opt_graph < 2 || (body & 1) || body < 2) return nullptr;
     for (const auto& cg : g->graphs)
         if (cg.a0 == op.A0 && cg.code == op.code && cg.b == kv.b && cg.x == kv.x && cg.y == kv.y && cg.hist == kv.hist &&
-            cg.precond == (int)precond && cg.tiled == ((int)tiled | (op.diag_code ? 2 : 0)) && cg.chunk == -body)
+            cg.precond == (int)precond && cg.tiled == ((int)tiled | (op.diag_code ? 2 : 0) | (c.solver ? 4 : 0)) && cg.chunk == -body)
             return cg.exec;
     if (!g->capture_stream &&
         cudaStreamCreateWithFlags(&g->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
@@ -356,6 +370,7 @@ cudaGraphExec_t loop_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, c
         if (ok) {
             cc.rb.more = (unsigned long long)more;
             for (int k = 0; k < body; ++k) enqueue_iteration(cc, op, kc, g->tma, tiled, precond, k & 1, nullptr);
+            if (cc.solver == 1) launch_finalize_loop(cc, kv.hist);    // takes the pending step, then sets the condition
             cudaGraph_t captured = nullptr;
             ok = cudaStreamEndCapture(cc.stream, &captured) == cudaSuccess;
         }
@@ -368,7 +383,7 @@ cudaGraphExec_t loop_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, c
         cudaGraphExecDestroy(g->graphs.front().exec);
         g->graphs.erase(g->graphs.begin());
     }
-    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled | (op.diag_code ? 2 : 0), -body, exec});
+    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled | (op.diag_code ? 2 : 0) | (c.solver ? 4 : 0), -body, exec});
     return exec;
 }
 
@@ -412,6 +427,9 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
     Scalars init;
     std::memset(&init, 0, sizeof(init));
     init.tol = tol; init.maxit = maxit; init.hist_cap = g->hist ? g->hist_cap : 0; init.norm_mode = g->opt_norm;
+    init.solver = g->opt_solver;
+    const bool merged = g->opt_solver == 1;
+    const int kpi = merged ? 2 : 3;           // kernels per iteration
     // How the iterations reach the GPU (PF_OPT_GRAPH).  The iterations that are bracketed by profiling events are
     // launched one by one (an even number of them); of the others, a device-side loop runs the whole bodies that fit
     // below maxit and the rest follows as stream launches.  Auto: the loop for solves expected to be short (the inner
@@ -437,6 +455,7 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
     KrylovVecs kv;
     kv.b = b; kv.x = x; kv.r = g->r; kv.rt = g->rt; kv.t = g->t; kv.hist = g->hist;
     kv.p_in = g->p0; kv.p_out = g->p1; kv.v_in = g->v0; kv.v_out = g->v1;
+    kv.r_out = merged ? g->r1 : nullptr;
     // D3: with the Jacobi preconditioner step 16 accumulates y = sum(alpha p + omega s); x = x0 + M^-1 y at the end
     kv.y = precond ? g->y : x;
     if (precond) PF_CUDA(g, cudaMemsetAsync(g->y, 0, sizeof(double) * dims.n, g->stream));
@@ -445,11 +464,18 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
         if (g->opt_kernels == 2) return fail(g, PF_ERR_CUDA, "tensor-map encoding failed");
         tiled = false;
     }
+    if (tiled && merged && !tma_merged_ok(g->tma)) {
+        // the merged kernels of the tiled family exist for operators in code form; stored coefficients use the direct ones
+        if (g->opt_kernels == 2) return fail(g, PF_ERR_ARG, "the tiled kernels of the merged solver need the on-the-fly stencil");
+        tiled = false;
+    }
     if (g->opt_kernels == 2 && allow_tiled && !op_faulted && !tiled)
         return fail(g, PF_ERR_ARG, "the tiled kernels need 16-byte aligned vectors");
     // Small grids: the whole solve in one cooperative kernel (pf_krylov_coop.cu)
     CoopPlan plan;
-    const bool coop = allow_tiled && allow_coop && use_coop(g, op, &plan);
+    const bool coop = allow_tiled && allow_coop && !merged && use_coop(g, op, &plan);
+    if (g->opt_kernels == 3 && merged)
+        return fail(g, PF_ERR_ARG, "the cooperative kernel implements Table 3 only (PF_OPT_SOLVER = 0)");
     if (g->opt_kernels == 3 && allow_tiled && !coop)
         return fail(g, PF_ERR_ARG, "the cooperative kernel needs an operator in code form and a grid whose bricks "
                                    "fit the shared memory of the SMs (about <= 72^3)");
@@ -479,7 +505,13 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
         fin = *g->sc_host[0];
         return finish_solve(g, c, op, kv, fin, false, iters_out, relres_out, true_relres_out);
     }
-    if (tiled) launch_residual_tma(c, op, kv, g->tma, 0); else launch_residual_direct(c, op, kv, 0);
+    if (tiled) launch_residual_tma(c, op, kv, g->tma, 0, precond); else launch_residual_direct(c, op, kv, 0);
+    if (merged && maxit > 0) {
+        // the merged recurrence starts from v = A M^-1 r0 (and r~.v): the ordinary k1 with p = r (first = 1)
+        if (tiled) launch_k1_tma(c, op, kv, g->tma, precond, 0); else launch_k1_direct(c, op, kv, precond);
+        std::swap(kv.p_in, kv.p_out);
+        std::swap(kv.v_in, kv.v_out);
+    }
 
     const int chunk = g->opt_check < 1 ? 1 : g->opt_check;
     int launched = 0, slot = 0;
@@ -505,9 +537,12 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
         // kernels the loop ran: whole bodies of 3 per iteration, up to loop_end; if the solve ended before that, the
         // body in which its last iteration ran is the last one unless that iteration was the body's last (its k3's
         // step is then taken by the next body's first kernel)
+        // (merged solver: a body ends with the finalize that sets the condition, so the state is exact: the body in
+        // which the last iteration ran is the last one)
         const int bodies = fin.it >= loop_end ? (loop_end - nprof_all) / LOOP_BODY
-                                              : std::max(fin.it - nprof_all, 0) / LOOP_BODY + 1;
-        pf::g_launch_count += 3ll * LOOP_BODY * bodies;
+                         : (merged ? std::max((std::max(fin.it - nprof_all, 0) + LOOP_BODY - 1) / LOOP_BODY, 1)
+                                   : std::max(fin.it - nprof_all, 0) / LOOP_BODY + 1);
+        pf::g_launch_count += ((long long)kpi * LOOP_BODY + (merged ? 1 : 0)) * bodies;
         done = true;
     }
     while (!done) {
@@ -520,7 +555,7 @@ int bicgstab_core(pf_grid* g, const GridDims& dims, const Operator& op, const do
         cudaGraphExec_t exec = (todo == chunk && !profiled) ? chunk_graph(g, c, op, kv, tiled, precond, chunk) : nullptr;
         if (exec) {
             PF_CUDA(g, cudaGraphLaunch(exec, g->stream));
-            pf::g_launch_count += 3ll * chunk;
+            pf::g_launch_count += (long long)kpi * chunk;
         } else {
             for (int k = 0; k < todo; ++k) {
                 const bool prof = g->opt_profile && (size_t)(4 * (launched + k) + 3) < g->prof_ev.size();
@@ -588,7 +623,7 @@ int bicgstab_device(pf_grid* g, const Operator& op, const double* b, double* x, 
                     int* iters_out, double* relres_out, double* true_relres_out) {
     CoopPlan plan;
     const bool widen = g->padx && (!op.stored || g->offdp[0]) && g->opt_kernels != 1 && g->opt_kernels != 3 &&
-                       use_tiled(g, g->gk) && !use_coop(g, op, &plan);
+                       use_tiled(g, g->gk) && (g->opt_solver == 1 || !use_coop(g, op, &plan));
     if (!widen)
         return bicgstab_core(g, g->g, op, b, x, tol, maxit, iters_out, relres_out, true_relres_out, true, true);
     launch_widen(g->stream, g->g, op.A0, g->A0p, 1.0);
@@ -689,7 +724,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->opt_profile = 0; g->prof_ms[0] = g->prof_ms[1] = g->prof_ms[2] = 0.0;
     g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
-    g->capture_stream = nullptr; g->opt_graph = 3; g->opt_diag_code = 1; g->opt_norm = 0;
+    g->capture_stream = nullptr; g->opt_graph = 3; g->opt_diag_code = 1; g->opt_norm = 0; g->opt_solver = 0;
     g->opt_charge_model = 0; g->charge_model = 0; g->phiL = g->phistar = g->A0_L = nullptr; g->code_L = nullptr;
     g->ctab_L = nullptr; g->laplace_iters = 0; g->fixv = nullptr; g->bc.fixv = nullptr;
     g->small = nullptr;
@@ -829,6 +864,9 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
             g->opt_charge_model = iv; return PF_OK;
         case PF_OPT_DIAG_FROM_CODE:
             g->opt_diag_code = iv != 0; return PF_OK;
+        case PF_OPT_SOLVER:
+            if (iv != 0 && iv != 1) return fail(g, PF_ERR_ARG, "solver must be 0 (Table 3) or 1 (merged)");
+            g->opt_solver = iv; return PF_OK;
         case PF_OPT_GRAPH:
             if (iv < 0 || iv > 3) return fail(g, PF_ERR_ARG, "graph must be 0, 1, 2 or 3");
             g->opt_graph = iv; return PF_OK;
@@ -862,7 +900,7 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     const size_t vec = align_up(sizeof(double) * (size_t)g->gk.n, 256);     // every vector has room for the widened box
     char* base = (char*)dev_ptr;
     auto take = [&]() { double* p = (double*)base; base += vec; return p; };
-    g->r = take(); g->rt = take(); g->p0 = take(); g->p1 = take(); g->v0 = take(); g->v1 = take();
+    g->r = take(); g->r1 = take(); g->rt = take(); g->p0 = take(); g->p1 = take(); g->v0 = take(); g->v1 = take();
     g->t = take(); g->y = take(); g->bw = take(); g->xw = take();
     g->A0 = take(); g->A0_pf1 = take(); g->A0_s = take(); g->fixed = take(); g->psi = take();
     g->phi0 = take(); g->phiw = take(); g->sigma = take(); g->bpf = take();

@@ -14,6 +14,7 @@ struct KrylovVecs {
     double* x;
     double* y;           // preconditioned solves accumulate step 16 here (reading D3); == x when M = I
     double* r;
+    double* r_out;       // merged solver: its fused kernel reads r at neighbour nodes while other blocks write the new r
     double* rt;          // r~ = r0
     double* p_in;  double* p_out;
     double* v_in;  double* v_out;
@@ -55,6 +56,7 @@ __device__ __forceinline__ void finish_init(Scalars* sc, double* hist, double bb
     sc->rnorm = sc->norm_mode == 1 ? rmax : __dsqrt_rn(rr);
     sc->it = 0; sc->first = 1; sc->done = 0; sc->status = 1;
     sc->rho = rr; sc->rho_old = 1.0; sc->alpha = 1.0; sc->omega = 1.0; sc->beta = 0.0;
+    sc->rhat = rr; sc->rho_next = rr; sc->rtt = 0.0;
     if (!finite2(bb, sc->rnorm)) {                      // D7
         sc->done = 1; sc->status = -3;
         if (hist && sc->hist_cap > 0) hist[0] = sc->rnorm;
@@ -105,6 +107,46 @@ __device__ __forceinline__ void finish_k3(Scalars* sc, double* hist, double rho_
     sc->first = 0;
 }
 
+// ---- the merged solver (SURVEY 8(d) "fully merged", 8(f) #3; reading M1 of DESIGN.md) ----------------------------
+// Two kernels and two reduction points per iteration instead of three:
+//   K2M  s = r - alpha v; t = A M^-1 s;                                   reduces t.s, t.t, r~.t
+//   K31  r' = s - omega t; y += alpha p + omega s; p' = r' + beta (p - omega v); v' = A M^-1 p';
+//                                                                         reduces r~.v', r'.r' (max |r'|), r~.r'
+// with rho_i = (r~.r_{i-1} - alpha r~.v) - omega r~.t, so that beta is known when K31 starts.  The first v = A M^-1 r0
+// comes from the ordinary k1 (first = 1).  Statement for statement the oracle's bicgstab_merged().
+
+// After K2M: omega (step 15), rho_i and beta.  Whether iteration i was the last one (convergence, omega = 0, maxit)
+// is only known once K31 has reduced ||r'||; beta may therefore be meaningless in the last iteration (its p', v' are
+// never used).
+__device__ __forceinline__ void finish_k2m(Scalars* sc, double ts, double tt, double rtt) {
+    sc->ts = ts; sc->tt = tt; sc->rtt = rtt;
+    sc->omega = (tt == 0.0) ? 0.0 : dvd(ts, tt);
+    if (!finite2(ts, tt)) { sc->done = 1; sc->status = -3; return; }                   // D7
+    const double rho_new = sub(sub(sc->rhat, mul(sc->alpha, sc->rtv)), mul(sc->omega, rtt));   // M1
+    sc->rho_next = rho_new;
+    sc->beta = mul(dvd(rho_new, sc->rho), dvd(sc->alpha, sc->omega));
+}
+
+// After K31: close iteration i (||r|| test, steps 18-20), then alpha of iteration i + 1.
+__device__ __forceinline__ void finish_k31(Scalars* sc, double* hist, double rtv, double rr, double rhat, double rmax) {
+    sc->rr = rr; sc->rmax = rmax;
+    sc->rnorm = sc->norm_mode == 1 ? rmax : __dsqrt_rn(rr);
+    const int it = sc->it + 1;
+    sc->it = it;
+    if (hist && it < sc->hist_cap) hist[it] = dvd(sc->rnorm, sc->bnorm);
+    sc->rho_old = sc->rho;
+    if (!isfinite(sc->rnorm)) { sc->done = 1; sc->status = -3; return; }              // D7
+    if (converged(sc)) { sc->done = 1; sc->status = 0; return; }
+    if (sc->omega == 0.0) { sc->done = 1; sc->status = -3; return; }
+    if (it >= sc->maxit) { sc->done = 1; sc->status = 1; return; }
+    const double rho_new = sc->rho_next;
+    if (rho_new == 0.0 || !isfinite(rho_new)) { sc->done = 1; sc->status = -3; return; }     // Q5, D7
+    sc->rho = rho_new; sc->rhat = rhat; sc->rtv = rtv;
+    sc->first = 0;
+    if (rtv == 0.0 || !isfinite(rtv)) { sc->done = 1; sc->status = -3; return; }
+    sc->alpha = dvd(rho_new, rtv);
+}
+
 // ---- start of every kernel of a solve (rows L7, L8) ---------------------------------------------
 // Copy the device scalars into the block's shared memory, combine the partial sums the previous kernel left
 // (pf_common.cuh), take the scalar step that was waiting for them, and note what THIS kernel (kind `kind`, a
@@ -122,17 +164,27 @@ __device__ __forceinline__ bool begin_kernel(int kind, Scalars* S, const Scalars
     // what usually precedes a kernel of this kind (k3 or the initial residual before k1, k1 before k2, k2 before
     // k3): its partials are requested together with the scalars
     const PartialPrefetch pre = prefetch_partials(
-        rb, kind == PEND_K1 ? PEND_K3 : (kind == PEND_K2 ? PEND_K1 : (kind == PEND_K3 ? PEND_K2 : PEND_NONE)));
+        rb, kind == PEND_K1 ? PEND_K3 : (kind == PEND_K2 ? PEND_K1 : (kind == PEND_K3 ? PEND_K2
+          : (kind == PEND_K2M ? PEND_K31 : (kind == PEND_K31 ? PEND_K2M : PEND_NONE)))));
     if ((int)threadIdx.x < NWORDS)
         reinterpret_cast<int*>(S)[threadIdx.x] = reinterpret_cast<const int*>(sc_in)[threadIdx.x];
     // a division range fault raised by an earlier kernel of this solve (dvd_nb, reading D4): requested with the scalars
     const int faulted = threadIdx.x == 0 ? *rb.fault : 0;
     __syncthreads();
     const int pend = S->pending, nblk = S->pending_nblk;        // the same in every thread of every block
+    // Thread 0 rewrites S->pending below.  With partial sums pending, the barriers of the combine separate these
+    // reads from that write; without (the first kernel after a finalize, i.e. at every polling-chunk boundary) nothing
+    // did, and a warp that read late saw the NEW value, entered a combine the other warps skipped and left the block
+    // with mismatched barriers: wrong sums or a hang, depending on timing (found in round 2 when two unrelated
+    // one-instruction changes each made it appear).
+    __syncthreads();
     dd q[2] = {dd_zero(), dd_zero()};
+    dd q3[3] = {dd_zero(), dd_zero(), dd_zero()};
     double m = 0.0;
     if (pend == PEND_K1) { dd q1[1]; combine_partials<1, false>(q1, m, nblk, scratch, rb, pend, pre); q[0] = q1[0]; }
     else if (pend == PEND_K2) combine_partials<2, false>(q, m, nblk, scratch, rb, pend, pre);
+    else if (pend == PEND_K2M) combine_partials<3, false>(q3, m, nblk, scratch, rb, pend, pre);
+    else if (pend == PEND_K31) combine_partials<3, true>(q3, m, nblk, scratch, rb, pend, pre);
     else if (pend != PEND_NONE) combine_partials<2, true>(q, m, nblk, scratch, rb, pend, pre);
     if (threadIdx.x == 0) {
         const bool lead = linear_block_id() == 0;
@@ -141,6 +193,8 @@ __device__ __forceinline__ bool begin_kernel(int kind, Scalars* S, const Scalars
         else if (pend == PEND_K1) finish_k1(S, dd_round(q[0]));
         else if (pend == PEND_K2) finish_k2(S, dd_round(q[0]), dd_round(q[1]));
         else if (pend == PEND_K3) finish_k3(S, h, dd_round(q[0]), dd_round(q[1]), m);
+        else if (pend == PEND_K2M) finish_k2m(S, dd_round(q3[0]), dd_round(q3[1]), dd_round(q3[2]));
+        else if (pend == PEND_K31) finish_k31(S, h, dd_round(q3[0]), dd_round(q3[1]), dd_round(q3[2]), m);
         else if (pend == PEND_TRUE) { S->true_rr = dd_round(q[1]); S->true_rmax = m; }
         // the iterates are invalid from the faulting kernel on: stop here (status stays PF_NOT_CONVERGED) instead of
         // iterating on them up to maxit; the host repeats the solve with the __ddiv_rn kernels (x is untouched, D3).

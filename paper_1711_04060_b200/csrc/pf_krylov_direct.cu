@@ -162,6 +162,88 @@ k2_direct(GridDims g, Operator op, KrylovVecs kv, const Scalars* sc_in, Scalars*
     store_partials<2, false>(q, 0.0, scratch, rb, PEND_K2);
 }
 
+// ---- the merged solver (pf_krylov.cuh; reading M1): two kernels per iteration -----------------------------------
+// K2M = k2 that also reduces r~.t.  The current (p, v) pair is (kv.p_in, kv.v_in).
+template <bool PRECOND>
+__global__ void __launch_bounds__(DIRECT_THREADS)
+k2m_direct(GridDims g, Operator op, KrylovVecs kv, const Scalars* sc_in, Scalars* sc_out, ReduceBuf rb) {
+    __shared__ double ctab_s[PF_CTAB];
+    __shared__ dd scratch[3 * 32];
+    __shared__ Scalars S;
+    if (!begin_kernel(PEND_K2M, &S, sc_in, sc_out, rb, kv.hist, scratch)) return;
+    load_ctab(op, ctab_s);
+    const double alpha = S.alpha;
+    dd q[3] = {dd_zero(), dd_zero(), dd_zero()};
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
+        Nbr n = neighbours(g, i);
+        double c[6];
+        row_coeffs(op, g, ctab_s, i, n, c);
+        const double a0 = op.A0[i];
+        const double si = s_at(alpha, kv.r[i], kv.v_in[i]);
+        double acc = mul(a0, jacobi<PRECOND>(si, a0));
+#pragma unroll
+        for (int d = 0; d < 6; ++d)
+            if (c[d] != 0.0) {
+                const long long j = n.j[d];
+                const double sj = s_at(alpha, kv.r[j], kv.v_in[j]);
+                acc = add(acc, mul(c[d], jacobi<PRECOND>(sj, op.A0[j])));
+            }
+        kv.t[i] = acc;
+        dd_fma(q[0], acc, si);
+        dd_fma(q[1], acc, acc);
+        dd_fma(q[2], kv.rt[i], acc);
+    }
+    store_partials<3, false>(q, 0.0, scratch, rb, PEND_K2M);
+}
+
+// K31 = steps 16-17 of iteration i fused with steps 5-11 of iteration i + 1: r' = s - omega t, y += alpha p + omega s,
+// p' = r' + beta (p - omega v), v' = A M^-1 p'; reduces r~.v', r'.r' (and max |r'|), r~.r'.  r' and p' are formed at
+// the node and at its six neighbours from the OLD r, p, v, t, which is why r', p', v' go to second buffers.
+template <bool PRECOND>
+__global__ void __launch_bounds__(DIRECT_THREADS)
+k31_direct(GridDims g, Operator op, KrylovVecs kv, const Scalars* sc_in, Scalars* sc_out, ReduceBuf rb) {
+    __shared__ double ctab_s[PF_CTAB];
+    __shared__ dd scratch[3 * 32];
+    __shared__ Scalars S;
+    if (!begin_kernel(PEND_K31, &S, sc_in, sc_out, rb, kv.hist, scratch)) return;
+    load_ctab(op, ctab_s);
+    const double alpha = S.alpha, omega = S.omega, beta = S.beta;
+    dd q[3] = {dd_zero(), dd_zero(), dd_zero()};
+    double rmax = 0.0;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
+        Nbr n = neighbours(g, i);
+        double c[6];
+        row_coeffs(op, g, ctab_s, i, n, c);
+        const double a0 = op.A0[i];
+        const double pi = kv.p_in[i], vi = kv.v_in[i];
+        const double si = s_at(alpha, kv.r[i], vi);
+        const double rn = sub(si, mul(omega, kv.t[i]));                          // step 17
+        const double pn = p_new_at<PRECOND>(false, beta, omega, rn, pi, vi);     // step 9 of the next iteration
+        double acc = mul(a0, jacobi<PRECOND>(pn, a0));
+#pragma unroll
+        for (int d = 0; d < 6; ++d)
+            if (c[d] != 0.0) {
+                const long long j = n.j[d];
+                const double vj = kv.v_in[j];
+                const double rj = sub(s_at(alpha, kv.r[j], vj), mul(omega, kv.t[j]));
+                const double pj = p_new_at<PRECOND>(false, beta, omega, rj, kv.p_in[j], vj);
+                acc = add(acc, mul(c[d], jacobi<PRECOND>(pj, op.A0[j])));
+            }
+        kv.y[i] = add(add(kv.y[i], mul(alpha, pi)), mul(omega, si));             // step 16 (reading D3)
+        kv.r_out[i] = rn;
+        kv.p_out[i] = pn;
+        kv.v_out[i] = acc;
+        const double rti = kv.rt[i];
+        dd_fma(q[0], rti, acc);
+        dd_fma(q[1], rn, rn);
+        dd_fma(q[2], rti, rn);
+        rmax = max_abs(rmax, rn);
+    }
+    store_partials<3, true>(q, rmax, scratch, rb, PEND_K31);
+}
+
 }  // namespace
 
 // Steps 16-17 are pointwise; this kernel serves both kernel families.  Reads r, v, p, y, t, r~ and
@@ -249,6 +331,19 @@ k_finalize(Scalars* sc, ReduceBuf rb, double* hist) {
     begin_kernel(PEND_NONE, &S, sc, sc, rb, hist, scratch);
 }
 
+// The same at the end of a body of the device-side loop of the merged solver (pf_api.cu loop_graph): the state is then
+// exact, and the body's WHILE node repeats while the solve is not over and iterations of the loop are left.  (The
+// three-kernel solver keeps this call in its k3 instead; kernels that can set a conditional handle are invisible to
+// Nsight Compute, so the hot kernels of the merged solver stay free of it.)
+__global__ void __launch_bounds__(256)
+k_finalize_loop(Scalars* sc, ReduceBuf rb, double* hist) {
+    __shared__ dd scratch[3 * 32];
+    __shared__ Scalars S;
+    begin_kernel(PEND_NONE, &S, sc, sc, rb, hist, scratch);
+    if (threadIdx.x == 0 && rb.more)
+        cudaGraphSetConditional((cudaGraphConditionalHandle)rb.more, (S.done || S.it >= S.loop_end) ? 0u : 1u);
+}
+
 // x = x + M^-1 y (reading D3).  y is exactly 0 on identity rows, so Dirichlet values of x are kept.
 __global__ void __launch_bounds__(256)
 k_finish_x(long long n, const double* __restrict__ A0, const double* __restrict__ y, double* __restrict__ x) {
@@ -322,6 +417,24 @@ void launch_k2_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& 
     else         { ++g_launch_count; k2_direct<false><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, sc_in, sc_out, c.rb); }
 }
 
+void launch_k2m_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond) {
+    const Scalars* sc_in; Scalars* sc_out;
+    c.next_scalars(sc_in, sc_out);
+    const int nb = direct_blocks(c.g.n, c.sm_count);
+    ++g_launch_count;
+    if (precond) k2m_direct<true><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, sc_in, sc_out, c.rb);
+    else         k2m_direct<false><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, sc_in, sc_out, c.rb);
+}
+
+void launch_k31_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond) {
+    const Scalars* sc_in; Scalars* sc_out;
+    c.next_scalars(sc_in, sc_out);
+    const int nb = direct_blocks(c.g.n, c.sm_count);
+    ++g_launch_count;
+    if (precond) k31_direct<true><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, sc_in, sc_out, c.rb);
+    else         k31_direct<false><<<nb, DIRECT_THREADS, 0, c.stream>>>(c.g, op, kv, sc_in, sc_out, c.rb);
+}
+
 void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond) {
     const Scalars* sc_in; Scalars* sc_out;
     c.next_scalars(sc_in, sc_out);
@@ -343,6 +456,11 @@ void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, boo
 void launch_finalize(const LaunchCtx& c, double* hist) {
     ++g_launch_count;
     k_finalize<<<1, 256, 0, c.stream>>>(c.current_scalars(), c.rb, hist);
+}
+
+void launch_finalize_loop(const LaunchCtx& c, double* hist) {
+    ++g_launch_count;
+    k_finalize_loop<<<1, 256, 0, c.stream>>>(c.current_scalars(), c.rb, hist);
 }
 
 void launch_finish_x(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv) {

@@ -58,9 +58,10 @@ constexpr int OWN_BYTES = TX * TY * 8;                            // 8192
 constexpr int NU = 3;                    // shared buffers of u (planes k, k+1 live, k+2 being written)
 static_assert(TY <= 32, "one halo column node per lane of a halo warp");
 
-enum { MODE_R0 = 0, MODE_R1 = 1, MODE_K1 = 2, MODE_K2 = 3, MODE_K1D = 4 };
+enum { MODE_R0 = 0, MODE_R1 = 1, MODE_K1 = 2, MODE_K2 = 3, MODE_K1D = 4, MODE_K2M = 5, MODE_K31 = 6, MODE_K31D = 7 };
 // MODE_K1D: k1 for operators whose diagonal is the sum of their face coefficients (Poisson without sigma): A0 is
 // not read but formed from the stencil code, whose box then covers the halo ring too.
+// MODE_K2M, MODE_K31 (MODE_K31D: diagonal from the codes): the two kernels of the merged solver (pf_krylov.cuh).
 constexpr int CXO = 8;                   // code box with halo: starts CXO nodes left of the tile (the TMA unit wants the
 constexpr int BXC = TX + 2 * CXO;        // box to start on a 16-byte boundary of the row: 8 two-byte entries), rows of 160 bytes
 
@@ -70,11 +71,14 @@ template <> struct ModeTraits<MODE_R1> { static constexpr int NF = 2; static con
 template <> struct ModeTraits<MODE_K1> { static constexpr int NF = 4; static constexpr bool OWN = true;  static constexpr int STAGES = 3; };
 template <> struct ModeTraits<MODE_K1D> { static constexpr int NF = 3; static constexpr bool OWN = true; static constexpr int STAGES = 3; };   // (4 fit, within 1.2 KB of the limit: 1 % faster)
 template <> struct ModeTraits<MODE_K2> { static constexpr int NF = 3; static constexpr bool OWN = false; static constexpr int STAGES = 4; };
+template <> struct ModeTraits<MODE_K2M> { static constexpr int NF = 3; static constexpr bool OWN = true; static constexpr int STAGES = 4; };
+template <> struct ModeTraits<MODE_K31> { static constexpr int NF = 5; static constexpr bool OWN = true; static constexpr int STAGES = 3; };
+template <> struct ModeTraits<MODE_K31D> { static constexpr int NF = 4; static constexpr bool OWN = true; static constexpr int STAGES = 3; };
 
-// Halo fields in stage order.  K1: r, p, v, A0.  K1D: r, p, v.  K2: r, v, A0.  R0/R1: x, A0.
-// Own-only field (tile without halo): K1: r~;  R0/R1: b.
+// Halo fields in stage order.  K1: r, p, v, A0.  K1D: r, p, v.  K2, K2M: r, v, A0.  K31: r, p, v, t, A0.  K31D: r, p, v, t.
+// R0/R1: x, A0.  Own-only field (tile without halo): K1, K2M, K31: r~;  R0/R1: b.
 struct TmaArgs {
-    CUtensorMap f[4];
+    CUtensorMap f[5];
     CUtensorMap own;
     CUtensorMap code;
 };
@@ -82,7 +86,7 @@ struct TmaArgs {
 template <int MODE, bool STORED, bool CODE32>
 struct Layout {
     using T = ModeTraits<MODE>;
-    static constexpr bool DIAG = MODE == MODE_K1D;
+    static constexpr bool DIAG = MODE == MODE_K1D || MODE == MODE_K31D;
     static constexpr int CODE_TX = DIAG ? BXC * BY * 2 : TX * TY * (CODE32 ? 4 : 2);   // bytes the TMA unit delivers
     static constexpr int CODE_BYTES = STORED ? 0 : ((CODE_TX + 127) / 128) * 128;
     static constexpr int STAGE_BYTES = T::NF * FIELD_BYTES + (T::OWN ? OWN_BYTES : 0) + CODE_BYTES;
@@ -101,20 +105,28 @@ struct Layout {
     static constexpr int BAR_OFF = SCRATCH_OFF + 3 * 32 * (int)sizeof(dd);
     static constexpr int SC_OFF = ((BAR_OFF + 16 * T::STAGES + 8 * NU + 15) / 16) * 16;   // after full[S], empty[S], ready[NU]
     static constexpr int TOTAL = SC_OFF + 256;                       // the block's copy of the scalars
+    static_assert(TOTAL <= 232448, "dynamic shared memory of a block (227 KB)");
     static_assert(CTAB_OFF % 128 == 0, "ctab_at ORs table offsets into the table address");
     static constexpr unsigned TX_BYTES = (unsigned)(T::NF * BX * BY * 8 + (T::OWN ? OWN_BYTES : 0) + (STORED ? 0 : CODE_TX));
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+// The mbarriers are addressed by 32-bit shared-memory addresses that every thread derives once from the block's
+// base (kept opaque to the compiler, which otherwise re-derives the base from special registers at every use).
+__device__ __forceinline__ unsigned opaque_u32(unsigned v) {
+    unsigned r;
+    asm volatile("mov.u32 %0, %1;" : "=r"(r) : "r"(v));
+    return r;
+}
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ bool mbar_try_wait(unsigned long long* bar, unsigned parity) {
+__device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity) {
     unsigned ok;
     asm volatile(
         "{\n"
@@ -123,25 +135,53 @@ __device__ __forceinline__ bool mbar_try_wait(unsigned long long* bar, unsigned 
         "selp.u32 %0, 1, 0, p;\n"
         "}\n"
         : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
+        : "r"(bar), "r"(parity)
         : "memory");
     return ok != 0;
 }
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, unsigned long long* bar, int x, int y,
-                                            int z) {
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) { while (!mbar_try_wait(bar, parity)) {} }
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* map, unsigned bar, int x, int y, int z) {
     asm volatile(
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z)
+        ::"r"(dst), "l"(map), "r"(bar), "r"(x), "r"(y), "r"(z)
         : "memory");
 }
 
+// Position in a ring of N slots that is walked one slot at a time: slot index and the parity of the current lap
+// (the phase bit an mbarrier of the slot is waited on with).  Advancing costs an add, a compare and two selects,
+// whatever N is -- the rings run on across the work items of a persistent block, so the position is run-time state.
+template <int N>
+struct Ring {
+    unsigned idx, par;
+    __device__ __forceinline__ void reset() { idx = 0u; par = 0u; }
+    __device__ __forceinline__ void next() {
+        const bool wrap = idx == (unsigned)(N - 1);
+        idx = wrap ? 0u : idx + 1u;
+        par ^= wrap ? 1u : 0u;
+    }
+};
+
 template <int MODE, bool PRECOND>
 __device__ __forceinline__ double u_of(double r, double p, double v, double a, bool first, double c1, double c2,
-                                       double& numer, unsigned& fault) {
+                                       double& numer, DivRange& range) {
     if (MODE == MODE_K1 || MODE == MODE_K1D) numer = p_new_at<PRECOND>(first, c1, c2, r, p, v);
-    else if (MODE == MODE_K2) numer = s_at(c1, r, v);
+    else if (MODE == MODE_K2 || MODE == MODE_K2M) numer = s_at(c1, r, v);
     else { numer = r; return r; }    // residual modes: the field is x itself (passed in r)
-    return PRECOND ? dvd_nb(numer, a, fault) : numer;   // == jacobi<PRECOND>(numer, a) of the direct kernels
+    return PRECOND ? dvd_nb(numer, a, range) : numer;   // == jacobi<PRECOND>(numer, a) of the direct kernels
+}
+
+// Merged solver, K31: from the old r, p, v, t of a node: s (step 13), the new r (step 17), the new p (step 9 of the next
+// iteration) and u = M^-1 p'.
+template <bool PRECOND>
+__device__ __forceinline__ double u31_of(double r, double p, double v, double t, double a, double alpha, double omega,
+                                         double beta, double& s, double& rn, double& pn, DivRange& range) {
+    s = s_at(alpha, r, v);
+    rn = sub(s, mul(omega, t));
+    pn = p_new_at<PRECOND>(false, beta, omega, rn, p, v);
+    return PRECOND ? dvd_nb(pn, a, range) : pn;
 }
 
 // Coefficient of field d of node e (0 or 1) of the thread's code word(s): one shift, one three-input logic
@@ -197,10 +237,6 @@ struct Slot {
     unsigned k0, k1;
 };
 
-__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-
 template <int MODE, bool PRECOND, bool STORED, bool CODE32>
 __global__ void __launch_bounds__(NT, 1)
 k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv, const Scalars* sc_in, Scalars* sc_out, ReduceBuf rb,
@@ -209,16 +245,22 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     using T = ModeTraits<MODE>;
     constexpr int NS = T::STAGES;
     constexpr int NF = T::NF;
-    constexpr bool DIAG = MODE == MODE_K1D;          // k1 with the diagonal formed from the codes
-    constexpr bool K1 = MODE == MODE_K1 || DIAG;
+    constexpr bool DIAG = L::DIAG;                   // the diagonal is formed from the codes
+    constexpr bool K1 = MODE == MODE_K1 || MODE == MODE_K1D;
+    constexpr bool K2 = MODE == MODE_K2 || MODE == MODE_K2M;        // K2M: the k2 of the merged solver, + r~.t
+    constexpr bool K2M = MODE == MODE_K2M;
+    constexpr bool K31 = MODE == MODE_K31 || MODE == MODE_K31D;     // the fused k3 + k1 of the merged solver
+    constexpr bool RES = MODE == MODE_R0 || MODE == MODE_R1;
     static_assert(!DIAG || (!STORED && !CODE32), "the diagonal is formed from 2-bit codes");
+    static_assert(!(K2M || K31) || !STORED, "the merged kernels exist for operators in code form");
     pdl_launch_dependents();
     extern __shared__ __align__(128) unsigned char smem[];
     double* ctab_s = reinterpret_cast<double*>(smem + L::CTAB_OFF);
     dd* scratch = reinterpret_cast<dd*>(smem + L::SCRATCH_OFF);
-    unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + L::BAR_OFF);
-    unsigned long long* empty = full + NS;
-    unsigned long long* ready = empty + NS;    // ready[b]: all 18 consumer warps have written their part of u buffer b
+    // full[s]: the TMA copies of stage s have landed; empty[s]: all 18 consumer warps are done with stage s;
+    // ready[b]: all 18 consumer warps have written their part of u buffer b
+    const unsigned sbase = opaque_u32(smem_u32(smem));
+    const unsigned full_a = sbase + (unsigned)L::BAR_OFF, empty_a = full_a + 8u * NS, ready_a = empty_a + 8u * NS;
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     // Persistent blocks: work item i = (tile i % ntiles, z chunk i / ntiles), x tiles fastest, so that the
@@ -226,16 +268,15 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     // L2.  Block b takes items b, b + gridDim.x, ...; the stage and u-buffer rings run on across items, so
     // the producer already loads the next item while the consumers finish the current one, and a launch leaves
     // at most one set of partial sums per SM for the next kernel to combine.
-    // (The stored variant, short of registers, runs one item per block: its ring counters are constants.)
+    // (The stored variant, short of registers, runs one item per block.)
     constexpr bool PERSIST = !STORED;
-    int sb_run = 0, ub_run = 0;            // stages loaded / u planes published in earlier items
     Scalars* S = reinterpret_cast<Scalars*>(smem + L::SC_OFF);
 
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW_CONSUMER); }
+        for (int s = 0; s < NS; ++s) { mbar_init(full_a + 8u * s, 1); mbar_init(empty_a + 8u * s, NW_CONSUMER); }
 #pragma unroll
-        for (int b = 0; b < NU; ++b) mbar_init(&ready[b], NW_CONSUMER);
+        for (int b = 0; b < NU; ++b) mbar_init(ready_a + 8u * b, NW_CONSUMER);
         fence_proxy_async();
     }
     if (!STORED && tid < PF_CTAB) ctab_s[tid] = op.ctab[tid];
@@ -257,18 +298,17 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
         __syncthreads();
     }
     pdl_wait();                                            // everything above is independent of the previous kernel
-    constexpr int KIND = K1 ? PEND_K1 : (MODE == MODE_K2 ? PEND_K2 : (MODE == MODE_R0 ? PEND_INIT : PEND_TRUE));
-    // plane k of the load sequence of work item `item` into stage (seq % NS); the producer lane only
-    auto issue_plane = [&](int item, int k, int seq) {
+    constexpr int KIND = K1 ? PEND_K1 : (K2M ? PEND_K2M : (K2 ? PEND_K2 : (K31 ? PEND_K31 : (MODE == MODE_R0 ? PEND_INIT : PEND_TRUE))));
+    // plane k of the load sequence of work item `item` into stage sidx; the producer lane only
+    auto issue_plane = [&](int item, int k, unsigned sidx) {
         const int tile = item % ntiles;
         const int px = (tile % ntx) * TX, py = (tile / ntx) * TY, pz = (item / ntiles) * zchunk - 1 + k;
-        const int s = seq % NS;
-        unsigned char* st = smem + s * L::STAGE_BYTES;
-        mbar_expect_tx(&full[s], L::TX_BYTES);
+        const unsigned st = sbase + sidx * (unsigned)L::STAGE_BYTES, bar = full_a + 8u * sidx;
+        mbar_expect_tx(bar, L::TX_BYTES);
 #pragma unroll
-        for (int f = 0; f < NF; ++f) tma_load_3d(st + f * FIELD_BYTES, &tm.f[f], &full[s], px - 2, py - 1, pz);
-        if (T::OWN) tma_load_3d(st + L::OWN_OFF, &tm.own, &full[s], px, py, pz);
-        if (!STORED) tma_load_3d(st + L::CODE_OFF, &tm.code, &full[s], DIAG ? px - CXO : px, DIAG ? py - 1 : py, pz);
+        for (int f = 0; f < NF; ++f) tma_load_3d(st + f * FIELD_BYTES, &tm.f[f], bar, px - 2, py - 1, pz);
+        if (T::OWN) tma_load_3d(st + L::OWN_OFF, &tm.own, bar, px, py, pz);
+        if (!STORED) tma_load_3d(st + L::CODE_OFF, &tm.code, bar, DIAG ? px - CXO : px, DIAG ? py - 1 : py, pz);
     };
     // The first stages do not depend on the scalars: they are requested before the block combines the previous
     // kernel's partial sums, so the loads fly while the scalar step is taken.
@@ -276,20 +316,44 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     if (tid == NT_CONSUMER && (int)blockIdx.x < nitems) {
         const int z0f = ((int)blockIdx.x / ntiles) * zchunk;
         const int nqf = min(z0f + zchunk, g.nz) - z0f + 2;
-        for (; pre_issued < NS && pre_issued < nqf; ++pre_issued) issue_plane(blockIdx.x, pre_issued, pre_issued);
+        for (; pre_issued < NS && pre_issued < nqf; ++pre_issued) issue_plane(blockIdx.x, pre_issued, (unsigned)pre_issued);
     }
     if (!begin_kernel(KIND, S, sc_in, sc_out, rb, kv.hist, scratch)) {
         // the solve is over: let the requested stages land before the block's shared memory is released
-        for (int k = 0; k < pre_issued; ++k) while (!mbar_try_wait(&full[k], 0u)) {}
+        for (int k = 0; k < pre_issued; ++k) mbar_wait(full_a + 8u * k, 0u);
         return;
     }
 
-    dd q[2] = {dd_zero(), dd_zero()};
-    double rmax = 0.0;                     // residual modes: ||b - A x||_inf
-    unsigned fault = 0u;
+    dd q[3] = {dd_zero(), dd_zero(), dd_zero()};
+    double rmax = 0.0;                     // residual modes: ||b - A x||_inf; K31: ||r'||_inf
+    DivRange range;                        // quotients of the branch-free division (reading D4)
+    range.reset();
+    bool diag_bad = false;                 // MODE_R0 of a preconditioned solve: the diagonal itself, once per solve
+
+    // Ring positions (run-time state: the rings run on across the items of a persistent block).
+    //   cr: stage of the next plane this thread consumes / (producer lane) fills
+    //   ur: u buffer of the next plane to be published; its predecessor in the ring is the plane published before
+    Ring<NS> cr;
+    Ring<NU> ur;
+    cr.reset(); ur.reset();
+    bool have_prev = false;                // a plane has been published before (by an earlier item)
+    if (wid == NW_CONSUMER) { for (int k = 0; k < pre_issued; ++k) cr.next(); }
+    int issued = pre_issued;               // producer: planes requested so far
+
+    bool first = false; double c1 = 0.0, c2 = 0.0, c3 = 0.0;     // (K31 reads its scalars from S where it uses them)
+    if (K1) { first = S->first != 0; c1 = S->beta; c2 = S->omega; }
+    else if (K2) { c1 = S->alpha; }
+    (void)c3;
+    const bool is_main = wid < TY;
+    // main thread: nodes (x, y) and (x+1, y) of box row wid+1; nx is even so both are inside or both outside.
+    // halo warp TY: box row 0 (pairs) and box column 1 (lanes 0..15); halo warp TY+1: row BY-1 and column BX-2.
+    const int brow = is_main ? wid + 1 : (wid == TY ? 0 : BY - 1);
+    const long long plane = (long long)g.nx * g.ny;
+    const int pair_box = brow * BX + 2 + 2 * lane;                 // element offset in a halo box
+    const int own_tile = (brow - 1) * TX + 2 * lane;               // element offset in an own-only box (main)
+    const int pair_code = brow * BXC + CXO + 2 * lane;             // MODE_K1D: element offset in the code box with halo
 
     for (int item = blockIdx.x; item < nitems; item += PERSIST ? (int)gridDim.x : nitems) {
-    const int sb = PERSIST ? sb_run : 0, ub = PERSIST ? ub_run : 0;
     const int tile = item % ntiles;
     const int x0 = (tile % ntx) * TX, y0 = (tile / ntx) * TY;
     const int z0 = (item / ntiles) * zchunk, z1 = min(z0 + zchunk, g.nz);
@@ -299,84 +363,69 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
         // ---- producer warp: one lane keeps the ring of stages filled ----------------------------
         if (lane == 0) {
             for (int k = (item == (int)blockIdx.x ? pre_issued : 0); k < nq; ++k) {
-                const int s = (sb + k) % NS;
-                if (sb + k >= NS) {
-                    const unsigned par = (unsigned)((sb + k) / NS - 1) & 1u;
-                    while (!mbar_try_wait(&empty[s], par)) {}
-                }
-                issue_plane(item, k, sb + k);
+                if (issued >= NS) mbar_wait(empty_a + 8u * cr.idx, cr.par ^ 1u);   // the consumers' release of the lap before
+                issue_plane(item, k, cr.idx);
+                cr.next();
+                ++issued;
             }
         }
         __syncwarp();
     } else {
-        bool first = false; double c1 = 0.0, c2 = 0.0;
-        if (K1) { first = S->first != 0; c1 = S->beta; c2 = S->omega; }
-        else if (MODE == MODE_K2) { c1 = S->alpha; }
-        const bool is_main = wid < TY;
-        // main thread: nodes (x, y) and (x+1, y) of box row wid+1; nx is even so both are inside or both outside.
-        // halo warp TY: box row 0 (pairs) and box column 1 (lanes 0..15); halo warp TY+1: row BY-1 and column BX-2.
-        const int brow = is_main ? wid + 1 : (wid == TY ? 0 : BY - 1);
         const int x = x0 + 2 * lane, y = y0 - 1 + brow;
         const bool pair_ok = x < g.nx && y >= 0 && y < g.ny;
-        const long long plane = (long long)g.nx * g.ny;
         const long long own_off = x + (long long)g.nx * y;
-        const int pair_box = brow * BX + 2 + 2 * lane;                 // element offset in a halo box
-        const int own_tile = (brow - 1) * TX + 2 * lane;               // element offset in an own-only box (main)
-        const int pair_code = brow * BXC + CXO + 2 * lane;               // MODE_K1D: element offset in the code box with halo
 
-        // operands of the thread's pair of nodes in plane z0-1+k -> u, numerator, diagonal
-        auto form_pair = [&](const unsigned char* st, bool ok, double (&u)[2], double (&n)[2], double (&a)[2]) {
+        // operands of the thread's pair of nodes in a plane -> u, numerator, diagonal (K31: also s, the new r and the old p)
+        auto form_pair = [&](const unsigned char* st, bool ok, double (&u)[2], double (&n)[2], double (&a)[2],
+                             double (&sx)[2], double (&rx)[2], double (&px)[2]) {
             const double* F0 = reinterpret_cast<const double*>(st);
             const double* F1 = reinterpret_cast<const double*>(st + FIELD_BYTES);
             const double* F2 = reinterpret_cast<const double*>(st + 2 * FIELD_BYTES);
             const double* F3 = reinterpret_cast<const double*>(st + 3 * FIELD_BYTES);
+            const double* F4 = reinterpret_cast<const double*>(st + 4 * FIELD_BYTES);
             double2 fr = *reinterpret_cast<const double2*>(F0 + pair_box), fp = make_double2(0, 0),
-                    fv = make_double2(0, 0), fa;
-            if (DIAG) {
+                    fv = make_double2(0, 0), ft = make_double2(0, 0), fa;
+            if (K1 || K31) {
                 fp = *reinterpret_cast<const double2*>(F1 + pair_box);
                 fv = *reinterpret_cast<const double2*>(F2 + pair_box);
-                const unsigned cw = *reinterpret_cast<const unsigned*>(st + L::CODE_OFF + 2 * pair_code);
-                fa = make_double2(dtab_at(dtab_addr, cw, 0), dtab_at(dtab_addr, cw, 1));
-            } else if (MODE == MODE_K1) {
-                fp = *reinterpret_cast<const double2*>(F1 + pair_box);
-                fv = *reinterpret_cast<const double2*>(F2 + pair_box);
-                fa = *reinterpret_cast<const double2*>(F3 + pair_box);
-            } else if (MODE == MODE_K2) {
+                if (K31) ft = *reinterpret_cast<const double2*>(F3 + pair_box);
+                if (DIAG) {
+                    const unsigned cw = *reinterpret_cast<const unsigned*>(st + L::CODE_OFF + 2 * pair_code);
+                    fa = make_double2(dtab_at(dtab_addr, cw, 0), dtab_at(dtab_addr, cw, 1));
+                } else {
+                    fa = *reinterpret_cast<const double2*>((K31 ? F4 : F3) + pair_box);
+                }
+            } else if (K2) {
                 fv = *reinterpret_cast<const double2*>(F1 + pair_box);
                 fa = *reinterpret_cast<const double2*>(F2 + pair_box);
             } else {
                 fa = *reinterpret_cast<const double2*>(F1 + pair_box);
             }
+            // the divisor of the branch-free division is tested once per solve, here (D4)
+            if (MODE == MODE_R0 && PRECOND && ok) diag_bad |= DivRange::diag_bad(fa.x) | DivRange::diag_bad(fa.y);
             if (!ok) fa = make_double2(1.0, 1.0);                       // zero-filled nodes: keep u finite (0/1)
-            u[0] = u_of<MODE, PRECOND>(fr.x, fp.x, fv.x, fa.x, first, c1, c2, n[0], fault);
-            u[1] = u_of<MODE, PRECOND>(fr.y, fp.y, fv.y, fa.y, first, c1, c2, n[1], fault);
+            if (K31) {
+                // alpha, omega, beta from the block's copy of the scalars at every use: three shared loads per plane
+                // instead of six registers held through the loop (this kernel is the one short of registers)
+                const double al = S->alpha, om = S->omega, be = S->beta;
+                u[0] = u31_of<PRECOND>(fr.x, fp.x, fv.x, ft.x, fa.x, al, om, be, sx[0], rx[0], n[0], range);
+                u[1] = u31_of<PRECOND>(fr.y, fp.y, fv.y, ft.y, fa.y, al, om, be, sx[1], rx[1], n[1], range);
+                px[0] = fp.x; px[1] = fp.y;
+            } else {
+                u[0] = u_of<MODE, PRECOND && !RES>(fr.x, fp.x, fv.x, fa.x, first, c1, c2, n[0], range);
+                u[1] = u_of<MODE, PRECOND && !RES>(fr.y, fp.y, fv.y, fa.y, first, c1, c2, n[1], range);
+            }
             a[0] = fa.x; a[1] = fa.y;
         };
-        auto wait_full = [&](int k) -> const unsigned char* {
-            const int s = (sb + k) % NS;
-            const unsigned par = (unsigned)((sb + k) / NS) & 1u;
-            while (!mbar_try_wait(&full[s], par)) {}
-            return smem + s * L::STAGE_BYTES;
+        // the stage of the next plane: wait until its copies have landed; data pointer
+        auto wait_full = [&]() -> const unsigned char* {
+            mbar_wait(full_a + 8u * cr.idx, cr.par);
+            return smem + cr.idx * (unsigned)L::STAGE_BYTES;
         };
-        auto release = [&](int k) {                                     // this warp is done with the stage of plane k
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[(sb + k) % NS]);
-        };
-        // u of plane k (k >= 1) lives in shared buffer (k-1) % NU.  publish: this warp's part is written (and its
-        // stage released); wait_ready: every consumer warp has published plane k.  No block-wide barrier: a warp
-        // that waits for plane k before it overwrites plane k-2's buffer with plane k+1 cannot race a reader
-        // (every warp that published plane k has finished differencing plane k-2).
-        auto u_buf = [&](int k) -> double* {
-            return reinterpret_cast<double*>(smem + L::U_OFF + ((ub + k - 1) % NU) * FIELD_BYTES);
-        };
-        auto publish = [&](int k) {
-            __syncwarp();
-            if (lane == 0) { mbar_arrive(&ready[(ub + k - 1) % NU]); mbar_arrive(&empty[(sb + k) % NS]); }
-        };
-        auto wait_ready = [&](int k) {
-            const unsigned par = (unsigned)((ub + k - 1) / NU) & 1u;
-            while (!mbar_try_wait(&ready[(ub + k - 1) % NU], par)) {}
-        };
+        // u of plane k (k >= 1) lives in the u buffer at ring position ur when it is published.  No block-wide
+        // barrier: a warp that waits for plane k before it overwrites plane k-2's buffer with plane k+1 cannot race
+        // a reader (every warp that published plane k has finished differencing plane k-2).
+        auto u_ptr = [&](unsigned idx) -> double* { return reinterpret_cast<double*>(smem + L::U_OFF + idx * (unsigned)FIELD_BYTES); };
 
         if (!is_main) {
             // ---- halo warps: u on the halo ring of every plane that gets differenced ---------------
@@ -388,36 +437,51 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 const int gx = x0 - 2 + hx, gy = y0 - 1 + hy;
                 col_ok = gx >= 0 && gx < g.nx && gy < g.ny;
             }
-            wait_full(0); release(0);                                   // plane z0-1 has no xy neighbours to serve
+            wait_full();                                                // plane z0-1 has no xy neighbours to serve
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_a + 8u * cr.idx);
+            cr.next();
             for (int k = 1; k < nq; ++k) {
-                if (ub + k >= 2) wait_ready(k - 1);                      // the plane written 3 publishes ago is no longer read
-                const unsigned char* st = wait_full(k);
+                if (have_prev) {                                         // the plane published before this one: the buffer
+                    const unsigned pi = ur.idx == 0u ? (unsigned)(NU - 1) : ur.idx - 1u;     // written 3 publishes ago is free
+                    mbar_wait(ready_a + 8u * pi, ur.par ^ (ur.idx == 0u ? 1u : 0u));
+                }
+                const unsigned char* st = wait_full();
                 const int z = z0 - 1 + k;
                 const bool zin = z >= 0 && z < g.nz;
-                double* u_s = u_buf(k);
-                double u[2], n[2], a[2];
-                form_pair(st, pair_ok && zin, u, n, a);
+                double* u_s = u_ptr(ur.idx);
+                double u[2], n[2], a[2], sx[2], rx[2], px[2];
+                form_pair(st, pair_ok && zin, u, n, a, sx, rx, px);
                 *reinterpret_cast<double2*>(u_s + pair_box) = make_double2(u[0], u[1]);
                 if (col_any) {
                     const double* F0 = reinterpret_cast<const double*>(st);
                     const double* F1 = reinterpret_cast<const double*>(st + FIELD_BYTES);
                     const double* F2 = reinterpret_cast<const double*>(st + 2 * FIELD_BYTES);
                     const double* F3 = reinterpret_cast<const double*>(st + 3 * FIELD_BYTES);
-                    double hr = F0[col_box], hp = 0.0, hv = 0.0, ha;
-                    if (DIAG) {
+                    const double* F4 = reinterpret_cast<const double*>(st + 4 * FIELD_BYTES);
+                    double hr = F0[col_box], hp = 0.0, hv = 0.0, ht = 0.0, ha;
+                    if (K1 || K31) {
                         hp = F1[col_box]; hv = F2[col_box];
-                        const int hxc = (wid == TY ? 1 : BX - 2) + CXO - 2; // the code box starts CXO - 2 columns further left
-                        const unsigned cw = *reinterpret_cast<const unsigned short*>(st + L::CODE_OFF + 2 * ((1 + lane) * BXC + hxc));
-                        ha = dtab_at(dtab_addr, cw, 0);
+                        if (K31) ht = F3[col_box];
+                        if (DIAG) {
+                            const int hxc = (wid == TY ? 1 : BX - 2) + CXO - 2; // the code box starts CXO - 2 columns further left
+                            const unsigned cw = *reinterpret_cast<const unsigned short*>(st + L::CODE_OFF + 2 * ((1 + lane) * BXC + hxc));
+                            ha = dtab_at(dtab_addr, cw, 0);
+                        } else {
+                            ha = (K31 ? F4 : F3)[col_box];
+                        }
                     }
-                    else if (MODE == MODE_K1) { hp = F1[col_box]; hv = F2[col_box]; ha = F3[col_box]; }
-                    else if (MODE == MODE_K2) { hv = F1[col_box]; ha = F2[col_box]; }
+                    else if (K2) { hv = F1[col_box]; ha = F2[col_box]; }
                     else ha = 1.0;
                     if (!(col_ok && zin)) ha = 1.0;
-                    double dummy;
-                    u_s[col_box] = u_of<MODE, PRECOND>(hr, hp, hv, ha, first, c1, c2, dummy, fault);
+                    double d0, d1, d2;
+                    if (K31) u_s[col_box] = u31_of<PRECOND>(hr, hp, hv, ht, ha, S->alpha, S->omega, S->beta, d0, d1, d2, range);
+                    else u_s[col_box] = u_of<MODE, PRECOND && !RES>(hr, hp, hv, ha, first, c1, c2, d0, range);
                 }
-                publish(k);
+                __syncwarp();                                           // publish: this warp's part of plane k is written
+                if (lane == 0) { mbar_arrive(ready_a + 8u * ur.idx); mbar_arrive(empty_a + 8u * cr.idx); }
+                ur.next(); cr.next();
+                have_prev = true;
             }
         } else {
             // ---- main warps -------------------------------------------------------------------------
@@ -426,11 +490,23 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             // one basic block: the divisions of plane z+1 and the stencil chain of plane z are independent and
             // get interleaved by the scheduler.  Nodes outside the grid see zero operands and zero codes, give
             // exact zeros and add nothing to the inner products; only their stores are predicated.
-            auto load_slot = [&](int k, Slot& up, bool to_shared, double* u_dst = nullptr) {
-                const unsigned char* st = wait_full(k);
-                const int z = z0 - 1 + k;
-                const bool ok = pair_ok && z >= 0 && z < g.nz;
-                form_pair(st, ok, up.u, up.n, up.a);
+            // Running global positions: op_row = index of the thread's pair in the plane that load_slot forms next
+            // (z0 - 1 + k), out_row = in the plane that step differences next.
+            long long form_i = own_off + plane * (z0 - 1);
+            long long out_i = own_off + plane * z0;
+            int zf = z0 - 1;                                            // plane load_slot forms next
+            // K31: y of the plane that load_slot forms next, requested one plane ahead (a global load in front of the
+            // dependent additions of step 16 would stall the whole basic block)
+            double2 ypre = make_double2(0, 0);
+            auto y_prefetch = [&]() {
+                if (K31 && pair_ok && zf >= z0 && zf < z1) ypre = *reinterpret_cast<const double2*>(kv.y + form_i);
+            };
+            auto load_slot = [&](Slot& up, bool to_shared, double* u_dst) {
+                const unsigned char* st = wait_full();
+                const bool zown = zf >= z0 && zf < z1;
+                const bool ok = pair_ok && zf >= 0 && zf < g.nz;
+                double sx[2], rx[2], px[2];
+                form_pair(st, ok, up.u, up.n, up.a, sx, rx, px);
                 if (T::OWN)
                     up.w = *reinterpret_cast<const double2*>(reinterpret_cast<const double*>(st + L::OWN_OFF) + own_tile);
                 if (!STORED) {
@@ -443,42 +519,60 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                         up.k0 = *reinterpret_cast<const unsigned*>(st + L::CODE_OFF + 2 * own_tile);
                     }
                 }
-                if (K1 && ok && z >= z0 && z < z1)                      // p' is an output of steps 5-9
-                    *reinterpret_cast<double2*>(kv.p_out + own_off + plane * z) = make_double2(up.n[0], up.n[1]);
-                if (to_shared)
-                    *reinterpret_cast<double2*>((u_dst ? u_dst : u_buf(k)) + pair_box) = make_double2(up.u[0], up.u[1]);
+                if (K1 && ok && zown)                                   // p' is an output of steps 5-9
+                    *reinterpret_cast<double2*>(kv.p_out + form_i) = make_double2(up.n[0], up.n[1]);
+                if (K31 && zown) {                                      // (uniform over the block)
+                    // steps 16-17 of the closing iteration and step 9 of the next: y, r', p' at the thread's own nodes;
+                    // r'.r', r~.r', max |r'| (nodes outside the grid hold zeros and add nothing)
+                    if (ok) {
+                        const double al = S->alpha, om = S->omega;
+                        const double y0n = add(add(ypre.x, mul(al, px[0])), mul(om, sx[0]));
+                        const double y1n = add(add(ypre.y, mul(al, px[1])), mul(om, sx[1]));
+                        *reinterpret_cast<double2*>(kv.y + form_i) = make_double2(y0n, y1n);
+                        *reinterpret_cast<double2*>(kv.r_out + form_i) = make_double2(rx[0], rx[1]);
+                        *reinterpret_cast<double2*>(kv.p_out + form_i) = make_double2(up.n[0], up.n[1]);
+                    }
+                    dd_fma(q[1], rx[0], rx[0]); dd_fma(q[1], rx[1], rx[1]);
+                    dd_fma(q[2], up.w.x, rx[0]); dd_fma(q[2], up.w.y, rx[1]);
+                    rmax = max_abs(max_abs(rmax, rx[0]), rx[1]);
+                }
+                if (to_shared) *reinterpret_cast<double2*>(u_dst + pair_box) = make_double2(up.u[0], up.u[1]);
+                form_i += plane; ++zf;
+                y_prefetch();
             };
-            constexpr bool DEFER = !STORED;                  // the stored variant has no registers to spare for it
+            constexpr bool DEFER = !STORED && !K31;          // the stored variant and K31 have no registers to spare for it
             double pa[2] = {0.0, 0.0}, pb[2] = {0.0, 0.0};   // operands of the deferred inner products (zeros add nothing)
+            double pc[2] = {0.0, 0.0};                       // K2M: r~ of the plane whose t is in pa
             // The loop below is unrolled three ways and NU = 3, so the u buffer of plane z0 + 3m + J is a fixed
             // rotation J of the item's first one and the parity of its `ready` barrier a fixed bit xor (m & 1):
-            // three pointers and three bits per item instead of a division by 3 per plane and use.
+            // three addresses and three bits per item instead of ring arithmetic per plane and use.
             static_assert(NU == 3, "the rotation below is written for three u buffers");
-            const int ub3 = ub % NU;
-            int bj[3];                                                  // buffer of rotation j
+            unsigned bj[3];                                             // buffer of rotation j
             unsigned pbits = 0u;                                        // bit j: parity of rotation j at m = 0
+            {
+                Ring<NU> t = ur;
 #pragma unroll
-            for (int j = 0; j < 3; ++j) {
-                bj[j] = ub3 + j >= NU ? ub3 + j - NU : ub3 + j;
-                pbits |= ((unsigned)(ub / NU + (ub3 + j >= NU ? 1 : 0)) & 1u) << j;
+                for (int j = 0; j < 3; ++j) { bj[j] = t.idx; pbits |= t.par << j; t.next(); }
             }
             unsigned mp = 0u;                                           // (z - z0) / 3 & 1
-            auto U = [&](int j) { return reinterpret_cast<double*>(smem + L::U_OFF + bj[j] * FIELD_BYTES); };
-            auto R = [&](int j) { return &ready[bj[j]]; };
-            auto step = [&](auto Jc, int z, const Slot& dn, const Slot& c, Slot& up) {
+            auto U = [&](int j) { return u_ptr(bj[j]); };
+            auto R = [&](int j) { return ready_a + 8u * bj[j]; };
+            auto step = [&](auto Jc, const Slot& dn, const Slot& c, Slot& up) {
                 constexpr int J = decltype(Jc)::value, J1 = (J + 1) % 3;
-                const int k = z - z0 + 1;                               // load-sequence index of plane z
-                const long long i = own_off + plane * z;
-                const double* u_s = U(J);                               // == u_buf(k)
-                { const unsigned par = ((pbits >> J) & 1u) ^ mp; while (!mbar_try_wait(R(J), par)) {} }   // == wait_ready(k)
-                load_slot(k + 1, up, true, U(J1));
+                const long long i = out_i;
+                const double* u_s = U(J);
+                mbar_wait(R(J), ((pbits >> J) & 1u) ^ mp);               // every warp has published the plane to difference
+                load_slot(up, true, U(J1));
                 // inner products of the PREVIOUS plane: a third independent chain beside the divisions of plane
                 // z+1 and the 7-point sums of plane z
                 if (DEFER && K1) {
                     dd_fma(q[0], pa[0], pb[0]); dd_fma(q[1], pa[1], pb[1]);
-                } else if (DEFER && MODE == MODE_K2) {
+                } else if (DEFER && K31) {
+                    dd_fma(q[0], pa[0], pb[0]); dd_fma(q[0], pa[1], pb[1]);
+                } else if (DEFER && K2) {
                     dd_fma(q[0], pa[0], pb[0]); dd_fma(q[0], pa[1], pb[1]);
                     dd_fma(q[1], pa[0], pa[0]); dd_fma(q[1], pa[1], pa[1]);
+                    if (K2M) { dd_fma(q[2], pc[0], pa[0]); dd_fma(q[2], pc[1], pa[1]); }
                 }
                 const double2 us = *reinterpret_cast<const double2*>(u_s + pair_box - BX);
                 const double2 un = *reinterpret_cast<const double2*>(u_s + pair_box + BX);
@@ -505,7 +599,9 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                         ctab3_at(t3_addr, c.k0, e, 0, c3); cc[0] = c3[0]; cc[1] = c3[1]; cc[2] = c3[2];
                         ctab3_at(t3_addr, c.k0, e, 1, c3); cc[3] = c3[0]; cc[4] = c3[1]; cc[5] = c3[2];
                     }
-                    double acc = mul(c.a[e], c.u[e]);
+                    // (DIAG: looked up again from the code rather than kept in three register slots)
+                    const double a_own = (DIAG && K31) ? dtab_at(dtab_addr, c.k0, e) : c.a[e];
+                    double acc = mul(a_own, c.u[e]);
                     acc = add(acc, mul(cc[0], e == 0 ? c.u[1] : ue));
                     acc = add(acc, mul(cc[1], e == 1 ? c.u[0] : uw));
                     acc = add(acc, mul(cc[2], e == 0 ? us.x : us.y));
@@ -514,17 +610,22 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     out[e] = acc;
                     c5[e] = cc[5];
                 }
-                __syncwarp();                                           // == publish(k + 1): u(z+1) is in shared memory
-                if (lane == 0) { mbar_arrive(R(J1)); mbar_arrive(&empty[(sb + k + 1) % NS]); }
+                __syncwarp();                                           // publish: u(z+1) is in shared memory
+                if (lane == 0) { mbar_arrive(R(J1)); mbar_arrive(empty_a + 8u * cr.idx); }
+                cr.next();
                 out[0] = add(out[0], mul(c5[0], up.u[0]));
                 out[1] = add(out[1], mul(c5[1], up.u[1]));
-                if (K1) {
+                if (K1 || K31) {
                     if (pair_ok) *reinterpret_cast<double2*>(kv.v_out + i) = make_double2(out[0], out[1]);
                     if (DEFER) { pa[0] = c.w.x; pa[1] = c.w.y; pb[0] = out[0]; pb[1] = out[1]; }   // r~ . v', next step
+                    else if (K31) { dd_fma(q[0], c.w.x, out[0]); dd_fma(q[0], c.w.y, out[1]); }
                     else { dd_fma(q[0], c.w.x, out[0]); dd_fma(q[1], c.w.y, out[1]); }
-                } else if (MODE == MODE_K2) {
+                } else if (K2) {
                     if (pair_ok) *reinterpret_cast<double2*>(kv.t + i) = make_double2(out[0], out[1]);
-                    if (DEFER) { pa[0] = out[0]; pa[1] = out[1]; pb[0] = c.n[0]; pb[1] = c.n[1]; }   // t . s, t . t, next step
+                    if (DEFER) {                                        // t . s, t . t (K2M: r~ . t), next step
+                        pa[0] = out[0]; pa[1] = out[1]; pb[0] = c.n[0]; pb[1] = c.n[1];
+                        if (K2M) { pc[0] = c.w.x; pc[1] = c.w.y; }
+                    }
                     else {
                         dd_fma(q[0], out[0], c.n[0]); dd_fma(q[0], out[1], c.n[1]);
                         dd_fma(q[1], out[0], out[0]); dd_fma(q[1], out[1], out[1]);
@@ -541,44 +642,69 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     dd_fma(q[1], r0, r0); dd_fma(q[1], r1, r1);
                     rmax = max_abs(max_abs(rmax, r0), r1);
                 }
+                out_i += plane;
             };
 
             Slot s0, s1, s2;
             s0.w = s1.w = s2.w = make_double2(0, 0);
             s0.k0 = s0.k1 = s1.k0 = s1.k1 = s2.k0 = s2.k1 = 0u;
-            load_slot(0, s0, false); release(0);   // plane z0-1: registers only
-            if (ub >= 1) wait_ready(0);            // last plane of the previous item: its buffer-mates are free
-            load_slot(1, s1, true);  publish(1);   // plane z0
+            load_slot(s0, false, nullptr);         // plane z0-1: registers only
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_a + 8u * cr.idx);
+            cr.next();
+            if (have_prev) {                       // last plane of the previous item: its buffer-mates are free
+                const unsigned pi = ur.idx == 0u ? (unsigned)(NU - 1) : ur.idx - 1u;
+                mbar_wait(ready_a + 8u * pi, ur.par ^ (ur.idx == 0u ? 1u : 0u));
+            }
+            load_slot(s1, true, U(0));             // plane z0
+            __syncwarp();
+            if (lane == 0) { mbar_arrive(R(0)); mbar_arrive(empty_a + 8u * cr.idx); }
+            cr.next();
             for (int z = z0; z < z1; z += 3) {     // slots rotate by renaming, not by moving registers
-                step(std::integral_constant<int, 0>{}, z, s0, s1, s2);
+                step(std::integral_constant<int, 0>{}, s0, s1, s2);
                 if (z + 1 >= z1) break;
-                step(std::integral_constant<int, 1>{}, z + 1, s1, s2, s0);
+                step(std::integral_constant<int, 1>{}, s1, s2, s0);
                 if (z + 2 >= z1) break;
-                step(std::integral_constant<int, 2>{}, z + 2, s2, s0, s1);
+                step(std::integral_constant<int, 2>{}, s2, s0, s1);
                 mp ^= 1u;
             }
             if (DEFER && K1) {                               // the last plane's inner products
                 dd_fma(q[0], pa[0], pb[0]); dd_fma(q[1], pa[1], pb[1]);
-            } else if (DEFER && MODE == MODE_K2) {
+            } else if (DEFER && K31) {
+                dd_fma(q[0], pa[0], pb[0]); dd_fma(q[0], pa[1], pb[1]);
+            } else if (DEFER && K2) {
                 dd_fma(q[0], pa[0], pb[0]); dd_fma(q[0], pa[1], pb[1]);
                 dd_fma(q[1], pa[0], pa[0]); dd_fma(q[1], pa[1], pa[1]);
+                if (K2M) { dd_fma(q[2], pc[0], pa[0]); dd_fma(q[2], pc[1], pa[1]); }
             }
+            pa[0] = pa[1] = pb[0] = pb[1] = pc[0] = pc[1] = 0.0;     // (the next item starts with nothing deferred)
+            // the item published nq - 1 planes
+            {
+                const int adv = nq - 1;
+                ur.par ^= (unsigned)(adv / NU) & 1u;
+                for (int r = adv % NU; r > 0; --r) ur.next();
+            }
+            have_prev = true;
         }
     }
-
-    sb_run += nq; ub_run += nq - 1;
     }
 
-    if (fault) *rb.fault = 1;              // the host repeats the solve with the __ddiv_rn kernels
+    if (range.bad() || diag_bad) *rb.fault = 1;     // the host repeats the solve with the __ddiv_rn kernels
     // this block's partial sums; the next kernel of the stream combines them (pf_common.cuh)
     if (K1) {
         dd_add(q[0], q[1]);                // two chains for instruction-level parallelism, one quantity
         dd q1[1] = {q[0]};
         store_partials<1, false>(q1, 0.0, scratch, rb, PEND_K1);
-    } else if (MODE == MODE_K2) {
-        store_partials<2, false>(q, 0.0, scratch, rb, PEND_K2);
+    } else if (K2M) {
+        store_partials<3, false>(q, 0.0, scratch, rb, PEND_K2M);
+    } else if (K2) {
+        dd q2[2] = {q[0], q[1]};
+        store_partials<2, false>(q2, 0.0, scratch, rb, PEND_K2);
+    } else if (K31) {
+        store_partials<3, true>(q, rmax, scratch, rb, PEND_K31);
     } else {
-        store_partials<2, true>(q, rmax, scratch, rb, KIND);
+        dd q2[2] = {q[0], q[1]};
+        store_partials<2, true>(q2, rmax, scratch, rb, KIND);
     }
 }
 
@@ -689,8 +815,9 @@ void launch_mode(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, c
 // Tensor maps of one solve: every vector a kernel reads through TMA.
 struct TmaSet {
     CUtensorMap r, p[2], v[2], a0, rt, x, b, code;
-    CUtensorMap codeh;       // 2-byte codes with the halo ring (MODE_K1D)
-    bool have_code, have_codeh;
+    CUtensorMap codeh;       // 2-byte codes with the halo ring (MODE_K1D, MODE_K31D)
+    CUtensorMap r1, th;      // merged solver: the second r buffer, and t with its halo ring
+    bool have_code, have_codeh, have_merged;
 };
 
 bool tma_available() { return encoder() != nullptr; }
@@ -699,6 +826,8 @@ bool tma_available() { return encoder() != nullptr; }
 bool tma_supported(const GridDims& g) {
     return (g.nx % 2 == 0) && g.nx >= 32 && g.ny >= 16 && g.nz >= 8;
 }
+
+bool tma_merged_ok(const TmaSet* t) { return t->have_merged; }
 
 bool tma_pointers_ok(const KrylovVecs& kv, const Operator& op) {
     return aligned16(kv.x) && aligned16(kv.b) && aligned16(op.A0) && aligned16(kv.r) && aligned16(kv.rt) &&
@@ -720,14 +849,21 @@ bool tma_set_build(TmaSet* t, const GridDims& g, const Operator& op, const Krylo
     }
     t->have_codeh = ok && !op.stored && !op.code32 && op.diag_code &&
                     make_map(&t->codeh, op.code, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, g, op.cpitch, BXC, BY);
+    t->have_merged = ok && kv.r_out && !op.stored && aligned16(kv.r_out) && halo_map(&t->r1, kv.r_out, g) &&
+                     halo_map(&t->th, kv.t, g);
     return ok;
 }
 
-void launch_residual_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, int mode) {
+bool tma_merged_supported(const Operator& op) { return !op.stored; }
+
+// precond: mode 0 of a preconditioned solve also tests the diagonal against the range of the branch-free division
+// that k1 and k2 will divide by it with (reading D4; the residual itself involves no division).
+void launch_residual_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, int mode,
+                         bool precond) {
     TmaArgs a;
     std::memset(&a, 0, sizeof(a));
     a.f[0] = t->x; a.f[1] = t->a0; a.own = t->b; a.code = t->code;
-    if (mode == 0) launch_mode<MODE_R0>(c, op, kv, a, false); else launch_mode<MODE_R1>(c, op, kv, a, false);
+    if (mode == 0) launch_mode<MODE_R0>(c, op, kv, a, precond); else launch_mode<MODE_R1>(c, op, kv, a, false);
 }
 
 void launch_k1_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond,
@@ -746,6 +882,53 @@ void launch_k1_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv,
     }
     a.f[0] = t->r; a.f[1] = t->p[parity]; a.f[2] = t->v[parity]; a.f[3] = t->a0; a.own = t->rt; a.code = t->code;
     launch_mode<MODE_K1>(c, op, kv, a, precond);
+}
+
+// grid of work items (x tiles, y tiles, z chunks) and the chunk depth
+static dim3 item_grid(const LaunchCtx& c, int* depth) {
+    const int tx = (c.g.nx + TX - 1) / TX, tyb = (c.g.ny + TY - 1) / TY;
+    const int chunks = choose_zchunks(c.g, tx * tyb, c.sm_count);
+    *depth = (c.g.nz + chunks - 1) / chunks;
+    return dim3(tx, tyb, (c.g.nz + *depth - 1) / *depth);
+}
+
+void launch_k2m_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond, int k) {
+    TmaArgs a;
+    std::memset(&a, 0, sizeof(a));
+    const int rb = k & 1, pb = rb ^ 1;
+    a.f[0] = rb ? t->r1 : t->r; a.f[1] = t->v[pb]; a.f[2] = t->a0; a.own = t->rt; a.code = t->code;
+    int depth;
+    const dim3 grid = item_grid(c, &depth);
+    if (op.code32) {
+        if (precond) launch_inst<MODE_K2M, true, false, true>(c, op, kv, a, grid, depth);
+        else         launch_inst<MODE_K2M, false, false, true>(c, op, kv, a, grid, depth);
+    } else {
+        if (precond) launch_inst<MODE_K2M, true, false, false>(c, op, kv, a, grid, depth);
+        else         launch_inst<MODE_K2M, false, false, false>(c, op, kv, a, grid, depth);
+    }
+}
+
+void launch_k31_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond, int k) {
+    TmaArgs a;
+    std::memset(&a, 0, sizeof(a));
+    const int rb = k & 1, pb = rb ^ 1;
+    a.f[0] = rb ? t->r1 : t->r; a.f[1] = t->p[pb]; a.f[2] = t->v[pb]; a.f[3] = t->th; a.own = t->rt;
+    int depth;
+    const dim3 grid = item_grid(c, &depth);
+    if (t->have_codeh) {     // the diagonal is the sum of the face coefficients: formed from the codes, A0 not read
+        a.code = t->codeh;
+        if (precond) launch_inst<MODE_K31D, true, false, false>(c, op, kv, a, grid, depth);
+        else         launch_inst<MODE_K31D, false, false, false>(c, op, kv, a, grid, depth);
+        return;
+    }
+    a.f[4] = t->a0; a.code = t->code;
+    if (op.code32) {
+        if (precond) launch_inst<MODE_K31, true, false, true>(c, op, kv, a, grid, depth);
+        else         launch_inst<MODE_K31, false, false, true>(c, op, kv, a, grid, depth);
+    } else {
+        if (precond) launch_inst<MODE_K31, true, false, false>(c, op, kv, a, grid, depth);
+        else         launch_inst<MODE_K31, false, false, false>(c, op, kv, a, grid, depth);
+    }
 }
 
 void launch_k2_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond,

@@ -36,6 +36,7 @@ struct LaunchCtx {
     ReduceBuf rb;     // device
     int sm_count;
     int device;       // CUDA device of the grid (per-device kernel attributes)
+    int solver;       // 0: Table 3, three kernels per iteration; 1: merged recurrence, two (pf_krylov.cuh)
     bool pdl;         // programmatic dependent launch allowed
     // the next kernel reads sc[*flip] and its block 0 writes sc[*flip ^ 1]
     void next_scalars(const Scalars*& in, Scalars*& out) const { in = sc[*flip]; out = sc[*flip ^ 1]; *flip ^= 1; }
@@ -52,8 +53,14 @@ void launch_residual_direct(const LaunchCtx& c, const Operator& op, const Krylov
 void launch_k1_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
 void launch_k2_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
 void launch_k3(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
+// The two kernels of an iteration of the merged solver (pf_krylov.cuh): current (p, v) = (kv.p_in, kv.v_in), current
+// r = kv.r; K31 writes kv.r_out, kv.p_out, kv.v_out.
+void launch_k2m_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
+void launch_k31_direct(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, bool precond);
 // One-block kernel that takes the pending scalar step in place, before the host reads the scalars.
 void launch_finalize(const LaunchCtx& c, double* hist);
+// The same, and sets the condition of the WHILE node whose body it closes (merged solver, device-side loop).
+void launch_finalize_loop(const LaunchCtx& c, double* hist);
 // x += M^-1 y at the end of a preconditioned solve (reading D3).
 void launch_finish_x(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv);
 
@@ -68,11 +75,19 @@ TmaSet* tma_set_create();
 void tma_set_destroy(TmaSet* t);
 // (Re)build the tensor maps for the vectors and operator of a solve; false on failure.
 bool tma_set_build(TmaSet* t, const GridDims& g, const Operator& op, const KrylovVecs& kv);
-void launch_residual_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, int mode);
+void launch_residual_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, int mode,
+                         bool precond = false);
 void launch_k1_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond,
                    int parity /* which of the two (p, v) buffer pairs is the input */);
 void launch_k2_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond,
                    int parity);
+// Merged solver, iteration k of a solve (0-based): r lives in buffer k & 1, the current (p, v) pair in buffer (k & 1) ^ 1
+// (buffer 0 = the pointers of the KrylovVecs the set was built from, buffer 1 = its r_out, p_out, v_out).
+void launch_k2m_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond, int k);
+void launch_k31_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond, int k);
+// Whether the tiled family has the merged kernels for this operator (code form; the stored variant uses the direct ones).
+bool tma_merged_supported(const Operator& op);
+bool tma_merged_ok(const TmaSet* t);             // the set just built holds the maps of the merged kernels
 
 // Cooperative family (pf_krylov_coop.cu): one persistent kernel per solve, one brick of the box per block, the
 // brick's vectors in shared memory.  For grids small enough that a brick fits one SM (about <= 72^3) and
