@@ -56,6 +56,10 @@ def parse():
                          "node repeats the iterations on the device; chunks = graph replays of 16 iterations polled "
                          "by the host (ncu does not profile kernel nodes of graphs with conditional nodes: launch "
                          "lists are taken with this mode); stream = plain launches")
+    ap.add_argument("--solver", choices=["table3", "merged"], default="table3",
+                    help="table3: BiCGSTAB as Table 3 writes it, three kernels per iteration (the default, whose parity "
+                         "reference is the oracle's Table 3); merged: the two-reduction recurrence (PF_OPT_SOLVER = 1, "
+                         "reading M1), two kernels per iteration")
     ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -122,13 +126,18 @@ def measured_peak_gbs():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def kernel_bytes_per_unknown(stored: bool) -> dict:
+def kernel_bytes_per_unknown(stored: bool, merged: bool = False) -> dict:
     """Algorithmic HBM bytes per unknown per launch: every input vector
     read once, every output written once, halos served on chip."""
     # k1 reads r, p, v, A0, r~ and writes p', v'; k2 reads r, v', A0 and writes t; k3 reads r, v', p', y, t, r~
     # and writes y, r; the on-the-fly variant adds a 2-byte stencil code per node to k1 and k2, the stored
     # variant six 8-byte off-diagonals.  The per-kernel events bracket iterations of the 200-iteration Poisson
     # solve only; there the on-the-fly k1 does not read A0 (it is a function of the code: PF_OPT_DIAG_FROM_CODE).
+    # Merged solver (on-the-fly stencil; the events bracket its two kernels in the slots of k2 and k3): K2M reads r, v, A0,
+    # r~ and the codes and writes t; K31 reads r, p, v, t, r~, y and the codes (the diagonal comes from them in a Poisson
+    # solve) and writes r', p', v', y.
+    if merged:
+        return {"k2": (4 + 1) * 8 + 2, "k3": (6 + 4) * 8 + 2}
     if stored:
         return {"k1": (5 + 6 + 2) * 8, "k2": (3 + 6 + 1) * 8, "k3": (6 + 2) * 8}
     return {"k1": (4 + 2) * 8 + 2, "k2": (3 + 1) * 8 + 2, "k3": (6 + 2) * 8}
@@ -238,6 +247,7 @@ def run_b200(args):
         if kernels:
             pf.pf_grid_set_option(h, pf.PF_OPT_KERNELS, kernels)
         pf.pf_grid_set_option(h, pf.PF_OPT_GRAPH, {"auto": 3, "loop": 2, "chunks": 1, "stream": 0}[args.launch_mode])
+        pf.pf_grid_set_option(h, pf.PF_OPT_SOLVER, 1 if args.solver == "merged" else 0)
         pf.pf_grid_set_option(h, pf.PF_OPT_LINEAR_TOL, 0.0)
         pf.pf_grid_set_option(h, pf.PF_OPT_LINEAR_MAXIT, PF_INNER_ITERS)
         pf.pf_grid_set_option(h, pf.PF_OPT_MAX_OUTER, 1)
@@ -306,10 +316,11 @@ def run_b200(args):
     if rank == 0:
         peak, peak_src = measured_peak_gbs()
         stored = args.stencil == "stored"
-        bpu = kernel_bytes_per_unknown(stored)
+        merged = args.solver == "merged"
+        bpu = kernel_bytes_per_unknown(stored, merged)
         kernels_rep = {}
         for k in ("k1", "k2", "k3"):
-            if prof_tot[k]["launches"]:
+            if prof_tot[k]["launches"] and k in bpu:
                 avg_ms = prof_tot[k]["ms"] / prof_tot[k]["launches"]
                 gbs = bpu[k] * n / (avg_ms * 1e-3) / 1e9
                 kernels_rep[k] = {"avg_ms": avg_ms, "launches": prof_tot[k]["launches"],
@@ -327,8 +338,12 @@ def run_b200(args):
                         traffic = int(c[3])
         except (OSError, ValueError):
             traffic = None
-        roofline = {"bound": "hbm", "kernel": {"k1": "k1 (p-update + matvec + r~.v)", "k2": "k2 (s-update + matvec + t.s,t.t)",
-                                                "k3": "k3 (x,r update + r~.r, r.r)"}[dom],
+        names = {"k1": "k1 (p-update + matvec + r~.v)", "k2": "k2 (s-update + matvec + t.s,t.t)",
+                 "k3": "k3 (x,r update + r~.r, r.r)"}
+        if merged:
+            names = {"k2": "K2M (s-update + matvec + t.s, t.t, r~.t)",
+                     "k3": "K31 (x, r, p update + matvec + r~.v, r.r, r~.r)"}
+        roofline = {"bound": "hbm", "kernel": names[dom],
                     "achieved": kernels_rep[dom]["gbs"], "peak": peak, "unit": "GB/s",
                     "frac": kernels_rep[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
                     "per_kernel": kernels_rep,
@@ -353,7 +368,8 @@ def run_b200(args):
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": f"{wdesc}; step = assembly + {lin_iters} fixed Jacobi-BiCGSTAB iterations + "
                                        f"one PF outer pass with 3x{PF_INNER_ITERS} inner iterations",
-                           "stencil": args.stencil, "kernels": args.kernels, "launch_mode": args.launch_mode, "unknowns": n,
+                           "stencil": args.stencil, "kernels": args.kernels, "launch_mode": args.launch_mode,
+                           "solver": args.solver, "unknowns": n,
                            "iterations_per_step": step_iters, "parallelism": "replicas only" if world > 1 else "1 GPU",
                            "l2": "inputs larger than L2 (working set %.1f GB)" % (ws.numel() / 1e9)},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,

@@ -245,8 +245,9 @@ def fermi_pointwise(valence, bath_molar, radii, phi, solvent=None, water_molar=5
 
 def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar, radii, l_c, tol,
              omega_pf=0.3, lin_tol=1e-10, lin_maxit=10000, max_outer=200, water_molar=55.5, norm=NORM_REL_L2,
-             fixed_override=None, fixed_nodes=None, solver=SOLVER_TABLE3):
-    """The outer loop of Table 2 / Table 4 (R5)."""
+             fixed_override=None, fixed_nodes=None, solver=SOLVER_TABLE3, want_fields=True):
+    """The outer loop of Table 2 / Table 4 (R5).  want_fields=False skips the final evaluation of C_k and S^trc
+    (out["conc"], out["steric"] are then None): at 512^3 it costs a minute and 4 GB that a truncated run does not need."""
     n = nx * ny * nz
     t, v = _bc(bc_type, bc_value)
     eps = _f64(eps)
@@ -257,8 +258,8 @@ def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar
     K = valence.size
     phi = np.zeros(n)
     psi = np.zeros(n)
-    conc = np.zeros((K + 1, n))
-    steric = np.zeros(n)
+    conc = np.zeros((K + 1, n)) if want_fields else None
+    steric = np.zeros(n) if want_fields else None
     outer = ctypes.c_int(0)
     lin = ctypes.c_int(0)
     cap = 2 * max_outer + 1

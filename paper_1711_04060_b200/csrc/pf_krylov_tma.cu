@@ -496,10 +496,17 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             long long out_i = own_off + plane * z0;
             int zf = z0 - 1;                                            // plane load_slot forms next
             // K31: y of the plane that load_slot forms next, requested one plane ahead (a global load in front of the
-            // dependent additions of step 16 would stall the whole basic block)
+            // dependent additions of step 16 would stall the whole basic block).  The request is issued right AFTER the
+            // warp's mbarrier arrivals, never before them: an arrive is a release, and the hardware holds it back until
+            // the thread's outstanding loads have returned -- with the load in front of it every `ready` barrier, and
+            // with it the whole block, waited a DRAM round trip per plane (0.287 ms per launch instead of ...).
             double2 ypre = make_double2(0, 0);
             auto y_prefetch = [&]() {
-                if (K31 && pair_ok && zf >= z0 && zf < z1) ypre = *reinterpret_cast<const double2*>(kv.y + form_i);
+                if (K31 && pair_ok && zf >= z0 && zf < z1) {
+                    ypre = *reinterpret_cast<const double2*>(kv.y + form_i);
+                    // and two planes further into L2 (no register): the register load above then finds its line there
+                    if (zf + 2 < z1) asm volatile("prefetch.global.L2 [%0];" ::"l"(kv.y + form_i + 2 * plane));
+                }
             };
             auto load_slot = [&](Slot& up, bool to_shared, double* u_dst) {
                 const unsigned char* st = wait_full();
@@ -538,9 +545,8 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 }
                 if (to_shared) *reinterpret_cast<double2*>(u_dst + pair_box) = make_double2(up.u[0], up.u[1]);
                 form_i += plane; ++zf;
-                y_prefetch();
             };
-            constexpr bool DEFER = !STORED && !K31;          // the stored variant and K31 have no registers to spare for it
+            constexpr bool DEFER = !STORED && !K31 && !K2M;  // the stored variant, K31 and K2M have no registers to spare for it
             double pa[2] = {0.0, 0.0}, pb[2] = {0.0, 0.0};   // operands of the deferred inner products (zeros add nothing)
             double pc[2] = {0.0, 0.0};                       // K2M: r~ of the plane whose t is in pa
             // The loop below is unrolled three ways and NU = 3, so the u buffer of plane z0 + 3m + J is a fixed
@@ -563,6 +569,14 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                 const double* u_s = U(J);
                 mbar_wait(R(J), ((pbits >> J) & 1u) ^ mp);               // every warp has published the plane to difference
                 load_slot(up, true, U(J1));
+                // Publish at once: u(z+1) is in shared memory and the stage is consumed.  Arriving here, before this
+                // plane's stencil, rather than after it lets the other warps (and the producer) run on up to a plane
+                // ahead.  Still race-free: whoever overwrites the buffer of plane z (with plane z+3) first waits for
+                // `ready` of plane z+2, on which this warp arrives in its next step, i.e. after the reads below.
+                __syncwarp();
+                if (lane == 0) { mbar_arrive(R(J1)); mbar_arrive(empty_a + 8u * cr.idx); }
+                cr.next();
+                y_prefetch();
                 // inner products of the PREVIOUS plane: a third independent chain beside the divisions of plane
                 // z+1 and the 7-point sums of plane z
                 if (DEFER && K1) {
@@ -610,9 +624,6 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     out[e] = acc;
                     c5[e] = cc[5];
                 }
-                __syncwarp();                                           // publish: u(z+1) is in shared memory
-                if (lane == 0) { mbar_arrive(R(J1)); mbar_arrive(empty_a + 8u * cr.idx); }
-                cr.next();
                 out[0] = add(out[0], mul(c5[0], up.u[0]));
                 out[1] = add(out[1], mul(c5[1], up.u[1]));
                 if (K1 || K31) {
@@ -629,6 +640,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     else {
                         dd_fma(q[0], out[0], c.n[0]); dd_fma(q[0], out[1], c.n[1]);
                         dd_fma(q[1], out[0], out[0]); dd_fma(q[1], out[1], out[1]);
+                        if (K2M) { dd_fma(q[2], c.w.x, out[0]); dd_fma(q[2], c.w.y, out[1]); }
                     }
                 } else {
                     const double r0 = sub(c.w.x, out[0]), r1 = sub(c.w.y, out[1]);
@@ -652,6 +664,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             __syncwarp();
             if (lane == 0) mbar_arrive(empty_a + 8u * cr.idx);
             cr.next();
+            y_prefetch();
             if (have_prev) {                       // last plane of the previous item: its buffer-mates are free
                 const unsigned pi = ur.idx == 0u ? (unsigned)(NU - 1) : ur.idx - 1u;
                 mbar_wait(ready_a + 8u * pi, ur.par ^ (ur.idx == 0u ? 1u : 0u));
@@ -660,6 +673,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             __syncwarp();
             if (lane == 0) { mbar_arrive(R(0)); mbar_arrive(empty_a + 8u * cr.idx); }
             cr.next();
+            y_prefetch();
             for (int z = z0; z < z1; z += 3) {     // slots rotate by renaming, not by moving registers
                 step(std::integral_constant<int, 0>{}, s0, s1, s2);
                 if (z + 1 >= z1) break;
