@@ -180,3 +180,110 @@ def test_split_system_sine_mode_closed_form(oracle):
     r0 = oracle.solve_pf(n, n, n, h, bt, bv, eps, np.zeros((0, 4)), [1.0, -1.0], [0.1, 0.1], [0.0, 0.0, 0.0], 0.0, 1e-14,
                          lin_tol=1e-13, max_outer=400, fixed_override=F * mode)
     assert np.abs(r0["phi"] - no_lc * mode).max() < 1e-6 * no_lc
+
+
+# ---- the combined path: l_c > 0 AND the steric term with unequal radii AND strong nonlinearity, in 3-D ----------------
+# No closed form exists and the paper prints no numbers, and the 1-D reduction that pins the l_c = 0 case is not
+# available here: reading Q15 puts Psi = 0 on every box-boundary and non-solvent node, so a column is never
+# one-dimensional for Psi once l_c > 0.  Two pins that need neither:
+#   (1) a manufactured discrete solution: pick phi*, build rho(phi*) (own root finder for S), Psi* (discrete sine
+#       transform: an exact solve of PF1 that shares nothing with BiCGSTAB) and the source that makes phi* satisfy PF2;
+#       the outer loop must converge to (phi*, Psi*, C_k*).  A dropped term, a wrong sign or a wrong lam_k anywhere in
+#       fermi_node / rhs_pf1 / rhs_pf2 / the relaxation moves the fixed point away from phi*.
+#   (2) grid-refinement consistency (SURVEY 8(c) "optional extra"): the same smooth continuous problem on h, h/2, h/4
+#       converges with second order, the order of every ingredient.
+
+def _independent_fermi(oracle, z, bath_molar, radii, phi, water_molar=55.5):
+    """Eq (1) with its three simultaneous definitions, solved by bisection in numpy (nothing from the oracle but the
+    two unit constants).  Returns C_k (K+1, N) and S."""
+    z = np.asarray(list(z) + [0.0])
+    cb = np.asarray(list(bath_molar) + [water_molar]) * MOLAR
+    vol = 4.0 * np.pi * np.asarray(radii) ** 3 / 3.0
+    lam = vol / vol.mean()
+    gamma_b = 1.0 - (vol * cb).sum()
+    phi = np.asarray(phi, dtype=np.float64)
+
+    def total(S):            # Gamma + sum v_k C_k as functions of S: must equal 1
+        t = gamma_b * np.exp(S)
+        for k in range(len(z)):
+            t = t + vol[k] * cb[k] * np.exp(-z[k] * phi + lam[k] * S)
+        return t
+    lo, hi = np.full_like(phi, -200.0), np.full_like(phi, 50.0)
+    for _ in range(200):
+        mid = 0.5 * (lo + hi)
+        big = total(mid) > 1.0
+        hi = np.where(big, mid, hi)
+        lo = np.where(big, lo, mid)
+    S = 0.5 * (lo + hi)
+    C = np.stack([cb[k] * np.exp(-z[k] * phi + lam[k] * S) for k in range(len(z))])
+    return C, S
+
+
+def _lap7_zero_bc(u3, h):
+    """7-point Laplacian of a field that vanishes on the box boundary, at the interior nodes."""
+    c = u3[1:-1, 1:-1, 1:-1]
+    return (u3[2:, 1:-1, 1:-1] + u3[:-2, 1:-1, 1:-1] + u3[1:-1, 2:, 1:-1] + u3[1:-1, :-2, 1:-1]
+            + u3[1:-1, 1:-1, 2:] + u3[1:-1, 1:-1, :-2] - 6.0 * c) / h ** 2
+
+
+def test_manufactured_solution_full_pf_unequal_radii(oracle):
+    from scipy.fft import dstn, idstn
+    n, h, eps, lc = 20, 0.5, 78.5, 1.2
+    sp = W.NACACL                                   # Na+ 0.95, Ca2+ 0.99, Cl- 1.81, water 1.4 A: unequal radii
+    L = (n - 1) * h
+    x = np.arange(n) * h
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    s = lambda a, u: np.sin(a * np.pi * u / L)
+    phi_star = 6.0 * s(1, X) * s(1, Y) * s(1, Z) - 3.0 * s(2, X) * s(1, Y) * s(3, Z)    # up to ~7.6 kT/e: Ca2+ and Cl- crowd
+    phi_star[[0, -1], :, :] = 0.0; phi_star[:, [0, -1], :] = 0.0; phi_star[:, :, [0, -1]] = 0.0
+    kap = oracle.kappa()
+    C, S = _independent_fermi(oracle, sp.valence, sp.bath_molar, sp.radii, phi_star.ravel())
+    rho = (np.asarray(sp.valence)[:, None] * C[:-1]).sum(0).reshape(n, n, n)
+    # PF1 at the interior nodes, Psi = 0 on the boundary: eps (l_c^2 Lap_h - 1) Psi = kappa rho, by sine transform
+    m = n - 2
+    k = np.arange(1, m + 1)
+    lam1 = -(4.0 / h ** 2) * np.sin(k * np.pi / (2 * (m + 1))) ** 2
+    lam3 = lam1[:, None, None] + lam1[None, :, None] + lam1[None, None, :]
+    rhs1 = kap * rho[1:-1, 1:-1, 1:-1] / eps
+    psi_in = idstn(dstn(rhs1, type=1) / (lc ** 2 * lam3 - 1.0), type=1)
+    psi_star = np.zeros((n, n, n)); psi_star[1:-1, 1:-1, 1:-1] = psi_in
+    assert np.abs(lc ** 2 * _lap7_zero_bc(psi_star, h) - psi_in - rhs1).max() <= 1e-9 * np.abs(rhs1).max()   # the transform solved PF1
+    # the source that makes phi* a solution of PF2 at the fixed point: -eps Lap_h phi* = -eps Psi* + f
+    f = np.zeros((n, n, n))
+    f[1:-1, 1:-1, 1:-1] = -eps * _lap7_zero_bc(phi_star, h) + eps * psi_in
+    bt, bv = [D] * 6, [0.0] * 6
+    r = oracle.solve_pf(n, n, n, h, bt, bv, np.full(n ** 3, eps), np.zeros((0, 4)), sp.valence, sp.bath_molar, sp.radii,
+                        lc, 1e-11, lin_tol=1e-13, max_outer=2000, fixed_override=f.ravel())
+    assert r["status"] == 0, r["outer_iters"]
+    assert np.abs(phi_star).max() > 7.0 and np.abs(S).max() > 0.5          # nonlinear and steric regime indeed (Gamma down to 0.46 Gamma^B)
+    assert np.linalg.norm(r["phi"] - phi_star.ravel()) <= 1e-8 * np.linalg.norm(phi_star)
+    assert np.linalg.norm(r["psi"] - psi_star.ravel()) <= 1e-8 * np.linalg.norm(psi_star)
+    inner = np.zeros((n, n, n), dtype=bool); inner[1:-1, 1:-1, 1:-1] = True
+    for kk in range(len(sp.valence) + 1):
+        assert np.allclose(r["conc"][kk], C[kk], rtol=1e-7)
+    assert np.allclose(r["steric"], S, rtol=1e-6, atol=1e-9)
+    # same fixed point with the merged linear solver
+    r2 = oracle.solve_pf(n, n, n, h, bt, bv, np.full(n ** 3, eps), np.zeros((0, 4)), sp.valence, sp.bath_molar, sp.radii,
+                         lc, 1e-11, lin_tol=1e-13, max_outer=2000, fixed_override=f.ravel(), solver=oracle.SOLVER_MERGED)
+    assert r2["status"] == 0 and np.linalg.norm(r2["phi"] - phi_star.ravel()) <= 1e-8 * np.linalg.norm(phi_star)
+
+
+def test_grid_refinement_second_order_full_pf(oracle):
+    """The same continuous problem (smooth source, uniform eps, Dirichlet 0, l_c = 1.2 A, Na+/Ca2+/Cl-/water with
+    their unequal radii, potentials of several kT/e) on n = 9, 17, 33: differences on the coincident nodes shrink by 4."""
+    sp = W.NACACL
+    L, eps, lc = 8.0, 78.5, 1.2
+    sols = []
+    for n in (9, 17, 33):
+        h = L / (n - 1)
+        x = np.arange(n) * h
+        Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+        src = 2000.0 * np.sin(np.pi * X / L) * np.sin(np.pi * Y / L) * np.sin(np.pi * Z / L) * (1.0 + 0.5 * np.cos(2 * np.pi * Z / L))
+        r = oracle.solve_pf(n, n, n, h, [D] * 6, [0.0] * 6, np.full(n ** 3, eps), np.zeros((0, 4)), sp.valence, sp.bath_molar,
+                            sp.radii, lc, 1e-10, lin_tol=1e-12, max_outer=2000, fixed_override=src.ravel())
+        assert r["status"] == 0
+        sols.append(r["phi"].reshape(n, n, n))
+    assert np.abs(sols[2]).max() > 2.0                                   # several kT/e: nonlinear regime
+    d1 = np.abs(sols[0] - sols[1][::2, ::2, ::2]).max()
+    d2 = np.abs(sols[1] - sols[2][::2, ::2, ::2]).max()
+    assert 3.0 < d1 / d2 < 5.5, (d1, d2)
