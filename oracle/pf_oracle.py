@@ -23,8 +23,22 @@ c_ip = ctypes.POINTER(ctypes.c_int)
 c_u8p = ctypes.POINTER(ctypes.c_uint8)
 
 
+def _sanitized() -> bool:
+    return os.environ.get("PF_ORACLE_SANITIZE", "") not in ("", "0")
+
+
 def build(force: bool = False) -> str:
-    """Compile the oracle: g++ -O2 -ffp-contract=off (every operation rounded as written)."""
+    """Compile the oracle: g++ -O2 -ffp-contract=off (every operation rounded as written).
+
+    PF_ORACLE_SANITIZE=1 builds (and lib() then loads) a second library with -fsanitize=address,undefined; the
+    interpreter then needs the sanitizer runtime preloaded, see profiles/r2_sanitizer.md for the command."""
+    if _sanitized():
+        out = os.path.join(_HERE, "libpf_oracle_san.so")
+        if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(_SRC):
+            cmd = ["g++", "-std=c++17", "-O1", "-g", "-fno-omit-frame-pointer", "-ffp-contract=off",
+                   "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fPIC", "-shared", _SRC, "-o", out]
+            subprocess.run(cmd, check=True)
+        return out
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", _SRC, "-o", _LIB]
         subprocess.run(cmd, check=True)
@@ -34,8 +48,7 @@ def build(force: bool = False) -> str:
 def lib():
     global _lib
     if _lib is None:
-        build()
-        _lib = ctypes.CDLL(_LIB)
+        _lib = ctypes.CDLL(build())
         _lib.pfo_kappa.restype = ctypes.c_double
         _lib.pfo_kT_over_e_volt.restype = ctypes.c_double
         _lib.pfo_molar_to_per_A3.restype = ctypes.c_double
