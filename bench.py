@@ -8,12 +8,20 @@
 One STEP = one pass of the whole hot path:
   rows L1-L2  pf_grid_create + pf_grid_set_workspace: eps scan, node classes, diagonal, (stored
               off-diagonals), fixed-charge deposition
-  rows L3-L8  pf_solve_linear, tol = 0, 200 fixed Jacobi-BiCGSTAB iterations (configs[3] (ii))
   rows N1-N5  pf_solve_pf capped at one outer iteration with 25 fixed iterations per linear solve:
               initial guess, fused Fermi kernel, PF1, PF2, relaxation + max-norm (3 x 25 iterations)
+  rows L3-L8  pf_solve_linear, tol = 0, 200 fixed Jacobi-BiCGSTAB iterations (configs[3] (ii))
 value = BiCGSTAB iterations of the step (275) / step time, whole job.  Inputs are resident in HBM
 for `value`; `e2e` repeats the step through the C ABI with HOST buffers (copies inside the timing).
 Multi-GPU: the path does not shard (replicas only) -- every rank runs the same step.
+
+Beside `value` the line carries, all measured in the same run (N = 1):
+  roofline   the whole BiCGSTAB iteration (every kernel of the hot loop bracketed by CUDA events on the library's
+             stream) against the measured HBM peak, per-kernel figures and the kernel furthest below its roofline
+  variants   the same step with the stored-coefficient stencil (configs[3]'s comparison) and with the merged
+             two-reduction solver (--solver merged) -- whichever is not the main configuration
+  pf_solve   wall time and iteration counts of the full nonlinear PF solve of configs[2] (the metric's third part)
+  cpu_baseline, e2e, clocks, gpu_launches as the contract says.
 """
 from __future__ import annotations
 
@@ -63,6 +71,8 @@ def parse():
     ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-variants", action="store_true", help="skip the stored / merged variants of the step")
+    ap.add_argument("--no-pf-solve", action="store_true", help="skip the full nonlinear PF solve of configs[2]")
     ap.add_argument("--ref-iters", type=int, default=4, help="oracle iterations per reference step")
     return ap.parse_args()
 
@@ -233,45 +243,62 @@ def run_b200(args):
     phi_dev = torch.zeros(n, dtype=torch.float64, device="cuda")
 
     # workspace is allocated once, outside the timing: it is caller-owned scratch by the ABI
-    probe = pf.pf_grid_create(w.nx, w.ny, w.nz, w.h, eps_dev, w.charges, w.bc_type, w.bc_value)
-    pf.pf_grid_set_option(probe, pf.PF_OPT_STENCIL, stencil)
-    ws = torch.empty(pf.pf_grid_workspace_bytes(probe), dtype=torch.uint8, device="cuda")
-    pf.pf_grid_destroy(probe)
-    prof_tot = {k: dict(ms=0.0, launches=0) for k in ("k1", "k2", "k3")}
+    def make_cfg(stencil_name: str, solver_name: str) -> dict:
+        st = pf.STENCIL_STORED if stencil_name == "stored" else pf.STENCIL_ONTHEFLY
+        probe = pf.pf_grid_create(w.nx, w.ny, w.nz, w.h, eps_dev, w.charges, w.bc_type, w.bc_value)
+        pf.pf_grid_set_option(probe, pf.PF_OPT_STENCIL, st)
+        wsp = torch.empty(pf.pf_grid_workspace_bytes(probe), dtype=torch.uint8, device="cuda")
+        pf.pf_grid_destroy(probe)
+        return dict(stencil=st, stencil_name=stencil_name, solver=1 if solver_name == "merged" else 0,
+                    solver_name=solver_name, ws=wsp, prof={k: dict(ms=0.0, launches=0) for k in ("k1", "k2", "k3")})
 
-    def step(host_buffers: bool, profile: bool):
+    main_cfg = make_cfg(args.stencil, args.solver)
+    side = torch.cuda.Stream()
+    ws, prof_tot = main_cfg["ws"], main_cfg["prof"]
+
+    def step(host_buffers: bool, profile: bool, cfg: dict = None):
+        cfg = cfg or main_cfg
+        ws, prof_tot = cfg["ws"], cfg["prof"]
         if host_buffers:
             eps_dev.copy_(eps_host, non_blocking=True)
         h = pf.pf_grid_create(w.nx, w.ny, w.nz, w.h, eps_dev, w.charges, w.bc_type, w.bc_value)
-        pf.pf_grid_set_option(h, pf.PF_OPT_STENCIL, stencil)
+        pf.pf_grid_set_option(h, pf.PF_OPT_STENCIL, cfg["stencil"])
         if kernels:
             pf.pf_grid_set_option(h, pf.PF_OPT_KERNELS, kernels)
         pf.pf_grid_set_option(h, pf.PF_OPT_GRAPH, {"auto": 3, "loop": 2, "chunks": 1, "stream": 0}[args.launch_mode])
-        pf.pf_grid_set_option(h, pf.PF_OPT_SOLVER, 1 if args.solver == "merged" else 0)
+        pf.pf_grid_set_option(h, pf.PF_OPT_SOLVER, cfg["solver"])
         pf.pf_grid_set_option(h, pf.PF_OPT_LINEAR_TOL, 0.0)
         pf.pf_grid_set_option(h, pf.PF_OPT_LINEAR_MAXIT, PF_INNER_ITERS)
         pf.pf_grid_set_option(h, pf.PF_OPT_MAX_OUTER, 1)
-        if profile:
-            pf.pf_grid_set_option(h, pf.PF_OPT_PROFILE, PROFILE_ITERS)
         pf.pf_grid_set_workspace(h, ws)                                            # rows L1, L2
         if host_buffers:
+            # the upload of rhs and x0 runs on the grid's copy stream while the PF pass computes
             x_host.zero_()
+            pf.pf_grid_stage_host(h, n, rhs_host, x_host)
+        res = pf.pf_solve_pf(h, n, sp.valence, sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol, phi_dev)  # N1-N5
+        assert res["linear_iters"] == 3 * PF_INNER_ITERS, res
+        if host_buffers:
+            # ... and phi goes back to the host on a side stream while the linear solve runs
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                phi_host.copy_(phi_dev, non_blocking=True)
+        if profile:      # the events bracket iterations of the long linear solve only (the PF pass runs unprofiled)
+            pf.pf_grid_set_option(h, pf.PF_OPT_PROFILE, PROFILE_ITERS)
+        if host_buffers:
             out = pf.pf_solve_linear_host(h, n, rhs_host, x_host, 0.0, lin_iters, true_residual=False)
         else:
             x_dev.zero_()
             out = pf.pf_solve_linear(h, n, rhs_dev, x_dev, 0.0, lin_iters, true_residual=False)   # rows L3-L8
         assert out["iters"] == lin_iters, out
-        if profile:      # the events bracket iterations of this solve only (the PF pass runs unprofiled)
+        if profile:
             p = pf.pf_grid_profile(h)
             for k in prof_tot:
                 prof_tot[k]["ms"] += p[k]["ms"]
                 prof_tot[k]["launches"] += p[k]["launches"]
             pf.pf_grid_set_option(h, pf.PF_OPT_PROFILE, 0)
-        res = pf.pf_solve_pf(h, n, sp.valence, sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol, phi_dev)  # N1-N5
-        assert res["linear_iters"] == 3 * PF_INNER_ITERS, res
         if host_buffers:
-            phi_host.copy_(phi_dev, non_blocking=True)
-            torch.cuda.current_stream().synchronize()
+            side.synchronize()
+            torch.cuda.current_stream().wait_stream(side)      # phi_dev is rewritten by the next step
         pf.pf_grid_destroy(h)
         return out
 
@@ -280,14 +307,21 @@ def run_b200(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed(nsteps, host_buffers, profile):
+    def timed(nsteps, host_buffers, profile, cfg=None, sync=True):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        barrier()
+        if sync:
+            barrier()
+        else:
+            torch.cuda.synchronize()
         e0.record()
         for _ in range(nsteps):
-            step(host_buffers, profile)
+            step(host_buffers, profile, cfg)
         e1.record()
-        barrier()
+        if sync:
+            barrier()
+        else:
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1)
         ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
         if world > 1:
             dist.all_reduce(ms, op=dist.ReduceOp.MAX)
@@ -311,47 +345,103 @@ def run_b200(args):
         e2e = {"value": world * step_iters * e2e_steps / (ms_e2e * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": 8 * n * 3, "d2h_bytes_per_step": 8 * n * 2,
                "ms_per_step": ms_e2e / e2e_steps,
-               "what": "eps, rhs, x0 host->device; x, phi device->host; C-ABI pf_solve_linear_host"}
+               "what": "eps, rhs, x0 host->device; x, phi device->host; C-ABI pf_grid_stage_host + pf_solve_linear_host: the "
+                       "rhs/x0 upload overlaps the PF pass, the phi download the linear solve; eps up and x down are exposed"}
 
     if rank == 0:
         peak, peak_src = measured_peak_gbs()
-        stored = args.stencil == "stored"
-        merged = args.solver == "merged"
-        bpu = kernel_bytes_per_unknown(stored, merged)
-        kernels_rep = {}
-        for k in ("k1", "k2", "k3"):
-            if prof_tot[k]["launches"] and k in bpu:
-                avg_ms = prof_tot[k]["ms"] / prof_tot[k]["launches"]
-                gbs = bpu[k] * n / (avg_ms * 1e-3) / 1e9
-                kernels_rep[k] = {"avg_ms": avg_ms, "launches": prof_tot[k]["launches"],
-                                  "bytes_per_unknown": bpu[k], "gbs": gbs, "frac": gbs / peak}
-        dom = max(kernels_rep, key=lambda k: kernels_rep[k]["avg_ms"] * kernels_rep[k]["launches"])
-        iter_ms = sum(kernels_rep[k]["avg_ms"] for k in kernels_rep)
-        iter_bytes = sum(bpu.values()) * n
-        # DRAM bytes per launch from the committed ncu --set full capture (profiles/traffic.csv: stencil,n,kernel,bytes)
-        traffic = None
-        try:
-            with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
-                for row in f:
-                    c = [x.strip() for x in row.split(",")]
-                    if len(c) >= 4 and c[0] == args.stencil and c[1] == str(args.n) and c[2] == dom:
-                        traffic = int(c[3])
-        except (OSError, ValueError):
-            traffic = None
-        names = {"k1": "k1 (p-update + matvec + r~.v)", "k2": "k2 (s-update + matvec + t.s,t.t)",
-                 "k3": "k3 (x,r update + r~.r, r.r)"}
-        if merged:
-            names = {"k2": "K2M (s-update + matvec + t.s, t.t, r~.t)",
-                     "k3": "K31 (x, r, p update + matvec + r~.v, r.r, r~.r)"}
-        roofline = {"bound": "hbm", "kernel": names[dom],
-                    "achieved": kernels_rep[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                    "frac": kernels_rep[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
-                    "per_kernel": kernels_rep,
-                    "iteration": {"ms": iter_ms, "bytes_per_unknown": sum(bpu.values()),
-                                  "gbs": iter_bytes / (iter_ms * 1e-3) / 1e9,
-                                  "frac": iter_bytes / (iter_ms * 1e-3) / 1e9 / peak,
-                                  "iterations_per_s_linear_solve": 1e3 / iter_ms,
-                                  "mupdates_per_s": n / iter_ms / 1e3}}
+
+        def roofline_of(cfg: dict) -> dict:
+            """Per-kernel and per-iteration roofline figures from the CUDA-event brackets of a configuration."""
+            stored, merged = cfg["stencil_name"] == "stored", cfg["solver_name"] == "merged"
+            bpu = kernel_bytes_per_unknown(stored, merged)
+            names = {"k1": "k1 (p-update + matvec + r~.v)", "k2": "k2 (s-update + matvec + t.s, t.t)",
+                     "k3": "k3 (x, r update + r~.r, r.r)"}
+            tnames = {"k1": "k1", "k2": "k2", "k3": "k3"}
+            if merged:
+                names = {"k2": "K2M (s-update + matvec + t.s, t.t, r~.t)",
+                         "k3": "K31 (x, r, p update + matvec + r~.v, r.r, r~.r)"}
+                tnames = {"k2": "k2m", "k3": "k31"}
+            # DRAM bytes per launch from the committed ncu --set full capture (profiles/traffic.csv); static, not
+            # measured in this run: the csv names the capture and its commit
+            tr, tr_src = {}, None
+            try:
+                with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+                    for row in f:
+                        c = [x.strip() for x in row.split(",")]
+                        if len(c) >= 5 and c[0] == cfg["stencil_name"] and c[1] == str(args.n):
+                            tr[c[2]] = int(c[3]); tr_src = c[4]
+            except (OSError, ValueError):
+                pass
+            per = {}
+            for k in ("k1", "k2", "k3"):
+                if cfg["prof"][k]["launches"] and k in bpu:
+                    avg_ms = cfg["prof"][k]["ms"] / cfg["prof"][k]["launches"]
+                    gbs = bpu[k] * n / (avg_ms * 1e-3) / 1e9
+                    per[k] = {"name": names[k], "avg_ms": avg_ms, "launches": cfg["prof"][k]["launches"],
+                              "bytes_per_unknown": bpu[k], "gbs": gbs, "frac": gbs / peak,
+                              "traffic": tr.get(tnames[k])}
+            if not per:
+                return None
+            iter_ms = sum(per[k]["avg_ms"] for k in per)
+            iter_b = sum(per[k]["bytes_per_unknown"] for k in per)
+            gbs = iter_b * n / (iter_ms * 1e-3) / 1e9
+            worst = min(per, key=lambda k: per[k]["frac"])
+            tsum = None if any(per[k]["traffic"] is None for k in per) else sum(per[k]["traffic"] for k in per)
+            # headline: the whole iteration (every kernel of the hot loop, launched one by one between CUDA events), not
+            # the kernel that happens to take longest; the kernel furthest below its roofline is named beside it
+            return {"bound": "hbm", "kernel": "one BiCGSTAB iteration = " + " + ".join(per[k]["name"].split(" ")[0] for k in per),
+                    "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                    "frac_of_nominal_8000": gbs / 8000.0, "traffic": tsum,
+                    "traffic_source": (("static: " + tr_src + "; not measured in this run") if tsum is not None else None),
+                    "peak_source": peak_src, "bytes_per_unknown": iter_b, "ms": iter_ms,
+                    "iterations_per_s_linear_solve": 1e3 / iter_ms, "mupdates_per_s": n / iter_ms / 1e3,
+                    "worst_kernel": {"kernel": per[worst]["name"], "frac": per[worst]["frac"], "gbs": per[worst]["gbs"]},
+                    "per_kernel": per}
+
+        roofline = roofline_of(main_cfg)
+
+        # configs[3] asks for the stored-coefficient stencil beside the on-the-fly one; SURVEY 8(f) #3 for the merged
+        # recurrence beside Table 3: the same step, each variant with its own workspace, timed in this run
+        variants = {}
+        if not args.no_variants and world == 1:      # (replicas: rank 0 must not keep the other ranks waiting)
+            for name, (st, so) in {"stored": ("stored", "table3"), "onthefly": ("onthefly", "table3"),
+                                   "merged": ("onthefly", "merged")}.items():
+                if (st, so) == (args.stencil, args.solver):
+                    continue
+                cfg = make_cfg(st, so)
+                for _ in range(3):
+                    step(False, False, cfg)
+                vsteps = max(1, min(args.steps, 5))
+                ms_v = timed(vsteps, False, True, cfg, sync=False)
+                r = roofline_of(cfg)
+                variants[name] = {"stencil": st, "solver": so, "value": step_iters * vsteps / (ms_v * 1e-3), "unit": UNIT,
+                                  "steps": vsteps, "ms_per_step": ms_v / vsteps,
+                                  "iteration": None if r is None else {k: r[k] for k in ("ms", "bytes_per_unknown", "achieved", "frac",
+                                                                                         "iterations_per_s_linear_solve")},
+                                  "per_kernel": None if r is None else {k: {kk: v[kk] for kk in ("name", "avg_ms", "bytes_per_unknown", "frac")}
+                                                                        for k, v in r["per_kernel"].items()}}
+                del cfg
+                torch.cuda.empty_cache()
+
+        # the metric's third part, "PF total solve time": the full nonlinear solve of configs[2] (128^3, +50 mV) to its
+        # own tolerances (linear 1e-10, increment 1e-8), wall clock around pf_solve_pf, after one warm-up solve
+        pf_solve = None
+        if not args.no_pf_solve and world == 1:
+            w2 = wl.config2(volt_mv=50.0)
+            g2 = pf.Grid.from_workload(w2, options={pf.PF_OPT_SOLVER: main_cfg["solver"]})
+            sp2 = w2.species
+            g2.solve_pf(sp2.valence, sp2.bath_molar, sp2.radii, w2.l_c, w2.nonlinear_tol, want_conc=False)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            o2 = g2.solve_pf(sp2.valence, sp2.bath_molar, sp2.radii, w2.l_c, w2.nonlinear_tol, want_conc=False)
+            torch.cuda.synchronize()
+            dt2 = time.perf_counter() - t0
+            g2.close()
+            pf_solve = {"workload": "configs[2] channel 128^3, Na+/Ca2+/Cl-/water, +50 mV, linear tol 1e-10, increment tol 1e-8",
+                        "seconds": dt2, "status": o2["status"], "outer_iterations": o2["outer_iters"],
+                        "linear_iterations": o2["linear_iters"], "solver": args.solver,
+                        "us_per_linear_iteration": 1e6 * dt2 / max(o2["linear_iters"], 1)}
         cpu = None
         if not args.no_cpu_baseline and world == 1:
             from oracle import pf_oracle as oracle
@@ -373,6 +463,7 @@ def run_b200(args):
                            "iterations_per_step": step_iters, "parallelism": "replicas only" if world > 1 else "1 GPU",
                            "l2": "inputs larger than L2 (working set %.1f GB)" % (ws.numel() / 1e9)},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+                "variants": variants, "pf_solve": pf_solve,
                 "paper_context": "paper: 22.8x linear-solver, 16.9x total speedup, GTX TITAN X vs Xeon E5-1650 "
                                  "(PAPER.md:305-311); other hardware, context only"}
         print(json.dumps(line), flush=True)

@@ -174,6 +174,13 @@ int pf_solve_linear_host(pf_grid *g, const double *rhs_host, double *x_host, con
                          double tol, int maxit,
                          int *iters_out, double *relres_out, double *true_relres_out);
 
+/* Start the upload of the host buffers of a later pf_solve_linear_host(g, rhs_host, x_host, ...) on a copy stream of
+ * the grid's own and return at once: the copy then overlaps whatever the grid's stream does in between (assembly of
+ * another operator, a pf_solve_pf).  rhs_host, x_host: host (pinned, or the copy is not asynchronous), N doubles; they
+ * must stay unchanged until that pf_solve_linear_host, which recognises the pair by its addresses and then waits for
+ * the copy instead of uploading again; any other pair of addresses is uploaded as usual.  Needs the workspace. */
+int pf_grid_stage_host(pf_grid *g, const double *rhs_host, const double *x_host);
+
 /* Nonlinear PF solve (Table 2 steps 2-5): initial guess from PF2 with rho' = Psi = 0, then
  * { Fermi update at phi0 -> PF1 for Psi -> PF2 for phi -> relax -> test ||phi - phi0||_inf <= tol }.
  *   nions K; valence, bath_conc (mol/L): host, K entries; radii: host, K+1 entries in Angstrom,

@@ -143,6 +143,12 @@ struct pf_grid {
     bool assembled;
     double pf1_lc;           // l_c the PF1 operator was assembled for (NaN = none)
     double *r, *r1, *rt, *p0, *p1, *v0, *v1, *t, *y, *bw, *xw;      // r1: second residual buffer of the merged solver
+    // host-buffer flavour (pf_solve_linear_host, pf_grid_stage_host): device staging of rhs and x, their own vectors so
+    // that an upload can run on the copy stream while other work of the grid (assembly, a PF solve) uses the scratch
+    double *hb, *hx;
+    cudaStream_t copy_stream;
+    cudaEvent_t staged_ev, main_ev;
+    const void *staged_rhs, *staged_x;
     double *A0, *A0_pf1, *A0_s, *fixed, *psi, *phi0, *phiw, *sigma, *bpf;
     void *code, *code_pf1;   // stencil codes of the on-the-fly variant (pf_common.cuh Operator)
     int code_mode;           // 0 none (palette overflow), 1 uint16, 2 uint32
@@ -200,7 +206,7 @@ int fail(pf_grid* g, int code, const char* fmt, ...) {
     } while (0)
 
 int n_vectors(bool stored, int charge_model, bool fixed_nodes, bool padx) {
-    return 20 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0) + (fixed_nodes ? 1 : 0) + (padx ? 3 + (stored ? 6 : 0) : 0);
+    return 22 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0) + (fixed_nodes ? 1 : 0) + (padx ? 3 + (stored ? 6 : 0) : 0);
 }
 
 int code_mode_of(const pf_grid* g) { return g->pal.count > PF_MAX_PALETTE ? 0 : (g->pal.count <= 2 ? 1 : 2); }
@@ -724,6 +730,8 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->opt_profile = 0; g->prof_ms[0] = g->prof_ms[1] = g->prof_ms[2] = 0.0;
     g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
+    g->hb = g->hx = nullptr; g->copy_stream = nullptr; g->staged_ev = g->main_ev = nullptr;
+    g->staged_rhs = g->staged_x = nullptr;
     g->capture_stream = nullptr; g->opt_graph = 3; g->opt_diag_code = 1; g->opt_norm = 0; g->opt_solver = 0;
     g->opt_charge_model = 0; g->charge_model = 0; g->phiL = g->phistar = g->A0_L = nullptr; g->code_L = nullptr;
     g->ctab_L = nullptr; g->laplace_iters = 0; g->fixv = nullptr; g->bc.fixv = nullptr;
@@ -783,6 +791,9 @@ void pf_grid_destroy(pf_grid* g) {
     small_set_release(g->small);
     for (auto& cg : g->graphs) cudaGraphExecDestroy(cg.exec);
     if (g->capture_stream) cudaStreamDestroy(g->capture_stream);
+    if (g->copy_stream) { cudaStreamSynchronize(g->copy_stream); cudaStreamDestroy(g->copy_stream); }
+    if (g->staged_ev) cudaEventDestroy(g->staged_ev);
+    if (g->main_ev) cudaEventDestroy(g->main_ev);
     cudaFree(g->hist);
     if (g->tma) tma_set_destroy(g->tma);
     for (cudaEvent_t e : g->prof_ev) cudaEventDestroy(e);
@@ -901,7 +912,8 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     char* base = (char*)dev_ptr;
     auto take = [&]() { double* p = (double*)base; base += vec; return p; };
     g->r = take(); g->r1 = take(); g->rt = take(); g->p0 = take(); g->p1 = take(); g->v0 = take(); g->v1 = take();
-    g->t = take(); g->y = take(); g->bw = take(); g->xw = take();
+    g->t = take(); g->y = take(); g->bw = take(); g->xw = take(); g->hb = take(); g->hx = take();
+    g->staged_rhs = g->staged_x = nullptr;
     g->A0 = take(); g->A0_pf1 = take(); g->A0_s = take(); g->fixed = take(); g->psi = take();
     g->phi0 = take(); g->phiw = take(); g->sigma = take(); g->bpf = take();
     g->charge_model = g->opt_charge_model;
@@ -991,18 +1003,43 @@ int pf_solve_linear(pf_grid* g, const double* rhs, double* x, const double* sigm
     return rc;
 }
 
+int pf_grid_stage_host(pf_grid* g, const double* rhs_host, const double* x_host) {
+    int rc = check_ready(g);
+    if (rc) return rc;
+    if (!rhs_host || !x_host) return fail(g, PF_ERR_ARG, "rhs and x must not be NULL");
+    if (!g->copy_stream) {
+        PF_CUDA(g, cudaStreamCreateWithFlags(&g->copy_stream, cudaStreamNonBlocking));
+        PF_CUDA(g, cudaEventCreateWithFlags(&g->staged_ev, cudaEventDisableTiming));
+        PF_CUDA(g, cudaEventCreateWithFlags(&g->main_ev, cudaEventDisableTiming));
+    }
+    const size_t nbytes = sizeof(double) * (size_t)g->g.n;
+    // work already enqueued on the grid's stream may still read the staging vectors (an earlier host solve)
+    PF_CUDA(g, cudaEventRecord(g->main_ev, g->stream));
+    PF_CUDA(g, cudaStreamWaitEvent(g->copy_stream, g->main_ev, 0));
+    PF_CUDA(g, cudaMemcpyAsync(g->hb, rhs_host, nbytes, cudaMemcpyHostToDevice, g->copy_stream));
+    PF_CUDA(g, cudaMemcpyAsync(g->hx, x_host, nbytes, cudaMemcpyHostToDevice, g->copy_stream));
+    PF_CUDA(g, cudaEventRecord(g->staged_ev, g->copy_stream));
+    g->staged_rhs = rhs_host; g->staged_x = x_host;
+    return PF_OK;
+}
+
 int pf_solve_linear_host(pf_grid* g, const double* rhs_host, double* x_host, const double* sigma, double tol,
                          int maxit, int* iters_out, double* relres_out, double* true_relres_out) {
     int rc = check_ready(g);
     if (rc) return rc;
     if (!rhs_host || !x_host) return fail(g, PF_ERR_ARG, "rhs and x must not be NULL");
     const size_t nbytes = sizeof(double) * (size_t)g->g.n;
-    // bpf and xw are scratch of the PF loop, free during a plain linear solve
-    PF_CUDA(g, cudaMemcpyAsync(g->bpf, rhs_host, nbytes, cudaMemcpyHostToDevice, g->stream));
-    PF_CUDA(g, cudaMemcpyAsync(g->xw, x_host, nbytes, cudaMemcpyHostToDevice, g->stream));
-    rc = pf_solve_linear(g, g->bpf, g->xw, sigma, tol, maxit, iters_out, relres_out, true_relres_out);
+    if (g->staged_rhs == rhs_host && g->staged_x == x_host) {
+        // uploaded ahead by pf_grid_stage_host on the copy stream: the solve only waits for that copy
+        PF_CUDA(g, cudaStreamWaitEvent(g->stream, g->staged_ev, 0));
+    } else {
+        PF_CUDA(g, cudaMemcpyAsync(g->hb, rhs_host, nbytes, cudaMemcpyHostToDevice, g->stream));
+        PF_CUDA(g, cudaMemcpyAsync(g->hx, x_host, nbytes, cudaMemcpyHostToDevice, g->stream));
+    }
+    g->staged_rhs = g->staged_x = nullptr;
+    rc = pf_solve_linear(g, g->hb, g->hx, sigma, tol, maxit, iters_out, relres_out, true_relres_out);
     if (rc < 0) return rc;
-    PF_CUDA(g, cudaMemcpyAsync(x_host, g->xw, nbytes, cudaMemcpyDeviceToHost, g->stream));
+    PF_CUDA(g, cudaMemcpyAsync(x_host, g->hx, nbytes, cudaMemcpyDeviceToHost, g->stream));
     PF_CUDA(g, cudaStreamSynchronize(g->stream));
     return rc;
 }

@@ -31,7 +31,7 @@ KERNELS_AUTO, KERNELS_DIRECT, KERNELS_TILED, KERNELS_COOP = 0, 1, 2, 3
 
 EXPORTS = [
     "pf_grid_create", "pf_grid_set_fixed_nodes", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
-    "pf_solve_linear", "pf_solve_linear_host", "pf_solve_pf", "pf_fermi_pointwise", "pf_grid_history",
+    "pf_solve_linear", "pf_solve_linear_host", "pf_grid_stage_host", "pf_solve_pf", "pf_fermi_pointwise", "pf_grid_history",
     "pf_grid_linear_iters", "pf_grid_increments", "pf_grid_fault_repeats", "pf_grid_laplace_iters", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_code_layout", "pf_grid_copy_array",
     "pf_grid_profile", "pf_launch_count", "pf_coop_plan", "pf_grid_destroy", "pf_last_error", "pf_version",
 ]
@@ -74,6 +74,7 @@ def load():
     L.pf_grid_set_option.argtypes = [_vp, ctypes.c_int, ctypes.c_double]
     L.pf_solve_linear.argtypes = [_vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_int, _ip, _dp, _dp]
     L.pf_solve_linear_host.argtypes = [_vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_int, _ip, _dp, _dp]
+    L.pf_grid_stage_host.argtypes = [_vp, _vp, _vp]
     L.pf_solve_pf.argtypes = [_vp, ctypes.c_int, _dp, _dp, _dp, ctypes.c_double, ctypes.c_double, _vp, _vp, _vp,
                               _ip, _ip]
     L.pf_fermi_pointwise.argtypes = [_vp, ctypes.c_int, _dp, _dp, _dp, _vp, _vp, _vp, _vp, _vp]
@@ -185,6 +186,14 @@ def pf_solve_linear_host(handle, n: int, rhs_host: torch.Tensor, x_host: torch.T
                                      ctypes.byref(tr) if true_residual else None)
     _check(handle, rc)
     return dict(status=rc, iters=it.value, relres=rr.value, true_relres=tr.value if true_residual else None)
+
+
+def pf_grid_stage_host(handle, n: int, rhs_host: torch.Tensor, x_host: torch.Tensor) -> None:
+    """Start the upload of the (pinned) host buffers of the next pf_solve_linear_host on the grid's copy stream."""
+    for t in (rhs_host, x_host):
+        if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous() or t.numel() != n:
+            raise ValueError("expected contiguous CPU float64 tensors of n elements")
+    _check(handle, load().pf_grid_stage_host(handle, rhs_host.data_ptr(), x_host.data_ptr()))
 
 
 def pf_solve_pf(handle, n: int, valence, bath_conc, radii, l_c: float, tol: float, phi: torch.Tensor,

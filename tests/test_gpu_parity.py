@@ -277,6 +277,30 @@ def test_linear_host_buffers(pf, oracle):
     assert out["status"] == 0 and rel_l2(x_h.numpy(), ref["x"]) <= 1e-9
 
 
+def test_linear_host_buffers_staged_upload(pf, oracle):
+    """pf_grid_stage_host: the upload runs on the grid's copy stream while a PF solve uses the grid; the host solve that
+    follows recognises the staged pair and gives the bits of the plain host solve.  Another pair is uploaded as usual."""
+    w = wl.config0(n=32)
+    sp = w.species
+    rhs = np.random.default_rng(2).standard_normal(w.n)
+    g = pf.Grid.from_workload(w, kernels=pf.KERNELS_TILED)
+    rhs_h = torch.tensor(rhs).pin_memory()
+    x_plain = torch.zeros(w.n, dtype=torch.float64).pin_memory()
+    a = pf.pf_solve_linear_host(g.handle, w.n, rhs_h, x_plain, 1e-10, 10000)
+    x_staged = torch.zeros(w.n, dtype=torch.float64).pin_memory()
+    pf.pf_grid_stage_host(g.handle, w.n, rhs_h, x_staged)
+    g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, 1e-3, want_conc=False)      # uses the PF scratch meanwhile
+    b = pf.pf_solve_linear_host(g.handle, w.n, rhs_h, x_staged, 1e-10, 10000)
+    assert a["status"] == 0 == b["status"] and a["iters"] == b["iters"]
+    assert torch.equal(x_plain, x_staged)
+    # staged for one pair, solved with another: the other pair is uploaded, the result is that pair's
+    x_other = torch.zeros(w.n, dtype=torch.float64).pin_memory()
+    pf.pf_grid_stage_host(g.handle, w.n, rhs_h, x_staged)
+    c = pf.pf_solve_linear_host(g.handle, w.n, (2.0 * rhs_h).pin_memory(), x_other, 1e-10, 10000)
+    assert c["status"] == 0 and rel_l2(x_other.numpy(), 2.0 * x_plain.numpy()) <= 1e-9
+    g.close()
+
+
 # ---- row N1: pointwise Fermi kernel --------------------------------------------------------------
 
 @pytest.mark.parametrize("species", ["nacl", "nacacl", "nosteric"])
