@@ -531,6 +531,40 @@ void fermi_field(const SpeciesTab& sp, int64_t N, const double* phi, const uint8
     }
 }
 
+// ---- Lagged reading of Eq (11) (readings G1-G2 of DESIGN.md) --------------------
+// Eq (11) writes C_k^0, S_0^trc and Gamma_0 with the same subscript 0 although each is defined through the others.
+// Besides solving the three definitions simultaneously per node (fermi_node, the default), one can take them as
+// assignments in the order written: C_k^0 from phi_0 and the S^trc that is at hand (that of the previous outer
+// iteration, 0 = the bath value before the first), then Gamma_0 from these C_k^0, then S_0^trc from Gamma_0 for the
+// NEXT outer iteration.  Both readings have the same fixed point.  G2: nothing keeps sum v_k C_k^0 below 1 here
+// (the saturation property C_k < 1/v_k of PAPER.md:45 belongs to the simultaneous solution), so Gamma_0 is floored
+// at GAMMA_FLOOR before the logarithm.  S (N, in/out): the state; null entries of the outputs are skipped.
+const double GAMMA_FLOOR = 1e-12;
+
+void fermi_field_lagged(const SpeciesTab& sp, int64_t N, const double* phi, const uint8_t* solvent, double* S,
+                        bool update, double* rho, double* sigma, double* conc /* (K+1)*N or null */) {
+    const double kap = kappa_angstrom();
+    std::vector<double> c(sp.K + 1);
+    for (int64_t i = 0; i < N; ++i) {
+        double r = 0.0, sg = 0.0;
+        if (solvent[i]) {
+            double occ = 0.0;
+            for (int k = 0; k <= sp.K; ++k) {
+                c[k] = sp.cb[k] * std::exp(-sp.z[k] * phi[i] + sp.lam[k] * S[i]);        // Eq (1) with the S at hand
+                if (k < sp.K) { r += sp.z[k] * c[k]; sg += sp.z[k] * sp.z[k] * c[k]; }
+                occ += sp.vol[k] * c[k];
+            }
+            sg = kap * sg;
+            if (update && sp.steric) S[i] = std::log(std::max(1.0 - occ, GAMMA_FLOOR) / sp.gammaB);   // G2
+        } else {
+            std::fill(c.begin(), c.end(), 0.0);
+        }
+        if (rho) rho[i] = r;
+        if (sigma) sigma[i] = sg;
+        if (conc) for (int k = 0; k <= sp.K; ++k) conc[(int64_t)k * N + i] = c[k];
+    }
+}
+
 // N2/N3 right-hand sides.
 void rhs_pf1(const Grid& g, const uint8_t* solvent, const double* rho, double* b) {
     const double kap = kappa_angstrom();
@@ -796,7 +830,8 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
                  int* outer_iters, int* linear_iters, int* lin_iters_hist, int hist_cap,
                  double* incr_hist, const double* fixed_override /* b^IF of the singular-charge model, or null */,
                  const uint8_t* fix_mask, const double* fix_val /* Omega_f, or null */,
-                 int solver /* linear solver of every step: 0 Table 3, 1 merged */) {
+                 int solver /* linear solver of every step: 0 Table 3, 1 merged */,
+                 int steric_mode /* 0: Eq (1) solved simultaneously per node (Q11); 1: lagged (G1) */) {
     Grid g = mk(nx, ny, nz, h, bct, bcv, fix_mask, fix_val);
     const int64_t N = g.n();
     SpeciesTab sp;
@@ -808,7 +843,7 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
     // Psi = 0); their PF2 rows are the identity rows that assemble_poisson and set_dirichlet produce
     if (fix_mask) for (int64_t i = 0; i < N; ++i) if (fix_mask[i]) solv[i] = 0;
     std::vector<double> fixed(N, 0.0), A0(7 * N), A1(7 * N), A2(7 * N), b(N);
-    std::vector<double> phi0(N, 0.0), Psi(N, 0.0), ph(N), rho(N), sigma(N), S(N);
+    std::vector<double> phi0(N, 0.0), Psi(N, 0.0), ph(N), rho(N), sigma(N), S(N), Slag(steric_mode == 1 ? N : 0, 0.0);
     if (fixed_override) std::memcpy(fixed.data(), fixed_override, N * sizeof(double));
     else deposit_charges(g, charges, M, fixed.data());
     int nsolve = 0, total = 0, its = 0;
@@ -827,7 +862,8 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
     int status = 1, outer = 0;
     while (outer < max_outer) {
         ++outer;
-        fermi_field(sp, N, phi0.data(), solv.data(), rho.data(), sigma.data(), S.data(), nullptr);
+        if (steric_mode == 1) fermi_field_lagged(sp, N, phi0.data(), solv.data(), Slag.data(), true, rho.data(), sigma.data(), nullptr);
+        else fermi_field(sp, N, phi0.data(), solv.data(), rho.data(), sigma.data(), S.data(), nullptr);
         // step 3 / 5: PF1 -> Psi (warm start: previous Psi)
         rhs_pf1(g, solv.data(), rho.data(), b.data());
         rc = krylov(solver, g, A1.data(), b.data(), Psi.data(), lin_tol, lin_maxit, 1, &its, &rr, &tr, nullptr, norm_mode);
@@ -853,7 +889,10 @@ int pfo_solve_pf(int nx, int ny, int nz, double h, const int* bct, const double*
     }
     std::memcpy(phi, phi0.data(), N * sizeof(double));
     if (psi) std::memcpy(psi, Psi.data(), N * sizeof(double));
-    if (conc || steric) fermi_field(sp, N, phi0.data(), solv.data(), nullptr, nullptr, steric, conc);
+    if (steric_mode == 1) {          // the fields that belong to the state: C_k from the final phi and the S at hand
+        if (conc) fermi_field_lagged(sp, N, phi0.data(), solv.data(), Slag.data(), false, nullptr, nullptr, conc);
+        if (steric) std::memcpy(steric, Slag.data(), N * sizeof(double));
+    } else if (conc || steric) fermi_field(sp, N, phi0.data(), solv.data(), nullptr, nullptr, steric, conc);
     *outer_iters = outer;
     *linear_iters = total;
     if (status == 0 && inner_maxit) return 2;    // converged on the increment, but an inner solve was cut off

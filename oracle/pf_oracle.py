@@ -163,6 +163,7 @@ def deposit_charges(nx, ny, nz, h, charges) -> np.ndarray:
 
 NORM_REL_L2, NORM_ABS_INF = 0, 1     # stopping test: BASELINE's relative 2-norm / the paper's absolute maximum norm
 SOLVER_TABLE3, SOLVER_MERGED = 0, 1  # Table 3 as written / the merged two-reduction rearrangement (reading M1)
+STERIC_SIMULTANEOUS, STERIC_LAGGED = 0, 1   # Eq (1) solved per node (Q11) / S^trc from the previous outer iteration (G1)
 
 
 def bicgstab(nx, ny, nz, A, b, x0=None, tol=1e-10, maxit=10000, precond=True, history=False, norm=NORM_REL_L2):
@@ -258,7 +259,7 @@ def fermi_pointwise(valence, bath_molar, radii, phi, solvent=None, water_molar=5
 
 def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar, radii, l_c, tol,
              omega_pf=0.3, lin_tol=1e-10, lin_maxit=10000, max_outer=200, water_molar=55.5, norm=NORM_REL_L2,
-             fixed_override=None, fixed_nodes=None, solver=SOLVER_TABLE3, want_fields=True):
+             fixed_override=None, fixed_nodes=None, solver=SOLVER_TABLE3, want_fields=True, steric_mode=STERIC_SIMULTANEOUS):
     """The outer loop of Table 2 / Table 4 (R5).  want_fields=False skips the final evaluation of C_k and S^trc
     (out["conc"], out["steric"] are then None): at 512^3 it costs a minute and 4 GB that a truncated run does not need."""
     n = nx * ny * nz
@@ -285,7 +286,7 @@ def solve_pf(nx, ny, nz, h, bc_type, bc_value, eps, charges, valence, bath_molar
                             ctypes.c_double(lin_tol), int(lin_maxit), int(max_outer), int(norm),
                             _d(phi), _d(psi), _d(conc), _d(steric), ctypes.byref(outer), ctypes.byref(lin),
                             _i(lhist), int(cap), _d(ihist), _d(None if fixed_override is None else _f64(fixed_override)),
-                            _u8(fm), _d(fv), int(solver))
+                            _u8(fm), _d(fv), int(solver), int(steric_mode))
     return dict(phi=phi, psi=psi, conc=conc, steric=steric, status=st, outer_iters=outer.value,
                 linear_iters=lin.value, lin_iters_hist=lhist[: 2 * outer.value + 1].copy(),
                 incr_hist=ihist[: outer.value].copy())

@@ -287,3 +287,80 @@ def test_grid_refinement_second_order_full_pf(oracle):
     d1 = np.abs(sols[0] - sols[1][::2, ::2, ::2]).max()
     d2 = np.abs(sols[1] - sols[2][::2, ::2, ::2]).max()
     assert 3.0 < d1 / d2 < 5.5, (d1, d2)
+
+
+# ---- the lagged reading of Eq (11) (readings G1, G2) ------------------------------------------
+
+def _cfg0(n, charge_scale=1.0):
+    w = W.config0(n=n)
+    w.charges = w.charges.copy()
+    w.charges[:, 3] *= charge_scale
+    return w
+
+
+def _solve_cfg(oracle, w, mode, **kw):
+    sp = w.species
+    return oracle.solve_pf(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, w.charges, sp.valence, sp.bath_molar,
+                           sp.radii, w.l_c, 1e-8, steric_mode=mode, **kw)
+
+
+def test_lagged_steric_same_fixed_point_on_a_mild_workload(oracle):
+    """PAPER.md:118 carries one subscript 0 on C_k, S^trc and Gamma: read as assignments in the order written (S^trc
+    of the previous outer iteration), the loop has the fixed point of the simultaneous reading.  configs[0]'s geometry
+    with the charges scaled to 0.1 e: potentials of a few kT/e, where the lagged iteration converges."""
+    w = _cfg0(16, 0.2)
+    a = _solve_cfg(oracle, w, oracle.STERIC_SIMULTANEOUS, max_outer=400)
+    b = _solve_cfg(oracle, w, oracle.STERIC_LAGGED, max_outer=400)
+    assert a["status"] == 0 and b["status"] == 0
+    assert np.abs(a["phi"]).max() > 1.0 and np.abs(a["steric"]).max() > 1e-3
+    assert np.linalg.norm(a["phi"] - b["phi"]) <= 1e-7 * np.linalg.norm(a["phi"])
+    # (S^trc trails phi by one outer iteration and the loop stops on the increment of phi alone: its state, and the
+    # C_k that carry it with weights v_k/v_0 up to 2.2, are converged a little less far than phi)
+    for k in range(3):
+        assert np.linalg.norm(a["conc"][k] - b["conc"][k]) <= 1e-5 * np.linalg.norm(a["conc"][k])
+    assert np.abs(a["steric"] - b["steric"]).max() <= 1e-3 * np.abs(a["steric"]).max()
+    # phi = 0 => the bath: no charges, zero boundary data (PAPER.md:47)
+    w0 = _cfg0(16, 0.0)
+    z = _solve_cfg(oracle, w0, oracle.STERIC_LAGGED, max_outer=5)
+    assert z["status"] == 0 and np.all(z["phi"] == 0.0) and np.all(z["steric"] == 0.0)
+    solvent = oracle.solvent_mask(w0.eps).astype(bool)
+    cb = np.append(w0.species.bath_molar, 55.5) * MOLAR
+    assert np.allclose(z["conc"][:, solvent], cb[:, None], rtol=1e-15) and np.all(z["conc"][:, ~solvent] == 0.0)
+
+
+def test_lagged_steric_first_step_by_hand_and_floor(oracle):
+    """One outer iteration of the lagged loop, recomputed in numpy: C_k^0 with S = 0 at the initial guess, Gamma_0
+    from them, S for the next iteration = ln(max(Gamma_0, 1e-12)/Gamma^B) (reading G2: the floor is reached next to
+    the charges of configs[0], where sum v_k C_k^0 > 1)."""
+    w = _cfg0(16)
+    sp = w.species
+    out = _solve_cfg(oracle, w, oracle.STERIC_LAGGED, max_outer=1)
+    rhs = oracle.deposit_charges(w.nx, w.ny, w.nz, w.h, w.charges)
+    phi_init = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, rhs, tol=1e-10)["x"]
+    solvent = oracle.solvent_mask(w.eps).astype(bool)
+    z = np.append(sp.valence, 0.0)
+    cb = np.append(sp.bath_molar, 55.5) * MOLAR
+    vol = 4.0 * np.pi * np.asarray(sp.radii) ** 3 / 3.0
+    gamma_b = 1.0 - (vol * cb).sum()
+    C0 = cb[:, None] * np.exp(-z[:, None] * phi_init[None, :])
+    gam = 1.0 - (vol[:, None] * C0).sum(0)
+    S1 = np.where(solvent, np.log(np.maximum(gam, 1e-12) / gamma_b), 0.0)
+    assert (gam[solvent] <= 0).sum() > 0                               # the floor is exercised
+    assert np.allclose(out["steric"], S1, rtol=1e-9, atol=1e-12)
+    # the returned C_k belong to the state: Eq (1) at the returned phi with that S
+    lam = vol / vol.mean()
+    Cn = np.where(solvent, cb[:, None] * np.exp(-z[:, None] * out["phi"][None, :] + lam[:, None] * S1[None, :]), 0.0)
+    assert np.allclose(out["conc"], Cn, rtol=1e-9)
+
+
+def test_lagged_steric_cycles_where_the_simultaneous_reading_converges(oracle):
+    """The finding behind reading Q11: on configs[0] as BASELINE states it (charges of 0.5 e next to the solvent) the
+    lagged iteration falls into a two-cycle between the floor and an almost empty state -- the map S -> ln Gamma(S)
+    has a slope far below -1 in crowded nodes -- while the simultaneous reading converges.  Kept as a test so that the
+    choice of the default is a recorded measurement, not an assertion."""
+    w = _cfg0(16)
+    a = _solve_cfg(oracle, w, oracle.STERIC_SIMULTANEOUS, max_outer=400)
+    b = _solve_cfg(oracle, w, oracle.STERIC_LAGGED, max_outer=120)
+    assert a["status"] == 0 and a["outer_iters"] < 400
+    assert b["status"] == 1 and b["outer_iters"] == 120
+    assert b["incr_hist"][-1] > 1e3 * 1e-8 and b["incr_hist"][-10:].min() > 0.5 * b["incr_hist"][-10:].max()   # stalled
