@@ -124,6 +124,13 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
                                      solve of the grid, those inside pf_solve_pf included.  Direct and tiled kernel families
                                      (tiled: on-the-fly stencil); the cooperative kernel implements Table 3 only. */
 
+#define PF_OPT_STERIC_MODE    17  /* how pf_solve_pf reads the three mutually dependent definitions of Eq (11).
+                                     0 (default, reading Q11): solved simultaneously per node.  1 (readings G1, G2): as
+                                     assignments in the order written -- C_k from phi_0 and the S^trc of the previous outer
+                                     iteration (0 before the first), then Gamma_0, floored at 1e-12, gives the next S^trc.
+                                     Same fixed point; converges for potentials of a few kT/e and two-cycles on crowded
+                                     nodes (on configs[0] as stated), which is why it is not the default. */
+
 /* Create a grid: store geometry and boundary conditions, scan eps_map for its palette of distinct
  * values, keep a device copy of the charges.  Assembly itself runs in pf_grid_set_workspace.
  *   eps_map : device, nx*ny*nz doubles, relative permittivity per node; borrowed.

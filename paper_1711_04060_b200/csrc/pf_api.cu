@@ -146,6 +146,8 @@ struct pf_grid {
     // host-buffer flavour (pf_solve_linear_host, pf_grid_stage_host): device staging of rhs and x, their own vectors so
     // that an upload can run on the copy stream while other work of the grid (assembly, a PF solve) uses the scratch
     double *hb, *hx;
+    double* sstate;          // S^trc state of the lagged reading of Eq (11) (PF_OPT_STERIC_MODE = 1)
+    int opt_steric_mode;
     cudaStream_t copy_stream;
     cudaEvent_t staged_ev, main_ev;
     const void *staged_rhs, *staged_x;
@@ -206,7 +208,7 @@ int fail(pf_grid* g, int code, const char* fmt, ...) {
     } while (0)
 
 int n_vectors(bool stored, int charge_model, bool fixed_nodes, bool padx) {
-    return 22 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0) + (fixed_nodes ? 1 : 0) + (padx ? 3 + (stored ? 6 : 0) : 0);
+    return 23 + (stored ? 12 : 0) + (charge_model == 1 ? 3 : 0) + (fixed_nodes ? 1 : 0) + (padx ? 3 + (stored ? 6 : 0) : 0);
 }
 
 int code_mode_of(const pf_grid* g) { return g->pal.count > PF_MAX_PALETTE ? 0 : (g->pal.count <= 2 ? 1 : 2); }
@@ -678,6 +680,7 @@ int make_species(pf_grid* g, int K, const double* valence, const double* bath, c
     const double gammaB = 1.0 - occ;
     if (!(gammaB > 0.0)) return fail(g, PF_ERR_NONPHYSICAL, "Gamma^B = %g <= 0", gammaB);
     sp->ln_gammaB = std::log(gammaB);
+    sp->gammaB = gammaB;
     double net = 0.0, tot = 0.0;
     for (int k = 0; k < K; ++k) { net += sp->z[k] * sp->cb[k]; tot += std::fabs(sp->z[k]) * sp->cb[k]; }
     if (std::fabs(net) > 1e-12 * tot) return fail(g, PF_ERR_NONPHYSICAL, "bath is not neutral");
@@ -730,7 +733,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->opt_profile = 0; g->prof_ms[0] = g->prof_ms[1] = g->prof_ms[2] = 0.0;
     g->prof_launches[0] = g->prof_launches[1] = g->prof_launches[2] = 0;
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
-    g->hb = g->hx = nullptr; g->copy_stream = nullptr; g->staged_ev = g->main_ev = nullptr;
+    g->hb = g->hx = g->sstate = nullptr; g->opt_steric_mode = 0; g->copy_stream = nullptr; g->staged_ev = g->main_ev = nullptr;
     g->staged_rhs = g->staged_x = nullptr;
     g->capture_stream = nullptr; g->opt_graph = 3; g->opt_diag_code = 1; g->opt_norm = 0; g->opt_solver = 0;
     g->opt_charge_model = 0; g->charge_model = 0; g->phiL = g->phistar = g->A0_L = nullptr; g->code_L = nullptr;
@@ -875,6 +878,9 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
             g->opt_charge_model = iv; return PF_OK;
         case PF_OPT_DIAG_FROM_CODE:
             g->opt_diag_code = iv != 0; return PF_OK;
+        case PF_OPT_STERIC_MODE:
+            if (iv != 0 && iv != 1) return fail(g, PF_ERR_ARG, "steric mode must be 0 (simultaneous) or 1 (lagged)");
+            g->opt_steric_mode = iv; return PF_OK;
         case PF_OPT_SOLVER:
             if (iv != 0 && iv != 1) return fail(g, PF_ERR_ARG, "solver must be 0 (Table 3) or 1 (merged)");
             g->opt_solver = iv; return PF_OK;
@@ -912,7 +918,7 @@ int pf_grid_set_workspace(pf_grid* g, void* dev_ptr, size_t bytes) {
     char* base = (char*)dev_ptr;
     auto take = [&]() { double* p = (double*)base; base += vec; return p; };
     g->r = take(); g->r1 = take(); g->rt = take(); g->p0 = take(); g->p1 = take(); g->v0 = take(); g->v1 = take();
-    g->t = take(); g->y = take(); g->bw = take(); g->xw = take(); g->hb = take(); g->hx = take();
+    g->t = take(); g->y = take(); g->bw = take(); g->xw = take(); g->hb = take(); g->hx = take(); g->sstate = take();
     g->staged_rhs = g->staged_x = nullptr;
     g->A0 = take(); g->A0_pf1 = take(); g->A0_s = take(); g->fixed = take(); g->psi = take();
     g->phi0 = take(); g->phiw = take(); g->sigma = take(); g->bpf = take();
@@ -1093,6 +1099,8 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
     if (rc < 0) return rc;
     inner_maxit |= rc == PF_NOT_CONVERGED;
     PF_CUDA(g, cudaMemsetAsync(g->psi, 0, nbytes, g->stream));
+    const bool lagged = g->opt_steric_mode == 1;
+    if (lagged) PF_CUDA(g, cudaMemsetAsync(g->sstate, 0, nbytes, g->stream));       // S^trc = 0: the bath (G1)
     int status = PF_NOT_CONVERGED, outer = 0;
     double* phi0 = g->phi0;
     double* phiw = g->phiw;
@@ -1100,7 +1108,7 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
         ++outer;
         // row N1: concentrations, steric potential, PF1 right-hand side, PF2 diagonal -- one kernel
         launch_fermi(g->stream, g->g, g->bc, sp, g->eps, g->eps_mid, g->uniform, phi0, nullptr, g->sigma, nullptr,
-                     nullptr, g->bpf, g->A0, g->A0_s);
+                     nullptr, g->bpf, g->A0, g->A0_s, lagged ? g->sstate : nullptr, lagged);
         // row N2 (step 3): PF1 -> Psi, warm start from the previous Psi
         rc = bicgstab_device(g, make_op(g, 1), g->bpf, g->psi, g->opt_lin_tol, g->opt_lin_maxit, &its, nullptr, nullptr);
         g->lin_iters.push_back(its); total += its;
@@ -1128,9 +1136,9 @@ int pf_solve_pf(pf_grid* g, int nions, const double* valence, const double* bath
     }
     PF_CUDA(g, cudaMemcpyAsync(phi, phi0, nbytes, cudaMemcpyDeviceToDevice, g->stream));
     if (g->charge_model == 1) launch_recombine(g->stream, g->g.n, g->phistar, g->phiL, phi);   // Eq (5)
-    if (conc || steric)
+    if (conc || steric)       // (lagged: the fields that belong to the state -- C_k at the final phi with the S at hand)
         launch_fermi(g->stream, g->g, g->bc, sp, g->eps, g->eps_mid, g->uniform, phi0, nullptr, nullptr, steric, conc,
-                     nullptr, nullptr, nullptr);
+                     nullptr, nullptr, nullptr, lagged ? g->sstate : nullptr, false);
     PF_CUDA(g, cudaStreamSynchronize(g->stream));
     PF_CUDA(g, cudaGetLastError());
     if (outer_iters_out) *outer_iters_out = outer;

@@ -163,7 +163,7 @@ struct SpeciesDev {
     double lam[PF_MAX_SPECIES];         // v_k/v_0
     double lnvc[PF_MAX_SPECIES];        // ln(v_k C_k^B) (unused when v_k = 0)
     double vol[PF_MAX_SPECIES];
-    double ln_gammaB;
+    double ln_gammaB, gammaB;
     double kappa;
 };
 
@@ -174,7 +174,9 @@ void launch_diag_plus_sigma(cudaStream_t s, const GridDims& g, const BcDev& bc, 
                             double* a2);
 void launch_fermi(cudaStream_t s, const GridDims& g, const BcDev& bc, const SpeciesDev& sp, const double* eps, double eps_mid,
                   bool uniform, const double* phi, double* rho, double* sigma, double* S, double* conc,
-                  double* b1, const double* a0, double* a2);
+                  double* b1, const double* a0, double* a2,
+                  double* S_state = nullptr /* lagged reading (G1): S^trc at hand, N doubles; null = solve Eq (1) per node */,
+                  bool lag_update = false /* ... and replace it by ln(max(Gamma_0, 1e-12)/Gamma^B) of these C_k */);
 // Row N3 right-hand side: b = [solvent](-(eps psi) + sigma phi0) + fixed, Dirichlet values forced.
 void launch_rhs_pf2(cudaStream_t s, const GridDims& g, const BcDev& bc, const double* eps, double eps_mid,
                     bool uniform, const double* psi, const double* sigma, const double* phi0,

@@ -47,7 +47,7 @@ __global__ void __launch_bounds__(PW_THREADS)
 k_fermi(GridDims g, BcDev bc, SpeciesDev sp, const double* __restrict__ eps, double eps_mid, bool uniform,
         const double* __restrict__ phi, double* __restrict__ rho_o, double* __restrict__ sigma_o,
         double* __restrict__ S_o, double* __restrict__ conc, double* __restrict__ b1,
-        const double* __restrict__ a0, double* __restrict__ a2) {
+        const double* __restrict__ a0, double* __restrict__ a2, double* S_state, int lag_update) {
     const int K = sp.K;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += stride) {
@@ -59,7 +59,10 @@ k_fermi(GridDims g, BcDev bc, SpeciesDev sp, const double* __restrict__ eps, dou
         for (int k = 0; k < PF_MAX_SPECIES; ++k) c[k] = 0.0;
         if (solvent) {
             const double ph = phi[i];
-            if (sp.steric) {
+            // Lagged reading of Eq (11) (PF_OPT_STERIC_MODE = 1; readings G1, G2): S^trc is the state left by the previous
+            // outer iteration (0 before the first); no simultaneous solve
+            if (S_state) S = S_state[i];
+            if (sp.steric && !S_state) {
                 for (int itn = 0; itn < 50; ++itn) {
                     const double t0 = sp.ln_gammaB + S;
                     double tmax = t0;
@@ -93,6 +96,14 @@ k_fermi(GridDims g, BcDev bc, SpeciesDev sp, const double* __restrict__ eps, dou
                     if (k < K) { rho += sp.z[k] * ck; sig += sp.z[k] * sp.z[k] * ck; }
                 }
             sig = sp.kappa * sig;
+            if (S_state && lag_update && sp.steric) {
+                // Gamma_0 from the C_k^0 just formed, floored (G2), gives S^trc of the NEXT outer iteration
+                double occ = 0.0;
+#pragma unroll
+                for (int k = 0; k < PF_MAX_SPECIES; ++k)
+                    if (k <= K) occ += sp.vol[k] * c[k];
+                S_state[i] = log(fmax(1.0 - occ, 1e-12) / sp.gammaB);
+            }
         }
         if (rho_o) rho_o[i] = rho;
         if (sigma_o) sigma_o[i] = sig;
@@ -162,9 +173,10 @@ void launch_diag_plus_sigma(cudaStream_t s, const GridDims& g, const BcDev& bc, 
 
 void launch_fermi(cudaStream_t s, const GridDims& g, const BcDev& bc, const SpeciesDev& sp, const double* eps, double eps_mid,
                   bool uniform, const double* phi, double* rho, double* sigma, double* S, double* conc, double* b1,
-                  const double* a0, double* a2) {
+                  const double* a0, double* a2, double* S_state, bool lag_update) {
     ++g_launch_count;
-    k_fermi<<<pw_blocks(g.n), PW_THREADS, 0, s>>>(g, bc, sp, eps, eps_mid, uniform, phi, rho, sigma, S, conc, b1, a0, a2);
+    k_fermi<<<pw_blocks(g.n), PW_THREADS, 0, s>>>(g, bc, sp, eps, eps_mid, uniform, phi, rho, sigma, S, conc, b1, a0, a2,
+                                                  S_state, lag_update ? 1 : 0);
 }
 
 void launch_rhs_pf2(cudaStream_t s, const GridDims& g, const BcDev& bc, const double* eps, double eps_mid,

@@ -370,6 +370,31 @@ def test_pf_channel_neumann_small(pf, oracle):
         assert rel_l2(conc[k], ref["conc"][k]) <= 1e-7, k
 
 
+@pytest.mark.parametrize("kernels", [0, 2])
+def test_pf_lagged_steric_mode(pf, oracle, kernels):
+    """PF_OPT_STERIC_MODE = 1 (readings G1, G2): S^trc of the previous outer iteration.  (a) configs[0]'s
+    geometry at 32^3 with the charges scaled to 0.1 e, where the lagged loop converges: phi, C_k, S^trc against the
+    oracle's lagged loop; (b) three outer iterations at full strength, where Gamma_0 meets its floor next to the charges."""
+    sp = wl.NACL
+    for scale, max_outer, tol in ((0.2, 400, 1e-8), (1.0, 3, 1e-8)):
+        w = wl.config0()
+        w.charges = w.charges.copy()
+        w.charges[:, 3] *= scale
+        ref = oracle.solve_pf(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, w.charges, sp.valence, sp.bath_molar,
+                              sp.radii, w.l_c, tol, max_outer=max_outer, steric_mode=oracle.STERIC_LAGGED)
+        g = pf.Grid.from_workload(w, kernels=kernels, options={pf.PF_OPT_STERIC_MODE: 1, pf.PF_OPT_MAX_OUTER: max_outer})
+        out = g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, tol)
+        g.close()
+        assert out["status"] == ref["status"] == (0 if scale < 1 else 1) and out["outer_iters"] == ref["outer_iters"]
+        assert abs(out["linear_iters"] - ref["linear_iters"]) <= 0.02 * ref["linear_iters"]
+        assert rel_l2(out["phi"].cpu().numpy(), ref["phi"]) <= 1e-7
+        for k in range(3):
+            assert rel_l2(out["conc"][k].cpu().numpy(), ref["conc"][k]) <= 1e-7
+        assert rel_l2(out["steric"].cpu().numpy(), ref["steric"]) <= 1e-7
+        if scale == 1.0:
+            assert ref["steric"].min() < -20.0               # ln(1e-12 / Gamma^B): the floor
+
+
 def test_pf_errors(pf):
     w = wl.config0(n=16)
     g = pf.Grid.from_workload(w)
