@@ -2,6 +2,7 @@
 
     python report.py [--out gpurun_out/report.md] [--skip-512]
     python report.py --launch-ab [--out gpurun_out/launch_ab.md]     (PF_OPT_GRAPH 0 / 1 / 2 / 3)
+    python report.py --omega-sweep [--out gpurun_out/omega.md]       (omega_PF 0 .. 0.7 on configs[2]'s PF solve)
 
 Needs a CUDA device (the GPU columns) and builds the oracle for the CPU columns; the oracle is only ever
 run where it finishes in about a minute (full solves up to 64^3, a few iterations beyond).
@@ -35,10 +36,26 @@ def measured_peak():
         return 6650.0
 
 
-def bytes_per_iter(stored: bool) -> int:
+def bytes_per_iter(stored: bool, merged: bool = False) -> int:
     # Poisson solves (all linear rows of the table): the on-the-fly k1 takes the diagonal from the stencil code
-    # (50 + 34 + 64 B); PF1 / PF2 solves move 156 B
-    return 248 if stored else 148
+    # (50 + 34 + 64 B); PF1 / PF2 solves move 156 B; merged solver: K2M 42 + K31 82 B
+    return 248 if stored else (124 if merged else 148)
+
+
+def ncu_dram_bytes_per_iter(stencil_name: str, n: int, merged: bool):
+    """Sum over the kernels of one iteration of the DRAM bytes per launch that the committed ncu --set full capture
+    measured (profiles/traffic.csv); None where no capture exists for this stencil and size."""
+    want = ("k2m", "k31") if merged else ("k1", "k2", "k3")
+    got = {}
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for row in f:
+                c = [x.strip() for x in row.split(",")]
+                if len(c) >= 4 and c[0] == stencil_name and c[1] == str(n) and c[2] in want:
+                    got[c[2]] = int(c[3])
+    except (OSError, ValueError):
+        return None
+    return sum(got.values()) if len(got) == len(want) else None
 
 
 def rel_l2(a, b):
@@ -46,9 +63,9 @@ def rel_l2(a, b):
     return float(np.linalg.norm(a - b) / (d if d > 0 else 1.0))
 
 
-def gpu_fixed_iterations(w, rhs, stencil, iters):
+def gpu_fixed_iterations(w, rhs, stencil, iters, solver=0):
     """ms per iteration of `iters` fixed iterations (second of two runs), whole-solve CUDA-event time."""
-    g = pf.Grid.from_workload(w, stencil=stencil)
+    g = pf.Grid.from_workload(w, stencil=stencil, options={pf.PF_OPT_SOLVER: solver})
     x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
     rhs_d = torch.as_tensor(rhs, dtype=torch.float64).cuda()
     ms = None
@@ -67,30 +84,37 @@ def gpu_fixed_iterations(w, rhs, stencil, iters):
 
 def linear_rows(name, w, rhs, oracle, oracle_full: bool, oracle_iters: int, peak):
     rows = []
-    ref = None
+    ref_t = None
     o_s_per_it = None
     if oracle_full:
         t0 = time.perf_counter()
-        ref = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, rhs, tol=1e-10)
-        o_s_per_it = (time.perf_counter() - t0) / max(ref["iters"], 1)
+        ref_t = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, rhs, tol=1e-10)
+        o_s_per_it = (time.perf_counter() - t0) / max(ref_t["iters"], 1)
     elif oracle_iters:
         t0 = time.perf_counter()
         oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, rhs, tol=0.0, maxit=oracle_iters)
         o_s_per_it = (time.perf_counter() - t0) / oracle_iters
-    for stencil, sname in ((pf.STENCIL_STORED, "stored"), (pf.STENCIL_ONTHEFLY, "on-the-fly")):
-        g = pf.Grid.from_workload(w, stencil=stencil)
+    ref_m = None
+    if oracle_full:
+        ref_m = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, rhs, tol=1e-10,
+                                    solver=oracle.SOLVER_MERGED)
+    for stencil, solver, sname in ((pf.STENCIL_STORED, 0, "stored"), (pf.STENCIL_ONTHEFLY, 0, "on-the-fly"),
+                                   (pf.STENCIL_ONTHEFLY, 1, "on-the-fly, merged solver")):
+        g = pf.Grid.from_workload(w, stencil=stencil, options={pf.PF_OPT_SOLVER: solver})
         out = g.solve_linear(rhs, tol=1e-10)
         x = out["x"].cpu().numpy()
         g.close()
-        ms = gpu_fixed_iterations(w, rhs, stencil, 200 if w.n >= 128 ** 3 else 400)
-        bpi = bytes_per_iter(stencil == pf.STENCIL_STORED)
+        ms = gpu_fixed_iterations(w, rhs, stencil, 200 if w.n >= 128 ** 3 else 400, solver)
+        bpi = bytes_per_iter(stencil == pf.STENCIL_STORED, solver == 1)
         gbs = bpi * w.n / (ms * 1e-3) / 1e9
+        nb = ncu_dram_bytes_per_iter("stored" if stencil == pf.STENCIL_STORED else "onthefly", w.nx, solver == 1)
+        ref = ref_m if solver == 1 else ref_t
         rows.append(dict(config=name, N=w.n, variant=sname,
                          iters=f"{out['iters']} / {ref['iters'] if ref else 'n/a'}",
                          relres=f"{out['true_relres']:.2e}",
                          diff=f"{rel_l2(x, ref['x']):.1e}" if ref else "n/a",
                          ms=f"{ms:.4f}", its=f"{1e3 / ms:.0f}", mup=f"{w.n / ms / 1e3:.0f}", bpi=bpi,
-                         gbs=f"{gbs:.0f}", p8=f"{100 * gbs / PEAK_NOMINAL:.0f} %", pm=f"{100 * gbs / peak:.0f} %",
+                         gbs=f"{gbs:.0f}", ncu=f"{nb / (ms * 1e-3) / 1e9:.0f}" if nb else "n/a", p8=f"{100 * gbs / PEAK_NOMINAL:.0f} %", pm=f"{100 * gbs / peak:.0f} %",
                          osit=f"{o_s_per_it:.3f}" if o_s_per_it else "n/a", outer="-", pft="-"))
     return rows
 
@@ -115,7 +139,7 @@ def pf_row(name, w, oracle, oracle_full: bool):
         oiters = f"{ref['outer_iters']} ({ref['linear_iters']} lin.)"
     return dict(config=name, N=w.n, variant="PF (auto)", iters=f"{out['linear_iters']} lin. / {oiters}",
                 relres="-", diff=diff, ms=f"{1e3 * tg / max(out['linear_iters'], 1):.4f}", its="-", mup="-", bpi="-",
-                gbs="-", p8="-", pm="-", osit="-", outer=str(out["outer_iters"]),
+                gbs="-", ncu="-", p8="-", pm="-", osit="-", outer=str(out["outer_iters"]),
                 pft=f"{tg:.2f} s / {to:.0f} s" if to else f"{tg:.2f} s / n/a")
 
 
@@ -170,17 +194,53 @@ def launch_mode_ab(out_path):
     print(text)
 
 
+def omega_sweep(out_path):
+    """omega_PF of Table 2 step 5 (PAPER.md:219 uses 0.3) on configs[2] (128^3, +50 mV): outer and linear iterations
+    and wall time of the full nonlinear solve to BASELINE's tolerances, Table 3 and merged solver, plus the agreement
+    of the converged potentials with the omega_PF = 0.3 result (the fixed point does not depend on the relaxation)."""
+    w = wl.config2(volt_mv=50.0)
+    sp = w.species
+    lines = ["| omega_PF | solver | status | outer iterations | linear iterations | seconds | rel. L2 diff of phi vs omega_PF = 0.3 |",
+             "|---:|---|---:|---:|---:|---:|---:|"]
+    ref = {}
+    for om in (0.3, 0.0, 0.1, 0.2, 0.4, 0.5, 0.6, 0.7):
+        for solver, sname in ((0, "Table 3"), (1, "merged")):
+            g = pf.Grid.from_workload(w, options={pf.PF_OPT_OMEGA_PF: om, pf.PF_OPT_SOLVER: solver, pf.PF_OPT_MAX_OUTER: 3000})
+            g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol, want_conc=False)   # warm-up
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            out = g.solve_pf(sp.valence, sp.bath_molar, sp.radii, w.l_c, w.nonlinear_tol, want_conc=False)
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            g.close()
+            phi = out["phi"].cpu().numpy()
+            if om == 0.3:
+                ref[solver] = phi
+            lines.append(f"| {om:.1f} | {sname} | {out['status']} | {out['outer_iters']} | {out['linear_iters']} | {dt:.2f} | "
+                         f"{rel_l2(phi, ref[solver]):.1e} |")
+    lines[2:] = sorted(lines[2:], key=lambda l: (float(l.split('|')[1]), l.split('|')[2]))
+    text = "\n".join(lines) + "\n"
+    os.makedirs(os.path.dirname(out_path), exist_ok=True)
+    with open(out_path, "w") as f:
+        f.write(text)
+    print(text)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "report.md"))
     ap.add_argument("--skip-512", action="store_true")
     ap.add_argument("--launch-ab", action="store_true", help="only the A/B table of the launch modes (PF_OPT_GRAPH)")
+    ap.add_argument("--omega-sweep", action="store_true", help="only the omega_PF sweep of configs[2]'s PF solve")
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise RuntimeError("report needs a CUDA device")
     pf.load()
     if args.launch_ab:
         launch_mode_ab(args.out)
+        return
+    if args.omega_sweep:
+        omega_sweep(args.out)
         return
     from oracle import pf_oracle as oracle
     oracle.build()
@@ -202,9 +262,10 @@ def main():
         w = wl.config4()
         rows += linear_rows("4 (512^3 spheres)", w, w.rhs, oracle, False, 0, peak)
     hdr = ["config", "N", "variant", "iters to 1e-10 (GPU / oracle)", "true rel. residual", "rel. L2 diff vs oracle",
-           "ms/iter", "iterations/s", "Mupdates/s", "model B/unknown/iter", "effective GB/s (model)", "% of 8.0 TB/s",
+           "ms/iter", "iterations/s", "Mupdates/s", "model B/unknown/iter", "effective GB/s (model)",
+           "ncu DRAM GB/s (bytes of the committed capture / this time)", "% of 8.0 TB/s",
            f"% of {peak / 1e3:.2f} TB/s", "oracle s/iter (1 core)", "PF outer iters", "PF total time GPU / oracle"]
-    keys = ["config", "N", "variant", "iters", "relres", "diff", "ms", "its", "mup", "bpi", "gbs", "p8", "pm", "osit",
+    keys = ["config", "N", "variant", "iters", "relres", "diff", "ms", "its", "mup", "bpi", "gbs", "ncu", "p8", "pm", "osit",
             "outer", "pft"]
     lines = ["| " + " | ".join(hdr) + " |", "|" + "---|" * len(hdr)]
     for r in rows:
