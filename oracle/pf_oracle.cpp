@@ -31,8 +31,12 @@
 //   outer loop    : l_c=0 + steric off => nonlinear PB (Gouy-Chapman closed form in 1-D);
 //                   independence of omega_PF; fixed-point residuals of PF1/PF2 at convergence
 //                   l_c > 0 coupling: closed form of the discrete split system for a sine-mode source
-//   full PF with l_c>0, steric term and strong nonlinearity together, 3-D: PARITY UNPINNED as a whole
-//                   (each ingredient is pinned above).
+//   full PF with l_c>0, steric term (unequal radii) and strong nonlinearity together, 3-D: a manufactured discrete
+//                   solution (independent Fermi root finder + sine-transform PF1 solve in numpy) that the outer loop
+//                   must converge to, and second-order grid refinement (tests/test_oracle_pf.py)
+//   merged BiCGSTAB (reading M1): dense LU, numpy transcription, the identity rho_i = r~.r_i, agreement with Table 3
+//                   (tests/test_oracle_merged.py);  lagged reading of Eq (11) (G1, G2): same fixed point, first step
+//                   by hand, the two-cycle on configs[0];  non-finite data (D7): breakdown, not success
 //   singular charges (Eqs 5-10): Coulomb sums vs numpy; 1-D closed form with a prescribed flux jump (c0, d0 of
 //                   Eqs 17-18); discrete Gauss law sum b^IF h^3 = kappa sum q; harmonic phi^L; Born ion;
 //                   agreement with the independent deposition model in the solvent (tests/test_oracle_singular.py)

@@ -15,7 +15,8 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libpf_b200.so")
+# PF_B200_LIB: another build of the same sources (e.g. the -DPF_EXPERIMENT_PLAIN_DOT measurement of profiles/r2_plain_dot.md)
+LIB_PATH = os.environ.get("PF_B200_LIB") or os.path.join(_HERE, "libpf_b200.so")
 
 PF_OK, PF_NOT_CONVERGED, PF_INNER_NOT_CONVERGED = 0, 1, 2
 PF_ERR_ARG, PF_ERR_CUDA, PF_ERR_BREAKDOWN, PF_ERR_NONPHYSICAL, PF_ERR_WORKSPACE = -1, -2, -3, -4, -5

@@ -194,6 +194,35 @@ def launch_mode_ab(out_path):
     print(text)
 
 
+def iteration_counts(out_path):
+    """Iterations to 1e-10 of the linear solve of configs 0-3, direct and tiled kernels, Table 3 and merged solver, beside
+    the oracle's (run where it finishes in a minute): the evidence behind the rounding contract of DESIGN.md section 4.
+    Run once with the product library and once with a -DPF_EXPERIMENT_PLAIN_DOT build (PF_B200_LIB)."""
+    from oracle import pf_oracle as oracle
+    oracle.build()
+    lines = [f"library: {pf.LIB_PATH}", "",
+             "| config | solver | kernels | iterations GPU | iterations oracle | true rel. residual | rel. L2 diff vs oracle |",
+             "|---|---|---|---:|---:|---:|---:|"]
+    for name, w in (("0 (32^3)", wl.config0()), ("1 (64^3)", wl.config1()), ("2 (128^3)", wl.config2(volt_mv=50.0)),
+                    ("3 (256^3)", wl.config3())):
+        rhs = w.rhs if w.rhs is not None else oracle.deposit_charges(w.nx, w.ny, w.nz, w.h, w.charges)
+        for solver, sname in ((0, "Table 3"), (1, "merged")):
+            ref = None
+            if w.n <= 64 ** 3:
+                ref = oracle.solve_linear(w.nx, w.ny, w.nz, w.h, w.bc_type, w.bc_value, w.eps, rhs, tol=1e-10, solver=solver)
+            for kern, kname in ((1, "direct"), (2, "tiled")):
+                g = pf.Grid.from_workload(w, stencil=pf.STENCIL_ONTHEFLY, kernels=kern, options={pf.PF_OPT_SOLVER: solver})
+                out = g.solve_linear(rhs, tol=1e-10)
+                g.close()
+                lines.append(f"| {name} | {sname} | {kname} | {out['iters']} | {ref['iters'] if ref else 'n/a'} | "
+                             f"{out['true_relres']:.2e} | " + (f"{rel_l2(out['x'].cpu().numpy(), ref['x']):.1e}" if ref else "n/a") + " |")
+    text = "\n".join(lines) + "\n"
+    os.makedirs(os.path.dirname(out_path), exist_ok=True)
+    with open(out_path, "w") as f:
+        f.write(text)
+    print(text)
+
+
 def omega_sweep(out_path):
     """omega_PF of Table 2 step 5 (PAPER.md:219 uses 0.3) on configs[2] (128^3, +50 mV): outer and linear iterations
     and wall time of the full nonlinear solve to BASELINE's tolerances, Table 3 and merged solver, plus the agreement
@@ -232,6 +261,8 @@ def main():
     ap.add_argument("--skip-512", action="store_true")
     ap.add_argument("--launch-ab", action="store_true", help="only the A/B table of the launch modes (PF_OPT_GRAPH)")
     ap.add_argument("--omega-sweep", action="store_true", help="only the omega_PF sweep of configs[2]'s PF solve")
+    ap.add_argument("--iteration-counts", action="store_true",
+                    help="only the iterations-to-tolerance table of configs 0-3 (both kernel families and solvers)")
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise RuntimeError("report needs a CUDA device")
@@ -241,6 +272,9 @@ def main():
         return
     if args.omega_sweep:
         omega_sweep(args.out)
+        return
+    if args.iteration_counts:
+        iteration_counts(args.out)
         return
     from oracle import pf_oracle as oracle
     oracle.build()

@@ -4,7 +4,8 @@ Table 2 steps 2-5 / Table 4 steps 4-7.  Pins: the PF
  against the Gouy-Chapman closed form with O(h^2) convergence, Psi = Laplacian(phi)
  evaluated with numpy, independence of the converged field from omega_PF, the
 discrete PF1/PF2 equations re-evaluated in numpy at the fixed point, and the relaxation formula.
-Full 3-D PF with l_c > 0 and unequal radii has no closed form: PARITY UNPINNED beyond these.
+Full 3-D PF with l_c > 0, unequal radii and strong nonlinearity has no closed form; it is pinned by a manufactured
+discrete solution and by second-order grid refinement (second half of this file).
 """
 import numpy as np
 import pytest
