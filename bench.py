@@ -238,6 +238,10 @@ def run_b200(args):
     x_host = torch.zeros(n, dtype=torch.float64).pin_memory()
     phi_host = torch.zeros(n, dtype=torch.float64).pin_memory()
     eps_dev = eps_host.cuda()
+    # e2e: the eps map of the NEXT step is uploaded into the other of two device buffers while the current step's linear
+    # solve runs (every step still uploads its own inputs inside the timed region; only the first upload is exposed)
+    eps_bufs = [torch.empty_like(eps_dev), torch.empty_like(eps_dev)]
+    eps_state = {"cur": 0, "ready": None}
     rhs_dev = rhs_host.cuda()
     x_dev = torch.zeros(n, dtype=torch.float64, device="cuda")
     phi_dev = torch.zeros(n, dtype=torch.float64, device="cuda")
@@ -259,9 +263,14 @@ def run_b200(args):
     def step(host_buffers: bool, profile: bool, cfg: dict = None):
         cfg = cfg or main_cfg
         ws, prof_tot = cfg["ws"], cfg["prof"]
+        eps_in = eps_dev
         if host_buffers:
-            eps_dev.copy_(eps_host, non_blocking=True)
-        h = pf.pf_grid_create(w.nx, w.ny, w.nz, w.h, eps_dev, w.charges, w.bc_type, w.bc_value)
+            eps_in = eps_bufs[eps_state["cur"]]
+            if eps_state["ready"] is None:
+                eps_in.copy_(eps_host, non_blocking=True)              # no step before this one: upload in line
+            else:
+                torch.cuda.current_stream().wait_event(eps_state["ready"])
+        h = pf.pf_grid_create(w.nx, w.ny, w.nz, w.h, eps_in, w.charges, w.bc_type, w.bc_value)
         pf.pf_grid_set_option(h, pf.PF_OPT_STENCIL, cfg["stencil"])
         if kernels:
             pf.pf_grid_set_option(h, pf.PF_OPT_KERNELS, kernels)
@@ -285,6 +294,11 @@ def run_b200(args):
         if profile:      # the events bracket iterations of the long linear solve only (the PF pass runs unprofiled)
             pf.pf_grid_set_option(h, pf.PF_OPT_PROFILE, PROFILE_ITERS)
         if host_buffers:
+            with torch.cuda.stream(side):                               # the next step's eps, behind the phi download
+                eps_bufs[eps_state["cur"] ^ 1].copy_(eps_host, non_blocking=True)
+                eps_state["ready"] = torch.cuda.Event()
+                eps_state["ready"].record(side)
+            eps_state["cur"] ^= 1
             out = pf.pf_solve_linear_host(h, n, rhs_host, x_host, 0.0, lin_iters, true_residual=False)
         else:
             x_dev.zero_()
@@ -346,7 +360,8 @@ def run_b200(args):
                "h2d_bytes_per_step": 8 * n * 3, "d2h_bytes_per_step": 8 * n * 2,
                "ms_per_step": ms_e2e / e2e_steps,
                "what": "eps, rhs, x0 host->device; x, phi device->host; C-ABI pf_grid_stage_host + pf_solve_linear_host: the "
-                       "rhs/x0 upload overlaps the PF pass, the phi download the linear solve; eps up and x down are exposed"}
+                       "rhs/x0 upload overlaps the PF pass, the phi download and the next step's eps upload the linear solve; "
+                       "the x download is exposed"}
 
     if rank == 0:
         peak, peak_src = measured_peak_gbs()
