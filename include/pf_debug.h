@@ -22,6 +22,11 @@ int pf_grid_profile(pf_grid *g, double *ms_out, long long *launches_out);
 /* Kernel launches issued by the library in this process so far. */
 long long pf_launch_count(void);
 
+/* Row N5 alone through the kernel and the per-grid scratch that pf_solve_pf uses (Table 2 step 5):
+ * phi := omega_pf phi0 + (1 - omega_pf) phi over the grid's N nodes; *incr_out (host) = ||phi - phi0||_inf.
+ * phi0, phi: device, N doubles.  The reference the no-allocation entry point (pf_noalloc.h) is tested against. */
+int pf_grid_relax(pf_grid *g, double omega_pf, const double *phi0, double *phi, double *incr_out);
+
 /* BiCGSTAB iterations of the Laplace solve for phi^L (charge model 1). */
 int pf_grid_laplace_iters(const pf_grid *g);
 

@@ -15,6 +15,8 @@
 
 using namespace pf;
 
+namespace pf { void set_create_error(const char* msg); }
+
 long long pf::g_launch_count = 0;
 thread_local cudaError_t pf::g_launch_error = cudaSuccess;
 
@@ -689,6 +691,9 @@ int make_species(pf_grid* g, int K, const double* valence, const double* bath, c
 
 }  // namespace
 
+// the message pf_last_error(NULL) returns, for entry points that take no grid (pf_noalloc.cu)
+void pf::set_create_error(const char* msg) { g_create_error = msg ? msg : ""; }
+
 // =========================================================================================
 // C ABI
 // =========================================================================================
@@ -1192,6 +1197,16 @@ int pf_grid_set_fixed_nodes(pf_grid* g, const long long* idx_host, const double*
     }
     g->fix_idx.assign(idx_host, idx_host + count);
     g->fix_val.assign(val_host, val_host + count);
+    return PF_OK;
+}
+
+int pf_grid_relax(pf_grid* g, double omega_pf, const double* phi0, double* phi, double* incr_out) {
+    if (!g || !phi0 || !phi || !incr_out) return PF_ERR_ARG;
+    launch_relax(g->stream, g->g.n, omega_pf, phi0, phi, g->dmax_bits);      // the kernel and scratch pf_solve_pf uses
+    unsigned long long bits = 0;
+    PF_CUDA(g, cudaMemcpyAsync(&bits, g->dmax_bits, sizeof(bits), cudaMemcpyDeviceToHost, g->stream));
+    PF_CUDA(g, cudaStreamSynchronize(g->stream));
+    std::memcpy(incr_out, &bits, sizeof(double));
     return PF_OK;
 }
 

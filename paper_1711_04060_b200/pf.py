@@ -35,7 +35,7 @@ EXPORTS = [
     "pf_grid_create", "pf_grid_set_fixed_nodes", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
     "pf_solve_linear", "pf_solve_linear_host", "pf_grid_stage_host", "pf_solve_pf", "pf_fermi_pointwise", "pf_grid_history",
     "pf_grid_linear_iters", "pf_grid_increments", "pf_grid_fault_repeats", "pf_grid_laplace_iters", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_code_layout", "pf_grid_copy_array",
-    "pf_grid_profile", "pf_launch_count", "pf_coop_plan", "pf_grid_destroy", "pf_last_error", "pf_version",
+    "pf_grid_profile", "pf_launch_count", "pf_coop_plan", "pf_grid_relax", "pf_relax_noalloc", "pf_grid_destroy", "pf_last_error", "pf_version",
 ]
 
 
@@ -84,6 +84,8 @@ def load():
     L.pf_grid_linear_iters.argtypes = [_vp, _ip, ctypes.c_int]
     L.pf_grid_increments.argtypes = [_vp, _dp, ctypes.c_int]
     L.pf_grid_fault_repeats.argtypes = [_vp]
+    L.pf_grid_relax.argtypes = [_vp, ctypes.c_double, _vp, _vp, _dp]
+    L.pf_relax_noalloc.argtypes = [ctypes.c_longlong, ctypes.c_double, _vp, _vp, _vp, _vp]
     L.pf_grid_laplace_iters.argtypes = [_vp]
     L.pf_grid_stencil.argtypes = [_vp]
     L.pf_grid_palette_size.argtypes = [_vp]
@@ -260,6 +262,23 @@ def pf_coop_plan(nx: int, ny: int, nz: int, max_blocks: int = 148, smem_cap: int
 
 def pf_grid_laplace_iters(handle) -> int:
     return load().pf_grid_laplace_iters(handle)
+
+
+def pf_grid_relax(handle, n: int, omega_pf: float, phi0: torch.Tensor, phi: torch.Tensor) -> float:
+    """Row N5 through pf_solve_pf's own kernel and scratch; phi is relaxed in place, the increment is returned."""
+    d = ctypes.c_double(0)
+    _check(handle, load().pf_grid_relax(handle, float(omega_pf), _dev_ptr(phi0, n), _dev_ptr(phi, n), ctypes.byref(d)))
+    return d.value
+
+
+def pf_relax_noalloc(n: int, omega_pf: float, phi0: Optional[torch.Tensor], phi: Optional[torch.Tensor],
+                     incr_out: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> None:
+    """The no-allocation entry point (include/pf_noalloc.h): needs no grid; phi is relaxed in place and the increment
+    written to the 1-element CUDA tensor incr_out; only enqueues work on the stream."""
+    s = (stream or torch.cuda.current_stream()).cuda_stream
+    rc = load().pf_relax_noalloc(int(n), float(omega_pf), None if phi0 is None else phi0.data_ptr(),
+                                 None if phi is None else phi.data_ptr(), _dev_ptr(incr_out, 1), _vp(s))
+    _check(None, rc)
 
 
 def pf_grid_fault_repeats(handle) -> int:

@@ -81,3 +81,15 @@ def test_product_package_never_touches_the_oracle():
             text = open(os.path.join(ROOT, "oracle", f), encoding="utf-8").read()
             assert "import paper_1711_04060_b200" not in text and "from paper_1711_04060_b200" not in text
             assert "csrc/" not in text.replace("(paper_1711_04060_b200/csrc)", "")
+
+
+def test_no_alloc_entry_point_source_allocates_nothing():
+    """include/pf_noalloc.h promises an entry point without cudaMalloc / cudaFree or allocating library calls, with its
+    scratch in a file-scope __device__ array whose device address comes from cudaGetSymbolAddress."""
+    src = open(os.path.join(ROOT, "paper_1711_04060_b200", "csrc", "pf_noalloc.cu")).read()
+    code = "\n".join(line.split("//")[0] for line in src.splitlines())
+    for banned in ("cudaMalloc", "cudaFree", "cudaHostAlloc", "cudaMallocAsync", "new ", "std::vector", "malloc("):
+        assert banned not in code, banned
+    assert re.search(r"static\s+__device__\s+__align__\(256\)", code) and "cudaGetSymbolAddress" in code
+    hdr = open(os.path.join(ROOT, "include", "pf_noalloc.h")).read()
+    assert "PF_NOALLOC_MAX_N" in hdr and "race" in hdr
