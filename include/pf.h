@@ -131,6 +131,11 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
                                      Same fixed point; converges for potentials of a few kT/e and two-cycles on crowded
                                      nodes (on configs[0] as stated), which is why it is not the default. */
 
+#define PF_OPT_TILE_ROWS      18  /* tiled kernels: rows of a tile = main warps of a block.  0 (default): chosen per kernel
+                                     and grid size (16 rows / 19 warps / 96 registers, or 13 rows / 16 warps / 128
+                                     registers); 13 or 16 force one geometry.  Same bits either way; a tuning and
+                                     measurement knob. */
+
 /* Create a grid: store geometry and boundary conditions, scan eps_map for its palette of distinct
  * values, keep a device copy of the charges.  Assembly itself runs in pf_grid_set_workspace.
  *   eps_map : device, nx*ny*nz doubles, relative permittivity per node; borrowed.

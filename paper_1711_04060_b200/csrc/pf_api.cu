@@ -176,6 +176,7 @@ struct pf_grid {
     int opt_diag_code;       // k1 forms the Poisson diagonal from the stencil codes (PF_OPT_DIAG_FROM_CODE)
     int opt_norm;            // 0: relative 2-norm (Q3), 1: the paper's absolute maximum norm
     int opt_solver;          // 0: Table 3 (three kernels per iteration), 1: merged recurrence (two; reading M1)
+    int opt_tile_rows;       // tiled kernels: 0 auto, 13 or 16 forced
     int opt_charge_model;    // 0: trilinear deposition (Q22), 1: singular-charge decomposition (Eqs 5-10)
     int charge_model;        // the model the workspace was laid out and assembled for
     double *phiL, *phistar, *A0_L;
@@ -272,7 +273,7 @@ Operator make_op(const pf_grid* g, int which /*0 poisson, 1 pf1, 2 poisson+sigma
 LaunchCtx make_ctx(const pf_grid* g) {
     LaunchCtx c;
     c.stream = g->stream; c.g = g->g; c.sc[0] = g->sc[0]; c.sc[1] = g->sc[1]; c.flip = const_cast<int*>(&g->flip);
-    c.rb = g->rb; c.sm_count = g->sm_count; c.device = g->device; c.pdl = true; c.solver = g->opt_solver;
+    c.rb = g->rb; c.sm_count = g->sm_count; c.device = g->device; c.pdl = true; c.solver = g->opt_solver; c.tile_rows = g->opt_tile_rows;
     return c;
 }
 
@@ -740,7 +741,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
     g->hb = g->hx = g->sstate = nullptr; g->opt_steric_mode = 0; g->copy_stream = nullptr; g->staged_ev = g->main_ev = nullptr;
     g->staged_rhs = g->staged_x = nullptr;
-    g->capture_stream = nullptr; g->opt_graph = 3; g->opt_diag_code = 1; g->opt_norm = 0; g->opt_solver = 0;
+    g->capture_stream = nullptr; g->opt_graph = 3; g->opt_diag_code = 1; g->opt_norm = 0; g->opt_solver = 0; g->opt_tile_rows = 0;
     g->opt_charge_model = 0; g->charge_model = 0; g->phiL = g->phistar = g->A0_L = nullptr; g->code_L = nullptr;
     g->ctab_L = nullptr; g->laplace_iters = 0; g->fixv = nullptr; g->bc.fixv = nullptr;
     g->small = nullptr;
@@ -883,6 +884,14 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
             g->opt_charge_model = iv; return PF_OK;
         case PF_OPT_DIAG_FROM_CODE:
             g->opt_diag_code = iv != 0; return PF_OK;
+        case PF_OPT_TILE_ROWS:
+            if (iv != 0 && iv != 13 && iv != 16) return fail(g, PF_ERR_ARG, "tile rows must be 0 (auto), 13 or 16");
+            if (iv != g->opt_tile_rows) {          // cached graphs hold kernels of the other geometry
+                cudaStreamSynchronize(g->stream);
+                for (auto& cg : g->graphs) cudaGraphExecDestroy(cg.exec);
+                g->graphs.clear();
+            }
+            g->opt_tile_rows = iv; return PF_OK;
         case PF_OPT_STERIC_MODE:
             if (iv != 0 && iv != 1) return fail(g, PF_ERR_ARG, "steric mode must be 0 (simultaneous) or 1 (lagged)");
             g->opt_steric_mode = iv; return PF_OK;

@@ -47,16 +47,26 @@ namespace pf {
 namespace {
 
 constexpr int TX = 64;                   // tile width in nodes (32 lanes x 2)
-constexpr int TY = 16;                   // tile height = main warps per block
-constexpr int NW_CONSUMER = TY + 2;      // 16 main warps (one tile row each) + 2 halo warps
-constexpr int NT_CONSUMER = 32 * NW_CONSUMER;
-constexpr int NT = NT_CONSUMER + 32;     // + the producer warp
 constexpr int BX = TX + 4;               // box: two halo columns each side (one used; two keep 16-byte alignment)
-constexpr int BY = TY + 2;
-constexpr int FIELD_BYTES = ((BX * BY * 8 + 127) / 128) * 128;   // 9856
-constexpr int OWN_BYTES = TX * TY * 8;                            // 8192
 constexpr int NU = 3;                    // shared buffers of u (planes k, k+1 live, k+2 being written)
-static_assert(TY <= 32, "one halo column node per lane of a halo warp");
+
+// Tile height = main warps per block.  Two geometries are compiled:
+//   16 rows: 16 main + 2 halo + 1 producer = 19 warps; five warps share an SM quarter, which caps a thread at 96 registers;
+//   13 rows: 13 + 2 + 1 = 16 warps, four per quarter, 128 registers: no spills and room to overlap the long dependent
+//            chains of a plane (K31 of the merged solver, and every kernel on grids where fixed costs dominate).
+// tile_rows() below picks per kernel and grid; the arithmetic does not depend on the tiling.
+template <int TYV>
+struct Geo {
+    static constexpr int TY = TYV;
+    static constexpr int NW_CONSUMER = TY + 2;
+    static constexpr int NT_CONSUMER = 32 * NW_CONSUMER;
+    static constexpr int NT = NT_CONSUMER + 32;     // + the producer warp
+    static constexpr int BY = TY + 2;
+    static constexpr int FIELD_BYTES = ((BX * BY * 8 + 127) / 128) * 128;   // 9856 (16 rows), 8192 (13 rows)
+    static constexpr int OWN_BYTES = TX * TY * 8;                            // 8192, 6656
+    static_assert(TY <= 16, "one halo column node per lane of a halo warp (lanes 0..15 left, 16..31 unused)");
+};
+constexpr int TY_WIDE = 16, TY_DEEP = 13;
 
 enum { MODE_R0 = 0, MODE_R1 = 1, MODE_K1 = 2, MODE_K2 = 3, MODE_K1D = 4, MODE_K2M = 5, MODE_K31 = 6, MODE_K31D = 7 };
 // MODE_K1D: k1 for operators whose diagonal is the sum of their face coefficients (Poisson without sigma): A0 is
@@ -83,9 +93,11 @@ struct TmaArgs {
     CUtensorMap code;
 };
 
-template <int MODE, bool STORED, bool CODE32>
+template <int MODE, bool STORED, bool CODE32, int TYV>
 struct Layout {
     using T = ModeTraits<MODE>;
+    static constexpr int TY = Geo<TYV>::TY, BY = Geo<TYV>::BY, FIELD_BYTES = Geo<TYV>::FIELD_BYTES,
+                         OWN_BYTES = Geo<TYV>::OWN_BYTES;
     static constexpr bool DIAG = MODE == MODE_K1D || MODE == MODE_K31D;
     static constexpr int CODE_TX = DIAG ? BXC * BY * 2 : TX * TY * (CODE32 ? 4 : 2);   // bytes the TMA unit delivers
     static constexpr int CODE_BYTES = STORED ? 0 : ((CODE_TX + 127) / 128) * 128;
@@ -237,11 +249,13 @@ struct Slot {
     unsigned k0, k1;
 };
 
-template <int MODE, bool PRECOND, bool STORED, bool CODE32>
-__global__ void __launch_bounds__(NT, 1)
+template <int MODE, bool PRECOND, bool STORED, bool CODE32, int TYV>
+__global__ void __launch_bounds__(Geo<TYV>::NT, 1)
 k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv, const Scalars* sc_in, Scalars* sc_out, ReduceBuf rb,
       int zchunk, int ntx, int ntiles, int nitems) {
-    using L = Layout<MODE, STORED, CODE32>;
+    using L = Layout<MODE, STORED, CODE32, TYV>;
+    constexpr int TY = Geo<TYV>::TY, NW_CONSUMER = Geo<TYV>::NW_CONSUMER, NT_CONSUMER = Geo<TYV>::NT_CONSUMER,
+                  BY = Geo<TYV>::BY, FIELD_BYTES = Geo<TYV>::FIELD_BYTES;
     using T = ModeTraits<MODE>;
     constexpr int NS = T::STAGES;
     constexpr int NF = T::NF;
@@ -776,15 +790,25 @@ bool make_map(CUtensorMap* m, const void* base, CUtensorMapDataType dt, int elem
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-bool halo_map(CUtensorMap* m, const double* base, const GridDims& g) {
-    return make_map(m, base, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 8, g, g.nx, BX, BY);
+bool halo_map(CUtensorMap* m, const double* base, const GridDims& g, int ty) {
+    return make_map(m, base, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 8, g, g.nx, BX, ty + 2);
 }
-bool own_map(CUtensorMap* m, const double* base, const GridDims& g) {
-    return make_map(m, base, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 8, g, g.nx, TX, TY);
+bool own_map(CUtensorMap* m, const double* base, const GridDims& g, int ty) {
+    return make_map(m, base, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 8, g, g.nx, TX, ty);
 }
 
-template <int MODE, bool PRECOND, bool STORED, bool CODE32>
-void launch_inst(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaArgs& tm, dim3 grid, int depth) {
+// grid of work items (x tiles, y tiles, z chunks) for tiles of `ty` rows, and the chunk depth
+dim3 item_grid(const LaunchCtx& c, int ty, int* depth) {
+    const int tx = (c.g.nx + TX - 1) / TX, tyb = (c.g.ny + ty - 1) / ty;
+    const int chunks = choose_zchunks(c.g, tx * tyb, c.sm_count);
+    *depth = (c.g.nz + chunks - 1) / chunks;
+    return dim3(tx, tyb, (c.g.nz + *depth - 1) / *depth);
+}
+
+template <int MODE, bool PRECOND, bool STORED, bool CODE32, int TYV>
+void launch_geo(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaArgs& tm) {
+    int depth;
+    const dim3 grid = item_grid(c, TYV, &depth);
     // grid = (x tiles, y tiles, z chunks) of work items; launched as min(#SMs, #items) persistent blocks
     const int ntx = (int)grid.x, ntiles = (int)(grid.x * grid.y), nitems = ntiles * (int)grid.z;
     // The stored variant (six more arrays per node straight from global memory, no registers to spare for the
@@ -792,46 +816,70 @@ void launch_inst(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, c
     const int blocks = STORED ? nitems : std::min(c.sm_count, nitems);
     const Scalars* sc_in; Scalars* sc_out;
     c.next_scalars(sc_in, sc_out);
-    using L = Layout<MODE, STORED, CODE32>;
+    using L = Layout<MODE, STORED, CODE32, TYV>;
     static std::atomic<unsigned long long> configured{0ull};      // bit d: the attribute is set on device d
-    auto kern = k_tma<MODE, PRECOND, STORED, CODE32>;
+    auto kern = k_tma<MODE, PRECOND, STORED, CODE32, TYV>;
     const unsigned long long bit = 1ull << (c.device & 63);
     if (c.device >= 64 || !(configured.load(std::memory_order_relaxed) & bit)) {
         note_launch(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L::TOTAL));
         configured.fetch_or(bit, std::memory_order_relaxed);
     }
     ++g_launch_count;
-    note_launch(launch_pdl(c.pdl, kern, dim3(blocks), dim3(NT), (size_t)L::TOTAL, c.stream, tm, c.g, op, kv, sc_in, sc_out,
+    note_launch(launch_pdl(c.pdl, kern, dim3(blocks), dim3(Geo<TYV>::NT), (size_t)L::TOTAL, c.stream, tm, c.g, op, kv, sc_in, sc_out,
                            c.rb, depth, ntx, ntiles, nitems));
 }
 
+// ty: tile rows (TY_WIDE or TY_DEEP); the stored variant is compiled for the wide tiles only
+template <int MODE, bool PRECOND, bool STORED, bool CODE32>
+void launch_inst(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaArgs& tm, int ty) {
+    if (!STORED && ty == TY_DEEP) launch_geo<MODE, PRECOND, STORED, CODE32, STORED ? TY_WIDE : TY_DEEP>(c, op, kv, tm);
+    else launch_geo<MODE, PRECOND, STORED, CODE32, TY_WIDE>(c, op, kv, tm);
+}
+
 template <int MODE>
-void launch_mode(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaArgs& tm, bool precond) {
-    const int tx = (c.g.nx + TX - 1) / TX, tyb = (c.g.ny + TY - 1) / TY;
-    const int chunks = choose_zchunks(c.g, tx * tyb, c.sm_count);
-    const int depth = (c.g.nz + chunks - 1) / chunks;
-    dim3 grid(tx, tyb, (c.g.nz + depth - 1) / depth);
+void launch_mode(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaArgs& tm, bool precond, int ty) {
     const bool c32 = op.code32 != 0;
-    if (op.stored) {
-        if (precond) launch_inst<MODE, true, true, false>(c, op, kv, tm, grid, depth);
-        else         launch_inst<MODE, false, true, false>(c, op, kv, tm, grid, depth);
-    } else if (c32) {
-        if (precond) launch_inst<MODE, true, false, true>(c, op, kv, tm, grid, depth);
-        else         launch_inst<MODE, false, false, true>(c, op, kv, tm, grid, depth);
-    } else {
-        if (precond) launch_inst<MODE, true, false, false>(c, op, kv, tm, grid, depth);
-        else         launch_inst<MODE, false, false, false>(c, op, kv, tm, grid, depth);
+    constexpr bool MERGED = MODE == MODE_K2M || MODE == MODE_K31 || MODE == MODE_K31D;    // code form only
+    if constexpr (!MERGED) {
+        if (op.stored) {
+            if (precond) launch_inst<MODE, true, true, false>(c, op, kv, tm, ty);
+            else         launch_inst<MODE, false, true, false>(c, op, kv, tm, ty);
+            return;
+        }
     }
+    if (c32) {
+        if (precond) launch_inst<MODE, true, false, true>(c, op, kv, tm, ty);
+        else         launch_inst<MODE, false, false, true>(c, op, kv, tm, ty);
+    } else {
+        if (precond) launch_inst<MODE, true, false, false>(c, op, kv, tm, ty);
+        else         launch_inst<MODE, false, false, false>(c, op, kv, tm, ty);
+    }
+}
+
+// Tile rows of a launch.  Measured on one B200, same box, boost clock (profiles/r2_tiles.md): the deep tiles (16 warps,
+// 128 registers, no spills) win for both kernels of the merged solver at every size (K31 -8 to -16 %, K2M -2 to -11 %)
+// and for the Table-3 kernels up to about 140^3, where a launch takes a few tens of microseconds and the fixed costs of
+// a block count (k1 -6 % at 128^3); from 160^3 on the wide tiles win for k1 (fewer halo rows per tile row: 0.155
+// against 0.161 ms at 256^3) and k2 does not care.  c.tile_rows != 0 forces one geometry (PF_OPT_TILE_ROWS).
+int tile_rows(const LaunchCtx& c, const Operator& op, int mode) {
+    if (op.stored) return TY_WIDE;
+    if (c.tile_rows == TY_WIDE || c.tile_rows == TY_DEEP) return c.tile_rows;
+    if (mode == MODE_K31 || mode == MODE_K31D || mode == MODE_K2M) return TY_DEEP;
+    return c.g.n <= 144ll * 144 * 144 ? TY_DEEP : TY_WIDE;
 }
 
 }  // namespace
 
-// Tensor maps of one solve: every vector a kernel reads through TMA.
-struct TmaSet {
+// Tensor maps of one solve: every vector a kernel reads through TMA, once per tile geometry (the boxes differ).
+struct TmaMaps {
     CUtensorMap r, p[2], v[2], a0, rt, x, b, code;
     CUtensorMap codeh;       // 2-byte codes with the halo ring (MODE_K1D, MODE_K31D)
     CUtensorMap r1, th;      // merged solver: the second r buffer, and t with its halo ring
+};
+struct TmaSet {
+    TmaMaps m[2];            // [0]: TY_WIDE, [1]: TY_DEEP
     bool have_code, have_codeh, have_merged;
+    const TmaMaps& of(int ty) const { return m[ty == TY_DEEP ? 1 : 0]; }
 };
 
 bool tma_available() { return encoder() != nullptr; }
@@ -852,19 +900,24 @@ TmaSet* tma_set_create() { return new TmaSet(); }
 void tma_set_destroy(TmaSet* t) { delete t; }
 
 bool tma_set_build(TmaSet* t, const GridDims& g, const Operator& op, const KrylovVecs& kv) {
-    bool ok = halo_map(&t->r, kv.r, g) && halo_map(&t->p[0], kv.p_in, g) && halo_map(&t->p[1], kv.p_out, g) &&
-              halo_map(&t->v[0], kv.v_in, g) && halo_map(&t->v[1], kv.v_out, g) && halo_map(&t->a0, op.A0, g) &&
-              own_map(&t->rt, kv.rt, g) && halo_map(&t->x, kv.x, g) && own_map(&t->b, kv.b, g);
-    t->have_code = false;
-    if (ok && !op.stored) {
-        ok = op.code32 ? make_map(&t->code, op.code, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, g, op.cpitch, TX, TY)
-                       : make_map(&t->code, op.code, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, g, op.cpitch, TX, TY);
-        t->have_code = ok;
+    bool ok = true;
+    t->have_code = !op.stored;
+    t->have_codeh = !op.stored && !op.code32 && op.diag_code;
+    t->have_merged = kv.r_out && !op.stored && aligned16(kv.r_out);
+    for (int k = 0; k < (op.stored ? 1 : 2) && ok; ++k) {
+        TmaMaps& M = t->m[k];
+        const int ty = k ? TY_DEEP : TY_WIDE;
+        ok = halo_map(&M.r, kv.r, g, ty) && halo_map(&M.p[0], kv.p_in, g, ty) && halo_map(&M.p[1], kv.p_out, g, ty) &&
+             halo_map(&M.v[0], kv.v_in, g, ty) && halo_map(&M.v[1], kv.v_out, g, ty) && halo_map(&M.a0, op.A0, g, ty) &&
+             own_map(&M.rt, kv.rt, g, ty) && halo_map(&M.x, kv.x, g, ty) && own_map(&M.b, kv.b, g, ty);
+        if (ok && t->have_code)
+            ok = op.code32 ? make_map(&M.code, op.code, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, g, op.cpitch, TX, ty)
+                           : make_map(&M.code, op.code, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, g, op.cpitch, TX, ty);
+        if (ok && t->have_codeh)
+            t->have_codeh = make_map(&M.codeh, op.code, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, g, op.cpitch, BXC, ty + 2);
+        if (ok && t->have_merged) t->have_merged = halo_map(&M.r1, kv.r_out, g, ty) && halo_map(&M.th, kv.t, g, ty);
     }
-    t->have_codeh = ok && !op.stored && !op.code32 && op.diag_code &&
-                    make_map(&t->codeh, op.code, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, g, op.cpitch, BXC, BY);
-    t->have_merged = ok && kv.r_out && !op.stored && aligned16(kv.r_out) && halo_map(&t->r1, kv.r_out, g) &&
-                     halo_map(&t->th, kv.t, g);
+    if (!ok) t->have_code = t->have_codeh = t->have_merged = false;
     return ok;
 }
 
@@ -874,10 +927,12 @@ bool tma_merged_supported(const Operator& op) { return !op.stored; }
 // that k1 and k2 will divide by it with (reading D4; the residual itself involves no division).
 void launch_residual_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, int mode,
                          bool precond) {
+    const int ty = tile_rows(c, op, mode == 0 ? MODE_R0 : MODE_R1);
+    const TmaMaps& M = t->of(ty);
     TmaArgs a;
     std::memset(&a, 0, sizeof(a));
-    a.f[0] = t->x; a.f[1] = t->a0; a.own = t->b; a.code = t->code;
-    if (mode == 0) launch_mode<MODE_R0>(c, op, kv, a, precond); else launch_mode<MODE_R1>(c, op, kv, a, false);
+    a.f[0] = M.x; a.f[1] = M.a0; a.own = M.b; a.code = M.code;
+    if (mode == 0) launch_mode<MODE_R0>(c, op, kv, a, precond, ty); else launch_mode<MODE_R1>(c, op, kv, a, false, ty);
 }
 
 void launch_k1_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond,
@@ -885,72 +940,54 @@ void launch_k1_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv,
     TmaArgs a;
     std::memset(&a, 0, sizeof(a));
     if (t->have_codeh) {     // the diagonal is the sum of the face coefficients: formed from the codes, A0 not read
-        a.f[0] = t->r; a.f[1] = t->p[parity]; a.f[2] = t->v[parity]; a.own = t->rt; a.code = t->codeh;
-        const int tx = (c.g.nx + TX - 1) / TX, tyb = (c.g.ny + TY - 1) / TY;
-        const int chunks = choose_zchunks(c.g, tx * tyb, c.sm_count);
-        const int depth = (c.g.nz + chunks - 1) / chunks;
-        dim3 grid(tx, tyb, (c.g.nz + depth - 1) / depth);
-        if (precond) launch_inst<MODE_K1D, true, false, false>(c, op, kv, a, grid, depth);
-        else         launch_inst<MODE_K1D, false, false, false>(c, op, kv, a, grid, depth);
+        const int ty = tile_rows(c, op, MODE_K1D);
+        const TmaMaps& M = t->of(ty);
+        a.f[0] = M.r; a.f[1] = M.p[parity]; a.f[2] = M.v[parity]; a.own = M.rt; a.code = M.codeh;
+        if (precond) launch_inst<MODE_K1D, true, false, false>(c, op, kv, a, ty);
+        else         launch_inst<MODE_K1D, false, false, false>(c, op, kv, a, ty);
         return;
     }
-    a.f[0] = t->r; a.f[1] = t->p[parity]; a.f[2] = t->v[parity]; a.f[3] = t->a0; a.own = t->rt; a.code = t->code;
-    launch_mode<MODE_K1>(c, op, kv, a, precond);
-}
-
-// grid of work items (x tiles, y tiles, z chunks) and the chunk depth
-static dim3 item_grid(const LaunchCtx& c, int* depth) {
-    const int tx = (c.g.nx + TX - 1) / TX, tyb = (c.g.ny + TY - 1) / TY;
-    const int chunks = choose_zchunks(c.g, tx * tyb, c.sm_count);
-    *depth = (c.g.nz + chunks - 1) / chunks;
-    return dim3(tx, tyb, (c.g.nz + *depth - 1) / *depth);
+    const int ty = tile_rows(c, op, MODE_K1);
+    const TmaMaps& M = t->of(ty);
+    a.f[0] = M.r; a.f[1] = M.p[parity]; a.f[2] = M.v[parity]; a.f[3] = M.a0; a.own = M.rt; a.code = M.code;
+    launch_mode<MODE_K1>(c, op, kv, a, precond, ty);
 }
 
 void launch_k2m_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond, int k) {
+    const int ty = tile_rows(c, op, MODE_K2M);
+    const TmaMaps& M = t->of(ty);
     TmaArgs a;
     std::memset(&a, 0, sizeof(a));
     const int rb = k & 1, pb = rb ^ 1;
-    a.f[0] = rb ? t->r1 : t->r; a.f[1] = t->v[pb]; a.f[2] = t->a0; a.own = t->rt; a.code = t->code;
-    int depth;
-    const dim3 grid = item_grid(c, &depth);
-    if (op.code32) {
-        if (precond) launch_inst<MODE_K2M, true, false, true>(c, op, kv, a, grid, depth);
-        else         launch_inst<MODE_K2M, false, false, true>(c, op, kv, a, grid, depth);
-    } else {
-        if (precond) launch_inst<MODE_K2M, true, false, false>(c, op, kv, a, grid, depth);
-        else         launch_inst<MODE_K2M, false, false, false>(c, op, kv, a, grid, depth);
-    }
+    a.f[0] = rb ? M.r1 : M.r; a.f[1] = M.v[pb]; a.f[2] = M.a0; a.own = M.rt; a.code = M.code;
+    launch_mode<MODE_K2M>(c, op, kv, a, precond, ty);
 }
 
 void launch_k31_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond, int k) {
     TmaArgs a;
     std::memset(&a, 0, sizeof(a));
     const int rb = k & 1, pb = rb ^ 1;
-    a.f[0] = rb ? t->r1 : t->r; a.f[1] = t->p[pb]; a.f[2] = t->v[pb]; a.f[3] = t->th; a.own = t->rt;
-    int depth;
-    const dim3 grid = item_grid(c, &depth);
+    const int ty = tile_rows(c, op, t->have_codeh ? MODE_K31D : MODE_K31);
+    const TmaMaps& M = t->of(ty);
+    a.f[0] = rb ? M.r1 : M.r; a.f[1] = M.p[pb]; a.f[2] = M.v[pb]; a.f[3] = M.th; a.own = M.rt;
     if (t->have_codeh) {     // the diagonal is the sum of the face coefficients: formed from the codes, A0 not read
-        a.code = t->codeh;
-        if (precond) launch_inst<MODE_K31D, true, false, false>(c, op, kv, a, grid, depth);
-        else         launch_inst<MODE_K31D, false, false, false>(c, op, kv, a, grid, depth);
+        a.code = M.codeh;
+        if (precond) launch_inst<MODE_K31D, true, false, false>(c, op, kv, a, ty);
+        else         launch_inst<MODE_K31D, false, false, false>(c, op, kv, a, ty);
         return;
     }
-    a.f[4] = t->a0; a.code = t->code;
-    if (op.code32) {
-        if (precond) launch_inst<MODE_K31, true, false, true>(c, op, kv, a, grid, depth);
-        else         launch_inst<MODE_K31, false, false, true>(c, op, kv, a, grid, depth);
-    } else {
-        if (precond) launch_inst<MODE_K31, true, false, false>(c, op, kv, a, grid, depth);
-        else         launch_inst<MODE_K31, false, false, false>(c, op, kv, a, grid, depth);
-    }
+    a.f[4] = M.a0; a.code = M.code;
+    launch_mode<MODE_K31>(c, op, kv, a, precond, ty);
 }
 
 void launch_k2_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond,
                    int parity) {
+    const int ty = tile_rows(c, op, MODE_K2);
+    const TmaMaps& M = t->of(ty);
     TmaArgs a;
     std::memset(&a, 0, sizeof(a));
-    a.f[0] = t->r; a.f[1] = t->v[parity ^ 1]; a.f[2] = t->a0; a.code = t->code;   // v' = the buffer k1 just wrote
-    launch_mode<MODE_K2>(c, op, kv, a, precond);
+    a.f[0] = M.r; a.f[1] = M.v[parity ^ 1]; a.f[2] = M.a0; a.code = M.code;   // v' = the buffer k1 just wrote
+    launch_mode<MODE_K2>(c, op, kv, a, precond, ty);
 }
 
 }  // namespace pf

@@ -37,6 +37,7 @@ struct LaunchCtx {
     int sm_count;
     int device;       // CUDA device of the grid (per-device kernel attributes)
     int solver;       // 0: Table 3, three kernels per iteration; 1: merged recurrence, two (pf_krylov.cuh)
+    int tile_rows;    // tiled family: 0 = chosen per kernel and grid, 13 or 16 = forced (PF_OPT_TILE_ROWS)
     bool pdl;         // programmatic dependent launch allowed
     // the next kernel reads sc[*flip] and its block 0 writes sc[*flip ^ 1]
     void next_scalars(const Scalars*& in, Scalars*& out) const { in = sc[*flip]; out = sc[*flip ^ 1]; *flip ^= 1; }

@@ -23,7 +23,8 @@ PF_ERR_ARG, PF_ERR_CUDA, PF_ERR_BREAKDOWN, PF_ERR_NONPHYSICAL, PF_ERR_WORKSPACE 
 PF_BC_DIRICHLET, PF_BC_NEUMANN = 0, 1
 (PF_OPT_STENCIL, PF_OPT_OMEGA_PF, PF_OPT_LINEAR_TOL, PF_OPT_LINEAR_MAXIT, PF_OPT_CHECK_INTERVAL,
  PF_OPT_WATER_MOLAR, PF_OPT_MAX_OUTER, PF_OPT_PRECOND, PF_OPT_HISTORY, PF_OPT_KERNELS, PF_OPT_PROFILE,
- PF_OPT_GRAPH, PF_OPT_NORM, PF_OPT_CHARGE_MODEL, PF_OPT_DIAG_FROM_CODE, PF_OPT_SOLVER, PF_OPT_STERIC_MODE) = range(1, 18)
+ PF_OPT_GRAPH, PF_OPT_NORM, PF_OPT_CHARGE_MODEL, PF_OPT_DIAG_FROM_CODE, PF_OPT_SOLVER, PF_OPT_STERIC_MODE,
+ PF_OPT_TILE_ROWS) = range(1, 19)
 STERIC_SIMULTANEOUS, STERIC_LAGGED = 0, 1
 SOLVER_TABLE3, SOLVER_MERGED = 0, 1
 CHARGES_DEPOSITED, CHARGES_SINGULAR = 0, 1

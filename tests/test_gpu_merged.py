@@ -186,3 +186,29 @@ def test_merged_pf_config0_32(pf, oracle, kernels):
     for k in range(len(sp.valence) + 1):
         assert rel_l2(out["conc"][k].cpu().numpy(), ref["conc"][k]) <= 1e-7
     print(f"merged PF 32^3 kernels {kernels}: outer {out['outer_iters']}, linear gpu/oracle {out['linear_iters']}/{ref['linear_iters']}")
+
+
+@pytest.mark.parametrize("rows", [13, 16])
+@pytest.mark.parametrize("solver", [0, 1])
+def test_both_tile_geometries_equal_direct(pf, rows, solver):
+    """PF_OPT_TILE_ROWS: the tiled kernels are compiled for tiles of 16 rows (19 warps) and of 13 rows (16 warps, 128
+    registers); the default picks per kernel and grid size.  Forced either way they give the bits of the direct kernels,
+    on shapes with partial tiles in x and y for both heights, Poisson (diagonal from the codes) and with a sigma."""
+    for shape in ((64, 29, 12), (130, 33, 21), (66, 53, 40)):
+        nx, ny, nz = shape
+        w = ragged_workload(nx=nx, ny=ny, nz=nz, seed=77 + ny)
+        sigma = np.random.default_rng(ny).uniform(0.0, 2.0, size=w.n)
+        for sg in (None, sigma):
+            outs = []
+            for kernels, r in ((pf.KERNELS_DIRECT, 0), (pf.KERNELS_TILED, rows)):
+                g = pf.Grid.from_workload(w, stencil=2, kernels=kernels,
+                                          options={pf.PF_OPT_SOLVER: solver, pf.PF_OPT_TILE_ROWS: r, pf.PF_OPT_HISTORY: 256})
+                o = g.solve_linear(w.rhs, tol=1e-10, maxit=150, sigma=None if sg is None else torch.tensor(sg, device="cuda"))
+                o["hist"] = g.history(256)
+                assert pf.pf_grid_fault_repeats(g.handle) == 0
+                g.close()
+                outs.append(o)
+            a, b = outs
+            assert a["status"] == b["status"] and a["iters"] == b["iters"]
+            assert torch.equal(a["x"], b["x"]) and np.array_equal(a["hist"], b["hist"])
+            assert a["true_relres"] == b["true_relres"]
