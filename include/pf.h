@@ -111,9 +111,10 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
                                      set before pf_grid_set_workspace; all charges are assumed to lie in Omega_m. */
 
 #define PF_OPT_DIAG_FROM_CODE 15  /* 1: in Poisson solves without sigma (pf_solve_linear, the initial guess of
-                                     pf_solve_pf) with 2-byte stencil codes, the tiled kernel of row L4 forms the
-                                     diagonal A0 = sum of the six face coefficients from the code instead of reading
-                                     it (8 bytes per unknown less; same bits).  0: A0 is read. */
+                                     pf_solve_pf) with 2-byte stencil codes, the tiled kernel of row L4 looks the
+                                     diagonal A0 = sum of the six face coefficients up from the code instead of
+                                     reading it (8 bytes per unknown less; same bits), together with the divisor's
+                                     half of the Jacobi division.  2: the kernel of row L5 as well.  0: A0 is read. */
 
 #define PF_OPT_SOLVER         16  /* 0 (default): BiCGSTAB as Table 3 writes it, three kernels and three reduction points per
                                      iteration.  1: the merged recurrence (SURVEY 8(d) "fully merged"; reading M1 of
@@ -135,6 +136,12 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
                                      and grid size (16 rows / 19 warps / 96 registers, or 13 rows / 16 warps / 128
                                      registers); 13 or 16 force one geometry.  Same bits either way; a tuning and
                                      measurement knob. */
+
+#define PF_OPT_SEGMENTS       19  /* tiled kernels: how tiles x z ranges are handed to the persistent blocks.  -1 (default):
+                                     chosen per grid; 0: z cut into equal chunks, blocks take (tile, chunk) items
+                                     round-robin; 1: for grids with fewer tiles than SMs, whole layers in step on most
+                                     SMs and the remaining planes split evenly over the other SMs.  Same bits either
+                                     way; a tuning and measurement knob. */
 
 /* Create a grid: store geometry and boundary conditions, scan eps_map for its palette of distinct
  * values, keep a device copy of the charges.  Assembly itself runs in pf_grid_set_workspace.

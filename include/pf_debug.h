@@ -43,6 +43,17 @@ int pf_grid_fault_repeats(const pf_grid *g);
  * three-kernel families) or an argument is invalid. */
 int pf_coop_plan(int nx, int ny, int nz, int max_blocks, size_t smem_cap, int *out);
 
+/* How the persistent tiled kernels (pf_krylov_tma.cu) hand the tiles x z ranges of an nx x ny x nz box to their blocks
+ * on a device with sm_count SMs, for tiles of tile_rows (13 or 16) rows and PF_OPT_SEGMENTS = mode (-1, 0, 1).  Host
+ * arithmetic only.  out (host, 9 ints): mode chosen (0 equal chunks, 1 two groups); tiles along x; tiles; mode 0: chunk
+ * depth, mode 1: layer depth of the main group; mode 0: items = tiles * chunks, mode 1: blocks of the main group; mode 1:
+ * first plane of the rest group, its number of planes, and the flattened (tile-major) positions per rest block; blocks
+ * launched.  Block b works on: mode 0 -- items b, b + blocks, ... with item i = tile i % tiles, planes
+ * [(i / tiles) * depth, min(+ depth, nz)); mode 1, b < main -- tile b % tiles, planes [(b / tiles) * depth, + depth);
+ * mode 1, rest block r = b - main -- positions [r q, min((r + 1) q, tiles * erest)), position p = tile p / erest, plane
+ * zrest + p % erest, cut into one segment per tile.  Returns PF_OK or PF_ERR_ARG. */
+int pf_tile_plan(int nx, int ny, int nz, int tile_rows, int sm_count, int mode, int *out);
+
 /* Introspection used by the tests: 1 = stored, 2 = on-the-fly; number of palette entries. */
 int pf_grid_stencil(const pf_grid *g);
 int pf_grid_palette_size(const pf_grid *g);

@@ -177,6 +177,7 @@ struct pf_grid {
     int opt_norm;            // 0: relative 2-norm (Q3), 1: the paper's absolute maximum norm
     int opt_solver;          // 0: Table 3 (three kernels per iteration), 1: merged recurrence (two; reading M1)
     int opt_tile_rows;       // tiled kernels: 0 auto, 13 or 16 forced
+    int opt_seg_mode;        // tiled kernels: -1 auto, 0 equal chunks, 1 two groups (PF_OPT_SEGMENTS)
     int opt_charge_model;    // 0: trilinear deposition (Q22), 1: singular-charge decomposition (Eqs 5-10)
     int charge_model;        // the model the workspace was laid out and assembled for
     double *phiL, *phistar, *A0_L;
@@ -264,7 +265,7 @@ Operator make_op(const pf_grid* g, int which /*0 poisson, 1 pf1, 2 poisson+sigma
         for (int d = 0; d < 6; ++d) op.offd[d] = g->offd_pf1[d];
     } else {
         op.A0 = which == 2 ? g->A0_s : g->A0; op.code = g->code; op.ctab = g->ctab_poisson;
-        op.diag_code = (which == 0 && g->opt_diag_code && !op.stored && !op.code32) ? 1 : 0;
+        op.diag_code = (which == 0 && !op.stored && !op.code32) ? g->opt_diag_code : 0;
         for (int d = 0; d < 6; ++d) op.offd[d] = g->offd[d];
     }
     return op;
@@ -274,6 +275,7 @@ LaunchCtx make_ctx(const pf_grid* g) {
     LaunchCtx c;
     c.stream = g->stream; c.g = g->g; c.sc[0] = g->sc[0]; c.sc[1] = g->sc[1]; c.flip = const_cast<int*>(&g->flip);
     c.rb = g->rb; c.sm_count = g->sm_count; c.device = g->device; c.pdl = true; c.solver = g->opt_solver; c.tile_rows = g->opt_tile_rows;
+    c.seg_mode = g->opt_seg_mode;
     return c;
 }
 
@@ -313,7 +315,7 @@ cudaGraphExec_t chunk_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, 
     if (!g->opt_graph || (chunk & 1)) return nullptr;
     for (const auto& cg : g->graphs)
         if (cg.a0 == op.A0 && cg.code == op.code && cg.b == kv.b && cg.x == kv.x && cg.y == kv.y && cg.hist == kv.hist &&
-            cg.precond == (int)precond && cg.tiled == ((int)tiled | (op.diag_code ? 2 : 0) | (c.solver ? 4 : 0)) && cg.chunk == chunk)
+            cg.precond == (int)precond && cg.tiled == ((int)tiled | (op.diag_code << 1) | (c.solver ? 8 : 0)) && cg.chunk == chunk)
             return cg.exec;
     if (!g->capture_stream &&
         cudaStreamCreateWithFlags(&g->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
@@ -338,7 +340,7 @@ cudaGraphExec_t chunk_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, 
         cudaGraphExecDestroy(g->graphs.front().exec);
         g->graphs.erase(g->graphs.begin());
     }
-    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled | (op.diag_code ? 2 : 0) | (c.solver ? 4 : 0), chunk, exec});
+    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled | (op.diag_code << 1) | (c.solver ? 8 : 0), chunk, exec});
     return exec;
 }
 
@@ -353,7 +355,7 @@ cudaGraphExec_t loop_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, c
     if (g->opt_graph < 2 || (body & 1) || body < 2) return nullptr;
     for (const auto& cg : g->graphs)
         if (cg.a0 == op.A0 && cg.code == op.code && cg.b == kv.b && cg.x == kv.x && cg.y == kv.y && cg.hist == kv.hist &&
-            cg.precond == (int)precond && cg.tiled == ((int)tiled | (op.diag_code ? 2 : 0) | (c.solver ? 4 : 0)) && cg.chunk == -body)
+            cg.precond == (int)precond && cg.tiled == ((int)tiled | (op.diag_code << 1) | (c.solver ? 8 : 0)) && cg.chunk == -body)
             return cg.exec;
     if (!g->capture_stream &&
         cudaStreamCreateWithFlags(&g->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
@@ -394,7 +396,7 @@ cudaGraphExec_t loop_graph(pf_grid* g, const LaunchCtx& c, const Operator& op, c
         cudaGraphExecDestroy(g->graphs.front().exec);
         g->graphs.erase(g->graphs.begin());
     }
-    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled | (op.diag_code ? 2 : 0) | (c.solver ? 4 : 0), -body, exec});
+    g->graphs.push_back({op.A0, op.code, kv.b, kv.x, kv.y, kv.hist, (int)precond, (int)tiled | (op.diag_code << 1) | (c.solver ? 8 : 0), -body, exec});
     return exec;
 }
 
@@ -741,7 +743,7 @@ int pf_grid_create(pf_grid** out, int nx, int ny, int nz, double h, const double
     g->hist = nullptr; g->hist_cap = 0; g->last_iters = 0; g->fault_repeats = 0;
     g->hb = g->hx = g->sstate = nullptr; g->opt_steric_mode = 0; g->copy_stream = nullptr; g->staged_ev = g->main_ev = nullptr;
     g->staged_rhs = g->staged_x = nullptr;
-    g->capture_stream = nullptr; g->opt_graph = 3; g->opt_diag_code = 1; g->opt_norm = 0; g->opt_solver = 0; g->opt_tile_rows = 0;
+    g->capture_stream = nullptr; g->opt_graph = 3; g->opt_diag_code = 1; g->opt_norm = 0; g->opt_solver = 0; g->opt_tile_rows = 0; g->opt_seg_mode = -1;
     g->opt_charge_model = 0; g->charge_model = 0; g->phiL = g->phistar = g->A0_L = nullptr; g->code_L = nullptr;
     g->ctab_L = nullptr; g->laplace_iters = 0; g->fixv = nullptr; g->bc.fixv = nullptr;
     g->small = nullptr;
@@ -883,7 +885,8 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
                 return fail(g, PF_ERR_ARG, "set the charge model before pf_grid_set_workspace");
             g->opt_charge_model = iv; return PF_OK;
         case PF_OPT_DIAG_FROM_CODE:
-            g->opt_diag_code = iv != 0; return PF_OK;
+            if (iv < 0 || iv > 2) return fail(g, PF_ERR_ARG, "diag-from-code must be 0, 1 (k1) or 2 (k1 and k2)");
+            g->opt_diag_code = iv; return PF_OK;
         case PF_OPT_TILE_ROWS:
             if (iv != 0 && iv != 13 && iv != 16) return fail(g, PF_ERR_ARG, "tile rows must be 0 (auto), 13 or 16");
             if (iv != g->opt_tile_rows) {          // cached graphs hold kernels of the other geometry
@@ -892,6 +895,14 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
                 g->graphs.clear();
             }
             g->opt_tile_rows = iv; return PF_OK;
+        case PF_OPT_SEGMENTS:
+            if (iv < -1 || iv > 1) return fail(g, PF_ERR_ARG, "segments must be -1 (auto), 0 (equal chunks) or 1 (two groups)");
+            if (iv != g->opt_seg_mode) {           // cached graphs hold launches of the other decomposition
+                cudaStreamSynchronize(g->stream);
+                for (auto& cg : g->graphs) cudaGraphExecDestroy(cg.exec);
+                g->graphs.clear();
+            }
+            g->opt_seg_mode = iv; return PF_OK;
         case PF_OPT_STERIC_MODE:
             if (iv != 0 && iv != 1) return fail(g, PF_ERR_ARG, "steric mode must be 0 (simultaneous) or 1 (lagged)");
             g->opt_steric_mode = iv; return PF_OK;
@@ -1233,6 +1244,15 @@ int pf_coop_plan(int nx, int ny, int nz, int max_blocks, size_t smem_cap, int* o
     if (!coop_plan(gd, op, max_blocks, smem_cap, &plan)) return PF_ERR_ARG;
     out[0] = plan.nbx; out[1] = plan.nby; out[2] = plan.nbz; out[3] = plan.vmax; out[4] = plan.hmax;
     out[5] = plan.nhmax; out[6] = plan.threads; out[7] = (int)plan.smem;
+    return PF_OK;
+}
+
+int pf_tile_plan(int nx, int ny, int nz, int tile_rows, int sm_count, int mode, int* out) {
+    if (!out || nx < 1 || ny < 1 || nz < 1 || sm_count < 1 || (tile_rows != 13 && tile_rows != 16) || mode < -1 || mode > 1)
+        return PF_ERR_ARG;
+    GridDims gd;
+    gd.nx = nx; gd.ny = ny; gd.nz = nz; gd.n = (long long)nx * ny * nz;
+    tma_plan(gd, tile_rows, sm_count, mode, out);
     return PF_OK;
 }
 

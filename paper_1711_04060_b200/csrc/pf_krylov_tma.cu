@@ -68,12 +68,56 @@ struct Geo {
 };
 constexpr int TY_WIDE = 16, TY_DEEP = 13;
 
-enum { MODE_R0 = 0, MODE_R1 = 1, MODE_K1 = 2, MODE_K2 = 3, MODE_K1D = 4, MODE_K2M = 5, MODE_K31 = 6, MODE_K31D = 7 };
+enum { MODE_R0 = 0, MODE_R1 = 1, MODE_K1 = 2, MODE_K2 = 3, MODE_K1D = 4, MODE_K2M = 5, MODE_K31 = 6, MODE_K31D = 7,
+       MODE_K2D = 8, MODE_K2MD = 9 };
 // MODE_K1D: k1 for operators whose diagonal is the sum of their face coefficients (Poisson without sigma): A0 is
-// not read but formed from the stencil code, whose box then covers the halo ring too.
-// MODE_K2M, MODE_K31 (MODE_K31D: diagonal from the codes): the two kernels of the merged solver (pf_krylov.cuh).
+// not read but looked up, together with the reciprocal the Jacobi division needs, in a table indexed by the node's
+// stencil code, whose box then covers the halo ring too.  MODE_K2D: the same for k2.
+// MODE_K2M, MODE_K31 (MODE_K2MD, MODE_K31D: diagonal from the codes): the two kernels of the merged solver (pf_krylov.cuh).
 constexpr int CXO = 8;                   // code box with halo: starts CXO nodes left of the tile (the TMA unit wants the
 constexpr int BXC = TX + 2 * CXO;        // box to start on a 16-byte boundary of the row: 8 two-byte entries), rows of 160 bytes
+
+// ---- work decomposition ------------------------------------------------------------------------
+// A segment is one tile marched along z over [z0, z1): z1 - z0 + 2 plane steps (the two extra planes only form u).
+// Two ways to hand segments to the persistent blocks (plan_segments below picks the one with the shorter longest block):
+//   mode 0  z is cut into equal chunks; item i = (tile i % ntiles, chunk i / ntiles); block b takes items b, b + G, ...
+//           Blocks that run at the same time work on neighbouring tiles of the same chunk, plane for plane, so halo
+//           rows are shared in L2.
+//   mode 1  for grids with fewer tiles than SMs, where mode 0 cannot fill the SMs evenly (256^3: 64 tiles x 9 chunks on
+//           148 SMs = 4 rounds of 31 steps with the last round short: 124 steps against 111 of the volume itself):
+//           `full` = #SMs / ntiles layers of `zchunk` planes are taken by ntiles * full blocks, one segment each, all
+//           in step; the remaining planes z >= zrest of all tiles, flattened tile-major, are split evenly over the
+//           remaining blocks (a few short segments each).  256^3: 114 steps.
+struct SegPlan {
+    int mode, ntx, ntiles;
+    int zchunk, nitems;       // mode 0: chunk depth and tiles * chunks; mode 1: layer depth of the main group, nmain
+    int zrest, erest, q;      // mode 1: the rest group's planes [zrest, zrest + erest), q flattened positions per block
+    int blocks;               // host: blocks to launch
+};
+// The segments of block b, one after the other (every thread of the block walks the same sequence).  PERSIST = false:
+// the block's one item of the equal-chunk plan (the stored variant has no registers to spare for a loop).
+template <bool PERSIST>
+struct SegIter {
+    int pos, end;
+    __device__ __forceinline__ void init(const SegPlan& P, int b) {
+        if (PERSIST && P.mode == 1 && b >= P.nitems) { pos = (b - P.nitems) * P.q; end = min(pos + P.q, P.ntiles * P.erest); }
+        else if (PERSIST && P.mode == 1) { pos = b; end = b + 1; }
+        else { pos = b; end = PERSIST ? P.nitems : min(b + 1, P.nitems); }
+    }
+    __device__ __forceinline__ bool next(const SegPlan& P, int nz, int b, int nblocks, int& tile, int& z0, int& z1) {
+        if (pos >= end) return false;
+        if (PERSIST && P.mode == 1 && b >= P.nitems) {          // rest group: flattened positions, one segment per tile
+            tile = pos / P.erest;
+            const int zz = pos - tile * P.erest, len = min(P.erest - zz, end - pos);
+            z0 = P.zrest + zz; z1 = z0 + len; pos += len;
+        } else {
+            tile = pos % P.ntiles;
+            z0 = (pos / P.ntiles) * P.zchunk; z1 = min(z0 + P.zchunk, (PERSIST && P.mode == 1) ? P.zrest : nz);
+            pos += PERSIST ? nblocks : 1;
+        }
+        return true;
+    }
+};
 
 template <int MODE> struct ModeTraits;
 template <> struct ModeTraits<MODE_R0> { static constexpr int NF = 2; static constexpr bool OWN = true;  static constexpr int STAGES = 4; };
@@ -84,8 +128,11 @@ template <> struct ModeTraits<MODE_K2> { static constexpr int NF = 3; static con
 template <> struct ModeTraits<MODE_K2M> { static constexpr int NF = 3; static constexpr bool OWN = true; static constexpr int STAGES = 4; };
 template <> struct ModeTraits<MODE_K31> { static constexpr int NF = 5; static constexpr bool OWN = true; static constexpr int STAGES = 3; };
 template <> struct ModeTraits<MODE_K31D> { static constexpr int NF = 4; static constexpr bool OWN = true; static constexpr int STAGES = 3; };
+template <> struct ModeTraits<MODE_K2D> { static constexpr int NF = 2; static constexpr bool OWN = false; static constexpr int STAGES = 4; };
+template <> struct ModeTraits<MODE_K2MD> { static constexpr int NF = 2; static constexpr bool OWN = true; static constexpr int STAGES = 4; };
 
-// Halo fields in stage order.  K1: r, p, v, A0.  K1D: r, p, v.  K2, K2M: r, v, A0.  K31: r, p, v, t, A0.  K31D: r, p, v, t.
+// Halo fields in stage order.  K1: r, p, v, A0.  K1D: r, p, v.  K2, K2M: r, v, A0.  K2D, K2MD: r, v.  K31: r, p, v, t, A0.
+// K31D: r, p, v, t.
 // R0/R1: x, A0.  Own-only field (tile without halo): K1, K2M, K31: r~;  R0/R1: b.
 struct TmaArgs {
     CUtensorMap f[5];
@@ -98,24 +145,27 @@ struct Layout {
     using T = ModeTraits<MODE>;
     static constexpr int TY = Geo<TYV>::TY, BY = Geo<TYV>::BY, FIELD_BYTES = Geo<TYV>::FIELD_BYTES,
                          OWN_BYTES = Geo<TYV>::OWN_BYTES;
-    static constexpr bool DIAG = MODE == MODE_K1D || MODE == MODE_K31D;
+    static constexpr bool DIAG = MODE == MODE_K1D || MODE == MODE_K31D || MODE == MODE_K2D || MODE == MODE_K2MD;
+    // (the wide K31D, which no policy picks, makes room for the table with a stage less)
+    static constexpr int STAGES = (MODE == MODE_K31D && TYV == 16) ? 2 : T::STAGES;
     static constexpr int CODE_TX = DIAG ? BXC * BY * 2 : TX * TY * (CODE32 ? 4 : 2);   // bytes the TMA unit delivers
     static constexpr int CODE_BYTES = STORED ? 0 : ((CODE_TX + 127) / 128) * 128;
     static constexpr int STAGE_BYTES = T::NF * FIELD_BYTES + (T::OWN ? OWN_BYTES : 0) + CODE_BYTES;
     static constexpr int OWN_OFF = T::NF * FIELD_BYTES;
     static constexpr int CODE_OFF = OWN_OFF + (T::OWN ? OWN_BYTES : 0);
-    static constexpr int U_OFF = T::STAGES * STAGE_BYTES;
+    static constexpr int U_OFF = STAGES * STAGE_BYTES;
     static constexpr int CTAB_OFF = U_OFF + NU * FIELD_BYTES;
     // 2-bit codes: the coefficients of three faces at once from a 64-entry table of 32-byte entries, placed at
     // the first 2048-byte boundary inside a 4 KB region (its address is ORed with the entry offset)
     static constexpr int T3_OFF = CTAB_OFF + PF_CTAB * 8;
     static constexpr int T3_BYTES = (STORED || CODE32) ? 0 : 4096;
-    // MODE_K1D: the diagonal as a function of the 12-bit code of a node, 4096 doubles, built by the block at its start
+    // DIAG modes: the diagonal and the reciprocal half of the Jacobi division (recip_nb) as functions of the 12-bit
+    // code of a node, 4096 pairs of doubles, built by the block at its start
     static constexpr int DTAB_OFF = T3_OFF + T3_BYTES;
-    static constexpr int DTAB_BYTES = DIAG ? 4096 * 8 : 0;
+    static constexpr int DTAB_BYTES = DIAG ? 4096 * 16 : 0;
     static constexpr int SCRATCH_OFF = DTAB_OFF + DTAB_BYTES;
     static constexpr int BAR_OFF = SCRATCH_OFF + 3 * 32 * (int)sizeof(dd);
-    static constexpr int SC_OFF = ((BAR_OFF + 16 * T::STAGES + 8 * NU + 15) / 16) * 16;   // after full[S], empty[S], ready[NU]
+    static constexpr int SC_OFF = ((BAR_OFF + 16 * STAGES + 8 * NU + 15) / 16) * 16;   // after full[S], empty[S], ready[NU]
     static constexpr int TOTAL = SC_OFF + 256;                       // the block's copy of the scalars
     static_assert(TOTAL <= 232448, "dynamic shared memory of a block (227 KB)");
     static_assert(CTAB_OFF % 128 == 0, "ctab_at ORs table offsets into the table address");
@@ -176,24 +226,27 @@ struct Ring {
     }
 };
 
+// rc: recip_nb(a) from the table of the DIAG modes (unused otherwise)
 template <int MODE, bool PRECOND>
-__device__ __forceinline__ double u_of(double r, double p, double v, double a, bool first, double c1, double c2,
+__device__ __forceinline__ double u_of(double r, double p, double v, double a, double rc, bool first, double c1, double c2,
                                        double& numer, DivRange& range) {
+    constexpr bool TAB = MODE == MODE_K1D || MODE == MODE_K2D || MODE == MODE_K2MD;
     if (MODE == MODE_K1 || MODE == MODE_K1D) numer = p_new_at<PRECOND>(first, c1, c2, r, p, v);
-    else if (MODE == MODE_K2 || MODE == MODE_K2M) numer = s_at(c1, r, v);
+    else if (MODE == MODE_K2 || MODE == MODE_K2M || MODE == MODE_K2D || MODE == MODE_K2MD) numer = s_at(c1, r, v);
     else { numer = r; return r; }    // residual modes: the field is x itself (passed in r)
-    return PRECOND ? dvd_nb(numer, a, range) : numer;   // == jacobi<PRECOND>(numer, a) of the direct kernels
+    // == jacobi<PRECOND>(numer, a) of the direct kernels
+    return PRECOND ? (TAB ? dvd_rcp(numer, a, rc, range) : dvd_nb(numer, a, range)) : numer;
 }
 
 // Merged solver, K31: from the old r, p, v, t of a node: s (step 13), the new r (step 17), the new p (step 9 of the next
 // iteration) and u = M^-1 p'.
-template <bool PRECOND>
-__device__ __forceinline__ double u31_of(double r, double p, double v, double t, double a, double alpha, double omega,
-                                         double beta, double& s, double& rn, double& pn, DivRange& range) {
+template <bool PRECOND, bool TAB>
+__device__ __forceinline__ double u31_of(double r, double p, double v, double t, double a, double rc, double alpha,
+                                         double omega, double beta, double& s, double& rn, double& pn, DivRange& range) {
     s = s_at(alpha, r, v);
     rn = sub(s, mul(omega, t));
     pn = p_new_at<PRECOND>(false, beta, omega, rn, p, v);
-    return PRECOND ? dvd_nb(pn, a, range) : pn;
+    return PRECOND ? (TAB ? dvd_rcp(pn, a, rc, range) : dvd_nb(pn, a, range)) : pn;
 }
 
 // Coefficient of field d of node e (0 or 1) of the thread's code word(s): one shift, one three-input logic
@@ -224,21 +277,27 @@ __device__ __forceinline__ void ctab3_at(unsigned t3_addr, unsigned w0, int e, i
     asm("ld.shared.f64 %0, [%1+16];" : "=d"(c[2]) : "r"(off));
 }
 
-// MODE_K1D: the diagonal of a node as a function of its 12-bit code (six 2-bit fields).  The Poisson assembly adds
+// DIAG modes: the diagonal of a node as a function of its 12-bit code (six 2-bit fields).  The Poisson assembly adds
 // the six face coefficients in the order of the fields, starting from 0.0, and the table holds their negatives, so
 // the negated sum of the table entries has the same bits; rows without a face (code 0) are the identity rows,
-// diagonal 1.  Every block tabulates the 4096 values once at its start (ctab: the 16-entry coefficient table).
+// diagonal 1.  Every block tabulates the 4096 values once at its start (ctab: the 16-entry coefficient table), each
+// with recip_nb of it: the divisor's half of the branch-free division, so that a Jacobi division costs a multiplication
+// and two fused operations per node instead of nine (same bits: the same instruction sequence, split in two).
 __device__ __forceinline__ double diag_of_code12(const double* ctab, unsigned code) {
     double sacc = 0.0;
 #pragma unroll
     for (int d = 0; d < 6; ++d) sacc = add(sacc, ctab[(code >> (2 * d)) & 3u]);
     return code == 0u ? 1.0 : -sacc;
 }
-__device__ __forceinline__ double dtab_at(unsigned dtab_addr, unsigned w0, int e) {
-    const unsigned off = (e ? (w0 >> 13) & 0x7ff8u : (w0 << 3) & 0x7ff8u) + dtab_addr;
+__device__ __forceinline__ double dtab_at(unsigned dtab_addr, unsigned w0, int e) {             // the diagonal alone
+    const unsigned off = (e ? (w0 >> 12) & 0xfff0u : (w0 << 4) & 0xfff0u) + dtab_addr;
     double a;
     asm("ld.shared.f64 %0, [%1];" : "=d"(a) : "r"(off));
     return a;
+}
+__device__ __forceinline__ void dtab2_at(unsigned dtab_addr, unsigned w0, int e, double& a, double& rc) {   // with its reciprocal
+    const unsigned off = (e ? (w0 >> 12) & 0xfff0u : (w0 << 4) & 0xfff0u) + dtab_addr;
+    asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(rc) : "r"(off));
 }
 
 // Registers of one plane of a main thread: u at its two nodes, the numerators (p' or s), the diagonal,
@@ -252,17 +311,17 @@ struct Slot {
 template <int MODE, bool PRECOND, bool STORED, bool CODE32, int TYV>
 __global__ void __launch_bounds__(Geo<TYV>::NT, 1)
 k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv, const Scalars* sc_in, Scalars* sc_out, ReduceBuf rb,
-      int zchunk, int ntx, int ntiles, int nitems) {
+      SegPlan plan) {
     using L = Layout<MODE, STORED, CODE32, TYV>;
     constexpr int TY = Geo<TYV>::TY, NW_CONSUMER = Geo<TYV>::NW_CONSUMER, NT_CONSUMER = Geo<TYV>::NT_CONSUMER,
                   BY = Geo<TYV>::BY, FIELD_BYTES = Geo<TYV>::FIELD_BYTES;
     using T = ModeTraits<MODE>;
-    constexpr int NS = T::STAGES;
+    constexpr int NS = L::STAGES;
     constexpr int NF = T::NF;
     constexpr bool DIAG = L::DIAG;                   // the diagonal is formed from the codes
     constexpr bool K1 = MODE == MODE_K1 || MODE == MODE_K1D;
-    constexpr bool K2 = MODE == MODE_K2 || MODE == MODE_K2M;        // K2M: the k2 of the merged solver, + r~.t
-    constexpr bool K2M = MODE == MODE_K2M;
+    constexpr bool K2M = MODE == MODE_K2M || MODE == MODE_K2MD;     // the k2 of the merged solver: + r~.t
+    constexpr bool K2 = MODE == MODE_K2 || MODE == MODE_K2D || K2M;
     constexpr bool K31 = MODE == MODE_K31 || MODE == MODE_K31D;     // the fused k3 + k1 of the merged solver
     constexpr bool RES = MODE == MODE_R0 || MODE == MODE_R1;
     static_assert(!DIAG || (!STORED && !CODE32), "the diagonal is formed from 2-bit codes");
@@ -308,15 +367,18 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     if (DIAG) {
         double* dtab = reinterpret_cast<double*>(smem + L::DTAB_OFF);
         dtab_addr = smem_u32(dtab);
-        for (int k = tid; k < 4096; k += blockDim.x) dtab[k] = diag_of_code12(ctab_s, (unsigned)k);
+        for (int k = tid; k < 4096; k += blockDim.x) {
+            const double a = diag_of_code12(ctab_s, (unsigned)k);
+            reinterpret_cast<double2*>(dtab)[k] = make_double2(a, recip_nb(a));
+        }
         __syncthreads();
     }
     pdl_wait();                                            // everything above is independent of the previous kernel
     constexpr int KIND = K1 ? PEND_K1 : (K2M ? PEND_K2M : (K2 ? PEND_K2 : (K31 ? PEND_K31 : (MODE == MODE_R0 ? PEND_INIT : PEND_TRUE))));
-    // plane k of the load sequence of work item `item` into stage sidx; the producer lane only
-    auto issue_plane = [&](int item, int k, unsigned sidx) {
-        const int tile = item % ntiles;
-        const int px = (tile % ntx) * TX, py = (tile / ntx) * TY, pz = (item / ntiles) * zchunk - 1 + k;
+    const int ntx = plan.ntx;
+    // plane k of the load sequence of the segment (tile, z0) into stage sidx; the producer lane only
+    auto issue_plane = [&](int tile, int z0, int k, unsigned sidx) {
+        const int px = (tile % ntx) * TX, py = (tile / ntx) * TY, pz = z0 - 1 + k;
         const unsigned st = sbase + sidx * (unsigned)L::STAGE_BYTES, bar = full_a + 8u * sidx;
         mbar_expect_tx(bar, L::TX_BYTES);
 #pragma unroll
@@ -327,10 +389,14 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     // The first stages do not depend on the scalars: they are requested before the block combines the previous
     // kernel's partial sums, so the loads fly while the scalar step is taken.
     int pre_issued = 0;
-    if (tid == NT_CONSUMER && (int)blockIdx.x < nitems) {
-        const int z0f = ((int)blockIdx.x / ntiles) * zchunk;
-        const int nqf = min(z0f + zchunk, g.nz) - z0f + 2;
-        for (; pre_issued < NS && pre_issued < nqf; ++pre_issued) issue_plane(blockIdx.x, pre_issued, (unsigned)pre_issued);
+    if (tid == NT_CONSUMER) {
+        SegIter<PERSIST> it0;
+        it0.init(plan, (int)blockIdx.x);
+        int tile_f, z0f, z1f;
+        if (it0.next(plan, g.nz, (int)blockIdx.x, (int)gridDim.x, tile_f, z0f, z1f)) {
+            const int nqf = z1f - z0f + 2;
+            for (; pre_issued < NS && pre_issued < nqf; ++pre_issued) issue_plane(tile_f, z0f, pre_issued, (unsigned)pre_issued);
+        }
     }
     if (!begin_kernel(KIND, S, sc_in, sc_out, rb, kv.hist, scratch)) {
         // the solve is over: let the requested stages land before the block's shared memory is released
@@ -367,21 +433,24 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     const int own_tile = (brow - 1) * TX + 2 * lane;               // element offset in an own-only box (main)
     const int pair_code = brow * BXC + CXO + 2 * lane;             // MODE_K1D: element offset in the code box with halo
 
-    for (int item = blockIdx.x; item < nitems; item += PERSIST ? (int)gridDim.x : nitems) {
-    const int tile = item % ntiles;
+    SegIter<PERSIST> seg;
+    seg.init(plan, (int)blockIdx.x);
+    int skip = pre_issued;                 // producer: planes of the first segment that are already requested
+    int tile, z0, z1;
+    while (seg.next(plan, g.nz, (int)blockIdx.x, (int)gridDim.x, tile, z0, z1)) {
     const int x0 = (tile % ntx) * TX, y0 = (tile / ntx) * TY;
-    const int z0 = (item / ntiles) * zchunk, z1 = min(z0 + zchunk, g.nz);
-    const int nq = z1 - z0 + 2;            // plane k of this item's load sequence is z0 - 1 + k
+    const int nq = z1 - z0 + 2;            // plane k of this segment's load sequence is z0 - 1 + k
 
     if (wid == NW_CONSUMER) {
         // ---- producer warp: one lane keeps the ring of stages filled ----------------------------
         if (lane == 0) {
-            for (int k = (item == (int)blockIdx.x ? pre_issued : 0); k < nq; ++k) {
+            for (int k = skip; k < nq; ++k) {
                 if (issued >= NS) mbar_wait(empty_a + 8u * cr.idx, cr.par ^ 1u);   // the consumers' release of the lap before
-                issue_plane(item, k, cr.idx);
+                issue_plane(tile, z0, k, cr.idx);
                 cr.next();
                 ++issued;
             }
+            skip = 0;
         }
         __syncwarp();
     } else {
@@ -398,36 +467,36 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
             const double* F3 = reinterpret_cast<const double*>(st + 3 * FIELD_BYTES);
             const double* F4 = reinterpret_cast<const double*>(st + 4 * FIELD_BYTES);
             double2 fr = *reinterpret_cast<const double2*>(F0 + pair_box), fp = make_double2(0, 0),
-                    fv = make_double2(0, 0), ft = make_double2(0, 0), fa;
+                    fv = make_double2(0, 0), ft = make_double2(0, 0), fa, frc = make_double2(1.0, 1.0);
             if (K1 || K31) {
                 fp = *reinterpret_cast<const double2*>(F1 + pair_box);
                 fv = *reinterpret_cast<const double2*>(F2 + pair_box);
                 if (K31) ft = *reinterpret_cast<const double2*>(F3 + pair_box);
-                if (DIAG) {
-                    const unsigned cw = *reinterpret_cast<const unsigned*>(st + L::CODE_OFF + 2 * pair_code);
-                    fa = make_double2(dtab_at(dtab_addr, cw, 0), dtab_at(dtab_addr, cw, 1));
-                } else {
-                    fa = *reinterpret_cast<const double2*>((K31 ? F4 : F3) + pair_box);
-                }
+                if (!DIAG) fa = *reinterpret_cast<const double2*>((K31 ? F4 : F3) + pair_box);
             } else if (K2) {
                 fv = *reinterpret_cast<const double2*>(F1 + pair_box);
-                fa = *reinterpret_cast<const double2*>(F2 + pair_box);
+                if (!DIAG) fa = *reinterpret_cast<const double2*>(F2 + pair_box);
             } else {
                 fa = *reinterpret_cast<const double2*>(F1 + pair_box);
             }
+            if (DIAG) {
+                const unsigned cw = *reinterpret_cast<const unsigned*>(st + L::CODE_OFF + 2 * pair_code);
+                dtab2_at(dtab_addr, cw, 0, fa.x, frc.x);
+                dtab2_at(dtab_addr, cw, 1, fa.y, frc.y);
+            }
             // the divisor of the branch-free division is tested once per solve, here (D4)
             if (MODE == MODE_R0 && PRECOND && ok) diag_bad |= DivRange::diag_bad(fa.x) | DivRange::diag_bad(fa.y);
-            if (!ok) fa = make_double2(1.0, 1.0);                       // zero-filled nodes: keep u finite (0/1)
+            if (!ok) { fa = make_double2(1.0, 1.0); frc = make_double2(1.0, 1.0); }   // zero-filled nodes: keep u finite (0/1)
             if (K31) {
                 // alpha, omega, beta from the block's copy of the scalars at every use: three shared loads per plane
                 // instead of six registers held through the loop (this kernel is the one short of registers)
                 const double al = S->alpha, om = S->omega, be = S->beta;
-                u[0] = u31_of<PRECOND>(fr.x, fp.x, fv.x, ft.x, fa.x, al, om, be, sx[0], rx[0], n[0], range);
-                u[1] = u31_of<PRECOND>(fr.y, fp.y, fv.y, ft.y, fa.y, al, om, be, sx[1], rx[1], n[1], range);
+                u[0] = u31_of<PRECOND, DIAG>(fr.x, fp.x, fv.x, ft.x, fa.x, frc.x, al, om, be, sx[0], rx[0], n[0], range);
+                u[1] = u31_of<PRECOND, DIAG>(fr.y, fp.y, fv.y, ft.y, fa.y, frc.y, al, om, be, sx[1], rx[1], n[1], range);
                 px[0] = fp.x; px[1] = fp.y;
             } else {
-                u[0] = u_of<MODE, PRECOND && !RES>(fr.x, fp.x, fv.x, fa.x, first, c1, c2, n[0], range);
-                u[1] = u_of<MODE, PRECOND && !RES>(fr.y, fp.y, fv.y, fa.y, first, c1, c2, n[1], range);
+                u[0] = u_of<MODE, PRECOND && !RES>(fr.x, fp.x, fv.x, fa.x, frc.x, first, c1, c2, n[0], range);
+                u[1] = u_of<MODE, PRECOND && !RES>(fr.y, fp.y, fv.y, fa.y, frc.y, first, c1, c2, n[1], range);
             }
             a[0] = fa.x; a[1] = fa.y;
         };
@@ -473,24 +542,22 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
                     const double* F2 = reinterpret_cast<const double*>(st + 2 * FIELD_BYTES);
                     const double* F3 = reinterpret_cast<const double*>(st + 3 * FIELD_BYTES);
                     const double* F4 = reinterpret_cast<const double*>(st + 4 * FIELD_BYTES);
-                    double hr = F0[col_box], hp = 0.0, hv = 0.0, ht = 0.0, ha;
+                    double hr = F0[col_box], hp = 0.0, hv = 0.0, ht = 0.0, ha = 1.0, hrc = 1.0;
                     if (K1 || K31) {
                         hp = F1[col_box]; hv = F2[col_box];
                         if (K31) ht = F3[col_box];
-                        if (DIAG) {
-                            const int hxc = (wid == TY ? 1 : BX - 2) + CXO - 2; // the code box starts CXO - 2 columns further left
-                            const unsigned cw = *reinterpret_cast<const unsigned short*>(st + L::CODE_OFF + 2 * ((1 + lane) * BXC + hxc));
-                            ha = dtab_at(dtab_addr, cw, 0);
-                        } else {
-                            ha = (K31 ? F4 : F3)[col_box];
-                        }
+                        if (!DIAG) ha = (K31 ? F4 : F3)[col_box];
                     }
-                    else if (K2) { hv = F1[col_box]; ha = F2[col_box]; }
-                    else ha = 1.0;
-                    if (!(col_ok && zin)) ha = 1.0;
+                    else if (K2) { hv = F1[col_box]; if (!DIAG) ha = F2[col_box]; }
+                    if (DIAG) {
+                        const int hxc = (wid == TY ? 1 : BX - 2) + CXO - 2;     // the code box starts CXO - 2 columns further left
+                        const unsigned cw = *reinterpret_cast<const unsigned short*>(st + L::CODE_OFF + 2 * ((1 + lane) * BXC + hxc));
+                        dtab2_at(dtab_addr, cw, 0, ha, hrc);
+                    }
+                    if (!(col_ok && zin)) { ha = 1.0; hrc = 1.0; }
                     double d0, d1, d2;
-                    if (K31) u_s[col_box] = u31_of<PRECOND>(hr, hp, hv, ht, ha, S->alpha, S->omega, S->beta, d0, d1, d2, range);
-                    else u_s[col_box] = u_of<MODE, PRECOND && !RES>(hr, hp, hv, ha, first, c1, c2, d0, range);
+                    if (K31) u_s[col_box] = u31_of<PRECOND, DIAG>(hr, hp, hv, ht, ha, hrc, S->alpha, S->omega, S->beta, d0, d1, d2, range);
+                    else u_s[col_box] = u_of<MODE, PRECOND && !RES>(hr, hp, hv, ha, hrc, first, c1, c2, d0, range);
                 }
                 __syncwarp();                                           // publish: this warp's part of plane k is written
                 if (lane == 0) { mbar_arrive(ready_a + 8u * ur.idx); mbar_arrive(empty_a + 8u * cr.idx); }
@@ -797,23 +864,72 @@ bool own_map(CUtensorMap* m, const double* base, const GridDims& g, int ty) {
     return make_map(m, base, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 8, g, g.nx, TX, ty);
 }
 
-// grid of work items (x tiles, y tiles, z chunks) for tiles of `ty` rows, and the chunk depth
-dim3 item_grid(const LaunchCtx& c, int ty, int* depth) {
-    const int tx = (c.g.nx + TX - 1) / TX, tyb = (c.g.ny + ty - 1) / ty;
-    const int chunks = choose_zchunks(c.g, tx * tyb, c.sm_count);
-    *depth = (c.g.nz + chunks - 1) / chunks;
-    return dim3(tx, tyb, (c.g.nz + *depth - 1) / *depth);
+// The decomposition of a launch for tiles of `ty` rows (SegPlan above): the equal-chunk plan, or the two-group plan
+// where its longest block is shorter by 3 % or more.  `persist`: blocks loop over segments (else one item per block).
+// Lengths are counted in plane steps, z1 - z0 + 2 per segment, which is what a block's time is proportional to.
+SegPlan plan_segments(const GridDims& g, int ty, int sm_count, bool persist, int mode_forced /* -1: choose */) {
+    SegPlan P;
+    std::memset(&P, 0, sizeof(P));
+    const int tx = (g.nx + TX - 1) / TX, tyb = (g.ny + ty - 1) / ty, T = tx * tyb;
+    P.ntx = tx; P.ntiles = T;
+    const int chunks0 = choose_zchunks(g, T, sm_count);
+    P.zchunk = (g.nz + chunks0 - 1) / chunks0;
+    const int chunks = (g.nz + P.zchunk - 1) / P.zchunk;
+    P.nitems = T * chunks;
+    P.blocks = persist ? std::min(sm_count, P.nitems) : P.nitems;
+    // (at least two whole layers in step: a plan whose rest group takes a large share of the volume gives up the
+    // sharing of halo rows in L2 between neighbouring tiles -- measured: K31 at 256^3 with 80 tiles, 0.233 -> 0.266 ms)
+    if (!persist || mode_forced == 0 || T * 2 > sm_count) return P;
+    // longest block of the equal-chunk plan
+    long long span0 = 0;
+    for (int b = 0; b < P.blocks; ++b) {
+        long long w = 0;
+        for (int i = b; i < P.nitems; i += P.blocks) {
+            const int z0 = (i / T) * P.zchunk;
+            w += std::min(P.zchunk, g.nz - z0) + 2;
+        }
+        span0 = std::max(span0, w);
+    }
+    // two-group plans: `full` layers of depth D in step, the rest flattened over the R remaining blocks
+    const int full = sm_count / T, R = sm_count - full * T;
+    long long best = -1; int bestD = 0, bestq = 0;
+    for (int D = 4; D * full <= g.nz; ++D) {
+        const int E = g.nz - D * full;
+        long long span = D + 2;
+        int q = 0;
+        if (E > 0) {
+            if (R == 0) continue;
+            q = (int)(((long long)T * E + R - 1) / R);
+            for (int r = 0; r < R; ++r) {
+                long long pos = (long long)r * q, end = std::min(pos + q, (long long)T * E), w = 0;
+                while (pos < end) {
+                    const long long zz = pos % E, len = std::min((long long)E - zz, end - pos);
+                    w += len + 2; pos += len;
+                }
+                span = std::max(span, w);
+            }
+        }
+        if (best < 0 || span < best) { best = span; bestD = D; bestq = q; }
+    }
+    if (best < 0 || (mode_forced != 1 && best * 100 > span0 * 97)) return P;
+    P.mode = 1; P.zchunk = bestD; P.nitems = T * full; P.zrest = bestD * full; P.erest = g.nz - P.zrest; P.q = bestq;
+    P.blocks = P.erest > 0 ? sm_count : P.nitems;
+    if (P.erest == 0) P.erest = 1;       // (never dereferenced: no rest block exists; keeps the divisions defined)
+    return P;
 }
 
 template <int MODE, bool PRECOND, bool STORED, bool CODE32, int TYV>
 void launch_geo(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaArgs& tm) {
-    int depth;
-    const dim3 grid = item_grid(c, TYV, &depth);
-    // grid = (x tiles, y tiles, z chunks) of work items; launched as min(#SMs, #items) persistent blocks
-    const int ntx = (int)grid.x, ntiles = (int)(grid.x * grid.y), nitems = ntiles * (int)grid.z;
     // The stored variant (six more arrays per node straight from global memory, no registers to spare for the
-    // item loop) keeps one item per block.
-    const int blocks = STORED ? nitems : std::min(c.sm_count, nitems);
+    // segment loop) keeps one item per block.  The plan of a grid is computed once per geometry and process.
+    static thread_local struct { GridDims g; int sm, forced; SegPlan P; bool valid; } cache = {};
+    if (!cache.valid || cache.g.nx != c.g.nx || cache.g.ny != c.g.ny || cache.g.nz != c.g.nz || cache.sm != c.sm_count ||
+        cache.forced != c.seg_mode) {
+        cache.P = plan_segments(c.g, TYV, c.sm_count, !STORED, c.seg_mode);
+        cache.g = c.g; cache.sm = c.sm_count; cache.forced = c.seg_mode; cache.valid = true;
+    }
+    const SegPlan& plan = cache.P;
+    const int blocks = plan.blocks;
     const Scalars* sc_in; Scalars* sc_out;
     c.next_scalars(sc_in, sc_out);
     using L = Layout<MODE, STORED, CODE32, TYV>;
@@ -826,7 +942,7 @@ void launch_geo(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, co
     }
     ++g_launch_count;
     note_launch(launch_pdl(c.pdl, kern, dim3(blocks), dim3(Geo<TYV>::NT), (size_t)L::TOTAL, c.stream, tm, c.g, op, kv, sc_in, sc_out,
-                           c.rb, depth, ntx, ntiles, nitems));
+                           c.rb, plan));
 }
 
 // ty: tile rows (TY_WIDE or TY_DEEP); the stored variant is compiled for the wide tiles only
@@ -839,7 +955,7 @@ void launch_inst(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, c
 template <int MODE>
 void launch_mode(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaArgs& tm, bool precond, int ty) {
     const bool c32 = op.code32 != 0;
-    constexpr bool MERGED = MODE == MODE_K2M || MODE == MODE_K31 || MODE == MODE_K31D;    // code form only
+    constexpr bool MERGED = MODE == MODE_K2M || MODE == MODE_K31 || MODE == MODE_K31D || MODE == MODE_K2MD;    // code form only
     if constexpr (!MERGED) {
         if (op.stored) {
             if (precond) launch_inst<MODE, true, true, false>(c, op, kv, tm, ty);
@@ -864,7 +980,7 @@ void launch_mode(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, c
 int tile_rows(const LaunchCtx& c, const Operator& op, int mode) {
     if (op.stored) return TY_WIDE;
     if (c.tile_rows == TY_WIDE || c.tile_rows == TY_DEEP) return c.tile_rows;
-    if (mode == MODE_K31 || mode == MODE_K31D || mode == MODE_K2M) return TY_DEEP;
+    if (mode == MODE_K31 || mode == MODE_K31D || mode == MODE_K2M || mode == MODE_K2MD) return TY_DEEP;
     return c.g.n <= 144ll * 144 * 144 ? TY_DEEP : TY_WIDE;
 }
 
@@ -879,6 +995,7 @@ struct TmaMaps {
 struct TmaSet {
     TmaMaps m[2];            // [0]: TY_WIDE, [1]: TY_DEEP
     bool have_code, have_codeh, have_merged;
+    bool k2_diag;            // k2 / K2M take the diagonal from the codes too (op.diag_code >= 2)
     const TmaMaps& of(int ty) const { return m[ty == TY_DEEP ? 1 : 0]; }
 };
 
@@ -903,6 +1020,7 @@ bool tma_set_build(TmaSet* t, const GridDims& g, const Operator& op, const Krylo
     bool ok = true;
     t->have_code = !op.stored;
     t->have_codeh = !op.stored && !op.code32 && op.diag_code;
+    t->k2_diag = op.diag_code >= 2;
     t->have_merged = kv.r_out && !op.stored && aligned16(kv.r_out);
     for (int k = 0; k < (op.stored ? 1 : 2) && ok; ++k) {
         TmaMaps& M = t->m[k];
@@ -922,6 +1040,12 @@ bool tma_set_build(TmaSet* t, const GridDims& g, const Operator& op, const Krylo
 }
 
 bool tma_merged_supported(const Operator& op) { return !op.stored; }
+
+void tma_plan(const GridDims& g, int tile_rows, int sm_count, int mode, int* out) {
+    const SegPlan P = plan_segments(g, tile_rows == TY_DEEP ? TY_DEEP : TY_WIDE, sm_count, true, mode);
+    out[0] = P.mode; out[1] = P.ntx; out[2] = P.ntiles; out[3] = P.zchunk; out[4] = P.nitems; out[5] = P.zrest;
+    out[6] = P.erest; out[7] = P.q; out[8] = P.blocks;
+}
 
 // precond: mode 0 of a preconditioned solve also tests the diagonal against the range of the branch-free division
 // that k1 and k2 will divide by it with (reading D4; the residual itself involves no division).
@@ -954,12 +1078,20 @@ void launch_k1_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv,
 }
 
 void launch_k2m_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond, int k) {
-    const int ty = tile_rows(c, op, MODE_K2M);
+    const bool diag = t->have_codeh && t->k2_diag;
+    const int ty = tile_rows(c, op, diag ? MODE_K2MD : MODE_K2M);
     const TmaMaps& M = t->of(ty);
     TmaArgs a;
     std::memset(&a, 0, sizeof(a));
     const int rb = k & 1, pb = rb ^ 1;
-    a.f[0] = rb ? M.r1 : M.r; a.f[1] = M.v[pb]; a.f[2] = M.a0; a.own = M.rt; a.code = M.code;
+    a.f[0] = rb ? M.r1 : M.r; a.f[1] = M.v[pb]; a.own = M.rt;
+    if (diag) {
+        a.code = M.codeh;
+        if (precond) launch_inst<MODE_K2MD, true, false, false>(c, op, kv, a, ty);
+        else         launch_inst<MODE_K2MD, false, false, false>(c, op, kv, a, ty);
+        return;
+    }
+    a.f[2] = M.a0; a.code = M.code;
     launch_mode<MODE_K2M>(c, op, kv, a, precond, ty);
 }
 
@@ -982,11 +1114,19 @@ void launch_k31_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv
 
 void launch_k2_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond,
                    int parity) {
-    const int ty = tile_rows(c, op, MODE_K2);
+    const bool diag = t->have_codeh && t->k2_diag;
+    const int ty = tile_rows(c, op, diag ? MODE_K2D : MODE_K2);
     const TmaMaps& M = t->of(ty);
     TmaArgs a;
     std::memset(&a, 0, sizeof(a));
-    a.f[0] = M.r; a.f[1] = M.v[parity ^ 1]; a.f[2] = M.a0; a.code = M.code;   // v' = the buffer k1 just wrote
+    a.f[0] = M.r; a.f[1] = M.v[parity ^ 1];                                   // v' = the buffer k1 just wrote
+    if (diag) {              // diagonal and reciprocal from the code table: A0 is not read
+        a.code = M.codeh;
+        if (precond) launch_inst<MODE_K2D, true, false, false>(c, op, kv, a, ty);
+        else         launch_inst<MODE_K2D, false, false, false>(c, op, kv, a, ty);
+        return;
+    }
+    a.f[2] = M.a0; a.code = M.code;
     launch_mode<MODE_K2>(c, op, kv, a, precond, ty);
 }
 

@@ -38,6 +38,7 @@ struct LaunchCtx {
     int device;       // CUDA device of the grid (per-device kernel attributes)
     int solver;       // 0: Table 3, three kernels per iteration; 1: merged recurrence, two (pf_krylov.cuh)
     int tile_rows;    // tiled family: 0 = chosen per kernel and grid, 13 or 16 = forced (PF_OPT_TILE_ROWS)
+    int seg_mode;     // tiled family: -1 = decomposition chosen per grid, 0 = equal chunks, 1 = two groups (PF_OPT_SEGMENTS)
     bool pdl;         // programmatic dependent launch allowed
     // the next kernel reads sc[*flip] and its block 0 writes sc[*flip ^ 1]
     void next_scalars(const Scalars*& in, Scalars*& out) const { in = sc[*flip]; out = sc[*flip ^ 1]; *flip ^= 1; }
@@ -86,6 +87,9 @@ void launch_k2_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv,
 // (buffer 0 = the pointers of the KrylovVecs the set was built from, buffer 1 = its r_out, p_out, v_out).
 void launch_k2m_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond, int k);
 void launch_k31_tma(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaSet* t, bool precond, int k);
+// The decomposition the persistent tiled kernels use on a device with sm_count SMs (SegPlan of pf_krylov_tma.cu; host
+// arithmetic only): out[9] = mode, x tiles, tiles, chunk / layer depth, items / main blocks, zrest, erest, q, blocks.
+void tma_plan(const GridDims& g, int tile_rows, int sm_count, int mode, int* out);
 // Whether the tiled family has the merged kernels for this operator (code form; the stored variant uses the direct ones).
 bool tma_merged_supported(const Operator& op);
 bool tma_merged_ok(const TmaSet* t);             // the set just built holds the maps of the merged kernels

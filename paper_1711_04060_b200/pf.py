@@ -24,7 +24,7 @@ PF_BC_DIRICHLET, PF_BC_NEUMANN = 0, 1
 (PF_OPT_STENCIL, PF_OPT_OMEGA_PF, PF_OPT_LINEAR_TOL, PF_OPT_LINEAR_MAXIT, PF_OPT_CHECK_INTERVAL,
  PF_OPT_WATER_MOLAR, PF_OPT_MAX_OUTER, PF_OPT_PRECOND, PF_OPT_HISTORY, PF_OPT_KERNELS, PF_OPT_PROFILE,
  PF_OPT_GRAPH, PF_OPT_NORM, PF_OPT_CHARGE_MODEL, PF_OPT_DIAG_FROM_CODE, PF_OPT_SOLVER, PF_OPT_STERIC_MODE,
- PF_OPT_TILE_ROWS) = range(1, 19)
+ PF_OPT_TILE_ROWS, PF_OPT_SEGMENTS) = range(1, 20)
 STERIC_SIMULTANEOUS, STERIC_LAGGED = 0, 1
 SOLVER_TABLE3, SOLVER_MERGED = 0, 1
 CHARGES_DEPOSITED, CHARGES_SINGULAR = 0, 1
@@ -36,7 +36,7 @@ EXPORTS = [
     "pf_grid_create", "pf_grid_set_fixed_nodes", "pf_grid_workspace_bytes", "pf_grid_set_workspace", "pf_grid_set_option",
     "pf_solve_linear", "pf_solve_linear_host", "pf_grid_stage_host", "pf_solve_pf", "pf_fermi_pointwise", "pf_grid_history",
     "pf_grid_linear_iters", "pf_grid_increments", "pf_grid_fault_repeats", "pf_grid_laplace_iters", "pf_grid_stencil", "pf_grid_palette_size", "pf_grid_code_layout", "pf_grid_copy_array",
-    "pf_grid_profile", "pf_launch_count", "pf_coop_plan", "pf_grid_relax", "pf_relax_noalloc", "pf_grid_destroy", "pf_last_error", "pf_version",
+    "pf_grid_profile", "pf_launch_count", "pf_coop_plan", "pf_tile_plan", "pf_grid_relax", "pf_relax_noalloc", "pf_grid_destroy", "pf_last_error", "pf_version",
 ]
 
 
@@ -95,6 +95,7 @@ def load():
     L.pf_grid_profile.argtypes = [_vp, _dp, ctypes.POINTER(ctypes.c_longlong)]
     L.pf_launch_count.restype = ctypes.c_longlong
     L.pf_coop_plan.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_size_t, _ip]
+    L.pf_tile_plan.argtypes = [ctypes.c_int] * 6 + [_ip]
     L.pf_grid_destroy.argtypes = [_vp]
     L.pf_grid_destroy.restype = None
     L.pf_last_error.argtypes = [_vp]
@@ -258,6 +259,16 @@ def pf_coop_plan(nx: int, ny: int, nz: int, max_blocks: int = 148, smem_cap: int
     if load().pf_coop_plan(nx, ny, nz, max_blocks, smem_cap, out) != PF_OK:
         return None
     keys = ("nbx", "nby", "nbz", "vmax", "hmax", "nhmax", "threads", "smem")
+    return dict(zip(keys, list(out)))
+
+
+def pf_tile_plan(nx: int, ny: int, nz: int, tile_rows: int, sm_count: int = 148, mode: int = -1) -> dict:
+    """Decomposition of the persistent tiled kernels (host arithmetic only; include/pf_debug.h)."""
+    out = (ctypes.c_int * 9)()
+    rc = load().pf_tile_plan(nx, ny, nz, tile_rows, sm_count, mode, out)
+    if rc != PF_OK:
+        raise PFError(rc, "pf_tile_plan: invalid argument")
+    keys = ("mode", "ntx", "ntiles", "depth", "nitems", "zrest", "erest", "q", "blocks")
     return dict(zip(keys, list(out)))
 
 

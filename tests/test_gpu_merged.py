@@ -212,3 +212,30 @@ def test_both_tile_geometries_equal_direct(pf, rows, solver):
             assert a["status"] == b["status"] and a["iters"] == b["iters"]
             assert torch.equal(a["x"], b["x"]) and np.array_equal(a["hist"], b["hist"])
             assert a["true_relres"] == b["true_relres"]
+
+
+@pytest.mark.parametrize("solver", [0, 1])
+def test_segment_plans_and_k2_diagonal_table_equal_direct(pf, solver):
+    """PF_OPT_SEGMENTS (how tiles x z ranges are handed to the persistent blocks) and PF_OPT_DIAG_FROM_CODE = 2 (k2 / K2M
+    take the diagonal and the divisor's half of the Jacobi division from the code table as k1 / K31 do) change no bit:
+    forced either way the tiled kernels give the iterates of the direct kernels, on shapes where the two-group plan
+    exists (several layers, a rest group of one to a few blocks with segments that cross tiles) and where it does not."""
+    for shape in ((64, 29, 200), (130, 33, 96), (66, 53, 40), (128, 64, 61)):
+        nx, ny, nz = shape
+        w = ragged_workload(nx=nx, ny=ny, nz=nz, seed=5 + nz)
+        ref = None
+        for kernels, seg, diag, rows in ((pf.KERNELS_DIRECT, -1, 1, 0), (pf.KERNELS_TILED, 0, 1, 0), (pf.KERNELS_TILED, 1, 1, 0),
+                                         (pf.KERNELS_TILED, 1, 2, 16), (pf.KERNELS_TILED, 0, 2, 13), (pf.KERNELS_TILED, -1, 2, 0),
+                                         (pf.KERNELS_TILED, 1, 0, 13)):
+            g = pf.Grid.from_workload(w, stencil=2, kernels=kernels,
+                                      options={pf.PF_OPT_SOLVER: solver, pf.PF_OPT_SEGMENTS: seg, pf.PF_OPT_TILE_ROWS: rows,
+                                               pf.PF_OPT_DIAG_FROM_CODE: diag, pf.PF_OPT_HISTORY: 256})
+            o = g.solve_linear(w.rhs, tol=1e-10, maxit=120)
+            o["hist"] = g.history(256)
+            assert pf.pf_grid_fault_repeats(g.handle) == 0
+            g.close()
+            if ref is None:
+                ref = o
+                continue
+            assert o["status"] == ref["status"] and o["iters"] == ref["iters"], (shape, seg, diag, rows)
+            assert torch.equal(o["x"], ref["x"]) and np.array_equal(o["hist"], ref["hist"]), (shape, seg, diag, rows)
