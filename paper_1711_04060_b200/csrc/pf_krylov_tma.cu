@@ -147,7 +147,11 @@ struct Layout {
                          OWN_BYTES = Geo<TYV>::OWN_BYTES;
     static constexpr bool DIAG = MODE == MODE_K1D || MODE == MODE_K31D || MODE == MODE_K2D || MODE == MODE_K2MD;
     // (the wide K31D, which no policy picks, makes room for the table with a stage less)
-    static constexpr int STAGES = (MODE == MODE_K31D && TYV == 16) ? 2 : T::STAGES;
+    // k1 on the deep tiles has room for a fourth stage (measured at 256^3, same box: k1 0.152 -> 0.142 ms with it, against
+    // 0.150 on the wide tiles; a fifth stage for k2 / K2M changes nothing)
+    static constexpr int STAGES = (MODE == MODE_K31D && TYV == 16) ? 2
+        : ((MODE == MODE_K1 || MODE == MODE_K1D) && TYV == 13 && !STORED) ? 4
+        : T::STAGES;
     static constexpr int CODE_TX = DIAG ? BXC * BY * 2 : TX * TY * (CODE32 ? 4 : 2);   // bytes the TMA unit delivers
     static constexpr int CODE_BYTES = STORED ? 0 : ((CODE_TX + 127) / 128) * 128;
     static constexpr int STAGE_BYTES = T::NF * FIELD_BYTES + (T::OWN ? OWN_BYTES : 0) + CODE_BYTES;
@@ -981,6 +985,12 @@ int tile_rows(const LaunchCtx& c, const Operator& op, int mode) {
     if (op.stored) return TY_WIDE;
     if (c.tile_rows == TY_WIDE || c.tile_rows == TY_DEEP) return c.tile_rows;
     if (mode == MODE_K31 || mode == MODE_K31D || mode == MODE_K2M || mode == MODE_K2MD) return TY_DEEP;
+    // k1 with the diagonal read from memory (PF1, PF2, sigma: four halo operands) spills at 96 registers: measured with
+    // a sigma diagonal, 16 against 13 rows: 0.182 / 0.166 ms at 256^3, 0.085 / 0.075 at 192^3, 1.62 / 1.27 at 512^3
+    if (mode == MODE_K1) return TY_DEEP;
+    // ... and k1 of the Poisson solves (diagonal from the codes) has room for a fourth stage on the deep tiles: 16 against
+    // 13 rows 0.149 / 0.142 ms at 256^3, 0.069 / 0.067 at 192^3, 1.22 / 1.07 at 512^3
+    if (mode == MODE_K1D) return TY_DEEP;
     return c.g.n <= 144ll * 144 * 144 ? TY_DEEP : TY_WIDE;
 }
 
