@@ -139,9 +139,12 @@ typedef struct { double x, y, z, q; } pf_charge; /* position in Angstrom (node 0
 
 #define PF_OPT_SEGMENTS       19  /* tiled kernels: how tiles x z ranges are handed to the persistent blocks.  -1 (default):
                                      chosen per grid; 0: z cut into equal chunks, blocks take (tile, chunk) items
-                                     round-robin; 1: for grids with fewer tiles than SMs, whole layers in step on most
-                                     SMs and the remaining planes split evenly over the other SMs.  Same bits either
-                                     way; a tuning and measurement knob. */
+                                     round-robin; 1: for grids with at most half as many tiles as SMs, whole layers in step
+                                     on most SMs and the remaining planes split evenly over the other SMs; 2: for grids
+                                     with between half and two thirds as many tiles as SMs, a deep lower layer on one
+                                     block per tile, the upper layer of as many tiles as blocks are left, and the upper
+                                     layer of the other tiles in pieces afterwards.  A forced plan that does not exist
+                                     for the grid falls back to 0.  Same bits either way; a tuning and measurement knob. */
 
 /* Create a grid: store geometry and boundary conditions, scan eps_map for its palette of distinct
  * values, keep a device copy of the charges.  Assembly itself runs in pf_grid_set_workspace.

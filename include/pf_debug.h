@@ -51,7 +51,10 @@ int pf_coop_plan(int nx, int ny, int nz, int max_blocks, size_t smem_cap, int *o
  * launched.  Block b works on: mode 0 -- items b, b + blocks, ... with item i = tile i % tiles, planes
  * [(i / tiles) * depth, min(+ depth, nz)); mode 1, b < main -- tile b % tiles, planes [(b / tiles) * depth, + depth);
  * mode 1, rest block r = b - main -- positions [r q, min((r + 1) q, tiles * erest)), position p = tile p / erest, plane
- * zrest + p % erest, cut into one segment per tile.  Returns PF_OK or PF_ERR_ARG. */
+ * zrest + p % erest, cut into one segment per tile.  Mode 2 (out[3] = depth of the lower layer, out[4] = tiles, zrest =
+ * that depth, erest = nz - zrest, q = pieces): block b < tiles -- tile b, planes [0, depth); block b >= tiles, r = b -
+ * tiles, R = blocks - tiles, L = tiles - R -- first tile r, planes [zrest, nz), then, if r < L q, tile R + r % L, planes
+ * [zrest + (r / L) dp, min(+ dp, nz)) with dp = ceil(erest / q).  Returns PF_OK or PF_ERR_ARG. */
 int pf_tile_plan(int nx, int ny, int nz, int tile_rows, int sm_count, int mode, int *out);
 
 /* Introspection used by the tests: 1 = stored, 2 = on-the-fly; number of palette entries. */

@@ -896,7 +896,7 @@ int pf_grid_set_option(pf_grid* g, int key, double value) {
             }
             g->opt_tile_rows = iv; return PF_OK;
         case PF_OPT_SEGMENTS:
-            if (iv < -1 || iv > 1) return fail(g, PF_ERR_ARG, "segments must be -1 (auto), 0 (equal chunks) or 1 (two groups)");
+            if (iv < -1 || iv > 2) return fail(g, PF_ERR_ARG, "segments must be -1 (auto), 0 (equal chunks), 1 (layers + rest) or 2 (two layers + pieces)");
             if (iv != g->opt_seg_mode) {           // cached graphs hold launches of the other decomposition
                 cudaStreamSynchronize(g->stream);
                 for (auto& cg : g->graphs) cudaGraphExecDestroy(cg.exec);
@@ -1248,7 +1248,7 @@ int pf_coop_plan(int nx, int ny, int nz, int max_blocks, size_t smem_cap, int* o
 }
 
 int pf_tile_plan(int nx, int ny, int nz, int tile_rows, int sm_count, int mode, int* out) {
-    if (!out || nx < 1 || ny < 1 || nz < 1 || sm_count < 1 || (tile_rows != 13 && tile_rows != 16) || mode < -1 || mode > 1)
+    if (!out || nx < 1 || ny < 1 || nz < 1 || sm_count < 1 || (tile_rows != 13 && tile_rows != 16) || mode < -1 || mode > 2)
         return PF_ERR_ARG;
     GridDims gd;
     gd.nx = nx; gd.ny = ny; gd.nz = nz; gd.n = (long long)nx * ny * nz;

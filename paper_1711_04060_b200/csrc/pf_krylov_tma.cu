@@ -88,10 +88,17 @@ constexpr int BXC = TX + 2 * CXO;        // box to start on a 16-byte boundary o
 //           `full` = #SMs / ntiles layers of `zchunk` planes are taken by ntiles * full blocks, one segment each, all
 //           in step; the remaining planes z >= zrest of all tiles, flattened tile-major, are split evenly over the
 //           remaining blocks (a few short segments each).  256^3: 114 steps.
+//   mode 2  for grids with more tiles than half the SMs but fewer than two thirds (256^3 with 13-row tiles: 80 tiles, 6
+//           rounds of 26 steps = 156 against 138 of the volume): every tile's planes [0, zchunk) on one block each
+//           (group A, in step); the planes above on the other R = #SMs - tiles blocks for the first R tiles (group B, in
+//           step, shallower); the same planes of the remaining tiles, cut into q pieces along z, are taken by group B's
+//           blocks when they are done (piece j of all these tiles by consecutive blocks, in step).  256^3: 143 steps.
 struct SegPlan {
     int mode, ntx, ntiles;
-    int zchunk, nitems;       // mode 0: chunk depth and tiles * chunks; mode 1: layer depth of the main group, nmain
+    int zchunk, nitems;       // mode 0: chunk depth and tiles * chunks; mode 1: layer depth of the main group, nmain;
+                              // mode 2: depth of group A's layer, tiles
     int zrest, erest, q;      // mode 1: the rest group's planes [zrest, zrest + erest), q flattened positions per block
+                              // mode 2: the upper layer [zrest, zrest + erest), q pieces per leftover tile
     int blocks;               // host: blocks to launch
 };
 // The segments of block b, one after the other (every thread of the block walks the same sequence).  PERSIST = false:
@@ -99,14 +106,28 @@ struct SegPlan {
 template <bool PERSIST>
 struct SegIter {
     int pos, end;
-    __device__ __forceinline__ void init(const SegPlan& P, int b) {
-        if (PERSIST && P.mode == 1 && b >= P.nitems) { pos = (b - P.nitems) * P.q; end = min(pos + P.q, P.ntiles * P.erest); }
+    __device__ __forceinline__ void init(const SegPlan& P, int b, int nblocks) {
+        if (PERSIST && P.mode == 2) {
+            // group A: one segment; group B block r: its own upper layer, then piece r / L of leftover tile R + r % L
+            const int R = nblocks - P.ntiles, L = P.ntiles - R;
+            pos = 0; end = b < P.ntiles ? 1 : ((b - P.ntiles) < L * P.q ? 2 : 1);
+        }
+        else if (PERSIST && P.mode == 1 && b >= P.nitems) { pos = (b - P.nitems) * P.q; end = min(pos + P.q, P.ntiles * P.erest); }
         else if (PERSIST && P.mode == 1) { pos = b; end = b + 1; }
         else { pos = b; end = PERSIST ? P.nitems : min(b + 1, P.nitems); }
     }
     __device__ __forceinline__ bool next(const SegPlan& P, int nz, int b, int nblocks, int& tile, int& z0, int& z1) {
         if (pos >= end) return false;
-        if (PERSIST && P.mode == 1 && b >= P.nitems) {          // rest group: flattened positions, one segment per tile
+        if (PERSIST && P.mode == 2) {
+            if (b < P.ntiles) { tile = b; z0 = 0; z1 = P.zchunk; }
+            else if (pos == 0) { tile = b - P.ntiles; z0 = P.zrest; z1 = nz; }
+            else {
+                const int R = nblocks - P.ntiles, L = P.ntiles - R, r = b - P.ntiles, dp = (P.erest + P.q - 1) / P.q;
+                tile = R + r % L;
+                z0 = P.zrest + (r / L) * dp; z1 = min(z0 + dp, nz);
+            }
+            ++pos;
+        } else if (PERSIST && P.mode == 1 && b >= P.nitems) {   // rest group: flattened positions, one segment per tile
             tile = pos / P.erest;
             const int zz = pos - tile * P.erest, len = min(P.erest - zz, end - pos);
             z0 = P.zrest + zz; z1 = z0 + len; pos += len;
@@ -395,7 +416,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     int pre_issued = 0;
     if (tid == NT_CONSUMER) {
         SegIter<PERSIST> it0;
-        it0.init(plan, (int)blockIdx.x);
+        it0.init(plan, (int)blockIdx.x, (int)gridDim.x);
         int tile_f, z0f, z1f;
         if (it0.next(plan, g.nz, (int)blockIdx.x, (int)gridDim.x, tile_f, z0f, z1f)) {
             const int nqf = z1f - z0f + 2;
@@ -438,7 +459,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     const int pair_code = brow * BXC + CXO + 2 * lane;             // MODE_K1D: element offset in the code box with halo
 
     SegIter<PERSIST> seg;
-    seg.init(plan, (int)blockIdx.x);
+    seg.init(plan, (int)blockIdx.x, (int)gridDim.x);
     int skip = pre_issued;                 // producer: planes of the first segment that are already requested
     int tile, z0, z1;
     while (seg.next(plan, g.nz, (int)blockIdx.x, (int)gridDim.x, tile, z0, z1)) {
@@ -881,9 +902,7 @@ SegPlan plan_segments(const GridDims& g, int ty, int sm_count, bool persist, int
     const int chunks = (g.nz + P.zchunk - 1) / P.zchunk;
     P.nitems = T * chunks;
     P.blocks = persist ? std::min(sm_count, P.nitems) : P.nitems;
-    // (at least two whole layers in step: a plan whose rest group takes a large share of the volume gives up the
-    // sharing of halo rows in L2 between neighbouring tiles -- measured: K31 at 256^3 with 80 tiles, 0.233 -> 0.266 ms)
-    if (!persist || mode_forced == 0 || T * 2 > sm_count) return P;
+    if (!persist || mode_forced == 0 || T >= sm_count) return P;
     // longest block of the equal-chunk plan
     long long span0 = 0;
     for (int b = 0; b < P.blocks; ++b) {
@@ -894,8 +913,27 @@ SegPlan plan_segments(const GridDims& g, int ty, int sm_count, bool persist, int
         }
         span0 = std::max(span0, w);
     }
-    // two-group plans: `full` layers of depth D in step, the rest flattened over the R remaining blocks
     const int full = sm_count / T, R = sm_count - full * T;
+    if (full == 1) {
+        // Mode 2.  (A plan like mode 1 with ONE layer in step, whose rest group takes almost half of the volume tile by
+        // tile, gives up the sharing of halo rows in L2 between neighbouring tiles -- measured: K31 at 256^3 with 80
+        // tiles, 0.233 -> 0.266 ms -- so here every group marches neighbouring tiles in step.)
+        const int L = T - R;                       // tiles whose upper layer waits for group B
+        if (mode_forced == 1 || L <= 0 || R / L < 1) return P;
+        const int pieces = std::min(R / L, 8);
+        long long best = -1; int bestD = 0;
+        for (int D = (g.nz + 1) / 2; D < g.nz - 4; ++D) {
+            const int E = g.nz - D, dp = (E + pieces - 1) / pieces;
+            if (dp < 4) break;
+            const long long span = std::max<long long>(D + 2, (E + 2) + (dp + 2));
+            if (best < 0 || span < best) { best = span; bestD = D; }
+        }
+        if (best < 0 || (mode_forced != 2 && best * 100 > span0 * 97)) return P;
+        P.mode = 2; P.zchunk = bestD; P.nitems = T; P.zrest = bestD; P.erest = g.nz - bestD; P.q = pieces; P.blocks = sm_count;
+        return P;
+    }
+    if (mode_forced == 2) return P;
+    // two-group plans: `full` layers of depth D in step, the rest flattened over the R remaining blocks
     long long best = -1; int bestD = 0, bestq = 0;
     for (int D = 4; D * full <= g.nz; ++D) {
         const int E = g.nz - D * full;
@@ -976,22 +1014,18 @@ void launch_mode(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, c
     }
 }
 
-// Tile rows of a launch.  Measured on one B200, same box, boost clock (profiles/r2_tiles.md): the deep tiles (16 warps,
-// 128 registers, no spills) win for both kernels of the merged solver at every size (K31 -8 to -16 %, K2M -2 to -11 %)
-// and for the Table-3 kernels up to about 140^3, where a launch takes a few tens of microseconds and the fixed costs of
-// a block count (k1 -6 % at 128^3); from 160^3 on the wide tiles win for k1 (fewer halo rows per tile row: 0.155
-// against 0.161 ms at 256^3) and k2 does not care.  c.tile_rows != 0 forces one geometry (PF_OPT_TILE_ROWS).
+// Tile rows of a launch.  Measured on one B200 (profiles/r2_tiles.md, r2_plans.md): the deep tiles (16 warps, 128
+// registers, no spills) win for both kernels of the merged solver at every size (K31 -8 to -16 %, K2M -2 to -11 %); for k1
+// since it has a fourth stage there (k1 with the diagonal from the codes 0.149 -> 0.142 ms at 256^3, 1.22 -> 1.07 at
+// 512^3; with the diagonal read, where the wide kernel spills, 0.182 -> 0.157 at 256^3, 1.62 -> 1.27 at 512^3); and for
+// k2 at every size once the decomposition of mode 2 exists (256^3: 0.112 wide with the plan of mode 1, 0.109 deep;
+// 192^3: 0.053 / 0.051; 512^3: equal).  So operators in code form run on the deep tiles; the wide ones serve the
+// stored variant (only geometry compiled for it).  c.tile_rows != 0 forces one geometry (PF_OPT_TILE_ROWS).
 int tile_rows(const LaunchCtx& c, const Operator& op, int mode) {
+    (void)mode;
     if (op.stored) return TY_WIDE;
     if (c.tile_rows == TY_WIDE || c.tile_rows == TY_DEEP) return c.tile_rows;
-    if (mode == MODE_K31 || mode == MODE_K31D || mode == MODE_K2M || mode == MODE_K2MD) return TY_DEEP;
-    // k1 with the diagonal read from memory (PF1, PF2, sigma: four halo operands) spills at 96 registers: measured with
-    // a sigma diagonal, 16 against 13 rows: 0.182 / 0.166 ms at 256^3, 0.085 / 0.075 at 192^3, 1.62 / 1.27 at 512^3
-    if (mode == MODE_K1) return TY_DEEP;
-    // ... and k1 of the Poisson solves (diagonal from the codes) has room for a fourth stage on the deep tiles: 16 against
-    // 13 rows 0.149 / 0.142 ms at 256^3, 0.069 / 0.067 at 192^3, 1.22 / 1.07 at 512^3
-    if (mode == MODE_K1D) return TY_DEEP;
-    return c.g.n <= 144ll * 144 * 144 ? TY_DEEP : TY_WIDE;
+    return TY_DEEP;
 }
 
 }  // namespace

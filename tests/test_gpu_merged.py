@@ -220,13 +220,14 @@ def test_segment_plans_and_k2_diagonal_table_equal_direct(pf, solver):
     take the diagonal and the divisor's half of the Jacobi division from the code table as k1 / K31 do) change no bit:
     forced either way the tiled kernels give the iterates of the direct kernels, on shapes where the two-group plan
     exists (several layers, a rest group of one to a few blocks with segments that cross tiles) and where it does not."""
-    for shape in ((64, 29, 200), (130, 33, 96), (66, 53, 40), (128, 64, 61)):
+    for shape in ((64, 29, 200), (130, 33, 96), (66, 53, 40), (128, 64, 61), (320, 208, 40)):
         nx, ny, nz = shape
         w = ragged_workload(nx=nx, ny=ny, nz=nz, seed=5 + nz)
         ref = None
+        # (320 x 208 x 40 on 148 SMs: 80 tiles of 13 rows -- the plan of mode 2; 65 tiles of 16 rows -- mode 1)
         for kernels, seg, diag, rows in ((pf.KERNELS_DIRECT, -1, 1, 0), (pf.KERNELS_TILED, 0, 1, 0), (pf.KERNELS_TILED, 1, 1, 0),
                                          (pf.KERNELS_TILED, 1, 2, 16), (pf.KERNELS_TILED, 0, 2, 13), (pf.KERNELS_TILED, -1, 2, 0),
-                                         (pf.KERNELS_TILED, 1, 0, 13)):
+                                         (pf.KERNELS_TILED, 1, 0, 13), (pf.KERNELS_TILED, 2, 1, 13), (pf.KERNELS_TILED, 2, 2, 0)):
             g = pf.Grid.from_workload(w, stencil=2, kernels=kernels,
                                       options={pf.PF_OPT_SOLVER: solver, pf.PF_OPT_SEGMENTS: seg, pf.PF_OPT_TILE_ROWS: rows,
                                                pf.PF_OPT_DIAG_FROM_CODE: diag, pf.PF_OPT_HISTORY: 256})

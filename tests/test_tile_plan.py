@@ -20,6 +20,18 @@ def segments(p, nz):
             for i in range(b, p["nitems"], p["blocks"]):
                 z0 = (i // p["ntiles"]) * p["depth"]
                 segs.append((i % p["ntiles"], z0, min(z0 + p["depth"], nz)))
+        elif p["mode"] == 2:
+            T = p["ntiles"]
+            R, r = p["blocks"] - T, b - T
+            L = T - R
+            if b < T:
+                segs.append((b, 0, p["depth"]))
+            else:
+                segs.append((r, p["zrest"], nz))
+                if r < L * p["q"]:
+                    dp = -(-p["erest"] // p["q"])
+                    z0 = p["zrest"] + (r // L) * dp
+                    segs.append((R + r % L, z0, min(z0 + dp, nz)))
         elif b < p["nitems"]:
             z0 = (b // p["ntiles"]) * p["depth"]
             segs.append((b % p["ntiles"], z0, min(z0 + p["depth"], p["zrest"])))
@@ -40,18 +52,21 @@ def longest(segs):
 
 
 SHAPES = [(256, 256, 256), (128, 128, 128), (160, 160, 160), (192, 192, 192), (144, 144, 144), (512, 512, 512),
-          (64, 29, 200), (130, 33, 96), (66, 53, 40), (64, 16, 8), (96, 100, 77), (255 + 1, 255, 255), (320, 64, 300)]
+          (64, 29, 200), (130, 33, 96), (66, 53, 40), (64, 16, 8), (96, 100, 77), (255 + 1, 255, 255), (320, 64, 300),
+          (320, 208, 90), (256, 300, 64), (64, 52, 40)]
 
 
 @pytest.mark.parametrize("rows", [13, 16])
-@pytest.mark.parametrize("mode", [-1, 0, 1])
+@pytest.mark.parametrize("mode", [-1, 0, 1, 2])
 @pytest.mark.parametrize("sms", [148, 132, 7])
 def test_plan_covers_every_tile_plane_once(rows, mode, sms):
     for nx, ny, nz in SHAPES:
         p = pf.pf_tile_plan(nx, ny, nz, rows, sms, mode)
         ntx, nty = -(-nx // TX), -(-ny // rows)
         assert p["ntx"] == ntx and p["ntiles"] == ntx * nty
-        assert 1 <= p["blocks"] <= max(sms, 1) and p["mode"] in (0, 1)
+        assert 1 <= p["blocks"] <= max(sms, 1) and p["mode"] in (0, 1, 2)
+        if mode in (1, 2):
+            assert p["mode"] in (0, mode)
         if mode == 0:
             assert p["mode"] == 0
         segs = segments(p, nz)
@@ -63,6 +78,12 @@ def test_plan_covers_every_tile_plane_once(rows, mode, sms):
                     assert (tile, z) not in cover, (nx, ny, nz, tile, z)
                     cover[(tile, z)] = 1
         assert len(cover) == p["ntiles"] * nz
+        if p["mode"] == 2:
+            # one block per tile for the lower layer; the other blocks start with the upper layer of one tile each
+            T = p["ntiles"]
+            assert p["blocks"] == sms and T < sms < 2 * T
+            assert all(s == [(b, 0, p["depth"])] for b, s in enumerate(segs[:T]))
+            assert all(s[0] == (r, p["zrest"], nz) for r, s in enumerate(segs[T:]))
         if p["mode"] == 1:
             # whole layers on tiles * full blocks, in step: equal depth, one segment each
             main = [s for s in segs[:p["nitems"]]]
@@ -80,9 +101,13 @@ def test_two_group_plan_is_chosen_only_where_it_is_shorter():
     assert l0 == 124 and l1 <= 0.97 * l0 and l1 >= 256 * 64 / 148
     # more tiles than half the SMs (512^3; 13-row tiles at 256^3): equal chunks
     assert pf.pf_tile_plan(512, 512, 512, 16, 148, -1)["mode"] == 0
-    assert pf.pf_tile_plan(256, 256, 256, 13, 148, -1)["mode"] == 0
+    # 256^3 with 13-row tiles: 80 tiles, 11 chunks in 6 rounds = 156 steps against a lower layer on 80 blocks, the upper
+    # layer of 68 tiles on the other 68 and the upper layer of the last 12 tiles in 5 pieces afterwards
+    deep = pf.pf_tile_plan(256, 256, 256, 13, 148, -1)
+    assert deep["mode"] == 2 and longest(segments(pf.pf_tile_plan(256, 256, 256, 13, 148, 0), 256)) == 156
+    assert longest(segments(deep, 256)) <= 146
     for shape in SHAPES:
         for rows in (13, 16):
             a, e = pf.pf_tile_plan(*shape, rows, 148, -1), pf.pf_tile_plan(*shape, rows, 148, 0)
-            if a["mode"] == 1:
+            if a["mode"] != 0:
                 assert longest(segments(a, shape[2])) <= 0.97 * longest(segments(e, shape[2]))
