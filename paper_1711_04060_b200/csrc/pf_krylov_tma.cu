@@ -109,8 +109,8 @@ struct SegIter {
     __device__ __forceinline__ void init(const SegPlan& P, int b, int nblocks) {
         if (PERSIST && P.mode == 2) {
             // group A: one segment; group B block r: its own upper layer, then piece r / L of leftover tile R + r % L
-            const int R = nblocks - P.ntiles, L = P.ntiles - R;
-            pos = 0; end = b < P.ntiles ? 1 : ((b - P.ntiles) < L * P.q ? 2 : 1);
+            const int R = nblocks - P.ntiles, L = P.ntiles - R, r = b - P.ntiles, dp = (P.erest + P.q - 1) / P.q;
+            pos = 0; end = (b >= P.ntiles && r < L * P.q && (r / L) * dp < P.erest) ? 2 : 1;
         }
         else if (PERSIST && P.mode == 1 && b >= P.nitems) { pos = (b - P.nitems) * P.q; end = min(pos + P.q, P.ntiles * P.erest); }
         else if (PERSIST && P.mode == 1) { pos = b; end = b + 1; }
@@ -921,15 +921,18 @@ SegPlan plan_segments(const GridDims& g, int ty, int sm_count, bool persist, int
         const int L = T - R;                       // tiles whose upper layer waits for group B
         if (mode_forced == 1 || L <= 0 || R / L < 1) return P;
         const int pieces = std::min(R / L, 8);
-        long long best = -1; int bestD = 0;
+        long long best = -1; int bestD = 0, bestq = 0;
         for (int D = (g.nz + 1) / 2; D < g.nz - 4; ++D) {
-            const int E = g.nz - D, dp = (E + pieces - 1) / pieces;
+            const int E = g.nz - D;
+            int q = pieces, dp = (E + q - 1) / q;
             if (dp < 4) break;
+            // as many pieces as there are non-empty ones of that depth (the kernel derives the depth from the count)
+            for (int q2 = (E + dp - 1) / dp; q2 != q; q2 = (E + dp - 1) / dp) { q = q2; dp = (E + q - 1) / q; }
             const long long span = std::max<long long>(D + 2, (E + 2) + (dp + 2));
-            if (best < 0 || span < best) { best = span; bestD = D; }
+            if (best < 0 || span < best) { best = span; bestD = D; bestq = q; }
         }
         if (best < 0 || (mode_forced != 2 && best * 100 > span0 * 97)) return P;
-        P.mode = 2; P.zchunk = bestD; P.nitems = T; P.zrest = bestD; P.erest = g.nz - bestD; P.q = pieces; P.blocks = sm_count;
+        P.mode = 2; P.zchunk = bestD; P.nitems = T; P.zrest = bestD; P.erest = g.nz - bestD; P.q = bestq; P.blocks = sm_count;
         return P;
     }
     if (mode_forced == 2) return P;

@@ -28,9 +28,10 @@ def segments(p, nz):
                 segs.append((b, 0, p["depth"]))
             else:
                 segs.append((r, p["zrest"], nz))
+                dp = -(-p["erest"] // p["q"])
                 if r < L * p["q"]:
-                    dp = -(-p["erest"] // p["q"])
                     z0 = p["zrest"] + (r // L) * dp
+                    assert z0 < nz, "the plan names an empty piece"
                     segs.append((R + r % L, z0, min(z0 + dp, nz)))
         elif b < p["nitems"]:
             z0 = (b // p["ntiles"]) * p["depth"]
@@ -111,3 +112,12 @@ def test_two_group_plan_is_chosen_only_where_it_is_shorter():
             a, e = pf.pf_tile_plan(*shape, rows, 148, -1), pf.pf_tile_plan(*shape, rows, 148, 0)
             if a["mode"] != 0:
                 assert longest(segments(a, shape[2])) <= 0.97 * longest(segments(e, shape[2]))
+
+
+def test_mode2_pieces_are_never_empty():
+    """Every depth of the upper layer must split into non-empty pieces (the kernel derives the piece depth from their number)."""
+    for nz in range(16, 400, 3):
+        for (nx, ny, rows, sms) in ((256, 256, 13, 148), (320, 208, 13, 148), (256, 300, 16, 148), (64, 52, 13, 7), (256, 256, 13, 132)):
+            p = pf.pf_tile_plan(nx, ny, nz, rows, sms, 2)
+            segs = segments(p, nz)          # asserts on an empty piece
+            assert sum(z1 - z0 for s in segs for _, z0, z1 in s) == p["ntiles"] * nz
