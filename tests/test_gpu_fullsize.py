@@ -225,3 +225,28 @@ def test_pf_tiled_config2_128_truncated_against_oracle(pf, oracle, solver):
     64^3 above and, through the fixed-point residuals of the oracle's operators, at 128^3 in
     test_config2_128_pf_properties.)"""
     _pf_tiled_vs_oracle(pf, oracle, wl.config2(volt_mv=50.0), max_outer=2, lin_maxit=10, solver=solver)
+
+
+def test_config3_256_decompositions_and_geometries_same_bits(pf):
+    """At the bench's size the persistent kernels get their work from the plans of tests/test_tile_plan.py: 13-row tiles
+    -> 80 tiles, mode 2 (a deep lower layer, a shallower upper one, the rest in pieces); 16-row tiles -> 64 tiles, mode 1
+    (two layers in step + a rest group).  Whatever the plan and the tile height, the iterates have the same bits as with
+    equal chunks (the default is also compared with the oracle above), for both solvers."""
+    w = wl.config3()
+    rng = np.random.default_rng(31)
+    rhs = torch.from_numpy(rng.standard_normal(w.n)).cuda()
+    assert pf.pf_tile_plan(256, 256, 256, 13, 148, -1)["mode"] == 2 and pf.pf_tile_plan(256, 256, 256, 16, 148, -1)["mode"] == 1
+    for solver in (0, 1):
+        ref = None
+        for rows, seg, diag in ((0, 0, 1), (0, -1, 1), (16, -1, 1), (16, 0, 2), (13, 2, 2)):
+            g = pf.Grid.from_workload(w, stencil=pf.STENCIL_ONTHEFLY, kernels=pf.KERNELS_TILED,
+                                      options={pf.PF_OPT_SOLVER: solver, pf.PF_OPT_TILE_ROWS: rows, pf.PF_OPT_SEGMENTS: seg,
+                                               pf.PF_OPT_DIAG_FROM_CODE: diag, pf.PF_OPT_HISTORY: 64})
+            o = g.solve_linear(rhs, tol=0.0, maxit=12, true_residual=False)
+            h = g.history(64)
+            assert pf.pf_grid_fault_repeats(g.handle) == 0
+            g.close()
+            if ref is None:
+                ref = (o["x"].clone(), h)
+                continue
+            assert o["iters"] == 12 and torch.equal(o["x"], ref[0]) and np.array_equal(h, ref[1]), (solver, rows, seg, diag)
