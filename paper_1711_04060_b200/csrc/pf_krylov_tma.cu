@@ -100,17 +100,23 @@ struct SegPlan {
     int zrest, erest, q;      // mode 1: the rest group's planes [zrest, zrest + erest), q flattened positions per block
                               // mode 2: the upper layer [zrest, zrest + erest), q pieces per leftover tile
     int blocks;               // host: blocks to launch
+    int m2_rest, m2_left, m2_depth;   // mode 2, precomputed so that the kernels divide by nothing: blocks of group B, tiles
+                                      // whose upper layer comes second, depth of a piece
 };
 // The segments of block b, one after the other (every thread of the block walks the same sequence).  PERSIST = false:
 // the block's one item of the equal-chunk plan (the stored variant has no registers to spare for a loop).
-template <bool PERSIST>
+// M2: the instance walks a plan of mode 2 (its own template parameter: kept apart, the walks of modes 0 / 1 are the code
+// they were before mode 2 existed -- with all three in one function the kernels, which sit at their register cap, lost
+// 3-5 % at 128^3 to a different register allocation and to divisions the compiler hoisted out of untaken branches).
+template <bool PERSIST, bool M2>
 struct SegIter {
     int pos, end;
     __device__ __forceinline__ void init(const SegPlan& P, int b, int nblocks) {
-        if (PERSIST && P.mode == 2) {
+        if (PERSIST && M2) {
             // group A: one segment; group B block r: its own upper layer, then piece r / L of leftover tile R + r % L
-            const int R = nblocks - P.ntiles, L = P.ntiles - R, r = b - P.ntiles, dp = (P.erest + P.q - 1) / P.q;
-            pos = 0; end = (b >= P.ntiles && r < L * P.q && (r / L) * dp < P.erest) ? 2 : 1;
+            // (plan_segments names non-empty pieces only)
+            (void)nblocks;
+            pos = 0; end = (b >= P.ntiles && b - P.ntiles < P.m2_left * P.q) ? 2 : 1;
         }
         else if (PERSIST && P.mode == 1 && b >= P.nitems) { pos = (b - P.nitems) * P.q; end = min(pos + P.q, P.ntiles * P.erest); }
         else if (PERSIST && P.mode == 1) { pos = b; end = b + 1; }
@@ -118,13 +124,16 @@ struct SegIter {
     }
     __device__ __forceinline__ bool next(const SegPlan& P, int nz, int b, int nblocks, int& tile, int& z0, int& z1) {
         if (pos >= end) return false;
-        if (PERSIST && P.mode == 2) {
+        if (PERSIST && M2) {
             if (b < P.ntiles) { tile = b; z0 = 0; z1 = P.zchunk; }
             else if (pos == 0) { tile = b - P.ntiles; z0 = P.zrest; z1 = nz; }
             else {
-                const int R = nblocks - P.ntiles, L = P.ntiles - R, r = b - P.ntiles, dp = (P.erest + P.q - 1) / P.q;
-                tile = R + r % L;
-                z0 = P.zrest + (r / L) * dp; z1 = min(z0 + dp, nz);
+                // r = piece * L + t with piece < q <= 8: found by subtraction (an integer division here would be
+                // evaluated, predicated off, by every thread of every kernel: the compiler hoists it)
+                int t = b - P.ntiles, piece = 0;
+                while (t >= P.m2_left) { t -= P.m2_left; ++piece; }
+                tile = P.m2_rest + t;
+                z0 = P.zrest + piece * P.m2_depth; z1 = min(z0 + P.m2_depth, nz);
             }
             ++pos;
         } else if (PERSIST && P.mode == 1 && b >= P.nitems) {   // rest group: flattened positions, one segment per tile
@@ -333,7 +342,7 @@ struct Slot {
     unsigned k0, k1;
 };
 
-template <int MODE, bool PRECOND, bool STORED, bool CODE32, int TYV>
+template <int MODE, bool PRECOND, bool STORED, bool CODE32, int TYV, bool M2>
 __global__ void __launch_bounds__(Geo<TYV>::NT, 1)
 k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv, const Scalars* sc_in, Scalars* sc_out, ReduceBuf rb,
       SegPlan plan) {
@@ -415,7 +424,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     // kernel's partial sums, so the loads fly while the scalar step is taken.
     int pre_issued = 0;
     if (tid == NT_CONSUMER) {
-        SegIter<PERSIST> it0;
+        SegIter<PERSIST, M2> it0;
         it0.init(plan, (int)blockIdx.x, (int)gridDim.x);
         int tile_f, z0f, z1f;
         if (it0.next(plan, g.nz, (int)blockIdx.x, (int)gridDim.x, tile_f, z0f, z1f)) {
@@ -458,7 +467,7 @@ k_tma(const __grid_constant__ TmaArgs tm, GridDims g, Operator op, KrylovVecs kv
     const int own_tile = (brow - 1) * TX + 2 * lane;               // element offset in an own-only box (main)
     const int pair_code = brow * BXC + CXO + 2 * lane;             // MODE_K1D: element offset in the code box with halo
 
-    SegIter<PERSIST> seg;
+    SegIter<PERSIST, M2> seg;
     seg.init(plan, (int)blockIdx.x, (int)gridDim.x);
     int skip = pre_issued;                 // producer: planes of the first segment that are already requested
     int tile, z0, z1;
@@ -915,6 +924,7 @@ SegPlan plan_segments(const GridDims& g, int ty, int sm_count, bool persist, int
     }
     const int full = sm_count / T, R = sm_count - full * T;
     if (full == 1) {
+        if (ty != TY_DEEP) return P;               // (the kernels of mode 2 are compiled for the 13-row tiles)
         // Mode 2.  (A plan like mode 1 with ONE layer in step, whose rest group takes almost half of the volume tile by
         // tile, gives up the sharing of halo rows in L2 between neighbouring tiles -- measured: K31 at 256^3 with 80
         // tiles, 0.233 -> 0.266 ms -- so here every group marches neighbouring tiles in step.)
@@ -933,6 +943,7 @@ SegPlan plan_segments(const GridDims& g, int ty, int sm_count, bool persist, int
         }
         if (best < 0 || (mode_forced != 2 && best * 100 > span0 * 97)) return P;
         P.mode = 2; P.zchunk = bestD; P.nitems = T; P.zrest = bestD; P.erest = g.nz - bestD; P.q = bestq; P.blocks = sm_count;
+        P.m2_rest = R; P.m2_left = L; P.m2_depth = (P.erest + bestq - 1) / bestq;
         return P;
     }
     if (mode_forced == 2) return P;
@@ -967,6 +978,8 @@ template <int MODE, bool PRECOND, bool STORED, bool CODE32, int TYV>
 void launch_geo(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, const TmaArgs& tm) {
     // The stored variant (six more arrays per node straight from global memory, no registers to spare for the
     // segment loop) keeps one item per block.  The plan of a grid is computed once per geometry and process.
+    // Plans of mode 2 exist for the 13-row tiles (their kernels are instances of their own).
+    constexpr bool M2_OK = !STORED && TYV == TY_DEEP;
     static thread_local struct { GridDims g; int sm, forced; SegPlan P; bool valid; } cache = {};
     if (!cache.valid || cache.g.nx != c.g.nx || cache.g.ny != c.g.ny || cache.g.nz != c.g.nz || cache.sm != c.sm_count ||
         cache.forced != c.seg_mode) {
@@ -979,10 +992,13 @@ void launch_geo(const LaunchCtx& c, const Operator& op, const KrylovVecs& kv, co
     c.next_scalars(sc_in, sc_out);
     using L = Layout<MODE, STORED, CODE32, TYV>;
     static std::atomic<unsigned long long> configured{0ull};      // bit d: the attribute is set on device d
-    auto kern = k_tma<MODE, PRECOND, STORED, CODE32, TYV>;
+    auto kern = k_tma<MODE, PRECOND, STORED, CODE32, TYV, false>;
+    if constexpr (M2_OK) { if (plan.mode == 2) kern = k_tma<MODE, PRECOND, STORED, CODE32, TYV, true>; }
     const unsigned long long bit = 1ull << (c.device & 63);
     if (c.device >= 64 || !(configured.load(std::memory_order_relaxed) & bit)) {
-        note_launch(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L::TOTAL));
+        note_launch(cudaFuncSetAttribute(k_tma<MODE, PRECOND, STORED, CODE32, TYV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, L::TOTAL));
+        if constexpr (M2_OK)
+            note_launch(cudaFuncSetAttribute(k_tma<MODE, PRECOND, STORED, CODE32, TYV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, L::TOTAL));
         configured.fetch_or(bit, std::memory_order_relaxed);
     }
     ++g_launch_count;
