@@ -157,6 +157,21 @@ __device__ __forceinline__ void finish_k31(Scalars* sc, double* hist, double rtv
 // LOOP: the kernel is the one of a loop body that keeps the condition of the body's WHILE node up to date
 // (pf_api.cu loop_graph; only k3 is compiled that way -- Nsight Compute does not profile kernel nodes that can set
 // conditional handles, in graphs of any kind, so every other kernel stays free of the call).
+// Which producer's partial sums a kernel of kind `kind` can find pending (besides none).  `kind` is a compile-time
+// constant at every call, so the tests fold and a kernel carries the combine and the scalar step of its possible
+// predecessors only: k1 follows k3 or the initial residual, k2 follows k1, k3 follows k2; K2M follows k1 (the first
+// matvec of a merged solve) or K31, K31 follows K2M; the residual kernels and the one-block finalize follow anything.
+__device__ __forceinline__ bool may_follow(int kind, int pend) {
+    switch (kind) {
+        case PEND_K1:  return pend == PEND_K3 || pend == PEND_INIT;
+        case PEND_K2:  return pend == PEND_K1;
+        case PEND_K3:  return pend == PEND_K2;
+        case PEND_K2M: return pend == PEND_K1 || pend == PEND_K31;
+        case PEND_K31: return pend == PEND_K2M;
+        default:       return true;
+    }
+}
+
 template <bool LOOP = false>
 __device__ __forceinline__ bool begin_kernel(int kind, Scalars* S, const Scalars* sc_in, Scalars* sc_out,
                                              const ReduceBuf& rb, double* hist, dd* scratch) {
@@ -181,21 +196,26 @@ __device__ __forceinline__ bool begin_kernel(int kind, Scalars* S, const Scalars
     dd q[2] = {dd_zero(), dd_zero()};
     dd q3[3] = {dd_zero(), dd_zero(), dd_zero()};
     double m = 0.0;
-    if (pend == PEND_K1) { dd q1[1]; combine_partials<1, false>(q1, m, nblk, scratch, rb, pend, pre); q[0] = q1[0]; }
-    else if (pend == PEND_K2) combine_partials<2, false>(q, m, nblk, scratch, rb, pend, pre);
-    else if (pend == PEND_K2M) combine_partials<3, false>(q3, m, nblk, scratch, rb, pend, pre);
-    else if (pend == PEND_K31) combine_partials<3, true>(q3, m, nblk, scratch, rb, pend, pre);
-    else if (pend != PEND_NONE) combine_partials<2, true>(q, m, nblk, scratch, rb, pend, pre);
+    const bool any2t = may_follow(kind, PEND_K3) || may_follow(kind, PEND_INIT) || may_follow(kind, PEND_TRUE);
+    bool unexpected = false;
+    if (may_follow(kind, PEND_K1) && pend == PEND_K1) { dd q1[1]; combine_partials<1, false>(q1, m, nblk, scratch, rb, pend, pre); q[0] = q1[0]; }
+    else if (may_follow(kind, PEND_K2) && pend == PEND_K2) combine_partials<2, false>(q, m, nblk, scratch, rb, pend, pre);
+    else if (may_follow(kind, PEND_K2M) && pend == PEND_K2M) combine_partials<3, false>(q3, m, nblk, scratch, rb, pend, pre);
+    else if (may_follow(kind, PEND_K31) && pend == PEND_K31) combine_partials<3, true>(q3, m, nblk, scratch, rb, pend, pre);
+    else if (any2t && may_follow(kind, pend) && (pend == PEND_K3 || pend == PEND_INIT || pend == PEND_TRUE))
+        combine_partials<2, true>(q, m, nblk, scratch, rb, pend, pre);
+    else if (pend != PEND_NONE) unexpected = true;       // (a launch order the driver never produces)
     if (threadIdx.x == 0) {
         const bool lead = linear_block_id() == 0;
         double* h = lead ? hist : nullptr;                       // one writer for the history
-        if (pend == PEND_INIT) finish_init(S, h, dd_round(q[0]), dd_round(q[1]), m);
-        else if (pend == PEND_K1) finish_k1(S, dd_round(q[0]));
-        else if (pend == PEND_K2) finish_k2(S, dd_round(q[0]), dd_round(q[1]));
-        else if (pend == PEND_K3) finish_k3(S, h, dd_round(q[0]), dd_round(q[1]), m);
-        else if (pend == PEND_K2M) finish_k2m(S, dd_round(q3[0]), dd_round(q3[1]), dd_round(q3[2]));
-        else if (pend == PEND_K31) finish_k31(S, h, dd_round(q3[0]), dd_round(q3[1]), dd_round(q3[2]), m);
-        else if (pend == PEND_TRUE) { S->true_rr = dd_round(q[1]); S->true_rmax = m; }
+        if (unexpected) { S->done = 1; S->status = -2; }
+        else if (may_follow(kind, PEND_INIT) && pend == PEND_INIT) finish_init(S, h, dd_round(q[0]), dd_round(q[1]), m);
+        else if (may_follow(kind, PEND_K1) && pend == PEND_K1) finish_k1(S, dd_round(q[0]));
+        else if (may_follow(kind, PEND_K2) && pend == PEND_K2) finish_k2(S, dd_round(q[0]), dd_round(q[1]));
+        else if (may_follow(kind, PEND_K3) && pend == PEND_K3) finish_k3(S, h, dd_round(q[0]), dd_round(q[1]), m);
+        else if (may_follow(kind, PEND_K2M) && pend == PEND_K2M) finish_k2m(S, dd_round(q3[0]), dd_round(q3[1]), dd_round(q3[2]));
+        else if (may_follow(kind, PEND_K31) && pend == PEND_K31) finish_k31(S, h, dd_round(q3[0]), dd_round(q3[1]), dd_round(q3[2]), m);
+        else if (may_follow(kind, PEND_TRUE) && pend == PEND_TRUE) { S->true_rr = dd_round(q[1]); S->true_rmax = m; }
         // the iterates are invalid from the faulting kernel on: stop here (status stays PF_NOT_CONVERGED) instead of
         // iterating on them up to maxit; the host repeats the solve with the __ddiv_rn kernels (x is untouched, D3).
         // Blocks of one launch may disagree for one kernel (a block of THIS launch can raise the flag while others
