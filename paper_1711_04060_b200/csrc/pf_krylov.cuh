@@ -160,7 +160,8 @@ __device__ __forceinline__ void finish_k31(Scalars* sc, double* hist, double rtv
 // Which producer's partial sums a kernel of kind `kind` can find pending (besides none).  `kind` is a compile-time
 // constant at every call, so the tests fold and a kernel carries the combine and the scalar step of its possible
 // predecessors only: k1 follows k3 or the initial residual, k2 follows k1, k3 follows k2; K2M follows k1 (the first
-// matvec of a merged solve) or K31, K31 follows K2M; the residual kernels and the one-block finalize follow anything.
+// matvec of a merged solve) or K31, K31 follows K2M; the residual kernels find nothing pending; the one-block finalize
+// follows anything.
 __device__ __forceinline__ bool may_follow(int kind, int pend) {
     switch (kind) {
         case PEND_K1:  return pend == PEND_K3 || pend == PEND_INIT;
@@ -168,7 +169,9 @@ __device__ __forceinline__ bool may_follow(int kind, int pend) {
         case PEND_K3:  return pend == PEND_K2;
         case PEND_K2M: return pend == PEND_K1 || pend == PEND_K31;
         case PEND_K31: return pend == PEND_K2M;
-        default:       return true;
+        case PEND_INIT:                          // the residual kernels start a solve (fresh scalars) or follow the
+        case PEND_TRUE: return false;            // one-block finalize: nothing is ever pending for them
+        default:       return true;              // the finalize itself follows anything
     }
 }
 
