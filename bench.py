@@ -64,6 +64,9 @@ def parse():
                          "node repeats the iterations on the device; chunks = graph replays of 16 iterations polled "
                          "by the host (ncu does not profile kernel nodes of graphs with conditional nodes: launch "
                          "lists are taken with this mode); stream = plain launches")
+    ap.add_argument("--diag-from-code", type=int, choices=[0, 1, 2], default=None,
+                    help="PF_OPT_DIAG_FROM_CODE of the timed steps (default: the library's own, 1): 0 the diagonal is read, "
+                         "1 k1 takes it from the stencil codes, 2 k2 as well")
     ap.add_argument("--solver", choices=["table3", "merged"], default="table3",
                     help="table3: BiCGSTAB as Table 3 writes it, three kernels per iteration (the default, whose parity "
                          "reference is the oracle's Table 3); merged: the two-reduction recurrence (PF_OPT_SOLVER = 1, "
@@ -276,6 +279,8 @@ def run_b200(args):
             pf.pf_grid_set_option(h, pf.PF_OPT_KERNELS, kernels)
         pf.pf_grid_set_option(h, pf.PF_OPT_GRAPH, {"auto": 3, "loop": 2, "chunks": 1, "stream": 0}[args.launch_mode])
         pf.pf_grid_set_option(h, pf.PF_OPT_SOLVER, cfg["solver"])
+        if args.diag_from_code is not None:
+            pf.pf_grid_set_option(h, pf.PF_OPT_DIAG_FROM_CODE, args.diag_from_code)
         pf.pf_grid_set_option(h, pf.PF_OPT_LINEAR_TOL, 0.0)
         pf.pf_grid_set_option(h, pf.PF_OPT_LINEAR_MAXIT, PF_INNER_ITERS)
         pf.pf_grid_set_option(h, pf.PF_OPT_MAX_OUTER, 1)
